@@ -1,0 +1,605 @@
+/*
+ * lasp_oracle.c -- plain, slow, fp64 CPU oracle for the LASP-Adam-GPU hot path.
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs may build, load or call it.
+ * It shares no code, header, table or constant generator with the CUDA path under
+ * paper_2512_24840_b200/csrc/.
+ *
+ * Every function follows /root/reference/PAPER.md ("P:n" = line n) in the reading
+ * fixed by SURVEY.md section 8(c) ("C.1" = the definition block, "C.2-n" = row n of the
+ * table of readings).  Nothing is blocked, fused or reordered beyond what the
+ * definition states: one spectrum at a time, one pixel at a time, one tap at a time.
+ *
+ *   emulator            Eq. 1   P:67-76, P:187     orc_monomials, emulator_row
+ *   shift + broadening  Eq. 5   P:111-119          orc_kernel_weights, stencil
+ *   Legendre continuum  Eq. 6   P:121-129          orc_legendre, orc_solve_continuum
+ *   residual            Eq. 7   P:133              chi2 / rho
+ *   objective           Eq. 9   P:163-167          sum_j w_j r_j^2 (C.2-2, C.2-3)
+ *   Adam                step 8  P:169              orc_adam_step
+ *   error estimate      step 9  P:173              errors_one
+ *
+ * Parity pins (tests/test_oracle_*.py): numpy legvander/legval, numpy lstsq,
+ * numpy convolve, central finite differences of chi2 (with re-solve), closed-form
+ * first Adam step and torch.optim.Adam, textbook OLS covariance, Monte-Carlo
+ * scatter, noise-free recovery, the 1327-pixel grid of P:227.  No function here
+ * is "parity unpinned".
+ *
+ * Build: gcc -O2 -fopenmp -shared -fPIC -o liblasp_oracle.so lasp_oracle.c -lm
+ * (threads run over spectra only; each spectrum is computed serially.)
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define ORC_C_KMS 299792.458 /* speed of light, km/s (C.1) */
+
+typedef struct {
+    int32_t n_pix, n_seg;
+    const int32_t *seg_offset;    /* [n_seg+1] */
+    const double *loglam;         /* [n_pix] log10(lambda/A) */
+    const double *seg_sigma_inst; /* [n_seg] km/s */
+    int32_t n_labels, n_terms;    /* L, K */
+    const uint8_t *term_exps;     /* [K*L] */
+    const double *coeffs;         /* [K*n_pix] row-major */
+    const double *lo, *hi;        /* [NP], NP = L+2: labels..., rv, sigma */
+    const uint8_t *label_log10;   /* [L] */
+    const double *emu_a, *emu_b;  /* [L] */
+    int32_t cont_degree;          /* D */
+    const int32_t *seg_n_edge;    /* [n_seg] */
+} orc_model;
+
+/* ------------------------------------------------------------------ grid */
+
+/* C.1: s_j = c ln10 (loglam_{j+1}-loglam_{j-1})/2, one-sided at segment ends. */
+static double pixel_kms(const orc_model *m, int seg, int j)
+{
+    int o = m->seg_offset[seg], e = m->seg_offset[seg + 1];
+    double d;
+    if (e - o < 2) return ORC_C_KMS * log(10.0) * 1e-4;
+    if (j == o) d = m->loglam[j + 1] - m->loglam[j];
+    else if (j == e - 1) d = m->loglam[j] - m->loglam[j - 1];
+    else d = 0.5 * (m->loglam[j + 1] - m->loglam[j - 1]);
+    return ORC_C_KMS * log(10.0) * d;
+}
+
+void orc_pixel_kms(const orc_model *m, double *s_out)
+{
+    for (int s = 0; s < m->n_seg; ++s)
+        for (int j = m->seg_offset[s]; j < m->seg_offset[s + 1]; ++j) s_out[j] = pixel_kms(m, s, j);
+}
+
+/* P:127 (0-based, per segment, C.2-7): x_j = -1 + 2 (j-o_s)/P_s ; never reaches +1. */
+static double node_x(const orc_model *m, int seg, int j)
+{
+    int o = m->seg_offset[seg], n = m->seg_offset[seg + 1] - o;
+    return -1.0 + 2.0 * (double)(j - o) / (double)n;
+}
+
+/* --------------------------------------------------------------- Legendre */
+
+/* P_0..P_D at x by Bonnet's recurrence (n+1)P_{n+1} = (2n+1) x P_n - n P_{n-1}. */
+void orc_legendre(double x, int D, double *P)
+{
+    P[0] = 1.0;
+    if (D >= 1) P[1] = x;
+    for (int n = 1; n < D; ++n) P[n + 1] = ((2.0 * n + 1.0) * x * P[n] - n * P[n - 1]) / (n + 1.0);
+}
+
+/* --------------------------------------------------------------- emulator */
+
+/* C.1: theta = lo + (u+1)(hi-lo)/2 */
+static void denorm(const orc_model *m, const double *u, double *theta)
+{
+    int NP = m->n_labels + 2;
+    for (int p = 0; p < NP; ++p) theta[p] = m->lo[p] + (u[p] + 1.0) * (m->hi[p] - m->lo[p]) * 0.5;
+}
+
+static void norm_u(const orc_model *m, const double *theta, double *u)
+{
+    int NP = m->n_labels + 2;
+    for (int p = 0; p < NP; ++p) u[p] = 2.0 * (theta[p] - m->lo[p]) / (m->hi[p] - m->lo[p]) - 1.0;
+}
+
+/* Eq. 1 in the single-polynomial reading (Delta-5): x_l = a_l tau_l(theta_l) + b_l ;
+ * phi_k = prod_l x_l^{e_kl} ; dphi[l*K+k] = d phi_k / d x_l ; dx_dtheta[l] (C.1 last line). */
+void orc_monomials(const orc_model *m, const double *theta, double *x, double *phi, double *dphi,
+                   double *dx_dtheta)
+{
+    int L = m->n_labels, K = m->n_terms;
+    for (int l = 0; l < L; ++l) {
+        if (m->label_log10[l]) {
+            x[l] = m->emu_a[l] * log10(theta[l]) + m->emu_b[l];
+            dx_dtheta[l] = m->emu_a[l] / (theta[l] * log(10.0));
+        } else {
+            x[l] = m->emu_a[l] * theta[l] + m->emu_b[l];
+            dx_dtheta[l] = m->emu_a[l];
+        }
+    }
+    for (int k = 0; k < K; ++k) {
+        double v = 1.0;
+        for (int l = 0; l < L; ++l)
+            for (int e = 0; e < m->term_exps[k * L + l]; ++e) v *= x[l];
+        phi[k] = v;
+        for (int l = 0; l < L; ++l) {
+            int el = m->term_exps[k * L + l];
+            double d = 0.0;
+            if (el > 0) {
+                d = (double)el;
+                for (int l2 = 0; l2 < L; ++l2) {
+                    int e2 = m->term_exps[k * L + l2] - (l2 == l ? 1 : 0);
+                    for (int e = 0; e < e2; ++e) d *= x[l2];
+                }
+            }
+            dphi[l * K + k] = d;
+        }
+    }
+}
+
+/* T_j = sum_k c_k C[k,j]  (Eq. 1 with the term vector c = phi or dphi/dx_l) */
+static void emulator_row(const orc_model *m, const double *c, double *T)
+{
+    int P = m->n_pix, K = m->n_terms;
+    for (int j = 0; j < P; ++j) {
+        double acc = 0.0;
+        for (int k = 0; k < K; ++k) acc += c[k] * m->coeffs[(size_t)k * P + j];
+        T[j] = acc;
+    }
+}
+
+/* ---------------------------------------------------------- kernel weights */
+
+/* Eq. 5 / P:115 with readings C.2-9, -10, -15: H = ceil(|mu| + 5 sigma); point-sampled
+ * Gaussian at integer offsets k = -H..H centred at +mu, unit sum over the truncated
+ * support; analytic d g/d mu and d g/d sigma with H held constant (C.1).
+ * Arrays hold 2H+1 entries, entry i is offset k = i - H.  Returns H. */
+int orc_kernel_weights(double mu, double sigma, int Hcap, double *g, double *dg_dmu, double *dg_dsig)
+{
+    int H = (int)ceil(fabs(mu) + 5.0 * sigma);
+    if (H > Hcap) return -H; /* caller sized the buffers too small */
+    double sum = 0.0;
+    for (int k = -H; k <= H; ++k) {
+        double e = exp(-(k - mu) * (k - mu) / (2.0 * sigma * sigma));
+        g[k + H] = e;
+        sum += e;
+    }
+    double kbar = 0.0, m2 = 0.0;
+    for (int k = -H; k <= H; ++k) {
+        g[k + H] /= sum;
+        kbar += g[k + H] * k;
+        m2 += g[k + H] * (k - mu) * (k - mu);
+    }
+    for (int k = -H; k <= H; ++k) {
+        if (dg_dmu) dg_dmu[k + H] = g[k + H] * (k - kbar) / (sigma * sigma);
+        if (dg_dsig) dg_dsig[k + H] = g[k + H] * ((k - mu) * (k - mu) - m2) / (sigma * sigma * sigma);
+    }
+    return H;
+}
+
+static int clampi(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
+
+/* Largest support over the prior box, used only to size scratch buffers. */
+static int support_cap(const orc_model *m)
+{
+    int L = m->n_labels;
+    double vmax = fmax(fabs(m->lo[L]), fabs(m->hi[L])) * 1.5 + 1.0;
+    double smax = fmax(fabs(m->lo[L + 1]), fabs(m->hi[L + 1])) * 1.5 + 1.0;
+    int cap = 0;
+    for (int s = 0; s < m->n_seg; ++s)
+        for (int j = m->seg_offset[s]; j < m->seg_offset[s + 1]; ++j) {
+            double sj = pixel_kms(m, s, j);
+            double st = sqrt(smax * smax + m->seg_sigma_inst[s] * m->seg_sigma_inst[s]);
+            int H = (int)ceil(vmax / sj + 5.0 * st / sj) + 2;
+            if (H > cap) cap = H;
+        }
+    return cap;
+}
+
+/* ------------------------------------------------------------ forward model */
+
+typedef struct {
+    int P, K, L, NP, D, nc, Hcap;
+    double *theta, *x, *phi, *dphi, *dxdt;
+    double *T, *dT;       /* [P], [L*P] */
+    double *S, *dS;       /* [P], [NP*P]  dS = d S / d u_p */
+    double *g, *gm, *gs;  /* [2Hcap+1] */
+    double *w, *c, *r;    /* [P] */
+    double *Pl;           /* [D+1] */
+    double *A, *rhs;      /* [(D+1)^2], [D+1] */
+    double *b;            /* [nc] */
+} work_t;
+
+static work_t *work_new(const orc_model *m)
+{
+    work_t *k = (work_t *)calloc(1, sizeof(work_t));
+    k->P = m->n_pix; k->K = m->n_terms; k->L = m->n_labels; k->NP = k->L + 2;
+    k->D = m->cont_degree; k->nc = m->n_seg * (k->D + 1); k->Hcap = support_cap(m);
+    int P = k->P, K = k->K, L = k->L, NP = k->NP, D = k->D;
+    k->theta = calloc(NP, 8); k->x = calloc(L, 8); k->phi = calloc(K, 8);
+    k->dphi = calloc((size_t)L * K, 8); k->dxdt = calloc(L, 8);
+    k->T = calloc(P, 8); k->dT = calloc((size_t)L * P, 8);
+    k->S = calloc(P, 8); k->dS = calloc((size_t)NP * P, 8);
+    k->g = calloc(2 * k->Hcap + 1, 8); k->gm = calloc(2 * k->Hcap + 1, 8); k->gs = calloc(2 * k->Hcap + 1, 8);
+    k->w = calloc(P, 8); k->c = calloc(P, 8); k->r = calloc(P, 8);
+    k->Pl = calloc(D + 1, 8); k->A = calloc((size_t)(D + 1) * (D + 1), 8); k->rhs = calloc(D + 1, 8);
+    k->b = calloc(k->nc, 8);
+    return k;
+}
+
+static void work_free(work_t *k)
+{
+    free(k->theta); free(k->x); free(k->phi); free(k->dphi); free(k->dxdt); free(k->T); free(k->dT);
+    free(k->S); free(k->dS); free(k->g); free(k->gm); free(k->gs); free(k->w); free(k->c); free(k->r);
+    free(k->Pl); free(k->A); free(k->rhs); free(k->b); free(k);
+}
+
+/* model(u) of C.1: fills k->S; with want_grad also k->dS[p][j] = dS_j/du_p (forward mode,
+ * one parameter at a time -- the plain derivative of the definition). */
+static void model_S(const orc_model *m, work_t *k, const double *u, int want_grad)
+{
+    int P = k->P, K = k->K, L = k->L;
+    denorm(m, u, k->theta);
+    orc_monomials(m, k->theta, k->x, k->phi, k->dphi, k->dxdt);
+    emulator_row(m, k->phi, k->T);
+    if (want_grad)
+        for (int l = 0; l < L; ++l) emulator_row(m, k->dphi + (size_t)l * K, k->dT + (size_t)l * P);
+    double v = k->theta[L], sig = k->theta[L + 1];
+    for (int s = 0; s < m->n_seg; ++s) {
+        int o = m->seg_offset[s], e = m->seg_offset[s + 1];
+        double si = m->seg_sigma_inst[s];
+        double stot = sqrt(sig * sig + si * si); /* C.2-13 */
+        for (int j = o; j < e; ++j) {
+            double sj = pixel_kms(m, s, j);
+            double mu = v / sj, sg = stot / sj; /* C.2-12, C.2-14 */
+            int H = orc_kernel_weights(mu, sg, k->Hcap, k->g, want_grad ? k->gm : NULL,
+                                       want_grad ? k->gs : NULL);
+            if (H < 0) { k->S[j] = NAN; continue; }
+            double acc = 0.0;
+            for (int t = -H; t <= H; ++t) acc += k->g[t + H] * k->T[clampi(j - t, o, e - 1)]; /* C.2-11, -16 */
+            k->S[j] = acc;
+            if (want_grad) {
+                double am = 0.0, as = 0.0;
+                for (int t = -H; t <= H; ++t) {
+                    double Tv = k->T[clampi(j - t, o, e - 1)];
+                    am += k->gm[t + H] * Tv;
+                    as += k->gs[t + H] * Tv;
+                }
+                for (int l = 0; l < L; ++l) {
+                    double al = 0.0;
+                    for (int t = -H; t <= H; ++t)
+                        al += k->g[t + H] * k->dT[(size_t)l * P + clampi(j - t, o, e - 1)];
+                    k->dS[(size_t)l * P + j] = al * k->dxdt[l] * (m->hi[l] - m->lo[l]) * 0.5;
+                }
+                k->dS[(size_t)L * P + j] = am / sj * (m->hi[L] - m->lo[L]) * 0.5;
+                k->dS[(size_t)(L + 1) * P + j] =
+                    as * (sig / (stot * sj)) * (m->hi[L + 1] - m->lo[L + 1]) * 0.5;
+            }
+        }
+    }
+}
+
+/* a0: w_j = mask_j ivar_j, zero on the n_edge first/last pixels of each segment (Eq. 8 P:161,
+ * edge exclusion P:167, C.2-2, -17). */
+static void make_weights(const orc_model *m, const double *ivar, const uint8_t *mask, double *w)
+{
+    for (int s = 0; s < m->n_seg; ++s) {
+        int o = m->seg_offset[s], e = m->seg_offset[s + 1], ne = m->seg_n_edge[s];
+        for (int j = o; j < e; ++j) {
+            double v = ivar[j] * ((mask == NULL || mask[j]) ? 1.0 : 0.0);
+            if (j - o < ne || e - 1 - j < ne) v = 0.0;
+            w[j] = v;
+        }
+    }
+}
+
+/* Cholesky A = G G^T in place (lower), returns 0 if SPD else 1.  n <= 64. */
+static int cholesky(double *A, int n)
+{
+    for (int i = 0; i < n; ++i) {
+        for (int j = 0; j <= i; ++j) {
+            double s = A[i * n + j];
+            for (int t = 0; t < j; ++t) s -= A[i * n + t] * A[j * n + t];
+            if (i == j) {
+                if (!(s > 0.0)) return 1;
+                A[i * n + i] = sqrt(s);
+            } else
+                A[i * n + j] = s / A[j * n + j];
+        }
+    }
+    return 0;
+}
+
+static void chol_solve(const double *G, int n, double *x)
+{
+    for (int i = 0; i < n; ++i) {
+        double s = x[i];
+        for (int t = 0; t < i; ++t) s -= G[i * n + t] * x[t];
+        x[i] = s / G[i * n + i];
+    }
+    for (int i = n - 1; i >= 0; --i) {
+        double s = x[i];
+        for (int t = i + 1; t < n; ++t) s -= G[t * n + i] * x[t];
+        x[i] = s / G[i * n + i];
+    }
+}
+
+/* solve(S) of C.1 (Eq. 6; C.2-4, -6): per segment
+ *   A = Phi^T diag(w) Phi, rhs = Phi^T diag(w) y, Phi_jn = S_j P_n(x_j); b = A^-1 rhs.
+ * A segment whose A is not positive definite gets b = 0 and status bit 1.
+ * Then c_j = sum_n b_n P_n(x_j).  Returns status bits. */
+static int solve_continuum(const orc_model *m, work_t *k, const double *y)
+{
+    int D = k->D, n = D + 1, status = 0;
+    for (int s = 0; s < m->n_seg; ++s) {
+        int o = m->seg_offset[s], e = m->seg_offset[s + 1];
+        memset(k->A, 0, sizeof(double) * n * n);
+        memset(k->rhs, 0, sizeof(double) * n);
+        for (int j = o; j < e; ++j) {
+            if (k->w[j] == 0.0) continue;
+            orc_legendre(node_x(m, s, j), D, k->Pl);
+            for (int a = 0; a < n; ++a) {
+                double fa = k->S[j] * k->Pl[a];
+                k->rhs[a] += fa * k->w[j] * y[j];
+                for (int b2 = 0; b2 < n; ++b2) k->A[a * n + b2] += fa * k->w[j] * k->S[j] * k->Pl[b2];
+            }
+        }
+        double *bs = k->b + s * n;
+        if (cholesky(k->A, n)) {
+            status |= 1;
+            for (int a = 0; a < n; ++a) bs[a] = 0.0;
+        } else {
+            for (int a = 0; a < n; ++a) bs[a] = k->rhs[a];
+            chol_solve(k->A, n, bs);
+        }
+        for (int j = o; j < e; ++j) {
+            orc_legendre(node_x(m, s, j), D, k->Pl);
+            double c = 0.0;
+            for (int a = 0; a < n; ++a) c += bs[a] * k->Pl[a];
+            k->c[j] = c;
+        }
+    }
+    return status;
+}
+
+/* chi2(u) of C.1: S = model(u); b = solve(S); r = y - c S; chi2 = sum w r^2.  k->w must be set. */
+static double chi2_at(const orc_model *m, work_t *k, const double *u, const double *y, int want_grad,
+                      int *status)
+{
+    model_S(m, k, u, want_grad);
+    int st = solve_continuum(m, k, y);
+    double chi2 = 0.0;
+    for (int j = 0; j < k->P; ++j) {
+        k->r[j] = y[j] - k->c[j] * k->S[j];
+        if (k->w[j] != 0.0) chi2 += k->w[j] * k->r[j] * k->r[j];
+    }
+    if (status) *status |= st;
+    return chi2;
+}
+
+/* grad(u) of C.1: d chi2/d u_p = sum_j (-2 w_j r_j c_j) dS_j/du_p with b held (C.2-5). */
+static void grad_from_work(const work_t *k, double *grad)
+{
+    for (int p = 0; p < k->NP; ++p) {
+        double acc = 0.0;
+        for (int j = 0; j < k->P; ++j)
+            if (k->w[j] != 0.0) acc += -2.0 * k->w[j] * k->r[j] * k->c[j] * k->dS[(size_t)p * k->P + j];
+        grad[p] = acc;
+    }
+}
+
+/* One Adam update (step 8; C.2-18, -20): t starts at 1, bias-corrected, eps outside
+ * the sqrt of the bias-corrected second moment, then clip to [-1,1]. */
+void orc_adam_step(int n, double *u, double *mom, double *vel, const double *g, int t, double lr,
+                   double b1, double b2, double eps)
+{
+    for (int p = 0; p < n; ++p) {
+        mom[p] = b1 * mom[p] + (1.0 - b1) * g[p];
+        vel[p] = b2 * vel[p] + (1.0 - b2) * g[p] * g[p];
+        double mh = mom[p] / (1.0 - pow(b1, (double)t));
+        double vh = vel[p] / (1.0 - pow(b2, (double)t));
+        double un = u[p] - lr * mh / (sqrt(vh) + eps);
+        u[p] = un < -1.0 ? -1.0 : (un > 1.0 ? 1.0 : un);
+    }
+}
+
+static int finite_all(const double *v, int n)
+{
+    for (int i = 0; i < n; ++i)
+        if (!isfinite(v[i])) return 0;
+    return 1;
+}
+
+/* Step 9 (C.2-22, -23): rho(u) = sqrt(w) (y - c S) with the continuum re-solved,
+ * J by central differences of step h in u, Sigma = rho^T rho/(N_good-NP) (J^T J)^-1,
+ * err_p = sqrt(Sigma_pp) (hi_p-lo_p)/2.  Non-invertible J^T J gives NaN errors. */
+static void errors_one(const orc_model *m, work_t *k, const double *u, const double *y, double h,
+                       double *err)
+{
+    int P = k->P, NP = k->NP;
+    double *J = calloc((size_t)NP * P, 8), *up = calloc(NP, 8), *rp = calloc(P, 8);
+    double *N = calloc((size_t)NP * NP, 8);
+    for (int p = 0; p < NP; ++p) {
+        memcpy(up, u, 8 * NP);
+        up[p] = u[p] + h;
+        chi2_at(m, k, up, y, 0, NULL);
+        for (int j = 0; j < P; ++j) rp[j] = sqrt(k->w[j]) * k->r[j];
+        up[p] = u[p] - h;
+        chi2_at(m, k, up, y, 0, NULL);
+        for (int j = 0; j < P; ++j) J[(size_t)p * P + j] = (rp[j] - sqrt(k->w[j]) * k->r[j]) / (2.0 * h);
+    }
+    double ss = chi2_at(m, k, u, y, 0, NULL);
+    int ngood = 0;
+    for (int j = 0; j < P; ++j) ngood += (k->w[j] > 0.0);
+    for (int a = 0; a < NP; ++a)
+        for (int b = 0; b < NP; ++b) {
+            double acc = 0.0;
+            for (int j = 0; j < P; ++j) acc += J[(size_t)a * P + j] * J[(size_t)b * P + j];
+            N[a * NP + b] = acc;
+        }
+    double s2 = ss / (double)(ngood - NP);
+    if (ngood <= NP || cholesky(N, NP)) {
+        for (int p = 0; p < NP; ++p) err[p] = NAN;
+    } else {
+        /* diag of (J^T J)^-1: solve N z = e_p */
+        for (int p = 0; p < NP; ++p) {
+            memset(up, 0, 8 * NP);
+            up[p] = 1.0;
+            chol_solve(N, NP, up);
+            err[p] = sqrt(s2 * up[p]) * (m->hi[p] - m->lo[p]) * 0.5;
+        }
+    }
+    free(J); free(up); free(rp); free(N);
+}
+
+/* status bits of SURVEY 8(b): 1 not SPD, 2 non-finite, 4 continuum <= 0 on a fitted pixel
+ * (the paper's failure criterion), 8 parameter on its bound. */
+static int final_status(const work_t *k, const double *u, double chi2, int st)
+{
+    if (!isfinite(chi2) || !finite_all(u, k->NP) || !finite_all(k->b, k->nc)) st |= 2;
+    for (int j = 0; j < k->P; ++j)
+        if (k->w[j] > 0.0 && k->c[j] <= 0.0) { st |= 4; break; }
+    for (int p = 0; p < k->NP; ++p)
+        if (u[p] <= -1.0 || u[p] >= 1.0) st |= 8;
+    return st;
+}
+
+/* ------------------------------------------------------------- public API */
+
+/* lasp_eval_model: model_j = c_j S_j at given physical params and plain-Legendre cont. */
+int orc_eval_model(const orc_model *m, int64_t B, const double *params, const double *cont,
+                   double *model)
+{
+    int NP = m->n_labels + 2, P = m->n_pix, n = m->cont_degree + 1, nc = m->n_seg * n;
+#pragma omp parallel
+    {
+        work_t *k = work_new(m);
+        double *u = calloc(NP, 8);
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t i = 0; i < B; ++i) {
+            norm_u(m, params + i * NP, u);
+            model_S(m, k, u, 0);
+            for (int s = 0; s < m->n_seg; ++s)
+                for (int j = m->seg_offset[s]; j < m->seg_offset[s + 1]; ++j) {
+                    orc_legendre(node_x(m, s, j), m->cont_degree, k->Pl);
+                    double c = 0.0;
+                    for (int a = 0; a < n; ++a) c += cont[i * nc + s * n + a] * k->Pl[a];
+                    model[i * P + j] = c * k->S[j];
+                }
+        }
+        free(u);
+        work_free(k);
+    }
+    return 0;
+}
+
+/* The bare broadened template S (no continuum), for pins. */
+int orc_eval_S(const orc_model *m, int64_t B, const double *params, double *S)
+{
+    int NP = m->n_labels + 2, P = m->n_pix;
+    work_t *k = work_new(m);
+    double *u = calloc(NP, 8);
+    for (int64_t i = 0; i < B; ++i) {
+        norm_u(m, params + i * NP, u);
+        model_S(m, k, u, 0);
+        memcpy(S + i * P, k->S, 8 * (size_t)P);
+    }
+    free(u);
+    work_free(k);
+    return 0;
+}
+
+/* lasp_eval_grad: chi2, d chi2/d u, continuum coefficients, status bit 1 at given params. */
+int orc_eval_grad(const orc_model *m, int64_t B, const double *flux, const double *ivar,
+                  const uint8_t *mask, const double *params, double *chi2, double *grad_u,
+                  double *cont, int32_t *status)
+{
+    int NP = m->n_labels + 2, P = m->n_pix, nc = m->n_seg * (m->cont_degree + 1);
+#pragma omp parallel
+    {
+        work_t *k = work_new(m);
+        double *u = calloc(NP, 8);
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t i = 0; i < B; ++i) {
+            int st = 0;
+            make_weights(m, ivar + i * P, mask ? mask + i * P : NULL, k->w);
+            norm_u(m, params + i * NP, u);
+            chi2[i] = chi2_at(m, k, u, flux + i * P, 1, &st);
+            grad_from_work(k, grad_u + i * NP);
+            if (cont) memcpy(cont + i * nc, k->b, 8 * (size_t)nc);
+            if (status) status[i] = st;
+        }
+        free(u);
+        work_free(k);
+    }
+    return 0;
+}
+
+/* chi2 only (re-solving the continuum), at normalised u -- used by the finite-difference pins. */
+int orc_chi2_u(const orc_model *m, const double *flux, const double *ivar, const uint8_t *mask,
+               const double *u, double *chi2)
+{
+    work_t *k = work_new(m);
+    make_weights(m, ivar, mask, k->w);
+    *chi2 = chi2_at(m, k, u, flux, 0, NULL);
+    work_free(k);
+    return 0;
+}
+
+/* lasp_fit_batch (fit + outputs + errors of C.1).  trace may be NULL, else [B*(n_iter+1)]
+ * receives chi2 at every iterate (trace[t] = chi2 at the u the t-th gradient was taken at,
+ * trace[n_iter] = final). */
+int orc_fit(const orc_model *m, int64_t B, const double *flux, const double *ivar,
+            const uint8_t *mask, const double *init, int n_iter, double lr, double b1, double b2,
+            double eps, double fd_h, double *params, double *cont, double *chi2, double *err,
+            int32_t *status, double *trace)
+{
+    int NP = m->n_labels + 2, P = m->n_pix, nc = m->n_seg * (m->cont_degree + 1);
+#pragma omp parallel
+    {
+        work_t *k = work_new(m);
+        double *u = calloc(NP, 8), *mom = calloc(NP, 8), *vel = calloc(NP, 8), *g = calloc(NP, 8);
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t i = 0; i < B; ++i) {
+            const double *y = flux + i * P;
+            make_weights(m, ivar + i * P, mask ? mask + i * P : NULL, k->w);
+            norm_u(m, init + i * NP, u);
+            memset(mom, 0, 8 * NP);
+            memset(vel, 0, 8 * NP);
+            for (int t = 1; t <= n_iter; ++t) {
+                double c2 = chi2_at(m, k, u, y, 1, NULL);
+                if (trace) trace[i * (n_iter + 1) + (t - 1)] = c2;
+                grad_from_work(k, g);
+                orc_adam_step(NP, u, mom, vel, g, t, lr, b1, b2, eps);
+            }
+            int st = 0;
+            double c2 = chi2_at(m, k, u, y, 0, &st); /* one more evaluation at the final u (C.2-21) */
+            if (trace) trace[i * (n_iter + 1) + n_iter] = c2;
+            chi2[i] = c2;
+            denorm(m, u, params + i * NP);
+            if (cont) memcpy(cont + i * nc, k->b, 8 * (size_t)nc);
+            st = final_status(k, u, c2, st);
+            if (status) status[i] = st;
+            if (err) errors_one(m, k, u, y, fd_h, err + i * NP);
+        }
+        free(u); free(mom); free(vel); free(g);
+        work_free(k);
+    }
+    return 0;
+}
+
+/* Pins call these two directly. */
+int orc_solve_continuum(const orc_model *m, const double *S, const double *y, const double *w,
+                        double *b, double *c)
+{
+    work_t *k = work_new(m);
+    memcpy(k->S, S, 8 * (size_t)k->P);
+    memcpy(k->w, w, 8 * (size_t)k->P);
+    int st = solve_continuum(m, k, y);
+    memcpy(b, k->b, 8 * (size_t)k->nc);
+    if (c) memcpy(c, k->c, 8 * (size_t)k->P);
+    work_free(k);
+    return st;
+}
+
+int orc_support_cap(const orc_model *m) { return support_cap(m); }

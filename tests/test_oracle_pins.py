@@ -1,0 +1,518 @@
+"""Pins for the fp64 oracle (oracle/lasp_oracle.c) against things OTHER than itself:
+values the paper prints (tests/golden/paper_values.txt), numpy library routines, closed forms,
+finite differences, brute force and statistical invariants.
+CPU only: `pytest -m "not gpu"`.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+from numpy.polynomial import legendre as npleg
+
+from paper_2512_24840_b200 import synth
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden", "paper_values.txt")
+
+
+def golden():
+    out = {}
+    for line in open(GOLD):
+        if line.startswith("#") or "|" not in line:
+            continue
+        k, v, _ = [t.strip() for t in line.split("|", 2)]
+        out[k] = float(v)
+    return out
+
+
+def small_config(**kw):
+    """A small single-segment log-grid model (592 px, K=10 cubic-ish, D=4)."""
+    base = dict(cfg=7, name="pin-small", B=4, grid="log10", lam_min=4800.0, lam_max=5500.0, step=1e-4,
+                seg_bounds=None, sigma_inst=(0.0,), K=10, L=3, D=4, n_iter=50, snr=(50.0, 50.0),
+                noise="const", mask_frac=0.03, parity_B=4)
+    base.update(kw)
+    return synth.Config(**base)
+
+
+def two_arm_config(**kw):
+    """Two segments on a LINEAR grid with instrumental widths (exercises C.2-13, -14)."""
+    base = dict(cfg=8, name="pin-2arm", B=3, grid="linear", lam_min=5000.0, lam_max=5000.0 + 0.8 * 699,
+                step=0.8, seg_bounds=(0, 380, 700), sigma_inst=(70.0, 45.0), K=10, L=3, D=3, n_iter=20,
+                snr=(80.0, 80.0), noise="poisson", mask_frac=0.05, parity_B=3)
+    base.update(kw)
+    return synth.Config(**base)
+
+
+def make(cfgobj, oracle_mod, B=None, noise_free=False):
+    synth.CONFIGS["_tmp"] = cfgobj
+    try:
+        return synth.make_case("_tmp", oracle_mod.forward, B=B, noise_free=noise_free)
+    finally:
+        del synth.CONFIGS["_tmp"]
+
+
+# ---------------------------------------------------------------- grid
+
+def test_grid_pixel_counts_match_paper():
+    g = golden()
+    assert synth.loglam_grid("log10", 4200.0, 5700.0, 1e-4).size == g["grid_pixels_4200_5700_log10_1e-4"]
+    assert synth.loglam_grid("log10", 3850.0, 5500.0, 1e-4).size == g["grid_pixels_3850_5500_log10_1e-4"]
+    assert synth.loglam_grid("linear", 3600.0, 9824.0, 0.8).size == 7781  # BASELINE.json configs[4]
+
+
+def test_pixel_velocity_scale(oracle_mod):
+    g = golden()
+    case = make(small_config(), oracle_mod, B=1)
+    s = oracle_mod.Oracle(case["desc"]).pixel_kms()
+    assert np.allclose(s, g["kms_per_pixel_log10_1e-4"], rtol=2e-6)
+    # linear grid: s_j = c * dlambda/lambda (Appendix of SURVEY.md: 66.6 km/s at 3600 A, 24.4 at 9824 A)
+    d = synth.make_model_desc(synth.CONFIGS[2]); d.pop("_rng")
+    s2 = oracle_mod.Oracle(d).pixel_kms()
+    lam = 10 ** d["loglam"]
+    ends = np.zeros(lam.size, dtype=bool)
+    ends[d["seg_offset"][:-1]] = True; ends[d["seg_offset"][1:] - 1] = True
+    assert np.allclose(s2[~ends], synth.C_KMS * 0.8 / lam[~ends], rtol=1e-6)   # centred differences
+    assert np.allclose(s2[ends], synth.C_KMS * 0.8 / lam[ends], rtol=2e-4)     # one-sided at segment ends
+    assert abs(s2[0] - 66.6) < 0.05 and abs(s2[-1] - 24.4) < 0.05
+
+
+def test_edge_exclusion_rule(oracle_mod):
+    # 28 px for configs 0/1/3, 47/61/79 for the three DESI segments
+    d = synth.make_model_desc(synth.CONFIGS[1]); d.pop("_rng")
+    assert list(d["seg_n_edge"]) == [28]
+    d2 = synth.make_model_desc(synth.CONFIGS[2]); d2.pop("_rng")
+    assert list(d2["seg_n_edge"]) == [47, 61, 79]
+    # and it really covers the largest support of the prior box
+    o = oracle_mod.Oracle(d2)
+    s = o.pixel_kms()
+    for k in range(3):
+        a, b = d2["seg_offset"][k], d2["seg_offset"][k + 1]
+        st = math.hypot(300.0, float(d2["seg_sigma_inst"][k]))
+        Hmax = math.ceil(400.0 / s[a:b].min() + 5 * st / s[a:b].min())
+        assert d2["seg_n_edge"][k] >= Hmax
+
+
+# ---------------------------------------------------------------- emulator (Eq. 1)
+
+def test_term_tables():
+    g = golden()
+    e = synth.monomial_exps(13, 105)
+    assert e.shape[0] == g["quadratic_terms_13_labels"] == 1 + 13 + 13 * 14 // 2
+    assert e.sum(axis=1).max() == 2 and len({tuple(r) for r in e}) == 105
+    e3 = synth.monomial_exps(3, 26)
+    assert (e3[:20].sum(axis=1) <= 3).all() and len({tuple(r) for r in e3[:20]}) == 20
+    # then x1^4, x1^3 x2, x1^3 x3, x1^2 x2^2, x1^2 x2 x3, x1^2 x3^2
+    assert [tuple(r) for r in e3[20:]] == [(4, 0, 0), (3, 1, 0), (3, 0, 1), (2, 2, 0), (2, 1, 1), (2, 0, 2)]
+
+
+def test_monomials_brute_force_and_fd(oracle_mod):
+    d = synth.make_model_desc(synth.CONFIGS[4]); d.pop("_rng")
+    o = oracle_mod.Oracle(d)
+    rng = np.random.default_rng(1)
+    theta = o.denorm(rng.uniform(-0.9, 0.9, o.NP))
+    x, phi, dphi, dxdt = o.monomials(theta[: o.L])
+    # x: Teff through log10, the rest affine; all inside [-1,1]
+    tau = theta[: o.L].copy()
+    tau[0] = math.log10(tau[0])  # only Teff goes through log10 (C.2-19)
+    xe = d["emu_a"].astype(np.float64) * tau + d["emu_b"].astype(np.float64)
+    assert np.allclose(x, xe, rtol=1e-13, atol=1e-13) and np.all(np.abs(x) <= 1)
+    # phi: product definition through numpy power
+    ref = np.prod(x[None, :] ** d["term_exps"].astype(np.float64), axis=1)
+    assert np.allclose(phi, ref, rtol=1e-13)
+    # dphi/dx_l by central differences of the numpy definition
+    for l in range(o.L):
+        h = 1e-6
+        xp, xm = x.copy(), x.copy()
+        xp[l] += h; xm[l] -= h
+        fd = (np.prod(xp[None, :] ** d["term_exps"], axis=1) - np.prod(xm[None, :] ** d["term_exps"], axis=1)) / (2 * h)
+        assert np.allclose(dphi[l], fd, rtol=1e-7, atol=1e-9)
+    # chain factor d x / d theta
+    assert np.isclose(dxdt[0], d["emu_a"][0] / (theta[0] * math.log(10.0)), rtol=1e-13)
+    assert np.allclose(dxdt[1:], d["emu_a"][1:], rtol=1e-13)
+
+
+def test_emulator_is_einsum_and_constant_term_at_origin(oracle_mod):
+    case = make(small_config(), oracle_mod, B=1)
+    d = case["desc"]; o = oracle_mod.Oracle(d)
+    # tiny broadening, zero shift => S == T to ~1e-12 (pure identity kernel: see test below)
+    theta = o.denorm(np.zeros(o.NP))
+    theta[o.L] = 0.0
+    _, phi, _, _ = o.monomials(theta[: o.L])
+    T = np.einsum("k,kp->p", phi, d["coeffs"].astype(np.float64))
+    # x = 0 for every label at the box centre (in the emulator's variable) -> only the constant term
+    x, phi0, _, _ = o.monomials(np.array([math.sqrt(3500.0 * 8000.0), 3.0, -1.0]))
+    assert np.allclose(x, 0.0, atol=1e-6)
+    assert np.isclose(phi0[0], 1.0) and np.allclose(phi0[1:], 0.0, atol=1e-6)
+    # brute-force triple loop on the first 7 pixels
+    for j in range(7):
+        acc = 0.0
+        for k in range(o.K):
+            acc += phi[k] * float(d["coeffs"][k, j])
+        assert abs(acc - T[j]) < 1e-13
+
+
+# ---------------------------------------------------------------- kernel (Eq. 5)
+
+def test_kernel_support_rule_and_unit_sum(oracle_mod):
+    g = golden()
+    H, w, _, _ = oracle_mod.Oracle.kernel_weights(1.3, 2.0)
+    assert w.size == g["kernel_length_mu_1.3_sigma_2.0"] and H == 12
+    H, w, _, _ = oracle_mod.Oracle.kernel_weights(-2.9, 0.72)
+    assert w.size == g["kernel_length_mu_-2.9_sigma_0.72"]
+    for mu, sg in [(0.0, 0.3), (2.5, 1.7), (-5.8, 4.3), (0.49, 0.29)]:
+        H, w, wm, ws = oracle_mod.Oracle.kernel_weights(mu, sg)
+        assert H == math.ceil(abs(mu) + 5 * sg) and w.size == 2 * H + 1
+        assert abs(w.sum() - 1.0) < 1e-14
+        assert abs(wm.sum()) < 1e-13 and abs(ws.sum()) < 1e-13  # derivatives of a unit-sum kernel
+        k = np.arange(-H, H + 1)
+        ref = np.exp(-0.5 * ((k - mu) / sg) ** 2)
+        assert np.allclose(w, ref / ref.sum(), rtol=1e-13)
+        assert np.argmax(w) == H + int(round(mu))  # centred at +mu (C.2-11)
+
+
+def test_kernel_derivatives_vs_finite_differences(oracle_mod):
+    kw = oracle_mod.Oracle.kernel_weights
+    for mu, sg in [(0.37, 1.9), (-2.2, 0.8), (3.05, 3.3)]:
+        H, w, wm, ws = kw(mu, sg)
+        h = 1e-6
+        # H held constant (C.2-15): rebuild the perturbed kernels on the same support by hand
+        k = np.arange(-H, H + 1)
+
+        def gk(m, s):
+            e = np.exp(-0.5 * ((k - m) / s) ** 2)
+            return e / e.sum()
+        assert np.allclose(wm, (gk(mu + h, sg) - gk(mu - h, sg)) / (2 * h), rtol=1e-6, atol=1e-9)
+        assert np.allclose(ws, (gk(mu, sg + h) - gk(mu, sg - h)) / (2 * h), rtol=1e-6, atol=1e-9)
+
+
+def _line_model(oracle_mod, a_pix=6.0, depth=0.5, **cfgkw):
+    """A model whose template is a single Gaussian absorption line: K=1 (constant term only),
+    C[0,:] = 1 - depth*exp(-(j-j0)^2/(2 a^2))."""
+    case = make(small_config(K=1, D=0, **cfgkw), oracle_mod, B=1)
+    d = case["desc"]
+    P = d["n_pix"]
+    j = np.arange(P)
+    d["coeffs"] = (1.0 - depth * np.exp(-0.5 * ((j - P // 2) / a_pix) ** 2))[None, :].astype(np.float32)
+    return d, j
+
+
+def test_shift_direction_and_width_addition(oracle_mod):
+    # textbook: Gaussian (width a) convolved with Gaussian (width s) is Gaussian width sqrt(a^2+s^2),
+    # centred at +mu: positive RV moves the line to LONGER wavelength (C.2-11, C.2-12).
+    d, j = _line_model(oracle_mod, a_pix=6.0)
+    o = oracle_mod.Oracle(d)
+    s = o.pixel_kms()[0]
+    v, sig = 150.0, 120.0
+    S = o.eval_S(np.array([[5000.0, 3.0, -1.0, v, sig]]))[0]
+    prof = 1.0 - S
+    cen = (prof * j).sum() / prof.sum()
+    wid = math.sqrt((prof * (j - cen) ** 2).sum() / prof.sum())
+    assert abs(cen - (d["n_pix"] // 2 + v / s)) < 2e-3
+    assert abs(wid - math.sqrt(6.0 ** 2 + (sig / s) ** 2)) < 2e-3
+    assert abs(prof.sum() - 0.5 * 6.0 * math.sqrt(2 * math.pi)) < 1e-4  # flux preserved (C.2-9)
+
+
+def test_constant_kernel_equals_numpy_convolve(oracle_mod):
+    case = make(small_config(), oracle_mod, B=1)
+    d = case["desc"]; o = oracle_mod.Oracle(d)
+    theta = case["truth"][0].astype(np.float64)
+    _, phi, _, _ = o.monomials(theta[: o.L])
+    T = phi @ d["coeffs"].astype(np.float64)
+    s = o.pixel_kms()[0]
+    H, w, _, _ = o.kernel_weights(theta[o.L] / s, theta[o.L + 1] / s)
+    S = o.eval_S(theta[None, :])[0]
+    ref = np.convolve(T, w, mode="valid")  # no padding involved: pixels H .. P-1-H
+    assert np.allclose(S[H: d["n_pix"] - H], ref, rtol=1e-12, atol=1e-13)
+    # replicate-edge clamp on the rest (C.2-16)
+    Tpad = np.concatenate([np.full(H, T[0]), T, np.full(H, T[-1])])
+    assert np.allclose(S, np.convolve(Tpad, w, mode="valid"), rtol=1e-12, atol=1e-13)
+    # fitted pixels never read padding: n_edge >= H for anything in the prior box
+    assert d["seg_n_edge"][0] >= H
+
+
+def test_integer_shift_and_constant_template(oracle_mod):
+    d, j = _line_model(oracle_mod, a_pix=3.0)
+    o = oracle_mod.Oracle(d)
+    s = o.pixel_kms()[0]
+    T = d["coeffs"][0].astype(np.float64)
+    # sigma -> small and integer mu: a pure integer shift (box lower bound is 20 km/s = 0.29 px:
+    # neighbours carry exp(-1/(2*0.29^2)) = 2.6e-3, so allow that much smearing)
+    S = o.eval_S(np.array([[5000.0, 3.0, -1.0, 2 * s, 1e-3 * s]]))[0]
+    assert np.allclose(S[5:-5], T[3:-7], atol=1e-12)
+    # a constant template stays constant whatever the kernel
+    d["coeffs"][:] = 0.7
+    S = oracle_mod.Oracle(d).eval_S(np.array([[5000.0, 3.0, -1.0, -133.0, 77.0]]))[0]
+    assert np.allclose(S, np.float64(np.float32(0.7)), rtol=1e-14)
+
+
+def test_per_pixel_kernel_on_linear_grid(oracle_mod):
+    # C.2-13/14: sigma_tot = sqrt(sigma*^2 + sigma_inst^2), mu_j = v/s_j, per pixel, per segment.
+    case = make(two_arm_config(), oracle_mod, B=1)
+    d = case["desc"]; o = oracle_mod.Oracle(d)
+    theta = case["truth"][0].astype(np.float64)
+    _, phi, _, _ = o.monomials(theta[: o.L])
+    T = phi @ d["coeffs"].astype(np.float64)
+    s = o.pixel_kms()
+    S = o.eval_S(theta[None, :])[0]
+    seg = d["seg_offset"]
+    for j in (5, 200, 379, 380, 550, 699):
+        k = 0 if j < seg[1] else 1
+        a, b = seg[k], seg[k + 1]
+        mu = theta[o.L] / s[j]
+        sg = math.hypot(theta[o.L + 1], float(d["seg_sigma_inst"][k])) / s[j]
+        H = math.ceil(abs(mu) + 5 * sg)
+        t = np.arange(-H, H + 1)
+        w = np.exp(-0.5 * ((t - mu) / sg) ** 2); w /= w.sum()
+        ref = sum(w[i] * T[min(max(j - t[i], a), b - 1)] for i in range(t.size))  # never crosses a segment
+        assert abs(S[j] - ref) < 1e-13
+
+
+# ---------------------------------------------------------------- Legendre continuum (Eq. 6)
+
+def test_legendre_matches_numpy(oracle_mod):
+    g = golden()
+    P = 1327
+    x = -1.0 + 2.0 * np.arange(P) / P  # P:127, 0-based
+    assert x[0] == g["legendre_node_first"] and abs(x[-1] - g["legendre_node_last_p1327"]) < 1e-15
+    V = npleg.legvander(x, 50)
+    assert V.shape[1] == g["legendre_table_columns"]
+    for j in (0, 1, 500, 1326):
+        assert np.allclose(oracle_mod.Oracle.legendre(float(x[j]), 50), V[j], rtol=1e-12, atol=1e-13)
+    assert np.allclose(oracle_mod.Oracle.legendre(-1.0, 50), (-1.0) ** np.arange(51))
+
+
+def test_wls_matches_lstsq_and_normal_equations(oracle_mod):
+    case = make(two_arm_config(), oracle_mod, B=2)
+    d = case["desc"]; o = oracle_mod.Oracle(d)
+    S = o.eval_S(case["truth"])
+    n = o.D + 1
+    for i in range(2):
+        y = case["flux"][i].astype(np.float64)
+        w = case["ivar"][i].astype(np.float64) * case["mask"][i]
+        for k in range(o.n_seg):  # apply the edge exclusion by hand
+            a, b = d["seg_offset"][k], d["seg_offset"][k + 1]
+            w[a: a + d["seg_n_edge"][k]] = 0.0
+            w[b - d["seg_n_edge"][k]: b] = 0.0
+        bb, c, st = o.solve_continuum(S[i], y, w)
+        assert st == 0
+        for k in range(o.n_seg):
+            a, b = d["seg_offset"][k], d["seg_offset"][k + 1]
+            x = -1.0 + 2.0 * np.arange(b - a) / (b - a)
+            Phi = S[i, a:b, None] * npleg.legvander(x, o.D)
+            sw = np.sqrt(w[a:b])
+            ref = np.linalg.lstsq(Phi * sw[:, None], y[a:b] * sw, rcond=None)[0]
+            assert np.allclose(bb[k * n:(k + 1) * n], ref, rtol=1e-8, atol=1e-10)
+            assert np.allclose(c[a:b], npleg.legval(x, bb[k * n:(k + 1) * n]), rtol=1e-12)  # C.2-8
+            r = y[a:b] - c[a:b] * S[i, a:b]
+            nrm = np.abs(Phi.T @ (w[a:b] * y[a:b])).max()
+            assert np.abs(Phi.T @ (w[a:b] * r)).max() < 1e-9 * nrm  # Phi^T W r = 0
+
+
+def test_wls_recovers_true_continuum_noise_free(oracle_mod):
+    case = make(two_arm_config(), oracle_mod, B=2, noise_free=True)
+    o = oracle_mod.Oracle(case["desc"])
+    chi2, grad, cont, st = o.eval_grad(case["flux"], case["ivar"], case["mask"], case["truth"])
+    # flux went through float32, so "exact" means float32 rounding of the data
+    assert np.allclose(cont, case["cont"], atol=2e-6)
+    assert np.all(st == 0)
+
+
+# ---------------------------------------------------------------- gradient / envelope
+
+@pytest.mark.parametrize("which", ["log1seg", "lin2seg"])
+def test_gradient_vs_fd_of_resolved_chi2(oracle_mod, which):
+    """north_star check 1 + SURVEY C.2-5: the analytic partial gradient at fixed b equals the
+    central difference of chi2(u) WITH the continuum re-solved (envelope theorem), every
+    parameter, both segment paths."""
+    case = make(small_config() if which == "log1seg" else two_arm_config(), oracle_mod, B=2)
+    o = oracle_mod.Oracle(case["desc"])
+    chi2, grad, cont, st = o.eval_grad(case["flux"], case["ivar"], case["mask"], case["init"])
+    for i in range(2):
+        u = o.norm_u(case["init"][i])
+        assert np.isclose(o.chi2_u(case["flux"][i], case["ivar"][i], case["mask"][i], u), chi2[i], rtol=1e-13)
+        for p in range(o.NP):
+            h = 1e-6
+            up, um = u.copy(), u.copy()
+            up[p] += h; um[p] -= h
+            fd = (o.chi2_u(case["flux"][i], case["ivar"][i], case["mask"][i], up)
+                  - o.chi2_u(case["flux"][i], case["ivar"][i], case["mask"][i], um)) / (2 * h)
+            assert abs(fd - grad[i, p]) <= 2e-6 * np.abs(grad[i]).max(), (which, i, p, fd, grad[i, p])
+
+
+def test_masked_pixels_do_not_leak(oracle_mod):
+    case = make(small_config(mask_frac=0.1), oracle_mod, B=1)
+    o = oracle_mod.Oracle(case["desc"])
+    f2 = case["flux"].copy()
+    assert (f2[case["mask"] == 0] == 1e3).all()
+    f2[case["mask"] == 0] = -77.0
+    # also scribble on the excluded edge pixels
+    ne = case["desc"]["seg_n_edge"][0]
+    f2[:, :ne] = 5.0; f2[:, -ne:] = -5.0
+    a = o.eval_grad(case["flux"], case["ivar"], case["mask"], case["init"])
+    b = o.eval_grad(f2, case["ivar"], case["mask"], case["init"])
+    assert a[0][0] == b[0][0] and np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2])
+
+
+def test_noise_free_stationarity_and_recovery(oracle_mod):
+    """north_star check 2: at the truth on noise-free self-generated data chi2 = 0 and grad = 0
+    (to the float32 rounding of the stored flux); from config-0 style offsets the fit returns."""
+    case = make(small_config(D=4, n_iter=400), oracle_mod, B=4, noise_free=True)
+    o = oracle_mod.Oracle(case["desc"])
+    chi2, grad, _, _ = o.eval_grad(case["flux"], case["ivar"], None, case["truth"])
+    npx = case["desc"]["n_pix"]
+    assert np.all(chi2 < npx * (2e-7) ** 2 * 4)
+    chi0, g0, _, _ = o.eval_grad(case["flux"], case["ivar"], None, case["init"])
+    assert np.all(np.abs(grad).max(axis=1) < 1e-5 * np.abs(g0).max(axis=1))
+    r = o.fit(case["flux"], case["ivar"], None, case["init"], 600, lr=0.03, want_err=False, want_trace=True)
+    rngs = (o.hi - o.lo)
+    assert np.all(r["chi2"] < 1e-6 * chi0)
+    assert np.all(np.abs(r["params"] - case["truth"]) < 1e-3 * rngs)
+    assert np.all(r["status"] == 0)
+
+
+# ---------------------------------------------------------------- Adam
+
+def test_adam_hand_computed_steps(oracle_mod):
+    """north_star check 3.  Step 1: m^ = g, v^ = g^2 => du = -lr g/(|g|+eps).
+    Step 2 from the closed forms of the bias-corrected moments with two given gradients."""
+    g = golden()
+    b1, b2, eps, lr = g["adam_beta1"], g["adam_beta2"], g["adam_eps"], 0.01
+    u0 = np.array([0.2, -0.5, 0.0])
+    g1 = np.array([3.0, -1e-3, 0.0])
+    g2 = np.array([-1.0, 2e-3, 5.0])
+    u1, m1, v1 = oracle_mod.Oracle.adam_step(u0, np.zeros(3), np.zeros(3), g1, 1, lr)
+    assert np.allclose(u1, u0 - lr * g1 / (np.abs(g1) + eps), rtol=1e-14, atol=1e-16)
+    assert u1[2] == u0[2]
+    u2, m2, v2 = oracle_mod.Oracle.adam_step(u1, m1, v1, g2, 2, lr)
+    mh = ((1 - b1) * (b1 * g1 + g2)) / (1 - b1 ** 2)
+    vh = ((1 - b2) * (b2 * g1 ** 2 + g2 ** 2)) / (1 - b2 ** 2)
+    assert np.allclose(u2, u1 - lr * mh / (np.sqrt(vh) + eps), rtol=1e-13, atol=1e-16)
+    # clip to [-1,1] (C.2-18)
+    u3, _, _ = oracle_mod.Oracle.adam_step(np.array([0.995]), np.zeros(1), np.zeros(1), np.array([-4.0]), 1, lr)
+    assert u3[0] == 1.0
+
+
+def test_adam_matches_torch_optimizer(oracle_mod):
+    torch = pytest.importorskip("torch")
+    A = np.array([[3.0, 0.5], [0.5, 1.0]]); c = np.array([0.3, -0.2])
+    u = np.array([0.5, -0.4]); m = np.zeros(2); v = np.zeros(2)
+    tu = torch.tensor(u, dtype=torch.float64, requires_grad=True)
+    opt = torch.optim.Adam([tu], lr=0.02)  # defaults: betas (0.9, 0.999), eps 1e-8
+    tA, tc = torch.tensor(A), torch.tensor(c)
+    for t in range(1, 41):
+        opt.zero_grad()
+        loss = 0.5 * (tu - tc) @ tA @ (tu - tc)
+        loss.backward()
+        opt.step()
+        u, m, v = oracle_mod.Oracle.adam_step(u, m, v, A @ (u - c), t, 0.02)
+        assert np.allclose(u, tu.detach().numpy(), rtol=1e-12, atol=1e-14)
+
+
+# ---------------------------------------------------------------- error estimate
+
+def _numpy_rho(o, d, y, w, u):
+    """Independent numpy restatement of rho(u) with the continuum re-solved (lstsq)."""
+    S = o.eval_S(o.denorm(u)[None, :])[0]
+    rho = np.zeros_like(S)
+    for k in range(o.n_seg):
+        a, b = d["seg_offset"][k], d["seg_offset"][k + 1]
+        x = -1.0 + 2.0 * np.arange(b - a) / (b - a)
+        Phi = S[a:b, None] * npleg.legvander(x, o.D)
+        sw = np.sqrt(w[a:b])
+        bb = np.linalg.lstsq(Phi * sw[:, None], y[a:b] * sw, rcond=None)[0]
+        rho[a:b] = sw * (y[a:b] - Phi @ bb)
+    return rho
+
+
+def test_error_estimate_formula(oracle_mod):
+    """Sigma = rho^T rho/(N_good-NP) (J^T J)^-1 with J from central differences of the re-solved
+    whitened residual, rebuilt here in numpy from eval_S + lstsq."""
+    case = make(small_config(n_iter=300, snr=(60.0, 60.0)), oracle_mod, B=2)
+    d = case["desc"]; o = oracle_mod.Oracle(d)
+    r = o.fit(case["flux"], case["ivar"], case["mask"], case["init"], 300, lr=0.03)
+    ne = d["seg_n_edge"][0]
+    for i in range(2):
+        y = case["flux"][i].astype(np.float64)
+        w = case["ivar"][i].astype(np.float64) * case["mask"][i]
+        w[:ne] = 0; w[-ne:] = 0
+        u = o.norm_u(r["params"][i])
+        h = 1e-5
+        J = np.empty((d["n_pix"], o.NP))
+        for p in range(o.NP):
+            up, um = u.copy(), u.copy()
+            up[p] += h; um[p] -= h
+            J[:, p] = (_numpy_rho(o, d, y, w, up) - _numpy_rho(o, d, y, w, um)) / (2 * h)
+        rho = _numpy_rho(o, d, y, w, u)
+        ngood = int((w > 0).sum())
+        cov = (rho @ rho) / (ngood - o.NP) * np.linalg.inv(J.T @ J)
+        ref = np.sqrt(np.diag(cov)) * (o.hi - o.lo) / 2
+        assert np.allclose(r["err"][i], ref, rtol=1e-5)
+        assert np.isclose(rho @ rho, r["chi2"][i], rtol=1e-9)
+
+
+def test_error_estimate_reduces_to_ols_covariance(oracle_mod):
+    """Textbook special case: for small perturbations the model is linear in (u, b); the
+    variable-projected J^T J is the Schur complement of the full Gauss-Newton matrix, so the
+    oracle's errors equal sqrt(diag) of the u-block of s^2 (Jf^T Jf)^-1 with Jf = [d/du, d/db]."""
+    case = make(small_config(n_iter=300, snr=(400.0, 400.0), mask_frac=0.0), oracle_mod, B=1)
+    d = case["desc"]; o = oracle_mod.Oracle(d)
+    r = o.fit(case["flux"], case["ivar"], None, case["init"], 400, lr=0.03)
+    ne = d["seg_n_edge"][0]
+    y = case["flux"][0].astype(np.float64)
+    w = case["ivar"][0].astype(np.float64).copy(); w[:ne] = 0; w[-ne:] = 0
+    sw = np.sqrt(w)
+    u = o.norm_u(r["params"][0])
+    x = -1.0 + 2.0 * np.arange(d["n_pix"]) / d["n_pix"]
+    V = npleg.legvander(x, o.D)
+    b = r["cont"][0]
+    S0 = o.eval_S(o.denorm(u)[None, :])[0]
+    cols = []
+    for p in range(o.NP):
+        h = 1e-6
+        up, um = u.copy(), u.copy(); up[p] += h; um[p] -= h
+        dS = (o.eval_S(o.denorm(up)[None, :])[0] - o.eval_S(o.denorm(um)[None, :])[0]) / (2 * h)
+        cols.append(-sw * (V @ b) * dS)
+    Jf = np.column_stack(cols + [-sw * S0 * V[:, n] for n in range(o.D + 1)])
+    ngood = int((w > 0).sum())
+    cov = r["chi2"][0] / (ngood - o.NP) * np.linalg.inv(Jf.T @ Jf)
+    ref = np.sqrt(np.diag(cov))[: o.NP] * (o.hi - o.lo) / 2
+    # equal up to the O(residual) Golub-Pereyra term, tiny at SNR 400
+    assert np.allclose(r["err"][0], ref, rtol=2e-3)
+
+
+@pytest.mark.slow
+def test_errors_match_monte_carlo_scatter(oracle_mod):
+    """The paper's own validation idea: reported errors ~ scatter over noise realisations."""
+    cfgobj = small_config(n_iter=250, snr=(40.0, 40.0), mask_frac=0.0, D=3)
+    case = make(cfgobj, oracle_mod, B=1, noise_free=True)
+    d = case["desc"]; o = oracle_mod.Oracle(d)
+    rng = np.random.default_rng(5)
+    R = 160
+    model = case["model"][0]
+    sig = np.median(model) / 40.0
+    flux = (model[None, :] + sig * rng.standard_normal((R, model.size))).astype(np.float32)
+    ivar = np.full_like(flux, 1.0 / sig ** 2)
+    init = np.repeat(case["truth"], R, axis=0)
+    r = o.fit(flux, ivar, None, init, 250, lr=0.03)
+    scatter = r["params"].std(axis=0, ddof=1)
+    ratio = np.median(r["err"], axis=0) / scatter
+    assert np.all(np.abs(ratio - 1.0) < 0.2), ratio
+    ne = d["seg_n_edge"][0]
+    dof = model.size - 2 * ne - o.NP - o.nc
+    assert abs(np.mean(r["chi2"]) / dof - 1.0) < 0.03  # C.3: chi2/(N_good-NP-n_c) ~ 1
+
+
+# ---------------------------------------------------------------- status bits (8(b))
+
+def test_status_bits(oracle_mod):
+    case = make(small_config(n_iter=5), oracle_mod, B=3)
+    d = case["desc"]; o = oracle_mod.Oracle(d)
+    mask = case["mask"].copy(); flux = case["flux"].copy(); init = case["init"].copy()
+    mask[0, :] = 0                      # nothing to fit: continuum system is not positive definite
+    flux[1, :] = -np.abs(flux[1, :])    # negative flux -> negative multiplicative correction
+    init[2, o.L] = 400.0                # RV on its bound, gradient pushes outward or not: force bound
+    r = o.fit(flux, case["ivar"], mask, init, 0, want_err=False)
+    assert r["status"][0] & 1 and r["chi2"][0] == 0.0 and np.all(r["cont"][0] == 0.0)
+    assert r["status"][1] & 4 and not (r["status"][1] & 1)
+    assert r["status"][2] & 8
+    assert np.allclose(r["params"][0], init[0], rtol=1e-12)  # zero steps: params = init
