@@ -1,0 +1,133 @@
+/*
+ * lasp_gpu.h -- C ABI of the B200-native LASP-Adam fitting hot path (arXiv 2512.24840).
+ *
+ * "P:n" = /root/reference/PAPER.md line n; "C.2-n" = row n of the table of readings in
+ * SURVEY.md section 8(c); DESIGN.md restates every reading.
+ *
+ * The library fits, for B observed spectra on one common wavelength grid, the NP = L+2
+ * non-linear parameters (L emulator labels, radial velocity v, stellar broadening sigma*)
+ * by a fixed number of Adam steps on  chi2 = sum_j w_j (y_j - c_j S_j)^2,
+ * w = mask*ivar (Eq. 7-9), where
+ *     S = G(mu,sigma) (*) T        Doppler shift + Gaussian broadening      (Eq. 5)
+ *     T_j = sum_k phi_k(x) C[k,j]  polynomial spectral emulator             (Eq. 1)
+ *     c = P(x^) b                  multiplicative Legendre continuum whose coefficients are
+ *                                  re-solved by weighted least squares in EVERY evaluation
+ *                                  (Eq. 6; C.2-4)
+ * and returns parameters, continuum coefficients, chi2, the error estimate of P:173 and status
+ * bits.  Every step runs in hand-written sm_100a CUDA kernels; there is no CPU fallback.
+ *
+ * Conventions
+ *  - All functions return 0 (LASP_OK) or a negative LASP_ERR_* code; they never throw or abort.
+ *  - lasp_model_desc and everything it points to is HOST memory, copied during lasp_create.
+ *  - Pointers named in the batch calls (flux, ivar, mask, init, params, cont, chi2, err, status,
+ *    model, grad_u) are DEVICE pointers owned by the caller (e.g. torch allocations).  The
+ *    library reads inputs, writes outputs, and neither frees nor retains them.  Inputs are never
+ *    modified.  Row-major, spectrum-major: element (i, j) at [i*n_pix + j].
+ *  - `stream` is a cudaStream_t passed as void* (NULL = default stream).  All work is enqueued on
+ *    it and the call returns without synchronising, except that the first call for a larger B
+ *    than seen before grows the ctx-owned workspace with cudaMalloc (use lasp_reserve to do that
+ *    up front).
+ *  - Parameter order everywhere: labels[0..L-1], rv (km/s), sigma* (km/s), physical units.
+ *  - A ctx may be used from one host thread at a time; different ctxs are independent.
+ *  - Per-spectrum problems never fail a call; they set bits in status[i].
+ */
+#ifndef LASP_GPU_H
+#define LASP_GPU_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LASP_OK 0
+#define LASP_ERR_INVALID_ARG (-1) /* null pointer, bad shape, non-monotone grid, lo>=hi, sigma lower bound <=0 */
+#define LASP_ERR_CUDA (-2)        /* a CUDA runtime call failed; see lasp_last_error */
+#define LASP_ERR_NOMEM (-3)       /* device or host allocation failed */
+#define LASP_ERR_UNSUPPORTED (-4) /* shape outside the compiled limits (see LASP_MAX_*) */
+
+#define LASP_MAX_SEG 8
+#define LASP_MAX_LABELS 30
+#define LASP_MAX_TERMS 512
+#define LASP_MAX_DEGREE 31 /* D+1 <= 32: one continuum row per warp lane in the solver */
+
+/* status[i] bits */
+#define LASP_ST_NOT_SPD 1   /* a segment's continuum system was not positive definite; its b = 0 */
+#define LASP_ST_NONFINITE 2 /* a non-finite value was met */
+#define LASP_ST_NEG_CONT 4  /* continuum c_j <= 0 on a fitted pixel at the solution */
+#define LASP_ST_ON_BOUND 8  /* a parameter ended on its prior bound */
+
+typedef struct lasp_ctx lasp_ctx; /* opaque; owns only its own device copies and workspace */
+
+typedef struct {
+    int32_t n_pix, n_seg;
+    const int32_t *seg_offset;   /* [n_seg+1], seg_offset[0]==0, seg_offset[n_seg]==n_pix; the stencil
+                                    never crosses a segment boundary (replicate-edge clamp, C.2-16) */
+    const double *loglam;        /* [n_pix] log10(lambda/Angstrom), strictly increasing inside each
+                                    segment; fp64 because the step is 1e-4 on values ~3.6 */
+    const float *seg_sigma_inst; /* [n_seg] km/s, added in quadrature to sigma* (C.2-13) */
+    int32_t n_labels, n_terms;   /* L, K */
+    const uint8_t *term_exps;    /* [K*L] monomial exponents, phi_k = prod_l x_l^e_kl (Eq. 1, C.2-24) */
+    const float *coeffs;         /* [K*n_pix] row-major emulator coefficients on the observed grid */
+    const float *lo, *hi;        /* [NP] prior box, physical units; parameters are optimised as
+                                    u = 2(theta-lo)/(hi-lo)-1 in [-1,1] (C.2-18) */
+    const uint8_t *label_log10;  /* [L] 1 => tau_l = log10 (C.2-19) */
+    const float *emu_a, *emu_b;  /* [L] emulator input x_l = emu_a*tau_l(theta_l) + emu_b */
+    int32_t cont_degree;         /* D <= LASP_MAX_DEGREE, same for every segment */
+    const int32_t *seg_n_edge;   /* [n_seg] pixels excluded from objective and WLS at each end of the
+                                    segment (C.2-17) */
+} lasp_model_desc;
+
+typedef struct {
+    int32_t n_iter;               /* fixed number of Adam steps (Delta-6) */
+    float lr, beta1, beta2, eps;  /* Adam hyper-parameters (defaults 1e-2, 0.9, 0.999, 1e-8) */
+    int32_t variant;              /* 0 auto; reserved (1 resident, 2 streaming) */
+    int32_t emulator_path;        /* 0 auto; reserved (1 fp32 fma, 2 3xTF32) */
+} lasp_fit_opts;
+
+/* Build a context on `cuda_device`: validates the description, derives the per-pixel velocity
+ * scale s_j = c ln10 dloglam (C.2-12), the padded device layout and the basis tables. */
+int lasp_create(const lasp_model_desc *desc, int cuda_device, lasp_ctx **out);
+int lasp_destroy(lasp_ctx *ctx);
+
+/* Pre-allocate the workspace for batches of up to B spectra (optional). */
+int lasp_reserve(lasp_ctx *ctx, int64_t B);
+
+/* Steps a0-a9 of SURVEY.md 8(a): n_iter Adam steps from `init`, then one evaluation at the
+ * final iterate (C.2-21).
+ *   flux, ivar [B*n_pix] f32; mask [B*n_pix] u8 (1 = good) or NULL; init [B*NP] physical.
+ *   params [B*NP] physical; cont [B*n_seg*(D+1)] plain-Legendre coefficients (numpy legval
+ *   convention, nodes x_j = -1 + 2(j-o_s)/P_s) or NULL; chi2 [B];
+ *   err [B*NP] = sqrt(diag(rho^T rho/(N_good-NP) (J^T J)^-1)) in physical units (P:173,
+ *   C.2-22/23; NaN when J^T J is singular) or NULL to skip; status [B] or NULL. */
+int lasp_fit_batch(lasp_ctx *ctx, int64_t B, const float *flux, const float *ivar,
+                   const uint8_t *mask, const float *init, const lasp_fit_opts *opts,
+                   float *params, float *cont, float *chi2, float *err, int32_t *status,
+                   void *stream);
+
+/* Inspection: model_j = c_j S_j at given physical params [B*NP] and plain-Legendre cont
+ * [B*n_seg*(D+1)]; model [B*n_pix]. */
+int lasp_eval_model(lasp_ctx *ctx, int64_t B, const float *params, const float *cont,
+                    float *model, void *stream);
+
+/* Inspection: one chi2/gradient evaluation at given physical params: chi2 [B], grad_u [B*NP]
+ * (d chi2 / d u, normalised parameters), cont [B*n_seg*(D+1)] or NULL, status [B] or NULL
+ * (bit LASP_ST_NOT_SPD only). */
+int lasp_eval_grad(lasp_ctx *ctx, int64_t B, const float *flux, const float *ivar,
+                   const uint8_t *mask, const float *params, float *chi2, float *grad_u,
+                   float *cont, int32_t *status, void *stream);
+
+/* Number of kernels launched by this ctx so far (bench.py reports it as gpu_launches). */
+int64_t lasp_launch_count(const lasp_ctx *ctx);
+
+/* Algorithmic FP32 work of one Adam step of one spectrum, in FMA (SURVEY.md 8(d) formula with
+ * the moment route) given the mean number of stencil taps 2H+1; for the roofline line. */
+double lasp_fma_per_spectrum_step(const lasp_ctx *ctx, double mean_taps);
+
+const char *lasp_last_error(const lasp_ctx *ctx); /* ctx-owned string; "" if none; ctx may be NULL */
+int lasp_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LASP_GPU_H */

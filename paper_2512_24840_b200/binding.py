@@ -1,0 +1,198 @@
+"""Thin ctypes binding over include/lasp_gpu.h: argument marshalling only.
+
+PyTorch is used for device memory and streams; every step of the path runs in liblasp_gpu.so.
+There is no CPU fallback: a missing library or a missing CUDA device raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "liblasp_gpu.so")
+
+SYMBOLS = ["lasp_create", "lasp_destroy", "lasp_reserve", "lasp_fit_batch", "lasp_eval_model",
+           "lasp_eval_grad", "lasp_launch_count", "lasp_fma_per_spectrum_step", "lasp_last_error",
+           "lasp_version"]
+
+LASP_ST_NOT_SPD, LASP_ST_NONFINITE, LASP_ST_NEG_CONT, LASP_ST_ON_BOUND = 1, 2, 4, 8
+
+_f32p = C.POINTER(C.c_float)
+_f64p = C.POINTER(C.c_double)
+_i32p = C.POINTER(C.c_int32)
+_u8p = C.POINTER(C.c_uint8)
+
+
+class ModelDesc(C.Structure):
+    _fields_ = [
+        ("n_pix", C.c_int32), ("n_seg", C.c_int32),
+        ("seg_offset", _i32p), ("loglam", _f64p), ("seg_sigma_inst", _f32p),
+        ("n_labels", C.c_int32), ("n_terms", C.c_int32),
+        ("term_exps", _u8p), ("coeffs", _f32p), ("lo", _f32p), ("hi", _f32p),
+        ("label_log10", _u8p), ("emu_a", _f32p), ("emu_b", _f32p),
+        ("cont_degree", C.c_int32), ("seg_n_edge", _i32p),
+    ]
+
+
+class FitOpts(C.Structure):
+    _fields_ = [("n_iter", C.c_int32), ("lr", C.c_float), ("beta1", C.c_float), ("beta2", C.c_float),
+                ("eps", C.c_float), ("variant", C.c_int32), ("emulator_path", C.c_int32)]
+
+
+class LaspError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def lib():
+    """Load liblasp_gpu.so (built in-tree by paper_2512_24840_b200/build.py); fail loudly if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise LaspError(f"{LIB_PATH} is missing: run `python -m paper_2512_24840_b200.build` "
+                            "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        L.lasp_create.argtypes = [C.POINTER(ModelDesc), C.c_int, C.POINTER(C.c_void_p)]
+        L.lasp_create.restype = C.c_int
+        L.lasp_destroy.argtypes = [C.c_void_p]
+        L.lasp_reserve.argtypes = [C.c_void_p, C.c_int64]
+        L.lasp_fit_batch.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 4 + [C.POINTER(FitOpts)] + \
+                                    [C.c_void_p] * 6
+        L.lasp_eval_model.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 4
+        L.lasp_eval_grad.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 9
+        L.lasp_launch_count.argtypes = [C.c_void_p]
+        L.lasp_launch_count.restype = C.c_int64
+        L.lasp_fma_per_spectrum_step.argtypes = [C.c_void_p, C.c_double]
+        L.lasp_fma_per_spectrum_step.restype = C.c_double
+        L.lasp_last_error.argtypes = [C.c_void_p]
+        L.lasp_last_error.restype = C.c_char_p
+        L.lasp_version.restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _p(a, t):
+    return a.ctypes.data_as(t)
+
+
+def _ptr(t):
+    return C.c_void_p(t.data_ptr()) if t is not None else None
+
+
+class LaspModel:
+    """A lasp_ctx bound to one model description (dict of numpy arrays, see synth.make_model_desc)."""
+
+    def __init__(self, desc: dict, device: int = 0):
+        import torch
+        if not torch.cuda.is_available():
+            raise LaspError("no CUDA device: the LASP path runs only in its sm_100a kernels")
+        self.torch = torch
+        self.device = torch.device("cuda", device)
+        self.L = int(desc["n_labels"]); self.K = int(desc["n_terms"]); self.P = int(desc["n_pix"])
+        self.NP = self.L + 2; self.D = int(desc["cont_degree"]); self.n_seg = int(desc["n_seg"])
+        self.nc = self.n_seg * (self.D + 1)
+        k = self._keep = {}
+        k["seg_offset"] = np.ascontiguousarray(desc["seg_offset"], dtype=np.int32)
+        k["loglam"] = np.ascontiguousarray(desc["loglam"], dtype=np.float64)
+        k["seg_sigma_inst"] = np.ascontiguousarray(desc["seg_sigma_inst"], dtype=np.float32)
+        k["term_exps"] = np.ascontiguousarray(desc["term_exps"], dtype=np.uint8)
+        k["coeffs"] = np.ascontiguousarray(desc["coeffs"], dtype=np.float32)
+        k["lo"] = np.ascontiguousarray(desc["lo"], dtype=np.float32)
+        k["hi"] = np.ascontiguousarray(desc["hi"], dtype=np.float32)
+        k["label_log10"] = np.ascontiguousarray(desc["label_log10"], dtype=np.uint8)
+        k["emu_a"] = np.ascontiguousarray(desc["emu_a"], dtype=np.float32)
+        k["emu_b"] = np.ascontiguousarray(desc["emu_b"], dtype=np.float32)
+        k["seg_n_edge"] = np.ascontiguousarray(desc["seg_n_edge"], dtype=np.int32)
+        d = ModelDesc(self.P, self.n_seg, _p(k["seg_offset"], _i32p), _p(k["loglam"], _f64p),
+                      _p(k["seg_sigma_inst"], _f32p), self.L, self.K, _p(k["term_exps"], _u8p),
+                      _p(k["coeffs"], _f32p), _p(k["lo"], _f32p), _p(k["hi"], _f32p),
+                      _p(k["label_log10"], _u8p), _p(k["emu_a"], _f32p), _p(k["emu_b"], _f32p),
+                      self.D, _p(k["seg_n_edge"], _i32p))
+        self.ctx = C.c_void_p()
+        rc = lib().lasp_create(C.byref(d), device, C.byref(self.ctx))
+        if rc != 0:
+            raise LaspError(f"lasp_create failed ({rc}): {lib().lasp_last_error(None).decode()}")
+
+    def close(self):
+        if getattr(self, "ctx", None) is not None and self.ctx:
+            lib().lasp_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc, what):
+        if rc != 0:
+            raise LaspError(f"{what} failed ({rc}): {lib().lasp_last_error(self.ctx).decode()}")
+
+    def _dev(self, a, dtype):
+        t = self.torch
+        if a is None:
+            return None
+        if not isinstance(a, t.Tensor):
+            a = t.from_numpy(np.ascontiguousarray(a))
+        return a.to(device=self.device, dtype=dtype).contiguous()
+
+    def _stream(self):
+        return C.c_void_p(self.torch.cuda.current_stream(self.device).cuda_stream)
+
+    def reserve(self, B: int):
+        self._check(lib().lasp_reserve(self.ctx, B), "lasp_reserve")
+
+    def launch_count(self) -> int:
+        return int(lib().lasp_launch_count(self.ctx))
+
+    def fma_per_spectrum_step(self, mean_taps: float) -> float:
+        return float(lib().lasp_fma_per_spectrum_step(self.ctx, mean_taps))
+
+    def fit_batch(self, flux, ivar, mask, init, n_iter, lr=1e-2, beta1=0.9, beta2=0.999, eps=1e-8,
+                  want_err=True, want_cont=True, out=None):
+        """lasp_fit_batch on device tensors; returns dict of device tensors."""
+        t = self.torch
+        flux = self._dev(flux, t.float32); ivar = self._dev(ivar, t.float32)
+        mask = self._dev(mask, t.uint8); init = self._dev(init, t.float32)
+        B = flux.shape[0]
+        assert flux.shape == (B, self.P) and ivar.shape == (B, self.P) and init.shape == (B, self.NP)
+        if out is None:
+            out = dict(params=t.empty((B, self.NP), device=self.device, dtype=t.float32),
+                       chi2=t.empty(B, device=self.device, dtype=t.float32),
+                       status=t.empty(B, device=self.device, dtype=t.int32),
+                       cont=t.empty((B, self.nc), device=self.device, dtype=t.float32) if want_cont else None,
+                       err=t.empty((B, self.NP), device=self.device, dtype=t.float32) if want_err else None)
+        opts = FitOpts(int(n_iter), lr, beta1, beta2, eps, 0, 0)
+        rc = lib().lasp_fit_batch(self.ctx, B, _ptr(flux), _ptr(ivar), _ptr(mask), _ptr(init), C.byref(opts),
+                                  _ptr(out["params"]), _ptr(out.get("cont")), _ptr(out["chi2"]),
+                                  _ptr(out.get("err")), _ptr(out["status"]), self._stream())
+        self._check(rc, "lasp_fit_batch")
+        return out
+
+    def eval_model(self, params, cont):
+        t = self.torch
+        params = self._dev(params, t.float32); cont = self._dev(cont, t.float32)
+        B = params.shape[0]
+        assert params.shape == (B, self.NP) and cont.shape == (B, self.nc)
+        model = t.empty((B, self.P), device=self.device, dtype=t.float32)
+        rc = lib().lasp_eval_model(self.ctx, B, _ptr(params), _ptr(cont), _ptr(model), self._stream())
+        self._check(rc, "lasp_eval_model")
+        return model
+
+    def eval_grad(self, flux, ivar, mask, params):
+        t = self.torch
+        flux = self._dev(flux, t.float32); ivar = self._dev(ivar, t.float32)
+        mask = self._dev(mask, t.uint8); params = self._dev(params, t.float32)
+        B = flux.shape[0]
+        chi2 = t.empty(B, device=self.device, dtype=t.float32)
+        grad = t.empty((B, self.NP), device=self.device, dtype=t.float32)
+        cont = t.empty((B, self.nc), device=self.device, dtype=t.float32)
+        status = t.empty(B, device=self.device, dtype=t.int32)
+        rc = lib().lasp_eval_grad(self.ctx, B, _ptr(flux), _ptr(ivar), _ptr(mask), _ptr(params), _ptr(chi2),
+                                  _ptr(grad), _ptr(cont), _ptr(status), self._stream())
+        self._check(rc, "lasp_eval_grad")
+        return dict(chi2=chi2, grad_u=grad, cont=cont, status=status)

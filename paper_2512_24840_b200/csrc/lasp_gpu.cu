@@ -1,0 +1,383 @@
+// lasp_gpu.cu -- C-ABI host side of the LASP-Adam fitting library (include/lasp_gpu.h).
+// Host work here is set-up only (validation, layout, basis tables); every step of the hot path
+// runs in the kernels of lasp_kernels.cuh.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "lasp_kernels.cuh"
+
+#define LASP_VERSION 100
+static const double kC_KMS = 299792.458;
+
+struct lasp_ctx {
+    ModelDev M;
+    int device = 0, num_sms = 0, wpb = 1;
+    size_t smem_per_warp = 0;
+    float *dC = nullptr, *dinv_s = nullptr;
+    uint8_t *dexps = nullptr;
+    double *dconv = nullptr;
+    int *dnedge = nullptr;
+    float2 *dYW = nullptr;
+    size_t yw_tiles = 0;
+    float *dscratch = nullptr;
+    size_t scratch_slots = 0;
+    long long launches = 0;
+    double mean_dlog = 0;
+    std::string err;
+};
+
+static std::string g_err;
+
+static int fail(lasp_ctx *c, int code, const std::string &msg)
+{
+    if (c) c->err = msg;
+    g_err = msg;
+    return code;
+}
+
+#define CUDA_TRY(c, call)                                                                     \
+    do {                                                                                      \
+        cudaError_t e_ = (call);                                                              \
+        if (e_ != cudaSuccess)                                                                \
+            return fail(c, e_ == cudaErrorMemoryAllocation ? LASP_ERR_NOMEM : LASP_ERR_CUDA,  \
+                        std::string(#call) + ": " + cudaGetErrorString(e_));                  \
+    } while (0)
+
+static int roundup(int v, int m) { return (v + m - 1) / m * m; }
+
+// Gauss-Legendre nodes and weights on [-1,1] (Newton on P_n), fp64
+static void gauss_legendre(int n, std::vector<double> &x, std::vector<double> &w)
+{
+    x.resize(n); w.resize(n);
+    for (int i = 0; i < n; ++i) {
+        double z = cos(M_PI * (i + 0.75) / (n + 0.5)), pp = 1.0;
+        for (int it = 0; it < 100; ++it) {
+            double p1 = 1.0, p2 = 0.0;
+            for (int j = 0; j < n; ++j) {
+                double p3 = p2;
+                p2 = p1;
+                p1 = ((2.0 * j + 1.0) * z * p2 - j * p3) / (j + 1.0);
+            }
+            pp = n * (z * p1 - p2) / (z * z - 1.0);
+            double dz = p1 / pp;
+            z -= dz;
+            if (fabs(dz) < 1e-15) break;
+        }
+        x[i] = z;
+        w[i] = 2.0 / ((1.0 - z * z) * pp * pp);
+    }
+}
+
+extern "C" int lasp_version(void) { return LASP_VERSION; }
+
+extern "C" const char *lasp_last_error(const lasp_ctx *ctx) { return ctx ? ctx->err.c_str() : g_err.c_str(); }
+
+extern "C" int64_t lasp_launch_count(const lasp_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+extern "C" int lasp_destroy(lasp_ctx *c)
+{
+    if (!c) return LASP_OK;
+    cudaSetDevice(c->device);
+    cudaFree(c->dC); cudaFree(c->dinv_s); cudaFree(c->dexps); cudaFree(c->dconv); cudaFree(c->dnedge);
+    cudaFree(c->dYW); cudaFree(c->dscratch);
+    delete c;
+    return LASP_OK;
+}
+
+extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx **out)
+{
+    if (!d || !out) return fail(nullptr, LASP_ERR_INVALID_ARG, "null desc/out");
+    *out = nullptr;
+    if (!d->seg_offset || !d->loglam || !d->seg_sigma_inst || !d->term_exps || !d->coeffs || !d->lo ||
+        !d->hi || !d->label_log10 || !d->emu_a || !d->emu_b || !d->seg_n_edge)
+        return fail(nullptr, LASP_ERR_INVALID_ARG, "null pointer in lasp_model_desc");
+    const int P = d->n_pix, nseg = d->n_seg, L = d->n_labels, K = d->n_terms, D = d->cont_degree;
+    if (P < 2 || nseg < 1 || L < 1 || K < 1 || D < 0)
+        return fail(nullptr, LASP_ERR_INVALID_ARG, "bad shape");
+    if (nseg > LASP_MAX_SEG || L > LASP_MAX_LABELS || K > LASP_MAX_TERMS || D > LASP_MAX_DEGREE)
+        return fail(nullptr, LASP_ERR_UNSUPPORTED, "shape exceeds LASP_MAX_* limits");
+    if (d->seg_offset[0] != 0 || d->seg_offset[nseg] != P)
+        return fail(nullptr, LASP_ERR_INVALID_ARG, "seg_offset must start at 0 and end at n_pix");
+    const int NP = L + 2;
+    for (int p = 0; p < NP; ++p)
+        if (!(d->lo[p] < d->hi[p])) return fail(nullptr, LASP_ERR_INVALID_ARG, "lo >= hi");
+    if (!(d->lo[L + 1] > 0.f)) return fail(nullptr, LASP_ERR_INVALID_ARG, "sigma lower bound must be > 0");
+    for (int l = 0; l < L; ++l)
+        if (d->label_log10[l] && !(d->lo[l] > 0.f))
+            return fail(nullptr, LASP_ERR_INVALID_ARG, "log10 label needs lo > 0");
+    for (int s = 0; s < nseg; ++s) {
+        int o = d->seg_offset[s], e = d->seg_offset[s + 1];
+        if (e - o < 2) return fail(nullptr, LASP_ERR_INVALID_ARG, "segment shorter than 2 pixels");
+        if (d->seg_n_edge[s] < 0) return fail(nullptr, LASP_ERR_INVALID_ARG, "negative n_edge");
+        if (!(d->seg_sigma_inst[s] >= 0.f)) return fail(nullptr, LASP_ERR_INVALID_ARG, "negative sigma_inst");
+        for (int j = o + 1; j < e; ++j)
+            if (!(d->loglam[j] > d->loglam[j - 1]))
+                return fail(nullptr, LASP_ERR_INVALID_ARG, "loglam not strictly increasing inside a segment");
+    }
+    lasp_ctx *c = new (std::nothrow) lasp_ctx();
+    if (!c) return fail(nullptr, LASP_ERR_NOMEM, "host allocation failed");
+    c->device = cuda_device;
+#define CUDA_TRY_C(call)                                                  \
+    do {                                                                  \
+        cudaError_t e_ = (call);                                          \
+        if (e_ != cudaSuccess) {                                          \
+            std::string m_ = std::string(#call) + ": " + cudaGetErrorString(e_); \
+            lasp_destroy(c);                                              \
+            return fail(nullptr, LASP_ERR_CUDA, m_);                      \
+        }                                                                 \
+    } while (0)
+    CUDA_TRY_C(cudaSetDevice(cuda_device));
+    cudaDeviceProp prop;
+    CUDA_TRY_C(cudaGetDeviceProperties(&prop, cuda_device));
+    c->num_sms = prop.multiProcessorCount;
+
+    ModelDev &M = c->M;
+    memset(&M, 0, sizeof(M));
+    M.n_seg = nseg; M.L = L; M.K = K; M.NP = NP; M.D = D; M.n1 = D + 1; M.nmom = 2 * D + 1;
+    M.P = P; M.nc = nseg * (D + 1);
+    for (int p = 0; p < NP; ++p) { M.lo[p] = d->lo[p]; M.hi[p] = d->hi[p]; }
+    for (int l = 0; l < L; ++l) {
+        M.emu_a[l] = d->emu_a[l]; M.emu_b[l] = d->emu_b[l]; M.label_log10[l] = d->label_log10[l];
+    }
+    // per-pixel velocity scale s_j = c ln10 dloglam (C.1), fp64
+    std::vector<double> s(P);
+    const double vmax = fmax(fabs((double)d->lo[L]), fabs((double)d->hi[L]));
+    const double smax = fmax(fabs((double)d->lo[L + 1]), fabs((double)d->hi[L + 1]));
+    int po = 0, g_rows = 0;
+    M.Hmax = 0;
+    std::vector<double> conv((size_t)nseg * M.n1 * M.n1, 0.0);
+    for (int sg = 0; sg < nseg; ++sg) {
+        const int o = d->seg_offset[sg], e = d->seg_offset[sg + 1], Ps = e - o;
+        double smin = 1e300, smx = 0, ssum = 0;
+        for (int j = o; j < e; ++j) {
+            double dl = (j == o) ? d->loglam[j + 1] - d->loglam[j]
+                      : (j == e - 1) ? d->loglam[j] - d->loglam[j - 1]
+                                     : 0.5 * (d->loglam[j + 1] - d->loglam[j - 1]);
+            s[j] = kC_KMS * log(10.0) * dl;
+            smin = fmin(smin, s[j]); smx = fmax(smx, s[j]); ssum += s[j];
+        }
+        SegDev &S = M.seg[sg];
+        const double si = d->seg_sigma_inst[sg];
+        const int Hm = (int)ceil((vmax + 5.0 * sqrt(smax * smax + si * si)) / smin) + 1;
+        S.halo = roundup(Hm, CH);
+        S.po = po; S.P = Ps; S.o = o;
+        S.len = S.halo + roundup(Ps, CH) + S.halo;
+        po += S.len;
+        S.uniform = (smx - smin) <= 1e-6 * smin ? 1 : 0;
+        S.inv_s = (float)(S.uniform ? (double)Ps / ssum : 1.0 / smin);
+        S.sig_inst = d->seg_sigma_inst[sg];
+        const int ne = d->seg_n_edge[sg];
+        const int jl = ne, jh = Ps - 1 - ne;
+        if (jh >= jl) {
+            S.fit_lo = S.po + S.halo + ne / CH * CH;
+            S.fit_hi = S.po + S.halo + roundup(Ps - ne, CH);
+        } else {
+            S.fit_lo = S.fit_hi = S.po + S.halo;
+        }
+        double ta = 0.0, tb = 0.0;
+        if (jh > jl) { ta = 2.0 / (jh - jl); tb = -(double)(jl + jh) / (jh - jl); }
+        S.ta = (float)ta; S.tb = (float)tb;
+        if (S.uniform) g_rows = std::max(g_rows, 2 * S.halo + 1);
+        M.Hmax = std::max(M.Hmax, S.halo);
+        // conv[m][n] = (2m+1)/2 int P_m(x) T_n(alpha x + beta) dx, exact by Gauss-Legendre (D+1 nodes)
+        // with the device's float ta, tb so that the conversion matches the basis actually used
+        const double alpha = (double)S.ta * Ps / 2.0, beta = (double)S.ta * Ps / 2.0 + (double)S.tb;
+        std::vector<double> gx, gw;
+        gauss_legendre(M.n1 + 1, gx, gw);
+        double *cv = conv.data() + (size_t)sg * M.n1 * M.n1;
+        for (size_t q = 0; q < gx.size(); ++q) {
+            std::vector<double> Pm(M.n1), Tn(M.n1);
+            const double x = gx[q], t = alpha * x + beta;
+            Pm[0] = 1.0; if (M.n1 > 1) Pm[1] = x;
+            for (int n = 1; n + 1 < M.n1; ++n) Pm[n + 1] = ((2.0 * n + 1.0) * x * Pm[n] - n * Pm[n - 1]) / (n + 1.0);
+            Tn[0] = 1.0; if (M.n1 > 1) Tn[1] = t;
+            for (int n = 1; n + 1 < M.n1; ++n) Tn[n + 1] = 2.0 * t * Tn[n] - Tn[n - 1];
+            for (int m = 0; m < M.n1; ++m)
+                for (int n = 0; n < M.n1; ++n) cv[m * M.n1 + n] += 0.5 * (2.0 * m + 1.0) * gw[q] * Pm[m] * Tn[n];
+        }
+    }
+    M.Ppad = po;
+    // padded tables: halos replicate the segment's edge pixel (the clamp of C.2-16 for free)
+    std::vector<float> Cp((size_t)K * M.Ppad), isp(M.Ppad);
+    for (int sg = 0; sg < nseg; ++sg) {
+        const SegDev &S = M.seg[sg];
+        for (int q = 0; q < S.len; ++q) {
+            int rel = q - S.halo;
+            rel = rel < 0 ? 0 : (rel > S.P - 1 ? S.P - 1 : rel);
+            isp[S.po + q] = (float)(1.0 / s[S.o + rel]);
+            for (int k = 0; k < K; ++k) Cp[(size_t)k * M.Ppad + S.po + q] = d->coeffs[(size_t)k * P + S.o + rel];
+        }
+    }
+    // shared-memory rows per warp
+    int r = 0;
+    M.r_U = r; r += NP; M.r_M = r; r += NP; M.r_V = r; r += NP;
+    M.r_PHI = r; r += K; M.r_Q = r; r += K;
+    M.r_G = r; r += g_rows;
+    M.r_MOM = r; r += M.nmom; M.r_RHS = r; r += M.n1; M.r_B = r; r += M.nc;
+    M.rows = r;
+    M.nscr = A_J0 + NP;
+    c->smem_per_warp = (size_t)M.rows * RS * sizeof(float);
+    const size_t smem_max = prop.sharedMemPerBlockOptin;
+    c->wpb = (int)std::min<size_t>(8, smem_max / c->smem_per_warp);
+    if (c->wpb < 1) { lasp_destroy(c); return fail(nullptr, LASP_ERR_UNSUPPORTED, "per-warp state exceeds shared memory"); }
+
+    CUDA_TRY_C(cudaMalloc(&c->dC, Cp.size() * sizeof(float)));
+    CUDA_TRY_C(cudaMemcpy(c->dC, Cp.data(), Cp.size() * sizeof(float), cudaMemcpyHostToDevice));
+    CUDA_TRY_C(cudaMalloc(&c->dinv_s, isp.size() * sizeof(float)));
+    CUDA_TRY_C(cudaMemcpy(c->dinv_s, isp.data(), isp.size() * sizeof(float), cudaMemcpyHostToDevice));
+    CUDA_TRY_C(cudaMalloc(&c->dexps, (size_t)K * L));
+    CUDA_TRY_C(cudaMemcpy(c->dexps, d->term_exps, (size_t)K * L, cudaMemcpyHostToDevice));
+    CUDA_TRY_C(cudaMalloc(&c->dconv, conv.size() * sizeof(double)));
+    CUDA_TRY_C(cudaMemcpy(c->dconv, conv.data(), conv.size() * sizeof(double), cudaMemcpyHostToDevice));
+    CUDA_TRY_C(cudaMalloc(&c->dnedge, nseg * sizeof(int)));
+    CUDA_TRY_C(cudaMemcpy(c->dnedge, d->seg_n_edge, nseg * sizeof(int), cudaMemcpyHostToDevice));
+    M.C = c->dC; M.inv_s = c->dinv_s; M.exps = c->dexps; M.conv = c->dconv;
+    const int smem_bytes = (int)(c->smem_per_warp * c->wpb);
+    CUDA_TRY_C(cudaFuncSetAttribute(lasp_fit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
+    CUDA_TRY_C(cudaFuncSetAttribute(lasp_grad_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
+    CUDA_TRY_C(cudaFuncSetAttribute(lasp_model_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
+    *out = c;
+    return LASP_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// workspace and launches
+// ------------------------------------------------------------------------------------------
+static int launch_shape(const lasp_ctx *c, int tiles, int &grid, int &wpb)
+{
+    wpb = std::max(1, std::min(c->wpb, (tiles + c->num_sms - 1) / c->num_sms));
+    grid = std::min(c->num_sms, (tiles + wpb - 1) / wpb);
+    return 0;
+}
+
+static int ensure_workspace(lasp_ctx *c, int64_t B, bool need_yw)
+{
+    const size_t tiles = (size_t)((B + 31) / 32);
+    CUDA_TRY(c, cudaSetDevice(c->device));
+    if (need_yw && tiles > c->yw_tiles) {
+        if (c->dYW) cudaFree(c->dYW);
+        c->dYW = nullptr; c->yw_tiles = 0;
+        CUDA_TRY(c, cudaMalloc(&c->dYW, tiles * (size_t)c->M.Ppad * 32 * sizeof(float2)));
+        c->yw_tiles = tiles;
+    }
+    const size_t slots = (size_t)c->num_sms * c->wpb;
+    if (slots > c->scratch_slots) {
+        if (c->dscratch) cudaFree(c->dscratch);
+        c->dscratch = nullptr; c->scratch_slots = 0;
+        CUDA_TRY(c, cudaMalloc(&c->dscratch, slots * (size_t)c->M.nscr * c->M.Ppad * 32 * sizeof(float)));
+        c->scratch_slots = slots;
+    }
+    return LASP_OK;
+}
+
+extern "C" int lasp_reserve(lasp_ctx *c, int64_t B)
+{
+    if (!c || B < 1) return fail(c, LASP_ERR_INVALID_ARG, "lasp_reserve: bad argument");
+    return ensure_workspace(c, B, true);
+}
+
+static int stage(lasp_ctx *c, int64_t B, const float *flux, const float *ivar, const uint8_t *mask,
+                 cudaStream_t st)
+{
+    const int tiles = (int)((B + 31) / 32);
+    CUDA_TRY(c, cudaMemsetAsync(c->dYW, 0, (size_t)tiles * c->M.Ppad * 32 * sizeof(float2), st));
+    dim3 grid((c->M.P + 31) / 32, tiles), block(32, 8);
+    lasp_stage_kernel<<<grid, block, 0, st>>>(c->M, flux, ivar, mask, B, c->dYW);
+    lasp_edge_kernel<<<tiles, 32, 0, st>>>(c->M, c->dnedge, c->dYW);
+    c->launches += 2;
+    CUDA_TRY(c, cudaGetLastError());
+    return LASP_OK;
+}
+
+extern "C" int lasp_fit_batch(lasp_ctx *c, int64_t B, const float *flux, const float *ivar,
+                              const uint8_t *mask, const float *init, const lasp_fit_opts *opts,
+                              float *params, float *cont, float *chi2, float *err, int32_t *status,
+                              void *stream)
+{
+    if (!c) return fail(nullptr, LASP_ERR_INVALID_ARG, "null ctx");
+    if (B < 1 || !flux || !ivar || !init || !opts || !params || !chi2)
+        return fail(c, LASP_ERR_INVALID_ARG, "lasp_fit_batch: null pointer or B < 1");
+    if (opts->n_iter < 0 || !(opts->lr > 0.f) || !(opts->beta1 >= 0.f && opts->beta1 < 1.f) ||
+        !(opts->beta2 >= 0.f && opts->beta2 < 1.f) || !(opts->eps >= 0.f))
+        return fail(c, LASP_ERR_INVALID_ARG, "lasp_fit_batch: bad Adam hyper-parameters");
+    if (B > (int64_t)1 << 36) return fail(c, LASP_ERR_UNSUPPORTED, "B too large");
+    int rc = ensure_workspace(c, B, true);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    rc = stage(c, B, flux, ivar, mask, st);
+    if (rc) return rc;
+    FitArgs a;
+    memset(&a, 0, sizeof(a));
+    a.YW = c->dYW; a.scratch = c->dscratch; a.B = B; a.tiles = (int)((B + 31) / 32);
+    a.init = init; a.n_iter = opts->n_iter; a.lr = opts->lr; a.b1 = opts->beta1; a.b2 = opts->beta2;
+    a.eps = opts->eps; a.fd_h = 2e-3f;  // fp32 central-difference step in u (C.2-22)
+    a.params = params; a.cont = cont; a.chi2 = chi2; a.err = err; a.status = status;
+    int grid, wpb;
+    launch_shape(c, a.tiles, grid, wpb);
+    lasp_fit_kernel<<<grid, wpb * 32, c->smem_per_warp * wpb, st>>>(c->M, a);
+    c->launches += 1;
+    CUDA_TRY(c, cudaGetLastError());
+    return LASP_OK;
+}
+
+extern "C" int lasp_eval_grad(lasp_ctx *c, int64_t B, const float *flux, const float *ivar,
+                              const uint8_t *mask, const float *params, float *chi2, float *grad_u,
+                              float *cont, int32_t *status, void *stream)
+{
+    if (!c) return fail(nullptr, LASP_ERR_INVALID_ARG, "null ctx");
+    if (B < 1 || !flux || !ivar || !params || !chi2 || !grad_u)
+        return fail(c, LASP_ERR_INVALID_ARG, "lasp_eval_grad: null pointer or B < 1");
+    int rc = ensure_workspace(c, B, true);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    rc = stage(c, B, flux, ivar, mask, st);
+    if (rc) return rc;
+    FitArgs a;
+    memset(&a, 0, sizeof(a));
+    a.YW = c->dYW; a.scratch = c->dscratch; a.B = B; a.tiles = (int)((B + 31) / 32);
+    a.gparams = params; a.chi2 = chi2; a.grad_u = grad_u; a.cont = cont; a.status = status;
+    int grid, wpb;
+    launch_shape(c, a.tiles, grid, wpb);
+    lasp_grad_kernel<<<grid, wpb * 32, c->smem_per_warp * wpb, st>>>(c->M, a);
+    c->launches += 1;
+    CUDA_TRY(c, cudaGetLastError());
+    return LASP_OK;
+}
+
+extern "C" int lasp_eval_model(lasp_ctx *c, int64_t B, const float *params, const float *cont,
+                               float *model, void *stream)
+{
+    if (!c) return fail(nullptr, LASP_ERR_INVALID_ARG, "null ctx");
+    if (B < 1 || !params || !cont || !model)
+        return fail(c, LASP_ERR_INVALID_ARG, "lasp_eval_model: null pointer or B < 1");
+    int rc = ensure_workspace(c, B, false);
+    if (rc) return rc;
+    FitArgs a;
+    memset(&a, 0, sizeof(a));
+    a.scratch = c->dscratch; a.B = B; a.tiles = (int)((B + 31) / 32);
+    a.gparams = params; a.mcont = cont; a.model = model;
+    int grid, wpb;
+    launch_shape(c, a.tiles, grid, wpb);
+    lasp_model_kernel<<<grid, wpb * 32, c->smem_per_warp * wpb, (cudaStream_t)stream>>>(c->M, a);
+    c->launches += 1;
+    CUDA_TRY(c, cudaGetLastError());
+    return LASP_OK;
+}
+
+// Algorithmic FMA of one Adam step of one spectrum: SURVEY.md 8(d) formula, moment route,
+// given the mean number of stencil taps (2H+1 averaged over spectra and pixels).
+extern "C" double lasp_fma_per_spectrum_step(const lasp_ctx *c, double mean_taps)
+{
+    if (!c) return 0.0;
+    const ModelDev &M = c->M;
+    const double P = M.P, K = M.K, n1 = M.n1, W = mean_taps;
+    bool linear = false;
+    for (int s = 0; s < M.n_seg; ++s) linear = linear || !M.seg[s].uniform;
+    double G = (2.0 * M.D + 1.0) * P + M.n_seg * n1 * n1 * n1 / 6.0;
+    return 2.0 * K * P + 4.0 * W * P + (linear ? 2.0 * W * P : 0.0) + G + 4.0 * n1 * P +
+           M.n_seg * (n1 * n1 * n1 / 6.0 + 4.0 * n1 * n1) + 8.0 * P;
+}

@@ -1,0 +1,66 @@
+"""CPU-side checks of the C-ABI library: it builds for sm_100a, loads, and exports every symbol
+that include/lasp_gpu.h declares.  No compute calls (no GPU here)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def libpath():
+    from paper_2512_24840_b200 import build
+    return build.build()
+
+
+def declared_symbols():
+    txt = open(os.path.join(ROOT, "include", "lasp_gpu.h")).read()
+    txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
+    return sorted(set(re.findall(r"\b(lasp_[a-z_]+)\s*\(", txt)))
+
+
+def test_header_symbols_are_exported(libpath):
+    L = ctypes.CDLL(libpath)
+    syms = declared_symbols()
+    assert "lasp_fit_batch" in syms and "lasp_eval_grad" in syms and len(syms) >= 9
+    for s in syms:
+        assert hasattr(L, s), s
+    from paper_2512_24840_b200 import binding
+    assert sorted(binding.SYMBOLS) == syms
+
+
+def test_version_and_error_string(libpath):
+    L = ctypes.CDLL(libpath)
+    L.lasp_version.restype = ctypes.c_int
+    assert L.lasp_version() >= 100
+    L.lasp_last_error.restype = ctypes.c_char_p
+    L.lasp_last_error.argtypes = [ctypes.c_void_p]
+    assert isinstance(L.lasp_last_error(None), bytes)
+
+
+def test_create_rejects_bad_arguments_without_gpu(libpath):
+    from paper_2512_24840_b200 import binding
+    L = binding.lib()
+    out = ctypes.c_void_p()
+    assert L.lasp_create(None, 0, ctypes.byref(out)) == -1  # LASP_ERR_INVALID_ARG
+    d = binding.ModelDesc()
+    assert L.lasp_create(ctypes.byref(d), 0, ctypes.byref(out)) == -1
+    assert b"null" in L.lasp_last_error(None)
+
+
+def test_binding_fails_loudly_without_cuda():
+    import torch
+    from paper_2512_24840_b200 import binding, synth
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    d = synth.make_model_desc(synth.CONFIGS[0]); d.pop("_rng")
+    with pytest.raises(binding.LaspError):
+        binding.LaspModel(d)
+
+
+def test_sass_is_sm100(libpath):
+    import subprocess
+    out = subprocess.run(["cuobjdump", "-lelf", libpath], capture_output=True, text=True).stdout
+    assert "sm_100a" in out
