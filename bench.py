@@ -1,0 +1,366 @@
+"""bench.py -- spectra fitted per second at a fixed number of Adam steps (BASELINE.json metric).
+
+A "step" is one pass of the whole hot path (SURVEY.md 8(a) rows a0-a9 = one `lasp_fit_batch`
+call: staging, n_iter Adam steps, final evaluation, error estimate) over one synthetic batch of
+the chosen config (default: config 1, LAMOST-like, B=65,536, 500 Adam steps -- the configuration
+the metric is quoted on).  Inputs are seeded and synthetic; the bulk
+spectra are produced by the parity-checked CUDA forward kernel (`lasp_eval_model`), noise and masks
+by a seeded torch generator on the device.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1] [--batch B] [--impl reference]
+
+Prints ONE JSON line (rank 0).  `--impl reference` times the fp64 CPU oracle instead (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "spectra fitted/sec (fixed Adam steps)"
+UNIT = "spectra/s"
+FP32_LANES_PER_SM = 128
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return dict(hbm_gbs=d.get("hbm_gbs"), sm_max_mhz=d.get("sm_max_mhz", 1965.0), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons with NVML during the timed region (B200_PROFILING.md)."""
+
+    def __init__(self, index: int, period: float = 0.1):
+        self.index, self.period = index, period
+        self.samples, self.reasons = [], set()
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._thr = None
+
+    def start(self):
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception as e:  # NVML missing: report that, never fake a clock
+            self.nv = None
+            self.reasons.add(f"nvml_unavailable:{type(e).__name__}")
+            return self
+        self._thr = threading.Thread(target=self._run, daemon=True)
+        self._thr.start()
+        return self
+
+    def _run(self):
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, nm in names.items():
+                    if r & bit:
+                        self.reasons.add(nm)
+            except Exception:
+                pass
+            self._stop.wait(self.period)
+
+    def stop(self):
+        self._stop.set()
+        if self._thr:
+            self._thr.join()
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def make_device_batch(model, cfg, desc, B, seed, torch):
+    """Seeded synthetic batch of B spectra on the device (recipe: synth.py docstring).  Truth,
+    continuum, SNR and initial guesses are drawn by numpy; the model spectra come from the CUDA
+    forward kernel; mask and noise from a seeded torch generator on the device."""
+    from paper_2512_24840_b200 import synth
+    rng = np.random.Generator(np.random.PCG64(seed))
+    pr = synth.draw_params(cfg, desc, B, rng)
+    dev = model.device
+    truth = torch.from_numpy(pr["truth"]).to(dev)
+    cont = torch.from_numpy(pr["cont"]).to(dev)
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(seed)
+    P = model.P
+    flux = torch.empty((B, P), device=dev, dtype=torch.float32)
+    ivar = torch.empty((B, P), device=dev, dtype=torch.float32)
+    mask = torch.empty((B, P), device=dev, dtype=torch.uint8)
+    snr = torch.from_numpy(pr["snr"]).to(dev, torch.float32)
+    chunk = 8192
+    for a in range(0, B, chunk):
+        b = min(B, a + chunk)
+        mod = model.eval_model(truth[a:b], cont[a:b])
+        med = mod.median(dim=1).values
+        if cfg.noise == "poisson":
+            rho2 = 0.2 * med ** 2 / snr[a:b] ** 2
+            alpha = med / (1.25 * snr[a:b] ** 2)
+            var = alpha[:, None] * mod.clamp_min(0.0) + rho2[:, None]
+        else:
+            var = ((med / snr[a:b]) ** 2)[:, None].expand_as(mod)
+        z = torch.randn(mod.shape, device=dev, generator=gen)
+        mk = (torch.rand(mod.shape, device=dev, generator=gen) >= cfg.mask_frac)
+        f = mod + var.sqrt() * z
+        flux[a:b] = torch.where(mk, f, torch.full_like(f, 1e3))
+        ivar[a:b] = 1.0 / var
+        mask[a:b] = mk.to(torch.uint8)
+    init = torch.from_numpy(pr["init"]).to(dev)
+    return dict(flux=flux, ivar=ivar, mask=mask, init=init, truth=truth)
+
+
+def mean_taps(desc, params):
+    """Mean stencil length 2H+1, H = ceil(|v|/s + 5 sigma_tot/s), over spectra and pixels."""
+    from paper_2512_24840_b200 import synth
+    L = desc["n_labels"]
+    ll = desc["loglam"]
+    tot, n = 0.0, 0
+    v = np.abs(params[:, L].astype(np.float64))
+    sg = params[:, L + 1].astype(np.float64)
+    for k in range(desc["n_seg"]):
+        a, b = desc["seg_offset"][k], desc["seg_offset"][k + 1]
+        s = synth.C_KMS * math.log(10.0) * np.gradient(ll[a:b])
+        st = np.hypot(sg, float(desc["seg_sigma_inst"][k]))
+        # sample the pixel scale at 16 points per segment (it varies slowly)
+        for sj in s[:: max(1, (b - a) // 16)][:16]:
+            H = np.ceil(v / sj + 5.0 * st / sj)
+            tot += float((2 * H + 1).mean()) * (b - a) / 16.0
+        n += (b - a)
+    return tot / n
+
+
+def oracle_sample(cfg_id, n_spec, n_iter, seed_offset=0):
+    """Time the fp64 oracle, as it stands, on `n_spec` spectra of the config (full n_iter steps)."""
+    from oracle import lasp_oracle
+    from paper_2512_24840_b200 import synth
+    lasp_oracle.build()
+    case = synth.make_case(cfg_id, lasp_oracle.forward, B=n_spec)
+    o = lasp_oracle.Oracle(case["desc"])
+    t0 = time.perf_counter()
+    o.fit(case["flux"], case["ivar"], case["mask"], case["init"], n_iter, lr=case["config"].lr)
+    dt = time.perf_counter() - t0
+    return n_spec / dt, dt
+
+
+def sample_size(cfg, cores, per_core):
+    """Oracle sample: `per_core` config-1-sized fits per core (about 2 s each), scaled by the work."""
+    from paper_2512_24840_b200 import synth
+    P = synth.loglam_grid(cfg.grid, cfg.lam_min, cfg.lam_max, cfg.step).size
+    rel = (P * cfg.n_iter * (cfg.K / 26.0) ** 0.5) / (1550.0 * 500.0)
+    return max(cores, int(per_core * cores / max(rel, 0.05)) // cores * cores)
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, a bounded sample of the workload per step."""
+    from paper_2512_24840_b200 import synth
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg = synth.CONFIGS[args.config]
+    cores = os.cpu_count() or 1
+    n_spec = args.ref_spectra or sample_size(cfg, cores, 4)
+    for _ in range(args.warmup):
+        oracle_sample(args.config, max(1, n_spec // 4), max(1, cfg.n_iter // 10))
+    vals, tot = [], 0.0
+    for _ in range(args.steps):
+        v, dt = oracle_sample(args.config, n_spec, cfg.n_iter)
+        vals.append(v)
+        tot += dt
+    value = n_spec * args.steps / tot
+    sample = f"{n_spec} spectra of config {args.config} per step, all {cfg.n_iter} Adam steps + error estimate"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "gpu_launches": 0,
+        "config": {"workload": f"config {args.config} ({cfg.name}) sample", "n_iter": cfg.n_iter,
+                   "n_pix": None, "sample_spectra": n_spec},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line), flush=True)
+
+
+def run_gpu(args):
+    import torch
+    from paper_2512_24840_b200 import binding, build, synth
+
+    build.build()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise binding.LaspError("bench.py needs a CUDA device: there is no CPU fallback for the LASP path")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    cfg = synth.CONFIGS[args.config]
+    desc = synth.make_model_desc(cfg)
+    desc.pop("_rng")
+    B = args.batch or cfg.B            # per GPU: spectra are independent units, weak scaling
+    n_iter = args.n_iter or cfg.n_iter
+    model = binding.LaspModel(desc, device=local)
+    model.reserve(B)
+    data = make_device_batch(model, cfg, desc, B, cfg.seed + 17 + rank, torch)
+    out = None
+    kw = dict(lr=cfg.lr, beta1=cfg.beta1, beta2=cfg.beta2, eps=cfg.eps)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step():
+        nonlocal out
+        out = model.fit_batch(data["flux"], data["ivar"], data["mask"], data["init"], n_iter, out=out, **kw)
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local).start() if rank == 0 else None
+    l0 = model.launch_count()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    ev[0].record()
+    for k in range(args.steps):
+        step()
+        ev[k + 1].record()
+    barrier()
+    launches = model.launch_count() - l0
+    ms_total = ev[0].elapsed_time(ev[-1])
+    step_ms = [ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)]
+    clocks = sampler.stop() if sampler else None
+    t = torch.tensor([ms_total], device="cuda", dtype=torch.float64)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total = float(t.item())
+    value = world * B * args.steps / (ms_total * 1e-3)
+
+    # ---- end to end through the public API with HOST buffers (pinned), copies inside the timed region
+    host = {k: data[k].cpu().pin_memory() for k in ("flux", "ivar", "mask", "init")}
+    hout = dict(params=torch.empty((B, model.NP), dtype=torch.float32).pin_memory(),
+                chi2=torch.empty(B, dtype=torch.float32).pin_memory(),
+                err=torch.empty((B, model.NP), dtype=torch.float32).pin_memory(),
+                cont=torch.empty((B, model.nc), dtype=torch.float32).pin_memory(),
+                status=torch.empty(B, dtype=torch.int32).pin_memory())
+    h2d = sum(v.numel() * v.element_size() for v in host.values())
+    d2h = sum(v.numel() * v.element_size() for v in hout.values())
+    dbuf = {k: torch.empty_like(data[k]) for k in host}
+
+    def e2e_step():
+        for k in host:
+            dbuf[k].copy_(host[k], non_blocking=True)
+        r = model.fit_batch(dbuf["flux"], dbuf["ivar"], dbuf["mask"], dbuf["init"], n_iter, out=out, **kw)
+        for k in hout:
+            hout[k].copy_(r[k], non_blocking=True)
+
+    e2e_steps = max(1, min(args.steps, 3))
+    e2e_step()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(e2e_steps):
+        e2e_step()
+    e1.record()
+    barrier()
+    t = torch.tensor([e0.elapsed_time(e1)], device="cuda", dtype=torch.float64)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_value = world * B * e2e_steps / (float(t.item()) * 1e-3)
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+    # ---- roofline of the dominant kernel (lasp_fit_kernel): plain-ALU FP32 bound
+    peaks = load_peaks()
+    prop = torch.cuda.get_device_properties(local)
+    params = out["params"].cpu().numpy()
+    taps = mean_taps(desc, params)
+    fma_step = model.fma_per_spectrum_step(taps)
+    flop_launch = 2.0 * fma_step * B * n_iter
+    kern_ms = float(np.mean(step_ms))          # events bracket stage + fit; stage share is in profiles/
+    achieved = flop_launch / (kern_ms * 1e-3) / 1e12
+    peak = prop.multi_processor_count * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+            "traffic": None, "kernel": "lasp_fit_kernel", "fma_per_spectrum_step": fma_step,
+            "mean_taps": taps, "peak_source": f"SMs x 128 FP32 lanes x 2 x sm_max_mhz ({peaks['source']})",
+            "frac_at_sampled_clock": (achieved / (peak * clocks["sm_mhz"] / peaks["sm_max_mhz"])
+                                      if clocks and clocks.get("sm_mhz") else None)}
+    st = out["status"].cpu().numpy()
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"config {args.config} ({cfg.name})", "spectra_per_gpu": B,
+                   "n_pix": model.P, "n_terms": model.K, "n_labels": model.L, "cont_degree": model.D,
+                   "n_seg": model.n_seg, "adam_steps": n_iter, "lr": cfg.lr, "errors": True,
+                   "l2": "inputs larger than L2 (flux+ivar+mask %.0f MB per step)" % (h2d / 1e6),
+                   "status_nonzero_frac": float((st != 0).mean())},
+        "clocks": clocks, "gpu_launches": int(launches),
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+                "d2h_bytes_per_step": int(d2h), "steps": e2e_steps},
+        "roofline": roof,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        cores = os.cpu_count() or 1
+        n_spec = args.ref_spectra or sample_size(cfg, cores, 8)
+        v, dt = oracle_sample(args.config, n_spec, n_iter)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": f"{n_spec} spectra of config {args.config}, all {n_iter} Adam steps "
+                                          f"+ error estimate, {dt:.1f} s"}
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="1")
+    ap.add_argument("--batch", type=int, default=0, help="spectra per GPU (default: the config's B)")
+    ap.add_argument("--n-iter", type=int, default=0, help="Adam steps (default: the config's)")
+    ap.add_argument("--ref-spectra", type=int, default=0, help="oracle sample size")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.config = int(args.config) if args.config.isdigit() else args.config
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()
