@@ -1,0 +1,1037 @@
+// lasp_fit_v1.cuh -- the fused LASP-Adam fitting kernel for sm_100a.
+//
+// Mapping.  A CTA advances a GROUP of GS = 4 spectra in lockstep through every Adam step.  Threads
+// own pixels: thread t owns the octet (8 consecutive padded pixels) t of the range being swept, for
+// all 4 spectra, so that every spectrum-independent operand (an emulator coefficient C[k,j], a
+// continuum basis value) is fetched once and used for 4 spectra x 8 pixels from registers, and every
+// per-spectrum scalar (phi_k, b_n, a tap weight) is one broadcast LDS.128 for the 4 spectra.  The
+// emulator output T and the adjoint a live in shared-memory rows (neighbour access by the stencils);
+// flux/weight rows are re-read from global memory, where the few hundred groups in flight keep them
+// L2-resident.  Sums over pixels (continuum moments, chi2, gradient) are reduced with a register
+// transpose over warp shuffles (32 values x 32 lanes in 31 shuffles) and one shared-memory slot per
+// warp; the continuum system is solved by one warp per spectrum (lanes = rows).
+//
+// Citations: Eq. n and P:n are /root/reference/PAPER.md; C.2-n the readings of SURVEY.md 8(c)
+// (restated in DESIGN.md); a0..a9 the steps of SURVEY.md 8(a).
+#pragma once
+#include "lasp_device.cuh"
+
+#define GS 4    // spectra per CTA group
+#define OCT 8   // pixels per thread tile
+
+struct V1Lay {
+    int RL, GUARD;          // shared-memory row length and guard (floats); row index = jp - po + GUARD
+    int NA;                 // largest number of 4-tap groups of a kernel
+    int n1r, nmomr, VR;     // n1 rounded to 4; moments rounded; reduction slots per warp (x GS)
+    int NW;                 // warps per CTA
+    int Hm;                 // support clamp (memory safety outside the prior box)
+    int refresh;            // re-accumulate the Gram moments and re-factor every `refresh` steps
+    // shared-memory offsets (floats)
+    int oT, oA, oU, oM, oV, oX, oPHI, oGW, oGR, oTAP, oMOM, oRHS, oB, oRED, oLF, oQ, oSC, total;
+};
+
+struct V1Args {
+    const float *Y, *W;   // staged flux and weight planes [B][Ppad] (halos and tails zero)
+    float *CP;            // [cta][GS][Ppad] previous continuum c_prev (a5, refinement form)
+    float *XJ;            // [cta][(1+NP)][GS][Ppad] rho and Jacobian columns (a9), may be null
+    long long B;
+    int ngroups;
+    const float *init;
+    int n_iter;
+    float lr, b1, b2, eps, fd_h;
+    float *params, *cont, *chi2, *err;
+    int *status;
+    const float *gparams;  // lasp_eval_grad
+    float *grad_u;
+};
+
+// slots of the per-warp reduction area (each slot holds GS floats)
+#define SLOT_MOM(L_, n) (n)
+#define SLOT_RHS(L_, n) ((L_).nmomr + (n))
+#define SLOT_Q(L_, k) ((L_).nmomr + (L_).n1r + (k))
+#define SLOT_STAT(L_) ((L_).VR - 4)   // chi2, ngood, min c
+
+// per-spectrum scalars in shared memory: SC[idx][GS]
+enum { SC_V = 0, SC_SIG, SC_CHI, SC_NGOOD, SC_CMIN, SC_GV, SC_GS, SC_FAIL, SC_N };
+
+// 32 values per lane -> lane l returns the warp total of value l (31 shuffles)
+__device__ __forceinline__ float xreduce32(float (&x)[32], int lane)
+{
+#pragma unroll
+    for (int s = 16; s >= 1; s >>= 1) {
+        const bool up = (lane & s) != 0;
+#pragma unroll
+        for (int i = 0; i < s; ++i) {
+            float send = up ? x[i] : x[i + s];
+            float keep = up ? x[i + s] : x[i];
+            x[i] = keep + __shfl_xor_sync(FULL, send, s);
+        }
+    }
+    return x[0];
+}
+
+__device__ __forceinline__ float warp_min_f(float v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fminf(v, __shfl_xor_sync(FULL, v, o));
+    return v;
+}
+
+struct V1Ctx {
+    const ModelDev *M;
+    const V1Lay *L;
+    float *sm;
+    int tid, lane, warp, nt;
+    long long spec[GS];   // clamped spectrum indices of the group
+    float *cp;            // this CTA's c_prev scratch
+};
+
+#define SMV(c, off, idx, g) (c).sm[(off) + (idx) * GS + (g)]
+
+// ------------------------------------------------------------------------------------------
+// a1: de-normalise, emulator inputs, monomials (Eq. 1, C.2-18/19).  Warp g, spectrum g.
+// ------------------------------------------------------------------------------------------
+__device__ void v1_param_setup(const V1Ctx &c, int g)
+{
+    const ModelDev &M = *c.M;
+    const V1Lay &L = *c.L;
+    for (int p = c.lane; p < M.NP; p += 32) {
+        float u = SMV(c, L.oU, p, g);
+        float th = M.lo[p] + (u + 1.f) * (M.hi[p] - M.lo[p]) * 0.5f;
+        if (p < M.L) SMV(c, L.oX, p, g) = label_x(M, p, th);
+        else SMV(c, L.oSC, p == M.L ? SC_V : SC_SIG, g) = th;
+    }
+    __syncwarp();
+    for (int k = c.lane; k < M.K; k += 32) {
+        float p = 1.f;
+        for (int l = 0; l < M.L; ++l) {
+            int e = M.exps[k * M.L + l];
+            float x = SMV(c, L.oX, l, g);
+            for (int q = 0; q < e; ++q) p *= x;
+        }
+        SMV(c, L.oPHI, k, g) = p;
+    }
+    __syncwarp();
+}
+
+// ------------------------------------------------------------------------------------------
+// a3: kernel weights of a uniform (log-grid) segment (Eq. 5; C.2-9/10/15), in groups of
+// four taps: group a holds taps k = 4a-3 .. 4a, a = a_lo .. a_lo+na-1, zero outside |k| <= H.
+//   GW [g][a][4]       forward kernel g_k
+//   GR [j][g][a][4]    reversed kernels for the adjoint pass: j=0: g_{-k}; j=1: d g_{-k}/dv;
+//                      j=2: d g_{-k}/d sigma* (chain factors of C.1 folded in)
+// ------------------------------------------------------------------------------------------
+__device__ void v1_setup_weights(const V1Ctx &c, const SegDev &sg, int g)
+{
+    const V1Lay &L = *c.L;
+    const float v = SMV(c, L.oSC, SC_V, g), sigstar = SMV(c, L.oSC, SC_SIG, g);
+    const float sigtot = sqrtf(sigstar * sigstar + sg.sig_inst * sg.sig_inst);
+    const float mu = v * sg.inv_s, s = sigtot * sg.inv_s;
+    int H = (int)ceilf(fabsf(mu) + 5.f * s);
+    H = min(max(H, 0), sg.halo - 18);   // memory safety outside the prior box (halo >= Hmax + 18)
+    const float i2 = 0.5f / (s * s);
+    float sum = 0.f, s1 = 0.f, s2 = 0.f;
+    for (int m = c.lane; m <= 2 * H; m += 32) {
+        float d = (float)(m - H) - mu;
+        float e = expf(-d * d * i2);
+        sum += e; s1 = fmaf(e, d, s1); s2 = fmaf(e * d, d, s2);
+    }
+    sum = warp_sum_f(sum); s1 = warp_sum_f(s1); s2 = warp_sum_f(s2);
+    const float inv = 1.f / sum;
+    const float e1n = s1 * inv, e2n = s2 * inv;       // kbar - mu ; second moment about mu
+    const float is2 = 2.f * i2;                        // 1/sigma^2 (pixels)
+    const float cmu = is2 * sg.inv_s;                  // dS/dv      = (1/s) sum dg/dmu T
+    const float csig = is2 * sqrtf(is2) * (sigstar / sigtot) * sg.inv_s;
+    const int a_lo = -(H / 4), na = (H + 3) / 4 - a_lo + 1;
+    float *gw = c.sm + L.oGW + g * L.NA * 4;
+    float *gr = c.sm + L.oGR + g * L.NA * 4;
+    const int rs = GS * L.NA * 4;
+    for (int idx = c.lane; idx < na * 4; idx += 32) {
+        const int k = 4 * (a_lo + (idx >> 2)) - 3 + (idx & 3);
+        const bool in = (k >= -H) && (k <= H);
+        float d = (float)k - mu;
+        gw[idx] = in ? expf(-d * d * i2) * inv : 0.f;
+        d = (float)(-k) - mu;
+        float gg = in ? expf(-d * d * i2) * inv : 0.f;
+        gr[idx] = gg;
+        gr[rs + idx] = gg * (d - e1n) * cmu;
+        gr[2 * rs + idx] = gg * (d * d - e2n) * csig;
+    }
+    if (c.lane == 0) {
+        int *tap = (int *)(c.sm + L.oTAP);
+        tap[g * 2] = a_lo; tap[g * 2 + 1] = na;
+    }
+    __syncwarp();
+}
+
+// ------------------------------------------------------------------------------------------
+// a4: sliding-window stencil for one octet and NK kernels sharing the window (Eq. 5).
+//   out[n][i] = sum_k w_n[k] row[j0 + i - k],  taps in groups a: k = 4a-3..4a.
+// row4 is the float4 view of a shared-memory row indexed by (padded pixel)/4; for group a the window
+// is row[j0-4a .. j0-4a+11]: one new LDS.128 per group feeds 32*NK FMAs.
+// ------------------------------------------------------------------------------------------
+template <int NK>
+__device__ __forceinline__ void v1_stencil_octet(const float4 *__restrict__ row4, int j0, int a_lo, int na,
+                                                 const float4 *__restrict__ w0, int wstride4,
+                                                 float (&acc)[NK][OCT])
+{
+#pragma unroll
+    for (int n = 0; n < NK; ++n)
+#pragma unroll
+        for (int i = 0; i < OCT; ++i) acc[n][i] = 0.f;
+    const int q = (j0 >> 2) - a_lo;
+    float4 qb = row4[q + 1], qc = row4[q + 2];
+#pragma unroll 3
+    for (int ai = 0; ai < na; ++ai) {
+        const float4 qa = row4[q - ai];
+        const float Wd[12] = {qa.x, qa.y, qa.z, qa.w, qb.x, qb.y, qb.z, qb.w, qc.x, qc.y, qc.z, qc.w};
+#pragma unroll
+        for (int n = 0; n < NK; ++n) {
+            const float4 w = w0[n * wstride4 + ai];
+#pragma unroll
+            for (int i = 0; i < OCT; ++i) {
+                float s = acc[n][i];
+                s = fmaf(w.x, Wd[i + 3], s);
+                s = fmaf(w.y, Wd[i + 2], s);
+                s = fmaf(w.z, Wd[i + 1], s);
+                s = fmaf(w.w, Wd[i], s);
+                acc[n][i] = s;
+            }
+        }
+        qc = qb; qb = qa;
+    }
+}
+
+// shared-memory row of spectrum g in buffer `off`, as a float pointer indexed by padded pixel jp
+__device__ __forceinline__ float *v1_row(const V1Ctx &c, int off, const SegDev &sg, int g)
+{
+    return c.sm + off + g * c.L->RL + c.L->GUARD - sg.po;
+}
+
+// largest support of the group (for the T range), from the tap tables
+__device__ __forceinline__ int v1_group_reach(const V1Ctx &c)
+{
+    const int *tap = (const int *)(c.sm + c.L->oTAP);
+    int r = 0;
+#pragma unroll
+    for (int g = 0; g < GS; ++g) {
+        int a_lo = tap[2 * g], na = tap[2 * g + 1];
+        r = max(r, max(-4 * a_lo + 3, 4 * (a_lo + na - 1)));   // |k| reach of the padded tap groups
+    }
+    return (r + OCT + OCT - 1) / OCT * OCT;   // window reads up to 8 pixels past the last tap
+}
+
+// ------------------------------------------------------------------------------------------
+// a2: T_j = sum_k phi_k C[k,j] over the padded range [lo,hi) -> shared row T (Eq. 1)
+// ------------------------------------------------------------------------------------------
+__device__ void v1_phase_emulator(const V1Ctx &c, const SegDev &sg, int lo, int hi)
+{
+    const ModelDev &M = *c.M;
+    const V1Lay &L = *c.L;
+    const float4 *phi4 = (const float4 *)(c.sm + L.oPHI);
+    const int P4 = M.Ppad >> 2;
+    for (int j0 = lo + c.tid * OCT; j0 < hi; j0 += c.nt * OCT) {
+        float acc[GS][OCT];
+#pragma unroll
+        for (int g = 0; g < GS; ++g)
+#pragma unroll
+            for (int i = 0; i < OCT; ++i) acc[g][i] = 0.f;
+        const float4 *c4 = (const float4 *)(M.C + j0);
+#pragma unroll 4
+        for (int k = 0; k < M.K; ++k) {
+            const float4 ca = __ldg(c4 + (size_t)k * P4), cb = __ldg(c4 + (size_t)k * P4 + 1);
+            const float4 ph = phi4[k];
+            const float cc[OCT] = {ca.x, ca.y, ca.z, ca.w, cb.x, cb.y, cb.z, cb.w};
+            const float pg[GS] = {ph.x, ph.y, ph.z, ph.w};
+#pragma unroll
+            for (int g = 0; g < GS; ++g)
+#pragma unroll
+                for (int i = 0; i < OCT; ++i) acc[g][i] = fmaf(pg[g], cc[i], acc[g][i]);
+        }
+#pragma unroll
+        for (int g = 0; g < GS; ++g) {
+            float4 *r = (float4 *)(v1_row(c, L.oT, sg, g) + j0);
+            r[0] = make_float4(acc[g][0], acc[g][1], acc[g][2], acc[g][3]);
+            r[1] = make_float4(acc[g][4], acc[g][5], acc[g][6], acc[g][7]);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// a4 + a5 (accumulation part).  For the thread's octet of the fitted range:
+//   S = G (*) T (or re-read from row A when `stencil` is false), stored to row A;
+//   u = w S^2, v = w S (y - c_prev S);
+//   Chebyshev moments  mom_n = sum_j u_j T_n(t_j), n < 2D+1 (only when `mom`), and the residual-form
+//   right-hand side    rhs_n = sum_j v_j T_n(t_j), n <= D      (SURVEY.md section 7 "moment route";
+//   T_m T_n = (T_{m+n} + T_{|m-n|})/2 turns the moments into the Gram matrix of Eq. 6's WLS).
+// Partial sums over the thread's 8 pixels are reduced over the warp by register transposes and
+// land in this warp's reduction slots.
+// ------------------------------------------------------------------------------------------
+__device__ void v1_phase_forward(const V1Ctx &c, const SegDev &sg, const V1Args &a, bool stencil, bool mom)
+{
+    const ModelDev &M = *c.M;
+    const V1Lay &L = *c.L;
+    const int *tap = (const int *)(c.sm + L.oTAP);
+    float *red = c.sm + L.oRED + c.warp * L.VR * GS;
+    bool first = true;
+    for (int jb = sg.fit_lo; jb < sg.fit_hi; jb += c.nt * OCT, first = false) {   // uniform trip count
+        const int j0 = jb + c.tid * OCT;
+        const bool act = j0 < sg.fit_hi;
+        float u[GS][OCT], v[GS][OCT];
+        if (act) {
+#pragma unroll
+            for (int g = 0; g < GS; ++g) {
+                float S[1][OCT];
+                float4 *ra = (float4 *)(v1_row(c, L.oA, sg, g) + j0);
+                if (stencil) {
+                    v1_stencil_octet<1>((const float4 *)v1_row(c, L.oT, sg, g), j0, tap[2 * g], tap[2 * g + 1],
+                                        (const float4 *)(c.sm + L.oGW + g * L.NA * 4), 0, S);
+                    ra[0] = make_float4(S[0][0], S[0][1], S[0][2], S[0][3]);
+                    ra[1] = make_float4(S[0][4], S[0][5], S[0][6], S[0][7]);
+                } else {
+                    const float4 s0 = ra[0], s1 = ra[1];
+                    S[0][0] = s0.x; S[0][1] = s0.y; S[0][2] = s0.z; S[0][3] = s0.w;
+                    S[0][4] = s1.x; S[0][5] = s1.y; S[0][6] = s1.z; S[0][7] = s1.w;
+                }
+                const size_t ro = (size_t)c.spec[g] * M.Ppad + j0;
+                const float4 y0 = __ldg((const float4 *)(a.Y + ro)), y1 = __ldg((const float4 *)(a.Y + ro) + 1);
+                const float4 w0 = __ldg((const float4 *)(a.W + ro)), w1 = __ldg((const float4 *)(a.W + ro) + 1);
+                const float4 *cp4 = (const float4 *)(c.cp + (size_t)g * M.Ppad + j0);
+                const float4 c0 = cp4[0], c1 = cp4[1];
+                const float yy[OCT] = {y0.x, y0.y, y0.z, y0.w, y1.x, y1.y, y1.z, y1.w};
+                const float ww[OCT] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
+                const float cc[OCT] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w};
+#pragma unroll
+                for (int i = 0; i < OCT; ++i) {
+                    const float ws = ww[i] * S[0][i];
+                    u[g][i] = ws * S[0][i];
+                    v[g][i] = ws * fmaf(-cc[i], S[0][i], yy[i]);
+                }
+            }
+        } else {
+#pragma unroll
+            for (int g = 0; g < GS; ++g)
+#pragma unroll
+                for (int i = 0; i < OCT; ++i) { u[g][i] = 0.f; v[g][i] = 0.f; }
+        }
+        // Chebyshev recurrence state: (pp, pc) = (T_{n-1}, T_n), started at (T_{-1}, T_0) = (t, 1)
+        float pp[OCT], pc[OCT], x2[OCT];
+#pragma unroll
+        for (int i = 0; i < OCT; ++i) {
+            const float t = fmaf(sg.ta, (float)(j0 + i - sg.po - sg.halo), sg.tb);
+            pp[i] = t; pc[i] = 1.f; x2[i] = 2.f * t;
+        }
+        if (mom) {
+            // region A: n < n1r, four n per transpose: value (nn, isrhs, g) at nn*8 + isrhs*4 + g
+            for (int n0 = 0; n0 < L.n1r; n0 += 4) {
+                float X[32];
+#pragma unroll
+                for (int nn = 0; nn < 4; ++nn) {
+#pragma unroll
+                    for (int g = 0; g < GS; ++g) {
+                        float sm_ = 0.f, sr = 0.f;
+#pragma unroll
+                        for (int i = 0; i < OCT; ++i) { sm_ = fmaf(u[g][i], pc[i], sm_); sr = fmaf(v[g][i], pc[i], sr); }
+                        X[nn * 8 + g] = sm_; X[nn * 8 + 4 + g] = sr;
+                    }
+#pragma unroll
+                    for (int i = 0; i < OCT; ++i) { const float nx = fmaf(x2[i], pc[i], -pp[i]); pp[i] = pc[i]; pc[i] = nx; }
+                }
+                const float tot = xreduce32(X, c.lane);
+                const int n = n0 + (c.lane >> 3), g = c.lane & 3;
+                const int slot = (c.lane & 4) ? SLOT_RHS(L, n) : SLOT_MOM(L, n);
+                if (first) red[slot * GS + g] = tot; else red[slot * GS + g] += tot;
+            }
+            // region B: n1r <= n < nmomr, moments only, eight n per transpose: value (nn, g) at nn*4 + g
+            for (int n0 = L.n1r; n0 < L.nmomr; n0 += 8) {
+                float X[32];
+#pragma unroll
+                for (int nn = 0; nn < 8; ++nn) {
+#pragma unroll
+                    for (int g = 0; g < GS; ++g) {
+                        float sm_ = 0.f;
+#pragma unroll
+                        for (int i = 0; i < OCT; ++i) sm_ = fmaf(u[g][i], pc[i], sm_);
+                        X[nn * 4 + g] = sm_;
+                    }
+#pragma unroll
+                    for (int i = 0; i < OCT; ++i) { const float nx = fmaf(x2[i], pc[i], -pp[i]); pp[i] = pc[i]; pc[i] = nx; }
+                }
+                const float tot = xreduce32(X, c.lane);
+                const int slot = SLOT_MOM(L, n0 + (c.lane >> 2));
+                if (first) red[slot * GS + (c.lane & 3)] = tot; else red[slot * GS + (c.lane & 3)] += tot;
+            }
+        } else {
+            // right-hand side only, eight n per transpose
+            for (int n0 = 0; n0 < L.n1r; n0 += 8) {
+                float X[32];
+#pragma unroll
+                for (int nn = 0; nn < 8; ++nn) {
+#pragma unroll
+                    for (int g = 0; g < GS; ++g) {
+                        float sr = 0.f;
+#pragma unroll
+                        for (int i = 0; i < OCT; ++i) sr = fmaf(v[g][i], pc[i], sr);
+                        X[nn * 4 + g] = sr;
+                    }
+#pragma unroll
+                    for (int i = 0; i < OCT; ++i) { const float nx = fmaf(x2[i], pc[i], -pp[i]); pp[i] = pc[i]; pc[i] = nx; }
+                }
+                const float tot = xreduce32(X, c.lane);
+                const int slot = SLOT_RHS(L, n0 + (c.lane >> 2));
+                if (first) red[slot * GS + (c.lane & 3)] = tot; else red[slot * GS + (c.lane & 3)] += tot;
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// a5 (solve part), warp g for spectrum g, lanes = rows of the (D+1)x(D+1) system padded to 32 with
+// the identity.  A_ij = (mom_{i+j} + mom_{|i-j|})/2 ; b += A^-1 rhs (one step of iterative
+// refinement whose residual was formed from the pixel data).  With
+// `refactor` false the Cholesky factor kept in shared memory from an earlier step is reused
+// (the refinement's fixed point does not depend on it).
+// Factor layout: LF[row*33 + col], then 32 reciprocal diagonals.
+// ------------------------------------------------------------------------------------------
+#define V1_LFS (32 * 33 + 32)
+
+__device__ void v1_phase_solve(const V1Ctx &c, int g, int seg, bool refactor)
+{
+    const ModelDev &M = *c.M;
+    const V1Lay &L = *c.L;
+    const int n1 = M.n1, lane = c.lane, rowB = seg * M.n1;
+    float *momS = c.sm + L.oMOM + g * L.nmomr;
+    float *rhsS = c.sm + L.oRHS + g * L.n1r;
+    float *lf = c.sm + L.oLF + g * V1_LFS;
+    float *invd = lf + 32 * 33;
+    const float *red = c.sm + L.oRED;
+    const int wst = L.VR * GS;
+    for (int n = lane; n < L.n1r; n += 32) {
+        float s = 0.f;
+        for (int w = 0; w < L.NW; ++w) s += red[w * wst + SLOT_RHS(L, n) * GS + g];
+        rhsS[n] = s;
+    }
+    if (refactor) {
+        for (int n = lane; n < L.nmomr; n += 32) {
+            float s = 0.f;
+            for (int w = 0; w < L.NW; ++w) s += red[w * wst + SLOT_MOM(L, n) * GS + g];
+            momS[n] = s;
+        }
+        __syncwarp();
+        float row[32];
+#pragma unroll
+        for (int j = 0; j < 32; ++j) {
+            float v = (j == lane) ? 1.f : 0.f;
+            if (j < n1 && lane < n1) {
+                int d = lane - j;
+                d = d < 0 ? -d : d;
+                v = 0.5f * (momS[lane + j] + momS[d]);
+            }
+            row[j] = v;
+        }
+        const float m0 = momS[0];
+        bool ok = true;
+        float *colbuf = invd;   // 32 floats, overwritten with the reciprocals at the end
+#pragma unroll
+        for (int k = 0; k < 32; ++k) {
+            if (k < n1) {
+                const float d0 = 0.5f * (momS[2 * k] + m0);
+                const float d = __shfl_sync(FULL, row[k], k);
+                if (!(d > 1e-6f * d0)) ok = false;
+                const float lik = row[k] * rsqrtf(d);
+                row[k] = lik;
+                colbuf[lane] = lik;
+                __syncwarp();
+#pragma unroll
+                for (int j = k + 1; j < 32; ++j) row[j] = fmaf(-lik, colbuf[j], row[j]);
+                __syncwarp();
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < 32; ++j) lf[lane * 33 + j] = row[j];
+        __syncwarp();
+        invd[lane] = 1.f / lf[lane * 33 + lane];
+        if (lane == 0) SMV(c, L.oSC, SC_N + seg, g) = ok ? 0.f : 1.f;
+    }
+    __syncwarp();
+    const bool ok = SMV(c, L.oSC, SC_N + seg, g) == 0.f;
+    float r = (lane < n1) ? rhsS[lane] : 0.f;
+    for (int k = 0; k < n1; ++k) {            // L y = rhs
+        const float yk = __shfl_sync(FULL, r, k) * invd[k];
+        const float l = lf[lane * 33 + k];
+        if (lane == k) r = yk;
+        else if (lane > k) r = fmaf(-l, yk, r);
+    }
+    for (int k = n1 - 1; k >= 0; --k) {       // L^T x = y
+        const float xk = __shfl_sync(FULL, r, k) * invd[k];
+        const float l = lf[k * 33 + lane];
+        if (lane == k) r = xk;
+        else if (lane < k) r = fmaf(-l, xk, r);
+    }
+    if (lane < n1) {
+        if (ok) SMV(c, L.oB, rowB + lane, g) += r;
+        else SMV(c, L.oB, rowB + lane, g) = 0.f;
+    }
+    __syncwarp();
+}
+
+// ------------------------------------------------------------------------------------------
+// a5 (evaluation part) + a6.  c_j = sum_n b_n T_n(t_j) on the thread's octet -> c_prev scratch;
+//   MODE 0: nothing else (between the two solves of a cold start);
+//   MODE 1: r = y - c S, chi2, adjoint a = -2 w r c -> row A (replaces S), ngood, min c;
+//   MODE 2: as 1, and rho = sqrt(w) r -> global row `xrow` (a9).
+// chi2 / ngood / cmin are reduced over the warp and accumulated in this warp's SLOT_STAT slots (zeroed by v1_evaluate).
+// ------------------------------------------------------------------------------------------
+template <int MODE>
+__device__ void v1_phase_residual(const V1Ctx &c, const SegDev &sg, const V1Args &a, int rowB, float *xrow)
+{
+    const ModelDev &M = *c.M;
+    const V1Lay &L = *c.L;
+    const float4 *b4 = (const float4 *)(c.sm + L.oB) + rowB;
+    float chi[GS], ng[GS], cmin[GS];
+#pragma unroll
+    for (int g = 0; g < GS; ++g) { chi[g] = 0.f; ng[g] = 0.f; cmin[g] = 3.0e38f; }
+    for (int j0 = sg.fit_lo + c.tid * OCT; j0 < sg.fit_hi; j0 += c.nt * OCT) {
+        float cc[GS][OCT], pp[OCT], pc[OCT], x2[OCT];
+#pragma unroll
+        for (int i = 0; i < OCT; ++i) {
+            const float t = fmaf(sg.ta, (float)(j0 + i - sg.po - sg.halo), sg.tb);
+            pp[i] = t; pc[i] = 1.f; x2[i] = 2.f * t;
+        }
+#pragma unroll
+        for (int g = 0; g < GS; ++g)
+#pragma unroll
+            for (int i = 0; i < OCT; ++i) cc[g][i] = 0.f;
+        for (int n = 0; n < M.n1; ++n) {
+            const float4 b = b4[n];
+            const float bg[GS] = {b.x, b.y, b.z, b.w};
+#pragma unroll
+            for (int g = 0; g < GS; ++g)
+#pragma unroll
+                for (int i = 0; i < OCT; ++i) cc[g][i] = fmaf(bg[g], pc[i], cc[g][i]);
+#pragma unroll
+            for (int i = 0; i < OCT; ++i) { const float nx = fmaf(x2[i], pc[i], -pp[i]); pp[i] = pc[i]; pc[i] = nx; }
+        }
+#pragma unroll
+        for (int g = 0; g < GS; ++g) {
+            float4 *cp4 = (float4 *)(c.cp + (size_t)g * M.Ppad + j0);
+            cp4[0] = make_float4(cc[g][0], cc[g][1], cc[g][2], cc[g][3]);
+            cp4[1] = make_float4(cc[g][4], cc[g][5], cc[g][6], cc[g][7]);
+            if (MODE == 0) continue;
+            float4 *ra = (float4 *)(v1_row(c, L.oA, sg, g) + j0);
+            const float4 s0 = ra[0], s1 = ra[1];
+            const size_t ro = (size_t)c.spec[g] * M.Ppad + j0;
+            const float4 y0 = __ldg((const float4 *)(a.Y + ro)), y1 = __ldg((const float4 *)(a.Y + ro) + 1);
+            const float4 w0 = __ldg((const float4 *)(a.W + ro)), w1 = __ldg((const float4 *)(a.W + ro) + 1);
+            const float SS[OCT] = {s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w};
+            const float yy[OCT] = {y0.x, y0.y, y0.z, y0.w, y1.x, y1.y, y1.z, y1.w};
+            const float ww[OCT] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
+            float av[OCT], rho[OCT];
+#pragma unroll
+            for (int i = 0; i < OCT; ++i) {
+                const float r = fmaf(-cc[g][i], SS[i], yy[i]);
+                const float wr = ww[i] * r;
+                chi[g] = fmaf(wr, r, chi[g]);
+                if (ww[i] > 0.f) { cmin[g] = fminf(cmin[g], cc[g][i]); ng[g] += 1.f; }
+                av[i] = -2.f * wr * cc[g][i];
+                if (MODE == 2) rho[i] = sqrtf(ww[i]) * r;
+            }
+            ra[0] = make_float4(av[0], av[1], av[2], av[3]);
+            ra[1] = make_float4(av[4], av[5], av[6], av[7]);
+            if (MODE == 2) {
+                float4 *x4 = (float4 *)(xrow + (size_t)g * M.Ppad + j0);
+                x4[0] = make_float4(rho[0], rho[1], rho[2], rho[3]);
+                x4[1] = make_float4(rho[4], rho[5], rho[6], rho[7]);
+            }
+        }
+    }
+    if (MODE != 0) {
+        float *red = c.sm + L.oRED + c.warp * L.VR * GS;
+#pragma unroll
+        for (int g = 0; g < GS; ++g) {
+            const float s = warp_sum_f(chi[g]), n = warp_sum_f(ng[g]), m = warp_min_f(cmin[g]);
+            if (c.lane == 0) {
+                float *st = red + SLOT_STAT(L) * GS + g;
+                st[0] += s; st[GS] += n; st[2 * GS] = fminf(st[2 * GS], m);
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// a7 (+ the two kernel-parameter gradients of a6), reverse mode.  For the thread's octet of the T range:
+//   t_i   = sum_k g_k a_{i+k}            (adjoint stencil; a = 0 outside the fitted range)
+//   tmu_i, tsg_i: the same with dg/dv, dg/dsigma*   =>  dchi2/dv = sum_i T_i tmu_i, dchi2/dsigma* likewise
+//   q_k   = sum_i t_i C[k,i]
+// Partial sums go through register transposes into this warp's Q slots (pseudo-terms K, K+1 carry
+// the two kernel-parameter gradients), which v1_evaluate zeroed.
+// ------------------------------------------------------------------------------------------
+__device__ void v1_phase_adjoint(const V1Ctx &c, const SegDev &sg, int lo, int hi)
+{
+    const ModelDev &M = *c.M;
+    const V1Lay &L = *c.L;
+    const int *tap = (const int *)(c.sm + L.oTAP);
+    float *red = c.sm + L.oRED + c.warp * L.VR * GS;
+    const int P4 = M.Ppad >> 2;
+    const int wstride4 = GS * L.NA;   // float4 stride between the three reversed kernels
+    const int K2 = M.K + 2;
+    for (int jb = lo; jb < hi; jb += c.nt * OCT) {
+        const int j0 = jb + c.tid * OCT;
+        const bool act = j0 < hi;
+        float t[GS][OCT], gv[GS], gs[GS];
+#pragma unroll
+        for (int g = 0; g < GS; ++g) {
+            gv[g] = 0.f; gs[g] = 0.f;
+            if (act) {
+                float acc[3][OCT];
+                v1_stencil_octet<3>((const float4 *)v1_row(c, L.oA, sg, g), j0, tap[2 * g], tap[2 * g + 1],
+                                    (const float4 *)(c.sm + L.oGR + g * L.NA * 4), wstride4, acc);
+                const float4 *rt = (const float4 *)(v1_row(c, L.oT, sg, g) + j0);
+                const float4 t0 = rt[0], t1 = rt[1];
+                const float TT[OCT] = {t0.x, t0.y, t0.z, t0.w, t1.x, t1.y, t1.z, t1.w};
+#pragma unroll
+                for (int i = 0; i < OCT; ++i) {
+                    t[g][i] = acc[0][i];
+                    gv[g] = fmaf(TT[i], acc[1][i], gv[g]);
+                    gs[g] = fmaf(TT[i], acc[2][i], gs[g]);
+                }
+            } else {
+#pragma unroll
+                for (int i = 0; i < OCT; ++i) t[g][i] = 0.f;
+            }
+        }
+        const float4 *c4 = (const float4 *)(M.C + (act ? j0 : lo));
+        for (int k0 = 0; k0 < K2; k0 += 8) {
+            float X[32];
+#pragma unroll
+            for (int kk = 0; kk < 8; ++kk) {
+                const int k = k0 + kk;
+                if (k < M.K) {
+                    const float4 ca = __ldg(c4 + (size_t)k * P4), cb = __ldg(c4 + (size_t)k * P4 + 1);
+                    const float cc[OCT] = {ca.x, ca.y, ca.z, ca.w, cb.x, cb.y, cb.z, cb.w};
+#pragma unroll
+                    for (int g = 0; g < GS; ++g) {
+                        float s = 0.f;
+#pragma unroll
+                        for (int i = 0; i < OCT; ++i) s = fmaf(t[g][i], cc[i], s);
+                        X[kk * 4 + g] = s;
+                    }
+                } else {
+#pragma unroll
+                    for (int g = 0; g < GS; ++g) X[kk * 4 + g] = (k == M.K) ? gv[g] : (k == M.K + 1 ? gs[g] : 0.f);
+                }
+            }
+            const float tot = xreduce32(X, c.lane);
+            const int slot = SLOT_Q(L, k0 + (c.lane >> 2));
+            red[slot * GS + (c.lane & 3)] += tot;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// One evaluation of chi2 (+ gradient) at the u held in shared memory (warps g < GS have run
+// v1_param_setup for their spectrum).  All threads of the CTA call this.
+//   cold: b = 0, c_prev = 0, solve twice (solve + one refinement);  else b, c_prev are warm.
+//   mom : re-accumulate the Gram moments and re-factor (always true when cold).
+//   MODE 0: chi2 + gradient partials (Q slots) ; MODE 1: chi2 only ; MODE 2: chi2 + rho -> xrow.
+// On return (after the closing barrier) the per-warp reduction slots hold chi2 / ngood / min c and,
+// for MODE 0, the q / dv / dsigma partials.
+// ------------------------------------------------------------------------------------------
+template <int MODE>
+__device__ void v1_evaluate(const V1Ctx &c, const V1Args &a, bool cold, bool mom, float *xrow)
+{
+    const ModelDev &M = *c.M;
+    const V1Lay &L = *c.L;
+    // This warp's Q and statistics slots accumulate over sweeps and segments.  They are zeroed after
+    // the first barrier of the evaluation: only then have warps g < GS finished reading the previous
+    // evaluation's slots (v1_gradient / v1_stats run between evaluations without a barrier).
+    bool zeroed = false;
+    auto zero_slots = [&]() {
+        float *red = c.sm + L.oRED + c.warp * L.VR * GS;
+        const int q0 = (L.nmomr + L.n1r) * GS;
+        for (int i = q0 + c.lane; i < L.VR * GS; i += 32) red[i] = 0.f;
+        __syncwarp();
+        if (c.lane < GS) red[(SLOT_STAT(L) + 2) * GS + c.lane] = 3.0e38f;
+        __syncwarp();
+        zeroed = true;
+    };
+    for (int s = 0; s < M.n_seg; ++s) {
+        const SegDev &sg = M.seg[s];
+        const int rowB = s * M.n1;
+        if (sg.fit_hi <= sg.fit_lo) {
+            if (c.warp < GS) {   // no fitted pixel: b = 0, not positive definite (as the oracle)
+                for (int n = c.lane; n < M.n1; n += 32) SMV(c, L.oB, rowB + n, c.warp) = 0.f;
+                if (c.lane == 0) SMV(c, L.oSC, SC_N + s, c.warp) = 1.f;
+            }
+            continue;
+        }
+        if (c.warp < GS) {
+            v1_setup_weights(c, sg, c.warp);
+            if (cold) for (int n = c.lane; n < M.n1; n += 32) SMV(c, L.oB, rowB + n, c.warp) = 0.f;
+        }
+        if (M.n_seg > 1 || cold) {
+            // row A must be zero outside the fitted range of THIS segment (the adjoint stencil reads it)
+            for (int i = c.tid; i < GS * L.RL / 4; i += c.nt) ((float4 *)(c.sm + L.oA))[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        if (cold) {
+            for (int g = 0; g < GS; ++g)
+                for (int j = sg.fit_lo + c.tid * 4; j < sg.fit_hi; j += c.nt * 4)
+                    *(float4 *)(c.cp + (size_t)g * M.Ppad + j) = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        __syncthreads();
+        if (!zeroed) zero_slots();
+        const int reach = v1_group_reach(c);
+        const int lo = sg.fit_lo - reach, hi = sg.fit_hi + reach;
+        v1_phase_emulator(c, sg, lo, hi);
+        __syncthreads();
+        v1_phase_forward(c, sg, a, true, mom || cold);
+        __syncthreads();
+        if (c.warp < GS) v1_phase_solve(c, c.warp, s, mom || cold);
+        __syncthreads();
+        if (cold) {
+            v1_phase_residual<0>(c, sg, a, rowB, nullptr);
+            __syncthreads();   // c_prev written by this thread only, but keep phases aligned
+            v1_phase_forward(c, sg, a, false, false);
+            __syncthreads();
+            if (c.warp < GS) v1_phase_solve(c, c.warp, s, false);
+            __syncthreads();
+        }
+        v1_phase_residual<(MODE == 2 ? 2 : 1)>(c, sg, a, rowB, xrow);
+        __syncthreads();
+        if (MODE == 0) {
+            v1_phase_adjoint(c, sg, lo, hi);
+            __syncthreads();
+        }
+    }
+    if (!zeroed) {   // no segment had a fitted pixel
+        __syncthreads();
+        zero_slots();
+        __syncthreads();
+    }
+}
+
+// sums of the per-warp statistics for spectrum g (any lane may call; all return the same)
+__device__ __forceinline__ void v1_stats(const V1Ctx &c, int g, float &chi2, float &ngood, float &cmin)
+{
+    const V1Lay &L = *c.L;
+    const float *red = c.sm + L.oRED + SLOT_STAT(L) * GS + g;
+    chi2 = 0.f; ngood = 0.f; cmin = 3.0e38f;
+    for (int w = 0; w < L.NW; ++w) {
+        const float *r = red + w * L.VR * GS;
+        chi2 += r[0]; ngood += r[GS]; cmin = fminf(cmin, r[2 * GS]);
+    }
+}
+
+// a7 (tail) + chain rule to u (C.1 last lines).  Warp g; grad[p] valid on lane p afterwards.
+__device__ float v1_gradient(const V1Ctx &c, int g)
+{
+    const ModelDev &M = *c.M;
+    const V1Lay &L = *c.L;
+    const float *red = c.sm + L.oRED;
+    const int wst = L.VR * GS;
+    for (int k = c.lane; k < M.K + 2; k += 32) {
+        float s = 0.f;
+        for (int w = 0; w < L.NW; ++w) s += red[w * wst + SLOT_Q(L, k) * GS + g];
+        SMV(c, L.oQ, k, g) = s;
+    }
+    __syncwarp();
+    float mine = 0.f;
+    for (int l = 0; l < M.L; ++l) {
+        float gx = 0.f;
+        for (int k = c.lane; k < M.K; k += 32) {
+            const int el = M.exps[k * M.L + l];
+            if (el == 0) continue;
+            float d = (float)el;
+            for (int l2 = 0; l2 < M.L; ++l2) {
+                const int e2 = M.exps[k * M.L + l2] - (l2 == l ? 1 : 0);
+                const float x = SMV(c, L.oX, l2, g);
+                for (int q = 0; q < e2; ++q) d *= x;
+            }
+            gx = fmaf(d, SMV(c, L.oQ, k, g), gx);
+        }
+        gx = warp_sum_f(gx);
+        const float u = SMV(c, L.oU, l, g);
+        const float half = (M.hi[l] - M.lo[l]) * 0.5f;
+        const float th = M.lo[l] + (u + 1.f) * half;
+        const float dxdt = M.label_log10[l] ? M.emu_a[l] / (th * 2.302585093f) : M.emu_a[l];
+        if (c.lane == l) mine = gx * dxdt * half;
+    }
+    if (c.lane == M.L) mine = SMV(c, L.oQ, M.K, g) * (M.hi[M.L] - M.lo[M.L]) * 0.5f;
+    if (c.lane == M.L + 1) mine = SMV(c, L.oQ, M.K + 1, g) * (M.hi[M.L + 1] - M.lo[M.L + 1]) * 0.5f;
+    return mine;
+}
+
+// internal Chebyshev(t) coefficients -> plain Legendre(x^) (C.2-8), fp64.  Warp g, lanes over rows.
+__device__ void v1_write_cont(const V1Ctx &c, int g, float *out)
+{
+    const ModelDev &M = *c.M;
+    for (int s = 0; s < M.n_seg; ++s) {
+        const double *cv = M.conv + (size_t)s * M.n1 * M.n1;
+        for (int m = c.lane; m < M.n1; m += 32) {
+            double acc = 0.0;
+            for (int n = 0; n < M.n1; ++n) acc += cv[m * M.n1 + n] * (double)SMV(c, c.L->oB, s * M.n1 + n, g);
+            out[s * M.n1 + m] = (float)acc;
+        }
+    }
+}
+
+__device__ __forceinline__ void v1_make_ctx(V1Ctx &c, const ModelDev &M, const V1Lay &L, float *sm, const V1Args &a)
+{
+    c.M = &M; c.L = &L; c.sm = sm;
+    c.tid = threadIdx.x; c.lane = threadIdx.x & 31; c.warp = threadIdx.x >> 5; c.nt = blockDim.x;
+    c.cp = a.CP + (size_t)blockIdx.x * GS * M.Ppad;
+}
+
+__device__ __forceinline__ void v1_set_group(V1Ctx &c, const V1Args &a, int grp)
+{
+#pragma unroll
+    for (int g = 0; g < GS; ++g) {
+        long long i = (long long)grp * GS + g;
+        c.spec[g] = i < a.B ? i : a.B - 1;
+    }
+}
+
+// a9: error estimate (C.2-22/23).  J by central differences of the re-solved whitened
+// residual rho(u), Sigma = rho^T rho/(N_good - NP) (J^T J)^-1, err_p = sqrt(Sigma_pp) (hi_p - lo_p)/2.
+__device__ void v1_errors(V1Ctx &c, const V1Args &a, float chi2_g, float ngood_g, bool valid_g)
+{
+    const ModelDev &M = *c.M;
+    const V1Lay &L = *c.L;
+    const int NP = M.NP;
+    const size_t plane = (size_t)GS * M.Ppad;
+    float *xj = a.XJ + (size_t)blockIdx.x * (1 + NP) * plane;
+    for (int p = 0; p < NP; ++p) {
+        float u0 = 0.f;
+        if (c.warp < GS) {
+            u0 = SMV(c, L.oU, p, c.warp);
+            __syncwarp();
+            if (c.lane == 0) SMV(c, L.oU, p, c.warp) = u0 + a.fd_h;
+            __syncwarp();
+            v1_param_setup(c, c.warp);
+        }
+        v1_evaluate<2>(c, a, false, true, xj);
+        if (c.warp < GS) {
+            if (c.lane == 0) SMV(c, L.oU, p, c.warp) = u0 - a.fd_h;
+            __syncwarp();
+            v1_param_setup(c, c.warp);
+        }
+        v1_evaluate<2>(c, a, false, true, xj + (1 + p) * plane);
+        if (c.warp < GS) {
+            if (c.lane == 0) SMV(c, L.oU, p, c.warp) = u0;
+            __syncwarp();
+        }
+        __syncthreads();
+        // J_p = (rho+ - rho-)/(u+ - u-) on the pixels this thread owns (it wrote both)
+        for (int s = 0; s < M.n_seg; ++s) {
+            const SegDev &sg = M.seg[s];
+            for (int j0 = sg.fit_lo + c.tid * OCT; j0 < sg.fit_hi; j0 += c.nt * OCT)
+                for (int g = 0; g < GS; ++g) {
+                    const float uu = SMV(c, L.oU, p, g);
+                    const float inv = 1.f / ((uu + a.fd_h) - (uu - a.fd_h));
+                    float4 *jp = (float4 *)(xj + (1 + p) * plane + (size_t)g * M.Ppad + j0);
+                    const float4 *xp = (const float4 *)(xj + (size_t)g * M.Ppad + j0);
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const float4 x = xp[h], m = jp[h];
+                        jp[h] = make_float4((x.x - m.x) * inv, (x.y - m.y) * inv, (x.z - m.z) * inv, (x.w - m.w) * inv);
+                    }
+                }
+        }
+        __syncthreads();
+    }
+    // N = J^T J (packed lower), fp64 accumulation across warps in shared memory (aliases the factor area)
+    double *N = (double *)(c.sm + L.oLF);
+    const int npair = NP * (NP + 1) / 2;
+    for (int i = c.tid; i < GS * npair; i += c.nt) N[i] = 0.0;
+    __syncthreads();
+    for (int s = 0; s < M.n_seg; ++s) {
+        const SegDev &sg = M.seg[s];
+        for (int jb = sg.fit_lo; jb < sg.fit_hi; jb += c.nt * OCT) {
+            const int j0 = jb + c.tid * OCT;
+            const bool act = j0 < sg.fit_hi;
+            for (int pi0 = 0; pi0 < npair; pi0 += 8) {
+                float X[32];
+#pragma unroll
+                for (int kk = 0; kk < 8; ++kk) {
+                    const int pi = pi0 + kk;
+                    int p = 0;
+                    while ((p + 1) * (p + 2) / 2 <= pi) ++p;
+                    const int q = pi - p * (p + 1) / 2;
+#pragma unroll
+                    for (int g = 0; g < GS; ++g) {
+                        float sacc = 0.f;
+                        if (act && pi < npair) {
+                            const float4 *A4 = (const float4 *)(xj + (1 + p) * plane + (size_t)g * M.Ppad + j0);
+                            const float4 *B4 = (const float4 *)(xj + (1 + q) * plane + (size_t)g * M.Ppad + j0);
+                            const float4 a0 = A4[0], a1 = A4[1], b0 = B4[0], b1 = B4[1];
+                            sacc = a0.x * b0.x + a0.y * b0.y + a0.z * b0.z + a0.w * b0.w +
+                                   a1.x * b1.x + a1.y * b1.y + a1.z * b1.z + a1.w * b1.w;
+                        }
+                        X[kk * 4 + g] = sacc;
+                    }
+                }
+                const float tot = xreduce32(X, c.lane);
+                const int pi = pi0 + (c.lane >> 2);
+                if (pi < npair) atomicAdd(&N[(c.lane & 3) * npair + pi], (double)tot);
+            }
+        }
+    }
+    __syncthreads();
+    if (c.warp < GS && c.lane == 0) {
+        const int g = c.warp;
+        double *Ng = N + g * npair;
+        bool ok = ngood_g > (float)NP;
+        for (int p = 0; p < NP && ok; ++p)
+            for (int q = 0; q <= p; ++q) {
+                double s = Ng[p * (p + 1) / 2 + q];
+                for (int k = 0; k < q; ++k) s -= Ng[p * (p + 1) / 2 + k] * Ng[q * (q + 1) / 2 + k];
+                if (p == q) {
+                    if (!(s > 0.0)) { ok = false; break; }
+                    Ng[p * (p + 1) / 2 + p] = sqrt(s);
+                } else
+                    Ng[p * (p + 1) / 2 + q] = s / Ng[q * (q + 1) / 2 + q];
+            }
+        const double s2 = (double)chi2_g / ((double)ngood_g - (double)NP);
+        for (int p = 0; p < NP; ++p) {
+            float e = __int_as_float(0x7fc00000);
+            if (ok) {   // (J^T J)^-1_pp = |L^-1 e_p|^2
+                double y[LASP_NPMAX];
+                double nrm = 0.0;
+                for (int r = p; r < NP; ++r) {
+                    double s = (r == p) ? 1.0 : 0.0;
+                    for (int k = p; k < r; ++k) s -= Ng[r * (r + 1) / 2 + k] * y[k];
+                    y[r] = s / Ng[r * (r + 1) / 2 + r];
+                    nrm += y[r] * y[r];
+                }
+                e = (float)(sqrt(s2 * nrm) * (double)(M.hi[p] - M.lo[p]) * 0.5);
+            }
+            if (valid_g) a.err[c.spec[g] * NP + p] = e;
+        }
+    }
+    __syncthreads();
+}
+
+// ------------------------------------------------------------------------------------------
+// lasp_fit_batch: a1-a9 for groups of GS spectra, persistent CTAs
+// ------------------------------------------------------------------------------------------
+template <int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB)
+lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V1Lay L, const V1Args a)
+{
+    extern __shared__ float4 v1_smem4[];
+    V1Ctx c;
+    v1_make_ctx(c, M, L, (float *)v1_smem4, a);
+    const int NP = M.NP, g = c.warp;
+    for (int grp = blockIdx.x; grp < a.ngroups; grp += gridDim.x) {
+        v1_set_group(c, a, grp);
+        __syncthreads();   // the previous group's last readers are done with shared memory
+        const bool valid = g < GS && (long long)grp * GS + g < a.B;
+        if (g < GS) {
+            for (int p = c.lane; p < NP; p += 32) {
+                const float th = a.init[c.spec[g] * NP + p];
+                const float u = 2.f * (th - M.lo[p]) / (M.hi[p] - M.lo[p]) - 1.f;
+                SMV(c, L.oU, p, g) = fminf(fmaxf(u, -1.f), 1.f);
+                SMV(c, L.oM, p, g) = 0.f;
+                SMV(c, L.oV, p, g) = 0.f;
+            }
+            __syncwarp();
+            v1_param_setup(c, g);
+        }
+        float pb1 = 1.f, pb2 = 1.f;
+        for (int t = 1; t <= a.n_iter; ++t) {
+            v1_evaluate<0>(c, a, t == 1, (t - 1) % L.refresh == 0, nullptr);
+            pb1 *= a.b1; pb2 *= a.b2;
+            if (g < GS) {
+                const float gr = v1_gradient(c, g);
+                // a8: Adam (C.2-20), then clip to the prior box (C.2-18); lane p owns parameter p
+                for (int p0 = 0; p0 < NP; p0 += 32) {   // NP <= 32
+                    const int p = p0 + c.lane;
+                    if (p < NP) {
+                        const float m = a.b1 * SMV(c, L.oM, p, g) + (1.f - a.b1) * gr;
+                        const float v = a.b2 * SMV(c, L.oV, p, g) + (1.f - a.b2) * gr * gr;
+                        SMV(c, L.oM, p, g) = m; SMV(c, L.oV, p, g) = v;
+                        const float mh = m / (1.f - pb1), vh = v / (1.f - pb2);
+                        float u = SMV(c, L.oU, p, g) - a.lr * mh / (sqrtf(vh) + a.eps);
+                        if (!(u == u)) u = SMV(c, L.oU, p, g);   // keep the iterate if the gradient was NaN
+                        SMV(c, L.oU, p, g) = fminf(fmaxf(u, -1.f), 1.f);
+                    }
+                }
+                __syncwarp();
+                v1_param_setup(c, g);
+            }
+        }
+        // a9: one more evaluation at the final iterate (C.2-21)
+        v1_evaluate<1>(c, a, a.n_iter == 0, true, nullptr);
+        float chi2 = 0.f, ngood = 0.f, cmin = 0.f;
+        if (g < GS) {
+            v1_stats(c, g, chi2, ngood, cmin);
+            int st = 0;
+            bool fin = isfinite(chi2);
+            bool bound = false;
+            for (int p = c.lane; p < NP; p += 32) {
+                const float u = SMV(c, L.oU, p, g);
+                fin = fin && isfinite(u);
+                bound = bound || (u <= -1.f || u >= 1.f);
+            }
+            for (int n = c.lane; n < M.nc; n += 32) fin = fin && isfinite(SMV(c, L.oB, n, g));
+            fin = __all_sync(FULL, fin);
+            bound = __any_sync(FULL, bound);
+            const bool anyfail = __any_sync(FULL, c.lane < M.n_seg && c.sm[L.oSC + (SC_N + c.lane) * GS + g] != 0.f);
+            if (anyfail) st |= LASP_ST_NOT_SPD;
+            if (bound) st |= LASP_ST_ON_BOUND;
+            if (!fin) st |= LASP_ST_NONFINITE;
+            if (ngood > 0.f && cmin <= 0.f) st |= LASP_ST_NEG_CONT;
+            if (valid) {
+                const long long i = c.spec[g];
+                for (int p = c.lane; p < NP; p += 32)
+                    a.params[i * NP + p] = M.lo[p] + (SMV(c, L.oU, p, g) + 1.f) * (M.hi[p] - M.lo[p]) * 0.5f;
+                if (c.lane == 0) {
+                    a.chi2[i] = chi2;
+                    if (a.status) a.status[i] = st;
+                }
+                if (a.cont) v1_write_cont(c, g, a.cont + i * M.nc);
+            }
+        }
+        if (a.err) v1_errors(c, a, chi2, ngood, valid);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// lasp_eval_grad: one cold evaluation of chi2 and d chi2/d u at given physical parameters
+// ------------------------------------------------------------------------------------------
+template <int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB)
+lasp_v1_grad_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V1Lay L, const V1Args a)
+{
+    extern __shared__ float4 v1_smem4[];
+    V1Ctx c;
+    v1_make_ctx(c, M, L, (float *)v1_smem4, a);
+    const int NP = M.NP, g = c.warp;
+    for (int grp = blockIdx.x; grp < a.ngroups; grp += gridDim.x) {
+        v1_set_group(c, a, grp);
+        __syncthreads();
+        const bool valid = g < GS && (long long)grp * GS + g < a.B;
+        if (g < GS) {
+            for (int p = c.lane; p < NP; p += 32)
+                SMV(c, L.oU, p, g) = 2.f * (a.gparams[c.spec[g] * NP + p] - M.lo[p]) / (M.hi[p] - M.lo[p]) - 1.f;
+            __syncwarp();
+            v1_param_setup(c, g);
+        }
+        v1_evaluate<0>(c, a, true, true, nullptr);
+        if (g < GS) {
+            const float gr = v1_gradient(c, g);
+            float chi2, ngood, cmin;
+            v1_stats(c, g, chi2, ngood, cmin);
+            const bool anyfail = __any_sync(FULL, c.lane < M.n_seg && c.sm[L.oSC + (SC_N + c.lane) * GS + g] != 0.f);
+            if (valid) {
+                const long long i = c.spec[g];
+                if (c.lane < NP) a.grad_u[i * NP + c.lane] = gr;
+                if (c.lane == 0) {
+                    a.chi2[i] = chi2;
+                    if (a.status) a.status[i] = anyfail ? LASP_ST_NOT_SPD : 0;
+                }
+                if (a.cont) v1_write_cont(c, g, a.cont + i * M.nc);
+            }
+        }
+    }
+}

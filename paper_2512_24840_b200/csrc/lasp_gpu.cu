@@ -3,12 +3,14 @@
 // runs in the kernels of lasp_kernels.cuh.
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
 #include <vector>
 
 #include "lasp_kernels.cuh"
+#include "lasp_fit_v1.cuh"
 
 #define LASP_VERSION 100
 static const double kC_KMS = 299792.458;
@@ -27,6 +29,14 @@ struct lasp_ctx {
     size_t scratch_slots = 0;
     long long launches = 0;
     double mean_dlog = 0;
+    // kernel v1 (uniform segments): layout, launch shape, staged planes and scratch
+    bool v1_ok = false;
+    V1Lay V1;
+    int v1_nt = 0, v1_maxt = 0, v1_cta_per_sm = 1;
+    float *dY = nullptr, *dW = nullptr;
+    size_t plane_rows = 0;
+    float *dCP = nullptr, *dXJ = nullptr;
+    size_t cp_ctas = 0, xj_ctas = 0;
     std::string err;
 };
 
@@ -84,9 +94,12 @@ extern "C" int lasp_destroy(lasp_ctx *c)
     cudaSetDevice(c->device);
     cudaFree(c->dC); cudaFree(c->dinv_s); cudaFree(c->dexps); cudaFree(c->dconv); cudaFree(c->dnedge);
     cudaFree(c->dYW); cudaFree(c->dscratch);
+    cudaFree(c->dY); cudaFree(c->dW); cudaFree(c->dCP); cudaFree(c->dXJ);
     delete c;
     return LASP_OK;
 }
+
+static int setup_v1(lasp_ctx *c, const cudaDeviceProp &prop);
 
 extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx **out)
 {
@@ -163,7 +176,7 @@ extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx *
         SegDev &S = M.seg[sg];
         const double si = d->seg_sigma_inst[sg];
         const int Hm = (int)ceil((vmax + 5.0 * sqrt(smax * smax + si * si)) / smin) + 1;
-        S.halo = roundup(Hm, CH);
+        S.halo = roundup(Hm + 18, CH);   // v1 reads up to 18 pixels past the largest support
         S.po = po; S.P = Ps; S.o = o;
         S.len = S.halo + roundup(Ps, CH) + S.halo;
         po += S.len;
@@ -240,7 +253,80 @@ extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx *
     CUDA_TRY_C(cudaFuncSetAttribute(lasp_fit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
     CUDA_TRY_C(cudaFuncSetAttribute(lasp_grad_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
     CUDA_TRY_C(cudaFuncSetAttribute(lasp_model_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
+    setup_v1(c, prop);
     *out = c;
+    return LASP_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// kernel v1: shared-memory layout and launch shape (lasp_fit_v1.cuh)
+// ------------------------------------------------------------------------------------------
+template <typename F>
+static void v1_for_kernels(F f)
+{
+    f((const void *)lasp_v1_fit_kernel<192, 2>, 192);
+    f((const void *)lasp_v1_grad_kernel<192, 2>, 192);
+    f((const void *)lasp_v1_fit_kernel<384, 1>, 384);
+    f((const void *)lasp_v1_grad_kernel<384, 1>, 384);
+}
+
+static int setup_v1(lasp_ctx *c, const cudaDeviceProp &prop)
+{
+    const ModelDev &M = c->M;
+    c->v1_ok = false;
+    int maxlen = 0, guard = 0, nfit = 0, hmax = 0;
+    for (int s = 0; s < M.n_seg; ++s) {
+        const SegDev &S = M.seg[s];
+        if (!S.uniform) return LASP_OK;   // per-pixel kernels (linear grids) stay on the v0 kernel
+        maxlen = std::max(maxlen, S.len);
+        guard = std::max(guard, S.halo);
+        nfit = std::max(nfit, (S.fit_hi - S.fit_lo) / OCT);
+        hmax = std::max(hmax, S.halo - 18);
+    }
+    if (M.NP > 32 || M.n1 > 32) return LASP_OK;
+    V1Lay &L = c->V1;
+    memset(&L, 0, sizeof(L));
+    int nt = std::max(GS * 32, roundup(std::max(nfit, 1), 32));
+    if (nt > 384) nt = 384;               // longer segments are swept in several passes
+    c->v1_nt = nt;
+    c->v1_maxt = nt <= 192 ? 192 : 384;
+    L.NW = nt / 32;
+    L.GUARD = guard;
+    L.RL = maxlen + 2 * guard;
+    L.Hm = hmax;
+    L.NA = (hmax + 3) / 4 + hmax / 4 + 2;
+    L.n1r = roundup(M.n1, 8);
+    L.nmomr = L.n1r + roundup(std::max(M.nmom - L.n1r, 0), 8);
+    L.VR = L.nmomr + L.n1r + roundup(M.K + 2, 8) + 4;
+    const char *rf = getenv("LASP_REFRESH");
+    L.refresh = rf ? std::max(1, atoi(rf)) : 1;
+    int o = 0;
+    auto take = [&](int n) { int r = o; o += roundup(n, 4); return r; };
+    L.oT = take(GS * L.RL); L.oA = take(GS * L.RL);
+    L.oU = take(GS * M.NP); L.oM = take(GS * M.NP); L.oV = take(GS * M.NP);
+    L.oX = take(GS * M.L); L.oPHI = take(GS * M.K);
+    L.oGW = take(GS * L.NA * 4); L.oGR = take(3 * GS * L.NA * 4); L.oTAP = take(2 * GS);
+    L.oMOM = take(GS * L.nmomr); L.oRHS = take(GS * L.n1r); L.oB = take(GS * M.nc);
+    L.oRED = take(L.NW * L.VR * GS);
+    const int npair = M.NP * (M.NP + 1) / 2;
+    L.oLF = take(std::max(GS * V1_LFS, 2 * GS * npair + 4));
+    L.oQ = take(GS * (M.K + 2)); L.oSC = take(GS * (SC_N + M.n_seg));
+    L.total = o;
+    const size_t bytes = (size_t)o * sizeof(float);
+    if (bytes > prop.sharedMemPerBlockOptin) return LASP_OK;   // does not fit: v0 handles it
+    bool ok = true;
+    v1_for_kernels([&](const void *f, int) {
+        if (cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess) ok = false;
+    });
+    if (!ok) { cudaGetLastError(); return LASP_OK; }
+    int per_sm = 0;
+    const void *fk = c->v1_maxt == 192 ? (const void *)lasp_v1_fit_kernel<192, 2> : (const void *)lasp_v1_fit_kernel<384, 1>;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fk, nt, bytes) != cudaSuccess || per_sm < 1) {
+        cudaGetLastError();
+        return LASP_OK;
+    }
+    c->v1_cta_per_sm = per_sm;
+    c->v1_ok = getenv("LASP_FORCE_V0") == nullptr;
     return LASP_OK;
 }
 
@@ -293,6 +379,87 @@ static int stage(lasp_ctx *c, int64_t B, const float *flux, const float *ivar, c
     return LASP_OK;
 }
 
+// ---- kernel v1: staging (a0), workspace, launches -----------------------------------------------
+// a0 for v1: w = mask*ivar, zero on the n_edge pixels at each end of each segment (Eq. 8),
+// non-finite or non-positive ivar treated as masked; rows go to the padded layout (halos zero).
+__global__ void lasp_v1_stage_kernel(const __grid_constant__ ModelDev M, const int *__restrict__ n_edge,
+                                     const float *__restrict__ flux, const float *__restrict__ ivar,
+                                     const uint8_t *__restrict__ mask, float *__restrict__ Y, float *__restrict__ W)
+{
+    const size_t row = blockIdx.x;
+    for (int jp = threadIdx.x; jp < M.Ppad; jp += blockDim.x) {
+        int s = 0;
+        while (s + 1 < M.n_seg && jp >= M.seg[s + 1].po) ++s;
+        const SegDev &sg = M.seg[s];
+        const int rel = jp - sg.po - sg.halo;
+        float y = 0.f, w = 0.f;
+        if (rel >= 0 && rel < sg.P) {
+            const size_t o = row * M.P + sg.o + rel;
+            y = flux[o]; w = ivar[o];
+            if (mask && mask[o] == 0) w = 0.f;
+            if (!(w > 0.f) || !isfinite(w) || !isfinite(y)) { w = 0.f; y = 0.f; }
+            const int ne = n_edge[s];
+            if (rel < ne || rel >= sg.P - ne) w = 0.f;
+        }
+        Y[row * M.Ppad + jp] = y;
+        W[row * M.Ppad + jp] = w;
+    }
+}
+
+static int v1_grid(const lasp_ctx *c, int64_t B, int &ngroups)
+{
+    ngroups = (int)((B + GS - 1) / GS);
+    return std::min(ngroups, c->num_sms * c->v1_cta_per_sm);
+}
+
+static int v1_workspace(lasp_ctx *c, int64_t B, bool need_xj)
+{
+    CUDA_TRY(c, cudaSetDevice(c->device));
+    const ModelDev &M = c->M;
+    if ((size_t)B > c->plane_rows) {
+        cudaFree(c->dY); cudaFree(c->dW);
+        c->dY = c->dW = nullptr; c->plane_rows = 0;
+        CUDA_TRY(c, cudaMalloc(&c->dY, (size_t)B * M.Ppad * sizeof(float)));
+        CUDA_TRY(c, cudaMalloc(&c->dW, (size_t)B * M.Ppad * sizeof(float)));
+        c->plane_rows = (size_t)B;
+    }
+    const size_t ctas = (size_t)c->num_sms * c->v1_cta_per_sm;
+    if (ctas > c->cp_ctas) {
+        cudaFree(c->dCP); c->dCP = nullptr; c->cp_ctas = 0;
+        CUDA_TRY(c, cudaMalloc(&c->dCP, ctas * GS * M.Ppad * sizeof(float)));
+        c->cp_ctas = ctas;
+    }
+    if (need_xj && ctas > c->xj_ctas) {
+        cudaFree(c->dXJ); c->dXJ = nullptr; c->xj_ctas = 0;
+        CUDA_TRY(c, cudaMalloc(&c->dXJ, ctas * (size_t)(1 + M.NP) * GS * M.Ppad * sizeof(float)));
+        c->xj_ctas = ctas;
+    }
+    return LASP_OK;
+}
+
+static int v1_stage(lasp_ctx *c, int64_t B, const float *flux, const float *ivar, const uint8_t *mask, cudaStream_t st)
+{
+    lasp_v1_stage_kernel<<<(unsigned)B, 256, 0, st>>>(c->M, c->dnedge, flux, ivar, mask, c->dY, c->dW);
+    c->launches += 1;
+    CUDA_TRY(c, cudaGetLastError());
+    return LASP_OK;
+}
+
+static int v1_launch(lasp_ctx *c, bool grad, const V1Args &a, int grid, cudaStream_t st)
+{
+    const size_t smem = (size_t)c->V1.total * sizeof(float);
+    if (c->v1_maxt == 192) {
+        if (grad) lasp_v1_grad_kernel<192, 2><<<grid, c->v1_nt, smem, st>>>(c->M, c->V1, a);
+        else lasp_v1_fit_kernel<192, 2><<<grid, c->v1_nt, smem, st>>>(c->M, c->V1, a);
+    } else {
+        if (grad) lasp_v1_grad_kernel<384, 1><<<grid, c->v1_nt, smem, st>>>(c->M, c->V1, a);
+        else lasp_v1_fit_kernel<384, 1><<<grid, c->v1_nt, smem, st>>>(c->M, c->V1, a);
+    }
+    c->launches += 1;
+    CUDA_TRY(c, cudaGetLastError());
+    return LASP_OK;
+}
+
 extern "C" int lasp_fit_batch(lasp_ctx *c, int64_t B, const float *flux, const float *ivar,
                               const uint8_t *mask, const float *init, const lasp_fit_opts *opts,
                               float *params, float *cont, float *chi2, float *err, int32_t *status,
@@ -304,7 +471,22 @@ extern "C" int lasp_fit_batch(lasp_ctx *c, int64_t B, const float *flux, const f
     if (opts->n_iter < 0 || !(opts->lr > 0.f) || !(opts->beta1 >= 0.f && opts->beta1 < 1.f) ||
         !(opts->beta2 >= 0.f && opts->beta2 < 1.f) || !(opts->eps >= 0.f))
         return fail(c, LASP_ERR_INVALID_ARG, "lasp_fit_batch: bad Adam hyper-parameters");
-    if (B > (int64_t)1 << 36) return fail(c, LASP_ERR_UNSUPPORTED, "B too large");
+    if (B > (int64_t)1 << 30) return fail(c, LASP_ERR_UNSUPPORTED, "B too large");
+    if (c->v1_ok) {
+        int rc = v1_workspace(c, B, err != nullptr);
+        if (rc) return rc;
+        cudaStream_t st = (cudaStream_t)stream;
+        rc = v1_stage(c, B, flux, ivar, mask, st);
+        if (rc) return rc;
+        V1Args a;
+        memset(&a, 0, sizeof(a));
+        a.Y = c->dY; a.W = c->dW; a.CP = c->dCP; a.XJ = c->dXJ; a.B = B;
+        const int grid = v1_grid(c, B, a.ngroups);
+        a.init = init; a.n_iter = opts->n_iter; a.lr = opts->lr; a.b1 = opts->beta1; a.b2 = opts->beta2;
+        a.eps = opts->eps; a.fd_h = 2e-3f;  // fp32 central-difference step in u (C.2-22)
+        a.params = params; a.cont = cont; a.chi2 = chi2; a.err = err; a.status = status;
+        return v1_launch(c, false, a, grid, st);
+    }
     int rc = ensure_workspace(c, B, true);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
@@ -331,6 +513,19 @@ extern "C" int lasp_eval_grad(lasp_ctx *c, int64_t B, const float *flux, const f
     if (!c) return fail(nullptr, LASP_ERR_INVALID_ARG, "null ctx");
     if (B < 1 || !flux || !ivar || !params || !chi2 || !grad_u)
         return fail(c, LASP_ERR_INVALID_ARG, "lasp_eval_grad: null pointer or B < 1");
+    if (c->v1_ok) {
+        int rc = v1_workspace(c, B, false);
+        if (rc) return rc;
+        cudaStream_t st = (cudaStream_t)stream;
+        rc = v1_stage(c, B, flux, ivar, mask, st);
+        if (rc) return rc;
+        V1Args a;
+        memset(&a, 0, sizeof(a));
+        a.Y = c->dY; a.W = c->dW; a.CP = c->dCP; a.B = B;
+        const int grid = v1_grid(c, B, a.ngroups);
+        a.gparams = params; a.chi2 = chi2; a.grad_u = grad_u; a.cont = cont; a.status = status;
+        return v1_launch(c, true, a, grid, st);
+    }
     int rc = ensure_workspace(c, B, true);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
