@@ -312,7 +312,7 @@ def run_gpu(args):
     achieved = flop_launch / (kern_ms * 1e-3) / 1e12
     peak = prop.multi_processor_count * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
     roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-            "traffic": None, "kernel": "lasp_fit_kernel", "fma_per_spectrum_step": fma_step,
+            "traffic": None, "kernel": "lasp_v1_fit_kernel" if model.uses_v1() else "lasp_fit_kernel", "fma_per_spectrum_step": fma_step,
             "mean_taps": taps, "peak_source": f"SMs x 128 FP32 lanes x 2 x sm_max_mhz ({peaks['source']})",
             "frac_at_sampled_clock": (achieved / (peak * clocks["sm_mhz"] / peaks["sm_max_mhz"])
                                       if clocks and clocks.get("sm_mhz") else None)}

@@ -117,6 +117,10 @@ int lasp_eval_grad(lasp_ctx *ctx, int64_t B, const float *flux, const float *iva
                    const uint8_t *mask, const float *params, float *chi2, float *grad_u,
                    float *cont, int32_t *status, void *stream);
 
+/* Which fit kernel serves this ctx: 1 = the fused group kernel (all segments on a uniform log grid),
+ * 0 = the lane-per-spectrum kernel with per-pixel broadening kernels (linear grids, C.2-14). */
+int lasp_kernel_variant(const lasp_ctx *ctx);
+
 /* Number of kernels launched by this ctx so far (bench.py reports it as gpu_launches). */
 int64_t lasp_launch_count(const lasp_ctx *ctx);
 

@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "liblasp_gpu.so")
 
 SYMBOLS = ["lasp_create", "lasp_destroy", "lasp_reserve", "lasp_fit_batch", "lasp_eval_model",
-           "lasp_eval_grad", "lasp_launch_count", "lasp_fma_per_spectrum_step", "lasp_last_error",
+           "lasp_eval_grad", "lasp_kernel_variant", "lasp_launch_count", "lasp_fma_per_spectrum_step", "lasp_last_error",
            "lasp_version"]
 
 LASP_ST_NOT_SPD, LASP_ST_NONFINITE, LASP_ST_NEG_CONT, LASP_ST_ON_BOUND = 1, 2, 4, 8
@@ -64,6 +64,8 @@ def lib():
                                     [C.c_void_p] * 6
         L.lasp_eval_model.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 4
         L.lasp_eval_grad.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 9
+        L.lasp_kernel_variant.argtypes = [C.c_void_p]
+        L.lasp_kernel_variant.restype = C.c_int
         L.lasp_launch_count.argtypes = [C.c_void_p]
         L.lasp_launch_count.restype = C.c_int64
         L.lasp_fma_per_spectrum_step.argtypes = [C.c_void_p, C.c_double]
@@ -145,6 +147,10 @@ class LaspModel:
 
     def reserve(self, B: int):
         self._check(lib().lasp_reserve(self.ctx, B), "lasp_reserve")
+
+    def uses_v1(self) -> bool:
+        """True when the fused group kernel (lasp_fit_v1.cuh) serves this model (uniform segments)."""
+        return bool(lib().lasp_kernel_variant(self.ctx) == 1)
 
     def launch_count(self) -> int:
         return int(lib().lasp_launch_count(self.ctx))

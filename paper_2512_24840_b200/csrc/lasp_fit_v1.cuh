@@ -16,6 +16,11 @@
 #pragma once
 #include "lasp_device.cuh"
 
+// All shared memory is addressed from this symbol so that the compiler emits LDS/STS (a pointer carried
+// in a struct is generic and costs LD/ST with global-memory scoreboarding).
+extern __shared__ float4 v1_smem4[];
+#define V1SM ((float *)v1_smem4)
+
 #define GS 4    // spectra per CTA group
 #define OCT 8   // pixels per thread tile
 
@@ -80,13 +85,12 @@ __device__ __forceinline__ float warp_min_f(float v)
 struct V1Ctx {
     const ModelDev *M;
     const V1Lay *L;
-    float *sm;
     int tid, lane, warp, nt;
     long long spec[GS];   // clamped spectrum indices of the group
     float *cp;            // this CTA's c_prev scratch
 };
 
-#define SMV(c, off, idx, g) (c).sm[(off) + (idx) * GS + (g)]
+#define SMV(c, off, idx, g) V1SM[(off) + (idx) * GS + (g)]
 
 // ------------------------------------------------------------------------------------------
 // a1: de-normalise, emulator inputs, monomials (Eq. 1, C.2-18/19).  Warp g, spectrum g.
@@ -143,8 +147,8 @@ __device__ void v1_setup_weights(const V1Ctx &c, const SegDev &sg, int g)
     const float cmu = is2 * sg.inv_s;                  // dS/dv      = (1/s) sum dg/dmu T
     const float csig = is2 * sqrtf(is2) * (sigstar / sigtot) * sg.inv_s;
     const int a_lo = -(H / 4), na = (H + 3) / 4 - a_lo + 1;
-    float *gw = c.sm + L.oGW + g * L.NA * 4;
-    float *gr = c.sm + L.oGR + g * L.NA * 4;
+    float *gw = V1SM + L.oGW + g * L.NA * 4;
+    float *gr = V1SM + L.oGR + g * L.NA * 4;
     const int rs = GS * L.NA * 4;
     for (int idx = c.lane; idx < na * 4; idx += 32) {
         const int k = 4 * (a_lo + (idx >> 2)) - 3 + (idx & 3);
@@ -158,7 +162,7 @@ __device__ void v1_setup_weights(const V1Ctx &c, const SegDev &sg, int g)
         gr[2 * rs + idx] = gg * (d * d - e2n) * csig;
     }
     if (c.lane == 0) {
-        int *tap = (int *)(c.sm + L.oTAP);
+        int *tap = (int *)(V1SM + L.oTAP);
         tap[g * 2] = a_lo; tap[g * 2 + 1] = na;
     }
     __syncwarp();
@@ -205,13 +209,13 @@ __device__ __forceinline__ void v1_stencil_octet(const float4 *__restrict__ row4
 // shared-memory row of spectrum g in buffer `off`, as a float pointer indexed by padded pixel jp
 __device__ __forceinline__ float *v1_row(const V1Ctx &c, int off, const SegDev &sg, int g)
 {
-    return c.sm + off + g * c.L->RL + c.L->GUARD - sg.po;
+    return V1SM + off + g * c.L->RL + c.L->GUARD - sg.po;
 }
 
 // largest support of the group (for the T range), from the tap tables
 __device__ __forceinline__ int v1_group_reach(const V1Ctx &c)
 {
-    const int *tap = (const int *)(c.sm + c.L->oTAP);
+    const int *tap = (const int *)(V1SM + c.L->oTAP);
     int r = 0;
 #pragma unroll
     for (int g = 0; g < GS; ++g) {
@@ -228,7 +232,7 @@ __device__ void v1_phase_emulator(const V1Ctx &c, const SegDev &sg, int lo, int 
 {
     const ModelDev &M = *c.M;
     const V1Lay &L = *c.L;
-    const float4 *phi4 = (const float4 *)(c.sm + L.oPHI);
+    const float4 *phi4 = (const float4 *)(V1SM + L.oPHI);
     const int P4 = M.Ppad >> 2;
     for (int j0 = lo + c.tid * OCT; j0 < hi; j0 += c.nt * OCT) {
         float acc[GS][OCT];
@@ -236,17 +240,40 @@ __device__ void v1_phase_emulator(const V1Ctx &c, const SegDev &sg, int lo, int 
         for (int g = 0; g < GS; ++g)
 #pragma unroll
             for (int i = 0; i < OCT; ++i) acc[g][i] = 0.f;
+        // C[k, j0..j0+7] streams from L2/L1: batches of 4 terms, the next batch in flight while this one
+        // is multiplied (two register buffers), so the L2 latency hides behind 128 FMAs
         const float4 *c4 = (const float4 *)(M.C + j0);
-#pragma unroll 4
-        for (int k = 0; k < M.K; ++k) {
-            const float4 ca = __ldg(c4 + (size_t)k * P4), cb = __ldg(c4 + (size_t)k * P4 + 1);
-            const float4 ph = phi4[k];
-            const float cc[OCT] = {ca.x, ca.y, ca.z, ca.w, cb.x, cb.y, cb.z, cb.w};
-            const float pg[GS] = {ph.x, ph.y, ph.z, ph.w};
+        const int K = M.K;
+        float4 bufA[8], bufB[8];
+        auto load4 = [&](int k0, float4 (&buf)[8]) {
 #pragma unroll
-            for (int g = 0; g < GS; ++g)
+            for (int u = 0; u < 4; ++u) {
+                const int k = min(k0 + u, K - 1);
+                buf[2 * u] = __ldg(c4 + (size_t)k * P4);
+                buf[2 * u + 1] = __ldg(c4 + (size_t)k * P4 + 1);
+            }
+        };
+        auto mul4 = [&](int k0, const float4 (&buf)[8]) {
 #pragma unroll
-                for (int i = 0; i < OCT; ++i) acc[g][i] = fmaf(pg[g], cc[i], acc[g][i]);
+            for (int u = 0; u < 4; ++u) {
+                if (k0 + u < K) {
+                    const float4 ph = phi4[k0 + u];
+                    const float4 ca = buf[2 * u], cb = buf[2 * u + 1];
+                    const float cc[OCT] = {ca.x, ca.y, ca.z, ca.w, cb.x, cb.y, cb.z, cb.w};
+                    const float pg[GS] = {ph.x, ph.y, ph.z, ph.w};
+#pragma unroll
+                    for (int g = 0; g < GS; ++g)
+#pragma unroll
+                        for (int i = 0; i < OCT; ++i) acc[g][i] = fmaf(pg[g], cc[i], acc[g][i]);
+                }
+            }
+        };
+        load4(0, bufA);
+        for (int k0 = 0; k0 < K; k0 += 8) {
+            load4(k0 + 4, bufB);
+            mul4(k0, bufA);
+            load4(k0 + 8, bufA);
+            mul4(k0 + 4, bufB);
         }
 #pragma unroll
         for (int g = 0; g < GS; ++g) {
@@ -271,8 +298,8 @@ __device__ void v1_phase_forward(const V1Ctx &c, const SegDev &sg, const V1Args 
 {
     const ModelDev &M = *c.M;
     const V1Lay &L = *c.L;
-    const int *tap = (const int *)(c.sm + L.oTAP);
-    float *red = c.sm + L.oRED + c.warp * L.VR * GS;
+    const int *tap = (const int *)(V1SM + L.oTAP);
+    float *red = V1SM + L.oRED + c.warp * L.VR * GS;
     bool first = true;
     for (int jb = sg.fit_lo; jb < sg.fit_hi; jb += c.nt * OCT, first = false) {   // uniform trip count
         const int j0 = jb + c.tid * OCT;
@@ -281,11 +308,17 @@ __device__ void v1_phase_forward(const V1Ctx &c, const SegDev &sg, const V1Args 
         if (act) {
 #pragma unroll
             for (int g = 0; g < GS; ++g) {
+                // flux / weight / c_prev rows come from L2: issue the loads first, the stencil hides them
+                const size_t ro = (size_t)c.spec[g] * M.Ppad + j0;
+                const float4 y0 = __ldg((const float4 *)(a.Y + ro)), y1 = __ldg((const float4 *)(a.Y + ro) + 1);
+                const float4 w0 = __ldg((const float4 *)(a.W + ro)), w1 = __ldg((const float4 *)(a.W + ro) + 1);
+                const float4 *cp4 = (const float4 *)(c.cp + (size_t)g * M.Ppad + j0);
+                const float4 c0 = __ldcg(cp4), c1 = __ldcg(cp4 + 1);
                 float S[1][OCT];
                 float4 *ra = (float4 *)(v1_row(c, L.oA, sg, g) + j0);
                 if (stencil) {
                     v1_stencil_octet<1>((const float4 *)v1_row(c, L.oT, sg, g), j0, tap[2 * g], tap[2 * g + 1],
-                                        (const float4 *)(c.sm + L.oGW + g * L.NA * 4), 0, S);
+                                        (const float4 *)(V1SM + L.oGW + g * L.NA * 4), 0, S);
                     ra[0] = make_float4(S[0][0], S[0][1], S[0][2], S[0][3]);
                     ra[1] = make_float4(S[0][4], S[0][5], S[0][6], S[0][7]);
                 } else {
@@ -293,11 +326,6 @@ __device__ void v1_phase_forward(const V1Ctx &c, const SegDev &sg, const V1Args 
                     S[0][0] = s0.x; S[0][1] = s0.y; S[0][2] = s0.z; S[0][3] = s0.w;
                     S[0][4] = s1.x; S[0][5] = s1.y; S[0][6] = s1.z; S[0][7] = s1.w;
                 }
-                const size_t ro = (size_t)c.spec[g] * M.Ppad + j0;
-                const float4 y0 = __ldg((const float4 *)(a.Y + ro)), y1 = __ldg((const float4 *)(a.Y + ro) + 1);
-                const float4 w0 = __ldg((const float4 *)(a.W + ro)), w1 = __ldg((const float4 *)(a.W + ro) + 1);
-                const float4 *cp4 = (const float4 *)(c.cp + (size_t)g * M.Ppad + j0);
-                const float4 c0 = cp4[0], c1 = cp4[1];
                 const float yy[OCT] = {y0.x, y0.y, y0.z, y0.w, y1.x, y1.y, y1.z, y1.w};
                 const float ww[OCT] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
                 const float cc[OCT] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w};
@@ -400,11 +428,11 @@ __device__ void v1_phase_solve(const V1Ctx &c, int g, int seg, bool refactor)
     const ModelDev &M = *c.M;
     const V1Lay &L = *c.L;
     const int n1 = M.n1, lane = c.lane, rowB = seg * M.n1;
-    float *momS = c.sm + L.oMOM + g * L.nmomr;
-    float *rhsS = c.sm + L.oRHS + g * L.n1r;
-    float *lf = c.sm + L.oLF + g * V1_LFS;
+    float *momS = V1SM + L.oMOM + g * L.nmomr;
+    float *rhsS = V1SM + L.oRHS + g * L.n1r;
+    float *lf = V1SM + L.oLF + g * V1_LFS;
     float *invd = lf + 32 * 33;
-    const float *red = c.sm + L.oRED;
+    const float *red = V1SM + L.oRED;
     const int wst = L.VR * GS;
     for (int n = lane; n < L.n1r; n += 32) {
         float s = 0.f;
@@ -487,12 +515,21 @@ __device__ void v1_phase_residual(const V1Ctx &c, const SegDev &sg, const V1Args
 {
     const ModelDev &M = *c.M;
     const V1Lay &L = *c.L;
-    const float4 *b4 = (const float4 *)(c.sm + L.oB) + rowB;
+    const float4 *b4 = (const float4 *)(V1SM + L.oB) + rowB;
     float chi[GS], ng[GS], cmin[GS];
 #pragma unroll
     for (int g = 0; g < GS; ++g) { chi[g] = 0.f; ng[g] = 0.f; cmin[g] = 3.0e38f; }
     for (int j0 = sg.fit_lo + c.tid * OCT; j0 < sg.fit_hi; j0 += c.nt * OCT) {
         float cc[GS][OCT], pp[OCT], pc[OCT], x2[OCT];
+        float4 yq[GS][2], wq[GS][2];   // flux / weight from L2, issued before the basis loop hides them
+        if (MODE != 0) {
+#pragma unroll
+            for (int g = 0; g < GS; ++g) {
+                const size_t ro = (size_t)c.spec[g] * M.Ppad + j0;
+                yq[g][0] = __ldg((const float4 *)(a.Y + ro)); yq[g][1] = __ldg((const float4 *)(a.Y + ro) + 1);
+                wq[g][0] = __ldg((const float4 *)(a.W + ro)); wq[g][1] = __ldg((const float4 *)(a.W + ro) + 1);
+            }
+        }
 #pragma unroll
         for (int i = 0; i < OCT; ++i) {
             const float t = fmaf(sg.ta, (float)(j0 + i - sg.po - sg.halo), sg.tb);
@@ -520,9 +557,7 @@ __device__ void v1_phase_residual(const V1Ctx &c, const SegDev &sg, const V1Args
             if (MODE == 0) continue;
             float4 *ra = (float4 *)(v1_row(c, L.oA, sg, g) + j0);
             const float4 s0 = ra[0], s1 = ra[1];
-            const size_t ro = (size_t)c.spec[g] * M.Ppad + j0;
-            const float4 y0 = __ldg((const float4 *)(a.Y + ro)), y1 = __ldg((const float4 *)(a.Y + ro) + 1);
-            const float4 w0 = __ldg((const float4 *)(a.W + ro)), w1 = __ldg((const float4 *)(a.W + ro) + 1);
+            const float4 y0 = yq[g][0], y1 = yq[g][1], w0 = wq[g][0], w1 = wq[g][1];
             const float SS[OCT] = {s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w};
             const float yy[OCT] = {y0.x, y0.y, y0.z, y0.w, y1.x, y1.y, y1.z, y1.w};
             const float ww[OCT] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
@@ -546,7 +581,7 @@ __device__ void v1_phase_residual(const V1Ctx &c, const SegDev &sg, const V1Args
         }
     }
     if (MODE != 0) {
-        float *red = c.sm + L.oRED + c.warp * L.VR * GS;
+        float *red = V1SM + L.oRED + c.warp * L.VR * GS;
 #pragma unroll
         for (int g = 0; g < GS; ++g) {
             const float s = warp_sum_f(chi[g]), n = warp_sum_f(ng[g]), m = warp_min_f(cmin[g]);
@@ -570,8 +605,8 @@ __device__ void v1_phase_adjoint(const V1Ctx &c, const SegDev &sg, int lo, int h
 {
     const ModelDev &M = *c.M;
     const V1Lay &L = *c.L;
-    const int *tap = (const int *)(c.sm + L.oTAP);
-    float *red = c.sm + L.oRED + c.warp * L.VR * GS;
+    const int *tap = (const int *)(V1SM + L.oTAP);
+    float *red = V1SM + L.oRED + c.warp * L.VR * GS;
     const int P4 = M.Ppad >> 2;
     const int wstride4 = GS * L.NA;   // float4 stride between the three reversed kernels
     const int K2 = M.K + 2;
@@ -585,7 +620,7 @@ __device__ void v1_phase_adjoint(const V1Ctx &c, const SegDev &sg, int lo, int h
             if (act) {
                 float acc[3][OCT];
                 v1_stencil_octet<3>((const float4 *)v1_row(c, L.oA, sg, g), j0, tap[2 * g], tap[2 * g + 1],
-                                    (const float4 *)(c.sm + L.oGR + g * L.NA * 4), wstride4, acc);
+                                    (const float4 *)(V1SM + L.oGR + g * L.NA * 4), wstride4, acc);
                 const float4 *rt = (const float4 *)(v1_row(c, L.oT, sg, g) + j0);
                 const float4 t0 = rt[0], t1 = rt[1];
                 const float TT[OCT] = {t0.x, t0.y, t0.z, t0.w, t1.x, t1.y, t1.z, t1.w};
@@ -600,27 +635,41 @@ __device__ void v1_phase_adjoint(const V1Ctx &c, const SegDev &sg, int lo, int h
                 for (int i = 0; i < OCT; ++i) t[g][i] = 0.f;
             }
         }
+        // C[k, octet] from L2/L1 in batches of 4 terms, the next batch in flight during the multiplies
         const float4 *c4 = (const float4 *)(M.C + (act ? j0 : lo));
+        const int K = M.K;
+        float4 bufA[8], bufB[8];
+        auto load4 = [&](int kb, float4 (&buf)[8]) {
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int k = min(kb + u, K - 1);
+                buf[2 * u] = __ldg(c4 + (size_t)k * P4);
+                buf[2 * u + 1] = __ldg(c4 + (size_t)k * P4 + 1);
+            }
+        };
+        load4(0, bufA);
         for (int k0 = 0; k0 < K2; k0 += 8) {
             float X[32];
+            auto dot4 = [&](int kb, int xo, const float4 (&buf)[8]) {
 #pragma unroll
-            for (int kk = 0; kk < 8; ++kk) {
-                const int k = k0 + kk;
-                if (k < M.K) {
-                    const float4 ca = __ldg(c4 + (size_t)k * P4), cb = __ldg(c4 + (size_t)k * P4 + 1);
+                for (int u = 0; u < 4; ++u) {
+                    const int k = kb + u;
+                    const float4 ca = buf[2 * u], cb = buf[2 * u + 1];
                     const float cc[OCT] = {ca.x, ca.y, ca.z, ca.w, cb.x, cb.y, cb.z, cb.w};
 #pragma unroll
                     for (int g = 0; g < GS; ++g) {
-                        float s = 0.f;
+                        float sacc = 0.f;
 #pragma unroll
-                        for (int i = 0; i < OCT; ++i) s = fmaf(t[g][i], cc[i], s);
-                        X[kk * 4 + g] = s;
+                        for (int i = 0; i < OCT; ++i) sacc = fmaf(t[g][i], cc[i], sacc);
+                        // pseudo-terms K and K+1 carry the kernel-parameter gradients
+                        X[xo + u * 4 + g] = k < K ? sacc : (k == K ? gv[g] : (k == K + 1 ? gs[g] : 0.f));
                     }
-                } else {
-#pragma unroll
-                    for (int g = 0; g < GS; ++g) X[kk * 4 + g] = (k == M.K) ? gv[g] : (k == M.K + 1 ? gs[g] : 0.f);
                 }
-            }
+            };
+            load4(k0 + 4, bufB);
+            dot4(k0, 0, bufA);
+            load4(k0 + 8, bufA);
+            dot4(k0 + 4, 16, bufB);
             const float tot = xreduce32(X, c.lane);
             const int slot = SLOT_Q(L, k0 + (c.lane >> 2));
             red[slot * GS + (c.lane & 3)] += tot;
@@ -647,7 +696,7 @@ __device__ void v1_evaluate(const V1Ctx &c, const V1Args &a, bool cold, bool mom
     // evaluation's slots (v1_gradient / v1_stats run between evaluations without a barrier).
     bool zeroed = false;
     auto zero_slots = [&]() {
-        float *red = c.sm + L.oRED + c.warp * L.VR * GS;
+        float *red = V1SM + L.oRED + c.warp * L.VR * GS;
         const int q0 = (L.nmomr + L.n1r) * GS;
         for (int i = q0 + c.lane; i < L.VR * GS; i += 32) red[i] = 0.f;
         __syncwarp();
@@ -671,7 +720,7 @@ __device__ void v1_evaluate(const V1Ctx &c, const V1Args &a, bool cold, bool mom
         }
         if (M.n_seg > 1 || cold) {
             // row A must be zero outside the fitted range of THIS segment (the adjoint stencil reads it)
-            for (int i = c.tid; i < GS * L.RL / 4; i += c.nt) ((float4 *)(c.sm + L.oA))[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+            for (int i = c.tid; i < GS * L.RL / 4; i += c.nt) ((float4 *)(V1SM + L.oA))[i] = make_float4(0.f, 0.f, 0.f, 0.f);
         }
         if (cold) {
             for (int g = 0; g < GS; ++g)
@@ -714,7 +763,7 @@ __device__ void v1_evaluate(const V1Ctx &c, const V1Args &a, bool cold, bool mom
 __device__ __forceinline__ void v1_stats(const V1Ctx &c, int g, float &chi2, float &ngood, float &cmin)
 {
     const V1Lay &L = *c.L;
-    const float *red = c.sm + L.oRED + SLOT_STAT(L) * GS + g;
+    const float *red = V1SM + L.oRED + SLOT_STAT(L) * GS + g;
     chi2 = 0.f; ngood = 0.f; cmin = 3.0e38f;
     for (int w = 0; w < L.NW; ++w) {
         const float *r = red + w * L.VR * GS;
@@ -727,7 +776,7 @@ __device__ float v1_gradient(const V1Ctx &c, int g)
 {
     const ModelDev &M = *c.M;
     const V1Lay &L = *c.L;
-    const float *red = c.sm + L.oRED;
+    const float *red = V1SM + L.oRED;
     const int wst = L.VR * GS;
     for (int k = c.lane; k < M.K + 2; k += 32) {
         float s = 0.f;
@@ -775,9 +824,9 @@ __device__ void v1_write_cont(const V1Ctx &c, int g, float *out)
     }
 }
 
-__device__ __forceinline__ void v1_make_ctx(V1Ctx &c, const ModelDev &M, const V1Lay &L, float *sm, const V1Args &a)
+__device__ __forceinline__ void v1_make_ctx(V1Ctx &c, const ModelDev &M, const V1Lay &L, const V1Args &a)
 {
-    c.M = &M; c.L = &L; c.sm = sm;
+    c.M = &M; c.L = &L;
     c.tid = threadIdx.x; c.lane = threadIdx.x & 31; c.warp = threadIdx.x >> 5; c.nt = blockDim.x;
     c.cp = a.CP + (size_t)blockIdx.x * GS * M.Ppad;
 }
@@ -840,7 +889,7 @@ __device__ void v1_errors(V1Ctx &c, const V1Args &a, float chi2_g, float ngood_g
         __syncthreads();
     }
     // N = J^T J (packed lower), fp64 accumulation across warps in shared memory (aliases the factor area)
-    double *N = (double *)(c.sm + L.oLF);
+    double *N = (double *)(V1SM + L.oLF);
     const int npair = NP * (NP + 1) / 2;
     for (int i = c.tid; i < GS * npair; i += c.nt) N[i] = 0.0;
     __syncthreads();
@@ -918,9 +967,8 @@ template <int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB)
 lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V1Lay L, const V1Args a)
 {
-    extern __shared__ float4 v1_smem4[];
     V1Ctx c;
-    v1_make_ctx(c, M, L, (float *)v1_smem4, a);
+    v1_make_ctx(c, M, L, a);
     const int NP = M.NP, g = c.warp;
     for (int grp = blockIdx.x; grp < a.ngroups; grp += gridDim.x) {
         v1_set_group(c, a, grp);
@@ -976,7 +1024,7 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
             for (int n = c.lane; n < M.nc; n += 32) fin = fin && isfinite(SMV(c, L.oB, n, g));
             fin = __all_sync(FULL, fin);
             bound = __any_sync(FULL, bound);
-            const bool anyfail = __any_sync(FULL, c.lane < M.n_seg && c.sm[L.oSC + (SC_N + c.lane) * GS + g] != 0.f);
+            const bool anyfail = __any_sync(FULL, c.lane < M.n_seg && V1SM[L.oSC + (SC_N + c.lane) * GS + g] != 0.f);
             if (anyfail) st |= LASP_ST_NOT_SPD;
             if (bound) st |= LASP_ST_ON_BOUND;
             if (!fin) st |= LASP_ST_NONFINITE;
@@ -1003,9 +1051,8 @@ template <int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB)
 lasp_v1_grad_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V1Lay L, const V1Args a)
 {
-    extern __shared__ float4 v1_smem4[];
     V1Ctx c;
-    v1_make_ctx(c, M, L, (float *)v1_smem4, a);
+    v1_make_ctx(c, M, L, a);
     const int NP = M.NP, g = c.warp;
     for (int grp = blockIdx.x; grp < a.ngroups; grp += gridDim.x) {
         v1_set_group(c, a, grp);
@@ -1022,7 +1069,7 @@ lasp_v1_grad_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ 
             const float gr = v1_gradient(c, g);
             float chi2, ngood, cmin;
             v1_stats(c, g, chi2, ngood, cmin);
-            const bool anyfail = __any_sync(FULL, c.lane < M.n_seg && c.sm[L.oSC + (SC_N + c.lane) * GS + g] != 0.f);
+            const bool anyfail = __any_sync(FULL, c.lane < M.n_seg && V1SM[L.oSC + (SC_N + c.lane) * GS + g] != 0.f);
             if (valid) {
                 const long long i = c.spec[g];
                 if (c.lane < NP) a.grad_u[i * NP + c.lane] = gr;

@@ -86,6 +86,8 @@ extern "C" int lasp_version(void) { return LASP_VERSION; }
 
 extern "C" const char *lasp_last_error(const lasp_ctx *ctx) { return ctx ? ctx->err.c_str() : g_err.c_str(); }
 
+extern "C" int lasp_kernel_variant(const lasp_ctx *ctx) { return ctx && ctx->v1_ok ? 1 : 0; }
+
 extern "C" int64_t lasp_launch_count(const lasp_ctx *ctx) { return ctx ? ctx->launches : 0; }
 
 extern "C" int lasp_destroy(lasp_ctx *c)
@@ -100,6 +102,7 @@ extern "C" int lasp_destroy(lasp_ctx *c)
 }
 
 static int setup_v1(lasp_ctx *c, const cudaDeviceProp &prop);
+static int v1_workspace(lasp_ctx *c, int64_t B, bool need_xj);
 
 extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx **out)
 {
@@ -299,7 +302,7 @@ static int setup_v1(lasp_ctx *c, const cudaDeviceProp &prop)
     L.nmomr = L.n1r + roundup(std::max(M.nmom - L.n1r, 0), 8);
     L.VR = L.nmomr + L.n1r + roundup(M.K + 2, 8) + 4;
     const char *rf = getenv("LASP_REFRESH");
-    L.refresh = rf ? std::max(1, atoi(rf)) : 1;
+    L.refresh = rf ? std::max(1, atoi(rf)) : 8;
     int o = 0;
     auto take = [&](int n) { int r = o; o += roundup(n, 4); return r; };
     L.oT = take(GS * L.RL); L.oA = take(GS * L.RL);
@@ -363,6 +366,7 @@ static int ensure_workspace(lasp_ctx *c, int64_t B, bool need_yw)
 extern "C" int lasp_reserve(lasp_ctx *c, int64_t B)
 {
     if (!c || B < 1) return fail(c, LASP_ERR_INVALID_ARG, "lasp_reserve: bad argument");
+    if (c->v1_ok) return v1_workspace(c, B, true);
     return ensure_workspace(c, B, true);
 }
 
