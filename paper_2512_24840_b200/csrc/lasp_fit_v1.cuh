@@ -32,7 +32,7 @@ struct V1Lay {
     int Hm;                 // support clamp (memory safety outside the prior box)
     int refresh;            // re-accumulate the Gram moments and re-factor every `refresh` steps
     // shared-memory offsets (floats)
-    int oT, oA, oU, oM, oV, oX, oPHI, oGW, oGR, oTAP, oMOM, oRHS, oB, oRED, oLF, oQ, oSC, total;
+    int oT, oA, oU, oM, oV, oX, oPHI, oGW, oGR, oTAP, oMOM, oRHS, oB, oRED, oLF, oQ, oSC, oEXP, total;
 };
 
 struct V1Args {
@@ -48,6 +48,7 @@ struct V1Args {
     int *status;
     const float *gparams;  // lasp_eval_grad
     float *grad_u;
+    unsigned long long *dbg;   // optional per-phase cycle counters (LASP_TIMING=1), else null
 };
 
 // slots of the per-warp reduction area (each slot holds GS floats)
@@ -95,7 +96,7 @@ struct V1Ctx {
 // ------------------------------------------------------------------------------------------
 // a1: de-normalise, emulator inputs, monomials (Eq. 1, C.2-18/19).  Warp g, spectrum g.
 // ------------------------------------------------------------------------------------------
-__device__ void v1_param_setup(const V1Ctx &c, int g)
+__device__ __noinline__ void v1_param_setup(const V1Ctx &c, int g)
 {
     const ModelDev &M = *c.M;
     const V1Lay &L = *c.L;
@@ -109,7 +110,7 @@ __device__ void v1_param_setup(const V1Ctx &c, int g)
     for (int k = c.lane; k < M.K; k += 32) {
         float p = 1.f;
         for (int l = 0; l < M.L; ++l) {
-            int e = M.exps[k * M.L + l];
+            int e = ((const uint8_t *)(V1SM + L.oEXP))[k * M.L + l];
             float x = SMV(c, L.oX, l, g);
             for (int q = 0; q < e; ++q) p *= x;
         }
@@ -125,7 +126,7 @@ __device__ void v1_param_setup(const V1Ctx &c, int g)
 //   GR [j][g][a][4]    reversed kernels for the adjoint pass: j=0: g_{-k}; j=1: d g_{-k}/dv;
 //                      j=2: d g_{-k}/d sigma* (chain factors of C.1 folded in)
 // ------------------------------------------------------------------------------------------
-__device__ void v1_setup_weights(const V1Ctx &c, const SegDev &sg, int g)
+__device__ __noinline__ void v1_setup_weights(const V1Ctx &c, const SegDev &sg, int g)
 {
     const V1Lay &L = *c.L;
     const float v = SMV(c, L.oSC, SC_V, g), sigstar = SMV(c, L.oSC, SC_SIG, g);
@@ -212,23 +213,27 @@ __device__ __forceinline__ float *v1_row(const V1Ctx &c, int off, const SegDev &
     return V1SM + off + g * c.L->RL + c.L->GUARD - sg.po;
 }
 
-// largest support of the group (for the T range), from the tap tables
-__device__ __forceinline__ int v1_group_reach(const V1Ctx &c)
+// padded pixel range [lo,hi) on which T is needed by the forward stencils of the group's fitted octets
+// (group a reads row[j0-4a .. j0-4a+11]); the adjoint pass runs on the same range.  Kept tight: config 1
+// has 188 fitted octets and 192 threads, so 16 pixels of reach on each side still fit one sweep.
+__device__ __forceinline__ void v1_group_range(const V1Ctx &c, const SegDev &sg, int &lo, int &hi)
 {
     const int *tap = (const int *)(V1SM + c.L->oTAP);
-    int r = 0;
+    int rl = 0, rh = 0;
 #pragma unroll
     for (int g = 0; g < GS; ++g) {
-        int a_lo = tap[2 * g], na = tap[2 * g + 1];
-        r = max(r, max(-4 * a_lo + 3, 4 * (a_lo + na - 1)));   // |k| reach of the padded tap groups
+        const int a_lo = tap[2 * g], na = tap[2 * g + 1];
+        rl = max(rl, 4 * (a_lo + na - 1));
+        rh = max(rh, -4 * a_lo + 4);
     }
-    return (r + OCT + OCT - 1) / OCT * OCT;   // window reads up to 8 pixels past the last tap
+    lo = sg.fit_lo - (rl + OCT - 1) / OCT * OCT;
+    hi = sg.fit_hi + (rh + OCT - 1) / OCT * OCT;
 }
 
 // ------------------------------------------------------------------------------------------
 // a2: T_j = sum_k phi_k C[k,j] over the padded range [lo,hi) -> shared row T (Eq. 1)
 // ------------------------------------------------------------------------------------------
-__device__ void v1_phase_emulator(const V1Ctx &c, const SegDev &sg, int lo, int hi)
+__device__ __noinline__ void v1_phase_emulator(const V1Ctx &c, const SegDev &sg, int lo, int hi)
 {
     const ModelDev &M = *c.M;
     const V1Lay &L = *c.L;
@@ -244,11 +249,12 @@ __device__ void v1_phase_emulator(const V1Ctx &c, const SegDev &sg, int lo, int 
         // is multiplied (two register buffers), so the L2 latency hides behind 128 FMAs
         const float4 *c4 = (const float4 *)(M.C + j0);
         const int K = M.K;
+        const bool dbgc0 = L.Hm == -1;   // experiment: every term reads row 0 (L1-resident)
         float4 bufA[8], bufB[8];
         auto load4 = [&](int k0, float4 (&buf)[8]) {
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                const int k = min(k0 + u, K - 1);
+                const int k = dbgc0 ? 0 : min(k0 + u, K - 1);
                 buf[2 * u] = __ldg(c4 + (size_t)k * P4);
                 buf[2 * u + 1] = __ldg(c4 + (size_t)k * P4 + 1);
             }
@@ -294,7 +300,7 @@ __device__ void v1_phase_emulator(const V1Ctx &c, const SegDev &sg, int lo, int 
 // Partial sums over the thread's 8 pixels are reduced over the warp by register transposes and
 // land in this warp's reduction slots.
 // ------------------------------------------------------------------------------------------
-__device__ void v1_phase_forward(const V1Ctx &c, const SegDev &sg, const V1Args &a, bool stencil, bool mom)
+__device__ __noinline__ void v1_phase_forward(const V1Ctx &c, const SegDev &sg, const V1Args &a, bool stencil, bool mom)
 {
     const ModelDev &M = *c.M;
     const V1Lay &L = *c.L;
@@ -419,11 +425,11 @@ __device__ void v1_phase_forward(const V1Ctx &c, const SegDev &sg, const V1Args 
 // refinement whose residual was formed from the pixel data).  With
 // `refactor` false the Cholesky factor kept in shared memory from an earlier step is reused
 // (the refinement's fixed point does not depend on it).
-// Factor layout: LF[row*33 + col], then 32 reciprocal diagonals.
+// LF[row*33 + col] holds the unit-diagonal factor Lt = L D^-1, then the 32 values 1/d^2.
 // ------------------------------------------------------------------------------------------
 #define V1_LFS (32 * 33 + 32)
 
-__device__ void v1_phase_solve(const V1Ctx &c, int g, int seg, bool refactor)
+__device__ __noinline__ void v1_phase_solve(const V1Ctx &c, int g, int seg, bool refactor)
 {
     const ModelDev &M = *c.M;
     const V1Lay &L = *c.L;
@@ -480,21 +486,32 @@ __device__ void v1_phase_solve(const V1Ctx &c, int g, int seg, bool refactor)
         __syncwarp();
         invd[lane] = 1.f / lf[lane * 33 + lane];
         if (lane == 0) SMV(c, L.oSC, SC_N + seg, g) = ok ? 0.f : 1.f;
+        __syncwarp();
+        // store the factor column-scaled to unit diagonal, Lt = L D^-1 (D = diag L): the two triangular
+        // solves of every step then have a shuffle + one FMA on their serial chain and no division;
+        // invd keeps 1/d^2 for the diagonal scaling between them:  A^-1 = Lt^-T D^-2 Lt^-1
+        {
+            const float mine = invd[lane];
+            float dj[32];
+#pragma unroll
+            for (int j = 0; j < 32; ++j) dj[j] = invd[j];
+            __syncwarp();
+#pragma unroll
+            for (int j = 0; j < 32; ++j) lf[lane * 33 + j] *= dj[j];
+            invd[lane] = mine * mine;
+        }
     }
     __syncwarp();
     const bool ok = SMV(c, L.oSC, SC_N + seg, g) == 0.f;
     float r = (lane < n1) ? rhsS[lane] : 0.f;
-    for (int k = 0; k < n1; ++k) {            // L y = rhs
-        const float yk = __shfl_sync(FULL, r, k) * invd[k];
-        const float l = lf[lane * 33 + k];
-        if (lane == k) r = yk;
-        else if (lane > k) r = fmaf(-l, yk, r);
+    for (int k = 0; k < n1; ++k) {            // Lt z = rhs (unit diagonal)
+        const float zk = __shfl_sync(FULL, r, k);
+        if (lane > k) r = fmaf(-lf[lane * 33 + k], zk, r);
     }
-    for (int k = n1 - 1; k >= 0; --k) {       // L^T x = y
-        const float xk = __shfl_sync(FULL, r, k) * invd[k];
-        const float l = lf[k * 33 + lane];
-        if (lane == k) r = xk;
-        else if (lane < k) r = fmaf(-l, xk, r);
+    r *= invd[lane];                          // D^-2
+    for (int k = n1 - 1; k >= 0; --k) {       // Lt^T x = D^-2 z
+        const float xk = __shfl_sync(FULL, r, k);
+        if (lane < k) r = fmaf(-lf[k * 33 + lane], xk, r);
     }
     if (lane < n1) {
         if (ok) SMV(c, L.oB, rowB + lane, g) += r;
@@ -511,7 +528,7 @@ __device__ void v1_phase_solve(const V1Ctx &c, int g, int seg, bool refactor)
 // chi2 / ngood / cmin are reduced over the warp and accumulated in this warp's SLOT_STAT slots (zeroed by v1_evaluate).
 // ------------------------------------------------------------------------------------------
 template <int MODE>
-__device__ void v1_phase_residual(const V1Ctx &c, const SegDev &sg, const V1Args &a, int rowB, float *xrow)
+__device__ __noinline__ void v1_phase_residual(const V1Ctx &c, const SegDev &sg, const V1Args &a, int rowB, float *xrow)
 {
     const ModelDev &M = *c.M;
     const V1Lay &L = *c.L;
@@ -601,7 +618,7 @@ __device__ void v1_phase_residual(const V1Ctx &c, const SegDev &sg, const V1Args
 // Partial sums go through register transposes into this warp's Q slots (pseudo-terms K, K+1 carry
 // the two kernel-parameter gradients), which v1_evaluate zeroed.
 // ------------------------------------------------------------------------------------------
-__device__ void v1_phase_adjoint(const V1Ctx &c, const SegDev &sg, int lo, int hi)
+__device__ __noinline__ void v1_phase_adjoint(const V1Ctx &c, const SegDev &sg, int lo, int hi)
 {
     const ModelDev &M = *c.M;
     const V1Lay &L = *c.L;
@@ -638,11 +655,12 @@ __device__ void v1_phase_adjoint(const V1Ctx &c, const SegDev &sg, int lo, int h
         // C[k, octet] from L2/L1 in batches of 4 terms, the next batch in flight during the multiplies
         const float4 *c4 = (const float4 *)(M.C + (act ? j0 : lo));
         const int K = M.K;
+        const bool dbgc0 = L.Hm == -1;   // experiment: every term reads row 0 (L1-resident)
         float4 bufA[8], bufB[8];
         auto load4 = [&](int kb, float4 (&buf)[8]) {
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                const int k = min(kb + u, K - 1);
+                const int k = dbgc0 ? 0 : min(kb + u, K - 1);
                 buf[2 * u] = __ldg(c4 + (size_t)k * P4);
                 buf[2 * u + 1] = __ldg(c4 + (size_t)k * P4 + 1);
             }
@@ -687,13 +705,17 @@ __device__ void v1_phase_adjoint(const V1Ctx &c, const SegDev &sg, int lo, int h
 // for MODE 0, the q / dv / dsigma partials.
 // ------------------------------------------------------------------------------------------
 template <int MODE>
-__device__ void v1_evaluate(const V1Ctx &c, const V1Args &a, bool cold, bool mom, float *xrow)
+__device__ __noinline__ void v1_evaluate(const V1Ctx &c, const V1Args &a, bool cold, bool mom, float *xrow)
 {
     const ModelDev &M = *c.M;
     const V1Lay &L = *c.L;
     // This warp's Q and statistics slots accumulate over sweeps and segments.  They are zeroed after
     // the first barrier of the evaluation: only then have warps g < GS finished reading the previous
     // evaluation's slots (v1_gradient / v1_stats run between evaluations without a barrier).
+    long long tk = a.dbg ? clock64() : 0;
+    auto tick = [&](int i) {
+        if (a.dbg && c.tid == 0) { const long long t = clock64(); atomicAdd(a.dbg + i, (unsigned long long)(t - tk)); tk = t; }
+    };
     bool zeroed = false;
     auto zero_slots = [&]() {
         float *red = V1SM + L.oRED + c.warp * L.VR * GS;
@@ -727,16 +749,24 @@ __device__ void v1_evaluate(const V1Ctx &c, const V1Args &a, bool cold, bool mom
                 for (int j = sg.fit_lo + c.tid * 4; j < sg.fit_hi; j += c.nt * 4)
                     *(float4 *)(c.cp + (size_t)g * M.Ppad + j) = make_float4(0.f, 0.f, 0.f, 0.f);
         }
+        tick(0);
         __syncthreads();
+        tick(1);
         if (!zeroed) zero_slots();
-        const int reach = v1_group_reach(c);
-        const int lo = sg.fit_lo - reach, hi = sg.fit_hi + reach;
+        int lo, hi;
+        v1_group_range(c, sg, lo, hi);
         v1_phase_emulator(c, sg, lo, hi);
+        tick(2);
         __syncthreads();
+        tick(3);
         v1_phase_forward(c, sg, a, true, mom || cold);
+        tick(4);
         __syncthreads();
+        tick(5);
         if (c.warp < GS) v1_phase_solve(c, c.warp, s, mom || cold);
+        tick(6);
         __syncthreads();
+        tick(7);
         if (cold) {
             v1_phase_residual<0>(c, sg, a, rowB, nullptr);
             __syncthreads();   // c_prev written by this thread only, but keep phases aligned
@@ -746,10 +776,14 @@ __device__ void v1_evaluate(const V1Ctx &c, const V1Args &a, bool cold, bool mom
             __syncthreads();
         }
         v1_phase_residual<(MODE == 2 ? 2 : 1)>(c, sg, a, rowB, xrow);
+        tick(8);
         __syncthreads();
+        tick(9);
         if (MODE == 0) {
             v1_phase_adjoint(c, sg, lo, hi);
+            tick(10);
             __syncthreads();
+            tick(11);
         }
     }
     if (!zeroed) {   // no segment had a fitted pixel
@@ -772,7 +806,7 @@ __device__ __forceinline__ void v1_stats(const V1Ctx &c, int g, float &chi2, flo
 }
 
 // a7 (tail) + chain rule to u (C.1 last lines).  Warp g; grad[p] valid on lane p afterwards.
-__device__ float v1_gradient(const V1Ctx &c, int g)
+__device__ __noinline__ float v1_gradient(const V1Ctx &c, int g)
 {
     const ModelDev &M = *c.M;
     const V1Lay &L = *c.L;
@@ -785,14 +819,15 @@ __device__ float v1_gradient(const V1Ctx &c, int g)
     }
     __syncwarp();
     float mine = 0.f;
+    const uint8_t *ex = (const uint8_t *)(V1SM + L.oEXP);
     for (int l = 0; l < M.L; ++l) {
         float gx = 0.f;
         for (int k = c.lane; k < M.K; k += 32) {
-            const int el = M.exps[k * M.L + l];
+            const int el = ex[k * M.L + l];
             if (el == 0) continue;
             float d = (float)el;
             for (int l2 = 0; l2 < M.L; ++l2) {
-                const int e2 = M.exps[k * M.L + l2] - (l2 == l ? 1 : 0);
+                const int e2 = ex[k * M.L + l2] - (l2 == l ? 1 : 0);
                 const float x = SMV(c, L.oX, l2, g);
                 for (int q = 0; q < e2; ++q) d *= x;
             }
@@ -811,7 +846,7 @@ __device__ float v1_gradient(const V1Ctx &c, int g)
 }
 
 // internal Chebyshev(t) coefficients -> plain Legendre(x^) (C.2-8), fp64.  Warp g, lanes over rows.
-__device__ void v1_write_cont(const V1Ctx &c, int g, float *out)
+__device__ __noinline__ void v1_write_cont(const V1Ctx &c, int g, float *out)
 {
     const ModelDev &M = *c.M;
     for (int s = 0; s < M.n_seg; ++s) {
@@ -829,6 +864,8 @@ __device__ __forceinline__ void v1_make_ctx(V1Ctx &c, const ModelDev &M, const V
     c.M = &M; c.L = &L;
     c.tid = threadIdx.x; c.lane = threadIdx.x & 31; c.warp = threadIdx.x >> 5; c.nt = blockDim.x;
     c.cp = a.CP + (size_t)blockIdx.x * GS * M.Ppad;
+    for (int i = threadIdx.x; i < M.K * M.L; i += blockDim.x) ((uint8_t *)(V1SM + L.oEXP))[i] = M.exps[i];
+    __syncthreads();
 }
 
 __device__ __forceinline__ void v1_set_group(V1Ctx &c, const V1Args &a, int grp)
@@ -842,7 +879,7 @@ __device__ __forceinline__ void v1_set_group(V1Ctx &c, const V1Args &a, int grp)
 
 // a9: error estimate (C.2-22/23).  J by central differences of the re-solved whitened
 // residual rho(u), Sigma = rho^T rho/(N_good - NP) (J^T J)^-1, err_p = sqrt(Sigma_pp) (hi_p - lo_p)/2.
-__device__ void v1_errors(V1Ctx &c, const V1Args &a, float chi2_g, float ngood_g, bool valid_g)
+__device__ __noinline__ void v1_errors(V1Ctx &c, const V1Args &a, float chi2_g, float ngood_g, bool valid_g)
 {
     const ModelDev &M = *c.M;
     const V1Lay &L = *c.L;
@@ -987,7 +1024,10 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
         }
         float pb1 = 1.f, pb2 = 1.f;
         for (int t = 1; t <= a.n_iter; ++t) {
+            const long long te0 = a.dbg ? clock64() : 0;
             v1_evaluate<0>(c, a, t == 1, (t - 1) % L.refresh == 0, nullptr);
+            if (a.dbg && c.tid == 0) { atomicAdd(a.dbg + 14, (unsigned long long)(clock64() - te0)); atomicAdd(a.dbg + 15, 1ull); }
+            const long long tu0 = a.dbg ? clock64() : 0;
             pb1 *= a.b1; pb2 *= a.b2;
             if (g < GS) {
                 const float gr = v1_gradient(c, g);
@@ -1007,6 +1047,7 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
                 __syncwarp();
                 v1_param_setup(c, g);
             }
+            if (a.dbg && c.tid == 0) atomicAdd(a.dbg + 13, (unsigned long long)(clock64() - tu0));
         }
         // a9: one more evaluation at the final iterate (C.2-21)
         v1_evaluate<1>(c, a, a.n_iter == 0, true, nullptr);

@@ -36,6 +36,7 @@ struct lasp_ctx {
     float *dY = nullptr, *dW = nullptr;
     size_t plane_rows = 0;
     float *dCP = nullptr, *dXJ = nullptr;
+    unsigned long long *ddbg = nullptr;   // LASP_TIMING=1: per-phase cycle counters (debug aid)
     size_t cp_ctas = 0, xj_ctas = 0;
     std::string err;
 };
@@ -87,6 +88,13 @@ extern "C" int lasp_version(void) { return LASP_VERSION; }
 extern "C" const char *lasp_last_error(const lasp_ctx *ctx) { return ctx ? ctx->err.c_str() : g_err.c_str(); }
 
 extern "C" int lasp_kernel_variant(const lasp_ctx *ctx) { return ctx && ctx->v1_ok ? 1 : 0; }
+
+// debug aid (not part of the public header): per-phase cycle sums of the last v1 fit (thread 0 of every CTA)
+extern "C" int lasp_debug_phase_cycles(lasp_ctx *c, unsigned long long *out16)
+{
+    if (!c || !c->ddbg) return LASP_ERR_INVALID_ARG;
+    return cudaMemcpy(out16, c->ddbg, 16 * sizeof(unsigned long long), cudaMemcpyDeviceToHost) == cudaSuccess ? LASP_OK : LASP_ERR_CUDA;
+}
 
 extern "C" int64_t lasp_launch_count(const lasp_ctx *ctx) { return ctx ? ctx->launches : 0; }
 
@@ -296,7 +304,7 @@ static int setup_v1(lasp_ctx *c, const cudaDeviceProp &prop)
     L.NW = nt / 32;
     L.GUARD = guard;
     L.RL = maxlen + 2 * guard;
-    L.Hm = hmax;
+    L.Hm = getenv("LASP_DEBUG_C0") ? -1 : hmax;
     L.NA = (hmax + 3) / 4 + hmax / 4 + 2;
     L.n1r = roundup(M.n1, 8);
     L.nmomr = L.n1r + roundup(std::max(M.nmom - L.n1r, 0), 8);
@@ -314,6 +322,7 @@ static int setup_v1(lasp_ctx *c, const cudaDeviceProp &prop)
     const int npair = M.NP * (M.NP + 1) / 2;
     L.oLF = take(std::max(GS * V1_LFS, 2 * GS * npair + 4));
     L.oQ = take(GS * (M.K + 2)); L.oSC = take(GS * (SC_N + M.n_seg));
+    L.oEXP = take((M.K * M.L + 3) / 4);
     L.total = o;
     const size_t bytes = (size_t)o * sizeof(float);
     if (bytes > prop.sharedMemPerBlockOptin) return LASP_OK;   // does not fit: v0 handles it
@@ -489,6 +498,11 @@ extern "C" int lasp_fit_batch(lasp_ctx *c, int64_t B, const float *flux, const f
         a.init = init; a.n_iter = opts->n_iter; a.lr = opts->lr; a.b1 = opts->beta1; a.b2 = opts->beta2;
         a.eps = opts->eps; a.fd_h = 2e-3f;  // fp32 central-difference step in u (C.2-22)
         a.params = params; a.cont = cont; a.chi2 = chi2; a.err = err; a.status = status;
+        if (getenv("LASP_TIMING")) {
+            if (!c->ddbg) { CUDA_TRY(c, cudaMalloc(&c->ddbg, 16 * sizeof(unsigned long long))); }
+            CUDA_TRY(c, cudaMemsetAsync(c->ddbg, 0, 16 * sizeof(unsigned long long), st));
+            a.dbg = c->ddbg;
+        }
         return v1_launch(c, false, a, grid, st);
     }
     int rc = ensure_workspace(c, B, true);
