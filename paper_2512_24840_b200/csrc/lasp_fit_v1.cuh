@@ -27,6 +27,7 @@ extern __shared__ float4 v1_smem4[];
 struct V1Lay {
     int RL, GUARD;          // shared-memory row length and guard (floats); row index = jp - po + GUARD
     int NA;                 // largest number of 4-tap groups of a kernel
+    int Kq;                 // K+2 rounded to 8: rows of the zero-padded coefficient table the loops sweep
     int n1r, nmomr, VR;     // n1 rounded to 4; moments rounded; reduction slots per warp (x GS)
     int NW;                 // warps per CTA
     int Hm;                 // support clamp (memory safety outside the prior box)
@@ -235,55 +236,62 @@ __device__ __forceinline__ void v1_group_range(const V1Ctx &c, const SegDev &sg,
 // ------------------------------------------------------------------------------------------
 __device__ __noinline__ void v1_phase_emulator(const V1Ctx &c, const SegDev &sg, int lo, int hi)
 {
-    const ModelDev &M = *c.M;
-    const V1Lay &L = *c.L;
-    const float4 *phi4 = (const float4 *)(V1SM + L.oPHI);
-    const int P4 = M.Ppad >> 2;
-    for (int j0 = lo + c.tid * OCT; j0 < hi; j0 += c.nt * OCT) {
+    // everything the loop needs is copied to registers first: the model lives in shared memory, and after
+    // any shared-memory store the compiler would otherwise have to re-read it
+    const float4 *phi4 = (const float4 *)(V1SM + c.L->oPHI);
+    const int P4 = c.M->Ppad >> 2, Kq = c.L->Kq, nt8 = c.nt * OCT;
+    const float *Cg = c.M->C;
+    float *rowT = V1SM + c.L->oT + c.L->GUARD - sg.po;
+    const int RL = c.L->RL;
+    for (int j0 = lo + c.tid * OCT; j0 < hi; j0 += nt8) {
         float acc[GS][OCT];
 #pragma unroll
         for (int g = 0; g < GS; ++g)
 #pragma unroll
             for (int i = 0; i < OCT; ++i) acc[g][i] = 0.f;
-        // C[k, j0..j0+7] streams from L2/L1: batches of 4 terms, the next batch in flight while this one
-        // is multiplied (two register buffers), so the L2 latency hides behind 128 FMAs
-        const float4 *c4 = (const float4 *)(M.C + j0);
-        const int K = M.K;
-        const bool dbgc0 = L.Hm == -1;   // experiment: every term reads row 0 (L1-resident)
+        // C[k, j0..j0+7] streams from L2/L1 in batches of 4 terms, the next batch in flight while this one is
+        // multiplied (two register buffers).  The table has Kq = K+2 rounded to 8 rows plus 8 more, all zero
+        // past K (and phi is zero there), so the loop has no bounds tests.
+        const float4 *c4 = (const float4 *)(Cg + j0);
         float4 bufA[8], bufB[8];
         auto load4 = [&](int k0, float4 (&buf)[8]) {
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                const int k = dbgc0 ? 0 : min(k0 + u, K - 1);
-                buf[2 * u] = __ldg(c4 + (size_t)k * P4);
-                buf[2 * u + 1] = __ldg(c4 + (size_t)k * P4 + 1);
+                buf[2 * u] = __ldg(c4 + (k0 + u) * P4);
+                buf[2 * u + 1] = __ldg(c4 + (k0 + u) * P4 + 1);
             }
         };
         auto mul4 = [&](int k0, const float4 (&buf)[8]) {
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                if (k0 + u < K) {
-                    const float4 ph = phi4[k0 + u];
-                    const float4 ca = buf[2 * u], cb = buf[2 * u + 1];
-                    const float cc[OCT] = {ca.x, ca.y, ca.z, ca.w, cb.x, cb.y, cb.z, cb.w};
-                    const float pg[GS] = {ph.x, ph.y, ph.z, ph.w};
+                const float4 ph = phi4[k0 + u];
+                const float4 ca = buf[2 * u], cb = buf[2 * u + 1];
+                const float cc[OCT] = {ca.x, ca.y, ca.z, ca.w, cb.x, cb.y, cb.z, cb.w};
+                const float pg[GS] = {ph.x, ph.y, ph.z, ph.w};
 #pragma unroll
-                    for (int g = 0; g < GS; ++g)
+                for (int g = 0; g < GS; ++g)
 #pragma unroll
-                        for (int i = 0; i < OCT; ++i) acc[g][i] = fmaf(pg[g], cc[i], acc[g][i]);
-                }
+                    for (int i = 0; i < OCT; ++i) acc[g][i] = fmaf(pg[g], cc[i], acc[g][i]);
             }
         };
+        // three buffers: two batches (16 x 128-bit loads per thread) are in flight while one is multiplied --
+        // an L2 hit costs ~1000 cycles under this load, a batch of FMAs ~150
+        float4 bufC[8];
         load4(0, bufA);
-        for (int k0 = 0; k0 < K; k0 += 8) {
-            load4(k0 + 4, bufB);
+        load4(4, bufB);
+        for (int k0 = 0; k0 < Kq; k0 += 12) {
+            load4(k0 + 8, bufC);
             mul4(k0, bufA);
-            load4(k0 + 8, bufA);
+            if (k0 + 4 >= Kq) break;
+            load4(k0 + 12, bufA);
             mul4(k0 + 4, bufB);
+            if (k0 + 8 >= Kq) break;
+            load4(k0 + 16, bufB);
+            mul4(k0 + 8, bufC);
         }
 #pragma unroll
         for (int g = 0; g < GS; ++g) {
-            float4 *r = (float4 *)(v1_row(c, L.oT, sg, g) + j0);
+            float4 *r = (float4 *)(rowT + g * RL + j0);
             r[0] = make_float4(acc[g][0], acc[g][1], acc[g][2], acc[g][3]);
             r[1] = make_float4(acc[g][4], acc[g][5], acc[g][6], acc[g][7]);
         }
@@ -302,29 +310,40 @@ __device__ __noinline__ void v1_phase_emulator(const V1Ctx &c, const SegDev &sg,
 // ------------------------------------------------------------------------------------------
 __device__ __noinline__ void v1_phase_forward(const V1Ctx &c, const SegDev &sg, const V1Args &a, bool stencil, bool mom)
 {
-    const ModelDev &M = *c.M;
     const V1Lay &L = *c.L;
     const int *tap = (const int *)(V1SM + L.oTAP);
     float *red = V1SM + L.oRED + c.warp * L.VR * GS;
+    // hoisted to registers (the model sits in shared memory; see v1_phase_emulator)
+    const int Ppad = c.M->Ppad, RL = L.RL, NA = L.NA, n1r = L.n1r, nmomr = L.nmomr, nt8 = c.nt * OCT;
+    const int fit_lo = sg.fit_lo, fit_hi = sg.fit_hi, torg = sg.po + sg.halo;
+    const float ta = sg.ta, tb = sg.tb;
+    float *rowA = V1SM + L.oA + L.GUARD - sg.po;
+    const float *rowT = V1SM + L.oT + L.GUARD - sg.po;
+    const float4 *gw4 = (const float4 *)(V1SM + L.oGW);
+    const float *Yg = a.Y, *Wg = a.W;
+    const float *cpg = c.cp;
+    int alo[GS], nag[GS];
+    size_t rowo[GS];
+#pragma unroll
+    for (int g = 0; g < GS; ++g) { alo[g] = tap[2 * g]; nag[g] = tap[2 * g + 1]; rowo[g] = (size_t)c.spec[g] * Ppad; }
     bool first = true;
-    for (int jb = sg.fit_lo; jb < sg.fit_hi; jb += c.nt * OCT, first = false) {   // uniform trip count
+    for (int jb = fit_lo; jb < fit_hi; jb += nt8, first = false) {   // uniform trip count
         const int j0 = jb + c.tid * OCT;
-        const bool act = j0 < sg.fit_hi;
+        const bool act = j0 < fit_hi;
         float u[GS][OCT], v[GS][OCT];
         if (act) {
 #pragma unroll
             for (int g = 0; g < GS; ++g) {
                 // flux / weight / c_prev rows come from L2: issue the loads first, the stencil hides them
-                const size_t ro = (size_t)c.spec[g] * M.Ppad + j0;
-                const float4 y0 = __ldg((const float4 *)(a.Y + ro)), y1 = __ldg((const float4 *)(a.Y + ro) + 1);
-                const float4 w0 = __ldg((const float4 *)(a.W + ro)), w1 = __ldg((const float4 *)(a.W + ro) + 1);
-                const float4 *cp4 = (const float4 *)(c.cp + (size_t)g * M.Ppad + j0);
+                const size_t ro = rowo[g] + j0;
+                const float4 y0 = __ldg((const float4 *)(Yg + ro)), y1 = __ldg((const float4 *)(Yg + ro) + 1);
+                const float4 w0 = __ldg((const float4 *)(Wg + ro)), w1 = __ldg((const float4 *)(Wg + ro) + 1);
+                const float4 *cp4 = (const float4 *)(cpg + g * Ppad + j0);
                 const float4 c0 = __ldcg(cp4), c1 = __ldcg(cp4 + 1);
                 float S[1][OCT];
-                float4 *ra = (float4 *)(v1_row(c, L.oA, sg, g) + j0);
+                float4 *ra = (float4 *)(rowA + g * RL + j0);
                 if (stencil) {
-                    v1_stencil_octet<1>((const float4 *)v1_row(c, L.oT, sg, g), j0, tap[2 * g], tap[2 * g + 1],
-                                        (const float4 *)(V1SM + L.oGW + g * L.NA * 4), 0, S);
+                    v1_stencil_octet<1>((const float4 *)(rowT + g * RL), j0, alo[g], nag[g], gw4 + g * NA, 0, S);
                     ra[0] = make_float4(S[0][0], S[0][1], S[0][2], S[0][3]);
                     ra[1] = make_float4(S[0][4], S[0][5], S[0][6], S[0][7]);
                 } else {
@@ -352,12 +371,12 @@ __device__ __noinline__ void v1_phase_forward(const V1Ctx &c, const SegDev &sg, 
         float pp[OCT], pc[OCT], x2[OCT];
 #pragma unroll
         for (int i = 0; i < OCT; ++i) {
-            const float t = fmaf(sg.ta, (float)(j0 + i - sg.po - sg.halo), sg.tb);
+            const float t = fmaf(ta, (float)(j0 + i - torg), tb);
             pp[i] = t; pc[i] = 1.f; x2[i] = 2.f * t;
         }
         if (mom) {
             // region A: n < n1r, four n per transpose: value (nn, isrhs, g) at nn*8 + isrhs*4 + g
-            for (int n0 = 0; n0 < L.n1r; n0 += 4) {
+            for (int n0 = 0; n0 < n1r; n0 += 4) {
                 float X[32];
 #pragma unroll
                 for (int nn = 0; nn < 4; ++nn) {
@@ -373,11 +392,11 @@ __device__ __noinline__ void v1_phase_forward(const V1Ctx &c, const SegDev &sg, 
                 }
                 const float tot = xreduce32(X, c.lane);
                 const int n = n0 + (c.lane >> 3), g = c.lane & 3;
-                const int slot = (c.lane & 4) ? SLOT_RHS(L, n) : SLOT_MOM(L, n);
+                const int slot = (c.lane & 4) ? nmomr + n : n;
                 if (first) red[slot * GS + g] = tot; else red[slot * GS + g] += tot;
             }
             // region B: n1r <= n < nmomr, moments only, eight n per transpose: value (nn, g) at nn*4 + g
-            for (int n0 = L.n1r; n0 < L.nmomr; n0 += 8) {
+            for (int n0 = n1r; n0 < nmomr; n0 += 8) {
                 float X[32];
 #pragma unroll
                 for (int nn = 0; nn < 8; ++nn) {
@@ -392,12 +411,12 @@ __device__ __noinline__ void v1_phase_forward(const V1Ctx &c, const SegDev &sg, 
                     for (int i = 0; i < OCT; ++i) { const float nx = fmaf(x2[i], pc[i], -pp[i]); pp[i] = pc[i]; pc[i] = nx; }
                 }
                 const float tot = xreduce32(X, c.lane);
-                const int slot = SLOT_MOM(L, n0 + (c.lane >> 2));
+                const int slot = n0 + (c.lane >> 2);
                 if (first) red[slot * GS + (c.lane & 3)] = tot; else red[slot * GS + (c.lane & 3)] += tot;
             }
         } else {
             // right-hand side only, eight n per transpose
-            for (int n0 = 0; n0 < L.n1r; n0 += 8) {
+            for (int n0 = 0; n0 < n1r; n0 += 8) {
                 float X[32];
 #pragma unroll
                 for (int nn = 0; nn < 8; ++nn) {
@@ -412,7 +431,7 @@ __device__ __noinline__ void v1_phase_forward(const V1Ctx &c, const SegDev &sg, 
                     for (int i = 0; i < OCT; ++i) { const float nx = fmaf(x2[i], pc[i], -pp[i]); pp[i] = pc[i]; pc[i] = nx; }
                 }
                 const float tot = xreduce32(X, c.lane);
-                const int slot = SLOT_RHS(L, n0 + (c.lane >> 2));
+                const int slot = nmomr + n0 + (c.lane >> 2);
                 if (first) red[slot * GS + (c.lane & 3)] = tot; else red[slot * GS + (c.lane & 3)] += tot;
             }
         }
@@ -530,33 +549,41 @@ __device__ __noinline__ void v1_phase_solve(const V1Ctx &c, int g, int seg, bool
 template <int MODE>
 __device__ __noinline__ void v1_phase_residual(const V1Ctx &c, const SegDev &sg, const V1Args &a, int rowB, float *xrow)
 {
-    const ModelDev &M = *c.M;
     const V1Lay &L = *c.L;
     const float4 *b4 = (const float4 *)(V1SM + L.oB) + rowB;
+    const int Ppad = c.M->Ppad, n1 = c.M->n1, RL = L.RL, nt8 = c.nt * OCT;
+    const int fit_lo = sg.fit_lo, fit_hi = sg.fit_hi, torg = sg.po + sg.halo;
+    const float ta = sg.ta, tb = sg.tb;
+    float *rowA = V1SM + L.oA + L.GUARD - sg.po;
+    const float *Yg = a.Y, *Wg = a.W;
+    float *cpg = c.cp;
+    size_t rowo[GS];
+#pragma unroll
+    for (int g = 0; g < GS; ++g) rowo[g] = (size_t)c.spec[g] * Ppad;
     float chi[GS], ng[GS], cmin[GS];
 #pragma unroll
     for (int g = 0; g < GS; ++g) { chi[g] = 0.f; ng[g] = 0.f; cmin[g] = 3.0e38f; }
-    for (int j0 = sg.fit_lo + c.tid * OCT; j0 < sg.fit_hi; j0 += c.nt * OCT) {
+    for (int j0 = fit_lo + c.tid * OCT; j0 < fit_hi; j0 += nt8) {
         float cc[GS][OCT], pp[OCT], pc[OCT], x2[OCT];
         float4 yq[GS][2], wq[GS][2];   // flux / weight from L2, issued before the basis loop hides them
         if (MODE != 0) {
 #pragma unroll
             for (int g = 0; g < GS; ++g) {
-                const size_t ro = (size_t)c.spec[g] * M.Ppad + j0;
-                yq[g][0] = __ldg((const float4 *)(a.Y + ro)); yq[g][1] = __ldg((const float4 *)(a.Y + ro) + 1);
-                wq[g][0] = __ldg((const float4 *)(a.W + ro)); wq[g][1] = __ldg((const float4 *)(a.W + ro) + 1);
+                const size_t ro = rowo[g] + j0;
+                yq[g][0] = __ldg((const float4 *)(Yg + ro)); yq[g][1] = __ldg((const float4 *)(Yg + ro) + 1);
+                wq[g][0] = __ldg((const float4 *)(Wg + ro)); wq[g][1] = __ldg((const float4 *)(Wg + ro) + 1);
             }
         }
 #pragma unroll
         for (int i = 0; i < OCT; ++i) {
-            const float t = fmaf(sg.ta, (float)(j0 + i - sg.po - sg.halo), sg.tb);
+            const float t = fmaf(ta, (float)(j0 + i - torg), tb);
             pp[i] = t; pc[i] = 1.f; x2[i] = 2.f * t;
         }
 #pragma unroll
         for (int g = 0; g < GS; ++g)
 #pragma unroll
             for (int i = 0; i < OCT; ++i) cc[g][i] = 0.f;
-        for (int n = 0; n < M.n1; ++n) {
+        for (int n = 0; n < n1; ++n) {
             const float4 b = b4[n];
             const float bg[GS] = {b.x, b.y, b.z, b.w};
 #pragma unroll
@@ -568,11 +595,11 @@ __device__ __noinline__ void v1_phase_residual(const V1Ctx &c, const SegDev &sg,
         }
 #pragma unroll
         for (int g = 0; g < GS; ++g) {
-            float4 *cp4 = (float4 *)(c.cp + (size_t)g * M.Ppad + j0);
+            float4 *cp4 = (float4 *)(cpg + g * Ppad + j0);
             cp4[0] = make_float4(cc[g][0], cc[g][1], cc[g][2], cc[g][3]);
             cp4[1] = make_float4(cc[g][4], cc[g][5], cc[g][6], cc[g][7]);
             if (MODE == 0) continue;
-            float4 *ra = (float4 *)(v1_row(c, L.oA, sg, g) + j0);
+            float4 *ra = (float4 *)(rowA + g * RL + j0);
             const float4 s0 = ra[0], s1 = ra[1];
             const float4 y0 = yq[g][0], y1 = yq[g][1], w0 = wq[g][0], w1 = wq[g][1];
             const float SS[OCT] = {s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w};
@@ -591,7 +618,7 @@ __device__ __noinline__ void v1_phase_residual(const V1Ctx &c, const SegDev &sg,
             ra[0] = make_float4(av[0], av[1], av[2], av[3]);
             ra[1] = make_float4(av[4], av[5], av[6], av[7]);
             if (MODE == 2) {
-                float4 *x4 = (float4 *)(xrow + (size_t)g * M.Ppad + j0);
+                float4 *x4 = (float4 *)(xrow + g * Ppad + j0);
                 x4[0] = make_float4(rho[0], rho[1], rho[2], rho[3]);
                 x4[1] = make_float4(rho[4], rho[5], rho[6], rho[7]);
             }
@@ -620,14 +647,19 @@ __device__ __noinline__ void v1_phase_residual(const V1Ctx &c, const SegDev &sg,
 // ------------------------------------------------------------------------------------------
 __device__ __noinline__ void v1_phase_adjoint(const V1Ctx &c, const SegDev &sg, int lo, int hi)
 {
-    const ModelDev &M = *c.M;
     const V1Lay &L = *c.L;
     const int *tap = (const int *)(V1SM + L.oTAP);
+    const int P4 = c.M->Ppad >> 2, K = c.M->K, Kq = L.Kq, NA = L.NA, RL = L.RL, nt8 = c.nt * OCT;
+    const int wstride4 = GS * NA;   // float4 stride between the three reversed kernels
+    const int qslot0 = SLOT_Q(L, 0);
     float *red = V1SM + L.oRED + c.warp * L.VR * GS;
-    const int P4 = M.Ppad >> 2;
-    const int wstride4 = GS * L.NA;   // float4 stride between the three reversed kernels
-    const int K2 = M.K + 2;
-    for (int jb = lo; jb < hi; jb += c.nt * OCT) {
+    const float *Cg = c.M->C;
+    const float *rowA = V1SM + L.oA + L.GUARD - sg.po, *rowT = V1SM + L.oT + L.GUARD - sg.po;
+    const float4 *gr4 = (const float4 *)(V1SM + L.oGR);
+    int alo[GS], nag[GS];
+#pragma unroll
+    for (int g = 0; g < GS; ++g) { alo[g] = tap[2 * g]; nag[g] = tap[2 * g + 1]; }
+    for (int jb = lo; jb < hi; jb += nt8) {
         const int j0 = jb + c.tid * OCT;
         const bool act = j0 < hi;
         float t[GS][OCT], gv[GS], gs[GS];
@@ -636,9 +668,8 @@ __device__ __noinline__ void v1_phase_adjoint(const V1Ctx &c, const SegDev &sg, 
             gv[g] = 0.f; gs[g] = 0.f;
             if (act) {
                 float acc[3][OCT];
-                v1_stencil_octet<3>((const float4 *)v1_row(c, L.oA, sg, g), j0, tap[2 * g], tap[2 * g + 1],
-                                    (const float4 *)(V1SM + L.oGR + g * L.NA * 4), wstride4, acc);
-                const float4 *rt = (const float4 *)(v1_row(c, L.oT, sg, g) + j0);
+                v1_stencil_octet<3>((const float4 *)(rowA + g * RL), j0, alo[g], nag[g], gr4 + g * NA, wstride4, acc);
+                const float4 *rt = (const float4 *)(rowT + g * RL + j0);
                 const float4 t0 = rt[0], t1 = rt[1];
                 const float TT[OCT] = {t0.x, t0.y, t0.z, t0.w, t1.x, t1.y, t1.z, t1.w};
 #pragma unroll
@@ -652,26 +683,23 @@ __device__ __noinline__ void v1_phase_adjoint(const V1Ctx &c, const SegDev &sg, 
                 for (int i = 0; i < OCT; ++i) t[g][i] = 0.f;
             }
         }
-        // C[k, octet] from L2/L1 in batches of 4 terms, the next batch in flight during the multiplies
-        const float4 *c4 = (const float4 *)(M.C + (act ? j0 : lo));
-        const int K = M.K;
-        const bool dbgc0 = L.Hm == -1;   // experiment: every term reads row 0 (L1-resident)
+        // C[k, octet] in batches of 4 terms, the next batch in flight during the multiplies; the table is
+        // zero past K, so rows K and K+1 are free to carry the two kernel-parameter gradients
+        const float4 *c4 = (const float4 *)(Cg + (act ? j0 : lo));
         float4 bufA[8], bufB[8];
         auto load4 = [&](int kb, float4 (&buf)[8]) {
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                const int k = dbgc0 ? 0 : min(kb + u, K - 1);
-                buf[2 * u] = __ldg(c4 + (size_t)k * P4);
-                buf[2 * u + 1] = __ldg(c4 + (size_t)k * P4 + 1);
+                buf[2 * u] = __ldg(c4 + (kb + u) * P4);
+                buf[2 * u + 1] = __ldg(c4 + (kb + u) * P4 + 1);
             }
         };
         load4(0, bufA);
-        for (int k0 = 0; k0 < K2; k0 += 8) {
+        for (int k0 = 0; k0 < Kq; k0 += 8) {
             float X[32];
-            auto dot4 = [&](int kb, int xo, const float4 (&buf)[8]) {
+            auto dot4 = [&](int xo, const float4 (&buf)[8]) {
 #pragma unroll
                 for (int u = 0; u < 4; ++u) {
-                    const int k = kb + u;
                     const float4 ca = buf[2 * u], cb = buf[2 * u + 1];
                     const float cc[OCT] = {ca.x, ca.y, ca.z, ca.w, cb.x, cb.y, cb.z, cb.w};
 #pragma unroll
@@ -679,18 +707,22 @@ __device__ __noinline__ void v1_phase_adjoint(const V1Ctx &c, const SegDev &sg, 
                         float sacc = 0.f;
 #pragma unroll
                         for (int i = 0; i < OCT; ++i) sacc = fmaf(t[g][i], cc[i], sacc);
-                        // pseudo-terms K and K+1 carry the kernel-parameter gradients
-                        X[xo + u * 4 + g] = k < K ? sacc : (k == K ? gv[g] : (k == K + 1 ? gs[g] : 0.f));
+                        X[xo + u * 4 + g] = sacc;
                     }
                 }
             };
             load4(k0 + 4, bufB);
-            dot4(k0, 0, bufA);
+            dot4(0, bufA);
             load4(k0 + 8, bufA);
-            dot4(k0 + 4, 16, bufB);
+            dot4(16, bufB);
+            if (k0 + 8 > K) {   // uniform: the block holding rows K and K+1 (K+1 < Kq always)
+#pragma unroll
+                for (int kk = 0; kk < 8; ++kk)
+#pragma unroll
+                    for (int g = 0; g < GS; ++g) X[kk * 4 + g] += (k0 + kk == K) ? gv[g] : ((k0 + kk == K + 1) ? gs[g] : 0.f);
+            }
             const float tot = xreduce32(X, c.lane);
-            const int slot = SLOT_Q(L, k0 + (c.lane >> 2));
-            red[slot * GS + (c.lane & 3)] += tot;
+            red[(qslot0 + k0 + (c.lane >> 2)) * GS + (c.lane & 3)] += tot;
         }
     }
 }
@@ -861,10 +893,17 @@ __device__ __noinline__ void v1_write_cont(const V1Ctx &c, int g, float *out)
 
 __device__ __forceinline__ void v1_make_ctx(V1Ctx &c, const ModelDev &M, const V1Lay &L, const V1Args &a)
 {
-    c.M = &M; c.L = &L;
+    // the model description is read by every phase through pointers: keep a copy in shared memory (a pointer
+    // to the kernel parameters is a generic load from the parameter window with global-memory latency)
+    __shared__ ModelDev sM;
+    __shared__ V1Lay sL;
+    for (int i = threadIdx.x; i < (int)(sizeof(ModelDev) / 4); i += blockDim.x) ((int *)&sM)[i] = ((const int *)&M)[i];
+    for (int i = threadIdx.x; i < (int)(sizeof(V1Lay) / 4); i += blockDim.x) ((int *)&sL)[i] = ((const int *)&L)[i];
+    c.M = &sM; c.L = &sL;
     c.tid = threadIdx.x; c.lane = threadIdx.x & 31; c.warp = threadIdx.x >> 5; c.nt = blockDim.x;
     c.cp = a.CP + (size_t)blockIdx.x * GS * M.Ppad;
     for (int i = threadIdx.x; i < M.K * M.L; i += blockDim.x) ((uint8_t *)(V1SM + L.oEXP))[i] = M.exps[i];
+    for (int i = threadIdx.x; i < GS * L.Kq; i += blockDim.x) V1SM[L.oPHI + i] = 0.f;   // phi is zero past K
     __syncthreads();
 }
 

@@ -226,7 +226,9 @@ extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx *
     }
     M.Ppad = po;
     // padded tables: halos replicate the segment's edge pixel (the clamp of C.2-16 for free)
-    std::vector<float> Cp((size_t)K * M.Ppad), isp(M.Ppad);
+    // K+2 rounded to 8 rows, plus 16 (prefetch overrun): zero past K, so the v1 loops sweep whole batches without bounds tests
+    const int Krows = roundup(K + 2, 8) + 16;
+    std::vector<float> Cp((size_t)Krows * M.Ppad, 0.f), isp(M.Ppad);
     for (int sg = 0; sg < nseg; ++sg) {
         const SegDev &S = M.seg[sg];
         for (int q = 0; q < S.len; ++q) {
@@ -315,7 +317,8 @@ static int setup_v1(lasp_ctx *c, const cudaDeviceProp &prop)
     auto take = [&](int n) { int r = o; o += roundup(n, 4); return r; };
     L.oT = take(GS * L.RL); L.oA = take(GS * L.RL);
     L.oU = take(GS * M.NP); L.oM = take(GS * M.NP); L.oV = take(GS * M.NP);
-    L.oX = take(GS * M.L); L.oPHI = take(GS * M.K);
+    L.Kq = roundup(M.K + 2, 8);
+    L.oX = take(GS * M.L); L.oPHI = take(GS * L.Kq);
     L.oGW = take(GS * L.NA * 4); L.oGR = take(3 * GS * L.NA * 4); L.oTAP = take(2 * GS);
     L.oMOM = take(GS * L.nmomr); L.oRHS = take(GS * L.n1r); L.oB = take(GS * M.nc);
     L.oRED = take(L.NW * L.VR * GS);
@@ -338,6 +341,7 @@ static int setup_v1(lasp_ctx *c, const cudaDeviceProp &prop)
         return LASP_OK;
     }
     c->v1_cta_per_sm = per_sm;
+    if (const char *e = getenv("LASP_CTAS_PER_SM")) c->v1_cta_per_sm = std::max(1, std::min(per_sm, atoi(e)));   // experiment knob
     c->v1_ok = getenv("LASP_FORCE_V0") == nullptr;
     return LASP_OK;
 }
