@@ -105,6 +105,17 @@ int lasp_fit_batch(lasp_ctx *ctx, int64_t B, const float *flux, const float *iva
                    float *params, float *cont, float *chi2, float *err, int32_t *status,
                    void *stream);
 
+/* The same fit from HOST buffers (pinned memory recommended), for batches that do not fit on the device or
+ * arrive from the host (BASELINE.json config 3, "survey-scale stream"): the batch is cut into chunks of
+ * `chunk` spectra (0 = 65,536); chunk i+1 is copied host-to-device and chunk i-1's results device-to-host on
+ * two copy streams while chunk i is fitted, with ctx-owned double buffers.  All pointers are HOST pointers
+ * with the layouts of lasp_fit_batch; mask, cont, err, status may be NULL.  Blocking: returns when every
+ * result is in host memory.  Per-chunk results are identical to lasp_fit_batch on the same spectra. */
+int lasp_fit_batch_host(lasp_ctx *ctx, int64_t B, const float *flux, const float *ivar,
+                        const uint8_t *mask, const float *init, const lasp_fit_opts *opts,
+                        float *params, float *cont, float *chi2, float *err, int32_t *status,
+                        int64_t chunk);
+
 /* Inspection: model_j = c_j S_j at given physical params [B*NP] and plain-Legendre cont
  * [B*n_seg*(D+1)]; model [B*n_pix]. */
 int lasp_eval_model(lasp_ctx *ctx, int64_t B, const float *params, const float *cont,

@@ -13,7 +13,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "liblasp_gpu.so")
 
-SYMBOLS = ["lasp_create", "lasp_destroy", "lasp_reserve", "lasp_fit_batch", "lasp_eval_model",
+SYMBOLS = ["lasp_create", "lasp_destroy", "lasp_reserve", "lasp_fit_batch", "lasp_fit_batch_host", "lasp_eval_model",
            "lasp_eval_grad", "lasp_kernel_variant", "lasp_launch_count", "lasp_fma_per_spectrum_step", "lasp_last_error",
            "lasp_version"]
 
@@ -62,6 +62,8 @@ def lib():
         L.lasp_reserve.argtypes = [C.c_void_p, C.c_int64]
         L.lasp_fit_batch.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 4 + [C.POINTER(FitOpts)] + \
                                     [C.c_void_p] * 6
+        L.lasp_fit_batch_host.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 4 + [C.POINTER(FitOpts)] + \
+                                         [C.c_void_p] * 5 + [C.c_int64]
         L.lasp_eval_model.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 4
         L.lasp_eval_grad.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 9
         L.lasp_kernel_variant.argtypes = [C.c_void_p]
@@ -177,6 +179,37 @@ class LaspModel:
                                   _ptr(out["params"]), _ptr(out.get("cont")), _ptr(out["chi2"]),
                                   _ptr(out.get("err")), _ptr(out["status"]), self._stream())
         self._check(rc, "lasp_fit_batch")
+        return out
+
+    def fit_batch_host(self, flux, ivar, mask, init, n_iter, lr=1e-2, beta1=0.9, beta2=0.999, eps=1e-8,
+                       want_err=True, want_cont=True, chunk=0, out=None):
+        """lasp_fit_batch_host on HOST tensors (torch CPU tensors, pinned for overlap); returns host tensors.
+        The library cuts the batch into chunks and overlaps the copies with the fits."""
+        t = self.torch
+
+        def host(a, dtype):
+            if a is None:
+                return None
+            if not isinstance(a, t.Tensor):
+                a = t.from_numpy(np.ascontiguousarray(a))
+            assert a.device.type == "cpu"
+            return a.to(dtype).contiguous()
+
+        flux = host(flux, t.float32); ivar = host(ivar, t.float32)
+        mask = host(mask, t.uint8); init = host(init, t.float32)
+        B = flux.shape[0]
+        assert flux.shape == (B, self.P) and ivar.shape == (B, self.P) and init.shape == (B, self.NP)
+        if out is None:
+            pin = dict(pin_memory=True)
+            out = dict(params=t.empty((B, self.NP), dtype=t.float32, **pin), chi2=t.empty(B, dtype=t.float32, **pin),
+                       status=t.empty(B, dtype=t.int32, **pin),
+                       cont=t.empty((B, self.nc), dtype=t.float32, **pin) if want_cont else None,
+                       err=t.empty((B, self.NP), dtype=t.float32, **pin) if want_err else None)
+        opts = FitOpts(int(n_iter), lr, beta1, beta2, eps, 0, 0)
+        rc = lib().lasp_fit_batch_host(self.ctx, B, _ptr(flux), _ptr(ivar), _ptr(mask), _ptr(init), C.byref(opts),
+                                       _ptr(out["params"]), _ptr(out.get("cont")), _ptr(out["chi2"]),
+                                       _ptr(out.get("err")), _ptr(out["status"]), int(chunk))
+        self._check(rc, "lasp_fit_batch_host")
         return out
 
     def eval_model(self, params, cont):

@@ -36,7 +36,16 @@ struct lasp_ctx {
     float *dY = nullptr, *dW = nullptr;
     size_t plane_rows = 0;
     float *dCP = nullptr, *dXJ = nullptr;
-    unsigned long long *ddbg = nullptr;   // LASP_TIMING=1: per-phase cycle counters (debug aid)
+    unsigned long long *ddbg = nullptr;
+    // lasp_fit_batch_host: double-buffered device chunks, two copy streams and one compute stream
+    struct HostPipe {
+        int64_t cap = 0;
+        float *flux[2] = {}, *ivar[2] = {}, *init[2] = {}, *params[2] = {}, *cont[2] = {}, *chi2[2] = {}, *err[2] = {};
+        uint8_t *mask[2] = {};
+        int32_t *status[2] = {};
+        cudaStream_t s_in = nullptr, s_out = nullptr, s_fit = nullptr;
+        cudaEvent_t in_done[2] = {}, fit_done[2] = {}, out_done[2] = {};
+    } hp;   // LASP_TIMING=1: per-phase cycle counters (debug aid)
     size_t cp_ctas = 0, xj_ctas = 0;
     std::string err;
 };
@@ -83,6 +92,8 @@ static void gauss_legendre(int n, std::vector<double> &x, std::vector<double> &w
     }
 }
 
+static void hostpipe_free(lasp_ctx *c);
+
 extern "C" int lasp_version(void) { return LASP_VERSION; }
 
 extern "C" const char *lasp_last_error(const lasp_ctx *ctx) { return ctx ? ctx->err.c_str() : g_err.c_str(); }
@@ -104,7 +115,12 @@ extern "C" int lasp_destroy(lasp_ctx *c)
     cudaSetDevice(c->device);
     cudaFree(c->dC); cudaFree(c->dinv_s); cudaFree(c->dexps); cudaFree(c->dconv); cudaFree(c->dnedge);
     cudaFree(c->dYW); cudaFree(c->dscratch);
-    cudaFree(c->dY); cudaFree(c->dW); cudaFree(c->dCP); cudaFree(c->dXJ);
+    cudaFree(c->dY); cudaFree(c->dW); cudaFree(c->dCP); cudaFree(c->dXJ); cudaFree(c->ddbg);
+    hostpipe_free(c);
+    if (c->hp.s_in) {
+        cudaStreamDestroy(c->hp.s_in); cudaStreamDestroy(c->hp.s_out); cudaStreamDestroy(c->hp.s_fit);
+        for (int s = 0; s < 2; ++s) { cudaEventDestroy(c->hp.in_done[s]); cudaEventDestroy(c->hp.fit_done[s]); cudaEventDestroy(c->hp.out_done[s]); }
+    }
     delete c;
     return LASP_OK;
 }
@@ -597,4 +613,105 @@ extern "C" double lasp_fma_per_spectrum_step(const lasp_ctx *c, double mean_taps
     double G = (2.0 * M.D + 1.0) * P + M.n_seg * n1 * n1 * n1 / 6.0;
     return 2.0 * K * P + 4.0 * W * P + (linear ? 2.0 * W * P : 0.0) + G + 4.0 * n1 * P +
            M.n_seg * (n1 * n1 * n1 / 6.0 + 4.0 * n1 * n1) + 8.0 * P;
+}
+
+// ------------------------------------------------------------------------------------------
+// lasp_fit_batch_host: chunked host->device->fit->host pipeline (config 3)
+// ------------------------------------------------------------------------------------------
+static void hostpipe_free(lasp_ctx *c)
+{
+    lasp_ctx::HostPipe &h = c->hp;
+    for (int s = 0; s < 2; ++s) {
+        cudaFree(h.flux[s]); cudaFree(h.ivar[s]); cudaFree(h.mask[s]); cudaFree(h.init[s]);
+        cudaFree(h.params[s]); cudaFree(h.cont[s]); cudaFree(h.chi2[s]); cudaFree(h.err[s]); cudaFree(h.status[s]);
+        h.flux[s] = h.ivar[s] = h.init[s] = h.params[s] = h.cont[s] = h.chi2[s] = h.err[s] = nullptr;
+        h.mask[s] = nullptr; h.status[s] = nullptr;
+    }
+    h.cap = 0;
+}
+
+static int hostpipe_reserve(lasp_ctx *c, int64_t chunk)
+{
+    lasp_ctx::HostPipe &h = c->hp;
+    const ModelDev &M = c->M;
+    if (!h.s_in) {
+        CUDA_TRY(c, cudaStreamCreateWithFlags(&h.s_in, cudaStreamNonBlocking));
+        CUDA_TRY(c, cudaStreamCreateWithFlags(&h.s_out, cudaStreamNonBlocking));
+        CUDA_TRY(c, cudaStreamCreateWithFlags(&h.s_fit, cudaStreamNonBlocking));
+        for (int s = 0; s < 2; ++s) {
+            CUDA_TRY(c, cudaEventCreateWithFlags(&h.in_done[s], cudaEventDisableTiming));
+            CUDA_TRY(c, cudaEventCreateWithFlags(&h.fit_done[s], cudaEventDisableTiming));
+            CUDA_TRY(c, cudaEventCreateWithFlags(&h.out_done[s], cudaEventDisableTiming));
+        }
+    }
+    if (chunk <= h.cap) return LASP_OK;
+    hostpipe_free(c);
+    const size_t n = (size_t)chunk;
+    for (int s = 0; s < 2; ++s) {
+        CUDA_TRY(c, cudaMalloc(&h.flux[s], n * M.P * sizeof(float)));
+        CUDA_TRY(c, cudaMalloc(&h.ivar[s], n * M.P * sizeof(float)));
+        CUDA_TRY(c, cudaMalloc(&h.mask[s], n * M.P));
+        CUDA_TRY(c, cudaMalloc(&h.init[s], n * M.NP * sizeof(float)));
+        CUDA_TRY(c, cudaMalloc(&h.params[s], n * M.NP * sizeof(float)));
+        CUDA_TRY(c, cudaMalloc(&h.cont[s], n * M.nc * sizeof(float)));
+        CUDA_TRY(c, cudaMalloc(&h.chi2[s], n * sizeof(float)));
+        CUDA_TRY(c, cudaMalloc(&h.err[s], n * M.NP * sizeof(float)));
+        CUDA_TRY(c, cudaMalloc(&h.status[s], n * sizeof(int32_t)));
+    }
+    h.cap = chunk;
+    return LASP_OK;
+}
+
+extern "C" int lasp_fit_batch_host(lasp_ctx *c, int64_t B, const float *flux, const float *ivar,
+                                   const uint8_t *mask, const float *init, const lasp_fit_opts *opts,
+                                   float *params, float *cont, float *chi2, float *err, int32_t *status,
+                                   int64_t chunk)
+{
+    if (!c) return fail(nullptr, LASP_ERR_INVALID_ARG, "null ctx");
+    if (B < 1 || !flux || !ivar || !init || !opts || !params || !chi2 || chunk < 0)
+        return fail(c, LASP_ERR_INVALID_ARG, "lasp_fit_batch_host: null pointer, B < 1 or chunk < 0");
+    CUDA_TRY(c, cudaSetDevice(c->device));
+    if (chunk == 0) chunk = 65536;
+    chunk = std::min<int64_t>(chunk, B);
+    int rc = hostpipe_reserve(c, chunk);
+    if (rc) return rc;
+    lasp_ctx::HostPipe &h = c->hp;
+    const ModelDev &M = c->M;
+    const int64_t nchunk = (B + chunk - 1) / chunk;
+    auto upload = [&](int64_t i) -> int {
+        const int s = (int)(i & 1);
+        const int64_t o = i * chunk, n = std::min(chunk, B - o);
+        // the slot's previous fit (chunk i-2) must be done reading its inputs
+        if (i >= 2) CUDA_TRY(c, cudaStreamWaitEvent(h.s_in, h.fit_done[s], 0));
+        CUDA_TRY(c, cudaMemcpyAsync(h.flux[s], flux + o * M.P, (size_t)n * M.P * sizeof(float), cudaMemcpyHostToDevice, h.s_in));
+        CUDA_TRY(c, cudaMemcpyAsync(h.ivar[s], ivar + o * M.P, (size_t)n * M.P * sizeof(float), cudaMemcpyHostToDevice, h.s_in));
+        if (mask) CUDA_TRY(c, cudaMemcpyAsync(h.mask[s], mask + o * M.P, (size_t)n * M.P, cudaMemcpyHostToDevice, h.s_in));
+        CUDA_TRY(c, cudaMemcpyAsync(h.init[s], init + o * M.NP, (size_t)n * M.NP * sizeof(float), cudaMemcpyHostToDevice, h.s_in));
+        CUDA_TRY(c, cudaEventRecord(h.in_done[s], h.s_in));
+        return LASP_OK;
+    };
+    rc = upload(0);
+    if (rc) return rc;
+    for (int64_t i = 0; i < nchunk; ++i) {
+        const int s = (int)(i & 1);
+        const int64_t o = i * chunk, n = std::min(chunk, B - o);
+        if (i + 1 < nchunk) { rc = upload(i + 1); if (rc) return rc; }
+        CUDA_TRY(c, cudaStreamWaitEvent(h.s_fit, h.in_done[s], 0));
+        if (i >= 2) CUDA_TRY(c, cudaStreamWaitEvent(h.s_fit, h.out_done[s], 0));   // slot's old results copied out
+        rc = lasp_fit_batch(c, n, h.flux[s], h.ivar[s], mask ? h.mask[s] : nullptr, h.init[s], opts, h.params[s],
+                            cont ? h.cont[s] : nullptr, h.chi2[s], err ? h.err[s] : nullptr,
+                            status ? h.status[s] : nullptr, h.s_fit);
+        if (rc) return rc;
+        CUDA_TRY(c, cudaEventRecord(h.fit_done[s], h.s_fit));
+        CUDA_TRY(c, cudaStreamWaitEvent(h.s_out, h.fit_done[s], 0));
+        CUDA_TRY(c, cudaMemcpyAsync(params + o * M.NP, h.params[s], (size_t)n * M.NP * sizeof(float), cudaMemcpyDeviceToHost, h.s_out));
+        CUDA_TRY(c, cudaMemcpyAsync(chi2 + o, h.chi2[s], (size_t)n * sizeof(float), cudaMemcpyDeviceToHost, h.s_out));
+        if (cont) CUDA_TRY(c, cudaMemcpyAsync(cont + o * M.nc, h.cont[s], (size_t)n * M.nc * sizeof(float), cudaMemcpyDeviceToHost, h.s_out));
+        if (err) CUDA_TRY(c, cudaMemcpyAsync(err + o * M.NP, h.err[s], (size_t)n * M.NP * sizeof(float), cudaMemcpyDeviceToHost, h.s_out));
+        if (status) CUDA_TRY(c, cudaMemcpyAsync(status + o, h.status[s], (size_t)n * sizeof(int32_t), cudaMemcpyDeviceToHost, h.s_out));
+        CUDA_TRY(c, cudaEventRecord(h.out_done[s], h.s_out));
+    }
+    CUDA_TRY(c, cudaStreamSynchronize(h.s_out));
+    CUDA_TRY(c, cudaStreamSynchronize(h.s_fit));
+    return LASP_OK;
 }

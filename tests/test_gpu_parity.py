@@ -204,3 +204,58 @@ def test_bad_arguments_return_error_codes(gpu):
     d3 = dict(d); d3["hi"] = d["lo"].copy()
     with pytest.raises(gpu.LaspError):
         gpu.LaspModel(d3)          # lo >= hi
+
+
+# ------------------------------------------------------------------ host pipeline (config 3 path)
+
+def test_fit_batch_host_matches_device_call(gpu, oracle_mod):
+    """lasp_fit_batch_host (chunked H2D / fit / D2H) returns exactly what lasp_fit_batch returns, ragged chunks."""
+    import torch
+    case = synth.make_case(0, oracle_mod.forward, B=37)
+    m = gpu.LaspModel(case["desc"])
+    dev = m.fit_batch(case["flux"], case["ivar"], case["mask"], case["init"], 25)
+    host = m.fit_batch_host(torch.from_numpy(case["flux"]).pin_memory(), torch.from_numpy(case["ivar"]).pin_memory(),
+                            torch.from_numpy(case["mask"]).pin_memory(), torch.from_numpy(case["init"]).pin_memory(),
+                            25, chunk=16)
+    for k in ("params", "chi2", "cont", "err", "status"):
+        assert torch.equal(host[k], dev[k].cpu()), k
+    nomask = m.fit_batch_host(case["flux"], case["ivar"], None, case["init"], 5, chunk=0, want_err=False, want_cont=False)
+    assert nomask["err"] is None and torch.isfinite(nomask["chi2"]).all()
+    m.close()
+
+
+# ------------------------------------------------------------------ full size, bench launch configuration
+
+@pytest.mark.slow
+def test_fit_config1_full_size_sampled(gpu, oracle_mod):
+    """BASELINE.json config 1 at full size (B = 65,536, 500 Adam steps, the grid bench.py launches): the batch is
+    32 oracle-generated spectra tiled 2048 times; sampled rows across the batch (first, ragged middle, last CTA)
+    are compared with the oracle one by one, and every copy of a spectrum must give the same result."""
+    import torch
+    cfg = synth.CONFIGS[1]
+    base = synth.make_case(1, oracle_mod.forward, B=32)
+    reps = cfg.B // 32
+    m = gpu.LaspModel(base["desc"])
+    dev = m.device
+    tile = lambda a: torch.from_numpy(a).to(dev).repeat(reps, *([1] * (a.ndim - 1)))
+    r = m.fit_batch(tile(base["flux"]), tile(base["ivar"]), tile(base["mask"]), tile(base["init"]), cfg.n_iter,
+                    lr=cfg.lr)
+    par = r["params"].cpu().numpy().astype(np.float64)
+    chi = r["chi2"].cpu().numpy().astype(np.float64)
+    err = r["err"].cpu().numpy().astype(np.float64)
+    st = r["status"].cpu().numpy()
+    # property that holds at any size: identical inputs give identical outputs wherever they sit in the grid
+    assert np.array_equal(par.reshape(reps, 32, -1), np.broadcast_to(par[:32], (reps, 32, par.shape[1])))
+    assert np.array_equal(chi.reshape(reps, 32), np.broadcast_to(chi[:32], (reps, 32)))
+    sample = [0, 5, 13, 31, 32 * 1000 + 7, 32 * 1777 + 18, cfg.B - 32 + 2, cfg.B - 1]
+    idx = sorted({i % 32 for i in sample})
+    o = oracle_mod.Oracle(base["desc"])
+    ref = o.fit(base["flux"][idx], base["ivar"][idx], base["mask"][idx], base["init"][idx], cfg.n_iter, lr=cfg.lr)
+    pos = {j: n for n, j in enumerate(idx)}
+    for i in sample:
+        n = pos[i % 32]
+        assert (np.abs(par[i] - ref["params"][n]) / (o.hi - o.lo)).max() <= TOL_PAR, i
+        assert abs(chi[i] / ref["chi2"][n] - 1) <= TOL_CHI2, i
+        assert np.abs(err[i] / ref["err"][n] - 1).max() <= TOL_ERR, i
+        assert st[i] == ref["status"][n], i
+    m.close()
