@@ -11,7 +11,7 @@
 // transpose over warp shuffles (32 values x 32 lanes in 31 shuffles) and one shared-memory slot per
 // warp; the continuum system is solved by one warp per spectrum (lanes = rows).
 //
-// Citations: Eq. n and P:n are /root/reference/PAPER.md; C.2-n the readings of SURVEY.md 8(c)
+// Citations: Eq. n and P:n are /root/reference/PAPER.md; C.2-n the readings of SURVEY.md 8()
 // (restated in DESIGN.md); a0..a9 the steps of SURVEY.md 8(a).
 #pragma once
 #include "lasp_device.cuh"
@@ -33,7 +33,8 @@ struct V1Lay {
     int Hm;                 // support clamp (memory safety outside the prior box)
     int refresh;            // re-accumulate the Gram moments and re-factor every `refresh` steps
     // shared-memory offsets (floats)
-    int oT, oA, oU, oM, oV, oX, oPHI, oGW, oGR, oTAP, oMOM, oRHS, oB, oRED, oLF, oQ, oSC, oEXP, total;
+    int oT, oA, oU, oM, oV, oX, oPHI, oGW, oGR, oTAP, oMOM, oRHS, oB, oRED, oLF, oQ, oSC, oEXP, oXP, oDPHI, oGSC, oEW, total;
+    int emax;               // largest exponent of the monomial table
 };
 
 struct V1Args {
@@ -84,38 +85,71 @@ __device__ __forceinline__ float warp_min_f(float v)
     return v;
 }
 
-struct V1Ctx {
-    const ModelDev *M;
-    const V1Lay *L;
-    int tid, lane, warp, nt;
+// Block-wide state.  It lives in static shared memory and the per-thread indices are recomputed from
+// threadIdx where needed: a context struct passed by reference to the (deliberately not inlined) phase
+// functions would sit in LOCAL memory, and with shared memory carved out to ~190 KB per SM the remaining L1
+// is thrashed by the coefficient stream, so every such access costs an L2 round trip.
+struct V1Block {
+    ModelDev M;
+    V1Lay L;
+    V1Args A;
     long long spec[GS];   // clamped spectrum indices of the group
     float *cp;            // this CTA's c_prev scratch
 };
+__shared__ V1Block v1_blk;
+#define V1_TID ((int)threadIdx.x)
+#define V1_LANE ((int)(threadIdx.x & 31))
+#define V1_WARP ((int)(threadIdx.x >> 5))
+#define V1_NT ((int)blockDim.x)
 
-#define SMV(c, off, idx, g) V1SM[(off) + (idx) * GS + (g)]
+#define SMV(off, idx, g) V1SM[(off) + (idx) * GS + (g)]
 
 // ------------------------------------------------------------------------------------------
 // a1: de-normalise, emulator inputs, monomials (Eq. 1, C.2-18/19).  Warp g, spectrum g.
 // ------------------------------------------------------------------------------------------
-__device__ __noinline__ void v1_param_setup(const V1Ctx &c, int g)
+__device__ __noinline__ void v1_param_setup(int g)
 {
-    const ModelDev &M = *c.M;
-    const V1Lay &L = *c.L;
-    for (int p = c.lane; p < M.NP; p += 32) {
-        float u = SMV(c, L.oU, p, g);
-        float th = M.lo[p] + (u + 1.f) * (M.hi[p] - M.lo[p]) * 0.5f;
-        if (p < M.L) SMV(c, L.oX, p, g) = label_x(M, p, th);
-        else SMV(c, L.oSC, p == M.L ? SC_V : SC_SIG, g) = th;
+    const ModelDev &M = v1_blk.M;
+    const V1Lay &L = v1_blk.L;
+    const int nl = M.L, K = M.K, ne = L.emax + 1;
+    const uint8_t *ex = (const uint8_t *)(V1SM + L.oEXP);
+    for (int p = V1_LANE; p < M.NP; p += 32) {
+        const float u = SMV(L.oU, p, g);
+        const float half = (M.hi[p] - M.lo[p]) * 0.5f;
+        const float th = M.lo[p] + (u + 1.f) * half;
+        float gsc = half;                       // d theta / d u
+        if (p < nl) {
+            SMV(L.oX, p, g) = label_x(M, p, th);
+            gsc *= M.label_log10[p] ? M.emu_a[p] / (th * 2.302585093f) : M.emu_a[p];   // d x / d theta (C.1)
+        } else
+            SMV(L.oSC, p == nl ? SC_V : SC_SIG, g) = th;
+        SMV(L.oGSC, p, g) = gsc;
     }
     __syncwarp();
-    for (int k = c.lane; k < M.K; k += 32) {
+    // powers x_l^e, e = 0..emax: XP[e*nl + l]
+    for (int i = V1_LANE; i < nl * ne; i += 32) {
+        const int e = i / nl, l = i - e * nl;
+        const float x = SMV(L.oX, l, g);
+        float pw = 1.f;
+        for (int q = 0; q < e; ++q) pw *= x;
+        SMV(L.oXP, i, g) = pw;
+    }
+    __syncwarp();
+    // phi_k = prod_l x_l^e_kl and d phi_k / d x_l = e_kl x_l^(e_kl - 1) prod_{l2 != l} x_l2^e_kl2  (Eq. 1)
+    for (int k = V1_LANE; k < K; k += 32) {
         float p = 1.f;
-        for (int l = 0; l < M.L; ++l) {
-            int e = ((const uint8_t *)(V1SM + L.oEXP))[k * M.L + l];
-            float x = SMV(c, L.oX, l, g);
-            for (int q = 0; q < e; ++q) p *= x;
+        for (int l = 0; l < nl; ++l) p *= SMV(L.oXP, ex[k * nl + l] * nl + l, g);
+        SMV(L.oPHI, k, g) = p;
+        for (int l = 0; l < nl; ++l) {
+            const int el = ex[k * nl + l];
+            float d = 0.f;
+            if (el > 0) {
+                d = (float)el * SMV(L.oXP, (el - 1) * nl + l, g);
+                for (int l2 = 0; l2 < nl; ++l2)
+                    if (l2 != l) d *= SMV(L.oXP, ex[k * nl + l2] * nl + l2, g);
+            }
+            SMV(L.oDPHI, l * K + k, g) = d;
         }
-        SMV(c, L.oPHI, k, g) = p;
     }
     __syncwarp();
 }
@@ -127,21 +161,26 @@ __device__ __noinline__ void v1_param_setup(const V1Ctx &c, int g)
 //   GR [j][g][a][4]    reversed kernels for the adjoint pass: j=0: g_{-k}; j=1: d g_{-k}/dv;
 //                      j=2: d g_{-k}/d sigma* (chain factors of C.1 folded in)
 // ------------------------------------------------------------------------------------------
-__device__ __noinline__ void v1_setup_weights(const V1Ctx &c, const SegDev &sg, int g)
+__device__ __noinline__ void v1_setup_weights(const SegDev &sg, int g)
 {
-    const V1Lay &L = *c.L;
-    const float v = SMV(c, L.oSC, SC_V, g), sigstar = SMV(c, L.oSC, SC_SIG, g);
+    const V1Lay &L = v1_blk.L;
+    const float v = SMV(L.oSC, SC_V, g), sigstar = SMV(L.oSC, SC_SIG, g);
     const float sigtot = sqrtf(sigstar * sigstar + sg.sig_inst * sg.sig_inst);
     const float mu = v * sg.inv_s, s = sigtot * sg.inv_s;
     int H = (int)ceilf(fabsf(mu) + 5.f * s);
     H = min(max(H, 0), sg.halo - 18);   // memory safety outside the prior box (halo >= Hmax + 18)
     const float i2 = 0.5f / (s * s);
+    // one exponential per tap, kept in shared memory; the grouped forward / reversed / derivative tables are
+    // filled from it
+    float *ew = V1SM + L.oEW + g * (2 * L.Hm + 2);
     float sum = 0.f, s1 = 0.f, s2 = 0.f;
-    for (int m = c.lane; m <= 2 * H; m += 32) {
-        float d = (float)(m - H) - mu;
-        float e = expf(-d * d * i2);
+    for (int m = V1_LANE; m <= 2 * H; m += 32) {
+        const float d = (float)(m - H) - mu;
+        const float e = expf(-d * d * i2);
+        ew[m] = e;
         sum += e; s1 = fmaf(e, d, s1); s2 = fmaf(e * d, d, s2);
     }
+    __syncwarp();
     sum = warp_sum_f(sum); s1 = warp_sum_f(s1); s2 = warp_sum_f(s2);
     const float inv = 1.f / sum;
     const float e1n = s1 * inv, e2n = s2 * inv;       // kbar - mu ; second moment about mu
@@ -152,18 +191,17 @@ __device__ __noinline__ void v1_setup_weights(const V1Ctx &c, const SegDev &sg, 
     float *gw = V1SM + L.oGW + g * L.NA * 4;
     float *gr = V1SM + L.oGR + g * L.NA * 4;
     const int rs = GS * L.NA * 4;
-    for (int idx = c.lane; idx < na * 4; idx += 32) {
+    for (int idx = V1_LANE; idx < na * 4; idx += 32) {
         const int k = 4 * (a_lo + (idx >> 2)) - 3 + (idx & 3);
         const bool in = (k >= -H) && (k <= H);
-        float d = (float)k - mu;
-        gw[idx] = in ? expf(-d * d * i2) * inv : 0.f;
-        d = (float)(-k) - mu;
-        float gg = in ? expf(-d * d * i2) * inv : 0.f;
+        gw[idx] = in ? ew[k + H] * inv : 0.f;
+        const float d = (float)(-k) - mu;
+        const float gg = in ? ew[H - k] * inv : 0.f;
         gr[idx] = gg;
         gr[rs + idx] = gg * (d - e1n) * cmu;
         gr[2 * rs + idx] = gg * (d * d - e2n) * csig;
     }
-    if (c.lane == 0) {
+    if (V1_LANE == 0) {
         int *tap = (int *)(V1SM + L.oTAP);
         tap[g * 2] = a_lo; tap[g * 2 + 1] = na;
     }
@@ -209,17 +247,17 @@ __device__ __forceinline__ void v1_stencil_octet(const float4 *__restrict__ row4
 }
 
 // shared-memory row of spectrum g in buffer `off`, as a float pointer indexed by padded pixel jp
-__device__ __forceinline__ float *v1_row(const V1Ctx &c, int off, const SegDev &sg, int g)
+__device__ __forceinline__ float *v1_row(int off, const SegDev &sg, int g)
 {
-    return V1SM + off + g * c.L->RL + c.L->GUARD - sg.po;
+    return V1SM + off + g * v1_blk.L.RL + v1_blk.L.GUARD - sg.po;
 }
 
 // padded pixel range [lo,hi) on which T is needed by the forward stencils of the group's fitted octets
 // (group a reads row[j0-4a .. j0-4a+11]); the adjoint pass runs on the same range.  Kept tight: config 1
 // has 188 fitted octets and 192 threads, so 16 pixels of reach on each side still fit one sweep.
-__device__ __forceinline__ void v1_group_range(const V1Ctx &c, const SegDev &sg, int &lo, int &hi)
+__device__ __forceinline__ void v1_group_range(const SegDev &sg, int &lo, int &hi)
 {
-    const int *tap = (const int *)(V1SM + c.L->oTAP);
+    const int *tap = (const int *)(V1SM + v1_blk.L.oTAP);
     int rl = 0, rh = 0;
 #pragma unroll
     for (int g = 0; g < GS; ++g) {
@@ -234,16 +272,16 @@ __device__ __forceinline__ void v1_group_range(const V1Ctx &c, const SegDev &sg,
 // ------------------------------------------------------------------------------------------
 // a2: T_j = sum_k phi_k C[k,j] over the padded range [lo,hi) -> shared row T (Eq. 1)
 // ------------------------------------------------------------------------------------------
-__device__ __noinline__ void v1_phase_emulator(const V1Ctx &c, const SegDev &sg, int lo, int hi)
+__device__ __noinline__ void v1_phase_emulator(const SegDev &sg, int lo, int hi)
 {
     // everything the loop needs is copied to registers first: the model lives in shared memory, and after
     // any shared-memory store the compiler would otherwise have to re-read it
-    const float4 *phi4 = (const float4 *)(V1SM + c.L->oPHI);
-    const int P4 = c.M->Ppad >> 2, Kq = c.L->Kq, nt8 = c.nt * OCT;
-    const float *Cg = c.M->C;
-    float *rowT = V1SM + c.L->oT + c.L->GUARD - sg.po;
-    const int RL = c.L->RL;
-    for (int j0 = lo + c.tid * OCT; j0 < hi; j0 += nt8) {
+    const float4 *phi4 = (const float4 *)(V1SM + v1_blk.L.oPHI);
+    const int P4 = v1_blk.M.Ppad >> 2, Kq = v1_blk.L.Kq, nt8 = V1_NT * OCT;
+    const float *Cg = v1_blk.M.C;
+    float *rowT = V1SM + v1_blk.L.oT + v1_blk.L.GUARD - sg.po;
+    const int RL = v1_blk.L.RL;
+    for (int j0 = lo + V1_TID * OCT; j0 < hi; j0 += nt8) {
         float acc[GS][OCT];
 #pragma unroll
         for (int g = 0; g < GS; ++g)
@@ -308,27 +346,28 @@ __device__ __noinline__ void v1_phase_emulator(const V1Ctx &c, const SegDev &sg,
 // Partial sums over the thread's 8 pixels are reduced over the warp by register transposes and
 // land in this warp's reduction slots.
 // ------------------------------------------------------------------------------------------
-__device__ __noinline__ void v1_phase_forward(const V1Ctx &c, const SegDev &sg, const V1Args &a, bool stencil, bool mom)
+__device__ __noinline__ void v1_phase_forward(const SegDev &sg, bool stencil, bool mom)
 {
-    const V1Lay &L = *c.L;
+    const V1Args &a = v1_blk.A;
+    const V1Lay &L = v1_blk.L;
     const int *tap = (const int *)(V1SM + L.oTAP);
-    float *red = V1SM + L.oRED + c.warp * L.VR * GS;
+    float *red = V1SM + L.oRED + V1_WARP * L.VR * GS;
     // hoisted to registers (the model sits in shared memory; see v1_phase_emulator)
-    const int Ppad = c.M->Ppad, RL = L.RL, NA = L.NA, n1r = L.n1r, nmomr = L.nmomr, nt8 = c.nt * OCT;
+    const int Ppad = v1_blk.M.Ppad, RL = L.RL, NA = L.NA, n1r = L.n1r, nmomr = L.nmomr, nt8 = V1_NT * OCT;
     const int fit_lo = sg.fit_lo, fit_hi = sg.fit_hi, torg = sg.po + sg.halo;
     const float ta = sg.ta, tb = sg.tb;
     float *rowA = V1SM + L.oA + L.GUARD - sg.po;
     const float *rowT = V1SM + L.oT + L.GUARD - sg.po;
     const float4 *gw4 = (const float4 *)(V1SM + L.oGW);
     const float *Yg = a.Y, *Wg = a.W;
-    const float *cpg = c.cp;
+    const float *cpg = v1_blk.cp;
     int alo[GS], nag[GS];
     size_t rowo[GS];
 #pragma unroll
-    for (int g = 0; g < GS; ++g) { alo[g] = tap[2 * g]; nag[g] = tap[2 * g + 1]; rowo[g] = (size_t)c.spec[g] * Ppad; }
+    for (int g = 0; g < GS; ++g) { alo[g] = tap[2 * g]; nag[g] = tap[2 * g + 1]; rowo[g] = (size_t)v1_blk.spec[g] * Ppad; }
     bool first = true;
     for (int jb = fit_lo; jb < fit_hi; jb += nt8, first = false) {   // uniform trip count
-        const int j0 = jb + c.tid * OCT;
+        const int j0 = jb + V1_TID * OCT;
         const bool act = j0 < fit_hi;
         float u[GS][OCT], v[GS][OCT];
         if (act) {
@@ -390,9 +429,9 @@ __device__ __noinline__ void v1_phase_forward(const V1Ctx &c, const SegDev &sg, 
 #pragma unroll
                     for (int i = 0; i < OCT; ++i) { const float nx = fmaf(x2[i], pc[i], -pp[i]); pp[i] = pc[i]; pc[i] = nx; }
                 }
-                const float tot = xreduce32(X, c.lane);
-                const int n = n0 + (c.lane >> 3), g = c.lane & 3;
-                const int slot = (c.lane & 4) ? nmomr + n : n;
+                const float tot = xreduce32(X, V1_LANE);
+                const int n = n0 + (V1_LANE >> 3), g = V1_LANE & 3;
+                const int slot = (V1_LANE & 4) ? nmomr + n : n;
                 if (first) red[slot * GS + g] = tot; else red[slot * GS + g] += tot;
             }
             // region B: n1r <= n < nmomr, moments only, eight n per transpose: value (nn, g) at nn*4 + g
@@ -410,9 +449,9 @@ __device__ __noinline__ void v1_phase_forward(const V1Ctx &c, const SegDev &sg, 
 #pragma unroll
                     for (int i = 0; i < OCT; ++i) { const float nx = fmaf(x2[i], pc[i], -pp[i]); pp[i] = pc[i]; pc[i] = nx; }
                 }
-                const float tot = xreduce32(X, c.lane);
-                const int slot = n0 + (c.lane >> 2);
-                if (first) red[slot * GS + (c.lane & 3)] = tot; else red[slot * GS + (c.lane & 3)] += tot;
+                const float tot = xreduce32(X, V1_LANE);
+                const int slot = n0 + (V1_LANE >> 2);
+                if (first) red[slot * GS + (V1_LANE & 3)] = tot; else red[slot * GS + (V1_LANE & 3)] += tot;
             }
         } else {
             // right-hand side only, eight n per transpose
@@ -430,9 +469,9 @@ __device__ __noinline__ void v1_phase_forward(const V1Ctx &c, const SegDev &sg, 
 #pragma unroll
                     for (int i = 0; i < OCT; ++i) { const float nx = fmaf(x2[i], pc[i], -pp[i]); pp[i] = pc[i]; pc[i] = nx; }
                 }
-                const float tot = xreduce32(X, c.lane);
-                const int slot = nmomr + n0 + (c.lane >> 2);
-                if (first) red[slot * GS + (c.lane & 3)] = tot; else red[slot * GS + (c.lane & 3)] += tot;
+                const float tot = xreduce32(X, V1_LANE);
+                const int slot = nmomr + n0 + (V1_LANE >> 2);
+                if (first) red[slot * GS + (V1_LANE & 3)] = tot; else red[slot * GS + (V1_LANE & 3)] += tot;
             }
         }
     }
@@ -448,11 +487,11 @@ __device__ __noinline__ void v1_phase_forward(const V1Ctx &c, const SegDev &sg, 
 // ------------------------------------------------------------------------------------------
 #define V1_LFS (32 * 33 + 32)
 
-__device__ __noinline__ void v1_phase_solve(const V1Ctx &c, int g, int seg, bool refactor)
+__device__ __noinline__ void v1_phase_solve(int g, int seg, bool refactor)
 {
-    const ModelDev &M = *c.M;
-    const V1Lay &L = *c.L;
-    const int n1 = M.n1, lane = c.lane, rowB = seg * M.n1;
+    const ModelDev &M = v1_blk.M;
+    const V1Lay &L = v1_blk.L;
+    const int n1 = M.n1, lane = V1_LANE, rowB = seg * M.n1;
     float *momS = V1SM + L.oMOM + g * L.nmomr;
     float *rhsS = V1SM + L.oRHS + g * L.n1r;
     float *lf = V1SM + L.oLF + g * V1_LFS;
@@ -504,7 +543,7 @@ __device__ __noinline__ void v1_phase_solve(const V1Ctx &c, int g, int seg, bool
         for (int j = 0; j < 32; ++j) lf[lane * 33 + j] = row[j];
         __syncwarp();
         invd[lane] = 1.f / lf[lane * 33 + lane];
-        if (lane == 0) SMV(c, L.oSC, SC_N + seg, g) = ok ? 0.f : 1.f;
+        if (lane == 0) SMV(L.oSC, SC_N + seg, g) = ok ? 0.f : 1.f;
         __syncwarp();
         // store the factor column-scaled to unit diagonal, Lt = L D^-1 (D = diag L): the two triangular
         // solves of every step then have a shuffle + one FMA on their serial chain and no division;
@@ -521,7 +560,7 @@ __device__ __noinline__ void v1_phase_solve(const V1Ctx &c, int g, int seg, bool
         }
     }
     __syncwarp();
-    const bool ok = SMV(c, L.oSC, SC_N + seg, g) == 0.f;
+    const bool ok = SMV(L.oSC, SC_N + seg, g) == 0.f;
     float r = (lane < n1) ? rhsS[lane] : 0.f;
     for (int k = 0; k < n1; ++k) {            // Lt z = rhs (unit diagonal)
         const float zk = __shfl_sync(FULL, r, k);
@@ -533,8 +572,8 @@ __device__ __noinline__ void v1_phase_solve(const V1Ctx &c, int g, int seg, bool
         if (lane < k) r = fmaf(-lf[k * 33 + lane], xk, r);
     }
     if (lane < n1) {
-        if (ok) SMV(c, L.oB, rowB + lane, g) += r;
-        else SMV(c, L.oB, rowB + lane, g) = 0.f;
+        if (ok) SMV(L.oB, rowB + lane, g) += r;
+        else SMV(L.oB, rowB + lane, g) = 0.f;
     }
     __syncwarp();
 }
@@ -547,23 +586,24 @@ __device__ __noinline__ void v1_phase_solve(const V1Ctx &c, int g, int seg, bool
 // chi2 / ngood / cmin are reduced over the warp and accumulated in this warp's SLOT_STAT slots (zeroed by v1_evaluate).
 // ------------------------------------------------------------------------------------------
 template <int MODE>
-__device__ __noinline__ void v1_phase_residual(const V1Ctx &c, const SegDev &sg, const V1Args &a, int rowB, float *xrow)
+__device__ __noinline__ void v1_phase_residual(const SegDev &sg, int rowB, float *xrow)
 {
-    const V1Lay &L = *c.L;
+    const V1Args &a = v1_blk.A;
+    const V1Lay &L = v1_blk.L;
     const float4 *b4 = (const float4 *)(V1SM + L.oB) + rowB;
-    const int Ppad = c.M->Ppad, n1 = c.M->n1, RL = L.RL, nt8 = c.nt * OCT;
+    const int Ppad = v1_blk.M.Ppad, n1 = v1_blk.M.n1, RL = L.RL, nt8 = V1_NT * OCT;
     const int fit_lo = sg.fit_lo, fit_hi = sg.fit_hi, torg = sg.po + sg.halo;
     const float ta = sg.ta, tb = sg.tb;
     float *rowA = V1SM + L.oA + L.GUARD - sg.po;
     const float *Yg = a.Y, *Wg = a.W;
-    float *cpg = c.cp;
+    float *cpg = v1_blk.cp;
     size_t rowo[GS];
 #pragma unroll
-    for (int g = 0; g < GS; ++g) rowo[g] = (size_t)c.spec[g] * Ppad;
+    for (int g = 0; g < GS; ++g) rowo[g] = (size_t)v1_blk.spec[g] * Ppad;
     float chi[GS], ng[GS], cmin[GS];
 #pragma unroll
     for (int g = 0; g < GS; ++g) { chi[g] = 0.f; ng[g] = 0.f; cmin[g] = 3.0e38f; }
-    for (int j0 = fit_lo + c.tid * OCT; j0 < fit_hi; j0 += nt8) {
+    for (int j0 = fit_lo + V1_TID * OCT; j0 < fit_hi; j0 += nt8) {
         float cc[GS][OCT], pp[OCT], pc[OCT], x2[OCT];
         float4 yq[GS][2], wq[GS][2];   // flux / weight from L2, issued before the basis loop hides them
         if (MODE != 0) {
@@ -625,11 +665,11 @@ __device__ __noinline__ void v1_phase_residual(const V1Ctx &c, const SegDev &sg,
         }
     }
     if (MODE != 0) {
-        float *red = V1SM + L.oRED + c.warp * L.VR * GS;
+        float *red = V1SM + L.oRED + V1_WARP * L.VR * GS;
 #pragma unroll
         for (int g = 0; g < GS; ++g) {
             const float s = warp_sum_f(chi[g]), n = warp_sum_f(ng[g]), m = warp_min_f(cmin[g]);
-            if (c.lane == 0) {
+            if (V1_LANE == 0) {
                 float *st = red + SLOT_STAT(L) * GS + g;
                 st[0] += s; st[GS] += n; st[2 * GS] = fminf(st[2 * GS], m);
             }
@@ -645,22 +685,22 @@ __device__ __noinline__ void v1_phase_residual(const V1Ctx &c, const SegDev &sg,
 // Partial sums go through register transposes into this warp's Q slots (pseudo-terms K, K+1 carry
 // the two kernel-parameter gradients), which v1_evaluate zeroed.
 // ------------------------------------------------------------------------------------------
-__device__ __noinline__ void v1_phase_adjoint(const V1Ctx &c, const SegDev &sg, int lo, int hi)
+__device__ __noinline__ void v1_phase_adjoint(const SegDev &sg, int lo, int hi)
 {
-    const V1Lay &L = *c.L;
+    const V1Lay &L = v1_blk.L;
     const int *tap = (const int *)(V1SM + L.oTAP);
-    const int P4 = c.M->Ppad >> 2, K = c.M->K, Kq = L.Kq, NA = L.NA, RL = L.RL, nt8 = c.nt * OCT;
+    const int P4 = v1_blk.M.Ppad >> 2, K = v1_blk.M.K, Kq = L.Kq, NA = L.NA, RL = L.RL, nt8 = V1_NT * OCT;
     const int wstride4 = GS * NA;   // float4 stride between the three reversed kernels
     const int qslot0 = SLOT_Q(L, 0);
-    float *red = V1SM + L.oRED + c.warp * L.VR * GS;
-    const float *Cg = c.M->C;
+    float *red = V1SM + L.oRED + V1_WARP * L.VR * GS;
+    const float *Cg = v1_blk.M.C;
     const float *rowA = V1SM + L.oA + L.GUARD - sg.po, *rowT = V1SM + L.oT + L.GUARD - sg.po;
     const float4 *gr4 = (const float4 *)(V1SM + L.oGR);
     int alo[GS], nag[GS];
 #pragma unroll
     for (int g = 0; g < GS; ++g) { alo[g] = tap[2 * g]; nag[g] = tap[2 * g + 1]; }
     for (int jb = lo; jb < hi; jb += nt8) {
-        const int j0 = jb + c.tid * OCT;
+        const int j0 = jb + V1_TID * OCT;
         const bool act = j0 < hi;
         float t[GS][OCT], gv[GS], gs[GS];
 #pragma unroll
@@ -714,15 +754,19 @@ __device__ __noinline__ void v1_phase_adjoint(const V1Ctx &c, const SegDev &sg, 
             load4(k0 + 4, bufB);
             dot4(0, bufA);
             load4(k0 + 8, bufA);
-            dot4(16, bufB);
+            if (k0 + 4 < Kq) dot4(16, bufB);
+            else {
+#pragma unroll
+                for (int i = 16; i < 32; ++i) X[i] = 0.f;
+            }
             if (k0 + 8 > K) {   // uniform: the block holding rows K and K+1 (K+1 < Kq always)
 #pragma unroll
                 for (int kk = 0; kk < 8; ++kk)
 #pragma unroll
                     for (int g = 0; g < GS; ++g) X[kk * 4 + g] += (k0 + kk == K) ? gv[g] : ((k0 + kk == K + 1) ? gs[g] : 0.f);
             }
-            const float tot = xreduce32(X, c.lane);
-            red[(qslot0 + k0 + (c.lane >> 2)) * GS + (c.lane & 3)] += tot;
+            const float tot = xreduce32(X, V1_LANE);
+            red[(qslot0 + k0 + (V1_LANE >> 2)) * GS + (V1_LANE & 3)] += tot;
         }
     }
 }
@@ -737,24 +781,25 @@ __device__ __noinline__ void v1_phase_adjoint(const V1Ctx &c, const SegDev &sg, 
 // for MODE 0, the q / dv / dsigma partials.
 // ------------------------------------------------------------------------------------------
 template <int MODE>
-__device__ __noinline__ void v1_evaluate(const V1Ctx &c, const V1Args &a, bool cold, bool mom, float *xrow)
+__device__ __noinline__ void v1_evaluate(bool cold, bool mom, float *xrow)
 {
-    const ModelDev &M = *c.M;
-    const V1Lay &L = *c.L;
+    const V1Args &a = v1_blk.A;
+    const ModelDev &M = v1_blk.M;
+    const V1Lay &L = v1_blk.L;
     // This warp's Q and statistics slots accumulate over sweeps and segments.  They are zeroed after
     // the first barrier of the evaluation: only then have warps g < GS finished reading the previous
     // evaluation's slots (v1_gradient / v1_stats run between evaluations without a barrier).
     long long tk = a.dbg ? clock64() : 0;
     auto tick = [&](int i) {
-        if (a.dbg && c.tid == 0) { const long long t = clock64(); atomicAdd(a.dbg + i, (unsigned long long)(t - tk)); tk = t; }
+        if (a.dbg && V1_TID == 0) { const long long t = clock64(); atomicAdd(a.dbg + i, (unsigned long long)(t - tk)); tk = t; }
     };
     bool zeroed = false;
     auto zero_slots = [&]() {
-        float *red = V1SM + L.oRED + c.warp * L.VR * GS;
+        float *red = V1SM + L.oRED + V1_WARP * L.VR * GS;
         const int q0 = (L.nmomr + L.n1r) * GS;
-        for (int i = q0 + c.lane; i < L.VR * GS; i += 32) red[i] = 0.f;
+        for (int i = q0 + V1_LANE; i < L.VR * GS; i += 32) red[i] = 0.f;
         __syncwarp();
-        if (c.lane < GS) red[(SLOT_STAT(L) + 2) * GS + c.lane] = 3.0e38f;
+        if (V1_LANE < GS) red[(SLOT_STAT(L) + 2) * GS + V1_LANE] = 3.0e38f;
         __syncwarp();
         zeroed = true;
     };
@@ -762,57 +807,57 @@ __device__ __noinline__ void v1_evaluate(const V1Ctx &c, const V1Args &a, bool c
         const SegDev &sg = M.seg[s];
         const int rowB = s * M.n1;
         if (sg.fit_hi <= sg.fit_lo) {
-            if (c.warp < GS) {   // no fitted pixel: b = 0, not positive definite (as the oracle)
-                for (int n = c.lane; n < M.n1; n += 32) SMV(c, L.oB, rowB + n, c.warp) = 0.f;
-                if (c.lane == 0) SMV(c, L.oSC, SC_N + s, c.warp) = 1.f;
+            if (V1_WARP < GS) {   // no fitted pixel: b = 0, not positive definite (as the oracle)
+                for (int n = V1_LANE; n < M.n1; n += 32) SMV(L.oB, rowB + n, V1_WARP) = 0.f;
+                if (V1_LANE == 0) SMV(L.oSC, SC_N + s, V1_WARP) = 1.f;
             }
             continue;
         }
-        if (c.warp < GS) {
-            v1_setup_weights(c, sg, c.warp);
-            if (cold) for (int n = c.lane; n < M.n1; n += 32) SMV(c, L.oB, rowB + n, c.warp) = 0.f;
+        if (V1_WARP < GS) {
+            v1_setup_weights(sg, V1_WARP);
+            if (cold) for (int n = V1_LANE; n < M.n1; n += 32) SMV(L.oB, rowB + n, V1_WARP) = 0.f;
         }
         if (M.n_seg > 1 || cold) {
             // row A must be zero outside the fitted range of THIS segment (the adjoint stencil reads it)
-            for (int i = c.tid; i < GS * L.RL / 4; i += c.nt) ((float4 *)(V1SM + L.oA))[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+            for (int i = V1_TID; i < GS * L.RL / 4; i += V1_NT) ((float4 *)(V1SM + L.oA))[i] = make_float4(0.f, 0.f, 0.f, 0.f);
         }
         if (cold) {
             for (int g = 0; g < GS; ++g)
-                for (int j = sg.fit_lo + c.tid * 4; j < sg.fit_hi; j += c.nt * 4)
-                    *(float4 *)(c.cp + (size_t)g * M.Ppad + j) = make_float4(0.f, 0.f, 0.f, 0.f);
+                for (int j = sg.fit_lo + V1_TID * 4; j < sg.fit_hi; j += V1_NT * 4)
+                    *(float4 *)(v1_blk.cp + (size_t)g * M.Ppad + j) = make_float4(0.f, 0.f, 0.f, 0.f);
         }
         tick(0);
         __syncthreads();
         tick(1);
         if (!zeroed) zero_slots();
         int lo, hi;
-        v1_group_range(c, sg, lo, hi);
-        v1_phase_emulator(c, sg, lo, hi);
+        v1_group_range(sg, lo, hi);
+        v1_phase_emulator(sg, lo, hi);
         tick(2);
         __syncthreads();
         tick(3);
-        v1_phase_forward(c, sg, a, true, mom || cold);
+        v1_phase_forward(sg, true, mom || cold);
         tick(4);
         __syncthreads();
         tick(5);
-        if (c.warp < GS) v1_phase_solve(c, c.warp, s, mom || cold);
+        if (V1_WARP < GS) v1_phase_solve(V1_WARP, s, mom || cold);
         tick(6);
         __syncthreads();
         tick(7);
         if (cold) {
-            v1_phase_residual<0>(c, sg, a, rowB, nullptr);
+            v1_phase_residual<0>(sg, rowB, nullptr);
             __syncthreads();   // c_prev written by this thread only, but keep phases aligned
-            v1_phase_forward(c, sg, a, false, false);
+            v1_phase_forward(sg, false, false);
             __syncthreads();
-            if (c.warp < GS) v1_phase_solve(c, c.warp, s, false);
+            if (V1_WARP < GS) v1_phase_solve(V1_WARP, s, false);
             __syncthreads();
         }
-        v1_phase_residual<(MODE == 2 ? 2 : 1)>(c, sg, a, rowB, xrow);
+        v1_phase_residual<(MODE == 2 ? 2 : 1)>(sg, rowB, xrow);
         tick(8);
         __syncthreads();
         tick(9);
         if (MODE == 0) {
-            v1_phase_adjoint(c, sg, lo, hi);
+            v1_phase_adjoint(sg, lo, hi);
             tick(10);
             __syncthreads();
             tick(11);
@@ -826,9 +871,9 @@ __device__ __noinline__ void v1_evaluate(const V1Ctx &c, const V1Args &a, bool c
 }
 
 // sums of the per-warp statistics for spectrum g (any lane may call; all return the same)
-__device__ __forceinline__ void v1_stats(const V1Ctx &c, int g, float &chi2, float &ngood, float &cmin)
+__device__ __forceinline__ void v1_stats(int g, float &chi2, float &ngood, float &cmin)
 {
-    const V1Lay &L = *c.L;
+    const V1Lay &L = v1_blk.L;
     const float *red = V1SM + L.oRED + SLOT_STAT(L) * GS + g;
     chi2 = 0.f; ngood = 0.f; cmin = 3.0e38f;
     for (int w = 0; w < L.NW; ++w) {
@@ -838,120 +883,103 @@ __device__ __forceinline__ void v1_stats(const V1Ctx &c, int g, float &chi2, flo
 }
 
 // a7 (tail) + chain rule to u (C.1 last lines).  Warp g; grad[p] valid on lane p afterwards.
-__device__ __noinline__ float v1_gradient(const V1Ctx &c, int g)
+__device__ __noinline__ float v1_gradient(int g)
 {
-    const ModelDev &M = *c.M;
-    const V1Lay &L = *c.L;
+    const ModelDev &M = v1_blk.M;
+    const V1Lay &L = v1_blk.L;
     const float *red = V1SM + L.oRED;
-    const int wst = L.VR * GS;
-    for (int k = c.lane; k < M.K + 2; k += 32) {
+    const int wst = L.VR * GS, nl = M.L, K = M.K, NW = L.NW, q0 = SLOT_Q(L, 0);
+    for (int k = V1_LANE; k < K + 2; k += 32) {
         float s = 0.f;
-        for (int w = 0; w < L.NW; ++w) s += red[w * wst + SLOT_Q(L, k) * GS + g];
-        SMV(c, L.oQ, k, g) = s;
+        for (int w = 0; w < NW; ++w) s += red[w * wst + (q0 + k) * GS + g];
+        SMV(L.oQ, k, g) = s;
     }
     __syncwarp();
     float mine = 0.f;
-    const uint8_t *ex = (const uint8_t *)(V1SM + L.oEXP);
-    for (int l = 0; l < M.L; ++l) {
+    for (int l = 0; l < nl; ++l) {      // d chi2 / d x_l = sum_k (d phi_k / d x_l) q_k
         float gx = 0.f;
-        for (int k = c.lane; k < M.K; k += 32) {
-            const int el = ex[k * M.L + l];
-            if (el == 0) continue;
-            float d = (float)el;
-            for (int l2 = 0; l2 < M.L; ++l2) {
-                const int e2 = ex[k * M.L + l2] - (l2 == l ? 1 : 0);
-                const float x = SMV(c, L.oX, l2, g);
-                for (int q = 0; q < e2; ++q) d *= x;
-            }
-            gx = fmaf(d, SMV(c, L.oQ, k, g), gx);
-        }
+        for (int k = V1_LANE; k < K; k += 32) gx = fmaf(SMV(L.oDPHI, l * K + k, g), SMV(L.oQ, k, g), gx);
         gx = warp_sum_f(gx);
-        const float u = SMV(c, L.oU, l, g);
-        const float half = (M.hi[l] - M.lo[l]) * 0.5f;
-        const float th = M.lo[l] + (u + 1.f) * half;
-        const float dxdt = M.label_log10[l] ? M.emu_a[l] / (th * 2.302585093f) : M.emu_a[l];
-        if (c.lane == l) mine = gx * dxdt * half;
+        if (V1_LANE == l) mine = gx;
     }
-    if (c.lane == M.L) mine = SMV(c, L.oQ, M.K, g) * (M.hi[M.L] - M.lo[M.L]) * 0.5f;
-    if (c.lane == M.L + 1) mine = SMV(c, L.oQ, M.K + 1, g) * (M.hi[M.L + 1] - M.lo[M.L + 1]) * 0.5f;
+    if (V1_LANE == nl) mine = SMV(L.oQ, K, g);
+    if (V1_LANE == nl + 1) mine = SMV(L.oQ, K + 1, g);
+    if (V1_LANE < M.NP) mine *= SMV(L.oGSC, V1_LANE, g);   // chain rule to u (C.1 last lines)
     return mine;
 }
 
 // internal Chebyshev(t) coefficients -> plain Legendre(x^) (C.2-8), fp64.  Warp g, lanes over rows.
-__device__ __noinline__ void v1_write_cont(const V1Ctx &c, int g, float *out)
+__device__ __noinline__ void v1_write_cont(int g, float *out)
 {
-    const ModelDev &M = *c.M;
+    const ModelDev &M = v1_blk.M;
     for (int s = 0; s < M.n_seg; ++s) {
         const double *cv = M.conv + (size_t)s * M.n1 * M.n1;
-        for (int m = c.lane; m < M.n1; m += 32) {
+        for (int m = V1_LANE; m < M.n1; m += 32) {
             double acc = 0.0;
-            for (int n = 0; n < M.n1; ++n) acc += cv[m * M.n1 + n] * (double)SMV(c, c.L->oB, s * M.n1 + n, g);
+            for (int n = 0; n < M.n1; ++n) acc += cv[m * M.n1 + n] * (double)SMV(v1_blk.L.oB, s * M.n1 + n, g);
             out[s * M.n1 + m] = (float)acc;
         }
     }
 }
 
-__device__ __forceinline__ void v1_make_ctx(V1Ctx &c, const ModelDev &M, const V1Lay &L, const V1Args &a)
+// copy the kernel parameters into the block state (a pointer to a kernel parameter is a generic load from
+// the parameter window; a struct passed by reference to a non-inlined function is a local-memory copy)
+__device__ __forceinline__ void v1_init_block(const ModelDev &M, const V1Lay &L, const V1Args &a)
 {
-    // the model description is read by every phase through pointers: keep a copy in shared memory (a pointer
-    // to the kernel parameters is a generic load from the parameter window with global-memory latency)
-    __shared__ ModelDev sM;
-    __shared__ V1Lay sL;
-    for (int i = threadIdx.x; i < (int)(sizeof(ModelDev) / 4); i += blockDim.x) ((int *)&sM)[i] = ((const int *)&M)[i];
-    for (int i = threadIdx.x; i < (int)(sizeof(V1Lay) / 4); i += blockDim.x) ((int *)&sL)[i] = ((const int *)&L)[i];
-    c.M = &sM; c.L = &sL;
-    c.tid = threadIdx.x; c.lane = threadIdx.x & 31; c.warp = threadIdx.x >> 5; c.nt = blockDim.x;
-    c.cp = a.CP + (size_t)blockIdx.x * GS * M.Ppad;
+    for (int i = threadIdx.x; i < (int)(sizeof(ModelDev) / 4); i += blockDim.x) ((int *)&v1_blk.M)[i] = ((const int *)&M)[i];
+    for (int i = threadIdx.x; i < (int)(sizeof(V1Lay) / 4); i += blockDim.x) ((int *)&v1_blk.L)[i] = ((const int *)&L)[i];
+    for (int i = threadIdx.x; i < (int)(sizeof(V1Args) / 4); i += blockDim.x) ((int *)&v1_blk.A)[i] = ((const int *)&a)[i];
+    if (threadIdx.x == 0) v1_blk.cp = a.CP + (size_t)blockIdx.x * GS * M.Ppad;
     for (int i = threadIdx.x; i < M.K * M.L; i += blockDim.x) ((uint8_t *)(V1SM + L.oEXP))[i] = M.exps[i];
     for (int i = threadIdx.x; i < GS * L.Kq; i += blockDim.x) V1SM[L.oPHI + i] = 0.f;   // phi is zero past K
     __syncthreads();
 }
 
-__device__ __forceinline__ void v1_set_group(V1Ctx &c, const V1Args &a, int grp)
+__device__ __forceinline__ void v1_set_group(int grp)
 {
-#pragma unroll
-    for (int g = 0; g < GS; ++g) {
-        long long i = (long long)grp * GS + g;
-        c.spec[g] = i < a.B ? i : a.B - 1;
+    if (threadIdx.x < GS) {
+        const long long i = (long long)grp * GS + threadIdx.x;
+        v1_blk.spec[threadIdx.x] = i < v1_blk.A.B ? i : v1_blk.A.B - 1;
     }
 }
 
 // a9: error estimate (C.2-22/23).  J by central differences of the re-solved whitened
 // residual rho(u), Sigma = rho^T rho/(N_good - NP) (J^T J)^-1, err_p = sqrt(Sigma_pp) (hi_p - lo_p)/2.
-__device__ __noinline__ void v1_errors(V1Ctx &c, const V1Args &a, float chi2_g, float ngood_g, bool valid_g)
+__device__ __noinline__ void v1_errors(float chi2_g, float ngood_g, bool valid_g)
 {
-    const ModelDev &M = *c.M;
-    const V1Lay &L = *c.L;
+    const V1Args &a = v1_blk.A;
+    const ModelDev &M = v1_blk.M;
+    const V1Lay &L = v1_blk.L;
     const int NP = M.NP;
     const size_t plane = (size_t)GS * M.Ppad;
     float *xj = a.XJ + (size_t)blockIdx.x * (1 + NP) * plane;
     for (int p = 0; p < NP; ++p) {
         float u0 = 0.f;
-        if (c.warp < GS) {
-            u0 = SMV(c, L.oU, p, c.warp);
+        if (V1_WARP < GS) {
+            u0 = SMV(L.oU, p, V1_WARP);
             __syncwarp();
-            if (c.lane == 0) SMV(c, L.oU, p, c.warp) = u0 + a.fd_h;
+            if (V1_LANE == 0) SMV(L.oU, p, V1_WARP) = u0 + a.fd_h;
             __syncwarp();
-            v1_param_setup(c, c.warp);
+            v1_param_setup(V1_WARP);
         }
-        v1_evaluate<2>(c, a, false, true, xj);
-        if (c.warp < GS) {
-            if (c.lane == 0) SMV(c, L.oU, p, c.warp) = u0 - a.fd_h;
+        v1_evaluate<2>(false, true, xj);
+        if (V1_WARP < GS) {
+            if (V1_LANE == 0) SMV(L.oU, p, V1_WARP) = u0 - a.fd_h;
             __syncwarp();
-            v1_param_setup(c, c.warp);
+            v1_param_setup(V1_WARP);
         }
-        v1_evaluate<2>(c, a, false, true, xj + (1 + p) * plane);
-        if (c.warp < GS) {
-            if (c.lane == 0) SMV(c, L.oU, p, c.warp) = u0;
+        v1_evaluate<2>(false, true, xj + (1 + p) * plane);
+        if (V1_WARP < GS) {
+            if (V1_LANE == 0) SMV(L.oU, p, V1_WARP) = u0;
             __syncwarp();
         }
         __syncthreads();
         // J_p = (rho+ - rho-)/(u+ - u-) on the pixels this thread owns (it wrote both)
         for (int s = 0; s < M.n_seg; ++s) {
             const SegDev &sg = M.seg[s];
-            for (int j0 = sg.fit_lo + c.tid * OCT; j0 < sg.fit_hi; j0 += c.nt * OCT)
+            for (int j0 = sg.fit_lo + V1_TID * OCT; j0 < sg.fit_hi; j0 += V1_NT * OCT)
                 for (int g = 0; g < GS; ++g) {
-                    const float uu = SMV(c, L.oU, p, g);
+                    const float uu = SMV(L.oU, p, g);
                     const float inv = 1.f / ((uu + a.fd_h) - (uu - a.fd_h));
                     float4 *jp = (float4 *)(xj + (1 + p) * plane + (size_t)g * M.Ppad + j0);
                     const float4 *xp = (const float4 *)(xj + (size_t)g * M.Ppad + j0);
@@ -967,12 +995,12 @@ __device__ __noinline__ void v1_errors(V1Ctx &c, const V1Args &a, float chi2_g, 
     // N = J^T J (packed lower), fp64 accumulation across warps in shared memory (aliases the factor area)
     double *N = (double *)(V1SM + L.oLF);
     const int npair = NP * (NP + 1) / 2;
-    for (int i = c.tid; i < GS * npair; i += c.nt) N[i] = 0.0;
+    for (int i = V1_TID; i < GS * npair; i += V1_NT) N[i] = 0.0;
     __syncthreads();
     for (int s = 0; s < M.n_seg; ++s) {
         const SegDev &sg = M.seg[s];
-        for (int jb = sg.fit_lo; jb < sg.fit_hi; jb += c.nt * OCT) {
-            const int j0 = jb + c.tid * OCT;
+        for (int jb = sg.fit_lo; jb < sg.fit_hi; jb += V1_NT * OCT) {
+            const int j0 = jb + V1_TID * OCT;
             const bool act = j0 < sg.fit_hi;
             for (int pi0 = 0; pi0 < npair; pi0 += 8) {
                 float X[32];
@@ -995,15 +1023,15 @@ __device__ __noinline__ void v1_errors(V1Ctx &c, const V1Args &a, float chi2_g, 
                         X[kk * 4 + g] = sacc;
                     }
                 }
-                const float tot = xreduce32(X, c.lane);
-                const int pi = pi0 + (c.lane >> 2);
-                if (pi < npair) atomicAdd(&N[(c.lane & 3) * npair + pi], (double)tot);
+                const float tot = xreduce32(X, V1_LANE);
+                const int pi = pi0 + (V1_LANE >> 2);
+                if (pi < npair) atomicAdd(&N[(V1_LANE & 3) * npair + pi], (double)tot);
             }
         }
     }
     __syncthreads();
-    if (c.warp < GS && c.lane == 0) {
-        const int g = c.warp;
+    if (V1_WARP < GS && V1_LANE == 0) {
+        const int g = V1_WARP;
         double *Ng = N + g * npair;
         bool ok = ngood_g > (float)NP;
         for (int p = 0; p < NP && ok; ++p)
@@ -1030,7 +1058,7 @@ __device__ __noinline__ void v1_errors(V1Ctx &c, const V1Args &a, float chi2_g, 
                 }
                 e = (float)(sqrt(s2 * nrm) * (double)(M.hi[p] - M.lo[p]) * 0.5);
             }
-            if (valid_g) a.err[c.spec[g] * NP + p] = e;
+            if (valid_g) a.err[v1_blk.spec[g] * NP + p] = e;
         }
     }
     __syncthreads();
@@ -1043,84 +1071,83 @@ template <int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB)
 lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V1Lay L, const V1Args a)
 {
-    V1Ctx c;
-    v1_make_ctx(c, M, L, a);
-    const int NP = M.NP, g = c.warp;
+    v1_init_block(M, L, a);
+    const int NP = M.NP, g = V1_WARP;
     for (int grp = blockIdx.x; grp < a.ngroups; grp += gridDim.x) {
-        v1_set_group(c, a, grp);
+        v1_set_group(grp);
         __syncthreads();   // the previous group's last readers are done with shared memory
         const bool valid = g < GS && (long long)grp * GS + g < a.B;
         if (g < GS) {
-            for (int p = c.lane; p < NP; p += 32) {
-                const float th = a.init[c.spec[g] * NP + p];
+            for (int p = V1_LANE; p < NP; p += 32) {
+                const float th = a.init[v1_blk.spec[g] * NP + p];
                 const float u = 2.f * (th - M.lo[p]) / (M.hi[p] - M.lo[p]) - 1.f;
-                SMV(c, L.oU, p, g) = fminf(fmaxf(u, -1.f), 1.f);
-                SMV(c, L.oM, p, g) = 0.f;
-                SMV(c, L.oV, p, g) = 0.f;
+                SMV(L.oU, p, g) = fminf(fmaxf(u, -1.f), 1.f);
+                SMV(L.oM, p, g) = 0.f;
+                SMV(L.oV, p, g) = 0.f;
             }
             __syncwarp();
-            v1_param_setup(c, g);
+            v1_param_setup(g);
         }
         float pb1 = 1.f, pb2 = 1.f;
         for (int t = 1; t <= a.n_iter; ++t) {
             const long long te0 = a.dbg ? clock64() : 0;
-            v1_evaluate<0>(c, a, t == 1, (t - 1) % L.refresh == 0, nullptr);
-            if (a.dbg && c.tid == 0) { atomicAdd(a.dbg + 14, (unsigned long long)(clock64() - te0)); atomicAdd(a.dbg + 15, 1ull); }
+            v1_evaluate<0>(t == 1, (t - 1) % L.refresh == 0, nullptr);
+            if (a.dbg && V1_TID == 0) { atomicAdd(a.dbg + 14, (unsigned long long)(clock64() - te0)); atomicAdd(a.dbg + 15, 1ull); }
             const long long tu0 = a.dbg ? clock64() : 0;
             pb1 *= a.b1; pb2 *= a.b2;
             if (g < GS) {
-                const float gr = v1_gradient(c, g);
+                const float gr = v1_gradient(g);
                 // a8: Adam (C.2-20), then clip to the prior box (C.2-18); lane p owns parameter p
                 for (int p0 = 0; p0 < NP; p0 += 32) {   // NP <= 32
-                    const int p = p0 + c.lane;
+                    const int p = p0 + V1_LANE;
                     if (p < NP) {
-                        const float m = a.b1 * SMV(c, L.oM, p, g) + (1.f - a.b1) * gr;
-                        const float v = a.b2 * SMV(c, L.oV, p, g) + (1.f - a.b2) * gr * gr;
-                        SMV(c, L.oM, p, g) = m; SMV(c, L.oV, p, g) = v;
+                        const float m = a.b1 * SMV(L.oM, p, g) + (1.f - a.b1) * gr;
+                        const float v = a.b2 * SMV(L.oV, p, g) + (1.f - a.b2) * gr * gr;
+                        SMV(L.oM, p, g) = m; SMV(L.oV, p, g) = v;
                         const float mh = m / (1.f - pb1), vh = v / (1.f - pb2);
-                        float u = SMV(c, L.oU, p, g) - a.lr * mh / (sqrtf(vh) + a.eps);
-                        if (!(u == u)) u = SMV(c, L.oU, p, g);   // keep the iterate if the gradient was NaN
-                        SMV(c, L.oU, p, g) = fminf(fmaxf(u, -1.f), 1.f);
+                        float u = SMV(L.oU, p, g) - a.lr * mh / (sqrtf(vh) + a.eps);
+                        if (!(u == u)) u = SMV(L.oU, p, g);   // keep the iterate if the gradient was NaN
+                        SMV(L.oU, p, g) = fminf(fmaxf(u, -1.f), 1.f);
                     }
                 }
                 __syncwarp();
-                v1_param_setup(c, g);
+                v1_param_setup(g);
             }
-            if (a.dbg && c.tid == 0) atomicAdd(a.dbg + 13, (unsigned long long)(clock64() - tu0));
+            if (a.dbg && V1_TID == 0) atomicAdd(a.dbg + 13, (unsigned long long)(clock64() - tu0));
         }
         // a9: one more evaluation at the final iterate (C.2-21)
-        v1_evaluate<1>(c, a, a.n_iter == 0, true, nullptr);
+        v1_evaluate<1>(a.n_iter == 0, true, nullptr);
         float chi2 = 0.f, ngood = 0.f, cmin = 0.f;
         if (g < GS) {
-            v1_stats(c, g, chi2, ngood, cmin);
+            v1_stats(g, chi2, ngood, cmin);
             int st = 0;
             bool fin = isfinite(chi2);
             bool bound = false;
-            for (int p = c.lane; p < NP; p += 32) {
-                const float u = SMV(c, L.oU, p, g);
+            for (int p = V1_LANE; p < NP; p += 32) {
+                const float u = SMV(L.oU, p, g);
                 fin = fin && isfinite(u);
                 bound = bound || (u <= -1.f || u >= 1.f);
             }
-            for (int n = c.lane; n < M.nc; n += 32) fin = fin && isfinite(SMV(c, L.oB, n, g));
+            for (int n = V1_LANE; n < M.nc; n += 32) fin = fin && isfinite(SMV(L.oB, n, g));
             fin = __all_sync(FULL, fin);
             bound = __any_sync(FULL, bound);
-            const bool anyfail = __any_sync(FULL, c.lane < M.n_seg && V1SM[L.oSC + (SC_N + c.lane) * GS + g] != 0.f);
+            const bool anyfail = __any_sync(FULL, V1_LANE < M.n_seg && V1SM[L.oSC + (SC_N + V1_LANE) * GS + g] != 0.f);
             if (anyfail) st |= LASP_ST_NOT_SPD;
             if (bound) st |= LASP_ST_ON_BOUND;
             if (!fin) st |= LASP_ST_NONFINITE;
             if (ngood > 0.f && cmin <= 0.f) st |= LASP_ST_NEG_CONT;
             if (valid) {
-                const long long i = c.spec[g];
-                for (int p = c.lane; p < NP; p += 32)
-                    a.params[i * NP + p] = M.lo[p] + (SMV(c, L.oU, p, g) + 1.f) * (M.hi[p] - M.lo[p]) * 0.5f;
-                if (c.lane == 0) {
+                const long long i = v1_blk.spec[g];
+                for (int p = V1_LANE; p < NP; p += 32)
+                    a.params[i * NP + p] = M.lo[p] + (SMV(L.oU, p, g) + 1.f) * (M.hi[p] - M.lo[p]) * 0.5f;
+                if (V1_LANE == 0) {
                     a.chi2[i] = chi2;
                     if (a.status) a.status[i] = st;
                 }
-                if (a.cont) v1_write_cont(c, g, a.cont + i * M.nc);
+                if (a.cont) v1_write_cont(g, a.cont + i * M.nc);
             }
         }
-        if (a.err) v1_errors(c, a, chi2, ngood, valid);
+        if (a.err) v1_errors(chi2, ngood, valid);
     }
 }
 
@@ -1131,33 +1158,32 @@ template <int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB)
 lasp_v1_grad_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V1Lay L, const V1Args a)
 {
-    V1Ctx c;
-    v1_make_ctx(c, M, L, a);
-    const int NP = M.NP, g = c.warp;
+    v1_init_block(M, L, a);
+    const int NP = M.NP, g = V1_WARP;
     for (int grp = blockIdx.x; grp < a.ngroups; grp += gridDim.x) {
-        v1_set_group(c, a, grp);
+        v1_set_group(grp);
         __syncthreads();
         const bool valid = g < GS && (long long)grp * GS + g < a.B;
         if (g < GS) {
-            for (int p = c.lane; p < NP; p += 32)
-                SMV(c, L.oU, p, g) = 2.f * (a.gparams[c.spec[g] * NP + p] - M.lo[p]) / (M.hi[p] - M.lo[p]) - 1.f;
+            for (int p = V1_LANE; p < NP; p += 32)
+                SMV(L.oU, p, g) = 2.f * (a.gparams[v1_blk.spec[g] * NP + p] - M.lo[p]) / (M.hi[p] - M.lo[p]) - 1.f;
             __syncwarp();
-            v1_param_setup(c, g);
+            v1_param_setup(g);
         }
-        v1_evaluate<0>(c, a, true, true, nullptr);
+        v1_evaluate<0>(true, true, nullptr);
         if (g < GS) {
-            const float gr = v1_gradient(c, g);
+            const float gr = v1_gradient(g);
             float chi2, ngood, cmin;
-            v1_stats(c, g, chi2, ngood, cmin);
-            const bool anyfail = __any_sync(FULL, c.lane < M.n_seg && V1SM[L.oSC + (SC_N + c.lane) * GS + g] != 0.f);
+            v1_stats(g, chi2, ngood, cmin);
+            const bool anyfail = __any_sync(FULL, V1_LANE < M.n_seg && V1SM[L.oSC + (SC_N + V1_LANE) * GS + g] != 0.f);
             if (valid) {
-                const long long i = c.spec[g];
-                if (c.lane < NP) a.grad_u[i * NP + c.lane] = gr;
-                if (c.lane == 0) {
+                const long long i = v1_blk.spec[g];
+                if (V1_LANE < NP) a.grad_u[i * NP + V1_LANE] = gr;
+                if (V1_LANE == 0) {
                     a.chi2[i] = chi2;
                     if (a.status) a.status[i] = anyfail ? LASP_ST_NOT_SPD : 0;
                 }
-                if (a.cont) v1_write_cont(c, g, a.cont + i * M.nc);
+                if (a.cont) v1_write_cont(g, a.cont + i * M.nc);
             }
         }
     }

@@ -125,7 +125,7 @@ extern "C" int lasp_destroy(lasp_ctx *c)
     return LASP_OK;
 }
 
-static int setup_v1(lasp_ctx *c, const cudaDeviceProp &prop);
+static int setup_v1(lasp_ctx *c, const cudaDeviceProp &prop, int emax);
 static int v1_workspace(lasp_ctx *c, int64_t B, bool need_xj);
 
 extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx **out)
@@ -243,7 +243,7 @@ extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx *
     M.Ppad = po;
     // padded tables: halos replicate the segment's edge pixel (the clamp of C.2-16 for free)
     // K+2 rounded to 8 rows, plus 16 (prefetch overrun): zero past K, so the v1 loops sweep whole batches without bounds tests
-    const int Krows = roundup(K + 2, 8) + 16;
+    const int Krows = roundup(K + 2, 4) + 16;
     std::vector<float> Cp((size_t)Krows * M.Ppad, 0.f), isp(M.Ppad);
     for (int sg = 0; sg < nseg; ++sg) {
         const SegDev &S = M.seg[sg];
@@ -282,7 +282,9 @@ extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx *
     CUDA_TRY_C(cudaFuncSetAttribute(lasp_fit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
     CUDA_TRY_C(cudaFuncSetAttribute(lasp_grad_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
     CUDA_TRY_C(cudaFuncSetAttribute(lasp_model_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
-    setup_v1(c, prop);
+    int emax = 0;
+    for (int i = 0; i < K * L; ++i) emax = std::max(emax, (int)d->term_exps[i]);
+    setup_v1(c, prop, emax);
     *out = c;
     return LASP_OK;
 }
@@ -299,7 +301,7 @@ static void v1_for_kernels(F f)
     f((const void *)lasp_v1_grad_kernel<384, 1>, 384);
 }
 
-static int setup_v1(lasp_ctx *c, const cudaDeviceProp &prop)
+static int setup_v1(lasp_ctx *c, const cudaDeviceProp &prop, int emax)
 {
     const ModelDev &M = c->M;
     c->v1_ok = false;
@@ -315,6 +317,7 @@ static int setup_v1(lasp_ctx *c, const cudaDeviceProp &prop)
     if (M.NP > 32 || M.n1 > 32) return LASP_OK;
     V1Lay &L = c->V1;
     memset(&L, 0, sizeof(L));
+    L.emax = emax;
     int nt = std::max(GS * 32, roundup(std::max(nfit, 1), 32));
     if (nt > 384) nt = 384;               // longer segments are swept in several passes
     c->v1_nt = nt;
@@ -322,7 +325,7 @@ static int setup_v1(lasp_ctx *c, const cudaDeviceProp &prop)
     L.NW = nt / 32;
     L.GUARD = guard;
     L.RL = maxlen + 2 * guard;
-    L.Hm = getenv("LASP_DEBUG_C0") ? -1 : hmax;
+    L.Hm = hmax;
     L.NA = (hmax + 3) / 4 + hmax / 4 + 2;
     L.n1r = roundup(M.n1, 8);
     L.nmomr = L.n1r + roundup(std::max(M.nmom - L.n1r, 0), 8);
@@ -333,7 +336,7 @@ static int setup_v1(lasp_ctx *c, const cudaDeviceProp &prop)
     auto take = [&](int n) { int r = o; o += roundup(n, 4); return r; };
     L.oT = take(GS * L.RL); L.oA = take(GS * L.RL);
     L.oU = take(GS * M.NP); L.oM = take(GS * M.NP); L.oV = take(GS * M.NP);
-    L.Kq = roundup(M.K + 2, 8);
+    L.Kq = roundup(M.K + 2, 4);
     L.oX = take(GS * M.L); L.oPHI = take(GS * L.Kq);
     L.oGW = take(GS * L.NA * 4); L.oGR = take(3 * GS * L.NA * 4); L.oTAP = take(2 * GS);
     L.oMOM = take(GS * L.nmomr); L.oRHS = take(GS * L.n1r); L.oB = take(GS * M.nc);
@@ -342,6 +345,8 @@ static int setup_v1(lasp_ctx *c, const cudaDeviceProp &prop)
     L.oLF = take(std::max(GS * V1_LFS, 2 * GS * npair + 4));
     L.oQ = take(GS * (M.K + 2)); L.oSC = take(GS * (SC_N + M.n_seg));
     L.oEXP = take((M.K * M.L + 3) / 4);
+    L.oXP = take(GS * M.L * (L.emax + 1)); L.oDPHI = take(GS * M.L * M.K); L.oGSC = take(GS * M.NP);
+    L.oEW = take(GS * (2 * hmax + 2));
     L.total = o;
     const size_t bytes = (size_t)o * sizeof(float);
     if (bytes > prop.sharedMemPerBlockOptin) return LASP_OK;   // does not fit: v0 handles it
