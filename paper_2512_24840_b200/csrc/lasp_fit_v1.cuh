@@ -932,6 +932,8 @@ __device__ __forceinline__ void v1_init_block(const ModelDev &M, const V1Lay &L,
     if (threadIdx.x == 0) v1_blk.cp = a.CP + (size_t)blockIdx.x * GS * M.Ppad;
     for (int i = threadIdx.x; i < M.K * M.L; i += blockDim.x) ((uint8_t *)(V1SM + L.oEXP))[i] = M.exps[i];
     for (int i = threadIdx.x; i < GS * L.Kq; i += blockDim.x) V1SM[L.oPHI + i] = 0.f;   // phi is zero past K
+    // rows T and A: zero-weight taps multiply whatever lies in the window, so it must at least be finite
+    for (int i = threadIdx.x; i < 2 * GS * L.RL; i += blockDim.x) V1SM[L.oT + i] = 0.f;
     __syncthreads();
 }
 

@@ -100,6 +100,14 @@ extern "C" const char *lasp_last_error(const lasp_ctx *ctx) { return ctx ? ctx->
 
 extern "C" int lasp_kernel_variant(const lasp_ctx *ctx) { return ctx && ctx->v1_ok ? 1 : 0; }
 
+// debug aid (not part of the public header): launch shape of the v1 kernel
+extern "C" int lasp_debug_launch_info(const lasp_ctx *c, int *out4)
+{
+    if (!c) return LASP_ERR_INVALID_ARG;
+    out4[0] = c->v1_ok; out4[1] = c->v1_nt; out4[2] = c->v1_cta_per_sm; out4[3] = c->V1.total * 4;
+    return LASP_OK;
+}
+
 // debug aid (not part of the public header): per-phase cycle sums of the last v1 fit (thread 0 of every CTA)
 extern "C" int lasp_debug_phase_cycles(lasp_ctx *c, unsigned long long *out16)
 {
