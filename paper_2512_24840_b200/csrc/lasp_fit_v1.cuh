@@ -38,7 +38,8 @@ struct V1Lay {
 };
 
 struct V1Args {
-    const float *Y, *W;   // staged flux and weight planes [B][Ppad] (halos and tails zero)
+    const float *Y, *W;   // staged flux and weight planes [B][Ppad] (halos and tails zero), split-octet layout
+    const float *C1;      // emulator coefficients [Kq+16][Ppad], zero past K, split-octet layout
     float *CP;            // [cta][GS][Ppad] previous continuum c_prev (a5, refinement form)
     float *XJ;            // [cta][(1+NP)][GS][Ppad] rho and Jacobian columns (a9), may be null
     long long B;
@@ -277,8 +278,8 @@ __device__ __noinline__ void v1_phase_emulator(const SegDev &sg, int lo, int hi)
     // everything the loop needs is copied to registers first: the model lives in shared memory, and after
     // any shared-memory store the compiler would otherwise have to re-read it
     const float4 *phi4 = (const float4 *)(V1SM + v1_blk.L.oPHI);
-    const int P4 = v1_blk.M.Ppad >> 2, Kq = v1_blk.L.Kq, nt8 = V1_NT * OCT;
-    const float *Cg = v1_blk.M.C;
+    const int P4 = v1_blk.M.Ppad >> 2, P8 = v1_blk.M.Ppad >> 3, Kq = v1_blk.L.Kq, nt8 = V1_NT * OCT;
+    const float *Cg = v1_blk.A.C1;
     float *rowT = V1SM + v1_blk.L.oT + v1_blk.L.GUARD - sg.po;
     const int RL = v1_blk.L.RL;
     for (int j0 = lo + V1_TID * OCT; j0 < hi; j0 += nt8) {
@@ -290,13 +291,13 @@ __device__ __noinline__ void v1_phase_emulator(const SegDev &sg, int lo, int hi)
         // C[k, j0..j0+7] streams from L2/L1 in batches of 4 terms, the next batch in flight while this one is
         // multiplied (two register buffers).  The table has Kq = K+2 rounded to 8 rows plus 8 more, all zero
         // past K (and phi is zero there), so the loop has no bounds tests.
-        const float4 *c4 = (const float4 *)(Cg + j0);
+        const float4 *c4 = (const float4 *)Cg + (j0 >> 3);
         float4 bufA[8], bufB[8];
         auto load4 = [&](int k0, float4 (&buf)[8]) {
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
                 buf[2 * u] = __ldg(c4 + (k0 + u) * P4);
-                buf[2 * u + 1] = __ldg(c4 + (k0 + u) * P4 + 1);
+                buf[2 * u + 1] = __ldg(c4 + (k0 + u) * P4 + P8);
             }
         };
         auto mul4 = [&](int k0, const float4 (&buf)[8]) {
@@ -353,7 +354,7 @@ __device__ __noinline__ void v1_phase_forward(const SegDev &sg, bool stencil, bo
     const int *tap = (const int *)(V1SM + L.oTAP);
     float *red = V1SM + L.oRED + V1_WARP * L.VR * GS;
     // hoisted to registers (the model sits in shared memory; see v1_phase_emulator)
-    const int Ppad = v1_blk.M.Ppad, RL = L.RL, NA = L.NA, n1r = L.n1r, nmomr = L.nmomr, nt8 = V1_NT * OCT;
+    const int Ppad = v1_blk.M.Ppad, P8 = Ppad >> 3, RL = L.RL, NA = L.NA, n1r = L.n1r, nmomr = L.nmomr, nt8 = V1_NT * OCT;
     const int fit_lo = sg.fit_lo, fit_hi = sg.fit_hi, torg = sg.po + sg.halo;
     const float ta = sg.ta, tb = sg.tb;
     float *rowA = V1SM + L.oA + L.GUARD - sg.po;
@@ -374,11 +375,11 @@ __device__ __noinline__ void v1_phase_forward(const SegDev &sg, bool stencil, bo
 #pragma unroll
             for (int g = 0; g < GS; ++g) {
                 // flux / weight / c_prev rows come from L2: issue the loads first, the stencil hides them
-                const size_t ro = rowo[g] + j0;
-                const float4 y0 = __ldg((const float4 *)(Yg + ro)), y1 = __ldg((const float4 *)(Yg + ro) + 1);
-                const float4 w0 = __ldg((const float4 *)(Wg + ro)), w1 = __ldg((const float4 *)(Wg + ro) + 1);
-                const float4 *cp4 = (const float4 *)(cpg + g * Ppad + j0);
-                const float4 c0 = __ldcg(cp4), c1 = __ldcg(cp4 + 1);
+                const size_t ro = rowo[g] + (j0 >> 1);   // split-octet layout: half h of octet o at h*Ppad/2 + 4 o
+                const float4 y0 = __ldg((const float4 *)(Yg + ro)), y1 = __ldg((const float4 *)(Yg + ro) + P8);
+                const float4 w0 = __ldg((const float4 *)(Wg + ro)), w1 = __ldg((const float4 *)(Wg + ro) + P8);
+                const float4 *cp4 = (const float4 *)(cpg + g * Ppad + (j0 >> 1));
+                const float4 c0 = __ldcg(cp4), c1 = __ldcg(cp4 + P8);
                 float S[1][OCT];
                 float4 *ra = (float4 *)(rowA + g * RL + j0);
                 if (stencil) {
@@ -591,7 +592,7 @@ __device__ __noinline__ void v1_phase_residual(const SegDev &sg, int rowB, float
     const V1Args &a = v1_blk.A;
     const V1Lay &L = v1_blk.L;
     const float4 *b4 = (const float4 *)(V1SM + L.oB) + rowB;
-    const int Ppad = v1_blk.M.Ppad, n1 = v1_blk.M.n1, RL = L.RL, nt8 = V1_NT * OCT;
+    const int Ppad = v1_blk.M.Ppad, P8 = Ppad >> 3, n1 = v1_blk.M.n1, RL = L.RL, nt8 = V1_NT * OCT;
     const int fit_lo = sg.fit_lo, fit_hi = sg.fit_hi, torg = sg.po + sg.halo;
     const float ta = sg.ta, tb = sg.tb;
     float *rowA = V1SM + L.oA + L.GUARD - sg.po;
@@ -609,9 +610,9 @@ __device__ __noinline__ void v1_phase_residual(const SegDev &sg, int rowB, float
         if (MODE != 0) {
 #pragma unroll
             for (int g = 0; g < GS; ++g) {
-                const size_t ro = rowo[g] + j0;
-                yq[g][0] = __ldg((const float4 *)(Yg + ro)); yq[g][1] = __ldg((const float4 *)(Yg + ro) + 1);
-                wq[g][0] = __ldg((const float4 *)(Wg + ro)); wq[g][1] = __ldg((const float4 *)(Wg + ro) + 1);
+                const size_t ro = rowo[g] + (j0 >> 1);
+                yq[g][0] = __ldg((const float4 *)(Yg + ro)); yq[g][1] = __ldg((const float4 *)(Yg + ro) + P8);
+                wq[g][0] = __ldg((const float4 *)(Wg + ro)); wq[g][1] = __ldg((const float4 *)(Wg + ro) + P8);
             }
         }
 #pragma unroll
@@ -635,9 +636,9 @@ __device__ __noinline__ void v1_phase_residual(const SegDev &sg, int rowB, float
         }
 #pragma unroll
         for (int g = 0; g < GS; ++g) {
-            float4 *cp4 = (float4 *)(cpg + g * Ppad + j0);
+            float4 *cp4 = (float4 *)(cpg + g * Ppad + (j0 >> 1));
             cp4[0] = make_float4(cc[g][0], cc[g][1], cc[g][2], cc[g][3]);
-            cp4[1] = make_float4(cc[g][4], cc[g][5], cc[g][6], cc[g][7]);
+            cp4[P8] = make_float4(cc[g][4], cc[g][5], cc[g][6], cc[g][7]);
             if (MODE == 0) continue;
             float4 *ra = (float4 *)(rowA + g * RL + j0);
             const float4 s0 = ra[0], s1 = ra[1];
@@ -689,11 +690,11 @@ __device__ __noinline__ void v1_phase_adjoint(const SegDev &sg, int lo, int hi)
 {
     const V1Lay &L = v1_blk.L;
     const int *tap = (const int *)(V1SM + L.oTAP);
-    const int P4 = v1_blk.M.Ppad >> 2, K = v1_blk.M.K, Kq = L.Kq, NA = L.NA, RL = L.RL, nt8 = V1_NT * OCT;
+    const int P4 = v1_blk.M.Ppad >> 2, P8 = v1_blk.M.Ppad >> 3, K = v1_blk.M.K, Kq = L.Kq, NA = L.NA, RL = L.RL, nt8 = V1_NT * OCT;
     const int wstride4 = GS * NA;   // float4 stride between the three reversed kernels
     const int qslot0 = SLOT_Q(L, 0);
     float *red = V1SM + L.oRED + V1_WARP * L.VR * GS;
-    const float *Cg = v1_blk.M.C;
+    const float *Cg = v1_blk.A.C1;
     const float *rowA = V1SM + L.oA + L.GUARD - sg.po, *rowT = V1SM + L.oT + L.GUARD - sg.po;
     const float4 *gr4 = (const float4 *)(V1SM + L.oGR);
     int alo[GS], nag[GS];
@@ -725,13 +726,13 @@ __device__ __noinline__ void v1_phase_adjoint(const SegDev &sg, int lo, int hi)
         }
         // C[k, octet] in batches of 4 terms, the next batch in flight during the multiplies; the table is
         // zero past K, so rows K and K+1 are free to carry the two kernel-parameter gradients
-        const float4 *c4 = (const float4 *)(Cg + (act ? j0 : lo));
+        const float4 *c4 = (const float4 *)Cg + ((act ? j0 : lo) >> 3);
         float4 bufA[8], bufB[8];
         auto load4 = [&](int kb, float4 (&buf)[8]) {
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
                 buf[2 * u] = __ldg(c4 + (kb + u) * P4);
-                buf[2 * u + 1] = __ldg(c4 + (kb + u) * P4 + 1);
+                buf[2 * u + 1] = __ldg(c4 + (kb + u) * P4 + P8);
             }
         };
         load4(0, bufA);
@@ -822,9 +823,8 @@ __device__ __noinline__ void v1_evaluate(bool cold, bool mom, float *xrow)
             for (int i = V1_TID; i < GS * L.RL / 4; i += V1_NT) ((float4 *)(V1SM + L.oA))[i] = make_float4(0.f, 0.f, 0.f, 0.f);
         }
         if (cold) {
-            for (int g = 0; g < GS; ++g)
-                for (int j = sg.fit_lo + V1_TID * 4; j < sg.fit_hi; j += V1_NT * 4)
-                    *(float4 *)(v1_blk.cp + (size_t)g * M.Ppad + j) = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (s == 0)
+                for (int i = V1_TID; i < GS * M.Ppad / 4; i += V1_NT) ((float4 *)v1_blk.cp)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
         }
         tick(0);
         __syncthreads();

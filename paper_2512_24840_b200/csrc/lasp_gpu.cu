@@ -33,7 +33,7 @@ struct lasp_ctx {
     bool v1_ok = false;
     V1Lay V1;
     int v1_nt = 0, v1_maxt = 0, v1_cta_per_sm = 1;
-    float *dY = nullptr, *dW = nullptr;
+    float *dY = nullptr, *dW = nullptr, *dC1 = nullptr;
     size_t plane_rows = 0;
     float *dCP = nullptr, *dXJ = nullptr;
     unsigned long long *ddbg = nullptr;
@@ -123,7 +123,7 @@ extern "C" int lasp_destroy(lasp_ctx *c)
     cudaSetDevice(c->device);
     cudaFree(c->dC); cudaFree(c->dinv_s); cudaFree(c->dexps); cudaFree(c->dconv); cudaFree(c->dnedge);
     cudaFree(c->dYW); cudaFree(c->dscratch);
-    cudaFree(c->dY); cudaFree(c->dW); cudaFree(c->dCP); cudaFree(c->dXJ); cudaFree(c->ddbg);
+    cudaFree(c->dC1); cudaFree(c->dY); cudaFree(c->dW); cudaFree(c->dCP); cudaFree(c->dXJ); cudaFree(c->ddbg);
     hostpipe_free(c);
     if (c->hp.s_in) {
         cudaStreamDestroy(c->hp.s_in); cudaStreamDestroy(c->hp.s_out); cudaStreamDestroy(c->hp.s_fit);
@@ -277,6 +277,14 @@ extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx *
 
     CUDA_TRY_C(cudaMalloc(&c->dC, Cp.size() * sizeof(float)));
     CUDA_TRY_C(cudaMemcpy(c->dC, Cp.data(), Cp.size() * sizeof(float), cudaMemcpyHostToDevice));
+    {   // v1's copy of the table in the split-octet layout
+        std::vector<float> C1(Cp.size());
+        for (int k = 0; k < Krows; ++k)
+            for (int jp = 0; jp < M.Ppad; ++jp)
+                C1[(size_t)k * M.Ppad + ((jp >> 2) & 1) * (M.Ppad >> 1) + (jp >> 3) * 4 + (jp & 3)] = Cp[(size_t)k * M.Ppad + jp];
+        CUDA_TRY_C(cudaMalloc(&c->dC1, C1.size() * sizeof(float)));
+        CUDA_TRY_C(cudaMemcpy(c->dC1, C1.data(), C1.size() * sizeof(float), cudaMemcpyHostToDevice));
+    }
     CUDA_TRY_C(cudaMalloc(&c->dinv_s, isp.size() * sizeof(float)));
     CUDA_TRY_C(cudaMemcpy(c->dinv_s, isp.data(), isp.size() * sizeof(float), cudaMemcpyHostToDevice));
     CUDA_TRY_C(cudaMalloc(&c->dexps, (size_t)K * L));
@@ -447,8 +455,10 @@ __global__ void lasp_v1_stage_kernel(const __grid_constant__ ModelDev M, const i
             const int ne = n_edge[s];
             if (rel < ne || rel >= sg.P - ne) w = 0.f;
         }
-        Y[row * M.Ppad + jp] = y;
-        W[row * M.Ppad + jp] = w;
+        // split-octet layout: half h of octet o at h*Ppad/2 + 4 o, so that a warp's 128-bit loads are contiguous
+        const size_t q = row * M.Ppad + ((jp >> 2) & 1) * (M.Ppad >> 1) + (jp >> 3) * 4 + (jp & 3);
+        Y[q] = y;
+        W[q] = w;
     }
 }
 
@@ -526,7 +536,7 @@ extern "C" int lasp_fit_batch(lasp_ctx *c, int64_t B, const float *flux, const f
         if (rc) return rc;
         V1Args a;
         memset(&a, 0, sizeof(a));
-        a.Y = c->dY; a.W = c->dW; a.CP = c->dCP; a.XJ = c->dXJ; a.B = B;
+        a.Y = c->dY; a.W = c->dW; a.C1 = c->dC1; a.CP = c->dCP; a.XJ = c->dXJ; a.B = B;
         const int grid = v1_grid(c, B, a.ngroups);
         a.init = init; a.n_iter = opts->n_iter; a.lr = opts->lr; a.b1 = opts->beta1; a.b2 = opts->beta2;
         a.eps = opts->eps; a.fd_h = 2e-3f;  // fp32 central-difference step in u (C.2-22)
@@ -572,7 +582,7 @@ extern "C" int lasp_eval_grad(lasp_ctx *c, int64_t B, const float *flux, const f
         if (rc) return rc;
         V1Args a;
         memset(&a, 0, sizeof(a));
-        a.Y = c->dY; a.W = c->dW; a.CP = c->dCP; a.B = B;
+        a.Y = c->dY; a.W = c->dW; a.C1 = c->dC1; a.CP = c->dCP; a.B = B;
         const int grid = v1_grid(c, B, a.ngroups);
         a.gparams = params; a.chi2 = chi2; a.grad_u = grad_u; a.cont = cont; a.status = status;
         return v1_launch(c, true, a, grid, st);
