@@ -21,6 +21,11 @@
 extern __shared__ float4 v1_smem4[];
 #define V1SM ((float *)v1_smem4)
 
+// 128-bit accesses to the shared rows go at a stride of two float4 between lanes (one octet per thread), which
+// would be a two-way bank conflict; flipping the low index bit of every other group of eight float4 makes the
+// eight lanes of a quarter-warp hit eight different 16-byte bank groups.  Applied to EVERY access of rows T / A.
+#define SW4(q) ((q) ^ (((q) >> 3) & 1))
+
 #define GS 4    // spectra per CTA group
 #define OCT 8   // pixels per thread tile
 
@@ -225,10 +230,10 @@ __device__ __forceinline__ void v1_stencil_octet(const float4 *__restrict__ row4
 #pragma unroll
         for (int i = 0; i < OCT; ++i) acc[n][i] = 0.f;
     const int q = (j0 >> 2) - a_lo;
-    float4 qb = row4[q + 1], qc = row4[q + 2];
+    float4 qb = row4[SW4(q + 1)], qc = row4[SW4(q + 2)];
 #pragma unroll 3
     for (int ai = 0; ai < na; ++ai) {
-        const float4 qa = row4[q - ai];
+        const float4 qa = row4[SW4(q - ai)];
         const float Wd[12] = {qa.x, qa.y, qa.z, qa.w, qb.x, qb.y, qb.z, qb.w, qc.x, qc.y, qc.z, qc.w};
 #pragma unroll
         for (int n = 0; n < NK; ++n) {
@@ -330,9 +335,10 @@ __device__ __noinline__ void v1_phase_emulator(const SegDev &sg, int lo, int hi)
         }
 #pragma unroll
         for (int g = 0; g < GS; ++g) {
-            float4 *r = (float4 *)(rowT + g * RL + j0);
-            r[0] = make_float4(acc[g][0], acc[g][1], acc[g][2], acc[g][3]);
-            r[1] = make_float4(acc[g][4], acc[g][5], acc[g][6], acc[g][7]);
+            float4 *r = (float4 *)(rowT + g * RL);
+            const int q = j0 >> 2;
+            r[SW4(q)] = make_float4(acc[g][0], acc[g][1], acc[g][2], acc[g][3]);
+            r[SW4(q + 1)] = make_float4(acc[g][4], acc[g][5], acc[g][6], acc[g][7]);
         }
     }
 }
@@ -381,13 +387,14 @@ __device__ __noinline__ void v1_phase_forward(const SegDev &sg, bool stencil, bo
                 const float4 *cp4 = (const float4 *)(cpg + g * Ppad + (j0 >> 1));
                 const float4 c0 = __ldcg(cp4), c1 = __ldcg(cp4 + P8);
                 float S[1][OCT];
-                float4 *ra = (float4 *)(rowA + g * RL + j0);
+                float4 *ra = (float4 *)(rowA + g * RL);
+                const int q0 = SW4(j0 >> 2), q1 = SW4((j0 >> 2) + 1);
                 if (stencil) {
                     v1_stencil_octet<1>((const float4 *)(rowT + g * RL), j0, alo[g], nag[g], gw4 + g * NA, 0, S);
-                    ra[0] = make_float4(S[0][0], S[0][1], S[0][2], S[0][3]);
-                    ra[1] = make_float4(S[0][4], S[0][5], S[0][6], S[0][7]);
+                    ra[q0] = make_float4(S[0][0], S[0][1], S[0][2], S[0][3]);
+                    ra[q1] = make_float4(S[0][4], S[0][5], S[0][6], S[0][7]);
                 } else {
-                    const float4 s0 = ra[0], s1 = ra[1];
+                    const float4 s0 = ra[q0], s1 = ra[q1];
                     S[0][0] = s0.x; S[0][1] = s0.y; S[0][2] = s0.z; S[0][3] = s0.w;
                     S[0][4] = s1.x; S[0][5] = s1.y; S[0][6] = s1.z; S[0][7] = s1.w;
                 }
@@ -640,8 +647,9 @@ __device__ __noinline__ void v1_phase_residual(const SegDev &sg, int rowB, float
             cp4[0] = make_float4(cc[g][0], cc[g][1], cc[g][2], cc[g][3]);
             cp4[P8] = make_float4(cc[g][4], cc[g][5], cc[g][6], cc[g][7]);
             if (MODE == 0) continue;
-            float4 *ra = (float4 *)(rowA + g * RL + j0);
-            const float4 s0 = ra[0], s1 = ra[1];
+            float4 *ra = (float4 *)(rowA + g * RL);
+            const int q0 = SW4(j0 >> 2), q1 = SW4((j0 >> 2) + 1);
+            const float4 s0 = ra[q0], s1 = ra[q1];
             const float4 y0 = yq[g][0], y1 = yq[g][1], w0 = wq[g][0], w1 = wq[g][1];
             const float SS[OCT] = {s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w};
             const float yy[OCT] = {y0.x, y0.y, y0.z, y0.w, y1.x, y1.y, y1.z, y1.w};
@@ -656,8 +664,8 @@ __device__ __noinline__ void v1_phase_residual(const SegDev &sg, int rowB, float
                 av[i] = -2.f * wr * cc[g][i];
                 if (MODE == 2) rho[i] = sqrtf(ww[i]) * r;
             }
-            ra[0] = make_float4(av[0], av[1], av[2], av[3]);
-            ra[1] = make_float4(av[4], av[5], av[6], av[7]);
+            ra[q0] = make_float4(av[0], av[1], av[2], av[3]);
+            ra[q1] = make_float4(av[4], av[5], av[6], av[7]);
             if (MODE == 2) {
                 float4 *x4 = (float4 *)(xrow + g * Ppad + j0);
                 x4[0] = make_float4(rho[0], rho[1], rho[2], rho[3]);
@@ -710,8 +718,8 @@ __device__ __noinline__ void v1_phase_adjoint(const SegDev &sg, int lo, int hi)
             if (act) {
                 float acc[3][OCT];
                 v1_stencil_octet<3>((const float4 *)(rowA + g * RL), j0, alo[g], nag[g], gr4 + g * NA, wstride4, acc);
-                const float4 *rt = (const float4 *)(rowT + g * RL + j0);
-                const float4 t0 = rt[0], t1 = rt[1];
+                const float4 *rt = (const float4 *)(rowT + g * RL);
+                const float4 t0 = rt[SW4(j0 >> 2)], t1 = rt[SW4((j0 >> 2) + 1)];
                 const float TT[OCT] = {t0.x, t0.y, t0.z, t0.w, t1.x, t1.y, t1.z, t1.w};
 #pragma unroll
                 for (int i = 0; i < OCT; ++i) {

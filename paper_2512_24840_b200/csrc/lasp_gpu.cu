@@ -347,7 +347,7 @@ static int setup_v1(lasp_ctx *c, const cudaDeviceProp &prop, int emax)
     L.nmomr = L.n1r + roundup(std::max(M.nmom - L.n1r, 0), 8);
     L.VR = L.nmomr + L.n1r + roundup(M.K + 2, 8) + 4;
     const char *rf = getenv("LASP_REFRESH");
-    L.refresh = rf ? std::max(1, atoi(rf)) : 8;
+    L.refresh = rf ? std::max(1, atoi(rf)) : 16;
     int o = 0;
     auto take = [&](int n) { int r = o; o += roundup(n, 4); return r; };
     L.oT = take(GS * L.RL); L.oA = take(GS * L.RL);
