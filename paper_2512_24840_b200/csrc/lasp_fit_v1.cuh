@@ -38,7 +38,7 @@ struct V1Lay {
     int Hm;                 // support clamp (memory safety outside the prior box)
     int refresh;            // re-accumulate the Gram moments and re-factor every `refresh` steps
     // shared-memory offsets (floats)
-    int oT, oA, oU, oM, oV, oX, oPHI, oGW, oGR, oTAP, oMOM, oRHS, oB, oRED, oLF, oQ, oSC, oEXP, oXP, oDPHI, oGSC, oEW, total;
+    int oT, oA, oU, oM, oV, oX, oPHI, oGW, oGR, oTAP, oMOM, oRHS, oB, oRED, oLF, oQ, oSC, oEXP, oXP, oDPHI, oGSC, oEW, oNP, total;
     int emax;               // largest exponent of the monomial table
 };
 
@@ -57,13 +57,23 @@ struct V1Args {
     const float *gparams;  // lasp_eval_grad
     float *grad_u;
     unsigned long long *dbg;   // optional per-phase cycle counters (LASP_TIMING=1), else null
+    // per-pixel broadening kernels (linear grids, C.2-14): 1/s_j and s_j^2 with V1_TPAD replicated entries on
+    // both sides, and per-CTA scratch [3][GS][Ppad] for dS/dv, dS/dsigma*, 1/E0 (thread-private pixels)
+    const float *IS, *S2;
+    float *DS;
 };
+#define V1_TPAD 256
+
+struct V1Np {          // per-spectrum scalars of a per-pixel-kernel segment
+    float v, sigstar, sigtot, hn, hbv, hcap;   // hn = -log2(e)/(2 sigma_tot^2); hbv = |v| + 5 sigma_tot (km/s)
+};
+
 
 // slots of the per-warp reduction area (each slot holds GS floats)
 #define SLOT_MOM(L_, n) (n)
 #define SLOT_RHS(L_, n) ((L_).nmomr + (n))
 #define SLOT_Q(L_, k) ((L_).nmomr + (L_).n1r + (k))
-#define SLOT_STAT(L_) ((L_).VR - 4)   // chi2, ngood, min c
+#define SLOT_STAT(L_) ((L_).VR - 6)   // chi2, ngood, min c, dchi2/dv and dchi2/dsigma* of per-pixel-kernel segments
 
 // per-spectrum scalars in shared memory: SC[idx][GS]
 enum { SC_V = 0, SC_SIG, SC_CHI, SC_NGOOD, SC_CMIN, SC_GV, SC_GS, SC_FAIL, SC_N };
@@ -101,6 +111,7 @@ struct V1Block {
     V1Args A;
     long long spec[GS];   // clamped spectrum indices of the group
     float *cp;            // this CTA's c_prev scratch
+    float *ds;            // this CTA's dS/dv, dS/dsigma*, 1/E0 scratch (per-pixel-kernel segments)
 };
 __shared__ V1Block v1_blk;
 #define V1_TID ((int)threadIdx.x)
@@ -172,6 +183,21 @@ __device__ __noinline__ void v1_setup_weights(const SegDev &sg, int g)
     const V1Lay &L = v1_blk.L;
     const float v = SMV(L.oSC, SC_V, g), sigstar = SMV(L.oSC, SC_SIG, g);
     const float sigtot = sqrtf(sigstar * sigstar + sg.sig_inst * sg.sig_inst);
+    if (!sg.uniform) {
+        // per-pixel kernels: only the spectrum's scalars and the segment-wide reach (sg.inv_s = largest 1/s_j)
+        if (V1_LANE == 0) {
+            V1Np *np = (V1Np *)(V1SM + L.oNP) + g;
+            np->v = v; np->sigstar = sigstar; np->sigtot = sigtot;
+            np->hn = -0.72134752044f / (sigtot * sigtot);        // -log2(e)/2 / sigma_tot^2
+            np->hbv = fabsf(v) + 5.f * sigtot;
+            np->hcap = (float)(sg.halo - 18);
+            const int H = (int)ceilf(fminf(np->hbv * sg.inv_s, np->hcap));
+            int *tap = (int *)(V1SM + L.oTAP);
+            tap[g * 2] = -(H / 4); tap[g * 2 + 1] = (H + 3) / 4 + (H / 4) + 1;
+        }
+        __syncwarp();
+        return;
+    }
     const float mu = v * sg.inv_s, s = sigtot * sg.inv_s;
     int H = (int)ceilf(fabsf(mu) + 5.f * s);
     H = min(max(H, 0), sg.halo - 18);   // memory safety outside the prior box (halo >= Hmax + 18)
@@ -256,6 +282,117 @@ __device__ __forceinline__ void v1_stencil_octet(const float4 *__restrict__ row4
 __device__ __forceinline__ float *v1_row(int off, const SegDev &sg, int g)
 {
     return V1SM + off + g * v1_blk.L.RL + v1_blk.L.GUARD - sg.po;
+}
+
+// ------------------------------------------------------------------------------------------
+// a3 + a4 on a linear grid (C.2-14): every pixel j has its own kernel, mu_j = v/s_j, sigma_j = sigma_tot/s_j,
+// H_j = ceil(|mu_j| + 5 sigma_j), e_jk = exp(-(k-mu_j)^2/(2 sigma_j^2)) on |k| <= H_j, normalised per pixel.
+// Weights are generated on the fly (one ex2 per pixel and tap); |k| <= ceil(x)  <=>  |k| - 1 < x.
+//   forward:  S_j = A0/E0, and dS_j/dv, dS_j/dsigma* from the first and second moments of e (C.1)
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ float v1_ex2(float x)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+__device__ __forceinline__ void v1_np_forward_octet(const float4 *__restrict__ row4, int j0, const V1Np &p,
+                                                    const float (&is)[OCT], const float (&s2)[OCT],
+                                                    float (&S)[OCT], float (&DSV)[OCT], float (&DSS)[OCT],
+                                                    float (&EI)[OCT])
+{
+    float mu[OCT], ni2[OCT], hb[OCT];
+    float A0[OCT], A1[OCT], A2[OCT], E0[OCT], E1[OCT], E2[OCT];
+    float hmx = 0.f;
+#pragma unroll
+    for (int i = 0; i < OCT; ++i) {
+        mu[i] = p.v * is[i];
+        ni2[i] = p.hn * s2[i];
+        hb[i] = fminf(p.hbv * is[i], p.hcap);
+        hmx = fmaxf(hmx, hb[i]);
+        A0[i] = A1[i] = A2[i] = E0[i] = E1[i] = E2[i] = 0.f;
+    }
+    const int H = (int)ceilf(hmx);
+    const int a_lo = -(H / 4), na = (H + 3) / 4 - a_lo + 1;
+    const int q = (j0 >> 2) - a_lo;
+    float4 qb = row4[SW4(q + 1)], qc = row4[SW4(q + 2)];
+    for (int ai = 0; ai < na; ++ai) {
+        const float4 qa = row4[SW4(q - ai)];
+        const float Wd[12] = {qa.x, qa.y, qa.z, qa.w, qb.x, qb.y, qb.z, qb.w, qc.x, qc.y, qc.z, qc.w};
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const float kf = (float)(4 * (a_lo + ai) - 3 + r);
+            const float ak1 = fabsf(kf) - 1.f;
+#pragma unroll
+            for (int i = 0; i < OCT; ++i) {
+                const float d = kf - mu[i];
+                float e = v1_ex2(d * d * ni2[i]);
+                e = (ak1 < hb[i]) ? e : 0.f;
+                const float Tv = Wd[i + 3 - r];
+                const float ed = e * d, edd = ed * d;
+                E0[i] += e; E1[i] += ed; E2[i] += edd;
+                A0[i] = fmaf(e, Tv, A0[i]); A1[i] = fmaf(ed, Tv, A1[i]); A2[i] = fmaf(edd, Tv, A2[i]);
+            }
+        }
+        qc = qb; qb = qa;
+    }
+    const float rs = p.sigstar / p.sigtot;
+#pragma unroll
+    for (int i = 0; i < OCT; ++i) {
+        const float inv = 1.f / E0[i];
+        S[i] = A0[i] * inv;
+        EI[i] = inv;
+        const float is2 = ni2[i] * -1.3862943611f;   // 1/sigma_j^2 = 2 i2 = -2 ln2 * ni2
+        const float smu = (A1[i] * inv - E1[i] * inv * S[i]) * is2;
+        const float ssg = (A2[i] * inv - E2[i] * inv * S[i]) * is2 * sqrtf(is2);
+        DSV[i] = smu * is[i];
+        DSS[i] = ssg * rs * is[i];
+    }
+}
+
+// adjoint:  t_i = sum_j a'_j e_{j,j-i},  a' = a/E0 (row A).  With k' = j... the window over SOURCE pixels slides
+// like the forward one; each source carries its own (mu, sigma, H).  istab/s2tab point at padded pixel 0.
+__device__ __forceinline__ void v1_np_adjoint_octet(const float4 *__restrict__ row4, int j0, int H, const V1Np &p,
+                                                    const float *__restrict__ istab, const float *__restrict__ s2tab,
+                                                    float (&t)[OCT])
+{
+#pragma unroll
+    for (int i = 0; i < OCT; ++i) t[i] = 0.f;
+    const int a_lo = -(H / 4), na = (H + 3) / 4 - a_lo + 1;
+    for (int ai = 0; ai < na; ++ai) {
+        const int a = a_lo + ai;
+        const int wb = j0 - 4 * a;                         // window base: sources wb .. wb+11
+        const int q = wb >> 2;
+        const float4 w0 = row4[SW4(q)], w1 = row4[SW4(q + 1)], w2 = row4[SW4(q + 2)];
+        const float Wd[12] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w, w2.x, w2.y, w2.z, w2.w};
+        float mu[12], ni2[12], hb[12];
+#pragma unroll
+        for (int m4 = 0; m4 < 3; ++m4) {
+            const float4 i4 = __ldg((const float4 *)(istab + wb) + m4), s4 = __ldg((const float4 *)(s2tab + wb) + m4);
+            const float ii[4] = {i4.x, i4.y, i4.z, i4.w}, ss[4] = {s4.x, s4.y, s4.z, s4.w};
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                mu[m4 * 4 + c] = p.v * ii[c];
+                ni2[m4 * 4 + c] = p.hn * ss[c];
+                hb[m4 * 4 + c] = fminf(p.hbv * ii[c], p.hcap);
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            // target i reads source m = i+3-r at lag k' = 4a-3+r, i.e. kernel offset k = j - i = -k'... (j = i - k')
+            const float kf = (float)(4 * a - 3 + r);
+            const float ak1 = fabsf(kf) - 1.f;
+#pragma unroll
+            for (int i = 0; i < OCT; ++i) {
+                const int m = i + 3 - r;
+                const float d = -kf - mu[m];               // source j = i - k' contributes e_{j, k = j - i = -k'}
+                float e = v1_ex2(d * d * ni2[m]);
+                e = (ak1 < hb[m]) ? e : 0.f;
+                t[i] = fmaf(Wd[m], e, t[i]);
+            }
+        }
+    }
 }
 
 // padded pixel range [lo,hi) on which T is needed by the forward stencils of the group's fitted octets
@@ -368,16 +505,30 @@ __device__ __noinline__ void v1_phase_forward(const SegDev &sg, bool stencil, bo
     const float4 *gw4 = (const float4 *)(V1SM + L.oGW);
     const float *Yg = a.Y, *Wg = a.W;
     const float *cpg = v1_blk.cp;
+    const bool uniform = sg.uniform != 0;
+    const float *ISg = a.IS + V1_TPAD, *S2g = a.S2 + V1_TPAD;
+    float *dsg = v1_blk.ds;
     int alo[GS], nag[GS];
     size_t rowo[GS];
+    V1Np npp[GS];
 #pragma unroll
-    for (int g = 0; g < GS; ++g) { alo[g] = tap[2 * g]; nag[g] = tap[2 * g + 1]; rowo[g] = (size_t)v1_blk.spec[g] * Ppad; }
+    for (int g = 0; g < GS; ++g) {
+        alo[g] = tap[2 * g]; nag[g] = tap[2 * g + 1]; rowo[g] = (size_t)v1_blk.spec[g] * Ppad;
+        npp[g] = ((const V1Np *)(V1SM + L.oNP))[g];
+    }
     bool first = true;
     for (int jb = fit_lo; jb < fit_hi; jb += nt8, first = false) {   // uniform trip count
         const int j0 = jb + V1_TID * OCT;
         const bool act = j0 < fit_hi;
         float u[GS][OCT], v[GS][OCT];
         if (act) {
+            float isv[OCT], s2v[OCT];
+            if (!uniform) {
+                const float4 a0 = __ldg((const float4 *)(ISg + j0)), a1 = __ldg((const float4 *)(ISg + j0) + 1);
+                const float4 b0 = __ldg((const float4 *)(S2g + j0)), b1 = __ldg((const float4 *)(S2g + j0) + 1);
+                isv[0] = a0.x; isv[1] = a0.y; isv[2] = a0.z; isv[3] = a0.w; isv[4] = a1.x; isv[5] = a1.y; isv[6] = a1.z; isv[7] = a1.w;
+                s2v[0] = b0.x; s2v[1] = b0.y; s2v[2] = b0.z; s2v[3] = b0.w; s2v[4] = b1.x; s2v[5] = b1.y; s2v[6] = b1.z; s2v[7] = b1.w;
+            }
 #pragma unroll
             for (int g = 0; g < GS; ++g) {
                 // flux / weight / c_prev rows come from L2: issue the loads first, the stencil hides them
@@ -389,7 +540,19 @@ __device__ __noinline__ void v1_phase_forward(const SegDev &sg, bool stencil, bo
                 float S[1][OCT];
                 float4 *ra = (float4 *)(rowA + g * RL);
                 const int q0 = SW4(j0 >> 2), q1 = SW4((j0 >> 2) + 1);
-                if (stencil) {
+                if (stencil && !uniform) {
+                    // per-pixel kernels: S and its two kernel-parameter derivatives now, kept in thread-private scratch
+                    float DV[OCT], DG[OCT], EI[OCT];
+                    v1_np_forward_octet((const float4 *)(rowT + g * RL), j0, npp[g], isv, s2v, S[0], DV, DG, EI);
+                    ra[q0] = make_float4(S[0][0], S[0][1], S[0][2], S[0][3]);
+                    ra[q1] = make_float4(S[0][4], S[0][5], S[0][6], S[0][7]);
+                    float4 *d4 = (float4 *)(dsg + g * Ppad + (j0 >> 1));
+                    d4[0] = make_float4(DV[0], DV[1], DV[2], DV[3]); d4[P8] = make_float4(DV[4], DV[5], DV[6], DV[7]);
+                    d4 += GS * (Ppad >> 2);
+                    d4[0] = make_float4(DG[0], DG[1], DG[2], DG[3]); d4[P8] = make_float4(DG[4], DG[5], DG[6], DG[7]);
+                    d4 += GS * (Ppad >> 2);
+                    d4[0] = make_float4(EI[0], EI[1], EI[2], EI[3]); d4[P8] = make_float4(EI[4], EI[5], EI[6], EI[7]);
+                } else if (stencil) {
                     v1_stencil_octet<1>((const float4 *)(rowT + g * RL), j0, alo[g], nag[g], gw4 + g * NA, 0, S);
                     ra[q0] = make_float4(S[0][0], S[0][1], S[0][2], S[0][3]);
                     ra[q1] = make_float4(S[0][4], S[0][5], S[0][6], S[0][7]);
@@ -608,9 +771,11 @@ __device__ __noinline__ void v1_phase_residual(const SegDev &sg, int rowB, float
     size_t rowo[GS];
 #pragma unroll
     for (int g = 0; g < GS; ++g) rowo[g] = (size_t)v1_blk.spec[g] * Ppad;
-    float chi[GS], ng[GS], cmin[GS];
+    float chi[GS], ng[GS], cmin[GS], gvv[GS], gss[GS];
+    const bool uniform = sg.uniform != 0;
+    const float *dsg = v1_blk.ds;
 #pragma unroll
-    for (int g = 0; g < GS; ++g) { chi[g] = 0.f; ng[g] = 0.f; cmin[g] = 3.0e38f; }
+    for (int g = 0; g < GS; ++g) { chi[g] = 0.f; ng[g] = 0.f; cmin[g] = 3.0e38f; gvv[g] = 0.f; gss[g] = 0.f; }
     for (int j0 = fit_lo + V1_TID * OCT; j0 < fit_hi; j0 += nt8) {
         float cc[GS][OCT], pp[OCT], pc[OCT], x2[OCT];
         float4 yq[GS][2], wq[GS][2];   // flux / weight from L2, issued before the basis loop hides them
@@ -664,6 +829,23 @@ __device__ __noinline__ void v1_phase_residual(const SegDev &sg, int rowB, float
                 av[i] = -2.f * wr * cc[g][i];
                 if (MODE == 2) rho[i] = sqrtf(ww[i]) * r;
             }
+            if (!uniform) {
+                // per-pixel kernels: the two kernel-parameter gradients close here (dS/dv, dS/dsigma* were kept by the
+                // forward pass), and the adjoint handed to the stencil is a/E0 (each source pixel's own normalisation)
+                const float4 *d4 = (const float4 *)(dsg + g * Ppad + (j0 >> 1));
+                const float4 v0 = __ldcg(d4), v1 = __ldcg(d4 + P8);
+                const float4 g0 = __ldcg(d4 + GS * (Ppad >> 2)), g1 = __ldcg(d4 + GS * (Ppad >> 2) + P8);
+                const float4 e0 = __ldcg(d4 + 2 * GS * (Ppad >> 2)), e1 = __ldcg(d4 + 2 * GS * (Ppad >> 2) + P8);
+                const float DV[OCT] = {v0.x, v0.y, v0.z, v0.w, v1.x, v1.y, v1.z, v1.w};
+                const float DG[OCT] = {g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, g1.z, g1.w};
+                const float EI[OCT] = {e0.x, e0.y, e0.z, e0.w, e1.x, e1.y, e1.z, e1.w};
+#pragma unroll
+                for (int i = 0; i < OCT; ++i) {
+                    gvv[g] = fmaf(av[i], DV[i], gvv[g]);
+                    gss[g] = fmaf(av[i], DG[i], gss[g]);
+                    av[i] *= EI[i];
+                }
+            }
             ra[q0] = make_float4(av[0], av[1], av[2], av[3]);
             ra[q1] = make_float4(av[4], av[5], av[6], av[7]);
             if (MODE == 2) {
@@ -678,9 +860,12 @@ __device__ __noinline__ void v1_phase_residual(const SegDev &sg, int rowB, float
 #pragma unroll
         for (int g = 0; g < GS; ++g) {
             const float s = warp_sum_f(chi[g]), n = warp_sum_f(ng[g]), m = warp_min_f(cmin[g]);
+            float sv = 0.f, sg2 = 0.f;
+            if (!uniform) { sv = warp_sum_f(gvv[g]); sg2 = warp_sum_f(gss[g]); }
             if (V1_LANE == 0) {
                 float *st = red + SLOT_STAT(L) * GS + g;
                 st[0] += s; st[GS] += n; st[2 * GS] = fminf(st[2 * GS], m);
+                st[3 * GS] += sv; st[4 * GS] += sg2;
             }
         }
     }
@@ -706,8 +891,11 @@ __device__ __noinline__ void v1_phase_adjoint(const SegDev &sg, int lo, int hi)
     const float *rowA = V1SM + L.oA + L.GUARD - sg.po, *rowT = V1SM + L.oT + L.GUARD - sg.po;
     const float4 *gr4 = (const float4 *)(V1SM + L.oGR);
     int alo[GS], nag[GS];
+    const bool uniform = sg.uniform != 0;
+    const float *ISg = v1_blk.A.IS + V1_TPAD, *S2g = v1_blk.A.S2 + V1_TPAD;
+    V1Np npp[GS];
 #pragma unroll
-    for (int g = 0; g < GS; ++g) { alo[g] = tap[2 * g]; nag[g] = tap[2 * g + 1]; }
+    for (int g = 0; g < GS; ++g) { alo[g] = tap[2 * g]; nag[g] = tap[2 * g + 1]; npp[g] = ((const V1Np *)(V1SM + L.oNP))[g]; }
     for (int jb = lo; jb < hi; jb += nt8) {
         const int j0 = jb + V1_TID * OCT;
         const bool act = j0 < hi;
@@ -715,7 +903,13 @@ __device__ __noinline__ void v1_phase_adjoint(const SegDev &sg, int lo, int hi)
 #pragma unroll
         for (int g = 0; g < GS; ++g) {
             gv[g] = 0.f; gs[g] = 0.f;
-            if (act) {
+            if (act && !uniform) {
+                // sources up to H_seg above this octet carry the widest kernels (1/s_j grows with wavelength on
+                // a linear grid): bound the loop by the kernel of the farthest source in reach
+                const int hseg = 4 * (alo[g] + nag[g] - 1);
+                const float hb = fminf(npp[g].hbv * fmaxf(__ldg(ISg + j0 + OCT - 1 + hseg), __ldg(ISg + j0 - hseg)), npp[g].hcap);
+                v1_np_adjoint_octet((const float4 *)(rowA + g * RL), j0, (int)ceilf(hb), npp[g], ISg, S2g, t[g]);
+            } else if (act) {
                 float acc[3][OCT];
                 v1_stencil_octet<3>((const float4 *)(rowA + g * RL), j0, alo[g], nag[g], gr4 + g * NA, wstride4, acc);
                 const float4 *rt = (const float4 *)(rowT + g * RL);
@@ -910,8 +1104,12 @@ __device__ __noinline__ float v1_gradient(int g)
         gx = warp_sum_f(gx);
         if (V1_LANE == l) mine = gx;
     }
-    if (V1_LANE == nl) mine = SMV(L.oQ, K, g);
-    if (V1_LANE == nl + 1) mine = SMV(L.oQ, K + 1, g);
+    if (V1_LANE == nl || V1_LANE == nl + 1) {     // + the part closed in the residual phase (per-pixel kernels)
+        const int which = V1_LANE - nl;
+        float sx = SMV(L.oQ, K + which, g);
+        for (int w = 0; w < NW; ++w) sx += red[w * wst + (SLOT_STAT(L) + 3 + which) * GS + g];
+        mine = sx;
+    }
     if (V1_LANE < M.NP) mine *= SMV(L.oGSC, V1_LANE, g);   // chain rule to u (C.1 last lines)
     return mine;
 }
@@ -937,7 +1135,10 @@ __device__ __forceinline__ void v1_init_block(const ModelDev &M, const V1Lay &L,
     for (int i = threadIdx.x; i < (int)(sizeof(ModelDev) / 4); i += blockDim.x) ((int *)&v1_blk.M)[i] = ((const int *)&M)[i];
     for (int i = threadIdx.x; i < (int)(sizeof(V1Lay) / 4); i += blockDim.x) ((int *)&v1_blk.L)[i] = ((const int *)&L)[i];
     for (int i = threadIdx.x; i < (int)(sizeof(V1Args) / 4); i += blockDim.x) ((int *)&v1_blk.A)[i] = ((const int *)&a)[i];
-    if (threadIdx.x == 0) v1_blk.cp = a.CP + (size_t)blockIdx.x * GS * M.Ppad;
+    if (threadIdx.x == 0) {
+        v1_blk.cp = a.CP + (size_t)blockIdx.x * GS * M.Ppad;
+        v1_blk.ds = a.DS ? a.DS + (size_t)blockIdx.x * 3 * GS * M.Ppad : nullptr;
+    }
     for (int i = threadIdx.x; i < M.K * M.L; i += blockDim.x) ((uint8_t *)(V1SM + L.oEXP))[i] = M.exps[i];
     for (int i = threadIdx.x; i < GS * L.Kq; i += blockDim.x) V1SM[L.oPHI + i] = 0.f;   // phi is zero past K
     // rows T and A: zero-weight taps multiply whatever lies in the window, so it must at least be finite

@@ -30,7 +30,9 @@ struct lasp_ctx {
     long long launches = 0;
     double mean_dlog = 0;
     // kernel v1 (uniform segments): layout, launch shape, staged planes and scratch
-    bool v1_ok = false;
+    bool v1_ok = false, v1_nonuniform = false;
+    float *dIS = nullptr, *dS2 = nullptr, *dDS = nullptr;
+    size_t ds_ctas = 0;
     V1Lay V1;
     int v1_nt = 0, v1_maxt = 0, v1_cta_per_sm = 1;
     float *dY = nullptr, *dW = nullptr, *dC1 = nullptr;
@@ -123,7 +125,7 @@ extern "C" int lasp_destroy(lasp_ctx *c)
     cudaSetDevice(c->device);
     cudaFree(c->dC); cudaFree(c->dinv_s); cudaFree(c->dexps); cudaFree(c->dconv); cudaFree(c->dnedge);
     cudaFree(c->dYW); cudaFree(c->dscratch);
-    cudaFree(c->dC1); cudaFree(c->dY); cudaFree(c->dW); cudaFree(c->dCP); cudaFree(c->dXJ); cudaFree(c->ddbg);
+    cudaFree(c->dC1); cudaFree(c->dIS); cudaFree(c->dS2); cudaFree(c->dDS); cudaFree(c->dY); cudaFree(c->dW); cudaFree(c->dCP); cudaFree(c->dXJ); cudaFree(c->ddbg);
     hostpipe_free(c);
     if (c->hp.s_in) {
         cudaStreamDestroy(c->hp.s_in); cudaStreamDestroy(c->hp.s_out); cudaStreamDestroy(c->hp.s_fit);
@@ -285,6 +287,18 @@ extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx *
         CUDA_TRY_C(cudaMalloc(&c->dC1, C1.size() * sizeof(float)));
         CUDA_TRY_C(cudaMemcpy(c->dC1, C1.data(), C1.size() * sizeof(float), cudaMemcpyHostToDevice));
     }
+    {   // 1/s_j and s_j^2 for v1's per-pixel kernels, V1_TPAD replicated entries on both sides
+        std::vector<float> is1(M.Ppad + 2 * V1_TPAD), s21(M.Ppad + 2 * V1_TPAD);
+        for (int q = 0; q < M.Ppad + 2 * V1_TPAD; ++q) {
+            const int jp = std::min(std::max(q - V1_TPAD, 0), M.Ppad - 1);
+            is1[q] = isp[jp];
+            s21[q] = (float)(1.0 / ((double)isp[jp] * (double)isp[jp]));
+        }
+        CUDA_TRY_C(cudaMalloc(&c->dIS, is1.size() * sizeof(float)));
+        CUDA_TRY_C(cudaMemcpy(c->dIS, is1.data(), is1.size() * sizeof(float), cudaMemcpyHostToDevice));
+        CUDA_TRY_C(cudaMalloc(&c->dS2, s21.size() * sizeof(float)));
+        CUDA_TRY_C(cudaMemcpy(c->dS2, s21.data(), s21.size() * sizeof(float), cudaMemcpyHostToDevice));
+    }
     CUDA_TRY_C(cudaMalloc(&c->dinv_s, isp.size() * sizeof(float)));
     CUDA_TRY_C(cudaMemcpy(c->dinv_s, isp.data(), isp.size() * sizeof(float), cudaMemcpyHostToDevice));
     CUDA_TRY_C(cudaMalloc(&c->dexps, (size_t)K * L));
@@ -321,15 +335,18 @@ static int setup_v1(lasp_ctx *c, const cudaDeviceProp &prop, int emax)
 {
     const ModelDev &M = c->M;
     c->v1_ok = false;
-    int maxlen = 0, guard = 0, nfit = 0, hmax = 0;
+    int maxlen = 0, guard = 0, nfit = 0, hmax = 1;
+    c->v1_nonuniform = false;
     for (int s = 0; s < M.n_seg; ++s) {
         const SegDev &S = M.seg[s];
-        if (!S.uniform) return LASP_OK;   // per-pixel kernels (linear grids) stay on the v0 kernel
         maxlen = std::max(maxlen, S.len);
         guard = std::max(guard, S.halo);
         nfit = std::max(nfit, (S.fit_hi - S.fit_lo) / OCT);
-        hmax = std::max(hmax, S.halo - 18);
+        if (S.uniform) hmax = std::max(hmax, S.halo - 18);   // tap tables exist only for uniform segments
+        else c->v1_nonuniform = true;                         // per-pixel kernels (linear grids, C.2-14)
+        if (S.halo > V1_TPAD) return LASP_OK;
     }
+    if (getenv("LASP_V1_UNIFORM_ONLY") && c->v1_nonuniform) return LASP_OK;
     if (M.NP > 32 || M.n1 > 32) return LASP_OK;
     V1Lay &L = c->V1;
     memset(&L, 0, sizeof(L));
@@ -345,7 +362,7 @@ static int setup_v1(lasp_ctx *c, const cudaDeviceProp &prop, int emax)
     L.NA = (hmax + 3) / 4 + hmax / 4 + 2;
     L.n1r = roundup(M.n1, 8);
     L.nmomr = L.n1r + roundup(std::max(M.nmom - L.n1r, 0), 8);
-    L.VR = L.nmomr + L.n1r + roundup(M.K + 2, 8) + 4;
+    L.VR = L.nmomr + L.n1r + roundup(M.K + 2, 8) + 6;
     const char *rf = getenv("LASP_REFRESH");
     L.refresh = rf ? std::max(1, atoi(rf)) : 16;
     int o = 0;
@@ -362,6 +379,7 @@ static int setup_v1(lasp_ctx *c, const cudaDeviceProp &prop, int emax)
     L.oQ = take(GS * (M.K + 2)); L.oSC = take(GS * (SC_N + M.n_seg));
     L.oEXP = take((M.K * M.L + 3) / 4);
     L.oXP = take(GS * M.L * (L.emax + 1)); L.oDPHI = take(GS * M.L * M.K); L.oGSC = take(GS * M.NP);
+    L.oNP = take(GS * 8);
     L.oEW = take(GS * (2 * hmax + 2));
     L.total = o;
     const size_t bytes = (size_t)o * sizeof(float);
@@ -485,6 +503,11 @@ static int v1_workspace(lasp_ctx *c, int64_t B, bool need_xj)
         CUDA_TRY(c, cudaMalloc(&c->dCP, ctas * GS * M.Ppad * sizeof(float)));
         c->cp_ctas = ctas;
     }
+    if (c->v1_nonuniform && ctas > c->ds_ctas) {
+        cudaFree(c->dDS); c->dDS = nullptr; c->ds_ctas = 0;
+        CUDA_TRY(c, cudaMalloc(&c->dDS, ctas * 3 * GS * M.Ppad * sizeof(float)));
+        c->ds_ctas = ctas;
+    }
     if (need_xj && ctas > c->xj_ctas) {
         cudaFree(c->dXJ); c->dXJ = nullptr; c->xj_ctas = 0;
         CUDA_TRY(c, cudaMalloc(&c->dXJ, ctas * (size_t)(1 + M.NP) * GS * M.Ppad * sizeof(float)));
@@ -537,6 +560,7 @@ extern "C" int lasp_fit_batch(lasp_ctx *c, int64_t B, const float *flux, const f
         V1Args a;
         memset(&a, 0, sizeof(a));
         a.Y = c->dY; a.W = c->dW; a.C1 = c->dC1; a.CP = c->dCP; a.XJ = c->dXJ; a.B = B;
+        a.IS = c->dIS; a.S2 = c->dS2; a.DS = c->dDS;
         const int grid = v1_grid(c, B, a.ngroups);
         a.init = init; a.n_iter = opts->n_iter; a.lr = opts->lr; a.b1 = opts->beta1; a.b2 = opts->beta2;
         a.eps = opts->eps; a.fd_h = 2e-3f;  // fp32 central-difference step in u (C.2-22)
@@ -583,6 +607,7 @@ extern "C" int lasp_eval_grad(lasp_ctx *c, int64_t B, const float *flux, const f
         V1Args a;
         memset(&a, 0, sizeof(a));
         a.Y = c->dY; a.W = c->dW; a.C1 = c->dC1; a.CP = c->dCP; a.B = B;
+        a.IS = c->dIS; a.S2 = c->dS2; a.DS = c->dDS;
         const int grid = v1_grid(c, B, a.ngroups);
         a.gparams = params; a.chi2 = chi2; a.grad_u = grad_u; a.cont = cont; a.status = status;
         return v1_launch(c, true, a, grid, st);
