@@ -20,6 +20,15 @@ def two_arm_config(**kw):
     return synth.Config(**base)
 
 
+def two_arm_log_config(**kw):
+    """Two segments on a LOG grid with different instrumental widths (uniform kernels, several segments)."""
+    base = dict(cfg=9, name="pin-2arm-log", B=5, grid="log10", lam_min=4500.0, lam_max=5600.0, step=1e-4,
+                seg_bounds=(0, 500, 950), sigma_inst=(30.0, 60.0), K=12, L=3, D=6, n_iter=40, snr=(60.0, 60.0),
+                noise="const", mask_frac=0.04, parity_B=5)
+    base.update(kw)
+    return synth.Config(**base)
+
+
 def make(cfgobj, oracle_mod, B=None, noise_free=False):
     synth.CONFIGS["_tmp"] = cfgobj
     try:

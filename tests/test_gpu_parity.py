@@ -8,7 +8,7 @@ import numpy as np
 import pytest
 from numpy.polynomial import legendre as npleg
 
-from helpers import make, small_config, two_arm_config
+from helpers import make, small_config, two_arm_config, two_arm_log_config
 from paper_2512_24840_b200 import synth
 
 pytestmark = pytest.mark.gpu
@@ -139,6 +139,11 @@ def test_grad_config4_high_dim(gpu, oracle_mod):
     check_grad(gpu, oracle_mod, case, case["init"])
 
 
+def test_grad_two_arm_log_grid(gpu, oracle_mod):
+    case = make(two_arm_log_config(), oracle_mod, B=6)   # several uniform segments: slots do not alias
+    check_grad(gpu, oracle_mod, case, case["init"])
+
+
 # ------------------------------------------------------------------ full fits
 
 def test_fit_config0_all_64(gpu, oracle_mod):
@@ -155,6 +160,16 @@ def test_fit_config1_subset(gpu, oracle_mod):
 def test_fit_two_arm_linear(gpu, oracle_mod):
     case = make(two_arm_config(n_iter=120), oracle_mod, B=9)
     check_fit(gpu, oracle_mod, case, 120)
+
+
+def test_fit_two_arm_log_grid(gpu, oracle_mod):
+    case = make(two_arm_log_config(n_iter=60), oracle_mod, B=7)
+    check_fit(gpu, oracle_mod, case, 60)
+
+
+def test_fit_config4_subset(gpu, oracle_mod):
+    case = synth.make_case(4, oracle_mod.forward, B=5)   # K = 105, 13 labels, three linear-grid arms
+    check_fit(gpu, oracle_mod, case, 40)
 
 
 @pytest.mark.slow
