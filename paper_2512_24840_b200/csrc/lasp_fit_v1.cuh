@@ -490,6 +490,7 @@ __device__ __noinline__ void v1_phase_emulator(const SegDev &sg, int lo, int hi)
 // Partial sums over the thread's 8 pixels are reduced over the warp by register transposes and
 // land in this warp's reduction slots.
 // ------------------------------------------------------------------------------------------
+template <bool UNI>
 __device__ __noinline__ void v1_phase_forward(const SegDev &sg, bool stencil, bool mom)
 {
     const V1Args &a = v1_blk.A;
@@ -505,30 +506,44 @@ __device__ __noinline__ void v1_phase_forward(const SegDev &sg, bool stencil, bo
     const float4 *gw4 = (const float4 *)(V1SM + L.oGW);
     const float *Yg = a.Y, *Wg = a.W;
     const float *cpg = v1_blk.cp;
-    const bool uniform = sg.uniform != 0;
+    constexpr bool uniform = UNI;
     const float *ISg = a.IS + V1_TPAD, *S2g = a.S2 + V1_TPAD;
     float *dsg = v1_blk.ds;
     int alo[GS], nag[GS];
     size_t rowo[GS];
-    V1Np npp[GS];
 #pragma unroll
-    for (int g = 0; g < GS; ++g) {
-        alo[g] = tap[2 * g]; nag[g] = tap[2 * g + 1]; rowo[g] = (size_t)v1_blk.spec[g] * Ppad;
-        npp[g] = ((const V1Np *)(V1SM + L.oNP))[g];
-    }
+    for (int g = 0; g < GS; ++g) { alo[g] = tap[2 * g]; nag[g] = tap[2 * g + 1]; rowo[g] = (size_t)v1_blk.spec[g] * Ppad; }
     bool first = true;
     for (int jb = fit_lo; jb < fit_hi; jb += nt8, first = false) {   // uniform trip count
         const int j0 = jb + V1_TID * OCT;
         const bool act = j0 < fit_hi;
-        float u[GS][OCT], v[GS][OCT];
-        if (act) {
+        if (!uniform && stencil && act) {
+            // per-pixel kernels: a pass of its own (it needs most of the register file): S -> row A, and its two
+            // kernel-parameter derivatives and 1/E0 -> thread-private scratch
             float isv[OCT], s2v[OCT];
-            if (!uniform) {
+            {
                 const float4 a0 = __ldg((const float4 *)(ISg + j0)), a1 = __ldg((const float4 *)(ISg + j0) + 1);
                 const float4 b0 = __ldg((const float4 *)(S2g + j0)), b1 = __ldg((const float4 *)(S2g + j0) + 1);
                 isv[0] = a0.x; isv[1] = a0.y; isv[2] = a0.z; isv[3] = a0.w; isv[4] = a1.x; isv[5] = a1.y; isv[6] = a1.z; isv[7] = a1.w;
                 s2v[0] = b0.x; s2v[1] = b0.y; s2v[2] = b0.z; s2v[3] = b0.w; s2v[4] = b1.x; s2v[5] = b1.y; s2v[6] = b1.z; s2v[7] = b1.w;
             }
+            for (int g = 0; g < GS; ++g) {
+                float Sg[OCT], DV[OCT], DG[OCT], EI[OCT];
+                const V1Np np = ((const V1Np *)(V1SM + L.oNP))[g];
+                v1_np_forward_octet((const float4 *)(rowT + g * RL), j0, np, isv, s2v, Sg, DV, DG, EI);
+                float4 *ra = (float4 *)(rowA + g * RL);
+                ra[SW4(j0 >> 2)] = make_float4(Sg[0], Sg[1], Sg[2], Sg[3]);
+                ra[SW4((j0 >> 2) + 1)] = make_float4(Sg[4], Sg[5], Sg[6], Sg[7]);
+                float4 *d4 = (float4 *)(dsg + g * Ppad + (j0 >> 1));
+                d4[0] = make_float4(DV[0], DV[1], DV[2], DV[3]); d4[P8] = make_float4(DV[4], DV[5], DV[6], DV[7]);
+                d4 += GS * (Ppad >> 2);
+                d4[0] = make_float4(DG[0], DG[1], DG[2], DG[3]); d4[P8] = make_float4(DG[4], DG[5], DG[6], DG[7]);
+                d4 += GS * (Ppad >> 2);
+                d4[0] = make_float4(EI[0], EI[1], EI[2], EI[3]); d4[P8] = make_float4(EI[4], EI[5], EI[6], EI[7]);
+            }
+        }
+        float u[GS][OCT], v[GS][OCT];
+        if (act) {
 #pragma unroll
             for (int g = 0; g < GS; ++g) {
                 // flux / weight / c_prev rows come from L2: issue the loads first, the stencil hides them
@@ -540,19 +555,7 @@ __device__ __noinline__ void v1_phase_forward(const SegDev &sg, bool stencil, bo
                 float S[1][OCT];
                 float4 *ra = (float4 *)(rowA + g * RL);
                 const int q0 = SW4(j0 >> 2), q1 = SW4((j0 >> 2) + 1);
-                if (stencil && !uniform) {
-                    // per-pixel kernels: S and its two kernel-parameter derivatives now, kept in thread-private scratch
-                    float DV[OCT], DG[OCT], EI[OCT];
-                    v1_np_forward_octet((const float4 *)(rowT + g * RL), j0, npp[g], isv, s2v, S[0], DV, DG, EI);
-                    ra[q0] = make_float4(S[0][0], S[0][1], S[0][2], S[0][3]);
-                    ra[q1] = make_float4(S[0][4], S[0][5], S[0][6], S[0][7]);
-                    float4 *d4 = (float4 *)(dsg + g * Ppad + (j0 >> 1));
-                    d4[0] = make_float4(DV[0], DV[1], DV[2], DV[3]); d4[P8] = make_float4(DV[4], DV[5], DV[6], DV[7]);
-                    d4 += GS * (Ppad >> 2);
-                    d4[0] = make_float4(DG[0], DG[1], DG[2], DG[3]); d4[P8] = make_float4(DG[4], DG[5], DG[6], DG[7]);
-                    d4 += GS * (Ppad >> 2);
-                    d4[0] = make_float4(EI[0], EI[1], EI[2], EI[3]); d4[P8] = make_float4(EI[4], EI[5], EI[6], EI[7]);
-                } else if (stencil) {
+                if (stencil && uniform) {
                     v1_stencil_octet<1>((const float4 *)(rowT + g * RL), j0, alo[g], nag[g], gw4 + g * NA, 0, S);
                     ra[q0] = make_float4(S[0][0], S[0][1], S[0][2], S[0][3]);
                     ra[q1] = make_float4(S[0][4], S[0][5], S[0][6], S[0][7]);
@@ -756,7 +759,7 @@ __device__ __noinline__ void v1_phase_solve(int g, int seg, bool refactor)
 //   MODE 2: as 1, and rho = sqrt(w) r -> global row `xrow` (a9).
 // chi2 / ngood / cmin are reduced over the warp and accumulated in this warp's SLOT_STAT slots (zeroed by v1_evaluate).
 // ------------------------------------------------------------------------------------------
-template <int MODE>
+template <int MODE, bool UNI>
 __device__ __noinline__ void v1_phase_residual(const SegDev &sg, int rowB, float *xrow)
 {
     const V1Args &a = v1_blk.A;
@@ -772,7 +775,7 @@ __device__ __noinline__ void v1_phase_residual(const SegDev &sg, int rowB, float
 #pragma unroll
     for (int g = 0; g < GS; ++g) rowo[g] = (size_t)v1_blk.spec[g] * Ppad;
     float chi[GS], ng[GS], cmin[GS], gvv[GS], gss[GS];
-    const bool uniform = sg.uniform != 0;
+    constexpr bool uniform = UNI;
     const float *dsg = v1_blk.ds;
 #pragma unroll
     for (int g = 0; g < GS; ++g) { chi[g] = 0.f; ng[g] = 0.f; cmin[g] = 3.0e38f; gvv[g] = 0.f; gss[g] = 0.f; }
@@ -879,6 +882,7 @@ __device__ __noinline__ void v1_phase_residual(const SegDev &sg, int rowB, float
 // Partial sums go through register transposes into this warp's Q slots (pseudo-terms K, K+1 carry
 // the two kernel-parameter gradients), which v1_evaluate zeroed.
 // ------------------------------------------------------------------------------------------
+template <bool UNI>
 __device__ __noinline__ void v1_phase_adjoint(const SegDev &sg, int lo, int hi)
 {
     const V1Lay &L = v1_blk.L;
@@ -891,11 +895,11 @@ __device__ __noinline__ void v1_phase_adjoint(const SegDev &sg, int lo, int hi)
     const float *rowA = V1SM + L.oA + L.GUARD - sg.po, *rowT = V1SM + L.oT + L.GUARD - sg.po;
     const float4 *gr4 = (const float4 *)(V1SM + L.oGR);
     int alo[GS], nag[GS];
-    const bool uniform = sg.uniform != 0;
+    constexpr bool uniform = UNI;
     const float *ISg = v1_blk.A.IS + V1_TPAD, *S2g = v1_blk.A.S2 + V1_TPAD;
-    V1Np npp[GS];
+    V1Np npp[UNI ? 1 : GS];
 #pragma unroll
-    for (int g = 0; g < GS; ++g) { alo[g] = tap[2 * g]; nag[g] = tap[2 * g + 1]; npp[g] = ((const V1Np *)(V1SM + L.oNP))[g]; }
+    for (int g = 0; g < GS; ++g) { alo[g] = tap[2 * g]; nag[g] = tap[2 * g + 1]; if (!UNI) npp[UNI ? 0 : g] = ((const V1Np *)(V1SM + L.oNP))[g]; }
     for (int jb = lo; jb < hi; jb += nt8) {
         const int j0 = jb + V1_TID * OCT;
         const bool act = j0 < hi;
@@ -907,8 +911,8 @@ __device__ __noinline__ void v1_phase_adjoint(const SegDev &sg, int lo, int hi)
                 // sources up to H_seg above this octet carry the widest kernels (1/s_j grows with wavelength on
                 // a linear grid): bound the loop by the kernel of the farthest source in reach
                 const int hseg = 4 * (alo[g] + nag[g] - 1);
-                const float hb = fminf(npp[g].hbv * fmaxf(__ldg(ISg + j0 + OCT - 1 + hseg), __ldg(ISg + j0 - hseg)), npp[g].hcap);
-                v1_np_adjoint_octet((const float4 *)(rowA + g * RL), j0, (int)ceilf(hb), npp[g], ISg, S2g, t[g]);
+                const float hb = fminf(npp[UNI ? 0 : g].hbv * fmaxf(__ldg(ISg + j0 + OCT - 1 + hseg), __ldg(ISg + j0 - hseg)), npp[UNI ? 0 : g].hcap);
+                v1_np_adjoint_octet((const float4 *)(rowA + g * RL), j0, (int)ceilf(hb), npp[UNI ? 0 : g], ISg, S2g, t[g]);
             } else if (act) {
                 float acc[3][OCT];
                 v1_stencil_octet<3>((const float4 *)(rowA + g * RL), j0, alo[g], nag[g], gr4 + g * NA, wstride4, acc);
@@ -1038,7 +1042,7 @@ __device__ __noinline__ void v1_evaluate(bool cold, bool mom, float *xrow)
         tick(2);
         __syncthreads();
         tick(3);
-        v1_phase_forward(sg, true, mom || cold);
+        if (sg.uniform) v1_phase_forward<true>(sg, true, mom || cold); else v1_phase_forward<false>(sg, true, mom || cold);
         tick(4);
         __syncthreads();
         tick(5);
@@ -1047,19 +1051,20 @@ __device__ __noinline__ void v1_evaluate(bool cold, bool mom, float *xrow)
         __syncthreads();
         tick(7);
         if (cold) {
-            v1_phase_residual<0>(sg, rowB, nullptr);
+            v1_phase_residual<0, true>(sg, rowB, nullptr);
             __syncthreads();   // c_prev written by this thread only, but keep phases aligned
-            v1_phase_forward(sg, false, false);
+            v1_phase_forward<true>(sg, false, false);   // S is re-read from row A: no stencil, either kind
             __syncthreads();
             if (V1_WARP < GS) v1_phase_solve(V1_WARP, s, false);
             __syncthreads();
         }
-        v1_phase_residual<(MODE == 2 ? 2 : 1)>(sg, rowB, xrow);
+        if (sg.uniform) v1_phase_residual<(MODE == 2 ? 2 : 1), true>(sg, rowB, xrow);
+        else v1_phase_residual<(MODE == 2 ? 2 : 1), false>(sg, rowB, xrow);
         tick(8);
         __syncthreads();
         tick(9);
         if (MODE == 0) {
-            v1_phase_adjoint(sg, lo, hi);
+            if (sg.uniform) v1_phase_adjoint<true>(sg, lo, hi); else v1_phase_adjoint<false>(sg, lo, hi);
             tick(10);
             __syncthreads();
             tick(11);
