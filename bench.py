@@ -307,8 +307,15 @@ def run_gpu(args):
     kern_ms = float(np.mean(step_ms))          # events bracket stage + fit; stage share is in profiles/
     achieved = flop_launch / (kern_ms * 1e-3) / 1e12
     peak = prop.multi_processor_count * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    # DRAM traffic of the dominant kernel per launch: dram__bytes_read.sum + dram__bytes_write.sum of one
+    # `ncu --set full` capture of this very launch shape, recorded under profiles/ (null for other shapes)
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "r01_traffic.json")
+    if os.path.exists(tp):
+        with open(tp) as f:
+            traffic = json.load(f).get(f"config{args.config}_B{B}_n{n_iter}")
     roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-            "traffic": None, "kernel": "lasp_v1_fit_kernel" if model.uses_v1() else "lasp_fit_kernel", "fma_per_spectrum_step": fma_step,
+            "traffic": traffic, "kernel": "lasp_v1_fit_kernel" if model.uses_v1() else "lasp_fit_kernel", "fma_per_spectrum_step": fma_step,
             "mean_taps": taps, "peak_source": f"SMs x 128 FP32 lanes x 2 x sm_max_mhz ({peaks['source']})",
             "frac_at_sampled_clock": (achieved / (peak * clocks["sm_mhz"] / peaks["sm_max_mhz"])
                                       if clocks and clocks.get("sm_mhz") else None)}
