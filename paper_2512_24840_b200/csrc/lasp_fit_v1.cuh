@@ -1290,6 +1290,7 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
     v1_init_block(M, L, a);
     const int NP = M.NP, g = V1_WARP;
     for (int grp = blockIdx.x; grp < a.ngroups; grp += gridDim.x) {
+        __syncthreads();   // the previous group's last readers (output writers included) are done with the block state
         v1_set_group(grp);
         __syncthreads();   // the previous group's last readers are done with shared memory
         const bool valid = g < GS && (long long)grp * GS + g < a.B;
@@ -1307,7 +1308,8 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
         float pb1 = 1.f, pb2 = 1.f;
         for (int t = 1; t <= a.n_iter; ++t) {
             const long long te0 = a.dbg ? clock64() : 0;
-            v1_evaluate<0>(t == 1, (t - 1) % L.refresh == 0, nullptr);
+            // fresh Gram factor on each of the first `refresh` steps (the model moves fastest there), then every `refresh`-th
+            v1_evaluate<0>(t == 1, t <= L.refresh || (t - 1) % L.refresh == 0, nullptr);
             if (a.dbg && V1_TID == 0) { atomicAdd(a.dbg + 14, (unsigned long long)(clock64() - te0)); atomicAdd(a.dbg + 15, 1ull); }
             const long long tu0 = a.dbg ? clock64() : 0;
             pb1 *= a.b1; pb2 *= a.b2;
@@ -1377,6 +1379,7 @@ lasp_v1_grad_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ 
     v1_init_block(M, L, a);
     const int NP = M.NP, g = V1_WARP;
     for (int grp = blockIdx.x; grp < a.ngroups; grp += gridDim.x) {
+        __syncthreads();   // the previous group's last readers (output writers included) are done with the block state
         v1_set_group(grp);
         __syncthreads();
         const bool valid = g < GS && (long long)grp * GS + g < a.B;
