@@ -8,7 +8,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblasp_gpu.so")
 SOURCES = ["lasp_gpu.cu"]
-DEPS = ["lasp_gpu.cu", "lasp_kernels.cuh", "lasp_device.cuh", os.path.join("..", "..", "include", "lasp_gpu.h")]
+DEPS = ["lasp_gpu.cu", "lasp_fit_v1.cuh", "lasp_kernels.cuh", "lasp_device.cuh", os.path.join("..", "..", "include", "lasp_gpu.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC"]
 
@@ -23,7 +23,8 @@ def stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + \
+        extra = ["-DLASP_PHASE_TIMING"] if os.environ.get("LASP_PHASE_TIMING") else []   # debug build: phase timers
+        cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + \
               [os.path.join(CSRC, s) for s in SOURCES]
         subprocess.run(cmd, check=True)
     return LIB

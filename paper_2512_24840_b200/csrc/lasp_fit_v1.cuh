@@ -257,7 +257,7 @@ __device__ __forceinline__ void v1_stencil_octet(const float4 *__restrict__ row4
         for (int i = 0; i < OCT; ++i) acc[n][i] = 0.f;
     const int q = (j0 >> 2) - a_lo;
     float4 qb = row4[SW4(q + 1)], qc = row4[SW4(q + 2)];
-#pragma unroll 3
+#pragma unroll 1
     for (int ai = 0; ai < na; ++ai) {
         const float4 qa = row4[SW4(q - ai)];
         const float Wd[12] = {qa.x, qa.y, qa.z, qa.w, qb.x, qb.y, qb.z, qb.w, qc.x, qc.y, qc.z, qc.w};
@@ -491,7 +491,7 @@ __device__ __noinline__ void v1_phase_emulator(const SegDev &sg, int lo, int hi)
 // land in this warp's reduction slots.
 // ------------------------------------------------------------------------------------------
 template <bool UNI>
-__device__ __noinline__ void v1_phase_forward(const SegDev &sg, bool stencil, bool mom)
+__device__ __noinline__ void v1_phase_forward(const SegDev &sg, bool stencil)
 {
     const V1Args &a = v1_blk.A;
     const V1Lay &L = v1_blk.L;
@@ -542,7 +542,7 @@ __device__ __noinline__ void v1_phase_forward(const SegDev &sg, bool stencil, bo
                 d4[0] = make_float4(EI[0], EI[1], EI[2], EI[3]); d4[P8] = make_float4(EI[4], EI[5], EI[6], EI[7]);
             }
         }
-        float u[GS][OCT], v[GS][OCT];
+        float v[GS][OCT];
         if (act) {
 #pragma unroll
             for (int g = 0; g < GS; ++g) {
@@ -569,16 +569,14 @@ __device__ __noinline__ void v1_phase_forward(const SegDev &sg, bool stencil, bo
                 const float cc[OCT] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w};
 #pragma unroll
                 for (int i = 0; i < OCT; ++i) {
-                    const float ws = ww[i] * S[0][i];
-                    u[g][i] = ws * S[0][i];
-                    v[g][i] = ws * fmaf(-cc[i], S[0][i], yy[i]);
+                    v[g][i] = ww[i] * S[0][i] * fmaf(-cc[i], S[0][i], yy[i]);
                 }
             }
         } else {
 #pragma unroll
             for (int g = 0; g < GS; ++g)
 #pragma unroll
-                for (int i = 0; i < OCT; ++i) { u[g][i] = 0.f; v[g][i] = 0.f; }
+                for (int i = 0; i < OCT; ++i) v[g][i] = 0.f;
         }
         // Chebyshev recurrence state: (pp, pc) = (T_{n-1}, T_n), started at (T_{-1}, T_0) = (t, 1)
         float pp[OCT], pc[OCT], x2[OCT];
@@ -587,66 +585,83 @@ __device__ __noinline__ void v1_phase_forward(const SegDev &sg, bool stencil, bo
             const float t = fmaf(ta, (float)(j0 + i - torg), tb);
             pp[i] = t; pc[i] = 1.f; x2[i] = 2.f * t;
         }
-        if (mom) {
-            // region A: n < n1r, four n per transpose: value (nn, isrhs, g) at nn*8 + isrhs*4 + g
-            for (int n0 = 0; n0 < n1r; n0 += 4) {
-                float X[32];
+        // right-hand side only, eight n per transpose
+        for (int n0 = 0; n0 < n1r; n0 += 8) {
+            float X[32];
 #pragma unroll
-                for (int nn = 0; nn < 4; ++nn) {
+            for (int nn = 0; nn < 8; ++nn) {
 #pragma unroll
-                    for (int g = 0; g < GS; ++g) {
-                        float sm_ = 0.f, sr = 0.f;
+                for (int g = 0; g < GS; ++g) {
+                    float sr = 0.f;
 #pragma unroll
-                        for (int i = 0; i < OCT; ++i) { sm_ = fmaf(u[g][i], pc[i], sm_); sr = fmaf(v[g][i], pc[i], sr); }
-                        X[nn * 8 + g] = sm_; X[nn * 8 + 4 + g] = sr;
-                    }
-#pragma unroll
-                    for (int i = 0; i < OCT; ++i) { const float nx = fmaf(x2[i], pc[i], -pp[i]); pp[i] = pc[i]; pc[i] = nx; }
+                    for (int i = 0; i < OCT; ++i) sr = fmaf(v[g][i], pc[i], sr);
+                    X[nn * 4 + g] = sr;
                 }
-                const float tot = xreduce32(X, V1_LANE);
-                const int n = n0 + (V1_LANE >> 3), g = V1_LANE & 3;
-                const int slot = (V1_LANE & 4) ? nmomr + n : n;
-                if (first) red[slot * GS + g] = tot; else red[slot * GS + g] += tot;
+#pragma unroll
+                for (int i = 0; i < OCT; ++i) { const float nx = fmaf(x2[i], pc[i], -pp[i]); pp[i] = pc[i]; pc[i] = nx; }
             }
-            // region B: n1r <= n < nmomr, moments only, eight n per transpose: value (nn, g) at nn*4 + g
-            for (int n0 = n1r; n0 < nmomr; n0 += 8) {
-                float X[32];
+            const float tot = xreduce32(X, V1_LANE);
+            const int slot = nmomr + n0 + (V1_LANE >> 2);
+            if (first) red[slot * GS + (V1_LANE & 3)] = tot; else red[slot * GS + (V1_LANE & 3)] += tot;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// a5, refresh steps only: Gram moments  mom_n = sum_j u_j T_n(t_j), u = w S^2, n < 2D+1  (S is in row A, w comes
+// from L2 again).  Kept apart from v1_phase_forward so that the every-step code stays small.
+// ------------------------------------------------------------------------------------------
+__device__ __noinline__ void v1_phase_moments(const SegDev &sg)
+{
+    const V1Lay &L = v1_blk.L;
+    float *red = V1SM + L.oRED + V1_WARP * L.VR * GS;
+    const int Ppad = v1_blk.M.Ppad, P8 = Ppad >> 3, RL = L.RL, nmomr = L.nmomr, nt8 = V1_NT * OCT;
+    const int fit_lo = sg.fit_lo, fit_hi = sg.fit_hi, torg = sg.po + sg.halo;
+    const float ta = sg.ta, tb = sg.tb;
+    const float *rowA = V1SM + L.oA + L.GUARD - sg.po;
+    const float *Wg = v1_blk.A.W;
+    bool first = true;
+    for (int jb = fit_lo; jb < fit_hi; jb += nt8, first = false) {
+        const int j0 = jb + V1_TID * OCT;
+        const bool act = j0 < fit_hi;
+        float u[GS][OCT], pp[OCT], pc[OCT], x2[OCT];
 #pragma unroll
-                for (int nn = 0; nn < 8; ++nn) {
+        for (int g = 0; g < GS; ++g) {
 #pragma unroll
-                    for (int g = 0; g < GS; ++g) {
-                        float sm_ = 0.f;
+            for (int i = 0; i < OCT; ++i) u[g][i] = 0.f;
+            if (act) {
+                const size_t ro = (size_t)v1_blk.spec[g] * Ppad + (j0 >> 1);
+                const float4 w0 = __ldg((const float4 *)(Wg + ro)), w1 = __ldg((const float4 *)(Wg + ro) + P8);
+                const float4 *ra = (const float4 *)(rowA + g * RL);
+                const float4 s0 = ra[SW4(j0 >> 2)], s1 = ra[SW4((j0 >> 2) + 1)];
+                const float ww[OCT] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
+                const float SS[OCT] = {s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w};
 #pragma unroll
-                        for (int i = 0; i < OCT; ++i) sm_ = fmaf(u[g][i], pc[i], sm_);
-                        X[nn * 4 + g] = sm_;
-                    }
+                for (int i = 0; i < OCT; ++i) u[g][i] = ww[i] * SS[i] * SS[i];
+            }
+        }
 #pragma unroll
-                    for (int i = 0; i < OCT; ++i) { const float nx = fmaf(x2[i], pc[i], -pp[i]); pp[i] = pc[i]; pc[i] = nx; }
+        for (int i = 0; i < OCT; ++i) {
+            const float t = fmaf(ta, (float)(j0 + i - torg), tb);
+            pp[i] = t; pc[i] = 1.f; x2[i] = 2.f * t;
+        }
+        for (int n0 = 0; n0 < nmomr; n0 += 8) {      // eight n per transpose: value (nn, g) at nn*4 + g
+            float X[32];
+#pragma unroll
+            for (int nn = 0; nn < 8; ++nn) {
+#pragma unroll
+                for (int g = 0; g < GS; ++g) {
+                    float sm_ = 0.f;
+#pragma unroll
+                    for (int i = 0; i < OCT; ++i) sm_ = fmaf(u[g][i], pc[i], sm_);
+                    X[nn * 4 + g] = sm_;
                 }
-                const float tot = xreduce32(X, V1_LANE);
-                const int slot = n0 + (V1_LANE >> 2);
-                if (first) red[slot * GS + (V1_LANE & 3)] = tot; else red[slot * GS + (V1_LANE & 3)] += tot;
+#pragma unroll
+                for (int i = 0; i < OCT; ++i) { const float nx = fmaf(x2[i], pc[i], -pp[i]); pp[i] = pc[i]; pc[i] = nx; }
             }
-        } else {
-            // right-hand side only, eight n per transpose
-            for (int n0 = 0; n0 < n1r; n0 += 8) {
-                float X[32];
-#pragma unroll
-                for (int nn = 0; nn < 8; ++nn) {
-#pragma unroll
-                    for (int g = 0; g < GS; ++g) {
-                        float sr = 0.f;
-#pragma unroll
-                        for (int i = 0; i < OCT; ++i) sr = fmaf(v[g][i], pc[i], sr);
-                        X[nn * 4 + g] = sr;
-                    }
-#pragma unroll
-                    for (int i = 0; i < OCT; ++i) { const float nx = fmaf(x2[i], pc[i], -pp[i]); pp[i] = pc[i]; pc[i] = nx; }
-                }
-                const float tot = xreduce32(X, V1_LANE);
-                const int slot = nmomr + n0 + (V1_LANE >> 2);
-                if (first) red[slot * GS + (V1_LANE & 3)] = tot; else red[slot * GS + (V1_LANE & 3)] += tot;
-            }
+            const float tot = xreduce32(X, V1_LANE);
+            const int slot = n0 + (V1_LANE >> 2);
+            if (first) red[slot * GS + (V1_LANE & 3)] = tot; else red[slot * GS + (V1_LANE & 3)] += tot;
         }
     }
 }
@@ -661,8 +676,77 @@ __device__ __noinline__ void v1_phase_forward(const SegDev &sg, bool stencil, bo
 // ------------------------------------------------------------------------------------------
 #define V1_LFS (32 * 33 + 32)
 
+// Gram matrix from the moments, Cholesky with lanes = rows, factor kept in shared memory.  Its own function so that
+// the every-step solve below stays a few hundred instructions.
+__device__ __noinline__ void v1_refactor(int g, int seg)
+{
+    const ModelDev &M = v1_blk.M;
+    const V1Lay &L = v1_blk.L;
+    const int n1 = M.n1, lane = V1_LANE;
+    float *momS = V1SM + L.oMOM + g * L.nmomr;
+    float *lf = V1SM + L.oLF + g * V1_LFS;
+    float *invd = lf + 32 * 33;
+    const float *red = V1SM + L.oRED;
+    const int wst = L.VR * GS;
+    for (int n = lane; n < L.nmomr; n += 32) {
+        float s = 0.f;
+        for (int w = 0; w < L.NW; ++w) s += red[w * wst + SLOT_MOM(L, n) * GS + g];
+        momS[n] = s;
+    }
+    __syncwarp();
+    float row[32];
+#pragma unroll
+    for (int j = 0; j < 32; ++j) {
+        float v = (j == lane) ? 1.f : 0.f;
+        if (j < n1 && lane < n1) {
+            int d = lane - j;
+            d = d < 0 ? -d : d;
+            v = 0.5f * (momS[lane + j] + momS[d]);
+        }
+        row[j] = v;
+    }
+    const float m0 = momS[0];
+    bool ok = true;
+    float *colbuf = invd;   // 32 floats, overwritten with the reciprocals at the end
+#pragma unroll
+    for (int k = 0; k < 32; ++k) {
+        if (k < n1) {
+            const float d0 = 0.5f * (momS[2 * k] + m0);
+            const float d = __shfl_sync(FULL, row[k], k);
+            if (!(d > 1e-6f * d0)) ok = false;
+            const float lik = row[k] * rsqrtf(d);
+            row[k] = lik;
+            colbuf[lane] = lik;
+            __syncwarp();
+#pragma unroll
+            for (int j = k + 1; j < 32; ++j) row[j] = fmaf(-lik, colbuf[j], row[j]);
+            __syncwarp();
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < 32; ++j) lf[lane * 33 + j] = row[j];
+    __syncwarp();
+    invd[lane] = 1.f / lf[lane * 33 + lane];
+    if (lane == 0) SMV(L.oSC, SC_N + seg, g) = ok ? 0.f : 1.f;
+    __syncwarp();
+    // store the factor column-scaled to unit diagonal, Lt = L D^-1 (D = diag L): the two triangular
+    // solves of every step then have a shuffle + one FMA on their serial chain and no division;
+    // invd keeps 1/d^2 for the diagonal scaling between them:  A^-1 = Lt^-T D^-2 Lt^-1
+    {
+        const float mine = invd[lane];
+        float dj[32];
+#pragma unroll
+        for (int j = 0; j < 32; ++j) dj[j] = invd[j];
+        __syncwarp();
+#pragma unroll
+        for (int j = 0; j < 32; ++j) lf[lane * 33 + j] *= dj[j];
+        invd[lane] = mine * mine;
+    }
+}
+
 __device__ __noinline__ void v1_phase_solve(int g, int seg, bool refactor)
 {
+    if (refactor) v1_refactor(g, seg);
     const ModelDev &M = v1_blk.M;
     const V1Lay &L = v1_blk.L;
     const int n1 = M.n1, lane = V1_LANE, rowB = seg * M.n1;
@@ -676,62 +760,6 @@ __device__ __noinline__ void v1_phase_solve(int g, int seg, bool refactor)
         float s = 0.f;
         for (int w = 0; w < L.NW; ++w) s += red[w * wst + SLOT_RHS(L, n) * GS + g];
         rhsS[n] = s;
-    }
-    if (refactor) {
-        for (int n = lane; n < L.nmomr; n += 32) {
-            float s = 0.f;
-            for (int w = 0; w < L.NW; ++w) s += red[w * wst + SLOT_MOM(L, n) * GS + g];
-            momS[n] = s;
-        }
-        __syncwarp();
-        float row[32];
-#pragma unroll
-        for (int j = 0; j < 32; ++j) {
-            float v = (j == lane) ? 1.f : 0.f;
-            if (j < n1 && lane < n1) {
-                int d = lane - j;
-                d = d < 0 ? -d : d;
-                v = 0.5f * (momS[lane + j] + momS[d]);
-            }
-            row[j] = v;
-        }
-        const float m0 = momS[0];
-        bool ok = true;
-        float *colbuf = invd;   // 32 floats, overwritten with the reciprocals at the end
-#pragma unroll
-        for (int k = 0; k < 32; ++k) {
-            if (k < n1) {
-                const float d0 = 0.5f * (momS[2 * k] + m0);
-                const float d = __shfl_sync(FULL, row[k], k);
-                if (!(d > 1e-6f * d0)) ok = false;
-                const float lik = row[k] * rsqrtf(d);
-                row[k] = lik;
-                colbuf[lane] = lik;
-                __syncwarp();
-#pragma unroll
-                for (int j = k + 1; j < 32; ++j) row[j] = fmaf(-lik, colbuf[j], row[j]);
-                __syncwarp();
-            }
-        }
-#pragma unroll
-        for (int j = 0; j < 32; ++j) lf[lane * 33 + j] = row[j];
-        __syncwarp();
-        invd[lane] = 1.f / lf[lane * 33 + lane];
-        if (lane == 0) SMV(L.oSC, SC_N + seg, g) = ok ? 0.f : 1.f;
-        __syncwarp();
-        // store the factor column-scaled to unit diagonal, Lt = L D^-1 (D = diag L): the two triangular
-        // solves of every step then have a shuffle + one FMA on their serial chain and no division;
-        // invd keeps 1/d^2 for the diagonal scaling between them:  A^-1 = Lt^-T D^-2 Lt^-1
-        {
-            const float mine = invd[lane];
-            float dj[32];
-#pragma unroll
-            for (int j = 0; j < 32; ++j) dj[j] = invd[j];
-            __syncwarp();
-#pragma unroll
-            for (int j = 0; j < 32; ++j) lf[lane * 33 + j] *= dj[j];
-            invd[lane] = mine * mine;
-        }
     }
     __syncwarp();
     const bool ok = SMV(L.oSC, SC_N + seg, g) == 0.f;
@@ -996,10 +1024,14 @@ __device__ __noinline__ void v1_evaluate(bool cold, bool mom, float *xrow)
     // This warp's Q and statistics slots accumulate over sweeps and segments.  They are zeroed after
     // the first barrier of the evaluation: only then have warps g < GS finished reading the previous
     // evaluation's slots (v1_gradient / v1_stats run between evaluations without a barrier).
+#ifdef LASP_PHASE_TIMING
     long long tk = a.dbg ? clock64() : 0;
     auto tick = [&](int i) {
         if (a.dbg && V1_TID == 0) { const long long t = clock64(); atomicAdd(a.dbg + i, (unsigned long long)(t - tk)); tk = t; }
     };
+#else
+    auto tick = [](int) {};   // per-phase cycle counters: build with -DLASP_PHASE_TIMING
+#endif
     bool zeroed = false;
     auto zero_slots = [&]() {
         float *red = V1SM + L.oRED + V1_WARP * L.VR * GS;
@@ -1042,7 +1074,8 @@ __device__ __noinline__ void v1_evaluate(bool cold, bool mom, float *xrow)
         tick(2);
         __syncthreads();
         tick(3);
-        if (sg.uniform) v1_phase_forward<true>(sg, true, mom || cold); else v1_phase_forward<false>(sg, true, mom || cold);
+        if (sg.uniform) v1_phase_forward<true>(sg, true); else v1_phase_forward<false>(sg, true);
+        if (mom || cold) v1_phase_moments(sg);   // own octets of row A only: no barrier needed in between
         tick(4);
         __syncthreads();
         tick(5);
@@ -1053,7 +1086,7 @@ __device__ __noinline__ void v1_evaluate(bool cold, bool mom, float *xrow)
         if (cold) {
             v1_phase_residual<0, true>(sg, rowB, nullptr);
             __syncthreads();   // c_prev written by this thread only, but keep phases aligned
-            v1_phase_forward<true>(sg, false, false);   // S is re-read from row A: no stencil, either kind
+            v1_phase_forward<true>(sg, false);   // S is re-read from row A: no stencil, either kind
             __syncthreads();
             if (V1_WARP < GS) v1_phase_solve(V1_WARP, s, false);
             __syncthreads();
@@ -1307,11 +1340,15 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
         }
         float pb1 = 1.f, pb2 = 1.f;
         for (int t = 1; t <= a.n_iter; ++t) {
+#ifdef LASP_PHASE_TIMING
             const long long te0 = a.dbg ? clock64() : 0;
+#endif
             // fresh Gram factor on each of the first `refresh` steps (the model moves fastest there), then every `refresh`-th
             v1_evaluate<0>(t == 1, t <= L.refresh || (t - 1) % L.refresh == 0, nullptr);
+#ifdef LASP_PHASE_TIMING
             if (a.dbg && V1_TID == 0) { atomicAdd(a.dbg + 14, (unsigned long long)(clock64() - te0)); atomicAdd(a.dbg + 15, 1ull); }
             const long long tu0 = a.dbg ? clock64() : 0;
+#endif
             pb1 *= a.b1; pb2 *= a.b2;
             if (g < GS) {
                 const float gr = v1_gradient(g);
@@ -1331,7 +1368,9 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
                 __syncwarp();
                 v1_param_setup(g);
             }
+#ifdef LASP_PHASE_TIMING
             if (a.dbg && V1_TID == 0) atomicAdd(a.dbg + 13, (unsigned long long)(clock64() - tu0));
+#endif
         }
         // a9: one more evaluation at the final iterate (C.2-21)
         v1_evaluate<1>(a.n_iter == 0, true, nullptr);
