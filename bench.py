@@ -200,8 +200,9 @@ def run_reference(args):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic", "gpu_launches": 0,
-        "config": {"workload": f"config {args.config} ({cfg.name}) sample", "n_iter": cfg.n_iter,
-                   "n_pix": None, "sample_spectra": n_spec},
+        "config": {"workload": f"config {args.config} ({cfg.name})", "adam_steps": cfg.n_iter, "lr": cfg.lr,
+                   "n_terms": cfg.K, "n_labels": cfg.L, "cont_degree": cfg.D, "errors": True,
+                   "oracle_sample_spectra_per_step": n_spec},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }
