@@ -274,3 +274,18 @@ def test_fit_config1_full_size_sampled(gpu, oracle_mod):
         assert np.abs(err[i] / ref["err"][n] - 1).max() <= TOL_ERR, i
         assert st[i] == ref["status"][n], i
     m.close()
+
+
+# ------------------------------------------------------------------ streaming variant (rows too long for shared memory)
+
+def test_fit_long_spectrum_uses_streaming_variant(gpu, oracle_mod):
+    """SURVEY.md 8(d) shape "S" (one 17.4 k-pixel segment): its rows do not fit the fused kernel's shared memory, so
+    the library falls back to the lane-per-spectrum kernel with work arrays in global memory; same parity bar."""
+    case = synth.make_case("S", oracle_mod.forward, B=3)
+    m = gpu.LaspModel(case["desc"])
+    assert not m.uses_v1()
+    m.close()
+    check_fit(gpu, oracle_mod, case, 15)
+    m1 = gpu.LaspModel(synth.make_case(0, oracle_mod.forward, B=1)["desc"])
+    assert m1.uses_v1()
+    m1.close()
