@@ -28,7 +28,9 @@
  *    than seen before grows the ctx-owned workspace with cudaMalloc (use lasp_reserve to do that
  *    up front).
  *  - Parameter order everywhere: labels[0..L-1], rv (km/s), sigma* (km/s), physical units.
- *  - A ctx may be used from one host thread at a time; different ctxs are independent.
+ *  - A ctx may be used from one host thread at a time; different ctxs are independent.  All calls on one ctx
+ *    share its workspace: the library orders them on the device (a call on stream B waits for the ctx's previous
+ *    call on stream A), so mixing streams is safe but does not overlap.
  *  - Per-spectrum problems never fail a call; they set bits in status[i].
  */
 #ifndef LASP_GPU_H

@@ -38,6 +38,10 @@ struct lasp_ctx {
     float *dY = nullptr, *dW = nullptr, *dC1 = nullptr;
     size_t plane_rows = 0;
     float *dCP = nullptr, *dXJ = nullptr;
+    // the workspace (staged planes, scratch) is shared by every call on this ctx: each call waits, on ITS stream, for
+    // the previous call's work (possibly on another stream) and records its own completion
+    cudaEvent_t ws_event = nullptr;
+    bool ws_pending = false;
     unsigned long long *ddbg = nullptr;
     // lasp_fit_batch_host: double-buffered device chunks, two copy streams and one compute stream
     struct HostPipe {
@@ -126,6 +130,7 @@ extern "C" int lasp_destroy(lasp_ctx *c)
     cudaFree(c->dC); cudaFree(c->dinv_s); cudaFree(c->dexps); cudaFree(c->dconv); cudaFree(c->dnedge);
     cudaFree(c->dYW); cudaFree(c->dscratch);
     cudaFree(c->dC1); cudaFree(c->dIS); cudaFree(c->dS2); cudaFree(c->dDS); cudaFree(c->dY); cudaFree(c->dW); cudaFree(c->dCP); cudaFree(c->dXJ); cudaFree(c->ddbg);
+    if (c->ws_event) cudaEventDestroy(c->ws_event);
     hostpipe_free(c);
     if (c->hp.s_in) {
         cudaStreamDestroy(c->hp.s_in); cudaStreamDestroy(c->hp.s_out); cudaStreamDestroy(c->hp.s_fit);
@@ -524,6 +529,20 @@ static int v1_stage(lasp_ctx *c, int64_t B, const float *flux, const float *ivar
     return LASP_OK;
 }
 
+static int ws_acquire(lasp_ctx *c, cudaStream_t st)
+{
+    if (!c->ws_event) CUDA_TRY(c, cudaEventCreateWithFlags(&c->ws_event, cudaEventDisableTiming));
+    if (c->ws_pending) CUDA_TRY(c, cudaStreamWaitEvent(st, c->ws_event, 0));
+    return LASP_OK;
+}
+
+static int ws_release(lasp_ctx *c, cudaStream_t st)
+{
+    CUDA_TRY(c, cudaEventRecord(c->ws_event, st));
+    c->ws_pending = true;
+    return LASP_OK;
+}
+
 static int v1_launch(lasp_ctx *c, bool grad, const V1Args &a, int grid, cudaStream_t st)
 {
     const size_t smem = (size_t)c->V1.total * sizeof(float);
@@ -536,7 +555,7 @@ static int v1_launch(lasp_ctx *c, bool grad, const V1Args &a, int grid, cudaStre
     }
     c->launches += 1;
     CUDA_TRY(c, cudaGetLastError());
-    return LASP_OK;
+    return ws_release(c, st);
 }
 
 extern "C" int lasp_fit_batch(lasp_ctx *c, int64_t B, const float *flux, const float *ivar,
@@ -555,6 +574,8 @@ extern "C" int lasp_fit_batch(lasp_ctx *c, int64_t B, const float *flux, const f
         int rc = v1_workspace(c, B, err != nullptr);
         if (rc) return rc;
         cudaStream_t st = (cudaStream_t)stream;
+        rc = ws_acquire(c, st);
+        if (rc) return rc;
         rc = v1_stage(c, B, flux, ivar, mask, st);
         if (rc) return rc;
         V1Args a;
@@ -575,6 +596,8 @@ extern "C" int lasp_fit_batch(lasp_ctx *c, int64_t B, const float *flux, const f
     int rc = ensure_workspace(c, B, true);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
+    rc = ws_acquire(c, st);
+    if (rc) return rc;
     rc = stage(c, B, flux, ivar, mask, st);
     if (rc) return rc;
     FitArgs a;
@@ -588,7 +611,7 @@ extern "C" int lasp_fit_batch(lasp_ctx *c, int64_t B, const float *flux, const f
     lasp_fit_kernel<<<grid, wpb * 32, c->smem_per_warp * wpb, st>>>(c->M, a);
     c->launches += 1;
     CUDA_TRY(c, cudaGetLastError());
-    return LASP_OK;
+    return ws_release(c, st);
 }
 
 extern "C" int lasp_eval_grad(lasp_ctx *c, int64_t B, const float *flux, const float *ivar,
@@ -602,6 +625,8 @@ extern "C" int lasp_eval_grad(lasp_ctx *c, int64_t B, const float *flux, const f
         int rc = v1_workspace(c, B, false);
         if (rc) return rc;
         cudaStream_t st = (cudaStream_t)stream;
+        rc = ws_acquire(c, st);
+        if (rc) return rc;
         rc = v1_stage(c, B, flux, ivar, mask, st);
         if (rc) return rc;
         V1Args a;
@@ -615,6 +640,8 @@ extern "C" int lasp_eval_grad(lasp_ctx *c, int64_t B, const float *flux, const f
     int rc = ensure_workspace(c, B, true);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
+    rc = ws_acquire(c, st);
+    if (rc) return rc;
     rc = stage(c, B, flux, ivar, mask, st);
     if (rc) return rc;
     FitArgs a;
@@ -626,7 +653,7 @@ extern "C" int lasp_eval_grad(lasp_ctx *c, int64_t B, const float *flux, const f
     lasp_grad_kernel<<<grid, wpb * 32, c->smem_per_warp * wpb, st>>>(c->M, a);
     c->launches += 1;
     CUDA_TRY(c, cudaGetLastError());
-    return LASP_OK;
+    return ws_release(c, st);
 }
 
 extern "C" int lasp_eval_model(lasp_ctx *c, int64_t B, const float *params, const float *cont,
@@ -643,10 +670,12 @@ extern "C" int lasp_eval_model(lasp_ctx *c, int64_t B, const float *params, cons
     a.gparams = params; a.mcont = cont; a.model = model;
     int grid, wpb;
     launch_shape(c, a.tiles, grid, wpb);
+    rc = ws_acquire(c, (cudaStream_t)stream);
+    if (rc) return rc;
     lasp_model_kernel<<<grid, wpb * 32, c->smem_per_warp * wpb, (cudaStream_t)stream>>>(c->M, a);
     c->launches += 1;
     CUDA_TRY(c, cudaGetLastError());
-    return LASP_OK;
+    return ws_release(c, (cudaStream_t)stream);
 }
 
 // Algorithmic FMA of one Adam step of one spectrum: SURVEY.md 8(d) formula, moment route,
