@@ -887,17 +887,20 @@ __device__ __noinline__ void v1_phase_residual(const SegDev &sg, int rowB, float
         }
     }
     if (MODE != 0) {
+        // one register transpose for the sums (chi2, ngood, and the two kernel-parameter gradients of per-pixel
+        // segments): value (kind, g) at kind*4 + g; the minimum of c by shuffles
         float *red = V1SM + L.oRED + V1_WARP * L.VR * GS;
+        float X[32];
+#pragma unroll
+        for (int i = 0; i < 32; ++i) X[i] = 0.f;
+#pragma unroll
+        for (int g = 0; g < GS; ++g) { X[g] = chi[g]; X[4 + g] = ng[g]; X[12 + g] = gvv[g]; X[16 + g] = gss[g]; }
+        const float tot = xreduce32(X, V1_LANE);
+        if (V1_LANE < 20 && (V1_LANE < 8 || V1_LANE >= 12)) red[SLOT_STAT(L) * GS + V1_LANE] += tot;   // kinds 0,1,3,4
 #pragma unroll
         for (int g = 0; g < GS; ++g) {
-            const float s = warp_sum_f(chi[g]), n = warp_sum_f(ng[g]), m = warp_min_f(cmin[g]);
-            float sv = 0.f, sg2 = 0.f;
-            if (!uniform) { sv = warp_sum_f(gvv[g]); sg2 = warp_sum_f(gss[g]); }
-            if (V1_LANE == 0) {
-                float *st = red + SLOT_STAT(L) * GS + g;
-                st[0] += s; st[GS] += n; st[2 * GS] = fminf(st[2 * GS], m);
-                st[3 * GS] += sv; st[4 * GS] += sg2;
-            }
+            const float m = warp_min_f(cmin[g]);
+            if (V1_LANE == 0) { float *st = red + (SLOT_STAT(L) + 2) * GS + g; *st = fminf(*st, m); }
         }
     }
 }
