@@ -311,10 +311,13 @@ def run_gpu(args):
     # DRAM traffic of the dominant kernel per launch: dram__bytes_read.sum + dram__bytes_write.sum of one
     # `ncu --set full` capture of this very launch shape, recorded under profiles/ (null for other shapes)
     traffic = None
-    tp = os.path.join(ROOT, "profiles", "r01_traffic.json")
+    tp = os.path.join(ROOT, "profiles", "r01_traffic.csv")
     if os.path.exists(tp):
         with open(tp) as f:
-            traffic = json.load(f).get(f"config{args.config}_B{B}_n{n_iter}")
+            for ln in f.read().splitlines()[1:]:
+                k, _, v = ln.partition(",")
+                if k == f"config{args.config}_B{B}_n{n_iter}":
+                    traffic = int(v)
     roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
             "traffic": traffic, "kernel": "lasp_v1_fit_kernel" if model.uses_v1() else "lasp_fit_kernel", "fma_per_spectrum_step": fma_step,
             "mean_taps": taps, "peak_source": f"SMs x 128 FP32 lanes x 2 x sm_max_mhz ({peaks['source']})",
