@@ -139,6 +139,17 @@ def test_grad_config4_high_dim(gpu, oracle_mod):
     check_grad(gpu, oracle_mod, case, case["init"])
 
 
+def test_grad_widest_kernels_need_two_sweeps(gpu, oracle_mod):
+    """|v| and sigma* near the edge of the prior box: support H = 28, the T range no longer fits one sweep of the
+    CTA's 192 threads (config-1 shapes), so the emulator / adjoint loops take their second pass."""
+    case = synth.make_case(1, oracle_mod.forward, B=9)
+    params = case["init"].copy()
+    L = case["desc"]["n_labels"]
+    params[:, L] = np.where(np.arange(9) % 2 == 0, 390.0, -385.0)
+    params[:, L + 1] = np.linspace(250.0, 298.0, 9)
+    check_grad(gpu, oracle_mod, case, params)
+
+
 def test_grad_two_arm_log_grid(gpu, oracle_mod):
     case = make(two_arm_log_config(), oracle_mod, B=6)   # several uniform segments: slots do not alias
     check_grad(gpu, oracle_mod, case, case["init"])
