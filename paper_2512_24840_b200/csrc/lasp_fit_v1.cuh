@@ -1355,6 +1355,9 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
             pb1 *= a.b1; pb2 *= a.b2;
             if (g < GS) {
                 const float gr = v1_gradient(g);
+#ifdef LASP_PHASE_TIMING
+                if (a.dbg && V1_TID == 0) atomicAdd(a.dbg + 16, (unsigned long long)(clock64() - tu0));
+#endif
                 // a8: Adam (C.2-20), then clip to the prior box (C.2-18); lane p owns parameter p
                 for (int p0 = 0; p0 < NP; p0 += 32) {   // NP <= 32
                     const int p = p0 + V1_LANE;
@@ -1369,6 +1372,9 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
                     }
                 }
                 __syncwarp();
+#ifdef LASP_PHASE_TIMING
+                if (a.dbg && V1_TID == 0) atomicAdd(a.dbg + 17, (unsigned long long)(clock64() - tu0));
+#endif
                 v1_param_setup(g);
             }
 #ifdef LASP_PHASE_TIMING

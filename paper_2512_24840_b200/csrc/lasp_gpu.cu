@@ -118,7 +118,7 @@ extern "C" int lasp_debug_launch_info(const lasp_ctx *c, int *out4)
 extern "C" int lasp_debug_phase_cycles(lasp_ctx *c, unsigned long long *out16)
 {
     if (!c || !c->ddbg) return LASP_ERR_INVALID_ARG;
-    return cudaMemcpy(out16, c->ddbg, 16 * sizeof(unsigned long long), cudaMemcpyDeviceToHost) == cudaSuccess ? LASP_OK : LASP_ERR_CUDA;
+    return cudaMemcpy(out16, c->ddbg, 24 * sizeof(unsigned long long), cudaMemcpyDeviceToHost) == cudaSuccess ? LASP_OK : LASP_ERR_CUDA;
 }
 
 extern "C" int64_t lasp_launch_count(const lasp_ctx *ctx) { return ctx ? ctx->launches : 0; }
@@ -587,8 +587,8 @@ extern "C" int lasp_fit_batch(lasp_ctx *c, int64_t B, const float *flux, const f
         a.eps = opts->eps; a.fd_h = 2e-3f;  // fp32 central-difference step in u (C.2-22)
         a.params = params; a.cont = cont; a.chi2 = chi2; a.err = err; a.status = status;
         if (getenv("LASP_TIMING")) {
-            if (!c->ddbg) { CUDA_TRY(c, cudaMalloc(&c->ddbg, 16 * sizeof(unsigned long long))); }
-            CUDA_TRY(c, cudaMemsetAsync(c->ddbg, 0, 16 * sizeof(unsigned long long), st));
+            if (!c->ddbg) { CUDA_TRY(c, cudaMalloc(&c->ddbg, 24 * sizeof(unsigned long long))); }
+            CUDA_TRY(c, cudaMemsetAsync(c->ddbg, 0, 24 * sizeof(unsigned long long), st));
             a.dbg = c->ddbg;
         }
         return v1_launch(c, false, a, grid, st);
