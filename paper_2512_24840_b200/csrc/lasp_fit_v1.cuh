@@ -61,6 +61,7 @@ struct V1Args {
     // both sides, and per-CTA scratch [3][GS][Ppad] for dS/dv, dS/dsigma*, 1/E0 (thread-private pixels)
     const float *IS, *S2;
     float *DS;
+    unsigned int *queue;   // work-queue counter for the fit kernel (zeroed before the launch), may be null
 };
 #define V1_TPAD 256
 
@@ -112,6 +113,7 @@ struct V1Block {
     long long spec[GS];   // clamped spectrum indices of the group
     float *cp;            // this CTA's c_prev scratch
     float *ds;            // this CTA's dS/dv, dS/dsigma*, 1/E0 scratch (per-pixel-kernel segments)
+    int next;             // next group of this CTA (dynamic work queue)
 };
 __shared__ V1Block v1_blk;
 #define V1_TID ((int)threadIdx.x)
@@ -1325,10 +1327,14 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
 {
     v1_init_block(M, L, a);
     const int NP = M.NP, g = V1_WARP;
-    for (int grp = blockIdx.x; grp < a.ngroups; grp += gridDim.x) {
+    // groups are handed out by a global counter (the first gridDim.x statically): fits differ a little in length
+    // (kernel supports, early cold steps), and the last wave would otherwise leave SMs idle
+    for (int grp = blockIdx.x; grp < a.ngroups;) {
         __syncthreads();   // the previous group's last readers (output writers included) are done with the block state
         v1_set_group(grp);
-        __syncthreads();   // the previous group's last readers are done with shared memory
+        if (threadIdx.x == 0) v1_blk.next = a.queue ? (int)gridDim.x + (int)atomicAdd(a.queue, 1u) : grp + (int)gridDim.x;
+        __syncthreads();
+        const int grp_next = v1_blk.next;
         const bool valid = g < GS && (long long)grp * GS + g < a.B;
         if (g < GS) {
             for (int p = V1_LANE; p < NP; p += 32) {
@@ -1414,6 +1420,7 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
             }
         }
         if (a.err) v1_errors(chi2, ngood, valid);
+        grp = grp_next;
     }
 }
 

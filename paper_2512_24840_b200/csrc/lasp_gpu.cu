@@ -40,6 +40,7 @@ struct lasp_ctx {
     float *dCP = nullptr, *dXJ = nullptr;
     // the workspace (staged planes, scratch) is shared by every call on this ctx: each call waits, on ITS stream, for
     // the previous call's work (possibly on another stream) and records its own completion
+    unsigned int *dqueue = nullptr;
     cudaEvent_t ws_event = nullptr;
     bool ws_pending = false;
     unsigned long long *ddbg = nullptr;
@@ -129,7 +130,7 @@ extern "C" int lasp_destroy(lasp_ctx *c)
     cudaSetDevice(c->device);
     cudaFree(c->dC); cudaFree(c->dinv_s); cudaFree(c->dexps); cudaFree(c->dconv); cudaFree(c->dnedge);
     cudaFree(c->dYW); cudaFree(c->dscratch);
-    cudaFree(c->dC1); cudaFree(c->dIS); cudaFree(c->dS2); cudaFree(c->dDS); cudaFree(c->dY); cudaFree(c->dW); cudaFree(c->dCP); cudaFree(c->dXJ); cudaFree(c->ddbg);
+    cudaFree(c->dC1); cudaFree(c->dIS); cudaFree(c->dS2); cudaFree(c->dDS); cudaFree(c->dY); cudaFree(c->dW); cudaFree(c->dCP); cudaFree(c->dXJ); cudaFree(c->ddbg); cudaFree(c->dqueue);
     if (c->ws_event) cudaEventDestroy(c->ws_event);
     hostpipe_free(c);
     if (c->hp.s_in) {
@@ -586,6 +587,9 @@ extern "C" int lasp_fit_batch(lasp_ctx *c, int64_t B, const float *flux, const f
         a.init = init; a.n_iter = opts->n_iter; a.lr = opts->lr; a.b1 = opts->beta1; a.b2 = opts->beta2;
         a.eps = opts->eps; a.fd_h = 2e-3f;  // fp32 central-difference step in u (C.2-22)
         a.params = params; a.cont = cont; a.chi2 = chi2; a.err = err; a.status = status;
+        if (!c->dqueue) CUDA_TRY(c, cudaMalloc(&c->dqueue, sizeof(unsigned int)));
+        CUDA_TRY(c, cudaMemsetAsync(c->dqueue, 0, sizeof(unsigned int), st));
+        a.queue = c->dqueue;
         if (getenv("LASP_TIMING")) {
             if (!c->ddbg) { CUDA_TRY(c, cudaMalloc(&c->ddbg, 24 * sizeof(unsigned long long))); }
             CUDA_TRY(c, cudaMemsetAsync(c->ddbg, 0, 24 * sizeof(unsigned long long), st));
