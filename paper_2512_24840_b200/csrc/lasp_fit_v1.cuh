@@ -36,6 +36,10 @@ struct V1Lay {
     int n1r, nmomr, VR;     // n1 rounded to 4; moments rounded; reduction slots per warp (x GS)
     int NW;                 // warps per CTA
     int Hm;                 // support clamp (memory safety outside the prior box)
+    int fastw;              // 1: v1_update_fast also prepares the next step's kernel weights (one uniform segment)
+    int fastupd;            // 1: v1_update_fast applies (L <= 4, K + 2 <= 32, NW <= 12)
+    int lfseg;              // 1: one factor slot per segment (0: one slot, re-factored every step when n_seg > 1)
+    int warm;               // the first `warm` steps always re-factor
     int refresh;            // re-accumulate the Gram moments and re-factor every `refresh` steps
     // shared-memory offsets (floats)
     int oT, oA, oU, oM, oV, oX, oPHI, oGW, oGR, oTAP, oMOM, oRHS, oB, oRED, oLF, oQ, oSC, oEXP, oXP, oDPHI, oGSC, oEW, oNP, total;
@@ -155,6 +159,36 @@ __device__ __noinline__ void v1_param_setup(int g)
     }
     __syncwarp();
     // phi_k = prod_l x_l^e_kl and d phi_k / d x_l = e_kl x_l^(e_kl - 1) prod_{l2 != l} x_l2^e_kl2  (Eq. 1)
+    if (nl <= 4) {
+        // up to four labels: the exponents of term k come packed in one word (v1_init_block), so every table read of
+        // a term issues at once instead of as a chain of byte loads (this phase is one warp's latency, nothing else)
+        const unsigned *exw = (const unsigned *)(V1SM + L.oEXP);
+        const float *xp = V1SM + L.oXP + g;
+        for (int k = V1_LANE; k < K; k += 32) {
+            const unsigned w = exw[k];
+            float pe[4], pm[4];
+#pragma unroll
+            for (int l = 0; l < 4; ++l) {
+                const int e = (w >> (8 * l)) & 255;
+                pe[l] = l < nl ? xp[(e * nl + l) * GS] : 1.f;
+                pm[l] = (l < nl && e > 0) ? (float)e * xp[((e - 1) * nl + l) * GS] : 0.f;
+            }
+            float ph = 1.f;
+#pragma unroll
+            for (int l = 0; l < 4; ++l) ph *= pe[l];
+            SMV(L.oPHI, k, g) = ph;
+#pragma unroll
+            for (int l = 0; l < 4; ++l) {
+                float d = pm[l];
+#pragma unroll
+                for (int l2 = 0; l2 < 4; ++l2)
+                    if (l2 != l) d *= pe[l2];
+                if (l < nl) SMV(L.oDPHI, l * K + k, g) = d;
+            }
+        }
+        __syncwarp();
+        return;
+    }
     for (int k = V1_LANE; k < K; k += 32) {
         float p = 1.f;
         for (int l = 0; l < nl; ++l) p *= SMV(L.oXP, ex[k * nl + l] * nl + l, g);
@@ -180,13 +214,67 @@ __device__ __noinline__ void v1_param_setup(int g)
 //   GR [j][g][a][4]    reversed kernels for the adjoint pass: j=0: g_{-k}; j=1: d g_{-k}/dv;
 //                      j=2: d g_{-k}/d sigma* (chain factors of C.1 folded in)
 // ------------------------------------------------------------------------------------------
+// Uniform segment, given (v, sigma*).  Lanes = table entries: entry idx is tap k = 4 (a_lo + idx/4) - 3 + idx%4, and the
+// lane evaluates the exponential of its forward tap k and of its reversed tap -k itself, so nothing is exchanged
+// between lanes except the three sums (this runs on one warp between two phases of all: its latency is the cost).
+__device__ __forceinline__ void v1_weights_uniform(const SegDev &sg, int g, float v, float sigstar)
+{
+    const V1Lay &L = v1_blk.L;
+    const float sig_inst = sg.sig_inst, inv_s = sg.inv_s;
+    const int hcap = sg.halo - 18;
+    float *gw = V1SM + L.oGW + g * L.NA * 4;
+    float *gr = V1SM + L.oGR + g * L.NA * 4;
+    const int rs = GS * L.NA * 4;
+    const float sigtot = sqrtf(sigstar * sigstar + sig_inst * sig_inst);
+    const float mu = v * inv_s, s = sigtot * inv_s;
+    int H = (int)ceilf(fabsf(mu) + 5.f * s);
+    H = min(max(H, 0), hcap);   // memory safety outside the prior box (halo >= Hmax + 18)
+    const float i2 = 0.5f / (s * s);
+    const int a_lo = -(H / 4), na = (H + 3) / 4 - a_lo + 1;
+    float sum = 0.f, s1 = 0.f, s2 = 0.f;
+    for (int i0 = 0; i0 < na * 4; i0 += 32) {
+        const int idx = i0 + V1_LANE;
+        const int k = 4 * (a_lo + (idx >> 2)) - 3 + (idx & 3);
+        const float d = (float)k - mu;
+        const float e = (idx < na * 4 && k >= -H && k <= H) ? expf(-d * d * i2) : 0.f;
+        sum += e; s1 = fmaf(e, d, s1); s2 = fmaf(e * d, d, s2);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        sum += __shfl_xor_sync(FULL, sum, o); s1 += __shfl_xor_sync(FULL, s1, o); s2 += __shfl_xor_sync(FULL, s2, o);
+    }
+    const float inv = 1.f / sum;
+    const float e1n = s1 * inv, e2n = s2 * inv;       // kbar - mu ; second moment about mu
+    const float is2 = 2.f * i2;                        // 1/sigma^2 (pixels)
+    const float cmu = is2 * inv_s;                     // dS/dv      = (1/s) sum dg/dmu T
+    const float csig = is2 * sqrtf(is2) * (sigstar / sigtot) * inv_s;
+    for (int i0 = 0; i0 < na * 4; i0 += 32) {
+        const int idx = i0 + V1_LANE;
+        if (idx < na * 4) {
+            const int k = 4 * (a_lo + (idx >> 2)) - 3 + (idx & 3);
+            const bool in = (k >= -H) && (k <= H);
+            const float df = (float)k - mu, dr = (float)(-k) - mu;
+            gw[idx] = in ? expf(-df * df * i2) * inv : 0.f;
+            const float gg = in ? expf(-dr * dr * i2) * inv : 0.f;
+            gr[idx] = gg;
+            gr[rs + idx] = gg * (dr - e1n) * cmu;
+            gr[2 * rs + idx] = gg * (dr * dr - e2n) * csig;
+        }
+    }
+    if (V1_LANE == 0) {
+        int *tap = (int *)(V1SM + L.oTAP);
+        tap[g * 2] = a_lo; tap[g * 2 + 1] = na;
+    }
+    __syncwarp();
+}
+
 __device__ __noinline__ void v1_setup_weights(const SegDev &sg, int g)
 {
     const V1Lay &L = v1_blk.L;
     const float v = SMV(L.oSC, SC_V, g), sigstar = SMV(L.oSC, SC_SIG, g);
-    const float sigtot = sqrtf(sigstar * sigstar + sg.sig_inst * sg.sig_inst);
     if (!sg.uniform) {
         // per-pixel kernels: only the spectrum's scalars and the segment-wide reach (sg.inv_s = largest 1/s_j)
+        const float sigtot = sqrtf(sigstar * sigstar + sg.sig_inst * sg.sig_inst);
         if (V1_LANE == 0) {
             V1Np *np = (V1Np *)(V1SM + L.oNP) + g;
             np->v = v; np->sigstar = sigstar; np->sigtot = sigtot;
@@ -200,46 +288,7 @@ __device__ __noinline__ void v1_setup_weights(const SegDev &sg, int g)
         __syncwarp();
         return;
     }
-    const float mu = v * sg.inv_s, s = sigtot * sg.inv_s;
-    int H = (int)ceilf(fabsf(mu) + 5.f * s);
-    H = min(max(H, 0), sg.halo - 18);   // memory safety outside the prior box (halo >= Hmax + 18)
-    const float i2 = 0.5f / (s * s);
-    // one exponential per tap, kept in shared memory; the grouped forward / reversed / derivative tables are
-    // filled from it
-    float *ew = V1SM + L.oEW + g * (2 * L.Hm + 2);
-    float sum = 0.f, s1 = 0.f, s2 = 0.f;
-    for (int m = V1_LANE; m <= 2 * H; m += 32) {
-        const float d = (float)(m - H) - mu;
-        const float e = expf(-d * d * i2);
-        ew[m] = e;
-        sum += e; s1 = fmaf(e, d, s1); s2 = fmaf(e * d, d, s2);
-    }
-    __syncwarp();
-    sum = warp_sum_f(sum); s1 = warp_sum_f(s1); s2 = warp_sum_f(s2);
-    const float inv = 1.f / sum;
-    const float e1n = s1 * inv, e2n = s2 * inv;       // kbar - mu ; second moment about mu
-    const float is2 = 2.f * i2;                        // 1/sigma^2 (pixels)
-    const float cmu = is2 * sg.inv_s;                  // dS/dv      = (1/s) sum dg/dmu T
-    const float csig = is2 * sqrtf(is2) * (sigstar / sigtot) * sg.inv_s;
-    const int a_lo = -(H / 4), na = (H + 3) / 4 - a_lo + 1;
-    float *gw = V1SM + L.oGW + g * L.NA * 4;
-    float *gr = V1SM + L.oGR + g * L.NA * 4;
-    const int rs = GS * L.NA * 4;
-    for (int idx = V1_LANE; idx < na * 4; idx += 32) {
-        const int k = 4 * (a_lo + (idx >> 2)) - 3 + (idx & 3);
-        const bool in = (k >= -H) && (k <= H);
-        gw[idx] = in ? ew[k + H] * inv : 0.f;
-        const float d = (float)(-k) - mu;
-        const float gg = in ? ew[H - k] * inv : 0.f;
-        gr[idx] = gg;
-        gr[rs + idx] = gg * (d - e1n) * cmu;
-        gr[2 * rs + idx] = gg * (d * d - e2n) * csig;
-    }
-    if (V1_LANE == 0) {
-        int *tap = (int *)(V1SM + L.oTAP);
-        tap[g * 2] = a_lo; tap[g * 2 + 1] = na;
-    }
-    __syncwarp();
+    v1_weights_uniform(sg, g, v, sigstar);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -677,6 +726,7 @@ __device__ __noinline__ void v1_phase_moments(const SegDev &sg)
 // LF[row*33 + col] holds the unit-diagonal factor Lt = L D^-1, then the 32 values 1/d^2.
 // ------------------------------------------------------------------------------------------
 #define V1_LFS (32 * 33 + 32)
+#define V1_INVC 16       // columns of the inverse per pass
 
 // Gram matrix from the moments, Cholesky with lanes = rows, factor kept in shared memory.  Its own function so that
 // the every-step solve below stays a few hundred instructions.
@@ -686,7 +736,7 @@ __device__ __noinline__ void v1_refactor(int g, int seg)
     const V1Lay &L = v1_blk.L;
     const int n1 = M.n1, lane = V1_LANE;
     float *momS = V1SM + L.oMOM + g * L.nmomr;
-    float *lf = V1SM + L.oLF + g * V1_LFS;
+    float *lf = V1SM + L.oLF + (seg * L.lfseg * GS + g) * V1_LFS;
     float *invd = lf + 32 * 33;
     const float *red = V1SM + L.oRED;
     const int wst = L.VR * GS;
@@ -696,90 +746,159 @@ __device__ __noinline__ void v1_refactor(int g, int seg)
         momS[n] = s;
     }
     __syncwarp();
-    float row[32];
+    // This function runs once per `refresh` steps, so its instructions are never in the instruction cache when it
+    // starts: everything is a short loop over shared memory (the fully unrolled register version spent most of its
+    // time fetching 50 KB of straight-line code).  Row `lane` of A, identity padding beyond n1.
+    float *own = lf + lane * 33;                  // this lane's row
+#pragma unroll 1
+    for (int j0 = 0; j0 < 32; j0 += 8) {
+        float v[8];
 #pragma unroll
-    for (int j = 0; j < 32; ++j) {
-        float v = (j == lane) ? 1.f : 0.f;
-        if (j < n1 && lane < n1) {
+        for (int u = 0; u < 8; ++u) {
+            const int j = j0 + u;
             int d = lane - j;
             d = d < 0 ? -d : d;
-            v = 0.5f * (momS[lane + j] + momS[d]);
+            v[u] = (j < n1 && lane < n1) ? 0.5f * (momS[lane + j] + momS[d]) : (j == lane ? 1.f : 0.f);
         }
-        row[j] = v;
+#pragma unroll
+        for (int u = 0; u < 8; ++u) own[j0 + u] = v[u];
     }
+    __syncwarp();
     const float m0 = momS[0];
     bool ok = true;
-    float *colbuf = invd;   // 32 floats, overwritten with the reciprocals at the end
+#pragma unroll 1
+    for (int k = 0; k < n1; ++k) {            // right-looking Cholesky, lanes = rows; column k travels by shuffle
+        const float d = lf[k * 33 + k];
+        if (!(d > 1e-6f * 0.5f * (momS[2 * k] + m0))) ok = false;
+        const float lik = lane >= k ? own[k] * rsqrtf(d) : 0.f;
+        __syncwarp();
+        own[k] = lik;
+#pragma unroll 1
+        for (int j0 = k + 1; j0 < n1; j0 += 8) {
+            float v[8];
 #pragma unroll
-    for (int k = 0; k < 32; ++k) {
-        if (k < n1) {
-            const float d0 = 0.5f * (momS[2 * k] + m0);
-            const float d = __shfl_sync(FULL, row[k], k);
-            if (!(d > 1e-6f * d0)) ok = false;
-            const float lik = row[k] * rsqrtf(d);
-            row[k] = lik;
-            colbuf[lane] = lik;
-            __syncwarp();
+            for (int u = 0; u < 8; ++u) v[u] = own[min(j0 + u, 31)];
 #pragma unroll
-            for (int j = k + 1; j < 32; ++j) row[j] = fmaf(-lik, colbuf[j], row[j]);
-            __syncwarp();
+            for (int u = 0; u < 8; ++u) v[u] = fmaf(-lik, __shfl_sync(FULL, lik, (j0 + u) & 31), v[u]);
+#pragma unroll
+            for (int u = 0; u < 8; ++u)
+                if (j0 + u < n1) own[j0 + u] = v[u];
         }
+        __syncwarp();
     }
-#pragma unroll
-    for (int j = 0; j < 32; ++j) lf[lane * 33 + j] = row[j];
-    __syncwarp();
-    invd[lane] = 1.f / lf[lane * 33 + lane];
+    const float mine = 1.f / own[lane];
+    invd[lane] = mine;
     if (lane == 0) SMV(L.oSC, SC_N + seg, g) = ok ? 0.f : 1.f;
     __syncwarp();
-    // store the factor column-scaled to unit diagonal, Lt = L D^-1 (D = diag L): the two triangular
-    // solves of every step then have a shuffle + one FMA on their serial chain and no division;
-    // invd keeps 1/d^2 for the diagonal scaling between them:  A^-1 = Lt^-T D^-2 Lt^-1
+    // unit-diagonal factor Lt = L D^-1 (D = diag L) and 1/d^2:  A^-1 = Lt^-T D^-2 Lt^-1
+#pragma unroll 1
+    for (int j0 = 0; j0 < n1; j0 += 8) {
+        float v[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) v[u] = own[min(j0 + u, 31)] * invd[min(j0 + u, 31)];
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+            if (j0 + u < n1) own[j0 + u] = v[u];
+    }
+    __syncwarp();
+    invd[lane] = mine * mine;
+    __syncwarp();
+    // Explicit inverse X = A^-1 = Lt^-T D^-2 Lt^-1, V1_INVC columns at a time with lanes = rows (the same shuffle
+    // chains as a triangular solve, V1_INVC of them interleaved).  X is symmetric: column c is parked in the unused
+    // upper triangle of LF (rows < c) while the lower triangle still holds Lt, and mirrored at the end, so that
+    // the solve of EVERY step is a 32x32 matrix-vector product without a serial chain.
     {
-        const float mine = invd[lane];
-        float dj[32];
+        const float id2 = invd[lane];
+        float diag = 1.f;
+#pragma unroll 1
+        for (int c0 = 0; c0 < n1; c0 += V1_INVC) {
+            float r[V1_INVC];
 #pragma unroll
-        for (int j = 0; j < 32; ++j) dj[j] = invd[j];
+            for (int c = 0; c < V1_INVC; ++c) r[c] = (lane == c0 + c) ? 1.f : 0.f;
+            for (int k = c0; k < n1; ++k) {          // Lt z = e_c: z is zero above row c
+                const float lk = lf[lane * 33 + k];
+#pragma unroll
+                for (int c = 0; c < V1_INVC; ++c) {
+                    const float zk = __shfl_sync(FULL, r[c], k);
+                    if (lane > k) r[c] = fmaf(-lk, zk, r[c]);
+                }
+            }
+#pragma unroll
+            for (int c = 0; c < V1_INVC; ++c) r[c] *= id2;
+            for (int k = n1 - 1; k > 0; --k) {       // Lt^T x = D^-2 z
+                const float lk = lf[k * 33 + lane];
+#pragma unroll
+                for (int c = 0; c < V1_INVC; ++c) {
+                    const float xk = __shfl_sync(FULL, r[c], k);
+                    if (lane < k) r[c] = fmaf(-lk, xk, r[c]);
+                }
+            }
+            __syncwarp();
+#pragma unroll
+            for (int c = 0; c < V1_INVC; ++c) {
+                if (lane == c0 + c) diag = r[c];
+                if (lane < c0 + c && c0 + c < 32) lf[lane * 33 + c0 + c] = r[c];
+            }
+            __syncwarp();
+        }
+        own[lane] = diag;
+#pragma unroll 1
+        for (int j0 = 0; j0 < n1; j0 += 8) {     // mirror: row `lane` left of the diagonal
+            float v[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) v[u] = lf[min(j0 + u, 31) * 33 + lane];
+#pragma unroll
+            for (int u = 0; u < 8; ++u)
+                if (j0 + u < n1 && j0 + u < lane) own[j0 + u] = v[u];
+        }
         __syncwarp();
-#pragma unroll
-        for (int j = 0; j < 32; ++j) lf[lane * 33 + j] *= dj[j];
-        invd[lane] = mine * mine;
     }
 }
 
 __device__ __noinline__ void v1_phase_solve(int g, int seg, bool refactor)
 {
-    if (refactor) v1_refactor(g, seg);
+#ifdef LASP_PHASE_TIMING
+    unsigned long long *dbg_ = v1_blk.A.dbg;
+    long long tk_ = clock64();
+#define SOLVE_TICK(i) do { if (dbg_ && V1_TID == 0) { const long long t_ = clock64(); atomicAdd(dbg_ + (i), (unsigned long long)(t_ - tk_)); tk_ = t_; } } while (0)
+#define SOLVE_COUNT(i) do { if (dbg_ && V1_TID == 0) atomicAdd(dbg_ + (i), 1ull); } while (0)
+#else
+#define SOLVE_COUNT(i) do { } while (0)
+#define SOLVE_TICK(i) do { } while (0)
+#endif
+    if (refactor) { v1_refactor(g, seg); SOLVE_TICK(18); SOLVE_COUNT(21); }
     const ModelDev &M = v1_blk.M;
     const V1Lay &L = v1_blk.L;
     const int n1 = M.n1, lane = V1_LANE, rowB = seg * M.n1;
-    float *momS = V1SM + L.oMOM + g * L.nmomr;
-    float *rhsS = V1SM + L.oRHS + g * L.n1r;
-    float *lf = V1SM + L.oLF + g * V1_LFS;
-    float *invd = lf + 32 * 33;
-    const float *red = V1SM + L.oRED;
-    const int wst = L.VR * GS;
-    for (int n = lane; n < L.n1r; n += 32) {
-        float s = 0.f;
-        for (int w = 0; w < L.NW; ++w) s += red[w * wst + SLOT_RHS(L, n) * GS + g];
-        rhsS[n] = s;
-    }
-    __syncwarp();
+    const float *lf = V1SM + L.oLF + (seg * L.lfseg * GS + g) * V1_LFS;
+    const float *red = V1SM + L.oRED + SLOT_RHS(L, lane) * GS + g;
+    const int wst = L.VR * GS, NW = L.NW;
+    // one batch of loads: this lane's right-hand side over the warps' slots, its column of A^-1 (symmetric: row
+    // reads are conflict-free; the identity beyond n1), the flag and the coefficient it updates
+    float rp[12], xc[32];
+#pragma unroll
+    for (int w = 0; w < 12; ++w) rp[w] = (w < NW && lane < n1) ? red[w * wst] : 0.f;
+#pragma unroll
+    for (int j = 0; j < 32; ++j) xc[j] = lf[j * 33 + lane];
     const bool ok = SMV(L.oSC, SC_N + seg, g) == 0.f;
-    float r = (lane < n1) ? rhsS[lane] : 0.f;
-    for (int k = 0; k < n1; ++k) {            // Lt z = rhs (unit diagonal)
-        const float zk = __shfl_sync(FULL, r, k);
-        if (lane > k) r = fmaf(-lf[lane * 33 + k], zk, r);
+    const float b0 = SMV(L.oB, rowB + min(lane, n1 - 1), g);
+    float rv = 0.f;
+#pragma unroll
+    for (int w = 0; w < 12; ++w) rv += rp[w];
+    SOLVE_TICK(19);
+    // x = A^-1 rhs, row `lane`; rhs_j travels by shuffle (zero beyond n1)
+    float r0 = 0.f, r1 = 0.f, r2 = 0.f, r3 = 0.f;
+#pragma unroll
+    for (int j = 0; j < 32; j += 4) {
+        r0 = fmaf(xc[j], __shfl_sync(FULL, rv, j), r0);
+        r1 = fmaf(xc[j + 1], __shfl_sync(FULL, rv, j + 1), r1);
+        r2 = fmaf(xc[j + 2], __shfl_sync(FULL, rv, j + 2), r2);
+        r3 = fmaf(xc[j + 3], __shfl_sync(FULL, rv, j + 3), r3);
     }
-    r *= invd[lane];                          // D^-2
-    for (int k = n1 - 1; k >= 0; --k) {       // Lt^T x = D^-2 z
-        const float xk = __shfl_sync(FULL, r, k);
-        if (lane < k) r = fmaf(-lf[k * 33 + lane], xk, r);
-    }
-    if (lane < n1) {
-        if (ok) SMV(L.oB, rowB + lane, g) += r;
-        else SMV(L.oB, rowB + lane, g) = 0.f;
-    }
+    const float r = (r0 + r1) + (r2 + r3);
+    if (lane < n1) SMV(L.oB, rowB + lane, g) = ok ? b0 + r : 0.f;
     __syncwarp();
+    SOLVE_TICK(20);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -1021,7 +1140,7 @@ __device__ __noinline__ void v1_phase_adjoint(const SegDev &sg, int lo, int hi)
 // for MODE 0, the q / dv / dsigma partials.
 // ------------------------------------------------------------------------------------------
 template <int MODE>
-__device__ __noinline__ void v1_evaluate(bool cold, bool mom, float *xrow)
+__device__ __noinline__ void v1_evaluate(bool cold, bool mom, float *xrow, bool wready = false)
 {
     const V1Args &a = v1_blk.A;
     const ModelDev &M = v1_blk.M;
@@ -1037,6 +1156,7 @@ __device__ __noinline__ void v1_evaluate(bool cold, bool mom, float *xrow)
 #else
     auto tick = [](int) {};   // per-phase cycle counters: build with -DLASP_PHASE_TIMING
 #endif
+    if (M.n_seg > 1 && !L.lfseg) mom = true;   // one factor slot shared by the segments: never stale
     bool zeroed = false;
     auto zero_slots = [&]() {
         float *red = V1SM + L.oRED + V1_WARP * L.VR * GS;
@@ -1058,7 +1178,7 @@ __device__ __noinline__ void v1_evaluate(bool cold, bool mom, float *xrow)
             continue;
         }
         if (V1_WARP < GS) {
-            v1_setup_weights(sg, V1_WARP);
+            if (!wready) v1_setup_weights(sg, V1_WARP);   // else v1_update_fast has left them in place
             if (cold) for (int n = V1_LANE; n < M.n1; n += 32) SMV(L.oB, rowB + n, V1_WARP) = 0.f;
         }
         if (M.n_seg > 1 || cold) {
@@ -1134,19 +1254,29 @@ __device__ __noinline__ float v1_gradient(int g)
     const V1Lay &L = v1_blk.L;
     const float *red = V1SM + L.oRED;
     const int wst = L.VR * GS, nl = M.L, K = M.K, NW = L.NW, q0 = SLOT_Q(L, 0);
-    for (int k = V1_LANE; k < K + 2; k += 32) {
-        float s = 0.f;
-        for (int w = 0; w < NW; ++w) s += red[w * wst + (q0 + k) * GS + g];
-        SMV(L.oQ, k, g) = s;
+    float mine = 0.f;
+    for (int l0 = 0; l0 < max(nl, 1); l0 += 4) {      // d chi2 / d x_l = sum_k (d phi_k / d x_l) q_k, four labels per butterfly
+        float gx[4] = {0.f, 0.f, 0.f, 0.f};
+        for (int k = V1_LANE; k < K + 2; k += 32) {
+            float qk = 0.f;
+            for (int w = 0; w < NW; ++w) qk += red[w * wst + (q0 + k) * GS + g];
+            if (k >= K) { if (l0 == 0) SMV(L.oQ, k, g) = qk; }
+            else {
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    if (l0 + u < nl) gx[u] = fmaf(SMV(L.oDPHI, (l0 + u) * K + k, g), qk, gx[u]);
+            }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+            for (int u = 0; u < 4; ++u) gx[u] += __shfl_xor_sync(FULL, gx[u], o);
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            if (V1_LANE == l0 + u) mine = gx[u];
     }
     __syncwarp();
-    float mine = 0.f;
-    for (int l = 0; l < nl; ++l) {      // d chi2 / d x_l = sum_k (d phi_k / d x_l) q_k
-        float gx = 0.f;
-        for (int k = V1_LANE; k < K; k += 32) gx = fmaf(SMV(L.oDPHI, l * K + k, g), SMV(L.oQ, k, g), gx);
-        gx = warp_sum_f(gx);
-        if (V1_LANE == l) mine = gx;
-    }
     if (V1_LANE == nl || V1_LANE == nl + 1) {     // + the part closed in the residual phase (per-pixel kernels)
         const int which = V1_LANE - nl;
         float sx = SMV(L.oQ, K + which, g);
@@ -1155,6 +1285,119 @@ __device__ __noinline__ float v1_gradient(int g)
     }
     if (V1_LANE < M.NP) mine *= SMV(L.oGSC, V1_LANE, g);   // chain rule to u (C.1 last lines)
     return mine;
+}
+
+// ------------------------------------------------------------------------------------------
+// a7 (tail) + a8 + a1 of the next step in one pass, for models with at most four labels and K + 2 <= 32
+// (L.fastupd): lane k owns term k, lane p owns parameter p.  These phases are one warp's latency and every
+// dependent shared-memory round trip costs it ~100 cycles while the other CTA's stencil keeps the LSU busy: all
+// loads are issued together at the top, the labels travel by shuffle and x^e is formed in registers, so the chain
+// is one load batch, one butterfly and one broadcast instead of ~40 round trips.  Same arithmetic, in the same
+// order, as v1_gradient + the Adam lines of the fit loop + v1_param_setup.
+// ------------------------------------------------------------------------------------------
+__device__ __noinline__ void v1_update_fast(int g, float ib1, float ib2)
+{
+    const V1Args &a = v1_blk.A;
+    const ModelDev &M = v1_blk.M;
+    const V1Lay &L = v1_blk.L;
+    const int lane = V1_LANE;
+#ifdef LASP_PHASE_TIMING
+    long long tk_ = clock64();
+#define UPD_TICK(i) do { if (a.dbg && V1_TID == 0) { const long long t_ = clock64(); atomicAdd(a.dbg + (i), (unsigned long long)(t_ - tk_)); tk_ = t_; } } while (0)
+#else
+#define UPD_TICK(i) do { } while (0)
+#endif
+    const int wst = L.VR * GS, nl = M.L, K = M.K, NW = L.NW, NP = M.NP, emax = L.emax;
+    const float *redq = V1SM + L.oRED + (SLOT_Q(L, 0) + min(lane, K + 1)) * GS + g;
+    const int which = min(max(lane - nl, 0), 1);
+    const float *reds = V1SM + L.oRED + (SLOT_STAT(L) + 3 + which) * GS + g;
+    const int pl = min(lane, NP - 1), kl = min(lane, K - 1), ll = min(lane, max(nl - 1, 0));
+    // ---- one batch of loads
+    float qp[12], sp[12];
+#pragma unroll
+    for (int w = 0; w < 12; ++w) {
+        qp[w] = w < NW ? redq[w * wst] : 0.f;
+        sp[w] = w < NW ? reds[w * wst] : 0.f;
+    }
+    float dphi[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) dphi[u] = u < nl ? SMV(L.oDPHI, u * K + kl, g) : 0.f;
+    const float gsc = SMV(L.oGSC, pl, g), m0 = SMV(L.oM, pl, g), v0 = SMV(L.oV, pl, g), u0 = SMV(L.oU, pl, g);
+    const unsigned exw = ((const unsigned *)(V1SM + L.oEXP))[kl];
+    const float lo = M.lo[pl], hi = M.hi[pl], ea = M.emu_a[ll], eb = M.emu_b[ll];
+    const bool lg = M.label_log10[ll] != 0;
+    const float b1 = a.b1, b2 = a.b2, lr = a.lr, eps = a.eps;
+    // ---- gradient (a7 tail): q_k, then d chi2 / d x_l = sum_k (d phi_k / d x_l) q_k
+    float qk = 0.f, sx = 0.f;
+#pragma unroll
+    for (int w = 0; w < 12; ++w) { qk += qp[w]; sx += sp[w]; }
+    UPD_TICK(16);
+    float gx[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) gx[u] = lane < K ? dphi[u] * qk : 0.f;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) gx[u] += __shfl_xor_sync(FULL, gx[u], o);
+    }
+    const float qvs = __shfl_sync(FULL, qk, K + which);   // the v / sigma* sums live on lanes K, K+1
+    float gr = lane < nl ? (lane == 0 ? gx[0] : lane == 1 ? gx[1] : lane == 2 ? gx[2] : gx[3]) : qvs + sx;
+    gr *= gsc;                                              // chain rule to u (C.1 last lines)
+    UPD_TICK(17);
+    // ---- a8: Adam (C.2-20), clip to the prior box (C.2-18)
+    const float mm = b1 * m0 + (1.f - b1) * gr;
+    const float vv = b2 * v0 + (1.f - b2) * gr * gr;
+    const float mh = mm * ib1, vh = vv * ib2;
+    float u = u0 - __fdividef(lr * mh, sqrtf(vh) + eps);
+    if (!(u == u)) u = u0;                                  // keep the iterate if the gradient was NaN
+    u = fminf(fmaxf(u, -1.f), 1.f);
+    // ---- a1: de-normalise, emulator inputs (C.2-18/19)
+    const float half = (hi - lo) * 0.5f;
+    const float th = lo + (u + 1.f) * half;
+    float xv = 0.f, gscn = half;
+    if (lane < nl) {
+        xv = ea * (lg ? log10f(th) : th) + eb;
+        gscn *= lg ? ea / (th * 2.302585093f) : ea;
+    }
+    if (lane < NP) {
+        SMV(L.oM, lane, g) = mm; SMV(L.oV, lane, g) = vv; SMV(L.oU, lane, g) = u;
+        SMV(L.oGSC, lane, g) = gscn;
+        if (lane < nl) SMV(L.oX, lane, g) = xv;
+        else SMV(L.oSC, lane == nl ? SC_V : SC_SIG, g) = th;
+    }
+    UPD_TICK(22);
+    // ---- monomials (Eq. 1): x^e and e x^(e-1) by repeated multiplication, as the power table does
+    float pe[4], pm[4];
+#pragma unroll
+    for (int l = 0; l < 4; ++l) {
+        const float x = __shfl_sync(FULL, xv, l);
+        const int e = (exw >> (8 * l)) & 255;
+        float pw = 1.f, pwm = 0.f;
+        for (int q = 0; q < emax; ++q)
+            if (q < e) { pwm = pw; pw *= x; }
+        pe[l] = l < nl ? pw : 1.f;
+        pm[l] = l < nl ? (float)e * pwm : 0.f;
+    }
+    if (lane < K) {
+        float ph = 1.f;
+#pragma unroll
+        for (int l = 0; l < 4; ++l) ph *= pe[l];
+        SMV(L.oPHI, lane, g) = ph;
+#pragma unroll
+        for (int l = 0; l < 4; ++l) {
+            float d = pm[l];
+#pragma unroll
+            for (int l2 = 0; l2 < 4; ++l2)
+                if (l2 != l) d *= pe[l2];
+            if (l < nl) SMV(L.oDPHI, l * K + lane, g) = d;
+        }
+    }
+    UPD_TICK(23);
+    if (L.fastw) {   // a3 of the next step (single uniform segment): v and sigma* are on lanes nl, nl+1
+        const float vn = __shfl_sync(FULL, th, nl), sn = __shfl_sync(FULL, th, nl + 1);
+        v1_weights_uniform(M.seg[0], g, vn, sn);
+    }
+    __syncwarp();
 }
 
 // internal Chebyshev(t) coefficients -> plain Legendre(x^) (C.2-8), fp64.  Warp g, lanes over rows.
@@ -1182,7 +1425,14 @@ __device__ __forceinline__ void v1_init_block(const ModelDev &M, const V1Lay &L,
         v1_blk.cp = a.CP + (size_t)blockIdx.x * GS * M.Ppad;
         v1_blk.ds = a.DS ? a.DS + (size_t)blockIdx.x * 3 * GS * M.Ppad : nullptr;
     }
-    for (int i = threadIdx.x; i < M.K * M.L; i += blockDim.x) ((uint8_t *)(V1SM + L.oEXP))[i] = M.exps[i];
+    if (M.L <= 4) {   // one word per term (v1_param_setup)
+        for (int k = threadIdx.x; k < M.K; k += blockDim.x) {
+            unsigned w = 0;
+            for (int l = 0; l < M.L; ++l) w |= (unsigned)M.exps[k * M.L + l] << (8 * l);
+            ((unsigned *)(V1SM + L.oEXP))[k] = w;
+        }
+    } else
+        for (int i = threadIdx.x; i < M.K * M.L; i += blockDim.x) ((uint8_t *)(V1SM + L.oEXP))[i] = M.exps[i];
     for (int i = threadIdx.x; i < GS * L.Kq; i += blockDim.x) V1SM[L.oPHI + i] = 0.f;   // phi is zero past K
     // rows T and A: zero-weight taps multiply whatever lies in the window, so it must at least be finite
     for (int i = threadIdx.x; i < 2 * GS * L.RL; i += blockDim.x) V1SM[L.oT + i] = 0.f;
@@ -1353,35 +1603,39 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
             const long long te0 = a.dbg ? clock64() : 0;
 #endif
             // fresh Gram factor on each of the first `refresh` steps (the model moves fastest there), then every `refresh`-th
-            v1_evaluate<0>(t == 1, t <= L.refresh || (t - 1) % L.refresh == 0, nullptr);
+            v1_evaluate<0>(t == 1, t <= L.warm || (t - 1) % L.refresh == 0, nullptr, t > 1 && L.fastw);
 #ifdef LASP_PHASE_TIMING
             if (a.dbg && V1_TID == 0) { atomicAdd(a.dbg + 14, (unsigned long long)(clock64() - te0)); atomicAdd(a.dbg + 15, 1ull); }
             const long long tu0 = a.dbg ? clock64() : 0;
 #endif
             pb1 *= a.b1; pb2 *= a.b2;
             if (g < GS) {
-                const float gr = v1_gradient(g);
+                const float ib1 = 1.f / (1.f - pb1), ib2 = 1.f / (1.f - pb2);   // bias corrections (C.2-20)
+                if (L.fastupd) v1_update_fast(g, ib1, ib2);
+                else {
+                    const float gr = v1_gradient(g);
 #ifdef LASP_PHASE_TIMING
-                if (a.dbg && V1_TID == 0) atomicAdd(a.dbg + 16, (unsigned long long)(clock64() - tu0));
+                    if (a.dbg && V1_TID == 0) atomicAdd(a.dbg + 16, (unsigned long long)(clock64() - tu0));
 #endif
-                // a8: Adam (C.2-20), then clip to the prior box (C.2-18); lane p owns parameter p
-                for (int p0 = 0; p0 < NP; p0 += 32) {   // NP <= 32
-                    const int p = p0 + V1_LANE;
-                    if (p < NP) {
-                        const float m = a.b1 * SMV(L.oM, p, g) + (1.f - a.b1) * gr;
-                        const float v = a.b2 * SMV(L.oV, p, g) + (1.f - a.b2) * gr * gr;
-                        SMV(L.oM, p, g) = m; SMV(L.oV, p, g) = v;
-                        const float mh = m / (1.f - pb1), vh = v / (1.f - pb2);
-                        float u = SMV(L.oU, p, g) - a.lr * mh / (sqrtf(vh) + a.eps);
-                        if (!(u == u)) u = SMV(L.oU, p, g);   // keep the iterate if the gradient was NaN
-                        SMV(L.oU, p, g) = fminf(fmaxf(u, -1.f), 1.f);
+                    // a8: Adam (C.2-20), then clip to the prior box (C.2-18); lane p owns parameter p
+                    for (int p0 = 0; p0 < NP; p0 += 32) {   // NP <= 32
+                        const int p = p0 + V1_LANE;
+                        if (p < NP) {
+                            const float m = a.b1 * SMV(L.oM, p, g) + (1.f - a.b1) * gr;
+                            const float v = a.b2 * SMV(L.oV, p, g) + (1.f - a.b2) * gr * gr;
+                            SMV(L.oM, p, g) = m; SMV(L.oV, p, g) = v;
+                            const float mh = m * ib1, vh = v * ib2;
+                            float u = SMV(L.oU, p, g) - __fdividef(a.lr * mh, sqrtf(vh) + a.eps);
+                            if (!(u == u)) u = SMV(L.oU, p, g);   // keep the iterate if the gradient was NaN
+                            SMV(L.oU, p, g) = fminf(fmaxf(u, -1.f), 1.f);
+                        }
                     }
-                }
-                __syncwarp();
+                    __syncwarp();
 #ifdef LASP_PHASE_TIMING
-                if (a.dbg && V1_TID == 0) atomicAdd(a.dbg + 17, (unsigned long long)(clock64() - tu0));
+                    if (a.dbg && V1_TID == 0) atomicAdd(a.dbg + 17, (unsigned long long)(clock64() - tu0));
 #endif
-                v1_param_setup(g);
+                    v1_param_setup(g);
+                }
             }
 #ifdef LASP_PHASE_TIMING
             if (a.dbg && V1_TID == 0) atomicAdd(a.dbg + 13, (unsigned long long)(clock64() - tu0));

@@ -370,7 +370,13 @@ static int setup_v1(lasp_ctx *c, const cudaDeviceProp &prop, int emax)
     L.nmomr = L.n1r + roundup(std::max(M.nmom - L.n1r, 0), 8);
     L.VR = L.nmomr + L.n1r + roundup(M.K + 2, 8) + 6;
     const char *rf = getenv("LASP_REFRESH");
-    L.refresh = rf ? std::max(1, atoi(rf)) : 16;
+    L.refresh = rf ? std::max(1, atoi(rf)) : 64;
+    const char *rw = getenv("LASP_REFRESH_WARM");
+    L.warm = rw ? std::max(1, atoi(rw)) : std::min(L.refresh, 4);
+    L.fastupd = (M.L >= 1 && M.L <= 4 && M.K + 2 <= 32 && L.NW <= 12 && !getenv("LASP_NO_FASTUPD")) ? 1 : 0;
+    L.fastw = (L.fastupd && M.n_seg == 1 && M.seg[0].uniform && M.seg[0].fit_hi > M.seg[0].fit_lo) ? 1 : 0;
+    size_t bytes = 0;
+    for (L.lfseg = 1; L.lfseg >= 0; --L.lfseg) {   // a factor slot per segment if shared memory allows it
     int o = 0;
     auto take = [&](int n) { int r = o; o += roundup(n, 4); return r; };
     L.oT = take(GS * L.RL); L.oA = take(GS * L.RL);
@@ -381,15 +387,17 @@ static int setup_v1(lasp_ctx *c, const cudaDeviceProp &prop, int emax)
     L.oMOM = take(GS * L.nmomr); L.oRHS = take(GS * L.n1r); L.oB = take(GS * M.nc);
     L.oRED = take(L.NW * L.VR * GS);
     const int npair = M.NP * (M.NP + 1) / 2;
-    L.oLF = take(std::max(GS * V1_LFS, 2 * GS * npair + 4));
+    L.oLF = take(std::max(GS * V1_LFS * (L.lfseg ? M.n_seg : 1), 2 * GS * npair + 4));
     L.oQ = take(GS * (M.K + 2)); L.oSC = take(GS * (SC_N + M.n_seg));
-    L.oEXP = take((M.K * M.L + 3) / 4);
+    L.oEXP = take(std::max((M.K * M.L + 3) / 4, M.K));   // bytes [K][L], or one packed word per term when L <= 4
     L.oXP = take(GS * M.L * (L.emax + 1)); L.oDPHI = take(GS * M.L * M.K); L.oGSC = take(GS * M.NP);
     L.oNP = take(GS * 8);
     L.oEW = take(GS * (2 * hmax + 2));
     L.total = o;
-    const size_t bytes = (size_t)o * sizeof(float);
-    if (bytes > prop.sharedMemPerBlockOptin) return LASP_OK;   // does not fit: v0 handles it
+    bytes = (size_t)o * sizeof(float);
+    if (bytes <= prop.sharedMemPerBlockOptin) break;
+    }
+    if (L.lfseg < 0) return LASP_OK;   // does not fit: v0 handles it
     bool ok = true;
     v1_for_kernels([&](const void *f, int) {
         if (cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess) ok = false;
