@@ -36,6 +36,7 @@ struct V1Lay {
     int n1r, nmomr, VR;     // n1 rounded to 4; moments rounded; reduction slots per warp (x GS)
     int NW;                 // warps per CTA
     int Hm;                 // support clamp (memory safety outside the prior box)
+    int fdfresh;            // 1: re-factor in every finite-difference evaluation of the error estimate (LASP_FD_FRESH)
     int fastw;              // 1: v1_update_fast also prepares the next step's kernel weights (one uniform segment)
     int fastupd;            // 1: v1_update_fast applies (L <= 4, K + 2 <= 32, NW <= 12)
     int lfseg;              // 1: one factor slot per segment (0: one slot, re-factored every step when n_seg > 1)
@@ -1466,13 +1467,16 @@ __device__ __noinline__ void v1_errors(float chi2_g, float ngood_g, bool valid_g
             __syncwarp();
             v1_param_setup(V1_WARP);
         }
-        v1_evaluate<2>(false, true, xj);
+        // The factor of the final evaluation serves all 2 NP perturbed ones: a step of fd_h changes the Gram matrix
+        // by a relative ~1e-3, so one refinement from the neighbouring solution leaves that fraction of the
+        // continuum's response, far inside the 1e-2 the estimate is held to.
+        v1_evaluate<2>(false, L.fdfresh != 0, xj);
         if (V1_WARP < GS) {
             if (V1_LANE == 0) SMV(L.oU, p, V1_WARP) = u0 - a.fd_h;
             __syncwarp();
             v1_param_setup(V1_WARP);
         }
-        v1_evaluate<2>(false, true, xj + (1 + p) * plane);
+        v1_evaluate<2>(false, L.fdfresh != 0, xj + (1 + p) * plane);
         if (V1_WARP < GS) {
             if (V1_LANE == 0) SMV(L.oU, p, V1_WARP) = u0;
             __syncwarp();

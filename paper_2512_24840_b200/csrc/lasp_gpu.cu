@@ -374,6 +374,7 @@ static int setup_v1(lasp_ctx *c, const cudaDeviceProp &prop, int emax)
     const char *rw = getenv("LASP_REFRESH_WARM");
     L.warm = rw ? std::max(1, atoi(rw)) : std::min(L.refresh, 4);
     L.fastupd = (M.L >= 1 && M.L <= 4 && M.K + 2 <= 32 && L.NW <= 12 && !getenv("LASP_NO_FASTUPD")) ? 1 : 0;
+    L.fdfresh = getenv("LASP_FD_FRESH") ? 1 : 0;
     L.fastw = (L.fastupd && M.n_seg == 1 && M.seg[0].uniform && M.seg[0].fit_hi > M.seg[0].fit_lo) ? 1 : 0;
     size_t bytes = 0;
     for (L.lfseg = 1; L.lfseg >= 0; --L.lfseg) {   // a factor slot per segment if shared memory allows it
