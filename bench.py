@@ -241,7 +241,7 @@ def run_gpu(args):
     model.reserve(B)
     data = make_device_batch(model, cfg, desc, B, cfg.seed + 17 + rank, torch)
     out = None
-    kw = dict(lr=cfg.lr, beta1=cfg.beta1, beta2=cfg.beta2, eps=cfg.eps)
+    kw = dict(lr=cfg.lr, beta1=cfg.beta1, beta2=cfg.beta2, eps=cfg.eps, emulator_path=args.emulator_path)
 
     def barrier():
         torch.cuda.synchronize()
@@ -330,7 +330,7 @@ def run_gpu(args):
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"config {args.config} ({cfg.name})", "spectra_per_gpu": B,
                    "n_pix": model.P, "n_terms": model.K, "n_labels": model.L, "cont_degree": model.D,
-                   "n_seg": model.n_seg, "adam_steps": n_iter, "lr": cfg.lr, "errors": True,
+                   "n_seg": model.n_seg, "adam_steps": n_iter, "lr": cfg.lr, "errors": True, "emulator_path": args.emulator_path,
                    "l2": "inputs larger than L2 (flux+ivar+mask %.0f MB per step)" % (h2d / 1e6),
                    "status_nonzero_frac": float((st != 0).mean())},
         "clocks": clocks, "gpu_launches": int(launches),
@@ -363,6 +363,8 @@ def main():
     ap.add_argument("--n-iter", type=int, default=0, help="Adam steps (default: the config's)")
     ap.add_argument("--ref-spectra", type=int, default=0, help="oracle sample size")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--emulator-path", type=int, default=0, choices=[0, 1, 2],
+                    help="lasp_fit_opts.emulator_path: 0 auto, 1 FP32 FMA, 2 tensor pipe (mma.sync TF32, split operands)")
     args = ap.parse_args()
     args.config = int(args.config) if args.config.isdigit() else args.config
     if args.impl == "reference":

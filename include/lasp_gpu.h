@@ -84,7 +84,10 @@ typedef struct {
     int32_t n_iter;               /* fixed number of Adam steps (Delta-6) */
     float lr, beta1, beta2, eps;  /* Adam hyper-parameters (defaults 1e-2, 0.9, 0.999, 1e-8) */
     int32_t variant;              /* 0 auto; reserved (1 resident, 2 streaming) */
-    int32_t emulator_path;        /* 0 auto; reserved (1 fp32 fma, 2 3xTF32) */
+    int32_t emulator_path;        /* emulator contraction T = phi.C (Eq. 1): 0 auto (= 1: measured faster),
+                                     1 FP32 FMA, 2 tensor pipe: mma.sync TF32 with both operands split x = hi + lo
+                                     (3xTF32-class accuracy); 2 needs the resident kernel and n_terms <= 32, else
+                                     LASP_ERR_UNSUPPORTED; other values LASP_ERR_INVALID_ARG */
 } lasp_fit_opts;
 
 /* Build a context on `cuda_device`: validates the description, derives the per-pixel velocity

@@ -161,7 +161,7 @@ class LaspModel:
         return float(lib().lasp_fma_per_spectrum_step(self.ctx, mean_taps))
 
     def fit_batch(self, flux, ivar, mask, init, n_iter, lr=1e-2, beta1=0.9, beta2=0.999, eps=1e-8,
-                  want_err=True, want_cont=True, out=None):
+                  want_err=True, want_cont=True, out=None, emulator_path=0):
         """lasp_fit_batch on device tensors; returns dict of device tensors."""
         t = self.torch
         flux = self._dev(flux, t.float32); ivar = self._dev(ivar, t.float32)
@@ -174,7 +174,7 @@ class LaspModel:
                        status=t.empty(B, device=self.device, dtype=t.int32),
                        cont=t.empty((B, self.nc), device=self.device, dtype=t.float32) if want_cont else None,
                        err=t.empty((B, self.NP), device=self.device, dtype=t.float32) if want_err else None)
-        opts = FitOpts(int(n_iter), lr, beta1, beta2, eps, 0, 0)
+        opts = FitOpts(int(n_iter), lr, beta1, beta2, eps, 0, int(emulator_path))
         rc = lib().lasp_fit_batch(self.ctx, B, _ptr(flux), _ptr(ivar), _ptr(mask), _ptr(init), C.byref(opts),
                                   _ptr(out["params"]), _ptr(out.get("cont")), _ptr(out["chi2"]),
                                   _ptr(out.get("err")), _ptr(out["status"]), self._stream())
@@ -182,7 +182,7 @@ class LaspModel:
         return out
 
     def fit_batch_host(self, flux, ivar, mask, init, n_iter, lr=1e-2, beta1=0.9, beta2=0.999, eps=1e-8,
-                       want_err=True, want_cont=True, chunk=0, out=None):
+                       want_err=True, want_cont=True, chunk=0, out=None, emulator_path=0):
         """lasp_fit_batch_host on HOST tensors (torch CPU tensors, pinned for overlap); returns host tensors.
         The library cuts the batch into chunks and overlaps the copies with the fits."""
         t = self.torch
@@ -205,7 +205,7 @@ class LaspModel:
                        status=t.empty(B, dtype=t.int32, **pin),
                        cont=t.empty((B, self.nc), dtype=t.float32, **pin) if want_cont else None,
                        err=t.empty((B, self.NP), dtype=t.float32, **pin) if want_err else None)
-        opts = FitOpts(int(n_iter), lr, beta1, beta2, eps, 0, 0)
+        opts = FitOpts(int(n_iter), lr, beta1, beta2, eps, 0, int(emulator_path))
         rc = lib().lasp_fit_batch_host(self.ctx, B, _ptr(flux), _ptr(ivar), _ptr(mask), _ptr(init), C.byref(opts),
                                        _ptr(out["params"]), _ptr(out.get("cont")), _ptr(out["chi2"]),
                                        _ptr(out.get("err")), _ptr(out["status"]), int(chunk))

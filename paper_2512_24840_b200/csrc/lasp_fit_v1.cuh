@@ -67,6 +67,8 @@ struct V1Args {
     const float *IS, *S2;
     float *DS;
     unsigned int *queue;   // work-queue counter for the fit kernel (zeroed before the launch), may be null
+    const float4 *CF;      // coefficient table as tf32 [hi|lo] MMA fragments (null: FP32-pipe emulator)
+    int ksteps;            // k-steps of 8 terms in CF (<= 4)
 };
 #define V1_TPAD 256
 
@@ -528,6 +530,91 @@ __device__ __noinline__ void v1_phase_emulator(const SegDev &sg, int lo, int hi)
             const int q = j0 >> 2;
             r[SW4(q)] = make_float4(acc[g][0], acc[g][1], acc[g][2], acc[g][3]);
             r[SW4(q + 1)] = make_float4(acc[g][4], acc[g][5], acc[g][6], acc[g][7]);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// a2 on the tensor pipe: the same contraction as mma.sync.m16n8k8 TF32 with both operands split in two
+// (x = hi + lo, each a tf32 number): rows = 16 pixels, k = 8 terms, and the 8 columns carry [phi_hi | phi_lo] of the
+// GS = 4 spectra, so that two MMAs (table hi, table lo) form all four partial products in FP32 accumulators.
+// Warp w owns pixels [lo + 256 w, lo + 256 w + 256) of every sweep; the table comes pre-split in fragment order
+// (lasp_gpu.cu), one LDG.128 per (octet, k-step).
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ float v1_tf32(float x)
+{
+    unsigned r;
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
+    return __uint_as_float(r);
+}
+
+__device__ __forceinline__ void v1_mma_tf32(float (&d)[4], float a0, float a1, float a2, float a3, float b0, float b1)
+{
+    asm("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+                 : "r"(__float_as_uint(a0)), "r"(__float_as_uint(a1)), "r"(__float_as_uint(a2)), "r"(__float_as_uint(a3)),
+                   "r"(__float_as_uint(b0)), "r"(__float_as_uint(b1)));
+}
+
+__device__ __noinline__ void v1_phase_emulator_mma(const SegDev &sg, int lo, int hi)
+{
+    const int lane = V1_LANE, gid = lane >> 2, tig = lane & 3, K = v1_blk.M.K, ks = v1_blk.A.ksteps;
+    const int RL = v1_blk.L.RL, sweep = v1_blk.L.NW * 256;
+    const float4 *CF = v1_blk.A.CF + lane;
+    float *rowT = V1SM + v1_blk.L.oT + v1_blk.L.GUARD - sg.po;
+    const float *phi = V1SM + v1_blk.L.oPHI + (gid & 3);
+    // B fragments (k = term, n = column): columns 0..3 carry phi_hi of spectrum n, columns 4..7 phi_lo of spectrum n - 4
+    float b0[4], b1[4];
+#pragma unroll
+    for (int s = 0; s < 4; ++s) {
+        const int k0 = 8 * s + tig, k1 = k0 + 4;
+        const float p0 = k0 < K ? phi[k0 * GS] : 0.f, p1 = k1 < K ? phi[k1 * GS] : 0.f;
+        const float h0 = v1_tf32(p0), h1 = v1_tf32(p1);
+        b0[s] = gid < 4 ? h0 : v1_tf32(p0 - h0);
+        b1[s] = gid < 4 ? h1 : v1_tf32(p1 - h1);
+    }
+    const int g0 = 2 * (tig & 1), half = tig >> 1;    // after the hi/lo fold: this lane stores spectra g0, g0+1 of octet o + half
+    for (int base = lo + V1_WARP * 256; base < hi; base += sweep) {
+        // two 16-pixel tiles per trip: their 4 ks LDG.128 are all in flight before the first MMA, and the four
+        // accumulation chains (tile x table hi/lo) are independent
+#pragma unroll 1
+        for (int mt = 0; mt < 16; mt += 2) {
+            const int jA = base + mt * 16;
+            if (jA >= hi) break;                           // warp-uniform
+            const int jB = jA + 16 < hi ? jA + 16 : jA;    // odd tail: the second tile repeats the first (not stored)
+            const float4 *fA = CF + (size_t)(jA >> 3) * ks * 32, *fB = CF + (size_t)(jB >> 3) * ks * 32;
+            float4 A0[4], A1[4], B0[4], B1[4];
+#pragma unroll
+            for (int s = 0; s < 4; ++s) {
+                const int sc = s < ks ? s : 0;             // k-steps past ks re-read step 0 (their B fragments are zero)
+                A0[s] = __ldg(fA + sc * 32); A1[s] = __ldg(fA + (ks + sc) * 32);
+                B0[s] = __ldg(fB + sc * 32); B1[s] = __ldg(fB + (ks + sc) * 32);
+            }
+            float ah[4] = {0.f, 0.f, 0.f, 0.f}, al[4] = {0.f, 0.f, 0.f, 0.f}, bh[4] = {0.f, 0.f, 0.f, 0.f}, bl[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+            for (int s = 0; s < 4; ++s) {
+                v1_mma_tf32(ah, A0[s].x, A1[s].x, A0[s].y, A1[s].y, b0[s], b1[s]);   // table hi
+                v1_mma_tf32(bh, B0[s].x, B1[s].x, B0[s].y, B1[s].y, b0[s], b1[s]);
+                v1_mma_tf32(al, A0[s].z, A1[s].z, A0[s].w, A1[s].w, b0[s], b1[s]);   // table lo
+                v1_mma_tf32(bl, B0[s].z, B1[s].z, B0[s].w, B1[s].w, b0[s], b1[s]);
+            }
+            // D[pixel][n]: lane holds n = 2 tig, 2 tig + 1 for pixels gid (d0, d1) and gid + 8 (d2, d3); T_g = D[g] + D[g+4]
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                ah[i] += al[i]; bh[i] += bl[i];
+                ah[i] += __shfl_xor_sync(FULL, ah[i], 2); bh[i] += __shfl_xor_sync(FULL, bh[i], 2);
+            }
+            const int jpA = jA + half * 8 + gid, jpB = jB + half * 8 + gid;
+            if (jpA < hi) {
+                float *e0 = (float *)((float4 *)(rowT + g0 * RL) + SW4(jpA >> 2)) + (jpA & 3);
+                float *e1 = (float *)((float4 *)(rowT + (g0 + 1) * RL) + SW4(jpA >> 2)) + (jpA & 3);
+                *e0 = half ? ah[2] : ah[0]; *e1 = half ? ah[3] : ah[1];
+            }
+            if (jB != jA && jpB < hi) {
+                float *e0 = (float *)((float4 *)(rowT + g0 * RL) + SW4(jpB >> 2)) + (jpB & 3);
+                float *e1 = (float *)((float4 *)(rowT + (g0 + 1) * RL) + SW4(jpB >> 2)) + (jpB & 3);
+                *e0 = half ? bh[2] : bh[0]; *e1 = half ? bh[3] : bh[1];
+            }
         }
     }
 }
@@ -1196,7 +1283,7 @@ __device__ __noinline__ void v1_evaluate(bool cold, bool mom, float *xrow, bool 
         if (!zeroed) zero_slots();
         int lo, hi;
         v1_group_range(sg, lo, hi);
-        v1_phase_emulator(sg, lo, hi);
+        if (v1_blk.A.CF) v1_phase_emulator_mma(sg, lo, hi); else v1_phase_emulator(sg, lo, hi);
         tick(2);
         __syncthreads();
         tick(3);

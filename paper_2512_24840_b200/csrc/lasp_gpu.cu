@@ -36,6 +36,8 @@ struct lasp_ctx {
     V1Lay V1;
     int v1_nt = 0, v1_maxt = 0, v1_cta_per_sm = 1;
     float *dY = nullptr, *dW = nullptr, *dC1 = nullptr;
+    float4 *dCF = nullptr;   // v1: coefficient table as tf32 [hi|lo] MMA fragments (emulator on the tensor pipe)
+    int cf_ksteps = 0;
     size_t plane_rows = 0;
     float *dCP = nullptr, *dXJ = nullptr;
     // the workspace (staged planes, scratch) is shared by every call on this ctx: each call waits, on ITS stream, for
@@ -130,7 +132,7 @@ extern "C" int lasp_destroy(lasp_ctx *c)
     cudaSetDevice(c->device);
     cudaFree(c->dC); cudaFree(c->dinv_s); cudaFree(c->dexps); cudaFree(c->dconv); cudaFree(c->dnedge);
     cudaFree(c->dYW); cudaFree(c->dscratch);
-    cudaFree(c->dC1); cudaFree(c->dIS); cudaFree(c->dS2); cudaFree(c->dDS); cudaFree(c->dY); cudaFree(c->dW); cudaFree(c->dCP); cudaFree(c->dXJ); cudaFree(c->ddbg); cudaFree(c->dqueue);
+    cudaFree(c->dC1); cudaFree(c->dCF); cudaFree(c->dIS); cudaFree(c->dS2); cudaFree(c->dDS); cudaFree(c->dY); cudaFree(c->dW); cudaFree(c->dCP); cudaFree(c->dXJ); cudaFree(c->ddbg); cudaFree(c->dqueue);
     if (c->ws_event) cudaEventDestroy(c->ws_event);
     hostpipe_free(c);
     if (c->hp.s_in) {
@@ -292,6 +294,30 @@ extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx *
                 C1[(size_t)k * M.Ppad + ((jp >> 2) & 1) * (M.Ppad >> 1) + (jp >> 3) * 4 + (jp & 3)] = Cp[(size_t)k * M.Ppad + jp];
         CUDA_TRY_C(cudaMalloc(&c->dC1, C1.size() * sizeof(float)));
         CUDA_TRY_C(cudaMemcpy(c->dC1, C1.data(), C1.size() * sizeof(float), cudaMemcpyHostToDevice));
+    }
+    if (K <= 32) {
+        // v1's tensor-pipe copy: A fragments of mma.m16n8k8 (rows = pixels, columns = terms), one float4 per
+        // (octet o, k-step s, lane l): {hi, hi', lo, lo'} of C[8s + l%4 (+4)][8o + l/4], hi = tf32(x), lo = tf32(x - hi)
+        auto tf32 = [](float x) {
+            uint32_t u; memcpy(&u, &x, 4);
+            u = (u + 0x1000u) & 0xFFFFE000u;            // round to nearest, ties away (cvt.rna.tf32)
+            float r; memcpy(&r, &u, 4); return r;
+        };
+        const int ks = (K + 7) / 8, noct = M.Ppad / 8 + 1;
+        std::vector<float> CF((size_t)noct * ks * 32 * 4, 0.f);
+        for (int o = 0; o + 1 < noct; ++o)
+            for (int sidx = 0; sidx < ks; ++sidx)
+                for (int l = 0; l < 32; ++l)
+                    for (int h = 0; h < 2; ++h) {
+                        const int k = 8 * sidx + (l & 3) + 4 * h, jp = 8 * o + (l >> 2);
+                        const float x = k < K ? Cp[(size_t)k * M.Ppad + jp] : 0.f;
+                        const float hi = tf32(x), lo = tf32(x - hi);
+                        float *f = &CF[(((size_t)o * ks + sidx) * 32 + l) * 4];
+                        f[h] = hi; f[2 + h] = lo;
+                    }
+        c->cf_ksteps = ks;
+        CUDA_TRY_C(cudaMalloc(&c->dCF, CF.size() * sizeof(float)));
+        CUDA_TRY_C(cudaMemcpy(c->dCF, CF.data(), CF.size() * sizeof(float), cudaMemcpyHostToDevice));
     }
     {   // 1/s_j and s_j^2 for v1's per-pixel kernels, V1_TPAD replicated entries on both sides
         std::vector<float> is1(M.Ppad + 2 * V1_TPAD), s21(M.Ppad + 2 * V1_TPAD);
@@ -580,6 +606,10 @@ extern "C" int lasp_fit_batch(lasp_ctx *c, int64_t B, const float *flux, const f
         !(opts->beta2 >= 0.f && opts->beta2 < 1.f) || !(opts->eps >= 0.f))
         return fail(c, LASP_ERR_INVALID_ARG, "lasp_fit_batch: bad Adam hyper-parameters");
     if (B > (int64_t)1 << 30) return fail(c, LASP_ERR_UNSUPPORTED, "B too large");
+    if (opts->emulator_path < 0 || opts->emulator_path > 2)
+        return fail(c, LASP_ERR_INVALID_ARG, "lasp_fit_batch: emulator_path must be 0, 1 or 2");
+    if (opts->emulator_path == 2 && !(c->v1_ok && c->dCF))
+        return fail(c, LASP_ERR_UNSUPPORTED, "emulator_path 2 (tensor pipe) needs the resident kernel and n_terms <= 32");
     if (c->v1_ok) {
         int rc = v1_workspace(c, B, err != nullptr);
         if (rc) return rc;
@@ -591,6 +621,8 @@ extern "C" int lasp_fit_batch(lasp_ctx *c, int64_t B, const float *flux, const f
         V1Args a;
         memset(&a, 0, sizeof(a));
         a.Y = c->dY; a.W = c->dW; a.C1 = c->dC1; a.CP = c->dCP; a.XJ = c->dXJ; a.B = B;
+        // emulator on the tensor pipe (opts->emulator_path == 2; LASP_EMU_MMA forces it, also for lasp_eval_grad)
+        if ((opts->emulator_path == 2 || getenv("LASP_EMU_MMA")) && c->dCF) { a.CF = c->dCF; a.ksteps = c->cf_ksteps; }
         a.IS = c->dIS; a.S2 = c->dS2; a.DS = c->dDS;
         const int grid = v1_grid(c, B, a.ngroups);
         a.init = init; a.n_iter = opts->n_iter; a.lr = opts->lr; a.b1 = opts->beta1; a.b2 = opts->beta2;
@@ -645,6 +677,7 @@ extern "C" int lasp_eval_grad(lasp_ctx *c, int64_t B, const float *flux, const f
         V1Args a;
         memset(&a, 0, sizeof(a));
         a.Y = c->dY; a.W = c->dW; a.C1 = c->dC1; a.CP = c->dCP; a.B = B;
+        if (getenv("LASP_EMU_MMA") && c->dCF) { a.CF = c->dCF; a.ksteps = c->cf_ksteps; }
         a.IS = c->dIS; a.S2 = c->dS2; a.DS = c->dDS;
         const int grid = v1_grid(c, B, a.ngroups);
         a.gparams = params; a.chi2 = chi2; a.grad_u = grad_u; a.cont = cont; a.status = status;

@@ -75,10 +75,11 @@ def check_grad(gpu, oracle_mod, case, params):
     m.close()
 
 
-def check_fit(gpu, oracle_mod, case, n_iter, lr=1e-2, want_err=True):
+def check_fit(gpu, oracle_mod, case, n_iter, lr=1e-2, want_err=True, emulator_path=0):
     m = gpu.LaspModel(case["desc"])
     o = oracle_mod.Oracle(case["desc"])
-    r = m.fit_batch(case["flux"], case["ivar"], case["mask"], case["init"], n_iter, lr=lr, want_err=want_err)
+    r = m.fit_batch(case["flux"], case["ivar"], case["mask"], case["init"], n_iter, lr=lr, want_err=want_err,
+                    emulator_path=emulator_path)
     ref = o.fit(case["flux"], case["ivar"], case["mask"], case["init"], n_iter, lr=lr, want_err=want_err)
     par = r["params"].cpu().numpy().astype(np.float64)
     dpar = np.abs(par - ref["params"]) / (o.hi - o.lo)
@@ -230,6 +231,37 @@ def test_bad_arguments_return_error_codes(gpu):
     d3 = dict(d); d3["hi"] = d["lo"].copy()
     with pytest.raises(gpu.LaspError):
         gpu.LaspModel(d3)          # lo >= hi
+
+
+# ------------------------------------------------------------------ emulator on the tensor pipe (emulator_path = 2)
+
+def test_grad_tensor_pipe_emulator(gpu, oracle_mod, monkeypatch):
+    """chi2 / gradient / continuum with T = phi.C formed by mma.sync TF32 on split operands (lasp_eval_grad has no
+    options argument: the LASP_EMU_MMA switch selects the path), ragged batch, masked pixels."""
+    monkeypatch.setenv("LASP_EMU_MMA", "1")
+    case = synth.make_case(1, oracle_mod.forward, B=40)
+    check_grad(gpu, oracle_mod, case, case["init"])
+
+
+def test_fit_tensor_pipe_emulator(gpu, oracle_mod):
+    case = synth.make_case(0, oracle_mod.forward)
+    check_fit(gpu, oracle_mod, case, case["config"].n_iter, emulator_path=2)
+    case = synth.make_case(1, oracle_mod.forward, B=24)
+    r2, _ = check_fit(gpu, oracle_mod, case, case["config"].n_iter, emulator_path=2)
+    m = gpu.LaspModel(case["desc"])
+    r1 = m.fit_batch(case["flux"], case["ivar"], case["mask"], case["init"], case["config"].n_iter, emulator_path=1)
+    # the two paths round differently, so they must not be bit-identical (else path 2 silently ran path 1) ...
+    assert not np.array_equal(r1["params"].cpu().numpy(), r2["params"].cpu().numpy())
+    # ... and a model the tensor-pipe path does not cover refuses it instead of falling back
+    with pytest.raises(gpu.LaspError):
+        m.fit_batch(case["flux"], case["ivar"], case["mask"], case["init"], 1, emulator_path=3)
+    m.close()
+    big = make(two_arm_config(n_iter=1), oracle_mod, B=2)
+    if big["desc"]["n_terms"] > 32:
+        mb = gpu.LaspModel(big["desc"])
+        with pytest.raises(gpu.LaspError):
+            mb.fit_batch(big["flux"], big["ivar"], big["mask"], big["init"], 1, emulator_path=2)
+        mb.close()
 
 
 # ------------------------------------------------------------------ host pipeline (config 3 path)
