@@ -86,7 +86,7 @@ typedef struct {
     int32_t variant;              /* 0 auto; reserved (1 resident, 2 streaming) */
     int32_t emulator_path;        /* emulator contraction T = phi.C (Eq. 1): 0 auto (= 1: measured faster),
                                      1 FP32 FMA, 2 tensor pipe: mma.sync TF32 with both operands split x = hi + lo
-                                     (3xTF32-class accuracy); 2 needs the resident kernel and n_terms <= 32, else
+                                     (3xTF32-class accuracy); 2 needs the resident kernel and n_terms <= 128, else
                                      LASP_ERR_UNSUPPORTED; other values LASP_ERR_INVALID_ARG */
 } lasp_fit_opts;
 

@@ -68,7 +68,7 @@ struct V1Args {
     float *DS;
     unsigned int *queue;   // work-queue counter for the fit kernel (zeroed before the launch), may be null
     const float4 *CF;      // coefficient table as tf32 [hi|lo] MMA fragments (null: FP32-pipe emulator)
-    int ksteps;            // k-steps of 8 terms in CF (<= 4)
+    int ksteps;            // k-steps of 8 terms in CF (<= 16)
 };
 #define V1_TPAD 256
 
@@ -539,7 +539,7 @@ __device__ __noinline__ void v1_phase_emulator(const SegDev &sg, int lo, int hi)
 // (x = hi + lo, each a tf32 number): rows = 16 pixels, k = 8 terms, and the 8 columns carry [phi_hi | phi_lo] of the
 // GS = 4 spectra, so that two MMAs (table hi, table lo) form all four partial products in FP32 accumulators.
 // Warp w owns pixels [lo + 256 w, lo + 256 w + 256) of every sweep; the table comes pre-split in fragment order
-// (lasp_gpu.cu), one LDG.128 per (octet, k-step).
+// (lasp_gpu.cu), one LDG.128 per (octet, k-step).  Models with up to 128 terms (NCH <= 4).
 // ------------------------------------------------------------------------------------------
 __device__ __forceinline__ float v1_tf32(float x)
 {
@@ -556,6 +556,8 @@ __device__ __forceinline__ void v1_mma_tf32(float (&d)[4], float a0, float a1, f
                    "r"(__float_as_uint(b0)), "r"(__float_as_uint(b1)));
 }
 
+// NCH = number of chunks of four k-steps (32 terms) whose B fragments are held in registers: K <= 32 * NCH
+template <int NCH>
 __device__ __noinline__ void v1_phase_emulator_mma(const SegDev &sg, int lo, int hi)
 {
     const int lane = V1_LANE, gid = lane >> 2, tig = lane & 3, K = v1_blk.M.K, ks = v1_blk.A.ksteps;
@@ -564,9 +566,9 @@ __device__ __noinline__ void v1_phase_emulator_mma(const SegDev &sg, int lo, int
     float *rowT = V1SM + v1_blk.L.oT + v1_blk.L.GUARD - sg.po;
     const float *phi = V1SM + v1_blk.L.oPHI + (gid & 3);
     // B fragments (k = term, n = column): columns 0..3 carry phi_hi of spectrum n, columns 4..7 phi_lo of spectrum n - 4
-    float b0[4], b1[4];
+    float b0[4 * NCH], b1[4 * NCH];
 #pragma unroll
-    for (int s = 0; s < 4; ++s) {
+    for (int s = 0; s < 4 * NCH; ++s) {
         const int k0 = 8 * s + tig, k1 = k0 + 4;
         const float p0 = k0 < K ? phi[k0 * GS] : 0.f, p1 = k1 < K ? phi[k1 * GS] : 0.f;
         const float h0 = v1_tf32(p0), h1 = v1_tf32(p1);
@@ -575,7 +577,7 @@ __device__ __noinline__ void v1_phase_emulator_mma(const SegDev &sg, int lo, int
     }
     const int g0 = 2 * (tig & 1), half = tig >> 1;    // after the hi/lo fold: this lane stores spectra g0, g0+1 of octet o + half
     for (int base = lo + V1_WARP * 256; base < hi; base += sweep) {
-        // two 16-pixel tiles per trip: their 4 ks LDG.128 are all in flight before the first MMA, and the four
+        // two 16-pixel tiles per trip: the 16 LDG.128 of a chunk are all in flight before its first MMA, and the four
         // accumulation chains (tile x table hi/lo) are independent
 #pragma unroll 1
         for (int mt = 0; mt < 16; mt += 2) {
@@ -583,20 +585,23 @@ __device__ __noinline__ void v1_phase_emulator_mma(const SegDev &sg, int lo, int
             if (jA >= hi) break;                           // warp-uniform
             const int jB = jA + 16 < hi ? jA + 16 : jA;    // odd tail: the second tile repeats the first (not stored)
             const float4 *fA = CF + (size_t)(jA >> 3) * ks * 32, *fB = CF + (size_t)(jB >> 3) * ks * 32;
-            float4 A0[4], A1[4], B0[4], B1[4];
-#pragma unroll
-            for (int s = 0; s < 4; ++s) {
-                const int sc = s < ks ? s : 0;             // k-steps past ks re-read step 0 (their B fragments are zero)
-                A0[s] = __ldg(fA + sc * 32); A1[s] = __ldg(fA + (ks + sc) * 32);
-                B0[s] = __ldg(fB + sc * 32); B1[s] = __ldg(fB + (ks + sc) * 32);
-            }
             float ah[4] = {0.f, 0.f, 0.f, 0.f}, al[4] = {0.f, 0.f, 0.f, 0.f}, bh[4] = {0.f, 0.f, 0.f, 0.f}, bl[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-            for (int s = 0; s < 4; ++s) {
-                v1_mma_tf32(ah, A0[s].x, A1[s].x, A0[s].y, A1[s].y, b0[s], b1[s]);   // table hi
-                v1_mma_tf32(bh, B0[s].x, B1[s].x, B0[s].y, B1[s].y, b0[s], b1[s]);
-                v1_mma_tf32(al, A0[s].z, A1[s].z, A0[s].w, A1[s].w, b0[s], b1[s]);   // table lo
-                v1_mma_tf32(bl, B0[s].z, B1[s].z, B0[s].w, B1[s].w, b0[s], b1[s]);
+            for (int ch = 0; ch < NCH; ++ch) {
+                float4 A0[4], A1[4], B0[4], B1[4];
+#pragma unroll
+                for (int s = 0; s < 4; ++s) {
+                    const int sc = 4 * ch + s < ks ? 4 * ch + s : 0;   // k-steps past ks re-read step 0 (their B fragments are zero)
+                    A0[s] = __ldg(fA + sc * 32); A1[s] = __ldg(fA + (ks + sc) * 32);
+                    B0[s] = __ldg(fB + sc * 32); B1[s] = __ldg(fB + (ks + sc) * 32);
+                }
+#pragma unroll
+                for (int s = 0; s < 4; ++s) {
+                    v1_mma_tf32(ah, A0[s].x, A1[s].x, A0[s].y, A1[s].y, b0[4 * ch + s], b1[4 * ch + s]);   // table hi
+                    v1_mma_tf32(bh, B0[s].x, B1[s].x, B0[s].y, B1[s].y, b0[4 * ch + s], b1[4 * ch + s]);
+                    v1_mma_tf32(al, A0[s].z, A1[s].z, A0[s].w, A1[s].w, b0[4 * ch + s], b1[4 * ch + s]);   // table lo
+                    v1_mma_tf32(bl, B0[s].z, B1[s].z, B0[s].w, B1[s].w, b0[4 * ch + s], b1[4 * ch + s]);
+                }
             }
             // D[pixel][n]: lane holds n = 2 tig, 2 tig + 1 for pixels gid (d0, d1) and gid + 8 (d2, d3); T_g = D[g] + D[g+4]
 #pragma unroll
@@ -1283,7 +1288,13 @@ __device__ __noinline__ void v1_evaluate(bool cold, bool mom, float *xrow, bool 
         if (!zeroed) zero_slots();
         int lo, hi;
         v1_group_range(sg, lo, hi);
-        if (v1_blk.A.CF) v1_phase_emulator_mma(sg, lo, hi); else v1_phase_emulator(sg, lo, hi);
+        if (v1_blk.A.CF) {
+            const int ks = v1_blk.A.ksteps;
+            if (ks <= 4) v1_phase_emulator_mma<1>(sg, lo, hi);
+            else if (ks <= 8) v1_phase_emulator_mma<2>(sg, lo, hi);
+            else v1_phase_emulator_mma<4>(sg, lo, hi);
+        } else
+            v1_phase_emulator(sg, lo, hi);
         tick(2);
         __syncthreads();
         tick(3);

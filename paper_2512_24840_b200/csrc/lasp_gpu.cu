@@ -295,7 +295,7 @@ extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx *
         CUDA_TRY_C(cudaMalloc(&c->dC1, C1.size() * sizeof(float)));
         CUDA_TRY_C(cudaMemcpy(c->dC1, C1.data(), C1.size() * sizeof(float), cudaMemcpyHostToDevice));
     }
-    if (K <= 32) {
+    if (K <= 128) {
         // v1's tensor-pipe copy: A fragments of mma.m16n8k8 (rows = pixels, columns = terms), one float4 per
         // (octet o, k-step s, lane l): {hi, hi', lo, lo'} of C[8s + l%4 (+4)][8o + l/4], hi = tf32(x), lo = tf32(x - hi)
         auto tf32 = [](float x) {
@@ -609,7 +609,7 @@ extern "C" int lasp_fit_batch(lasp_ctx *c, int64_t B, const float *flux, const f
     if (opts->emulator_path < 0 || opts->emulator_path > 2)
         return fail(c, LASP_ERR_INVALID_ARG, "lasp_fit_batch: emulator_path must be 0, 1 or 2");
     if (opts->emulator_path == 2 && !(c->v1_ok && c->dCF))
-        return fail(c, LASP_ERR_UNSUPPORTED, "emulator_path 2 (tensor pipe) needs the resident kernel and n_terms <= 32");
+        return fail(c, LASP_ERR_UNSUPPORTED, "emulator_path 2 (tensor pipe) needs the resident kernel and n_terms <= 128");
     if (c->v1_ok) {
         int rc = v1_workspace(c, B, err != nullptr);
         if (rc) return rc;

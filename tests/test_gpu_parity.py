@@ -256,12 +256,14 @@ def test_fit_tensor_pipe_emulator(gpu, oracle_mod):
     with pytest.raises(gpu.LaspError):
         m.fit_batch(case["flux"], case["ivar"], case["mask"], case["init"], 1, emulator_path=3)
     m.close()
-    big = make(two_arm_config(n_iter=1), oracle_mod, B=2)
-    if big["desc"]["n_terms"] > 32:
-        mb = gpu.LaspModel(big["desc"])
-        with pytest.raises(gpu.LaspError):
-            mb.fit_batch(big["flux"], big["ivar"], big["mask"], big["init"], 1, emulator_path=2)
-        mb.close()
+
+
+def test_tensor_pipe_emulator_config4_high_dim(gpu, oracle_mod, monkeypatch):
+    """K = 105 terms, 13 labels, three linear-grid arms: 14 k-steps in four register chunks; gradient and a short fit."""
+    case = synth.make_case(4, oracle_mod.forward, B=6)
+    check_fit(gpu, oracle_mod, case, 40, emulator_path=2)
+    monkeypatch.setenv("LASP_EMU_MMA", "1")
+    check_grad(gpu, oracle_mod, case, case["init"])
 
 
 # ------------------------------------------------------------------ host pipeline (config 3 path)
