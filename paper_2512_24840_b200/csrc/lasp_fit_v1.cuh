@@ -998,7 +998,9 @@ __device__ __noinline__ void v1_phase_solve(int g, int seg, bool refactor)
 // a5 (evaluation part) + a6.  c_j = sum_n b_n T_n(t_j) on the thread's octet -> c_prev scratch;
 //   MODE 0: nothing else (between the two solves of a cold start);
 //   MODE 1: r = y - c S, chi2, adjoint a = -2 w r c -> row A (replaces S), ngood, min c;
-//   MODE 2: as 1, and rho = sqrt(w) r -> global row `xrow` (a9).
+//   MODE 2: as 1, and rho = sqrt(w) r -> global row `xrow` (a9);
+//   MODE 3: the adjoint only (Adam steps on uniform segments: chi2, ngood and min c are not needed until the final
+//           evaluation, so their per-pixel updates and the reduction are left out).
 // chi2 / ngood / cmin are reduced over the warp and accumulated in this warp's SLOT_STAT slots (zeroed by v1_evaluate).
 // ------------------------------------------------------------------------------------------
 template <int MODE, bool UNI>
@@ -1069,8 +1071,10 @@ __device__ __noinline__ void v1_phase_residual(const SegDev &sg, int rowB, float
             for (int i = 0; i < OCT; ++i) {
                 const float r = fmaf(-cc[g][i], SS[i], yy[i]);
                 const float wr = ww[i] * r;
-                chi[g] = fmaf(wr, r, chi[g]);
-                if (ww[i] > 0.f) { cmin[g] = fminf(cmin[g], cc[g][i]); ng[g] += 1.f; }
+                if (MODE != 3) {
+                    chi[g] = fmaf(wr, r, chi[g]);
+                    if (ww[i] > 0.f) { cmin[g] = fminf(cmin[g], cc[g][i]); ng[g] += 1.f; }
+                }
                 av[i] = -2.f * wr * cc[g][i];
                 if (MODE == 2) rho[i] = sqrtf(ww[i]) * r;
             }
@@ -1100,7 +1104,7 @@ __device__ __noinline__ void v1_phase_residual(const SegDev &sg, int rowB, float
             }
         }
     }
-    if (MODE != 0) {
+    if (MODE == 1 || MODE == 2) {
         // one register transpose for the sums (chi2, ngood, and the two kernel-parameter gradients of per-pixel
         // segments): value (kind, g) at kind*4 + g; the minimum of c by shuffles
         float *red = V1SM + L.oRED + V1_WARP * L.VR * GS;
@@ -1229,11 +1233,11 @@ __device__ __noinline__ void v1_phase_adjoint(const SegDev &sg, int lo, int hi)
 //   cold: b = 0, c_prev = 0, solve twice (solve + one refinement);  else b, c_prev are warm.
 //   mom : re-accumulate the Gram moments and re-factor (always true when cold).
 //   MODE 0: chi2 + gradient partials (Q slots) ; MODE 1: chi2 only ; MODE 2: chi2 + rho -> xrow.
-// On return (after the closing barrier) the per-warp reduction slots hold chi2 / ngood / min c and,
-// for MODE 0, the q / dv / dsigma partials.
+// On return (after the closing barrier) the per-warp reduction slots hold chi2 / ngood / min c (not with `stats`
+// false on uniform segments: the Adam steps do not read them) and, for MODE 0, the q / dv / dsigma partials.
 // ------------------------------------------------------------------------------------------
 template <int MODE>
-__device__ __noinline__ void v1_evaluate(bool cold, bool mom, float *xrow, bool wready = false)
+__device__ __noinline__ void v1_evaluate(bool cold, bool mom, float *xrow, bool wready = false, bool stats = true)
 {
     const V1Args &a = v1_blk.A;
     const ModelDev &M = v1_blk.M;
@@ -1315,7 +1319,8 @@ __device__ __noinline__ void v1_evaluate(bool cold, bool mom, float *xrow, bool 
             if (V1_WARP < GS) v1_phase_solve(V1_WARP, s, false);
             __syncthreads();
         }
-        if (sg.uniform) v1_phase_residual<(MODE == 2 ? 2 : 1), true>(sg, rowB, xrow);
+        if (MODE == 0 && !stats && sg.uniform) v1_phase_residual<3, true>(sg, rowB, xrow);   // Adam step: no statistics
+        else if (sg.uniform) v1_phase_residual<(MODE == 2 ? 2 : 1), true>(sg, rowB, xrow);
         else v1_phase_residual<(MODE == 2 ? 2 : 1), false>(sg, rowB, xrow);
         tick(8);
         __syncthreads();
@@ -1705,7 +1710,7 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
             const long long te0 = a.dbg ? clock64() : 0;
 #endif
             // fresh Gram factor on each of the first `refresh` steps (the model moves fastest there), then every `refresh`-th
-            v1_evaluate<0>(t == 1, t <= L.warm || (t - 1) % L.refresh == 0, nullptr, t > 1 && L.fastw);
+            v1_evaluate<0>(t == 1, t <= L.warm || (t - 1) % L.refresh == 0, nullptr, t > 1 && L.fastw, false);
 #ifdef LASP_PHASE_TIMING
             if (a.dbg && V1_TID == 0) { atomicAdd(a.dbg + 14, (unsigned long long)(clock64() - te0)); atomicAdd(a.dbg + 15, 1ull); }
             const long long tu0 = a.dbg ? clock64() : 0;
