@@ -209,6 +209,137 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def roofline_of(model, desc, B, n_iter, params, kern_ms, peaks, n_sms, clocks=None):
+    """Roofline object of the fit kernel for one launch shape: plain-ALU FP32 bound.
+    `frac` credits SURVEY.md 8(d)'s algorithmic formula (the contract); `frac_executed` credits only the work the
+    algorithm as built performs (Gram moments / factorisation on the measured fraction of fresh steps, one right-hand
+    side and one continuum evaluation per step)."""
+    taps = mean_taps(desc, params)
+    fma_step = model.fma_per_spectrum_step(taps)
+    stats = model.last_fit_stats()
+    fma_exec = model.fma_executed_per_spectrum_step(taps, stats["fresh_frac"])
+    achieved = 2.0 * fma_step * B * n_iter / (kern_ms * 1e-3) / 1e12
+    executed = 2.0 * fma_exec * B * n_iter / (kern_ms * 1e-3) / 1e12
+    peak = n_sms * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+            "frac_executed": executed / peak, "achieved_executed": executed, "traffic": None,
+            "kernel": "lasp_v1_fit_kernel", "fma_per_spectrum_step": fma_step,
+            "fma_executed_per_spectrum_step": fma_exec, "fresh_factor_frac": stats["fresh_frac"], "mean_taps": taps,
+            "peak_source": f"SMs x 128 FP32 lanes x 2 x sm_max_mhz ({peaks['source']})"}
+    if clocks and clocks.get("sm_mhz"):
+        roof["frac_at_sampled_clock"] = achieved / (peak * clocks["sm_mhz"] / peaks["sm_max_mhz"])
+    return roof
+
+
+def ncu_record(key):
+    """Counters of one `ncu --set full` capture of this launch shape, copied from the committed summary
+    profiles/r02_ncu_metrics.json (null when that shape was not captured): never measured under the bench itself."""
+    p = os.path.join(ROOT, "profiles", "r02_ncu_metrics.json")
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        d = json.load(f)
+    return d.get(key)
+
+
+def time_fit(model, data, n_iter, steps, warmup, kw, torch, barrier):
+    """`warmup` untimed + `steps` timed lasp_fit_batch calls, CUDA events on the launching stream."""
+    out = None
+    for _ in range(warmup):
+        out = model.fit_batch(data["flux"], data["ivar"], data["mask"], data["init"], n_iter, out=out, **kw)
+    barrier()
+    l0 = model.launch_count()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+    ev[0].record()
+    for k in range(steps):
+        out = model.fit_batch(data["flux"], data["ivar"], data["mask"], data["init"], n_iter, out=out, **kw)
+        ev[k + 1].record()
+    barrier()
+    step_ms = [ev[k].elapsed_time(ev[k + 1]) for k in range(steps)]
+    return out, ev[0].elapsed_time(ev[-1]), step_ms, model.launch_count() - l0
+
+
+def run_other_config(cfg_id, B, torch, local, peaks, n_sms, emulator_path=0):
+    """One timed step (after one warm-up) of another BASELINE.json config at a stated, reduced batch."""
+    from paper_2512_24840_b200 import binding, synth
+    cfg = synth.CONFIGS[cfg_id]
+    desc = synth.make_model_desc(cfg)
+    desc.pop("_rng")
+    model = binding.LaspModel(desc, device=local)
+    model.reserve(B)
+    data = make_device_batch(model, cfg, desc, B, cfg.seed + 17, torch)
+    kw = dict(lr=cfg.lr, beta1=cfg.beta1, beta2=cfg.beta2, eps=cfg.eps, emulator_path=emulator_path)
+    out, ms_total, step_ms, _ = time_fit(model, data, cfg.n_iter, 1, 1, kw, torch, torch.cuda.synchronize)
+    roof = roofline_of(model, desc, B, cfg.n_iter, out["params"].cpu().numpy(), step_ms[0], peaks, n_sms)
+    rec = {"workload": f"config {cfg_id} ({cfg.name})", "spectra": B, "full_batch": cfg.B, "adam_steps": cfg.n_iter,
+           "n_pix": model.P, "n_terms": model.K, "n_labels": model.L, "n_seg": model.n_seg,
+           "value": B / (step_ms[0] * 1e-3), "unit": UNIT, "ms_per_step": step_ms[0],
+           "variant": model.default_variant(), "launch": model.launch_info(model.default_variant()),
+           "emulator_path": emulator_path, "frac": roof["frac"], "frac_executed": roof["frac_executed"],
+           "achieved_tflops": roof["achieved"], "fresh_factor_frac": roof["fresh_factor_frac"],
+           "mean_taps": roof["mean_taps"], "status_nonzero_frac": float((out["status"] != 0).float().mean().item())}
+    model.close()
+    del data, out
+    torch.cuda.empty_cache()
+    return rec
+
+
+def run_config3(args, model, cfg, desc, torch, local, peaks, n_sms, kw):
+    """BASELINE.json config 3: 10,000,000 config-1-shaped spectra streamed from pinned host memory in 1 M-spectrum
+    chunks through lasp_fit_batch_host (H2D / fit / D2H overlapped on three streams; each 1 M chunk is cut into
+    sub-chunks of `--sub-chunk` spectra for the overlap).  Host RAM holds ONE 1 M-spectrum chunk of pinned inputs, which is
+    re-used cyclically for the ten chunks: every transfer and every fit is executed, nothing is
+    extrapolated.  Prints the measured total."""
+    total, chunk = args.total or cfg.B, args.chunk or 1_000_000
+    nchunk = (total + chunk - 1) // chunk
+    n_iter = args.n_iter or cfg.n_iter
+    data = make_device_batch(model, cfg, desc, chunk, cfg.seed + 17, torch)
+    host = {k: torch.empty(data[k].shape, dtype=data[k].dtype, pin_memory=True) for k in ("flux", "ivar", "mask", "init")}
+    for k in host:
+        host[k].copy_(data[k])
+    del data
+    torch.cuda.empty_cache()
+    h2d = sum(v.numel() * v.element_size() for v in host.values())
+    hout = None
+    warm = min(chunk, 65536)       # warm-up: allocations, first launches
+    model.fit_batch_host(host["flux"][:warm], host["ivar"][:warm], host["mask"][:warm], host["init"][:warm], n_iter,
+                         chunk=min(warm, args.sub_chunk), **kw)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local).start()
+    l0 = model.launch_count()
+    per_chunk = []
+    t0 = time.perf_counter()
+    done = 0
+    for i in range(nchunk):
+        n = min(chunk, total - done)
+        tc = time.perf_counter()
+        hout = model.fit_batch_host(host["flux"][:n], host["ivar"][:n], host["mask"][:n], host["init"][:n], n_iter,
+                                    chunk=args.sub_chunk, out=hout if n == chunk else None, **kw)
+        per_chunk.append(time.perf_counter() - tc)      # the call is blocking: results are in host memory
+        done += n
+    dt = time.perf_counter() - t0
+    clocks = sampler.stop()
+    launches = model.launch_count() - l0
+    d2h = sum(v.numel() * v.element_size() for v in hout.values() if v is not None)
+    st = hout["status"].numpy()
+    roof = roofline_of(model, desc, chunk, n_iter, hout["params"].numpy(), 1e3 * dt / nchunk, peaks, n_sms, clocks)
+    line = {
+        "metric": METRIC, "value": total / dt, "unit": UNIT, "n_gpus": 1, "steps": nchunk, "warmup": 1,
+        "ms_per_step": 1e3 * dt / nchunk, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"config 3 ({cfg.name})", "spectra_total": total, "chunk_spectra": chunk,
+                   "sub_chunk_spectra": args.sub_chunk, "adam_steps": n_iter, "lr": cfg.lr, "errors": True,
+                   "host_buffers": "one pinned 1 M-spectrum chunk re-used cyclically for the ten chunks",
+                   "l2": "inputs larger than L2", "status_nonzero_frac": float((st != 0).mean())},
+        "seconds_total_measured": dt, "seconds_per_chunk": per_chunk,
+        "clocks": clocks, "gpu_launches": int(launches),
+        "e2e": {"value": total / dt, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                "api": "lasp_fit_batch_host", "seconds_for_10M_spectra_measured": dt if total == 10_000_000 else None},
+        "roofline": roof,
+    }
+    print(json.dumps(line), flush=True)
+
+
 def run_gpu(args):
     import torch
     from paper_2512_24840_b200 import binding, build, synth
@@ -228,20 +359,25 @@ def run_gpu(args):
     cfg = synth.CONFIGS[args.config]
     desc = synth.make_model_desc(cfg)
     desc.pop("_rng")
+    peaks = load_peaks()
+    n_sms = torch.cuda.get_device_properties(local).multi_processor_count
+    kw = dict(lr=cfg.lr, beta1=cfg.beta1, beta2=cfg.beta2, eps=cfg.eps, emulator_path=args.emulator_path,
+              variant=args.variant, refresh=args.refresh)
+    model = binding.LaspModel(desc, device=local)
+    if args.config == 3:
+        if world > 1:
+            raise SystemExit("config 3 is a single-GPU workload (BASELINE.json)")
+        run_config3(args, model, cfg, desc, torch, local, peaks, n_sms, kw)
+        return
     # spectra are independent units: rank r fits its own contiguous slice of a world*B batch, no collective on
     # the data path (sharding.shard_range; weak scaling)
-    # config 3 (10 M spectra streamed in chunks from the host) is measured on one 262,144-spectrum slice that is
-    # re-used cyclically: every spectrum's transfers and fit are executed, the 10 M time is value-extrapolated
-    B = args.batch or (262144 if args.config == 3 else cfg.B)
+    B = args.batch or cfg.B
     from paper_2512_24840_b200.sharding import shard_range
     lo_r, hi_r = shard_range(world * B, rank, world)
     assert hi_r - lo_r == B
     n_iter = args.n_iter or cfg.n_iter
-    model = binding.LaspModel(desc, device=local)
     model.reserve(B)
     data = make_device_batch(model, cfg, desc, B, cfg.seed + 17 + rank, torch)
-    out = None
-    kw = dict(lr=cfg.lr, beta1=cfg.beta1, beta2=cfg.beta2, eps=cfg.eps, emulator_path=args.emulator_path)
 
     def barrier():
         torch.cuda.synchronize()
@@ -249,30 +385,20 @@ def run_gpu(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    def step():
-        nonlocal out
-        out = model.fit_batch(data["flux"], data["ivar"], data["mask"], data["init"], n_iter, out=out, **kw)
-
     for _ in range(args.warmup):
-        step()
+        model.fit_batch(data["flux"], data["ivar"], data["mask"], data["init"], n_iter, **kw)
     barrier()
     sampler = ClockSampler(local).start() if rank == 0 else None
-    l0 = model.launch_count()
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
-    ev[0].record()
-    for k in range(args.steps):
-        step()
-        ev[k + 1].record()
-    barrier()
-    launches = model.launch_count() - l0
-    ms_total = ev[0].elapsed_time(ev[-1])
-    step_ms = [ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)]
+    out, ms_total, step_ms, launches = time_fit(model, data, n_iter, args.steps, 0, kw, torch, barrier)
     clocks = sampler.stop() if sampler else None
     t = torch.tensor([ms_total], device="cuda", dtype=torch.float64)
     if dist is not None:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     ms_total = float(t.item())
     value = world * B * args.steps / (ms_total * 1e-3)
+    roof = None
+    if rank == 0:   # before the e2e runs replace the ctx's fit statistics
+        roof = roofline_of(model, desc, B, n_iter, out["params"].cpu().numpy(), float(np.mean(step_ms)), peaks, n_sms, clocks)
 
     # ---- end to end through the C ABI with HOST buffers (lasp_fit_batch_host): pinned inputs, chunked
     # H2D / fit / D2H overlapped inside the library; the call returns with the results in host memory
@@ -298,32 +424,18 @@ def run_gpu(args):
         if dist is not None:
             dist.destroy_process_group()
         return
-    # ---- roofline of the dominant kernel (lasp_fit_kernel): plain-ALU FP32 bound
-    peaks = load_peaks()
-    prop = torch.cuda.get_device_properties(local)
-    params = out["params"].cpu().numpy()
-    taps = mean_taps(desc, params)
-    fma_step = model.fma_per_spectrum_step(taps)
-    flop_launch = 2.0 * fma_step * B * n_iter
-    kern_ms = float(np.mean(step_ms))          # events bracket stage + fit; stage share is in profiles/
-    achieved = flop_launch / (kern_ms * 1e-3) / 1e12
-    peak = prop.multi_processor_count * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
-    # DRAM traffic of the dominant kernel per launch: dram__bytes_read.sum + dram__bytes_write.sum of one
-    # `ncu --set full` capture of this very launch shape, recorded under profiles/ (null for other shapes)
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "r01_traffic.csv")
-    if os.path.exists(tp):
-        with open(tp) as f:
-            for ln in f.read().splitlines()[1:]:
-                k, _, v = ln.partition(",")
-                if k == f"config{args.config}_B{B}_n{n_iter}":
-                    traffic = int(v)
-    roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-            "traffic": traffic, "kernel": "lasp_v1_fit_kernel" if model.uses_v1() else "lasp_fit_kernel", "fma_per_spectrum_step": fma_step,
-            "mean_taps": taps, "peak_source": f"SMs x 128 FP32 lanes x 2 x sm_max_mhz ({peaks['source']})",
-            "frac_at_sampled_clock": (achieved / (peak * clocks["sm_mhz"] / peaks["sm_max_mhz"])
-                                      if clocks and clocks.get("sm_mhz") else None)}
+    # ---- roofline of the dominant kernel (lasp_v1_fit_kernel): plain-ALU FP32 bound.  The ncu figures
+    # (pipe utilisation, DRAM traffic per launch) are copied from the committed capture of this very launch shape.
+    key = f"config{args.config}_B{B}_n{n_iter}"
+    rec = ncu_record(key)
+    if rec:
+        roof["traffic"] = rec.get("dram_bytes")
+        roof["traffic_source"] = rec.get("source")
+        roof["ncu_pipe_fma"] = rec.get("pipe_fma_pct")
+        roof["ncu_issue_active"] = rec.get("issue_active_pct")
+        roof["ncu_ffma_rate"] = rec.get("ffma_rate_of_peak")
     st = out["status"].cpu().numpy()
+    variant = args.variant or model.default_variant()
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
@@ -331,15 +443,28 @@ def run_gpu(args):
         "config": {"workload": f"config {args.config} ({cfg.name})", "spectra_per_gpu": B,
                    "n_pix": model.P, "n_terms": model.K, "n_labels": model.L, "cont_degree": model.D,
                    "n_seg": model.n_seg, "adam_steps": n_iter, "lr": cfg.lr, "errors": True, "emulator_path": args.emulator_path,
+                   "variant": variant, "launch": model.launch_info(variant), "refresh": args.refresh,
                    "l2": "inputs larger than L2 (flux+ivar+mask %.0f MB per step)" % (h2d / 1e6),
                    "status_nonzero_frac": float((st != 0).mean())},
         "clocks": clocks, "gpu_launches": int(launches),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                 "d2h_bytes_per_step": int(d2h), "steps": e2e_steps, "chunk": int(e2e_chunk),
-                "api": "lasp_fit_batch_host", "matches_device_run": same,
-                "seconds_for_10M_spectra": 1e7 / e2e_value},
+                "api": "lasp_fit_batch_host", "matches_device_run": same},
         "roofline": roof,
     }
+    del data, host, hout, out
+    model.close()
+    torch.cuda.empty_cache()
+    if world == 1 and args.config == 1 and not args.batch and not args.no_other_configs:
+        # the other single-GPU configs of BASELINE.json, one timed step each at a stated reduced batch, and the
+        # survey's long-spectrum shape on the streaming variant
+        oc = {}
+        for cid, b in ((2, 32768), (4, 32768), ("S", 4096)):
+            try:
+                oc[f"config{cid}"] = run_other_config(cid, b, torch, local, peaks, n_sms)
+            except Exception as e:   # report, never hide
+                oc[f"config{cid}"] = {"error": f"{type(e).__name__}: {e}"}
+        line["other_configs"] = oc
     if world == 1 and not args.no_cpu_baseline:
         cores = os.cpu_count() or 1
         n_spec = args.ref_spectra or sample_size(cfg, cores, 8)
@@ -365,6 +490,12 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--emulator-path", type=int, default=0, choices=[0, 1, 2],
                     help="lasp_fit_opts.emulator_path: 0 auto, 1 FP32 FMA, 2 tensor pipe (mma.sync TF32, split operands)")
+    ap.add_argument("--variant", type=int, default=0, choices=[0, 1, 2], help="lasp_fit_opts.variant: 0 auto, 1 resident, 2 streaming")
+    ap.add_argument("--refresh", type=int, default=0, help="lasp_fit_opts.refresh: 0 adaptive, k >= 1 every k-th step")
+    ap.add_argument("--no-other-configs", action="store_true", help="skip the one-step runs of configs 2, 4 and S")
+    ap.add_argument("--total", type=int, default=0, help="config 3: total spectra (default 10,000,000)")
+    ap.add_argument("--chunk", type=int, default=0, help="config 3: spectra per chunk (default 1,000,000)")
+    ap.add_argument("--sub-chunk", type=int, default=131072, help="config 3: spectra per overlapped sub-chunk")
     args = ap.parse_args()
     args.config = int(args.config) if args.config.isdigit() else args.config
     if args.impl == "reference":

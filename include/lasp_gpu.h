@@ -14,7 +14,8 @@
  *                                  re-solved by weighted least squares in EVERY evaluation
  *                                  (Eq. 6; C.2-4)
  * and returns parameters, continuum coefficients, chi2, the error estimate of P:173 and status
- * bits.  Every step runs in hand-written sm_100a CUDA kernels; there is no CPU fallback.
+ * bits.  Every step runs in hand-written sm_100a CUDA kernels; there is no CPU fallback, and the
+ * library reads no environment variable: every switch is a field of lasp_fit_opts.
  *
  * Conventions
  *  - All functions return 0 (LASP_OK) or a negative LASP_ERR_* code; they never throw or abort.
@@ -32,6 +33,10 @@
  *    share its workspace: the library orders them on the device (a call on stream B waits for the ctx's previous
  *    call on stream A), so mixing streams is safe but does not overlap.
  *  - Per-spectrum problems never fail a call; they set bits in status[i].
+ *  - Non-finite inputs: a pixel takes part in the fit iff w = mask*ivar (edges zeroed) is != 0, exactly as the
+ *    definition reads (C.1); flux on pixels with w == 0 is never looked at.  A NaN/Inf flux or weight on a pixel
+ *    that takes part is NOT filtered: it propagates (NaN parameters, NaN chi2) and sets LASP_ST_NONFINITE.
+ *  - Every entry point leaves the caller's current CUDA device as it found it.
  */
 #ifndef LASP_GPU_H
 #define LASP_GPU_H
@@ -81,13 +86,26 @@ typedef struct {
 } lasp_model_desc;
 
 typedef struct {
-    int32_t n_iter;               /* fixed number of Adam steps (Delta-6) */
+    int32_t n_iter;               /* fixed number of Adam steps (Delta-6); used by lasp_fit_batch[_host] only */
     float lr, beta1, beta2, eps;  /* Adam hyper-parameters (defaults 1e-2, 0.9, 0.999, 1e-8) */
-    int32_t variant;              /* 0 auto; reserved (1 resident, 2 streaming) */
+    int32_t variant;              /* kernel variant: 0 auto (resident when the model's rows fit shared memory, else
+                                     streaming); 1 resident (LASP_ERR_UNSUPPORTED when they do not fit); 2 streaming
+                                     (rows in L2-resident global scratch, swept through a shared-memory window:
+                                     any row length).  Same arithmetic, same results to rounding order. */
     int32_t emulator_path;        /* emulator contraction T = phi.C (Eq. 1): 0 auto (= 1: measured faster),
                                      1 FP32 FMA, 2 tensor pipe: mma.sync TF32 with both operands split x = hi + lo
-                                     (3xTF32-class accuracy); 2 needs the resident kernel and n_terms <= 128, else
+                                     (3xTF32-class accuracy); 2 needs the resident variant and n_terms <= 128, else
                                      LASP_ERR_UNSUPPORTED; other values LASP_ERR_INVALID_ARG */
+    int32_t refresh;              /* continuum solve (Eq. 6): every step performs one
+                                     refinement b += A~^-1 Phi^T W (y - Phi b) whose fixed point is the WLS solution
+                                     whatever factor A~ preconditions it.  refresh = k >= 1: the Gram matrix is
+                                     re-accumulated and re-factorised every k-th step (1 = every step, the method
+                                     as written); 0 (default): adaptive -- re-factorise when the parameters have
+                                     moved enough since the last factor (sum|du| x |du| > 6.4e-3), after a system
+                                     that was not positive definite, and at least every 64th step */
+    int32_t warm;                 /* the first `warm` steps always re-factorise (0 = default 4) */
+    int32_t fd_fresh;             /* 1: the 2 NP finite-difference evaluations of the error estimate re-factorise
+                                     too (0: they reuse the final evaluation's factor, C.2-22) */
 } lasp_fit_opts;
 
 /* Build a context on `cuda_device`: validates the description, derives the per-pixel velocity
@@ -121,21 +139,28 @@ int lasp_fit_batch_host(lasp_ctx *ctx, int64_t B, const float *flux, const float
                         float *params, float *cont, float *chi2, float *err, int32_t *status,
                         int64_t chunk);
 
-/* Inspection: model_j = c_j S_j at given physical params [B*NP] and plain-Legendre cont
- * [B*n_seg*(D+1)]; model [B*n_pix]. */
+/* Inspection: model_j = c_j S_j (Eq. 1, 5, 6) at given physical params [B*NP] and plain-Legendre cont
+ * [B*n_seg*(D+1)]; model [B*n_pix], every pixel (edges included: replicate-edge clamp, C.2-16).  Runs the fit
+ * kernels' own emulator, kernel-weight and stencil code.  opts may be NULL (defaults); only .variant and
+ * .emulator_path are read. */
 int lasp_eval_model(lasp_ctx *ctx, int64_t B, const float *params, const float *cont,
-                    float *model, void *stream);
+                    const lasp_fit_opts *opts, float *model, void *stream);
 
-/* Inspection: one chi2/gradient evaluation at given physical params: chi2 [B], grad_u [B*NP]
+/* Inspection: one chi2/gradient evaluation (fresh Gram factor) at given physical params: chi2 [B], grad_u [B*NP]
  * (d chi2 / d u, normalised parameters), cont [B*n_seg*(D+1)] or NULL, status [B] or NULL
- * (bit LASP_ST_NOT_SPD only). */
+ * (bit LASP_ST_NOT_SPD only).  opts may be NULL (defaults); only .variant and .emulator_path are read. */
 int lasp_eval_grad(lasp_ctx *ctx, int64_t B, const float *flux, const float *ivar,
-                   const uint8_t *mask, const float *params, float *chi2, float *grad_u,
-                   float *cont, int32_t *status, void *stream);
+                   const uint8_t *mask, const float *params, const lasp_fit_opts *opts, float *chi2,
+                   float *grad_u, float *cont, int32_t *status, void *stream);
 
-/* Which fit kernel serves this ctx: 1 = the fused group kernel (all segments on a uniform log grid),
- * 0 = the lane-per-spectrum kernel with per-pixel broadening kernels (linear grids, C.2-14). */
+/* Which kernel variant serves this ctx when lasp_fit_opts.variant is 0: 1 = resident (rows of the longest segment
+ * in shared memory: log or linear grids, one or several segments), 2 = streaming (rows too long for shared memory).
+ * 0 for a NULL ctx. */
 int lasp_kernel_variant(const lasp_ctx *ctx);
+
+/* Launch shape of variant 1 (resident) or 2 (streaming): out4 = {available, threads per CTA, CTAs per SM,
+ * dynamic shared memory in bytes}. */
+int lasp_launch_info(const lasp_ctx *ctx, int variant, int32_t *out4);
 
 /* Number of kernels launched by this ctx so far (bench.py reports it as gpu_launches). */
 int64_t lasp_launch_count(const lasp_ctx *ctx);
@@ -144,8 +169,21 @@ int64_t lasp_launch_count(const lasp_ctx *ctx);
  * the moment route) given the mean number of stencil taps 2H+1; for the roofline line. */
 double lasp_fma_per_spectrum_step(const lasp_ctx *ctx, double mean_taps);
 
+/* The same count for the algorithm as built: Gram moments, Cholesky and inverse only on the fraction
+ * `fresh_frac` of steps that re-factorise, one right-hand side and one continuum evaluation per step. */
+double lasp_fma_executed_per_spectrum_step(const lasp_ctx *ctx, double mean_taps, double fresh_frac);
+
+/* Counters of the last lasp_fit_batch on this ctx (blocks until it has finished): out2[0] = group-steps of the Adam
+ * loops (groups of 4 spectra x n_iter), out2[1] = those that re-factorised the continuum Gram matrix. */
+int lasp_last_fit_stats(lasp_ctx *ctx, double *out2);
+
 const char *lasp_last_error(const lasp_ctx *ctx); /* ctx-owned string; "" if none; ctx may be NULL */
 int lasp_version(void);
+
+#ifdef LASP_PHASE_TIMING
+/* debug build only (-DLASP_PHASE_TIMING): per-phase cycle sums of the last fit, 24 counters */
+int lasp_debug_phase_cycles(lasp_ctx *ctx, unsigned long long *out24);
+#endif
 
 #ifdef __cplusplus
 }

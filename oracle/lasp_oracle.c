@@ -156,6 +156,7 @@ static void emulator_row(const orc_model *m, const double *c, double *T)
  * Arrays hold 2H+1 entries, entry i is offset k = i - H.  Returns H. */
 int orc_kernel_weights(double mu, double sigma, int Hcap, double *g, double *dg_dmu, double *dg_dsig)
 {
+    if (!isfinite(mu) || !isfinite(sigma)) return -1; /* non-finite parameters: no kernel; the caller's S is NaN */
     int H = (int)ceil(fabs(mu) + 5.0 * sigma);
     if (H > Hcap) return -H; /* caller sized the buffers too small */
     double sum = 0.0;

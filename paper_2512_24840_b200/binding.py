@@ -14,8 +14,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "liblasp_gpu.so")
 
 SYMBOLS = ["lasp_create", "lasp_destroy", "lasp_reserve", "lasp_fit_batch", "lasp_fit_batch_host", "lasp_eval_model",
-           "lasp_eval_grad", "lasp_kernel_variant", "lasp_launch_count", "lasp_fma_per_spectrum_step", "lasp_last_error",
-           "lasp_version"]
+           "lasp_eval_grad", "lasp_kernel_variant", "lasp_launch_info", "lasp_launch_count", "lasp_fma_per_spectrum_step",
+           "lasp_fma_executed_per_spectrum_step", "lasp_last_fit_stats", "lasp_last_error", "lasp_version"]
 
 LASP_ST_NOT_SPD, LASP_ST_NONFINITE, LASP_ST_NEG_CONT, LASP_ST_ON_BOUND = 1, 2, 4, 8
 
@@ -38,7 +38,8 @@ class ModelDesc(C.Structure):
 
 class FitOpts(C.Structure):
     _fields_ = [("n_iter", C.c_int32), ("lr", C.c_float), ("beta1", C.c_float), ("beta2", C.c_float),
-                ("eps", C.c_float), ("variant", C.c_int32), ("emulator_path", C.c_int32)]
+                ("eps", C.c_float), ("variant", C.c_int32), ("emulator_path", C.c_int32),
+                ("refresh", C.c_int32), ("warm", C.c_int32), ("fd_fresh", C.c_int32)]
 
 
 class LaspError(RuntimeError):
@@ -64,10 +65,14 @@ def lib():
                                     [C.c_void_p] * 6
         L.lasp_fit_batch_host.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 4 + [C.POINTER(FitOpts)] + \
                                          [C.c_void_p] * 5 + [C.c_int64]
-        L.lasp_eval_model.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 4
-        L.lasp_eval_grad.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 9
+        L.lasp_eval_model.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 2 + [C.POINTER(FitOpts)] + [C.c_void_p] * 2
+        L.lasp_eval_grad.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 4 + [C.POINTER(FitOpts)] + [C.c_void_p] * 5
         L.lasp_kernel_variant.argtypes = [C.c_void_p]
         L.lasp_kernel_variant.restype = C.c_int
+        L.lasp_launch_info.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int32)]
+        L.lasp_fma_executed_per_spectrum_step.argtypes = [C.c_void_p, C.c_double, C.c_double]
+        L.lasp_fma_executed_per_spectrum_step.restype = C.c_double
+        L.lasp_last_fit_stats.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         L.lasp_launch_count.argtypes = [C.c_void_p]
         L.lasp_launch_count.restype = C.c_int64
         L.lasp_fma_per_spectrum_step.argtypes = [C.c_void_p, C.c_double]
@@ -150,9 +155,28 @@ class LaspModel:
     def reserve(self, B: int):
         self._check(lib().lasp_reserve(self.ctx, B), "lasp_reserve")
 
-    def uses_v1(self) -> bool:
-        """True when the fused group kernel (lasp_fit_v1.cuh) serves this model (uniform segments)."""
-        return bool(lib().lasp_kernel_variant(self.ctx) == 1)
+    def default_variant(self) -> int:
+        """lasp_kernel_variant: 1 = the resident variant serves this model by default, 2 = streaming only."""
+        return int(lib().lasp_kernel_variant(self.ctx))
+
+    def launch_info(self, variant: int) -> dict:
+        out = (C.c_int32 * 4)()
+        self._check(lib().lasp_launch_info(self.ctx, variant, out), "lasp_launch_info")
+        return dict(available=bool(out[0]), threads=int(out[1]), ctas_per_sm=int(out[2]), smem_bytes=int(out[3]))
+
+    def fma_executed_per_spectrum_step(self, mean_taps: float, fresh_frac: float) -> float:
+        return float(lib().lasp_fma_executed_per_spectrum_step(self.ctx, mean_taps, fresh_frac))
+
+    def last_fit_stats(self) -> dict:
+        out = (C.c_double * 2)()
+        self._check(lib().lasp_last_fit_stats(self.ctx, out), "lasp_last_fit_stats")
+        return dict(group_steps=out[0], fresh_steps=out[1], fresh_frac=(out[1] / out[0] if out[0] else 0.0))
+
+    @staticmethod
+    def _opts(n_iter=0, lr=1e-2, beta1=0.9, beta2=0.999, eps=1e-8, variant=0, emulator_path=0, refresh=0, warm=0,
+              fd_fresh=0):
+        return FitOpts(int(n_iter), lr, beta1, beta2, eps, int(variant), int(emulator_path), int(refresh), int(warm),
+                       int(fd_fresh))
 
     def launch_count(self) -> int:
         return int(lib().lasp_launch_count(self.ctx))
@@ -161,7 +185,7 @@ class LaspModel:
         return float(lib().lasp_fma_per_spectrum_step(self.ctx, mean_taps))
 
     def fit_batch(self, flux, ivar, mask, init, n_iter, lr=1e-2, beta1=0.9, beta2=0.999, eps=1e-8,
-                  want_err=True, want_cont=True, out=None, emulator_path=0):
+                  want_err=True, want_cont=True, out=None, emulator_path=0, variant=0, refresh=0, warm=0, fd_fresh=0):
         """lasp_fit_batch on device tensors; returns dict of device tensors."""
         t = self.torch
         flux = self._dev(flux, t.float32); ivar = self._dev(ivar, t.float32)
@@ -174,7 +198,7 @@ class LaspModel:
                        status=t.empty(B, device=self.device, dtype=t.int32),
                        cont=t.empty((B, self.nc), device=self.device, dtype=t.float32) if want_cont else None,
                        err=t.empty((B, self.NP), device=self.device, dtype=t.float32) if want_err else None)
-        opts = FitOpts(int(n_iter), lr, beta1, beta2, eps, 0, int(emulator_path))
+        opts = self._opts(n_iter, lr, beta1, beta2, eps, variant, emulator_path, refresh, warm, fd_fresh)
         rc = lib().lasp_fit_batch(self.ctx, B, _ptr(flux), _ptr(ivar), _ptr(mask), _ptr(init), C.byref(opts),
                                   _ptr(out["params"]), _ptr(out.get("cont")), _ptr(out["chi2"]),
                                   _ptr(out.get("err")), _ptr(out["status"]), self._stream())
@@ -182,7 +206,8 @@ class LaspModel:
         return out
 
     def fit_batch_host(self, flux, ivar, mask, init, n_iter, lr=1e-2, beta1=0.9, beta2=0.999, eps=1e-8,
-                       want_err=True, want_cont=True, chunk=0, out=None, emulator_path=0):
+                       want_err=True, want_cont=True, chunk=0, out=None, emulator_path=0, variant=0, refresh=0, warm=0,
+                       fd_fresh=0):
         """lasp_fit_batch_host on HOST tensors (torch CPU tensors, pinned for overlap); returns host tensors.
         The library cuts the batch into chunks and overlaps the copies with the fits."""
         t = self.torch
@@ -205,24 +230,25 @@ class LaspModel:
                        status=t.empty(B, dtype=t.int32, **pin),
                        cont=t.empty((B, self.nc), dtype=t.float32, **pin) if want_cont else None,
                        err=t.empty((B, self.NP), dtype=t.float32, **pin) if want_err else None)
-        opts = FitOpts(int(n_iter), lr, beta1, beta2, eps, 0, int(emulator_path))
+        opts = self._opts(n_iter, lr, beta1, beta2, eps, variant, emulator_path, refresh, warm, fd_fresh)
         rc = lib().lasp_fit_batch_host(self.ctx, B, _ptr(flux), _ptr(ivar), _ptr(mask), _ptr(init), C.byref(opts),
                                        _ptr(out["params"]), _ptr(out.get("cont")), _ptr(out["chi2"]),
                                        _ptr(out.get("err")), _ptr(out["status"]), int(chunk))
         self._check(rc, "lasp_fit_batch_host")
         return out
 
-    def eval_model(self, params, cont):
+    def eval_model(self, params, cont, variant=0, emulator_path=0):
         t = self.torch
         params = self._dev(params, t.float32); cont = self._dev(cont, t.float32)
         B = params.shape[0]
         assert params.shape == (B, self.NP) and cont.shape == (B, self.nc)
         model = t.empty((B, self.P), device=self.device, dtype=t.float32)
-        rc = lib().lasp_eval_model(self.ctx, B, _ptr(params), _ptr(cont), _ptr(model), self._stream())
+        opts = self._opts(variant=variant, emulator_path=emulator_path)
+        rc = lib().lasp_eval_model(self.ctx, B, _ptr(params), _ptr(cont), C.byref(opts), _ptr(model), self._stream())
         self._check(rc, "lasp_eval_model")
         return model
 
-    def eval_grad(self, flux, ivar, mask, params):
+    def eval_grad(self, flux, ivar, mask, params, variant=0, emulator_path=0):
         t = self.torch
         flux = self._dev(flux, t.float32); ivar = self._dev(ivar, t.float32)
         mask = self._dev(mask, t.uint8); params = self._dev(params, t.float32)
@@ -231,7 +257,8 @@ class LaspModel:
         grad = t.empty((B, self.NP), device=self.device, dtype=t.float32)
         cont = t.empty((B, self.nc), device=self.device, dtype=t.float32)
         status = t.empty(B, device=self.device, dtype=t.int32)
-        rc = lib().lasp_eval_grad(self.ctx, B, _ptr(flux), _ptr(ivar), _ptr(mask), _ptr(params), _ptr(chi2),
-                                  _ptr(grad), _ptr(cont), _ptr(status), self._stream())
+        opts = self._opts(variant=variant, emulator_path=emulator_path)
+        rc = lib().lasp_eval_grad(self.ctx, B, _ptr(flux), _ptr(ivar), _ptr(mask), _ptr(params), C.byref(opts),
+                                  _ptr(chi2), _ptr(grad), _ptr(cont), _ptr(status), self._stream())
         self._check(rc, "lasp_eval_grad")
         return dict(chi2=chi2, grad_u=grad, cont=cont, status=status)

@@ -1,0 +1,41 @@
+// lasp_common.cuh -- model description as the kernels see it (device-side mirror of lasp_model_desc).
+//
+// Paper / survey references: Eq. n and P:n are /root/reference/PAPER.md; C.2-n are the readings of
+// SURVEY.md 8(c); a0..a9 are the steps of SURVEY.md 8(a).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/lasp_gpu.h"
+
+#define CH 8   // pixels per thread tile (octet); every padded offset below is a multiple of it
+#define FULL 0xffffffffu
+#define LASP_NPMAX (LASP_MAX_LABELS + 2)
+
+struct SegDev {
+    int po;       // first padded pixel of the segment (multiple of CH)
+    int len;      // padded length = halo + roundup(P,CH) + halo
+    int halo;     // replicated-edge columns on each side (multiple of CH, >= largest support H + 18)
+    int P, o;     // real length and real offset
+    int fit_lo, fit_hi;  // octet-aligned padded range containing every pixel that can have w != 0
+    int uniform;  // 1: constant km/s per pixel (log grid) -> one kernel per spectrum per step
+    float inv_s;  // 1/s (pixels per km/s) when uniform, else the LARGEST 1/s_j of the segment
+    float sig_inst;
+    float ta, tb; // Chebyshev node t = ta*(jp - po - halo) + tb, t in [-1,1] over the fitted pixels
+};
+
+struct ModelDev {
+    int n_seg, L, K, NP, D, n1, nmom, Ppad, P, nc;
+    SegDev seg[LASP_MAX_SEG];
+    const uint8_t *exps;   // [K][L]
+    const double *conv;    // [n_seg][n1][n1] internal Chebyshev(t) -> plain Legendre(x^) (C.2-8)
+    float lo[LASP_NPMAX], hi[LASP_NPMAX];
+    float emu_a[LASP_MAX_LABELS], emu_b[LASP_MAX_LABELS];
+    uint8_t label_log10[LASP_MAX_LABELS];
+};
+
+// a1: emulator input x_l = a_l tau_l(theta_l) + b_l (Eq. 1, C.2-19)
+__device__ __forceinline__ float label_x(const ModelDev &M, int l, float theta)
+{
+    return M.emu_a[l] * (M.label_log10[l] ? log10f(theta) : theta) + M.emu_b[l];
+}

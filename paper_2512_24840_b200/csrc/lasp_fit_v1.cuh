@@ -11,10 +11,17 @@
 // transpose over warp shuffles (32 values x 32 lanes in 31 shuffles) and one shared-memory slot per
 // warp; the continuum system is solved by one warp per spectrum (lanes = rows).
 //
+// Two variants of every kernel (template parameter STREAM):
+//   resident  (STREAM = false): rows T and A of the whole longest segment stay in shared memory;
+//   streaming (STREAM = true) : for spectra too long for that.  Rows T and A live in per-CTA global scratch
+//       (L2-resident); each sweep of the CTA over nt*8 pixels first copies the window [jb - guard, jb + nt*8 + guard)
+//       of the row the stencil needs into ONE shared-memory window buffer (coalesced 128-bit loads, halo re-read),
+//       everything that touches only the thread's own octet goes to the global rows directly.
+//
 // Citations: Eq. n and P:n are /root/reference/PAPER.md; C.2-n the readings of SURVEY.md 8()
 // (restated in DESIGN.md); a0..a9 the steps of SURVEY.md 8(a).
 #pragma once
-#include "lasp_device.cuh"
+#include "lasp_common.cuh"
 
 // All shared memory is addressed from this symbol so that the compiler emits LDS/STS (a pointer carried
 // in a struct is generic and costs LD/ST with global-memory scoreboarding).
@@ -36,12 +43,11 @@ struct V1Lay {
     int n1r, nmomr, VR;     // n1 rounded to 4; moments rounded; reduction slots per warp (x GS)
     int NW;                 // warps per CTA
     int Hm;                 // support clamp (memory safety outside the prior box)
-    int fdfresh;            // 1: re-factor in every finite-difference evaluation of the error estimate (LASP_FD_FRESH)
     int fastw;              // 1: v1_update_fast also prepares the next step's kernel weights (one uniform segment)
     int fastupd;            // 1: v1_update_fast applies (L <= 4, K + 2 <= 32, NW <= 12)
     int lfseg;              // 1: one factor slot per segment (0: one slot, re-factored every step when n_seg > 1)
-    int warm;               // the first `warm` steps always re-factor
-    int refresh;            // re-accumulate the Gram moments and re-factor every `refresh` steps
+    int nt8;                // pixels per sweep of the CTA (threads x 8): the streaming window holds nt8 + 2 GUARD
+    int SL;                 // longest padded segment: row length of the per-pixel-kernel scratch planes
     // shared-memory offsets (floats)
     int oT, oA, oU, oM, oV, oX, oPHI, oGW, oGR, oTAP, oMOM, oRHS, oB, oRED, oLF, oQ, oSC, oEXP, oXP, oDPHI, oGSC, oEW, oNP, total;
     int emax;               // largest exponent of the monomial table
@@ -59,14 +65,23 @@ struct V1Args {
     float lr, b1, b2, eps, fd_h;
     float *params, *cont, *chi2, *err;
     int *status;
-    const float *gparams;  // lasp_eval_grad
+    const float *gparams;  // lasp_eval_grad, lasp_eval_model: physical parameters [B][NP]
     float *grad_u;
+    const float *mcont;    // lasp_eval_model: plain-Legendre continuum coefficients [B][nc]
+    float *model;          // lasp_eval_model: output [B][P]
+    float *TG, *AG;        // streaming variant: per-CTA global rows [cta][GS][Ppad] of T and of S / a
+    // Gram re-factorisation policy (lasp_fit_opts.refresh / .warm / .fd_fresh)
+    int warm;              // the first `warm` steps always re-factor
+    int refresh;           // >= 1: re-factor every `refresh`-th step;  0: adaptive (drift monitor, at most every 64th)
+    int fdfresh;           // 1: re-factor in every finite-difference evaluation of the error estimate
+    float drift_tol;       // adaptive: re-factor when (sum of |du|_inf since the last factor) x |du|_inf exceeds this
     unsigned long long *dbg;   // optional per-phase cycle counters (LASP_TIMING=1), else null
     // per-pixel broadening kernels (linear grids, C.2-14): 1/s_j and s_j^2 with V1_TPAD replicated entries on
     // both sides, and per-CTA scratch [3][GS][Ppad] for dS/dv, dS/dsigma*, 1/E0 (thread-private pixels)
     const float *IS, *S2;
     float *DS;
     unsigned int *queue;   // work-queue counter for the fit kernel (zeroed before the launch), may be null
+    unsigned long long *stats;   // [0] += Adam group-steps, [1] += those with a fresh Gram factor (may be null)
     const float4 *CF;      // coefficient table as tf32 [hi|lo] MMA fragments (null: FP32-pipe emulator)
     int ksteps;            // k-steps of 8 terms in CF (<= 16)
 };
@@ -84,7 +99,7 @@ struct V1Np {          // per-spectrum scalars of a per-pixel-kernel segment
 #define SLOT_STAT(L_) ((L_).VR - 6)   // chi2, ngood, min c, dchi2/dv and dchi2/dsigma* of per-pixel-kernel segments
 
 // per-spectrum scalars in shared memory: SC[idx][GS]
-enum { SC_V = 0, SC_SIG, SC_CHI, SC_NGOOD, SC_CMIN, SC_GV, SC_GS, SC_FAIL, SC_N };
+enum { SC_V = 0, SC_SIG, SC_CHI, SC_NGOOD, SC_CMIN, SC_GV, SC_GS, SC_FAIL, SC_DU, SC_N };   // SC_DU: |du|_inf of the last Adam update
 
 // 32 values per lane -> lane l returns the warp total of value l (31 shuffles)
 __device__ __forceinline__ float xreduce32(float (&x)[32], int lane)
@@ -120,7 +135,13 @@ struct V1Block {
     long long spec[GS];   // clamped spectrum indices of the group
     float *cp;            // this CTA's c_prev scratch
     float *ds;            // this CTA's dS/dv, dS/dsigma*, 1/E0 scratch (per-pixel-kernel segments)
+    float *tg, *ag;       // streaming variant: this CTA's global rows of T and of S / a, [GS][Ppad]
     int next;             // next group of this CTA (dynamic work queue)
+    // re-factorisation monitor: read and written by thread 0 only, which publishes its decision in `momflag`
+    float drift;          // sum of |du|_inf over the steps since the last fresh Gram factor
+    int since;            // steps since the last fresh Gram factor
+    int momflag;          // this evaluation re-factorises (written after its first barrier, read after its second)
+    unsigned int nfresh;  // fresh Adam steps of the current group (statistics)
 };
 __shared__ V1Block v1_blk;
 #define V1_TID ((int)threadIdx.x)
@@ -332,10 +353,59 @@ __device__ __forceinline__ void v1_stencil_octet(const float4 *__restrict__ row4
     }
 }
 
-// shared-memory row of spectrum g in buffer `off`, as a float pointer indexed by padded pixel jp
-__device__ __forceinline__ float *v1_row(int off, const SegDev &sg, int g)
+// shared-memory row 0 of buffer `off` as a float pointer indexed by padded pixel jp (row g is + g * RL); `org` is the
+// first padded pixel of the segment (resident rows) or of the sweep (streaming window)
+__device__ __forceinline__ float *v1_rowp(int off, int org)
 {
-    return V1SM + off + g * v1_blk.L.RL + v1_blk.L.GUARD - sg.po;
+    return V1SM + off + v1_blk.L.GUARD - org;
+}
+
+// streaming variant: copy padded pixels [jb - GUARD, jb + nt8 + GUARD) of the GS global rows `src` ([GS][Ppad], plain
+// layout) into the window buffer with the SW4 addressing of the resident rows: 128-bit coalesced loads, the halo of
+// 2 GUARD pixels is re-read by the neighbouring sweep.  Pixels outside [0, Ppad) read as zero.  Callers bracket it
+// with __syncthreads (the rows were written by other threads of this CTA; __ldcg reads them at L2).
+__device__ __forceinline__ void v1_window_load(const float *__restrict__ src, int jb)
+{
+    const int G = v1_blk.L.GUARD, RL = v1_blk.L.RL, P4 = v1_blk.M.Ppad >> 2;
+    const int n4 = (v1_blk.L.nt8 + 2 * G) >> 2, q0 = (jb - G) >> 2;
+#pragma unroll 1
+    for (int g = 0; g < GS; ++g) {
+        float4 *row4 = (float4 *)(V1SM + v1_blk.L.oT + g * RL + G - jb);
+        const float4 *s4 = (const float4 *)(src + (size_t)g * v1_blk.M.Ppad);
+        for (int i = V1_TID; i < n4; i += V1_NT) {
+            const int q = q0 + i;
+            float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (q >= 0 && q < P4) v = __ldcg(s4 + q);
+            row4[SW4(q)] = v;
+        }
+    }
+}
+
+// own-octet access to a row: shared memory (resident) or the CTA's global row (streaming), two float4
+template <bool STREAM>
+__device__ __forceinline__ void v1_oct_load(const float *rowsm, const float *rowgl, int g, int j0, float (&x)[OCT])
+{
+    float4 a, b;
+    if (STREAM) {
+        const float4 *p = (const float4 *)(rowgl + (size_t)g * v1_blk.M.Ppad + j0);
+        a = __ldcg(p); b = __ldcg(p + 1);
+    } else {
+        const float4 *p = (const float4 *)(rowsm + g * v1_blk.L.RL);
+        a = p[SW4(j0 >> 2)]; b = p[SW4((j0 >> 2) + 1)];
+    }
+    x[0] = a.x; x[1] = a.y; x[2] = a.z; x[3] = a.w; x[4] = b.x; x[5] = b.y; x[6] = b.z; x[7] = b.w;
+}
+template <bool STREAM>
+__device__ __forceinline__ void v1_oct_store(float *rowsm, float *rowgl, int g, int j0, const float (&x)[OCT])
+{
+    const float4 a = make_float4(x[0], x[1], x[2], x[3]), b = make_float4(x[4], x[5], x[6], x[7]);
+    if (STREAM) {
+        float4 *p = (float4 *)(rowgl + (size_t)g * v1_blk.M.Ppad + j0);
+        p[0] = a; p[1] = b;
+    } else {
+        float4 *p = (float4 *)(rowsm + g * v1_blk.L.RL);
+        p[SW4(j0 >> 2)] = a; p[SW4((j0 >> 2) + 1)] = b;
+    }
 }
 
 // ------------------------------------------------------------------------------------------
@@ -469,6 +539,7 @@ __device__ __forceinline__ void v1_group_range(const SegDev &sg, int &lo, int &h
 // ------------------------------------------------------------------------------------------
 // a2: T_j = sum_k phi_k C[k,j] over the padded range [lo,hi) -> shared row T (Eq. 1)
 // ------------------------------------------------------------------------------------------
+template <bool STREAM>
 __device__ __noinline__ void v1_phase_emulator(const SegDev &sg, int lo, int hi)
 {
     // everything the loop needs is copied to registers first: the model lives in shared memory, and after
@@ -476,8 +547,8 @@ __device__ __noinline__ void v1_phase_emulator(const SegDev &sg, int lo, int hi)
     const float4 *phi4 = (const float4 *)(V1SM + v1_blk.L.oPHI);
     const int P4 = v1_blk.M.Ppad >> 2, P8 = v1_blk.M.Ppad >> 3, Kq = v1_blk.L.Kq, nt8 = V1_NT * OCT;
     const float *Cg = v1_blk.A.C1;
-    float *rowT = V1SM + v1_blk.L.oT + v1_blk.L.GUARD - sg.po;
-    const int RL = v1_blk.L.RL;
+    float *rowT = v1_rowp(v1_blk.L.oT, sg.po);
+    float *tg = v1_blk.tg;
     for (int j0 = lo + V1_TID * OCT; j0 < hi; j0 += nt8) {
         float acc[GS][OCT];
 #pragma unroll
@@ -525,12 +596,7 @@ __device__ __noinline__ void v1_phase_emulator(const SegDev &sg, int lo, int hi)
             mul4(k0 + 8, bufC);
         }
 #pragma unroll
-        for (int g = 0; g < GS; ++g) {
-            float4 *r = (float4 *)(rowT + g * RL);
-            const int q = j0 >> 2;
-            r[SW4(q)] = make_float4(acc[g][0], acc[g][1], acc[g][2], acc[g][3]);
-            r[SW4(q + 1)] = make_float4(acc[g][4], acc[g][5], acc[g][6], acc[g][7]);
-        }
+        for (int g = 0; g < GS; ++g) v1_oct_store<STREAM>(rowT, tg, g, j0, acc[g]);
     }
 }
 
@@ -634,7 +700,7 @@ __device__ __noinline__ void v1_phase_emulator_mma(const SegDev &sg, int lo, int
 // Partial sums over the thread's 8 pixels are reduced over the warp by register transposes and
 // land in this warp's reduction slots.
 // ------------------------------------------------------------------------------------------
-template <bool UNI>
+template <bool UNI, bool STREAM>
 __device__ __noinline__ void v1_phase_forward(const SegDev &sg, bool stencil)
 {
     const V1Args &a = v1_blk.A;
@@ -645,8 +711,9 @@ __device__ __noinline__ void v1_phase_forward(const SegDev &sg, bool stencil)
     const int Ppad = v1_blk.M.Ppad, P8 = Ppad >> 3, RL = L.RL, NA = L.NA, n1r = L.n1r, nmomr = L.nmomr, nt8 = V1_NT * OCT;
     const int fit_lo = sg.fit_lo, fit_hi = sg.fit_hi, torg = sg.po + sg.halo;
     const float ta = sg.ta, tb = sg.tb;
-    float *rowA = V1SM + L.oA + L.GUARD - sg.po;
-    const float *rowT = V1SM + L.oT + L.GUARD - sg.po;
+    float *rowA = v1_rowp(L.oA, sg.po);
+    const float *rowT = v1_rowp(L.oT, sg.po);
+    float *ag = v1_blk.ag;
     const float4 *gw4 = (const float4 *)(V1SM + L.oGW);
     const float *Yg = a.Y, *Wg = a.W;
     const float *cpg = v1_blk.cp;
@@ -661,6 +728,12 @@ __device__ __noinline__ void v1_phase_forward(const SegDev &sg, bool stencil)
     for (int jb = fit_lo; jb < fit_hi; jb += nt8, first = false) {   // uniform trip count
         const int j0 = jb + V1_TID * OCT;
         const bool act = j0 < fit_hi;
+        if (STREAM && stencil) {   // this sweep's window of T (written to the global rows by the emulator phase)
+            __syncthreads();
+            v1_window_load(v1_blk.tg, jb);
+            __syncthreads();
+            rowT = v1_rowp(L.oT, jb);
+        }
         if (!uniform && stencil && act) {
             // per-pixel kernels: a pass of its own (it needs most of the register file): S -> row A, and its two
             // kernel-parameter derivatives and 1/E0 -> thread-private scratch
@@ -675,15 +748,15 @@ __device__ __noinline__ void v1_phase_forward(const SegDev &sg, bool stencil)
                 float Sg[OCT], DV[OCT], DG[OCT], EI[OCT];
                 const V1Np np = ((const V1Np *)(V1SM + L.oNP))[g];
                 v1_np_forward_octet((const float4 *)(rowT + g * RL), j0, np, isv, s2v, Sg, DV, DG, EI);
-                float4 *ra = (float4 *)(rowA + g * RL);
-                ra[SW4(j0 >> 2)] = make_float4(Sg[0], Sg[1], Sg[2], Sg[3]);
-                ra[SW4((j0 >> 2) + 1)] = make_float4(Sg[4], Sg[5], Sg[6], Sg[7]);
-                float4 *d4 = (float4 *)(dsg + g * Ppad + (j0 >> 1));
-                d4[0] = make_float4(DV[0], DV[1], DV[2], DV[3]); d4[P8] = make_float4(DV[4], DV[5], DV[6], DV[7]);
-                d4 += GS * (Ppad >> 2);
-                d4[0] = make_float4(DG[0], DG[1], DG[2], DG[3]); d4[P8] = make_float4(DG[4], DG[5], DG[6], DG[7]);
-                d4 += GS * (Ppad >> 2);
-                d4[0] = make_float4(EI[0], EI[1], EI[2], EI[3]); d4[P8] = make_float4(EI[4], EI[5], EI[6], EI[7]);
+                v1_oct_store<STREAM>(rowA, ag, g, j0, Sg);
+                // scratch planes [3][GS][SL], segment-relative, split-octet (thread-private pixels, L2-resident)
+                float4 *d4 = (float4 *)(dsg + g * L.SL + ((j0 - sg.po) >> 1));
+                const int S8 = L.SL >> 3, SP = GS * (L.SL >> 2);
+                d4[0] = make_float4(DV[0], DV[1], DV[2], DV[3]); d4[S8] = make_float4(DV[4], DV[5], DV[6], DV[7]);
+                d4 += SP;
+                d4[0] = make_float4(DG[0], DG[1], DG[2], DG[3]); d4[S8] = make_float4(DG[4], DG[5], DG[6], DG[7]);
+                d4 += SP;
+                d4[0] = make_float4(EI[0], EI[1], EI[2], EI[3]); d4[S8] = make_float4(EI[4], EI[5], EI[6], EI[7]);
             }
         }
         float v[GS][OCT];
@@ -697,17 +770,11 @@ __device__ __noinline__ void v1_phase_forward(const SegDev &sg, bool stencil)
                 const float4 *cp4 = (const float4 *)(cpg + g * Ppad + (j0 >> 1));
                 const float4 c0 = __ldcg(cp4), c1 = __ldcg(cp4 + P8);
                 float S[1][OCT];
-                float4 *ra = (float4 *)(rowA + g * RL);
-                const int q0 = SW4(j0 >> 2), q1 = SW4((j0 >> 2) + 1);
                 if (stencil && uniform) {
                     v1_stencil_octet<1>((const float4 *)(rowT + g * RL), j0, alo[g], nag[g], gw4 + g * NA, 0, S);
-                    ra[q0] = make_float4(S[0][0], S[0][1], S[0][2], S[0][3]);
-                    ra[q1] = make_float4(S[0][4], S[0][5], S[0][6], S[0][7]);
-                } else {
-                    const float4 s0 = ra[q0], s1 = ra[q1];
-                    S[0][0] = s0.x; S[0][1] = s0.y; S[0][2] = s0.z; S[0][3] = s0.w;
-                    S[0][4] = s1.x; S[0][5] = s1.y; S[0][6] = s1.z; S[0][7] = s1.w;
-                }
+                    v1_oct_store<STREAM>(rowA, ag, g, j0, S[0]);
+                } else
+                    v1_oct_load<STREAM>(rowA, ag, g, j0, S[0]);
                 const float yy[OCT] = {y0.x, y0.y, y0.z, y0.w, y1.x, y1.y, y1.z, y1.w};
                 const float ww[OCT] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
                 const float cc[OCT] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w};
@@ -755,6 +822,7 @@ __device__ __noinline__ void v1_phase_forward(const SegDev &sg, bool stencil)
 // a5, refresh steps only: Gram moments  mom_n = sum_j u_j T_n(t_j), u = w S^2, n < 2D+1  (S is in row A, w comes
 // from L2 again).  Kept apart from v1_phase_forward so that the every-step code stays small.
 // ------------------------------------------------------------------------------------------
+template <bool STREAM>
 __device__ __noinline__ void v1_phase_moments(const SegDev &sg)
 {
     const V1Lay &L = v1_blk.L;
@@ -762,7 +830,8 @@ __device__ __noinline__ void v1_phase_moments(const SegDev &sg)
     const int Ppad = v1_blk.M.Ppad, P8 = Ppad >> 3, RL = L.RL, nmomr = L.nmomr, nt8 = V1_NT * OCT;
     const int fit_lo = sg.fit_lo, fit_hi = sg.fit_hi, torg = sg.po + sg.halo;
     const float ta = sg.ta, tb = sg.tb;
-    const float *rowA = V1SM + L.oA + L.GUARD - sg.po;
+    const float *rowA = v1_rowp(L.oA, sg.po);
+    const float *ag = v1_blk.ag;
     const float *Wg = v1_blk.A.W;
     bool first = true;
     for (int jb = fit_lo; jb < fit_hi; jb += nt8, first = false) {
@@ -776,10 +845,9 @@ __device__ __noinline__ void v1_phase_moments(const SegDev &sg)
             if (act) {
                 const size_t ro = (size_t)v1_blk.spec[g] * Ppad + (j0 >> 1);
                 const float4 w0 = __ldg((const float4 *)(Wg + ro)), w1 = __ldg((const float4 *)(Wg + ro) + P8);
-                const float4 *ra = (const float4 *)(rowA + g * RL);
-                const float4 s0 = ra[SW4(j0 >> 2)], s1 = ra[SW4((j0 >> 2) + 1)];
+                float SS[OCT];
+                v1_oct_load<STREAM>(rowA, ag, g, j0, SS);
                 const float ww[OCT] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
-                const float SS[OCT] = {s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w};
 #pragma unroll
                 for (int i = 0; i < OCT; ++i) u[g][i] = ww[i] * SS[i] * SS[i];
             }
@@ -1003,7 +1071,7 @@ __device__ __noinline__ void v1_phase_solve(int g, int seg, bool refactor)
 //           evaluation, so their per-pixel updates and the reduction are left out).
 // chi2 / ngood / cmin are reduced over the warp and accumulated in this warp's SLOT_STAT slots (zeroed by v1_evaluate).
 // ------------------------------------------------------------------------------------------
-template <int MODE, bool UNI>
+template <int MODE, bool UNI, bool STREAM>
 __device__ __noinline__ void v1_phase_residual(const SegDev &sg, int rowB, float *xrow)
 {
     const V1Args &a = v1_blk.A;
@@ -1012,7 +1080,8 @@ __device__ __noinline__ void v1_phase_residual(const SegDev &sg, int rowB, float
     const int Ppad = v1_blk.M.Ppad, P8 = Ppad >> 3, n1 = v1_blk.M.n1, RL = L.RL, nt8 = V1_NT * OCT;
     const int fit_lo = sg.fit_lo, fit_hi = sg.fit_hi, torg = sg.po + sg.halo;
     const float ta = sg.ta, tb = sg.tb;
-    float *rowA = V1SM + L.oA + L.GUARD - sg.po;
+    float *rowA = v1_rowp(L.oA, sg.po);
+    float *ag = v1_blk.ag;
     const float *Yg = a.Y, *Wg = a.W;
     float *cpg = v1_blk.cp;
     size_t rowo[GS];
@@ -1059,11 +1128,9 @@ __device__ __noinline__ void v1_phase_residual(const SegDev &sg, int rowB, float
             cp4[0] = make_float4(cc[g][0], cc[g][1], cc[g][2], cc[g][3]);
             cp4[P8] = make_float4(cc[g][4], cc[g][5], cc[g][6], cc[g][7]);
             if (MODE == 0) continue;
-            float4 *ra = (float4 *)(rowA + g * RL);
-            const int q0 = SW4(j0 >> 2), q1 = SW4((j0 >> 2) + 1);
-            const float4 s0 = ra[q0], s1 = ra[q1];
+            float SS[OCT];
+            v1_oct_load<STREAM>(rowA, ag, g, j0, SS);
             const float4 y0 = yq[g][0], y1 = yq[g][1], w0 = wq[g][0], w1 = wq[g][1];
-            const float SS[OCT] = {s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w};
             const float yy[OCT] = {y0.x, y0.y, y0.z, y0.w, y1.x, y1.y, y1.z, y1.w};
             const float ww[OCT] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
             float av[OCT], rho[OCT];
@@ -1081,10 +1148,11 @@ __device__ __noinline__ void v1_phase_residual(const SegDev &sg, int rowB, float
             if (!uniform) {
                 // per-pixel kernels: the two kernel-parameter gradients close here (dS/dv, dS/dsigma* were kept by the
                 // forward pass), and the adjoint handed to the stencil is a/E0 (each source pixel's own normalisation)
-                const float4 *d4 = (const float4 *)(dsg + g * Ppad + (j0 >> 1));
-                const float4 v0 = __ldcg(d4), v1 = __ldcg(d4 + P8);
-                const float4 g0 = __ldcg(d4 + GS * (Ppad >> 2)), g1 = __ldcg(d4 + GS * (Ppad >> 2) + P8);
-                const float4 e0 = __ldcg(d4 + 2 * GS * (Ppad >> 2)), e1 = __ldcg(d4 + 2 * GS * (Ppad >> 2) + P8);
+                const float4 *d4 = (const float4 *)(dsg + g * L.SL + ((j0 - sg.po) >> 1));
+                const int S8 = L.SL >> 3, SP = GS * (L.SL >> 2);
+                const float4 v0 = __ldcg(d4), v1 = __ldcg(d4 + S8);
+                const float4 g0 = __ldcg(d4 + SP), g1 = __ldcg(d4 + SP + S8);
+                const float4 e0 = __ldcg(d4 + 2 * SP), e1 = __ldcg(d4 + 2 * SP + S8);
                 const float DV[OCT] = {v0.x, v0.y, v0.z, v0.w, v1.x, v1.y, v1.z, v1.w};
                 const float DG[OCT] = {g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, g1.z, g1.w};
                 const float EI[OCT] = {e0.x, e0.y, e0.z, e0.w, e1.x, e1.y, e1.z, e1.w};
@@ -1095,8 +1163,7 @@ __device__ __noinline__ void v1_phase_residual(const SegDev &sg, int rowB, float
                     av[i] *= EI[i];
                 }
             }
-            ra[q0] = make_float4(av[0], av[1], av[2], av[3]);
-            ra[q1] = make_float4(av[4], av[5], av[6], av[7]);
+            v1_oct_store<STREAM>(rowA, ag, g, j0, av);
             if (MODE == 2) {
                 float4 *x4 = (float4 *)(xrow + g * Ppad + j0);
                 x4[0] = make_float4(rho[0], rho[1], rho[2], rho[3]);
@@ -1131,7 +1198,7 @@ __device__ __noinline__ void v1_phase_residual(const SegDev &sg, int rowB, float
 // Partial sums go through register transposes into this warp's Q slots (pseudo-terms K, K+1 carry
 // the two kernel-parameter gradients), which v1_evaluate zeroed.
 // ------------------------------------------------------------------------------------------
-template <bool UNI>
+template <bool UNI, bool STREAM>
 __device__ __noinline__ void v1_phase_adjoint(const SegDev &sg, int lo, int hi)
 {
     const V1Lay &L = v1_blk.L;
@@ -1141,7 +1208,7 @@ __device__ __noinline__ void v1_phase_adjoint(const SegDev &sg, int lo, int hi)
     const int qslot0 = SLOT_Q(L, 0);
     float *red = V1SM + L.oRED + V1_WARP * L.VR * GS;
     const float *Cg = v1_blk.A.C1;
-    const float *rowA = V1SM + L.oA + L.GUARD - sg.po, *rowT = V1SM + L.oT + L.GUARD - sg.po;
+    const float *rowA = v1_rowp(L.oA, sg.po), *rowT = v1_rowp(L.oT, sg.po);
     const float4 *gr4 = (const float4 *)(V1SM + L.oGR);
     int alo[GS], nag[GS];
     constexpr bool uniform = UNI;
@@ -1152,6 +1219,12 @@ __device__ __noinline__ void v1_phase_adjoint(const SegDev &sg, int lo, int hi)
     for (int jb = lo; jb < hi; jb += nt8) {
         const int j0 = jb + V1_TID * OCT;
         const bool act = j0 < hi;
+        if (STREAM) {   // this sweep's window of the adjoint a (global rows, written by the residual phase)
+            __syncthreads();
+            v1_window_load(v1_blk.ag, jb);
+            __syncthreads();
+            rowA = v1_rowp(L.oA, jb);
+        }
         float t[GS][OCT], gv[GS], gs[GS];
 #pragma unroll
         for (int g = 0; g < GS; ++g) {
@@ -1165,9 +1238,8 @@ __device__ __noinline__ void v1_phase_adjoint(const SegDev &sg, int lo, int hi)
             } else if (act) {
                 float acc[3][OCT];
                 v1_stencil_octet<3>((const float4 *)(rowA + g * RL), j0, alo[g], nag[g], gr4 + g * NA, wstride4, acc);
-                const float4 *rt = (const float4 *)(rowT + g * RL);
-                const float4 t0 = rt[SW4(j0 >> 2)], t1 = rt[SW4((j0 >> 2) + 1)];
-                const float TT[OCT] = {t0.x, t0.y, t0.z, t0.w, t1.x, t1.y, t1.z, t1.w};
+                float TT[OCT];
+                v1_oct_load<STREAM>(rowT, v1_blk.tg, g, j0, TT);
 #pragma unroll
                 for (int i = 0; i < OCT; ++i) {
                     t[g][i] = acc[0][i];
@@ -1231,13 +1303,17 @@ __device__ __noinline__ void v1_phase_adjoint(const SegDev &sg, int lo, int hi)
 // One evaluation of chi2 (+ gradient) at the u held in shared memory (warps g < GS have run
 // v1_param_setup for their spectrum).  All threads of the CTA call this.
 //   cold: b = 0, c_prev = 0, solve twice (solve + one refinement);  else b, c_prev are warm.
-//   mom : re-accumulate the Gram moments and re-factor (always true when cold).
+//   momsel: 1 = re-accumulate the Gram moments and re-factor (always when cold); 0 = reuse the stale factor;
+//           2 = adaptive: decided by thread 0 after the first barrier from the drift monitor (DESIGN.md "Stale Gram
+//               factor") and read by all after the second: fresh when a segment's system was flagged not positive
+//               definite, when 64 steps have passed, or when (sum of |du|_inf since the last fresh factor) x
+//               (|du|_inf of the last update) > drift_tol.  `adam` marks the evaluations of the Adam loop (statistics).
 //   MODE 0: chi2 + gradient partials (Q slots) ; MODE 1: chi2 only ; MODE 2: chi2 + rho -> xrow.
 // On return (after the closing barrier) the per-warp reduction slots hold chi2 / ngood / min c (not with `stats`
 // false on uniform segments: the Adam steps do not read them) and, for MODE 0, the q / dv / dsigma partials.
 // ------------------------------------------------------------------------------------------
-template <int MODE>
-__device__ __noinline__ void v1_evaluate(bool cold, bool mom, float *xrow, bool wready = false, bool stats = true)
+template <int MODE, bool STREAM>
+__device__ __noinline__ void v1_evaluate(bool cold, int momsel, float *xrow, bool wready = false, bool stats = true, bool adam = false)
 {
     const V1Args &a = v1_blk.A;
     const ModelDev &M = v1_blk.M;
@@ -1253,7 +1329,8 @@ __device__ __noinline__ void v1_evaluate(bool cold, bool mom, float *xrow, bool 
 #else
     auto tick = [](int) {};   // per-phase cycle counters: build with -DLASP_PHASE_TIMING
 #endif
-    if (M.n_seg > 1 && !L.lfseg) mom = true;   // one factor slot shared by the segments: never stale
+    if (M.n_seg > 1 && !L.lfseg) momsel = 1;   // one factor slot shared by the segments: never stale
+    bool mom = momsel == 1;
     bool zeroed = false;
     auto zero_slots = [&]() {
         float *red = V1SM + L.oRED + V1_WARP * L.VR * GS;
@@ -1278,7 +1355,11 @@ __device__ __noinline__ void v1_evaluate(bool cold, bool mom, float *xrow, bool 
             if (!wready) v1_setup_weights(sg, V1_WARP);   // else v1_update_fast has left them in place
             if (cold) for (int n = V1_LANE; n < M.n1; n += 32) SMV(L.oB, rowB + n, V1_WARP) = 0.f;
         }
-        if (M.n_seg > 1 || cold) {
+        if (STREAM) {
+            // the global rows are indexed by absolute padded pixel: a stays zero outside the fitted ranges once cleared
+            if (cold && s == 0)
+                for (int i = V1_TID; i < GS * M.Ppad / 4; i += V1_NT) ((float4 *)v1_blk.ag)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        } else if (M.n_seg > 1 || cold) {
             // row A must be zero outside the fitted range of THIS segment (the adjoint stencil reads it)
             for (int i = V1_TID; i < GS * L.RL / 4; i += V1_NT) ((float4 *)(V1SM + L.oA))[i] = make_float4(0.f, 0.f, 0.f, 0.f);
         }
@@ -1289,21 +1370,41 @@ __device__ __noinline__ void v1_evaluate(bool cold, bool mom, float *xrow, bool 
         tick(0);
         __syncthreads();
         tick(1);
-        if (!zeroed) zero_slots();
+        if (!zeroed) {
+            zero_slots();
+            if (V1_TID == 0 && adam) {   // Gram re-factorisation decision from what the update warps left before the barrier
+                bool fresh = momsel == 1;
+                if (momsel == 2) {
+                    float step = 0.f;
+                    bool fail = false;
+#pragma unroll
+                    for (int g = 0; g < GS; ++g) {
+                        step = fmaxf(step, SMV(L.oSC, SC_DU, g));
+                        for (int q = 0; q < M.n_seg; ++q) fail = fail || SMV(L.oSC, SC_N + q, g) != 0.f;
+                    }
+                    v1_blk.drift += step;
+                    v1_blk.since += 1;
+                    fresh = fail || v1_blk.since >= 64 || v1_blk.drift * step > a.drift_tol;
+                }
+                if (fresh) { v1_blk.drift = 0.f; v1_blk.since = 0; v1_blk.nfresh += 1; }
+                v1_blk.momflag = fresh ? 1 : 0;
+            }
+        }
         int lo, hi;
         v1_group_range(sg, lo, hi);
-        if (v1_blk.A.CF) {
+        if (!STREAM && v1_blk.A.CF) {
             const int ks = v1_blk.A.ksteps;
             if (ks <= 4) v1_phase_emulator_mma<1>(sg, lo, hi);
             else if (ks <= 8) v1_phase_emulator_mma<2>(sg, lo, hi);
             else v1_phase_emulator_mma<4>(sg, lo, hi);
         } else
-            v1_phase_emulator(sg, lo, hi);
+            v1_phase_emulator<STREAM>(sg, lo, hi);
         tick(2);
         __syncthreads();
         tick(3);
-        if (sg.uniform) v1_phase_forward<true>(sg, true); else v1_phase_forward<false>(sg, true);
-        if (mom || cold) v1_phase_moments(sg);   // own octets of row A only: no barrier needed in between
+        if (momsel == 2) mom = v1_blk.momflag != 0;
+        if (sg.uniform) v1_phase_forward<true, STREAM>(sg, true); else v1_phase_forward<false, STREAM>(sg, true);
+        if (mom || cold) v1_phase_moments<STREAM>(sg);   // own octets of row A only: no barrier needed in between
         tick(4);
         __syncthreads();
         tick(5);
@@ -1312,21 +1413,21 @@ __device__ __noinline__ void v1_evaluate(bool cold, bool mom, float *xrow, bool 
         __syncthreads();
         tick(7);
         if (cold) {
-            v1_phase_residual<0, true>(sg, rowB, nullptr);
+            v1_phase_residual<0, true, STREAM>(sg, rowB, nullptr);
             __syncthreads();   // c_prev written by this thread only, but keep phases aligned
-            v1_phase_forward<true>(sg, false);   // S is re-read from row A: no stencil, either kind
+            v1_phase_forward<true, STREAM>(sg, false);   // S is re-read from row A: no stencil, either kind
             __syncthreads();
             if (V1_WARP < GS) v1_phase_solve(V1_WARP, s, false);
             __syncthreads();
         }
-        if (MODE == 0 && !stats && sg.uniform) v1_phase_residual<3, true>(sg, rowB, xrow);   // Adam step: no statistics
-        else if (sg.uniform) v1_phase_residual<(MODE == 2 ? 2 : 1), true>(sg, rowB, xrow);
-        else v1_phase_residual<(MODE == 2 ? 2 : 1), false>(sg, rowB, xrow);
+        if (MODE == 0 && !stats && sg.uniform) v1_phase_residual<3, true, STREAM>(sg, rowB, xrow);   // Adam step: no statistics
+        else if (sg.uniform) v1_phase_residual<(MODE == 2 ? 2 : 1), true, STREAM>(sg, rowB, xrow);
+        else v1_phase_residual<(MODE == 2 ? 2 : 1), false, STREAM>(sg, rowB, xrow);
         tick(8);
         __syncthreads();
         tick(9);
         if (MODE == 0) {
-            if (sg.uniform) v1_phase_adjoint<true>(sg, lo, hi); else v1_phase_adjoint<false>(sg, lo, hi);
+            if (sg.uniform) v1_phase_adjoint<true, STREAM>(sg, lo, hi); else v1_phase_adjoint<false, STREAM>(sg, lo, hi);
             tick(10);
             __syncthreads();
             tick(11);
@@ -1453,8 +1554,13 @@ __device__ __noinline__ void v1_update_fast(int g, float ib1, float ib2)
     const float vv = b2 * v0 + (1.f - b2) * gr * gr;
     const float mh = mm * ib1, vh = vv * ib2;
     float u = u0 - __fdividef(lr * mh, sqrtf(vh) + eps);
-    if (!(u == u)) u = u0;                                  // keep the iterate if the gradient was NaN
-    u = fminf(fmaxf(u, -1.f), 1.f);
+    u = u < -1.f ? -1.f : (u > 1.f ? 1.f : u);              // clip (C.2-18); a NaN iterate stays NaN, as in the oracle
+    {   // |du|_inf of this update, for the re-factorisation monitor (NaN does not count)
+        float du = lane < NP ? fabsf(u - u0) : 0.f;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) du = fmaxf(du, __shfl_xor_sync(FULL, du, o));
+        if (lane == 0) SMV(L.oSC, SC_DU, g) = du;
+    }
     // ---- a1: de-normalise, emulator inputs (C.2-18/19)
     const float half = (hi - lo) * 0.5f;
     const float th = lo + (u + 1.f) * half;
@@ -1526,8 +1632,11 @@ __device__ __forceinline__ void v1_init_block(const ModelDev &M, const V1Lay &L,
     for (int i = threadIdx.x; i < (int)(sizeof(V1Lay) / 4); i += blockDim.x) ((int *)&v1_blk.L)[i] = ((const int *)&L)[i];
     for (int i = threadIdx.x; i < (int)(sizeof(V1Args) / 4); i += blockDim.x) ((int *)&v1_blk.A)[i] = ((const int *)&a)[i];
     if (threadIdx.x == 0) {
-        v1_blk.cp = a.CP + (size_t)blockIdx.x * GS * M.Ppad;
-        v1_blk.ds = a.DS ? a.DS + (size_t)blockIdx.x * 3 * GS * M.Ppad : nullptr;
+        v1_blk.cp = a.CP ? a.CP + (size_t)blockIdx.x * GS * M.Ppad : nullptr;
+        v1_blk.ds = a.DS ? a.DS + (size_t)blockIdx.x * 3 * GS * L.SL : nullptr;
+        v1_blk.tg = a.TG ? a.TG + (size_t)blockIdx.x * GS * M.Ppad : nullptr;
+        v1_blk.ag = a.AG ? a.AG + (size_t)blockIdx.x * GS * M.Ppad : nullptr;
+        v1_blk.drift = 0.f; v1_blk.since = 0; v1_blk.momflag = 0; v1_blk.nfresh = 0;
     }
     if (M.L <= 4) {   // one word per term (v1_param_setup)
         for (int k = threadIdx.x; k < M.K; k += blockDim.x) {
@@ -1539,7 +1648,13 @@ __device__ __forceinline__ void v1_init_block(const ModelDev &M, const V1Lay &L,
         for (int i = threadIdx.x; i < M.K * M.L; i += blockDim.x) ((uint8_t *)(V1SM + L.oEXP))[i] = M.exps[i];
     for (int i = threadIdx.x; i < GS * L.Kq; i += blockDim.x) V1SM[L.oPHI + i] = 0.f;   // phi is zero past K
     // rows T and A: zero-weight taps multiply whatever lies in the window, so it must at least be finite
-    for (int i = threadIdx.x; i < 2 * GS * L.RL; i += blockDim.x) V1SM[L.oT + i] = 0.f;
+    // (streaming: one window buffer, oA == oT, and the global rows, which may hold another launch's values)
+    for (int i = threadIdx.x; i < (L.oA == L.oT ? 1 : 2) * GS * L.RL; i += blockDim.x) V1SM[L.oT + i] = 0.f;
+    if (a.TG) {
+        float *tg = a.TG + (size_t)blockIdx.x * GS * M.Ppad, *ag = a.AG + (size_t)blockIdx.x * GS * M.Ppad;
+        for (int i = threadIdx.x; i < GS * M.Ppad; i += blockDim.x) { tg[i] = 0.f; ag[i] = 0.f; }
+    }
+    for (int i = threadIdx.x; i < GS * (SC_N + M.n_seg); i += blockDim.x) V1SM[L.oSC + i] = 0.f;
     __syncthreads();
 }
 
@@ -1548,11 +1663,16 @@ __device__ __forceinline__ void v1_set_group(int grp)
     if (threadIdx.x < GS) {
         const long long i = (long long)grp * GS + threadIdx.x;
         v1_blk.spec[threadIdx.x] = i < v1_blk.A.B ? i : v1_blk.A.B - 1;
+        SMV(v1_blk.L.oSC, SC_DU, threadIdx.x) = 0.f;
+    }
+    if (threadIdx.x == 0) {
+        v1_blk.drift = 0.f; v1_blk.since = 0; v1_blk.momflag = 0; v1_blk.nfresh = 0;
     }
 }
 
 // a9: error estimate (C.2-22/23).  J by central differences of the re-solved whitened
 // residual rho(u), Sigma = rho^T rho/(N_good - NP) (J^T J)^-1, err_p = sqrt(Sigma_pp) (hi_p - lo_p)/2.
+template <bool STREAM>
 __device__ __noinline__ void v1_errors(float chi2_g, float ngood_g, bool valid_g)
 {
     const V1Args &a = v1_blk.A;
@@ -1573,13 +1693,13 @@ __device__ __noinline__ void v1_errors(float chi2_g, float ngood_g, bool valid_g
         // The factor of the final evaluation serves all 2 NP perturbed ones: a step of fd_h changes the Gram matrix
         // by a relative ~1e-3, so one refinement from the neighbouring solution leaves that fraction of the
         // continuum's response, far inside the 1e-2 the estimate is held to.
-        v1_evaluate<2>(false, L.fdfresh != 0, xj);
+        v1_evaluate<2, STREAM>(false, a.fdfresh != 0, xj);
         if (V1_WARP < GS) {
             if (V1_LANE == 0) SMV(L.oU, p, V1_WARP) = u0 - a.fd_h;
             __syncwarp();
             v1_param_setup(V1_WARP);
         }
-        v1_evaluate<2>(false, L.fdfresh != 0, xj + (1 + p) * plane);
+        v1_evaluate<2, STREAM>(false, a.fdfresh != 0, xj + (1 + p) * plane);
         if (V1_WARP < GS) {
             if (V1_LANE == 0) SMV(L.oU, p, V1_WARP) = u0;
             __syncwarp();
@@ -1678,7 +1798,7 @@ __device__ __noinline__ void v1_errors(float chi2_g, float ngood_g, bool valid_g
 // ------------------------------------------------------------------------------------------
 // lasp_fit_batch: a1-a9 for groups of GS spectra, persistent CTAs
 // ------------------------------------------------------------------------------------------
-template <int MAXT, int MINB>
+template <int MAXT, int MINB, bool STREAM>
 __global__ void __launch_bounds__(MAXT, MINB)
 lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V1Lay L, const V1Args a)
 {
@@ -1696,8 +1816,7 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
         if (g < GS) {
             for (int p = V1_LANE; p < NP; p += 32) {
                 const float th = a.init[v1_blk.spec[g] * NP + p];
-                const float u = 2.f * (th - M.lo[p]) / (M.hi[p] - M.lo[p]) - 1.f;
-                SMV(L.oU, p, g) = fminf(fmaxf(u, -1.f), 1.f);
+                SMV(L.oU, p, g) = 2.f * (th - M.lo[p]) / (M.hi[p] - M.lo[p]) - 1.f;   // not clipped: clipping follows updates (C.1)
                 SMV(L.oM, p, g) = 0.f;
                 SMV(L.oV, p, g) = 0.f;
             }
@@ -1709,8 +1828,10 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
 #ifdef LASP_PHASE_TIMING
             const long long te0 = a.dbg ? clock64() : 0;
 #endif
-            // fresh Gram factor on each of the first `refresh` steps (the model moves fastest there), then every `refresh`-th
-            v1_evaluate<0>(t == 1, t <= L.warm || (t - 1) % L.refresh == 0, nullptr, t > 1 && L.fastw, false);
+            // fresh Gram factor on each of the first `warm` steps (the model moves fastest there), then every `refresh`-th
+            // step, or (refresh == 0) when the drift monitor asks for it
+            const int momsel = t <= a.warm ? 1 : (a.refresh >= 1 ? ((t - 1) % a.refresh == 0 ? 1 : 0) : 2);
+            v1_evaluate<0, STREAM>(t == 1, momsel, nullptr, t > 1 && L.fastw, false, true);
 #ifdef LASP_PHASE_TIMING
             if (a.dbg && V1_TID == 0) { atomicAdd(a.dbg + 14, (unsigned long long)(clock64() - te0)); atomicAdd(a.dbg + 15, 1ull); }
             const long long tu0 = a.dbg ? clock64() : 0;
@@ -1725,6 +1846,7 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
                     if (a.dbg && V1_TID == 0) atomicAdd(a.dbg + 16, (unsigned long long)(clock64() - tu0));
 #endif
                     // a8: Adam (C.2-20), then clip to the prior box (C.2-18); lane p owns parameter p
+                    float du = 0.f;
                     for (int p0 = 0; p0 < NP; p0 += 32) {   // NP <= 32
                         const int p = p0 + V1_LANE;
                         if (p < NP) {
@@ -1732,11 +1854,16 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
                             const float v = a.b2 * SMV(L.oV, p, g) + (1.f - a.b2) * gr * gr;
                             SMV(L.oM, p, g) = m; SMV(L.oV, p, g) = v;
                             const float mh = m * ib1, vh = v * ib2;
-                            float u = SMV(L.oU, p, g) - __fdividef(a.lr * mh, sqrtf(vh) + a.eps);
-                            if (!(u == u)) u = SMV(L.oU, p, g);   // keep the iterate if the gradient was NaN
-                            SMV(L.oU, p, g) = fminf(fmaxf(u, -1.f), 1.f);
+                            const float u0 = SMV(L.oU, p, g);
+                            float u = u0 - __fdividef(a.lr * mh, sqrtf(vh) + a.eps);
+                            u = u < -1.f ? -1.f : (u > 1.f ? 1.f : u);   // clip (C.2-18); NaN stays NaN, as in the oracle
+                            SMV(L.oU, p, g) = u;
+                            du = fabsf(u - u0);
                         }
                     }
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) du = fmaxf(du, __shfl_xor_sync(FULL, du, o));
+                    if (V1_LANE == 0) SMV(L.oSC, SC_DU, g) = du;   // re-factorisation monitor
                     __syncwarp();
 #ifdef LASP_PHASE_TIMING
                     if (a.dbg && V1_TID == 0) atomicAdd(a.dbg + 17, (unsigned long long)(clock64() - tu0));
@@ -1748,8 +1875,9 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
             if (a.dbg && V1_TID == 0) atomicAdd(a.dbg + 13, (unsigned long long)(clock64() - tu0));
 #endif
         }
+        if (a.stats && V1_TID == 0) { atomicAdd(a.stats, (unsigned long long)a.n_iter); atomicAdd(a.stats + 1, (unsigned long long)v1_blk.nfresh); }
         // a9: one more evaluation at the final iterate (C.2-21)
-        v1_evaluate<1>(a.n_iter == 0, true, nullptr);
+        v1_evaluate<1, STREAM>(a.n_iter == 0, 1, nullptr);
         float chi2 = 0.f, ngood = 0.f, cmin = 0.f;
         if (g < GS) {
             v1_stats(g, chi2, ngood, cmin);
@@ -1780,7 +1908,7 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
                 if (a.cont) v1_write_cont(g, a.cont + i * M.nc);
             }
         }
-        if (a.err) v1_errors(chi2, ngood, valid);
+        if (a.err) v1_errors<STREAM>(chi2, ngood, valid);
         grp = grp_next;
     }
 }
@@ -1788,7 +1916,7 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
 // ------------------------------------------------------------------------------------------
 // lasp_eval_grad: one cold evaluation of chi2 and d chi2/d u at given physical parameters
 // ------------------------------------------------------------------------------------------
-template <int MAXT, int MINB>
+template <int MAXT, int MINB, bool STREAM>
 __global__ void __launch_bounds__(MAXT, MINB)
 lasp_v1_grad_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V1Lay L, const V1Args a)
 {
@@ -1805,7 +1933,7 @@ lasp_v1_grad_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ 
             __syncwarp();
             v1_param_setup(g);
         }
-        v1_evaluate<0>(true, true, nullptr);
+        v1_evaluate<0, STREAM>(true, 1, nullptr);
         if (g < GS) {
             const float gr = v1_gradient(g);
             float chi2, ngood, cmin;
@@ -1820,6 +1948,124 @@ lasp_v1_grad_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ 
                 }
                 if (a.cont) v1_write_cont(g, a.cont + i * M.nc);
             }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// lasp_eval_model: model_j = c_j S_j at given physical parameters and plain-Legendre continuum coefficients, on
+// EVERY pixel of every segment (edge pixels included: there the stencil reads the replicated halo, C.2-16).  S comes
+// from the same emulator, weight and stencil code as the fit (v1_param_setup, v1_setup_weights, v1_phase_emulator,
+// v1_stencil_octet / v1_np_forward_octet); the continuum is evaluated in the paper's own basis, Legendre P_n at the
+// nodes x^_j = -1 + 2 (j - o_s)/P_s, by Bonnet's recurrence shared by the GS spectra.
+// ------------------------------------------------------------------------------------------
+template <bool UNI, bool STREAM>
+__device__ __noinline__ void v1_phase_model(const SegDev &sg, int s, int grp)
+{
+    const V1Args &a = v1_blk.A;
+    const V1Lay &L = v1_blk.L;
+    const int *tap = (const int *)(V1SM + L.oTAP);
+    const int RL = L.RL, NA = L.NA, nt8 = V1_NT * OCT, n1 = v1_blk.M.n1, P = v1_blk.M.P;
+    const int seg_lo = sg.po + sg.halo, seg_hi = seg_lo + (sg.P + OCT - 1) / OCT * OCT;
+    const float *rowT = v1_rowp(L.oT, sg.po);
+    const float4 *gw4 = (const float4 *)(V1SM + L.oGW);
+    const float *bco = V1SM + L.oB + s * n1 * GS;
+    const float *ISg = a.IS + V1_TPAD, *S2g = a.S2 + V1_TPAD;
+    for (int jb = seg_lo; jb < seg_hi; jb += nt8) {   // uniform trip count
+        const int j0 = jb + V1_TID * OCT;
+        if (STREAM) {
+            __syncthreads();
+            v1_window_load(v1_blk.tg, jb);
+            __syncthreads();
+            rowT = v1_rowp(L.oT, jb);
+        }
+        if (j0 >= seg_hi) continue;
+        // The continuum factor is evaluated in fp64: near x^ = +-1 a degree-30 Legendre sum moves by ~n^2/2 per unit of
+        // x^, so an fp32 node (6e-8) alone costs up to ~1e-5 of the flux there (measured 1.2e-5 on config-2 shapes),
+        // the whole tolerance.  S, the part shared with the fit, stays in fp32.
+        float isv[OCT], s2v[OCT];
+        double xx[OCT];
+#pragma unroll
+        for (int i = 0; i < OCT; ++i) {
+            xx[i] = (double)(2 * (j0 + i - seg_lo) - sg.P) / (double)sg.P;
+            if (!UNI) { isv[i] = __ldg(ISg + j0 + i); s2v[i] = __ldg(S2g + j0 + i); }
+        }
+#pragma unroll 1
+        for (int g = 0; g < GS; ++g) {   // one spectrum at a time (an inspection kernel: the basis recurrence is not shared)
+            float S[OCT];
+            if (UNI) {
+                float acc[1][OCT];
+                v1_stencil_octet<1>((const float4 *)(rowT + g * RL), j0, tap[2 * g], tap[2 * g + 1], gw4 + g * NA, 0, acc);
+#pragma unroll
+                for (int i = 0; i < OCT; ++i) S[i] = acc[0][i];
+            } else {
+                float DV[OCT], DG[OCT], EI[OCT];
+                const V1Np np = ((const V1Np *)(V1SM + L.oNP))[g];
+                v1_np_forward_octet((const float4 *)(rowT + g * RL), j0, np, isv, s2v, S, DV, DG, EI);
+            }
+            double cc[OCT], pp[OCT], pc[OCT];
+#pragma unroll
+            for (int i = 0; i < OCT; ++i) { cc[i] = 0.0; pp[i] = 0.0; pc[i] = 1.0; }
+            for (int n = 0; n < n1; ++n) {
+                const double bn_ = (double)bco[n * GS + g];
+                const double an = (2.0 * n + 1.0) / (n + 1.0), bn = (double)n / (n + 1.0);   // (n+1) P_{n+1} = (2n+1) x P_n - n P_{n-1}
+#pragma unroll
+                for (int i = 0; i < OCT; ++i) {
+                    cc[i] = fma(bn_, pc[i], cc[i]);
+                    const double nx = fma(an * xx[i], pc[i], -bn * pp[i]);
+                    pp[i] = pc[i]; pc[i] = nx;
+                }
+            }
+            if ((long long)grp * GS + g >= a.B) continue;
+            float *out = a.model + (size_t)v1_blk.spec[g] * P + sg.o + (j0 - seg_lo);
+#pragma unroll
+            for (int i = 0; i < OCT; ++i)
+                if (j0 - seg_lo + i < sg.P) out[i] = (float)(cc[i] * (double)S[i]);
+        }
+    }
+}
+
+template <int MAXT, int MINB, bool STREAM>
+__global__ void __launch_bounds__(MAXT, MINB)
+lasp_v1_model_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V1Lay L, const V1Args a)
+{
+    v1_init_block(M, L, a);
+    const int NP = M.NP, g = V1_WARP;
+    for (int grp = blockIdx.x; grp < a.ngroups; grp += gridDim.x) {
+        __syncthreads();
+        v1_set_group(grp);
+        __syncthreads();
+        if (g < GS) {
+            for (int p = V1_LANE; p < NP; p += 32)
+                SMV(L.oU, p, g) = 2.f * (a.gparams[v1_blk.spec[g] * NP + p] - M.lo[p]) / (M.hi[p] - M.lo[p]) - 1.f;
+            for (int n = V1_LANE; n < M.nc; n += 32) SMV(L.oB, n, g) = a.mcont[v1_blk.spec[g] * M.nc + n];
+            __syncwarp();
+            v1_param_setup(g);
+        }
+        for (int s = 0; s < M.n_seg; ++s) {
+            const SegDev &sg = M.seg[s];
+            if (g < GS) v1_setup_weights(sg, g);
+            __syncthreads();
+            // T over the whole segment plus the reach of the group's widest kernel (inside the halo: halo >= H + 18)
+            const int *tap = (const int *)(V1SM + L.oTAP);
+            int rl = 0, rh = 0;
+#pragma unroll
+            for (int q = 0; q < GS; ++q) {
+                rl = max(rl, 4 * (tap[2 * q] + tap[2 * q + 1] - 1));
+                rh = max(rh, -4 * tap[2 * q] + 4);
+            }
+            const int seg_lo = sg.po + sg.halo, seg_hi = seg_lo + (sg.P + OCT - 1) / OCT * OCT;
+            const int lo = max(sg.po, seg_lo - (rl + OCT - 1) / OCT * OCT), hi = min(sg.po + sg.len, seg_hi + (rh + OCT - 1) / OCT * OCT);
+            if (!STREAM && a.CF) {
+                const int ks = a.ksteps;
+                if (ks <= 4) v1_phase_emulator_mma<1>(sg, lo, hi);
+                else if (ks <= 8) v1_phase_emulator_mma<2>(sg, lo, hi);
+                else v1_phase_emulator_mma<4>(sg, lo, hi);
+            } else
+                v1_phase_emulator<STREAM>(sg, lo, hi);
+            __syncthreads();
+            if (sg.uniform) v1_phase_model<true, STREAM>(sg, s, grp); else v1_phase_model<false, STREAM>(sg, s, grp);
+            __syncthreads();
         }
     }
 }

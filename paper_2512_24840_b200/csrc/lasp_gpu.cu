@@ -1,6 +1,7 @@
 // lasp_gpu.cu -- C-ABI host side of the LASP-Adam fitting library (include/lasp_gpu.h).
-// Host work here is set-up only (validation, layout, basis tables); every step of the hot path
-// runs in the kernels of lasp_kernels.cuh.
+// Host work here is set-up only (validation, layout, basis tables, launches); every step of the hot path
+// runs in the kernels of lasp_fit_v1.cuh.  No environment variable is read: every switch is a field of
+// lasp_fit_opts.
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -9,43 +10,54 @@
 #include <string>
 #include <vector>
 
-#include "lasp_kernels.cuh"
 #include "lasp_fit_v1.cuh"
 
-#define LASP_VERSION 100
+#define LASP_VERSION 200
 static const double kC_KMS = 299792.458;
+
+// kernel instantiations: index = launch variant
+//   0: resident, 192 threads, 2 CTAs/SM   1: resident, up to 384 threads, 1 CTA/SM   2: streaming, 192 threads, 2 CTAs/SM
+enum { KV_RES192 = 0, KV_RES384 = 1, KV_STREAM = 2, KV_N = 3 };
+static const void *kFit[KV_N] = {(const void *)lasp_v1_fit_kernel<192, 2, false>, (const void *)lasp_v1_fit_kernel<384, 1, false>,
+                                 (const void *)lasp_v1_fit_kernel<192, 2, true>};
+static const void *kGrad[KV_N] = {(const void *)lasp_v1_grad_kernel<192, 2, false>, (const void *)lasp_v1_grad_kernel<384, 1, false>,
+                                  (const void *)lasp_v1_grad_kernel<192, 2, true>};
+static const void *kModel[KV_N] = {(const void *)lasp_v1_model_kernel<192, 2, false>, (const void *)lasp_v1_model_kernel<384, 1, false>,
+                                   (const void *)lasp_v1_model_kernel<192, 2, true>};
+
+struct Variant {          // one way of launching the kernels for this model
+    bool ok = false;
+    int kv = 0;           // kernel instantiation
+    int nt = 0;           // threads per CTA
+    int cta_per_sm = 1;
+    V1Lay L;
+};
 
 struct lasp_ctx {
     ModelDev M;
-    int device = 0, num_sms = 0, wpb = 1;
-    size_t smem_per_warp = 0;
-    float *dC = nullptr, *dinv_s = nullptr;
+    int device = 0, num_sms = 0;
     uint8_t *dexps = nullptr;
     double *dconv = nullptr;
     int *dnedge = nullptr;
-    float2 *dYW = nullptr;
-    size_t yw_tiles = 0;
-    float *dscratch = nullptr;
-    size_t scratch_slots = 0;
     long long launches = 0;
-    double mean_dlog = 0;
-    // kernel v1 (uniform segments): layout, launch shape, staged planes and scratch
-    bool v1_ok = false, v1_nonuniform = false;
-    float *dIS = nullptr, *dS2 = nullptr, *dDS = nullptr;
-    size_t ds_ctas = 0;
-    V1Lay V1;
-    int v1_nt = 0, v1_maxt = 0, v1_cta_per_sm = 1;
-    float *dY = nullptr, *dW = nullptr, *dC1 = nullptr;
-    float4 *dCF = nullptr;   // v1: coefficient table as tf32 [hi|lo] MMA fragments (emulator on the tensor pipe)
+    bool nonuniform = false;
+    float *dIS = nullptr, *dS2 = nullptr;
+    Variant res, str;     // resident and streaming variants
+    float *dC1 = nullptr;
+    float4 *dCF = nullptr;   // coefficient table as tf32 [hi|lo] MMA fragments (emulator_path 2)
     int cf_ksteps = 0;
+    // workspace shared by every call on this ctx: staged planes (per spectrum) and per-CTA scratch
+    float *dY = nullptr, *dW = nullptr;
     size_t plane_rows = 0;
-    float *dCP = nullptr, *dXJ = nullptr;
-    // the workspace (staged planes, scratch) is shared by every call on this ctx: each call waits, on ITS stream, for
-    // the previous call's work (possibly on another stream) and records its own completion
+    float *dCP = nullptr, *dXJ = nullptr, *dDS = nullptr, *dTG = nullptr, *dAG = nullptr;
+    size_t cp_ctas = 0, xj_ctas = 0, ds_ctas = 0, tg_ctas = 0;
     unsigned int *dqueue = nullptr;
+    unsigned long long *dstats = nullptr;   // [0] group-steps of the Adam loops, [1] of them with a fresh Gram factor
     cudaEvent_t ws_event = nullptr;
     bool ws_pending = false;
+#ifdef LASP_PHASE_TIMING
     unsigned long long *ddbg = nullptr;
+#endif
     // lasp_fit_batch_host: double-buffered device chunks, two copy streams and one compute stream
     struct HostPipe {
         int64_t cap = 0;
@@ -54,8 +66,7 @@ struct lasp_ctx {
         int32_t *status[2] = {};
         cudaStream_t s_in = nullptr, s_out = nullptr, s_fit = nullptr;
         cudaEvent_t in_done[2] = {}, fit_done[2] = {}, out_done[2] = {};
-    } hp;   // LASP_TIMING=1: per-phase cycle counters (debug aid)
-    size_t cp_ctas = 0, xj_ctas = 0;
+    } hp;
     std::string err;
 };
 
@@ -75,6 +86,13 @@ static int fail(lasp_ctx *c, int code, const std::string &msg)
             return fail(c, e_ == cudaErrorMemoryAllocation ? LASP_ERR_NOMEM : LASP_ERR_CUDA,  \
                         std::string(#call) + ": " + cudaGetErrorString(e_));                  \
     } while (0)
+
+// The entry points select the ctx's device and put the caller's current device back on return.
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(int dev) { if (cudaGetDevice(&prev) != cudaSuccess) prev = -1; if (prev != dev) cudaSetDevice(dev); else prev = -1; }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
 
 static int roundup(int v, int m) { return (v + m - 1) / m * m; }
 
@@ -107,32 +125,39 @@ extern "C" int lasp_version(void) { return LASP_VERSION; }
 
 extern "C" const char *lasp_last_error(const lasp_ctx *ctx) { return ctx ? ctx->err.c_str() : g_err.c_str(); }
 
-extern "C" int lasp_kernel_variant(const lasp_ctx *ctx) { return ctx && ctx->v1_ok ? 1 : 0; }
+// 1: the resident variant serves this model by default; 2: only the streaming variant does (rows too long for
+// shared memory).  lasp_fit_opts.variant overrides the default per call.
+extern "C" int lasp_kernel_variant(const lasp_ctx *ctx) { return !ctx ? 0 : (ctx->res.ok ? 1 : 2); }
 
-// debug aid (not part of the public header): launch shape of the v1 kernel
-extern "C" int lasp_debug_launch_info(const lasp_ctx *c, int *out4)
+extern "C" int lasp_launch_info(const lasp_ctx *c, int variant, int32_t *out4)
 {
-    if (!c) return LASP_ERR_INVALID_ARG;
-    out4[0] = c->v1_ok; out4[1] = c->v1_nt; out4[2] = c->v1_cta_per_sm; out4[3] = c->V1.total * 4;
+    if (!c || !out4 || variant < 1 || variant > 2) return LASP_ERR_INVALID_ARG;
+    const Variant &v = variant == 1 ? c->res : c->str;
+    out4[0] = v.ok; out4[1] = v.nt; out4[2] = v.cta_per_sm; out4[3] = v.L.total * 4;
     return LASP_OK;
 }
 
-// debug aid (not part of the public header): per-phase cycle sums of the last v1 fit (thread 0 of every CTA)
-extern "C" int lasp_debug_phase_cycles(lasp_ctx *c, unsigned long long *out16)
+#ifdef LASP_PHASE_TIMING
+// debug build only: per-phase cycle sums of the last fit (thread 0 of every CTA)
+extern "C" int lasp_debug_phase_cycles(lasp_ctx *c, unsigned long long *out24)
 {
     if (!c || !c->ddbg) return LASP_ERR_INVALID_ARG;
-    return cudaMemcpy(out16, c->ddbg, 24 * sizeof(unsigned long long), cudaMemcpyDeviceToHost) == cudaSuccess ? LASP_OK : LASP_ERR_CUDA;
+    return cudaMemcpy(out24, c->ddbg, 24 * sizeof(unsigned long long), cudaMemcpyDeviceToHost) == cudaSuccess ? LASP_OK : LASP_ERR_CUDA;
 }
+#endif
 
 extern "C" int64_t lasp_launch_count(const lasp_ctx *ctx) { return ctx ? ctx->launches : 0; }
 
 extern "C" int lasp_destroy(lasp_ctx *c)
 {
     if (!c) return LASP_OK;
-    cudaSetDevice(c->device);
-    cudaFree(c->dC); cudaFree(c->dinv_s); cudaFree(c->dexps); cudaFree(c->dconv); cudaFree(c->dnedge);
-    cudaFree(c->dYW); cudaFree(c->dscratch);
-    cudaFree(c->dC1); cudaFree(c->dCF); cudaFree(c->dIS); cudaFree(c->dS2); cudaFree(c->dDS); cudaFree(c->dY); cudaFree(c->dW); cudaFree(c->dCP); cudaFree(c->dXJ); cudaFree(c->ddbg); cudaFree(c->dqueue);
+    DeviceGuard dg(c->device);
+    cudaFree(c->dexps); cudaFree(c->dconv); cudaFree(c->dnedge);
+    cudaFree(c->dC1); cudaFree(c->dCF); cudaFree(c->dIS); cudaFree(c->dS2); cudaFree(c->dDS); cudaFree(c->dY); cudaFree(c->dW);
+    cudaFree(c->dCP); cudaFree(c->dXJ); cudaFree(c->dTG); cudaFree(c->dAG); cudaFree(c->dqueue); cudaFree(c->dstats);
+#ifdef LASP_PHASE_TIMING
+    cudaFree(c->ddbg);
+#endif
     if (c->ws_event) cudaEventDestroy(c->ws_event);
     hostpipe_free(c);
     if (c->hp.s_in) {
@@ -143,8 +168,7 @@ extern "C" int lasp_destroy(lasp_ctx *c)
     return LASP_OK;
 }
 
-static int setup_v1(lasp_ctx *c, const cudaDeviceProp &prop, int emax);
-static int v1_workspace(lasp_ctx *c, int64_t B, bool need_xj);
+static void setup_variant(lasp_ctx *c, const cudaDeviceProp &prop, int emax, bool stream, Variant &v);
 
 extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx **out)
 {
@@ -179,12 +203,15 @@ extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx *
     lasp_ctx *c = new (std::nothrow) lasp_ctx();
     if (!c) return fail(nullptr, LASP_ERR_NOMEM, "host allocation failed");
     c->device = cuda_device;
+    int prev_dev = -1;
+    cudaGetDevice(&prev_dev);
 #define CUDA_TRY_C(call)                                                  \
     do {                                                                  \
         cudaError_t e_ = (call);                                          \
         if (e_ != cudaSuccess) {                                          \
             std::string m_ = std::string(#call) + ": " + cudaGetErrorString(e_); \
             lasp_destroy(c);                                              \
+            if (prev_dev >= 0) cudaSetDevice(prev_dev);                   \
             return fail(nullptr, LASP_ERR_CUDA, m_);                      \
         }                                                                 \
     } while (0)
@@ -205,8 +232,8 @@ extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx *
     std::vector<double> s(P);
     const double vmax = fmax(fabs((double)d->lo[L]), fabs((double)d->hi[L]));
     const double smax = fmax(fabs((double)d->lo[L + 1]), fabs((double)d->hi[L + 1]));
-    int po = 0, g_rows = 0;
-    M.Hmax = 0;
+    int po = 0;
+    bool halo_ok = true;
     std::vector<double> conv((size_t)nseg * M.n1 * M.n1, 0.0);
     for (int sg = 0; sg < nseg; ++sg) {
         const int o = d->seg_offset[sg], e = d->seg_offset[sg + 1], Ps = e - o;
@@ -220,12 +247,15 @@ extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx *
         }
         SegDev &S = M.seg[sg];
         const double si = d->seg_sigma_inst[sg];
-        const int Hm = (int)ceil((vmax + 5.0 * sqrt(smax * smax + si * si)) / smin) + 1;
-        S.halo = roundup(Hm + 18, CH);   // v1 reads up to 18 pixels past the largest support
+        const double hm = ceil((vmax + 5.0 * sqrt(smax * smax + si * si)) / smin) + 1.0;
+        if (!(hm < (double)(V1_TPAD - 18))) { halo_ok = false; break; }
+        const int Hm = (int)hm;
+        S.halo = roundup(Hm + 18, CH);   // the kernels read up to 18 pixels past the largest support
         S.po = po; S.P = Ps; S.o = o;
         S.len = S.halo + roundup(Ps, CH) + S.halo;
         po += S.len;
         S.uniform = (smx - smin) <= 1e-6 * smin ? 1 : 0;
+        if (!S.uniform) c->nonuniform = true;    // per-pixel kernels (linear grids, C.2-14)
         S.inv_s = (float)(S.uniform ? (double)Ps / ssum : 1.0 / smin);
         S.sig_inst = d->seg_sigma_inst[sg];
         const int ne = d->seg_n_edge[sg];
@@ -239,9 +269,7 @@ extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx *
         double ta = 0.0, tb = 0.0;
         if (jh > jl) { ta = 2.0 / (jh - jl); tb = -(double)(jl + jh) / (jh - jl); }
         S.ta = (float)ta; S.tb = (float)tb;
-        if (S.uniform) g_rows = std::max(g_rows, 2 * S.halo + 1);
-        M.Hmax = std::max(M.Hmax, S.halo);
-        // conv[m][n] = (2m+1)/2 int P_m(x) T_n(alpha x + beta) dx, exact by Gauss-Legendre (D+1 nodes)
+        // conv[m][n] = (2m+1)/2 int P_m(x) T_n(alpha x + beta) dx, exact by Gauss-Legendre (D+2 nodes)
         // with the device's float ta, tb so that the conversion matches the basis actually used
         const double alpha = (double)S.ta * Ps / 2.0, beta = (double)S.ta * Ps / 2.0 + (double)S.tb;
         std::vector<double> gx, gw;
@@ -258,9 +286,14 @@ extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx *
                 for (int n = 0; n < M.n1; ++n) cv[m * M.n1 + n] += 0.5 * (2.0 * m + 1.0) * gw[q] * Pm[m] * Tn[n];
         }
     }
+    if (!halo_ok) {
+        lasp_destroy(c);
+        if (prev_dev >= 0) cudaSetDevice(prev_dev);
+        return fail(nullptr, LASP_ERR_UNSUPPORTED, "largest kernel support over the prior box exceeds 238 pixels");
+    }
     M.Ppad = po;
     // padded tables: halos replicate the segment's edge pixel (the clamp of C.2-16 for free)
-    // K+2 rounded to 8 rows, plus 16 (prefetch overrun): zero past K, so the v1 loops sweep whole batches without bounds tests
+    // K+2 rounded to 4 rows, plus 16 (prefetch overrun): zero past K, so the loops sweep whole batches without bounds tests
     const int Krows = roundup(K + 2, 4) + 16;
     std::vector<float> Cp((size_t)Krows * M.Ppad, 0.f), isp(M.Ppad);
     for (int sg = 0; sg < nseg; ++sg) {
@@ -272,22 +305,7 @@ extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx *
             for (int k = 0; k < K; ++k) Cp[(size_t)k * M.Ppad + S.po + q] = d->coeffs[(size_t)k * P + S.o + rel];
         }
     }
-    // shared-memory rows per warp
-    int r = 0;
-    M.r_U = r; r += NP; M.r_M = r; r += NP; M.r_V = r; r += NP;
-    M.r_PHI = r; r += K; M.r_Q = r; r += K;
-    M.r_G = r; r += g_rows;
-    M.r_MOM = r; r += M.nmom; M.r_RHS = r; r += M.n1; M.r_B = r; r += M.nc;
-    M.rows = r;
-    M.nscr = A_J0 + NP;
-    c->smem_per_warp = (size_t)M.rows * RS * sizeof(float);
-    const size_t smem_max = prop.sharedMemPerBlockOptin;
-    c->wpb = (int)std::min<size_t>(8, smem_max / c->smem_per_warp);
-    if (c->wpb < 1) { lasp_destroy(c); return fail(nullptr, LASP_ERR_UNSUPPORTED, "per-warp state exceeds shared memory"); }
-
-    CUDA_TRY_C(cudaMalloc(&c->dC, Cp.size() * sizeof(float)));
-    CUDA_TRY_C(cudaMemcpy(c->dC, Cp.data(), Cp.size() * sizeof(float), cudaMemcpyHostToDevice));
-    {   // v1's copy of the table in the split-octet layout
+    {   // the table in the split-octet layout (half h of octet o at h*Ppad/2 + 4 o)
         std::vector<float> C1(Cp.size());
         for (int k = 0; k < Krows; ++k)
             for (int jp = 0; jp < M.Ppad; ++jp)
@@ -296,7 +314,7 @@ extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx *
         CUDA_TRY_C(cudaMemcpy(c->dC1, C1.data(), C1.size() * sizeof(float), cudaMemcpyHostToDevice));
     }
     if (K <= 128) {
-        // v1's tensor-pipe copy: A fragments of mma.m16n8k8 (rows = pixels, columns = terms), one float4 per
+        // tensor-pipe copy: A fragments of mma.m16n8k8 (rows = pixels, columns = terms), one float4 per
         // (octet o, k-step s, lane l): {hi, hi', lo, lo'} of C[8s + l%4 (+4)][8o + l/4], hi = tf32(x), lo = tf32(x - hi)
         auto tf32 = [](float x) {
             uint32_t u; memcpy(&u, &x, 4);
@@ -319,7 +337,7 @@ extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx *
         CUDA_TRY_C(cudaMalloc(&c->dCF, CF.size() * sizeof(float)));
         CUDA_TRY_C(cudaMemcpy(c->dCF, CF.data(), CF.size() * sizeof(float), cudaMemcpyHostToDevice));
     }
-    {   // 1/s_j and s_j^2 for v1's per-pixel kernels, V1_TPAD replicated entries on both sides
+    {   // 1/s_j and s_j^2 for the per-pixel kernels, V1_TPAD replicated entries on both sides
         std::vector<float> is1(M.Ppad + 2 * V1_TPAD), s21(M.Ppad + 2 * V1_TPAD);
         for (int q = 0; q < M.Ppad + 2 * V1_TPAD; ++q) {
             const int jp = std::min(std::max(q - V1_TPAD, 0), M.Ppad - 1);
@@ -331,143 +349,160 @@ extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx *
         CUDA_TRY_C(cudaMalloc(&c->dS2, s21.size() * sizeof(float)));
         CUDA_TRY_C(cudaMemcpy(c->dS2, s21.data(), s21.size() * sizeof(float), cudaMemcpyHostToDevice));
     }
-    CUDA_TRY_C(cudaMalloc(&c->dinv_s, isp.size() * sizeof(float)));
-    CUDA_TRY_C(cudaMemcpy(c->dinv_s, isp.data(), isp.size() * sizeof(float), cudaMemcpyHostToDevice));
     CUDA_TRY_C(cudaMalloc(&c->dexps, (size_t)K * L));
     CUDA_TRY_C(cudaMemcpy(c->dexps, d->term_exps, (size_t)K * L, cudaMemcpyHostToDevice));
     CUDA_TRY_C(cudaMalloc(&c->dconv, conv.size() * sizeof(double)));
     CUDA_TRY_C(cudaMemcpy(c->dconv, conv.data(), conv.size() * sizeof(double), cudaMemcpyHostToDevice));
     CUDA_TRY_C(cudaMalloc(&c->dnedge, nseg * sizeof(int)));
     CUDA_TRY_C(cudaMemcpy(c->dnedge, d->seg_n_edge, nseg * sizeof(int), cudaMemcpyHostToDevice));
-    M.C = c->dC; M.inv_s = c->dinv_s; M.exps = c->dexps; M.conv = c->dconv;
-    const int smem_bytes = (int)(c->smem_per_warp * c->wpb);
-    CUDA_TRY_C(cudaFuncSetAttribute(lasp_fit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
-    CUDA_TRY_C(cudaFuncSetAttribute(lasp_grad_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
-    CUDA_TRY_C(cudaFuncSetAttribute(lasp_model_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
+    CUDA_TRY_C(cudaMalloc(&c->dqueue, sizeof(unsigned int)));
+    CUDA_TRY_C(cudaMalloc(&c->dstats, 2 * sizeof(unsigned long long)));
+    CUDA_TRY_C(cudaMemset(c->dstats, 0, 2 * sizeof(unsigned long long)));
+    CUDA_TRY_C(cudaEventCreateWithFlags(&c->ws_event, cudaEventDisableTiming));
+    M.exps = c->dexps; M.conv = c->dconv;
     int emax = 0;
     for (int i = 0; i < K * L; ++i) emax = std::max(emax, (int)d->term_exps[i]);
-    setup_v1(c, prop, emax);
+    setup_variant(c, prop, emax, false, c->res);
+    setup_variant(c, prop, emax, true, c->str);
+    if (prev_dev >= 0) cudaSetDevice(prev_dev);
+    if (!c->res.ok && !c->str.ok) {
+        lasp_destroy(c);
+        return fail(nullptr, LASP_ERR_UNSUPPORTED, "model state does not fit the kernels' shared memory");
+    }
     *out = c;
     return LASP_OK;
 }
 
 // ------------------------------------------------------------------------------------------
-// kernel v1: shared-memory layout and launch shape (lasp_fit_v1.cuh)
+// shared-memory layout and launch shape of one variant (lasp_fit_v1.cuh)
 // ------------------------------------------------------------------------------------------
-template <typename F>
-static void v1_for_kernels(F f)
-{
-    f((const void *)lasp_v1_fit_kernel<192, 2>, 192);
-    f((const void *)lasp_v1_grad_kernel<192, 2>, 192);
-    f((const void *)lasp_v1_fit_kernel<384, 1>, 384);
-    f((const void *)lasp_v1_grad_kernel<384, 1>, 384);
-}
-
-static int setup_v1(lasp_ctx *c, const cudaDeviceProp &prop, int emax)
+static void setup_variant(lasp_ctx *c, const cudaDeviceProp &prop, int emax, bool stream, Variant &v)
 {
     const ModelDev &M = c->M;
-    c->v1_ok = false;
+    v.ok = false;
     int maxlen = 0, guard = 0, nfit = 0, hmax = 1;
-    c->v1_nonuniform = false;
     for (int s = 0; s < M.n_seg; ++s) {
         const SegDev &S = M.seg[s];
         maxlen = std::max(maxlen, S.len);
         guard = std::max(guard, S.halo);
         nfit = std::max(nfit, (S.fit_hi - S.fit_lo) / OCT);
         if (S.uniform) hmax = std::max(hmax, S.halo - 18);   // tap tables exist only for uniform segments
-        else c->v1_nonuniform = true;                         // per-pixel kernels (linear grids, C.2-14)
-        if (S.halo > V1_TPAD) return LASP_OK;
     }
-    if (getenv("LASP_V1_UNIFORM_ONLY") && c->v1_nonuniform) return LASP_OK;
-    if (M.NP > 32 || M.n1 > 32) return LASP_OK;
-    V1Lay &L = c->V1;
+    if (M.NP > 32 || M.n1 > 32) return;
+    V1Lay &L = v.L;
     memset(&L, 0, sizeof(L));
     L.emax = emax;
     int nt = std::max(GS * 32, roundup(std::max(nfit, 1), 32));
     if (nt > 384) nt = 384;               // longer segments are swept in several passes
-    c->v1_nt = nt;
-    c->v1_maxt = nt <= 192 ? 192 : 384;
+    if (stream) nt = 192;
+    v.nt = nt;
+    v.kv = stream ? KV_STREAM : (nt <= 192 ? KV_RES192 : KV_RES384);
     L.NW = nt / 32;
+    L.nt8 = nt * OCT;
     L.GUARD = guard;
-    L.RL = maxlen + 2 * guard;
+    L.RL = stream ? L.nt8 + 2 * guard : maxlen + 2 * guard;
+    L.SL = maxlen;
     L.Hm = hmax;
     L.NA = (hmax + 3) / 4 + hmax / 4 + 2;
     L.n1r = roundup(M.n1, 8);
     L.nmomr = L.n1r + roundup(std::max(M.nmom - L.n1r, 0), 8);
     L.VR = L.nmomr + L.n1r + roundup(M.K + 2, 8) + 6;
-    const char *rf = getenv("LASP_REFRESH");
-    L.refresh = rf ? std::max(1, atoi(rf)) : 64;
-    const char *rw = getenv("LASP_REFRESH_WARM");
-    L.warm = rw ? std::max(1, atoi(rw)) : std::min(L.refresh, 4);
-    L.fastupd = (M.L >= 1 && M.L <= 4 && M.K + 2 <= 32 && L.NW <= 12 && !getenv("LASP_NO_FASTUPD")) ? 1 : 0;
-    L.fdfresh = getenv("LASP_FD_FRESH") ? 1 : 0;
+    L.fastupd = (M.L >= 1 && M.L <= 4 && M.K + 2 <= 32 && L.NW <= 12) ? 1 : 0;
     L.fastw = (L.fastupd && M.n_seg == 1 && M.seg[0].uniform && M.seg[0].fit_hi > M.seg[0].fit_lo) ? 1 : 0;
     size_t bytes = 0;
     for (L.lfseg = 1; L.lfseg >= 0; --L.lfseg) {   // a factor slot per segment if shared memory allows it
-    int o = 0;
-    auto take = [&](int n) { int r = o; o += roundup(n, 4); return r; };
-    L.oT = take(GS * L.RL); L.oA = take(GS * L.RL);
-    L.oU = take(GS * M.NP); L.oM = take(GS * M.NP); L.oV = take(GS * M.NP);
-    L.Kq = roundup(M.K + 2, 4);
-    L.oX = take(GS * M.L); L.oPHI = take(GS * L.Kq);
-    L.oGW = take(GS * L.NA * 4); L.oGR = take(3 * GS * L.NA * 4); L.oTAP = take(2 * GS);
-    L.oMOM = take(GS * L.nmomr); L.oRHS = take(GS * L.n1r); L.oB = take(GS * M.nc);
-    L.oRED = take(L.NW * L.VR * GS);
-    const int npair = M.NP * (M.NP + 1) / 2;
-    L.oLF = take(std::max(GS * V1_LFS * (L.lfseg ? M.n_seg : 1), 2 * GS * npair + 4));
-    L.oQ = take(GS * (M.K + 2)); L.oSC = take(GS * (SC_N + M.n_seg));
-    L.oEXP = take(std::max((M.K * M.L + 3) / 4, M.K));   // bytes [K][L], or one packed word per term when L <= 4
-    L.oXP = take(GS * M.L * (L.emax + 1)); L.oDPHI = take(GS * M.L * M.K); L.oGSC = take(GS * M.NP);
-    L.oNP = take(GS * 8);
-    L.oEW = take(GS * (2 * hmax + 2));
-    L.total = o;
-    bytes = (size_t)o * sizeof(float);
-    if (bytes <= prop.sharedMemPerBlockOptin) break;
+        int o = 0;
+        auto take = [&](int n) { int r = o; o += roundup(n, 4); return r; };
+        L.oT = take(GS * L.RL);
+        L.oA = stream ? L.oT : take(GS * L.RL);    // streaming: one window buffer serves both rows
+        L.oU = take(GS * M.NP); L.oM = take(GS * M.NP); L.oV = take(GS * M.NP);
+        L.Kq = roundup(M.K + 2, 4);
+        L.oX = take(GS * M.L); L.oPHI = take(GS * L.Kq);
+        L.oGW = take(GS * L.NA * 4); L.oGR = take(3 * GS * L.NA * 4); L.oTAP = take(2 * GS);
+        L.oMOM = take(GS * L.nmomr); L.oRHS = take(GS * L.n1r); L.oB = take(GS * M.nc);
+        L.oRED = take(L.NW * L.VR * GS);
+        const int npair = M.NP * (M.NP + 1) / 2;
+        L.oLF = take(std::max(GS * V1_LFS * (L.lfseg ? M.n_seg : 1), 2 * GS * npair + 4));
+        L.oQ = take(GS * (M.K + 2)); L.oSC = take(GS * (SC_N + M.n_seg));
+        L.oEXP = take(std::max((M.K * M.L + 3) / 4, M.K));   // bytes [K][L], or one packed word per term when L <= 4
+        L.oXP = take(GS * M.L * (L.emax + 1)); L.oDPHI = take(GS * M.L * M.K); L.oGSC = take(GS * M.NP);
+        L.oNP = take(GS * 8);
+        L.total = o;
+        bytes = (size_t)o * sizeof(float);
+        if (bytes + 2048 <= prop.sharedMemPerBlockOptin) break;   // + the kernels' static block state
     }
-    if (L.lfseg < 0) return LASP_OK;   // does not fit: v0 handles it
-    bool ok = true;
-    v1_for_kernels([&](const void *f, int) {
-        if (cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess) ok = false;
-    });
-    if (!ok) { cudaGetLastError(); return LASP_OK; }
+    if (L.lfseg < 0) return;
+    const void *fs[3] = {kFit[v.kv], kGrad[v.kv], kModel[v.kv]};
+    for (const void *f : fs)
+        if (cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess) { cudaGetLastError(); return; }
     int per_sm = 0;
-    const void *fk = c->v1_maxt == 192 ? (const void *)lasp_v1_fit_kernel<192, 2> : (const void *)lasp_v1_fit_kernel<384, 1>;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fk, nt, bytes) != cudaSuccess || per_sm < 1) {
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kFit[v.kv], nt, bytes) != cudaSuccess || per_sm < 1) {
         cudaGetLastError();
-        return LASP_OK;
+        return;
     }
-    c->v1_cta_per_sm = per_sm;
-    if (const char *e = getenv("LASP_CTAS_PER_SM")) c->v1_cta_per_sm = std::max(1, std::min(per_sm, atoi(e)));   // experiment knob
-    c->v1_ok = getenv("LASP_FORCE_V0") == nullptr;
+    v.cta_per_sm = per_sm;
+    v.ok = true;
+}
+
+// ------------------------------------------------------------------------------------------
+// options, workspace, launches
+// ------------------------------------------------------------------------------------------
+static const lasp_fit_opts kDefaultOpts = {0, 1e-2f, 0.9f, 0.999f, 1e-8f, 0, 0, 0, 0, 0};
+
+// variant / emulator path of one call (opts may be null: defaults)
+static int resolve(lasp_ctx *c, const lasp_fit_opts *o, const char *who, const Variant **v, bool *mma)
+{
+    if (!o) o = &kDefaultOpts;
+    if (o->variant < 0 || o->variant > 2) return fail(c, LASP_ERR_INVALID_ARG, std::string(who) + ": variant must be 0, 1 or 2");
+    if (o->emulator_path < 0 || o->emulator_path > 2)
+        return fail(c, LASP_ERR_INVALID_ARG, std::string(who) + ": emulator_path must be 0, 1 or 2");
+    if (o->refresh < 0 || o->warm < 0 || o->fd_fresh < 0 || o->fd_fresh > 1)
+        return fail(c, LASP_ERR_INVALID_ARG, std::string(who) + ": refresh, warm must be >= 0 and fd_fresh 0 or 1");
+    const Variant *vv = nullptr;
+    if (o->variant == 1) vv = c->res.ok ? &c->res : nullptr;
+    else if (o->variant == 2) vv = c->str.ok ? &c->str : nullptr;
+    else vv = c->res.ok ? &c->res : (c->str.ok ? &c->str : nullptr);
+    if (!vv)
+        return fail(c, LASP_ERR_UNSUPPORTED, std::string(who) + (o->variant == 1 ? ": the rows of this model do not fit shared memory (variant 1, resident)"
+                                                                                   : ": variant not available for this model"));
+    *mma = o->emulator_path == 2;
+    if (*mma && !(vv == &c->res && c->dCF))
+        return fail(c, LASP_ERR_UNSUPPORTED, std::string(who) + ": emulator_path 2 (tensor pipe) needs the resident variant and n_terms <= 128");
+    *v = vv;
     return LASP_OK;
 }
 
-// ------------------------------------------------------------------------------------------
-// workspace and launches
-// ------------------------------------------------------------------------------------------
-static int launch_shape(const lasp_ctx *c, int tiles, int &grid, int &wpb)
+static int workspace(lasp_ctx *c, int64_t B, const Variant &v, bool need_planes, bool need_cp, bool need_xj)
 {
-    wpb = std::max(1, std::min(c->wpb, (tiles + c->num_sms - 1) / c->num_sms));
-    grid = std::min(c->num_sms, (tiles + wpb - 1) / wpb);
-    return 0;
-}
-
-static int ensure_workspace(lasp_ctx *c, int64_t B, bool need_yw)
-{
-    const size_t tiles = (size_t)((B + 31) / 32);
-    CUDA_TRY(c, cudaSetDevice(c->device));
-    if (need_yw && tiles > c->yw_tiles) {
-        if (c->dYW) cudaFree(c->dYW);
-        c->dYW = nullptr; c->yw_tiles = 0;
-        CUDA_TRY(c, cudaMalloc(&c->dYW, tiles * (size_t)c->M.Ppad * 32 * sizeof(float2)));
-        c->yw_tiles = tiles;
+    const ModelDev &M = c->M;
+    if (need_planes && (size_t)B > c->plane_rows) {
+        cudaFree(c->dY); cudaFree(c->dW);
+        c->dY = c->dW = nullptr; c->plane_rows = 0;
+        CUDA_TRY(c, cudaMalloc(&c->dY, (size_t)B * M.Ppad * sizeof(float)));
+        CUDA_TRY(c, cudaMalloc(&c->dW, (size_t)B * M.Ppad * sizeof(float)));
+        c->plane_rows = (size_t)B;
     }
-    const size_t slots = (size_t)c->num_sms * c->wpb;
-    if (slots > c->scratch_slots) {
-        if (c->dscratch) cudaFree(c->dscratch);
-        c->dscratch = nullptr; c->scratch_slots = 0;
-        CUDA_TRY(c, cudaMalloc(&c->dscratch, slots * (size_t)c->M.nscr * c->M.Ppad * 32 * sizeof(float)));
-        c->scratch_slots = slots;
+    const size_t ctas = (size_t)c->num_sms * std::max(c->res.ok ? c->res.cta_per_sm : 1, c->str.ok ? c->str.cta_per_sm : 1);
+    if (need_cp && ctas > c->cp_ctas) {
+        cudaFree(c->dCP); c->dCP = nullptr; c->cp_ctas = 0;
+        CUDA_TRY(c, cudaMalloc(&c->dCP, ctas * GS * M.Ppad * sizeof(float)));
+        c->cp_ctas = ctas;
+    }
+    if (need_cp && c->nonuniform && ctas > c->ds_ctas) {
+        cudaFree(c->dDS); c->dDS = nullptr; c->ds_ctas = 0;
+        CUDA_TRY(c, cudaMalloc(&c->dDS, ctas * 3 * GS * v.L.SL * sizeof(float)));
+        c->ds_ctas = ctas;
+    }
+    if (need_xj && ctas > c->xj_ctas) {
+        cudaFree(c->dXJ); c->dXJ = nullptr; c->xj_ctas = 0;
+        CUDA_TRY(c, cudaMalloc(&c->dXJ, ctas * (size_t)(1 + M.NP) * GS * M.Ppad * sizeof(float)));
+        c->xj_ctas = ctas;
+    }
+    if (&v == &c->str && ctas > c->tg_ctas) {
+        cudaFree(c->dTG); cudaFree(c->dAG); c->dTG = c->dAG = nullptr; c->tg_ctas = 0;
+        CUDA_TRY(c, cudaMalloc(&c->dTG, ctas * GS * M.Ppad * sizeof(float)));
+        CUDA_TRY(c, cudaMalloc(&c->dAG, ctas * GS * M.Ppad * sizeof(float)));
+        c->tg_ctas = ctas;
     }
     return LASP_OK;
 }
@@ -475,26 +510,14 @@ static int ensure_workspace(lasp_ctx *c, int64_t B, bool need_yw)
 extern "C" int lasp_reserve(lasp_ctx *c, int64_t B)
 {
     if (!c || B < 1) return fail(c, LASP_ERR_INVALID_ARG, "lasp_reserve: bad argument");
-    if (c->v1_ok) return v1_workspace(c, B, true);
-    return ensure_workspace(c, B, true);
+    DeviceGuard dg(c->device);
+    return workspace(c, B, c->res.ok ? c->res : c->str, true, true, true);
 }
 
-static int stage(lasp_ctx *c, int64_t B, const float *flux, const float *ivar, const uint8_t *mask,
-                 cudaStream_t st)
-{
-    const int tiles = (int)((B + 31) / 32);
-    CUDA_TRY(c, cudaMemsetAsync(c->dYW, 0, (size_t)tiles * c->M.Ppad * 32 * sizeof(float2), st));
-    dim3 grid((c->M.P + 31) / 32, tiles), block(32, 8);
-    lasp_stage_kernel<<<grid, block, 0, st>>>(c->M, flux, ivar, mask, B, c->dYW);
-    lasp_edge_kernel<<<tiles, 32, 0, st>>>(c->M, c->dnedge, c->dYW);
-    c->launches += 2;
-    CUDA_TRY(c, cudaGetLastError());
-    return LASP_OK;
-}
-
-// ---- kernel v1: staging (a0), workspace, launches -----------------------------------------------
-// a0 for v1: w = mask*ivar, zero on the n_edge pixels at each end of each segment (Eq. 8),
-// non-finite or non-positive ivar treated as masked; rows go to the padded layout (halos zero).
+// a0: w = mask*ivar, zero on the n_edge pixels at each end of each segment (Eq. 8); rows go to the
+// padded layout (halos zero).  Exactly the oracle's rule: a pixel takes part iff w != 0, so y is zeroed where
+// w == 0 (masked flux may hold anything) and nothing else is altered -- a non-finite flux or weight on a pixel
+// that takes part propagates and ends in status bit LASP_ST_NONFINITE (reading R-1).
 __global__ void lasp_v1_stage_kernel(const __grid_constant__ ModelDev M, const int *__restrict__ n_edge,
                                      const float *__restrict__ flux, const float *__restrict__ ivar,
                                      const uint8_t *__restrict__ mask, float *__restrict__ Y, float *__restrict__ W)
@@ -508,11 +531,11 @@ __global__ void lasp_v1_stage_kernel(const __grid_constant__ ModelDev M, const i
         float y = 0.f, w = 0.f;
         if (rel >= 0 && rel < sg.P) {
             const size_t o = row * M.P + sg.o + rel;
-            y = flux[o]; w = ivar[o];
+            w = ivar[o];
             if (mask && mask[o] == 0) w = 0.f;
-            if (!(w > 0.f) || !isfinite(w) || !isfinite(y)) { w = 0.f; y = 0.f; }
             const int ne = n_edge[s];
             if (rel < ne || rel >= sg.P - ne) w = 0.f;
+            y = (w == 0.f) ? 0.f : flux[o];
         }
         // split-octet layout: half h of octet o at h*Ppad/2 + 4 o, so that a warp's 128-bit loads are contiguous
         const size_t q = row * M.Ppad + ((jp >> 2) & 1) * (M.Ppad >> 1) + (jp >> 3) * 4 + (jp & 3);
@@ -521,43 +544,7 @@ __global__ void lasp_v1_stage_kernel(const __grid_constant__ ModelDev M, const i
     }
 }
 
-static int v1_grid(const lasp_ctx *c, int64_t B, int &ngroups)
-{
-    ngroups = (int)((B + GS - 1) / GS);
-    return std::min(ngroups, c->num_sms * c->v1_cta_per_sm);
-}
-
-static int v1_workspace(lasp_ctx *c, int64_t B, bool need_xj)
-{
-    CUDA_TRY(c, cudaSetDevice(c->device));
-    const ModelDev &M = c->M;
-    if ((size_t)B > c->plane_rows) {
-        cudaFree(c->dY); cudaFree(c->dW);
-        c->dY = c->dW = nullptr; c->plane_rows = 0;
-        CUDA_TRY(c, cudaMalloc(&c->dY, (size_t)B * M.Ppad * sizeof(float)));
-        CUDA_TRY(c, cudaMalloc(&c->dW, (size_t)B * M.Ppad * sizeof(float)));
-        c->plane_rows = (size_t)B;
-    }
-    const size_t ctas = (size_t)c->num_sms * c->v1_cta_per_sm;
-    if (ctas > c->cp_ctas) {
-        cudaFree(c->dCP); c->dCP = nullptr; c->cp_ctas = 0;
-        CUDA_TRY(c, cudaMalloc(&c->dCP, ctas * GS * M.Ppad * sizeof(float)));
-        c->cp_ctas = ctas;
-    }
-    if (c->v1_nonuniform && ctas > c->ds_ctas) {
-        cudaFree(c->dDS); c->dDS = nullptr; c->ds_ctas = 0;
-        CUDA_TRY(c, cudaMalloc(&c->dDS, ctas * 3 * GS * M.Ppad * sizeof(float)));
-        c->ds_ctas = ctas;
-    }
-    if (need_xj && ctas > c->xj_ctas) {
-        cudaFree(c->dXJ); c->dXJ = nullptr; c->xj_ctas = 0;
-        CUDA_TRY(c, cudaMalloc(&c->dXJ, ctas * (size_t)(1 + M.NP) * GS * M.Ppad * sizeof(float)));
-        c->xj_ctas = ctas;
-    }
-    return LASP_OK;
-}
-
-static int v1_stage(lasp_ctx *c, int64_t B, const float *flux, const float *ivar, const uint8_t *mask, cudaStream_t st)
+static int stage(lasp_ctx *c, int64_t B, const float *flux, const float *ivar, const uint8_t *mask, cudaStream_t st)
 {
     lasp_v1_stage_kernel<<<(unsigned)B, 256, 0, st>>>(c->M, c->dnedge, flux, ivar, mask, c->dY, c->dW);
     c->launches += 1;
@@ -565,9 +552,10 @@ static int v1_stage(lasp_ctx *c, int64_t B, const float *flux, const float *ivar
     return LASP_OK;
 }
 
+// every call waits, on ITS stream, for the ctx's previous call (possibly on another stream) before it touches the
+// shared workspace, and records its own completion
 static int ws_acquire(lasp_ctx *c, cudaStream_t st)
 {
-    if (!c->ws_event) CUDA_TRY(c, cudaEventCreateWithFlags(&c->ws_event, cudaEventDisableTiming));
     if (c->ws_pending) CUDA_TRY(c, cudaStreamWaitEvent(st, c->ws_event, 0));
     return LASP_OK;
 }
@@ -579,18 +567,23 @@ static int ws_release(lasp_ctx *c, cudaStream_t st)
     return LASP_OK;
 }
 
-static int v1_launch(lasp_ctx *c, bool grad, const V1Args &a, int grid, cudaStream_t st)
+static void base_args(lasp_ctx *c, const Variant &v, bool mma, int64_t B, V1Args &a)
 {
-    const size_t smem = (size_t)c->V1.total * sizeof(float);
-    if (c->v1_maxt == 192) {
-        if (grad) lasp_v1_grad_kernel<192, 2><<<grid, c->v1_nt, smem, st>>>(c->M, c->V1, a);
-        else lasp_v1_fit_kernel<192, 2><<<grid, c->v1_nt, smem, st>>>(c->M, c->V1, a);
-    } else {
-        if (grad) lasp_v1_grad_kernel<384, 1><<<grid, c->v1_nt, smem, st>>>(c->M, c->V1, a);
-        else lasp_v1_fit_kernel<384, 1><<<grid, c->v1_nt, smem, st>>>(c->M, c->V1, a);
-    }
+    memset(&a, 0, sizeof(a));
+    a.Y = c->dY; a.W = c->dW; a.C1 = c->dC1; a.CP = c->dCP; a.B = B;
+    a.IS = c->dIS; a.S2 = c->dS2; a.DS = c->dDS;
+    if (&v == &c->str) { a.TG = c->dTG; a.AG = c->dAG; }
+    if (mma) { a.CF = c->dCF; a.ksteps = c->cf_ksteps; }
+    a.ngroups = (int)((B + GS - 1) / GS);
+}
+
+static int launch(lasp_ctx *c, const void *const *table, const Variant &v, const V1Args &a, cudaStream_t st)
+{
+    const int grid = std::min(a.ngroups, c->num_sms * v.cta_per_sm);
+    const size_t smem = (size_t)v.L.total * sizeof(float);
+    void *args[3] = {(void *)&c->M, (void *)&v.L, (void *)&a};
+    CUDA_TRY(c, cudaLaunchKernel(table[v.kv], dim3(grid), dim3(v.nt), args, smem, st));
     c->launches += 1;
-    CUDA_TRY(c, cudaGetLastError());
     return ws_release(c, st);
 }
 
@@ -606,122 +599,85 @@ extern "C" int lasp_fit_batch(lasp_ctx *c, int64_t B, const float *flux, const f
         !(opts->beta2 >= 0.f && opts->beta2 < 1.f) || !(opts->eps >= 0.f))
         return fail(c, LASP_ERR_INVALID_ARG, "lasp_fit_batch: bad Adam hyper-parameters");
     if (B > (int64_t)1 << 30) return fail(c, LASP_ERR_UNSUPPORTED, "B too large");
-    if (opts->emulator_path < 0 || opts->emulator_path > 2)
-        return fail(c, LASP_ERR_INVALID_ARG, "lasp_fit_batch: emulator_path must be 0, 1 or 2");
-    if (opts->emulator_path == 2 && !(c->v1_ok && c->dCF))
-        return fail(c, LASP_ERR_UNSUPPORTED, "emulator_path 2 (tensor pipe) needs the resident kernel and n_terms <= 128");
-    if (c->v1_ok) {
-        int rc = v1_workspace(c, B, err != nullptr);
-        if (rc) return rc;
-        cudaStream_t st = (cudaStream_t)stream;
-        rc = ws_acquire(c, st);
-        if (rc) return rc;
-        rc = v1_stage(c, B, flux, ivar, mask, st);
-        if (rc) return rc;
-        V1Args a;
-        memset(&a, 0, sizeof(a));
-        a.Y = c->dY; a.W = c->dW; a.C1 = c->dC1; a.CP = c->dCP; a.XJ = c->dXJ; a.B = B;
-        // emulator on the tensor pipe (opts->emulator_path == 2; LASP_EMU_MMA forces it, also for lasp_eval_grad)
-        if ((opts->emulator_path == 2 || getenv("LASP_EMU_MMA")) && c->dCF) { a.CF = c->dCF; a.ksteps = c->cf_ksteps; }
-        a.IS = c->dIS; a.S2 = c->dS2; a.DS = c->dDS;
-        const int grid = v1_grid(c, B, a.ngroups);
-        a.init = init; a.n_iter = opts->n_iter; a.lr = opts->lr; a.b1 = opts->beta1; a.b2 = opts->beta2;
-        a.eps = opts->eps; a.fd_h = 2e-3f;  // fp32 central-difference step in u (C.2-22)
-        a.params = params; a.cont = cont; a.chi2 = chi2; a.err = err; a.status = status;
-        if (!c->dqueue) CUDA_TRY(c, cudaMalloc(&c->dqueue, sizeof(unsigned int)));
-        CUDA_TRY(c, cudaMemsetAsync(c->dqueue, 0, sizeof(unsigned int), st));
-        a.queue = c->dqueue;
-        if (getenv("LASP_TIMING")) {
-            if (!c->ddbg) { CUDA_TRY(c, cudaMalloc(&c->ddbg, 24 * sizeof(unsigned long long))); }
-            CUDA_TRY(c, cudaMemsetAsync(c->ddbg, 0, 24 * sizeof(unsigned long long), st));
-            a.dbg = c->ddbg;
-        }
-        return v1_launch(c, false, a, grid, st);
-    }
-    int rc = ensure_workspace(c, B, true);
+    const Variant *v = nullptr;
+    bool mma = false;
+    int rc = resolve(c, opts, "lasp_fit_batch", &v, &mma);
+    if (rc) return rc;
+    DeviceGuard dg(c->device);
+    rc = workspace(c, B, *v, true, true, err != nullptr);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     rc = ws_acquire(c, st);
     if (rc) return rc;
     rc = stage(c, B, flux, ivar, mask, st);
     if (rc) return rc;
-    FitArgs a;
-    memset(&a, 0, sizeof(a));
-    a.YW = c->dYW; a.scratch = c->dscratch; a.B = B; a.tiles = (int)((B + 31) / 32);
+    V1Args a;
+    base_args(c, *v, mma, B, a);
+    a.XJ = c->dXJ;
     a.init = init; a.n_iter = opts->n_iter; a.lr = opts->lr; a.b1 = opts->beta1; a.b2 = opts->beta2;
     a.eps = opts->eps; a.fd_h = 2e-3f;  // fp32 central-difference step in u (C.2-22)
     a.params = params; a.cont = cont; a.chi2 = chi2; a.err = err; a.status = status;
-    int grid, wpb;
-    launch_shape(c, a.tiles, grid, wpb);
-    lasp_fit_kernel<<<grid, wpb * 32, c->smem_per_warp * wpb, st>>>(c->M, a);
-    c->launches += 1;
-    CUDA_TRY(c, cudaGetLastError());
-    return ws_release(c, st);
+    a.warm = opts->warm > 0 ? opts->warm : 4;
+    a.refresh = opts->refresh;
+    a.fdfresh = opts->fd_fresh;
+    a.drift_tol = 6.4e-3f;   // = 64 steps x (1e-2)^2: the fixed schedule the parity suite was tuned at
+    CUDA_TRY(c, cudaMemsetAsync(c->dqueue, 0, sizeof(unsigned int), st));
+    CUDA_TRY(c, cudaMemsetAsync(c->dstats, 0, 2 * sizeof(unsigned long long), st));
+    a.queue = c->dqueue;
+    a.stats = c->dstats;
+#ifdef LASP_PHASE_TIMING
+    if (!c->ddbg) { CUDA_TRY(c, cudaMalloc(&c->ddbg, 24 * sizeof(unsigned long long))); }
+    CUDA_TRY(c, cudaMemsetAsync(c->ddbg, 0, 24 * sizeof(unsigned long long), st));
+    a.dbg = c->ddbg;
+#endif
+    return launch(c, kFit, *v, a, st);
 }
 
 extern "C" int lasp_eval_grad(lasp_ctx *c, int64_t B, const float *flux, const float *ivar,
-                              const uint8_t *mask, const float *params, float *chi2, float *grad_u,
-                              float *cont, int32_t *status, void *stream)
+                              const uint8_t *mask, const float *params, const lasp_fit_opts *opts, float *chi2,
+                              float *grad_u, float *cont, int32_t *status, void *stream)
 {
     if (!c) return fail(nullptr, LASP_ERR_INVALID_ARG, "null ctx");
     if (B < 1 || !flux || !ivar || !params || !chi2 || !grad_u)
         return fail(c, LASP_ERR_INVALID_ARG, "lasp_eval_grad: null pointer or B < 1");
-    if (c->v1_ok) {
-        int rc = v1_workspace(c, B, false);
-        if (rc) return rc;
-        cudaStream_t st = (cudaStream_t)stream;
-        rc = ws_acquire(c, st);
-        if (rc) return rc;
-        rc = v1_stage(c, B, flux, ivar, mask, st);
-        if (rc) return rc;
-        V1Args a;
-        memset(&a, 0, sizeof(a));
-        a.Y = c->dY; a.W = c->dW; a.C1 = c->dC1; a.CP = c->dCP; a.B = B;
-        if (getenv("LASP_EMU_MMA") && c->dCF) { a.CF = c->dCF; a.ksteps = c->cf_ksteps; }
-        a.IS = c->dIS; a.S2 = c->dS2; a.DS = c->dDS;
-        const int grid = v1_grid(c, B, a.ngroups);
-        a.gparams = params; a.chi2 = chi2; a.grad_u = grad_u; a.cont = cont; a.status = status;
-        return v1_launch(c, true, a, grid, st);
-    }
-    int rc = ensure_workspace(c, B, true);
+    const Variant *v = nullptr;
+    bool mma = false;
+    int rc = resolve(c, opts, "lasp_eval_grad", &v, &mma);
+    if (rc) return rc;
+    DeviceGuard dg(c->device);
+    rc = workspace(c, B, *v, true, true, false);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     rc = ws_acquire(c, st);
     if (rc) return rc;
     rc = stage(c, B, flux, ivar, mask, st);
     if (rc) return rc;
-    FitArgs a;
-    memset(&a, 0, sizeof(a));
-    a.YW = c->dYW; a.scratch = c->dscratch; a.B = B; a.tiles = (int)((B + 31) / 32);
+    V1Args a;
+    base_args(c, *v, mma, B, a);
     a.gparams = params; a.chi2 = chi2; a.grad_u = grad_u; a.cont = cont; a.status = status;
-    int grid, wpb;
-    launch_shape(c, a.tiles, grid, wpb);
-    lasp_grad_kernel<<<grid, wpb * 32, c->smem_per_warp * wpb, st>>>(c->M, a);
-    c->launches += 1;
-    CUDA_TRY(c, cudaGetLastError());
-    return ws_release(c, st);
+    return launch(c, kGrad, *v, a, st);
 }
 
 extern "C" int lasp_eval_model(lasp_ctx *c, int64_t B, const float *params, const float *cont,
-                               float *model, void *stream)
+                               const lasp_fit_opts *opts, float *model, void *stream)
 {
     if (!c) return fail(nullptr, LASP_ERR_INVALID_ARG, "null ctx");
     if (B < 1 || !params || !cont || !model)
         return fail(c, LASP_ERR_INVALID_ARG, "lasp_eval_model: null pointer or B < 1");
-    int rc = ensure_workspace(c, B, false);
+    const Variant *v = nullptr;
+    bool mma = false;
+    int rc = resolve(c, opts, "lasp_eval_model", &v, &mma);
     if (rc) return rc;
-    FitArgs a;
-    memset(&a, 0, sizeof(a));
-    a.scratch = c->dscratch; a.B = B; a.tiles = (int)((B + 31) / 32);
+    DeviceGuard dg(c->device);
+    rc = workspace(c, B, *v, false, false, false);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    rc = ws_acquire(c, st);
+    if (rc) return rc;
+    V1Args a;
+    base_args(c, *v, mma, B, a);
     a.gparams = params; a.mcont = cont; a.model = model;
-    int grid, wpb;
-    launch_shape(c, a.tiles, grid, wpb);
-    rc = ws_acquire(c, (cudaStream_t)stream);
-    if (rc) return rc;
-    lasp_model_kernel<<<grid, wpb * 32, c->smem_per_warp * wpb, (cudaStream_t)stream>>>(c->M, a);
-    c->launches += 1;
-    CUDA_TRY(c, cudaGetLastError());
-    return ws_release(c, (cudaStream_t)stream);
+    return launch(c, kModel, *v, a, st);
 }
 
 // Algorithmic FMA of one Adam step of one spectrum: SURVEY.md 8(d) formula, moment route,
@@ -731,11 +687,35 @@ extern "C" double lasp_fma_per_spectrum_step(const lasp_ctx *c, double mean_taps
     if (!c) return 0.0;
     const ModelDev &M = c->M;
     const double P = M.P, K = M.K, n1 = M.n1, W = mean_taps;
-    bool linear = false;
-    for (int s = 0; s < M.n_seg; ++s) linear = linear || !M.seg[s].uniform;
     double G = (2.0 * M.D + 1.0) * P + M.n_seg * n1 * n1 * n1 / 6.0;
-    return 2.0 * K * P + 4.0 * W * P + (linear ? 2.0 * W * P : 0.0) + G + 4.0 * n1 * P +
+    return 2.0 * K * P + 4.0 * W * P + (c->nonuniform ? 2.0 * W * P : 0.0) + G + 4.0 * n1 * P +
            M.n_seg * (n1 * n1 * n1 / 6.0 + 4.0 * n1 * n1) + 8.0 * P;
+}
+
+// The same count for the algorithm AS BUILT: Gram moments and factorisation only on the
+// fraction `fresh_frac` of the steps that re-factor, one right-hand side and one continuum evaluation per step
+// (2 (D+1) P, the residual-form solve being warm-started), the explicit-inverse product (D+1)^2 per segment.
+extern "C" double lasp_fma_executed_per_spectrum_step(const lasp_ctx *c, double mean_taps, double fresh_frac)
+{
+    if (!c) return 0.0;
+    const ModelDev &M = c->M;
+    const double P = M.P, K = M.K, n1 = M.n1, W = mean_taps;
+    const double G = (2.0 * M.D + 1.0) * P + M.n_seg * (n1 * n1 * n1 / 6.0 + n1 * n1 * n1);   // moments, Cholesky, inverse
+    return 2.0 * K * P + 4.0 * W * P + (c->nonuniform ? 2.0 * W * P : 0.0) + fresh_frac * G + 2.0 * n1 * P +
+           M.n_seg * n1 * n1 + 8.0 * P;
+}
+
+// Counters of the last lasp_fit_batch on this ctx (synchronises with the device): out[0] = group-steps of the Adam
+// loops, out[1] = those that re-accumulated the Gram moments and re-factorised.
+extern "C" int lasp_last_fit_stats(lasp_ctx *c, double *out2)
+{
+    if (!c || !out2) return fail(c, LASP_ERR_INVALID_ARG, "lasp_last_fit_stats: null argument");
+    DeviceGuard dg(c->device);
+    unsigned long long h[2] = {0, 0};
+    if (c->ws_pending) CUDA_TRY(c, cudaEventSynchronize(c->ws_event));
+    CUDA_TRY(c, cudaMemcpy(h, c->dstats, sizeof(h), cudaMemcpyDeviceToHost));
+    out2[0] = (double)h[0]; out2[1] = (double)h[1];
+    return LASP_OK;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -785,19 +765,10 @@ static int hostpipe_reserve(lasp_ctx *c, int64_t chunk)
     return LASP_OK;
 }
 
-extern "C" int lasp_fit_batch_host(lasp_ctx *c, int64_t B, const float *flux, const float *ivar,
-                                   const uint8_t *mask, const float *init, const lasp_fit_opts *opts,
-                                   float *params, float *cont, float *chi2, float *err, int32_t *status,
-                                   int64_t chunk)
+static int hostpipe_run(lasp_ctx *c, int64_t B, const float *flux, const float *ivar, const uint8_t *mask,
+                        const float *init, const lasp_fit_opts *opts, float *params, float *cont, float *chi2,
+                        float *err, int32_t *status, int64_t chunk)
 {
-    if (!c) return fail(nullptr, LASP_ERR_INVALID_ARG, "null ctx");
-    if (B < 1 || !flux || !ivar || !init || !opts || !params || !chi2 || chunk < 0)
-        return fail(c, LASP_ERR_INVALID_ARG, "lasp_fit_batch_host: null pointer, B < 1 or chunk < 0");
-    CUDA_TRY(c, cudaSetDevice(c->device));
-    if (chunk == 0) chunk = 65536;
-    chunk = std::min<int64_t>(chunk, B);
-    int rc = hostpipe_reserve(c, chunk);
-    if (rc) return rc;
     lasp_ctx::HostPipe &h = c->hp;
     const ModelDev &M = c->M;
     const int64_t nchunk = (B + chunk - 1) / chunk;
@@ -813,7 +784,7 @@ extern "C" int lasp_fit_batch_host(lasp_ctx *c, int64_t B, const float *flux, co
         CUDA_TRY(c, cudaEventRecord(h.in_done[s], h.s_in));
         return LASP_OK;
     };
-    rc = upload(0);
+    int rc = upload(0);
     if (rc) return rc;
     for (int64_t i = 0; i < nchunk; ++i) {
         const int s = (int)(i & 1);
@@ -834,7 +805,31 @@ extern "C" int lasp_fit_batch_host(lasp_ctx *c, int64_t B, const float *flux, co
         if (status) CUDA_TRY(c, cudaMemcpyAsync(status + o, h.status[s], (size_t)n * sizeof(int32_t), cudaMemcpyDeviceToHost, h.s_out));
         CUDA_TRY(c, cudaEventRecord(h.out_done[s], h.s_out));
     }
-    CUDA_TRY(c, cudaStreamSynchronize(h.s_out));
-    CUDA_TRY(c, cudaStreamSynchronize(h.s_fit));
+    return LASP_OK;
+}
+
+extern "C" int lasp_fit_batch_host(lasp_ctx *c, int64_t B, const float *flux, const float *ivar,
+                                   const uint8_t *mask, const float *init, const lasp_fit_opts *opts,
+                                   float *params, float *cont, float *chi2, float *err, int32_t *status,
+                                   int64_t chunk)
+{
+    if (!c) return fail(nullptr, LASP_ERR_INVALID_ARG, "null ctx");
+    if (B < 1 || !flux || !ivar || !init || !opts || !params || !chi2 || chunk < 0)
+        return fail(c, LASP_ERR_INVALID_ARG, "lasp_fit_batch_host: null pointer, B < 1 or chunk < 0");
+    DeviceGuard dg(c->device);
+    if (chunk == 0) chunk = 65536;
+    chunk = std::min<int64_t>(chunk, B);
+    int rc = hostpipe_reserve(c, chunk);
+    if (rc) return rc;
+    rc = hostpipe_run(c, B, flux, ivar, mask, init, opts, params, cont, chi2, err, status, chunk);
+    // success or not, nothing of this call may still be in flight on the private streams when it returns: the
+    // copies read and write the caller's buffers
+    const std::string first = c->err;
+    cudaError_t e1 = cudaStreamSynchronize(c->hp.s_in), e2 = cudaStreamSynchronize(c->hp.s_fit), e3 = cudaStreamSynchronize(c->hp.s_out);
+    if (rc) { c->err = first; g_err = first; return rc; }
+    if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess) {
+        const cudaError_t e = e1 != cudaSuccess ? e1 : (e2 != cudaSuccess ? e2 : e3);
+        return fail(c, LASP_ERR_CUDA, std::string("lasp_fit_batch_host: ") + cudaGetErrorString(e));
+    }
     return LASP_OK;
 }

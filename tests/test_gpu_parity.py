@@ -3,6 +3,10 @@ same seeded inputs.  Tolerances are BASELINE.json north_star's, made operational
 C.4:  flux <= 1e-5 * median|model|;  gradient <= 1e-4 * |g|_inf;  continuum ratio <= 1e-4 on fitted
 pixels;  after the fit every parameter within 1e-3 of its prior range, chi2 within 1e-4 relative,
 errors within 1e-2 relative, status words equal.
+
+Every entry point is exercised on the kernels that are benchmarked: `lasp_eval_model`, `lasp_eval_grad` and
+`lasp_fit_batch` all run the group kernels of csrc/lasp_fit_v1.cuh, in the resident variant (variant 1) and in the
+streaming variant (variant 2), with the emulator on the FP32 pipe (emulator_path 1) and on the tensor pipe (2).
 """
 import numpy as np
 import pytest
@@ -47,20 +51,23 @@ def fit_weights(case, i):
     return w
 
 
-def check_model(gpu, oracle_mod, case):
+def check_model(gpu, oracle_mod, case, params=None, **kw):
+    """lasp_eval_model vs the oracle on EVERY pixel (edges included), at identical (theta, b)."""
     m = gpu.LaspModel(case["desc"])
-    got = m.eval_model(case["truth"], case["cont"]).cpu().numpy().astype(np.float64)
-    ref = oracle_mod.Oracle(case["desc"]).eval_model(case["truth"], case["cont"])
+    params = case["truth"] if params is None else params
+    got = m.eval_model(params, case["cont"], **kw).cpu().numpy().astype(np.float64)
+    ref = oracle_mod.Oracle(case["desc"]).eval_model(params, case["cont"])
     scale = np.median(np.abs(ref), axis=1, keepdims=True)
     err = np.abs(got - ref) / scale
     assert err.max() <= TOL_FLUX, err.max()
     m.close()
+    return got
 
 
-def check_grad(gpu, oracle_mod, case, params):
+def check_grad(gpu, oracle_mod, case, params, **kw):
     m = gpu.LaspModel(case["desc"])
     o = oracle_mod.Oracle(case["desc"])
-    g = m.eval_grad(case["flux"], case["ivar"], case["mask"], params)
+    g = m.eval_grad(case["flux"], case["ivar"], case["mask"], params, **kw)
     chi2, grad, cont, st = o.eval_grad(case["flux"], case["ivar"], case["mask"], params)
     gg = g["grad_u"].cpu().numpy().astype(np.float64)
     assert np.allclose(g["chi2"].cpu().numpy(), chi2, rtol=TOL_CHI2)
@@ -73,49 +80,101 @@ def check_grad(gpu, oracle_mod, case, params):
         assert np.abs(ratio - 1).max() <= TOL_CONT
     assert np.array_equal(g["status"].cpu().numpy(), st)
     m.close()
+    return gg
 
 
-def check_fit(gpu, oracle_mod, case, n_iter, lr=1e-2, want_err=True, emulator_path=0):
-    m = gpu.LaspModel(case["desc"])
-    o = oracle_mod.Oracle(case["desc"])
-    r = m.fit_batch(case["flux"], case["ivar"], case["mask"], case["init"], n_iter, lr=lr, want_err=want_err,
-                    emulator_path=emulator_path)
-    ref = o.fit(case["flux"], case["ivar"], case["mask"], case["init"], n_iter, lr=lr, want_err=want_err)
+def compare_fit(case, o, r, ref, want_err=True, tol_par=TOL_PAR, tol_chi2=TOL_CHI2):
     par = r["params"].cpu().numpy().astype(np.float64)
     dpar = np.abs(par - ref["params"]) / (o.hi - o.lo)
-    assert dpar.max() <= TOL_PAR, dpar.max(axis=0)
+    assert dpar.max() <= tol_par, dpar.max(axis=0)
     chi = r["chi2"].cpu().numpy().astype(np.float64)
     good = ref["chi2"] > 0
-    assert np.abs(chi[good] / ref["chi2"][good] - 1).max() <= TOL_CHI2
+    assert np.abs(chi[good] / ref["chi2"][good] - 1).max() <= tol_chi2
     assert np.array_equal(r["status"].cpu().numpy(), ref["status"])
+    # Continuum: the WLS solution is a function of the parameters, so like the flux it is compared AT IDENTICAL
+    # PARAMETERS -- the oracle's solve at the parameters the kernel returned -- at 1e-4 on every fitted pixel.  (Against
+    # the oracle's OWN final iterate a parameter difference the 1e-3 tolerance allows moves the edge of a degree-30
+    # continuum by more than 1e-4: measured 1.9e-4 for dparam = 6e-4 on config-4 shapes with a fresh factor on every
+    # step; that comparison is therefore held to the parameter tolerance, 1e-3.)
+    n = ref["params"].shape[0]
     gc = r["cont"].cpu().numpy().astype(np.float64)
-    for i in range(case["B"]):
+    same = o.eval_grad(case["flux"][:n], case["ivar"][:n], case["mask"][:n], par)[2]
+    for i in range(n):
         w = fit_weights(case, i)
-        if ref["status"][i] & 1 or not (w > 0).any():
+        if ref["status"][i] & 3 or not (w > 0).any():
             continue
-        ratio = cont_values(case["desc"], gc, i)[w > 0] / cont_values(case["desc"], ref["cont"], i)[w > 0]
+        cg = cont_values(case["desc"], gc, i)[w > 0]
+        ratio = cg / cont_values(case["desc"], same, i)[w > 0]
         assert np.abs(ratio - 1).max() <= TOL_CONT, (i, np.abs(ratio - 1).max())
+        ratio = cg / cont_values(case["desc"], ref["cont"], i)[w > 0]
+        assert np.abs(ratio - 1).max() <= max(TOL_PAR, tol_par), (i, np.abs(ratio - 1).max())
     if want_err:
         e = r["err"].cpu().numpy().astype(np.float64)
         ok = np.isfinite(ref["err"]).all(axis=1)
         assert np.array_equal(np.isfinite(e).all(axis=1), ok)
         assert np.abs(e[ok] / ref["err"][ok] - 1).max() <= TOL_ERR, np.abs(e[ok] / ref["err"][ok] - 1).max(axis=0)
+
+
+def check_fit(gpu, oracle_mod, case, n_iter, lr=1e-2, want_err=True, **kw):
+    m = gpu.LaspModel(case["desc"])
+    o = oracle_mod.Oracle(case["desc"])
+    r = m.fit_batch(case["flux"], case["ivar"], case["mask"], case["init"], n_iter, lr=lr, want_err=want_err, **kw)
+    ref = o.fit(case["flux"], case["ivar"], case["mask"], case["init"], n_iter, lr=lr, want_err=want_err)
+    compare_fit(case, o, r, ref, want_err)
     m.close()
     return r, ref
 
 
-# ------------------------------------------------------------------ forward model
+def widest_params(case):
+    """|v| and sigma* near the edge of the prior box: the widest supports the layout allows."""
+    B, L = case["B"], case["desc"]["n_labels"]
+    params = case["init"].copy()
+    params[:, L] = np.where(np.arange(B) % 2 == 0, 390.0, -385.0)
+    params[:, L + 1] = np.linspace(250.0, 298.0, B)
+    return params
 
-def test_model_flux_config0(gpu, oracle_mod):
-    check_model(gpu, oracle_mod, synth.make_case(0, oracle_mod.forward, B=64))
+
+# ------------------------------------------------------------------ forward model (lasp_eval_model, group kernels)
+# north_star: model flux relative error <= 1e-5, Eq. 5 P:113-115, Eq. 6 P:121-129
+
+@pytest.mark.parametrize("path", [1, 2])
+def test_model_flux_config0(gpu, oracle_mod, path):
+    check_model(gpu, oracle_mod, synth.make_case(0, oracle_mod.forward, B=64), emulator_path=path)
 
 
-def test_model_flux_two_arm_linear(gpu, oracle_mod):
-    check_model(gpu, oracle_mod, make(two_arm_config(), oracle_mod, B=37))
+@pytest.mark.parametrize("path", [1, 2])
+def test_model_flux_config1_widest_support(gpu, oracle_mod, path):
+    """config-1 shapes at the widest supports of the prior box (H = 28): the T range takes two sweeps of the CTA."""
+    case = synth.make_case(1, oracle_mod.forward, B=9)
+    check_model(gpu, oracle_mod, case, emulator_path=path)
+    check_model(gpu, oracle_mod, case, params=widest_params(case), emulator_path=path)
 
 
-def test_model_flux_config2_desi_shape(gpu, oracle_mod):
-    check_model(gpu, oracle_mod, synth.make_case(2, oracle_mod.forward, B=8))
+@pytest.mark.parametrize("path", [1, 2])
+def test_model_flux_two_arm_linear(gpu, oracle_mod, path):
+    check_model(gpu, oracle_mod, make(two_arm_config(), oracle_mod, B=37), emulator_path=path)
+
+
+@pytest.mark.parametrize("path", [1, 2])
+def test_model_flux_config2_desi_shape(gpu, oracle_mod, path):
+    case = synth.make_case(2, oracle_mod.forward, B=8)
+    check_model(gpu, oracle_mod, case, emulator_path=path)
+    check_model(gpu, oracle_mod, case, params=widest_params(case), emulator_path=path)
+
+
+@pytest.mark.parametrize("path", [1, 2])
+def test_model_flux_config4_high_dim(gpu, oracle_mod, path):
+    check_model(gpu, oracle_mod, synth.make_case(4, oracle_mod.forward, B=6), emulator_path=path)
+
+
+def test_model_flux_streaming_variant(gpu, oracle_mod):
+    """variant 2 on shapes that also run resident: config 0, the two-arm linear grid, config 2, and bit-for-bit the same
+    stencil inputs give the same flux to rounding order."""
+    for case in (synth.make_case(0, oracle_mod.forward, B=13), make(two_arm_config(), oracle_mod, B=5),
+                 synth.make_case(2, oracle_mod.forward, B=5)):
+        a = check_model(gpu, oracle_mod, case, variant=2)
+        b = check_model(gpu, oracle_mod, case, variant=1)
+        assert np.abs(a - b).max() <= 2e-6 * np.abs(b).max()
 
 
 # ------------------------------------------------------------------ chi2 + gradient
@@ -126,7 +185,7 @@ def test_grad_config0(gpu, oracle_mod):
 
 
 def test_grad_config1_masked(gpu, oracle_mod):
-    case = synth.make_case(1, oracle_mod.forward, B=40)  # ragged: one full tile + 8
+    case = synth.make_case(1, oracle_mod.forward, B=40)  # ragged: ten groups of four
     check_grad(gpu, oracle_mod, case, case["init"])
 
 
@@ -144,16 +203,24 @@ def test_grad_widest_kernels_need_two_sweeps(gpu, oracle_mod):
     """|v| and sigma* near the edge of the prior box: support H = 28, the T range no longer fits one sweep of the
     CTA's 192 threads (config-1 shapes), so the emulator / adjoint loops take their second pass."""
     case = synth.make_case(1, oracle_mod.forward, B=9)
-    params = case["init"].copy()
-    L = case["desc"]["n_labels"]
-    params[:, L] = np.where(np.arange(9) % 2 == 0, 390.0, -385.0)
-    params[:, L + 1] = np.linspace(250.0, 298.0, 9)
-    check_grad(gpu, oracle_mod, case, params)
+    check_grad(gpu, oracle_mod, case, widest_params(case))
 
 
 def test_grad_two_arm_log_grid(gpu, oracle_mod):
     case = make(two_arm_log_config(), oracle_mod, B=6)   # several uniform segments: slots do not alias
     check_grad(gpu, oracle_mod, case, case["init"])
+
+
+def test_grad_streaming_variant(gpu, oracle_mod):
+    """variant 2 (rows in global scratch, shared-memory window per sweep) on config-1 shapes incl. the widest supports,
+    on several uniform segments and on a linear grid."""
+    case = synth.make_case(1, oracle_mod.forward, B=10)
+    check_grad(gpu, oracle_mod, case, case["init"], variant=2)
+    check_grad(gpu, oracle_mod, case, widest_params(case), variant=2)
+    case = make(two_arm_log_config(), oracle_mod, B=6)
+    check_grad(gpu, oracle_mod, case, case["init"], variant=2)
+    case = make(two_arm_config(), oracle_mod, B=5)
+    check_grad(gpu, oracle_mod, case, case["init"], variant=2)
 
 
 # ------------------------------------------------------------------ full fits
@@ -179,15 +246,69 @@ def test_fit_two_arm_log_grid(gpu, oracle_mod):
     check_fit(gpu, oracle_mod, case, 60)
 
 
-def test_fit_config4_subset(gpu, oracle_mod):
-    case = synth.make_case(4, oracle_mod.forward, B=5)   # K = 105, 13 labels, three linear-grid arms
-    check_fit(gpu, oracle_mod, case, 40)
+@pytest.mark.slow
+def test_fit_config2_first_64_at_500_steps(gpu, oracle_mod):
+    """config 2 (DESI three-arm, per-pixel kernels), first 64 spectra, all 500 Adam steps."""
+    case = synth.make_case(2, oracle_mod.forward, B=64)
+    check_fit(gpu, oracle_mod, case, case["config"].n_iter)
 
 
 @pytest.mark.slow
-def test_fit_config2_subset(gpu, oracle_mod):
-    case = synth.make_case(2, oracle_mod.forward, B=8)
-    check_fit(gpu, oracle_mod, case, 100)
+@pytest.mark.parametrize("path", [1, 2])
+def test_fit_config4_first_64_at_300_steps(gpu, oracle_mod, path):
+    """config 4 (K = 105, 13 labels, three linear-grid arms), first 64 spectra, all 300 steps, emulator on
+    the FP32 pipe and on the tensor pipe: the run crosses several mid-run re-factorisations."""
+    case = synth.make_case(4, oracle_mod.forward, B=64)
+    check_fit(gpu, oracle_mod, case, case["config"].n_iter, emulator_path=path)
+
+
+# ------------------------------------------------------------------ the stale-factor steps (DESIGN.md "Stale Gram factor")
+
+@pytest.mark.parametrize("policy", [dict(refresh=64), dict(refresh=0), dict(refresh=1)])
+def test_iterates_across_refactorisations(gpu, oracle_mod, policy):
+    """The iterate u_t itself (not only the end of the fit) against the oracle's at the same t, ten times inside the
+    parameter tolerance, for step counts just before, at and after the re-factorisation steps of the fixed schedule
+    (fresh on t <= 4 and t = 65, 129): t = 20, 40, 63, 64 end on stale steps up to 60 after a factor, 65, 66 and 129
+    right after one.  chi2 at an iterate that has NOT converged magnifies a parameter difference by the (large)
+    gradient there: with a stale factor it is held to 1e-3 mid-run (measured <= 3e-4 at t = 20..66, DESIGN.md
+    "Stale Gram factor"), with a fresh factor on every step (refresh = 1, the method as written) to the 1e-4 of the
+    converged fits."""
+    case = synth.make_case(1, oracle_mod.forward, B=8)
+    m = gpu.LaspModel(case["desc"])
+    o = oracle_mod.Oracle(case["desc"])
+    for n_iter in (1, 5, 20, 40, 63, 64, 65, 66, 129):
+        r = m.fit_batch(case["flux"], case["ivar"], case["mask"], case["init"], n_iter, **policy)
+        ref = o.fit(case["flux"], case["ivar"], case["mask"], case["init"], n_iter)
+        compare_fit(case, o, r, ref, tol_par=1e-4, tol_chi2=TOL_CHI2 if policy["refresh"] == 1 else 1e-3)
+    st = m.last_fit_stats()
+    assert st["group_steps"] == 2 * 129
+    expect = {64: 2 * 6, 1: 2 * 129}.get(policy["refresh"])   # warm steps 1-4, then t = 65 and 129
+    if expect is not None:
+        assert st["fresh_steps"] == expect
+    else:
+        assert 2 * 5 <= st["fresh_steps"] <= 2 * 129
+    m.close()
+
+
+def test_fit_at_the_papers_learning_rate(gpu, oracle_mod):
+    """lr = 0.1 for 80 steps, before Adam's late-time bursts make fp32 and fp64 trajectories diverge (SURVEY.md
+    section 7): per-step changes are 10x those of the configs, so the adaptive policy must re-factorise far more
+    often than every 64th step, and the fit stays inside the tolerances."""
+    case = synth.make_case(1, oracle_mod.forward, B=16)
+    m = gpu.LaspModel(case["desc"])
+    o = oracle_mod.Oracle(case["desc"])
+    r = m.fit_batch(case["flux"], case["ivar"], case["mask"], case["init"], 80, lr=0.1)
+    ref = o.fit(case["flux"], case["ivar"], case["mask"], case["init"], 80, lr=0.1)
+    compare_fit(case, o, r, ref)
+    st = m.last_fit_stats()
+    assert st["fresh_frac"] > 0.1
+    m.close()
+
+
+def test_fit_linear_grid_long_enough_to_refactor(gpu, oracle_mod):
+    """A linear-grid (per-pixel-kernel) fit of 140 steps on config-2 shapes: crosses the re-factorisations at 65 and 129."""
+    case = synth.make_case(2, oracle_mod.forward, B=4)
+    check_fit(gpu, oracle_mod, case, 140, refresh=64)
 
 
 # ------------------------------------------------------------------ edge cases
@@ -212,18 +333,50 @@ def test_status_bits_and_all_masked(gpu, oracle_mod):
 
 
 def test_masked_pixels_do_not_leak(gpu, oracle_mod):
+    """Flux on pixels with w == 0 is never looked at -- not even when it is NaN or Inf (reading R-1)."""
     case = make(small_config(mask_frac=0.1), oracle_mod, B=2)
     m = gpu.LaspModel(case["desc"])
     a = m.eval_grad(case["flux"], case["ivar"], case["mask"], case["init"])
     f2 = case["flux"].copy()
     f2[case["mask"] == 0] = -77.0
+    f2[0, np.flatnonzero(case["mask"][0] == 0)[:3]] = [np.nan, np.inf, -np.inf]
+    f2[:, :5] = np.nan                       # excluded edge pixels
     b = m.eval_grad(f2, case["ivar"], case["mask"], case["init"])
+    assert np.isfinite(a["chi2"].cpu().numpy()).all()
     assert np.array_equal(a["chi2"].cpu().numpy(), b["chi2"].cpu().numpy())
     assert np.array_equal(a["grad_u"].cpu().numpy(), b["grad_u"].cpu().numpy())
     m.close()
 
 
-def test_bad_arguments_return_error_codes(gpu):
+def test_nonfinite_input_sets_status_bit_2(gpu, oracle_mod):
+    """LASP_ST_NONFINITE on both sides.  Spectrum 0: an infinite weight on a fitted pixel, no Adam step (chi2 = inf,
+    system not positive definite).  Spectrum 1: a NaN flux on a fitted pixel with Adam steps -- the gradient is NaN and
+    the iterate becomes NaN in the oracle (lasp_oracle.c orc_adam_step) and in the kernel alike: parameters and chi2
+    come back NaN with the same status word.  Spectrum 2 is healthy and shares spectrum 1's CTA group: untouched."""
+    case = make(small_config(), oracle_mod, B=3)
+    o = oracle_mod.Oracle(case["desc"])
+    j = case["desc"]["n_pix"] // 2
+    case["mask"][:, j] = 1
+    iv = case["ivar"].copy(); iv[0, j] = np.inf
+    fl = case["flux"].copy(); fl[1, j] = np.nan
+    m = gpu.LaspModel(case["desc"])
+    for n_iter, flux, ivar in ((0, case["flux"], iv), (6, fl, case["ivar"])):
+        r = m.fit_batch(flux, ivar, case["mask"], case["init"], n_iter)
+        ref = o.fit(flux, ivar, case["mask"], case["init"], n_iter)
+        st = r["status"].cpu().numpy()
+        assert np.array_equal(st, ref["status"]), (st, ref["status"])
+        bad = 0 if n_iter == 0 else 1
+        assert st[bad] & gpu.LASP_ST_NONFINITE and not (st[2] & gpu.LASP_ST_NONFINITE)
+        par = r["params"].cpu().numpy()
+        assert np.array_equal(np.isnan(par), np.isnan(ref["params"]))
+        assert not np.isfinite(r["chi2"][bad].item()) and not np.isfinite(ref["chi2"][bad])
+        good = [i for i in range(3) if i != bad]
+        assert (np.abs(par[good] - ref["params"][good]) / (o.hi - o.lo)).max() <= TOL_PAR
+        assert np.abs(r["chi2"].cpu().numpy()[good] / ref["chi2"][good] - 1).max() <= TOL_CHI2
+    m.close()
+
+
+def test_bad_arguments_return_error_codes(gpu, oracle_mod):
     d = synth.make_model_desc(synth.CONFIGS[0]); d.pop("_rng")
     d2 = dict(d); d2["cont_degree"] = 40
     with pytest.raises(gpu.LaspError):
@@ -231,16 +384,25 @@ def test_bad_arguments_return_error_codes(gpu):
     d3 = dict(d); d3["hi"] = d["lo"].copy()
     with pytest.raises(gpu.LaspError):
         gpu.LaspModel(d3)          # lo >= hi
+    case = make(small_config(), oracle_mod, B=2)
+    m = gpu.LaspModel(case["desc"])
+    for bad in (dict(variant=3), dict(emulator_path=3), dict(refresh=-1), dict(fd_fresh=2),
+                dict(variant=2, emulator_path=2)):           # the tensor-pipe emulator exists in the resident variant only
+        with pytest.raises(gpu.LaspError):
+            m.fit_batch(case["flux"], case["ivar"], case["mask"], case["init"], 1, **bad)
+    m.close()
 
 
 # ------------------------------------------------------------------ emulator on the tensor pipe (emulator_path = 2)
 
-def test_grad_tensor_pipe_emulator(gpu, oracle_mod, monkeypatch):
-    """chi2 / gradient / continuum with T = phi.C formed by mma.sync TF32 on split operands (lasp_eval_grad has no
-    options argument: the LASP_EMU_MMA switch selects the path), ragged batch, masked pixels."""
-    monkeypatch.setenv("LASP_EMU_MMA", "1")
+def test_grad_tensor_pipe_emulator(gpu, oracle_mod):
+    """chi2 / gradient / continuum with T = phi.C formed by mma.sync TF32 on split operands, ragged batch, masked pixels."""
     case = synth.make_case(1, oracle_mod.forward, B=40)
-    check_grad(gpu, oracle_mod, case, case["init"])
+    g2 = check_grad(gpu, oracle_mod, case, case["init"], emulator_path=2)
+    g1 = check_grad(gpu, oracle_mod, case, case["init"], emulator_path=1)
+    assert not np.array_equal(g1, g2)      # the two paths round differently: path 2 did not silently run path 1
+    case = synth.make_case(4, oracle_mod.forward, B=6)     # K = 105: 14 k-steps in four register chunks
+    check_grad(gpu, oracle_mod, case, case["init"], emulator_path=2)
 
 
 def test_fit_tensor_pipe_emulator(gpu, oracle_mod):
@@ -250,20 +412,8 @@ def test_fit_tensor_pipe_emulator(gpu, oracle_mod):
     r2, _ = check_fit(gpu, oracle_mod, case, case["config"].n_iter, emulator_path=2)
     m = gpu.LaspModel(case["desc"])
     r1 = m.fit_batch(case["flux"], case["ivar"], case["mask"], case["init"], case["config"].n_iter, emulator_path=1)
-    # the two paths round differently, so they must not be bit-identical (else path 2 silently ran path 1) ...
     assert not np.array_equal(r1["params"].cpu().numpy(), r2["params"].cpu().numpy())
-    # ... and a model the tensor-pipe path does not cover refuses it instead of falling back
-    with pytest.raises(gpu.LaspError):
-        m.fit_batch(case["flux"], case["ivar"], case["mask"], case["init"], 1, emulator_path=3)
     m.close()
-
-
-def test_tensor_pipe_emulator_config4_high_dim(gpu, oracle_mod, monkeypatch):
-    """K = 105 terms, 13 labels, three linear-grid arms: 14 k-steps in four register chunks; gradient and a short fit."""
-    case = synth.make_case(4, oracle_mod.forward, B=6)
-    check_fit(gpu, oracle_mod, case, 40, emulator_path=2)
-    monkeypatch.setenv("LASP_EMU_MMA", "1")
-    check_grad(gpu, oracle_mod, case, case["init"])
 
 
 # ------------------------------------------------------------------ host pipeline (config 3 path)
@@ -284,17 +434,43 @@ def test_fit_batch_host_matches_device_call(gpu, oracle_mod):
     m.close()
 
 
+@pytest.mark.slow
+def test_fit_config3_stream_first_and_last_chunk_vs_oracle(gpu, oracle_mod):
+    """BASELINE.json config 3 in miniature: ten chunks streamed from pinned host memory through lasp_fit_batch_host, all
+    500 Adam steps; the first 128 spectra of chunk 0 and of chunk 9 are compared with the oracle."""
+    import torch
+    cfg = synth.CONFIGS[3]
+    base = synth.make_case(3, oracle_mod.forward, B=256)
+    chunk, nchunk = 384, 10
+    idx = np.arange(chunk * nchunk) % 256
+    idx[:128] = np.arange(128)                                   # chunk 0 starts with base spectra 0..127
+    idx[9 * chunk:9 * chunk + 128] = np.arange(128, 256)         # chunk 9 with base spectra 128..255
+    m = gpu.LaspModel(base["desc"])
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a[idx])).pin_memory()
+    r = m.fit_batch_host(pin(base["flux"]), pin(base["ivar"]), pin(base["mask"]), pin(base["init"]), cfg.n_iter,
+                         lr=cfg.lr, chunk=chunk)
+    o = oracle_mod.Oracle(base["desc"])
+    ref = o.fit(base["flux"], base["ivar"], base["mask"], base["init"], cfg.n_iter, lr=cfg.lr)
+    for lo, sel in ((0, slice(0, 128)), (9 * chunk, slice(128, 256))):
+        sub = {k: (v[lo:lo + 128] if v is not None else None) for k, v in r.items()}
+        subcase = dict(base, flux=base["flux"][sel], ivar=base["ivar"][sel], mask=base["mask"][sel])
+        subref = {k: v[sel] for k, v in ref.items()}
+        compare_fit(subcase, o, sub, subref)
+    m.close()
+
+
 # ------------------------------------------------------------------ full size, bench launch configuration
 
 @pytest.mark.slow
 def test_fit_config1_full_size_sampled(gpu, oracle_mod):
-    """BASELINE.json config 1 at full size (B = 65,536, 500 Adam steps, the grid bench.py launches): the batch is
-    32 oracle-generated spectra tiled 2048 times; sampled rows across the batch (first, ragged middle, last CTA)
+    """BASELINE.json config 1 at full size (B = 65,536, 500 Adam steps, the grid bench.py launches): the batch is 256
+    DISTINCT oracle-generated spectra tiled 256 times; sampled rows across the batch (first, ragged middle, last CTA)
     are compared with the oracle one by one, and every copy of a spectrum must give the same result."""
     import torch
     cfg = synth.CONFIGS[1]
-    base = synth.make_case(1, oracle_mod.forward, B=32)
-    reps = cfg.B // 32
+    nb = 256
+    base = synth.make_case(1, oracle_mod.forward, B=nb)
+    reps = cfg.B // nb
     m = gpu.LaspModel(base["desc"])
     dev = m.device
     tile = lambda a: torch.from_numpy(a).to(dev).repeat(reps, *([1] * (a.ndim - 1)))
@@ -305,15 +481,15 @@ def test_fit_config1_full_size_sampled(gpu, oracle_mod):
     err = r["err"].cpu().numpy().astype(np.float64)
     st = r["status"].cpu().numpy()
     # property that holds at any size: identical inputs give identical outputs wherever they sit in the grid
-    assert np.array_equal(par.reshape(reps, 32, -1), np.broadcast_to(par[:32], (reps, 32, par.shape[1])))
-    assert np.array_equal(chi.reshape(reps, 32), np.broadcast_to(chi[:32], (reps, 32)))
-    sample = [0, 5, 13, 31, 32 * 1000 + 7, 32 * 1777 + 18, cfg.B - 32 + 2, cfg.B - 1]
-    idx = sorted({i % 32 for i in sample})
+    assert np.array_equal(par.reshape(reps, nb, -1), np.broadcast_to(par[:nb], (reps, nb, par.shape[1])))
+    assert np.array_equal(chi.reshape(reps, nb), np.broadcast_to(chi[:nb], (reps, nb)))
+    sample = [0, 5, 77, 255, nb * 100 + 131, nb * 177 + 18, nb * 201 + 200, cfg.B - nb + 2, cfg.B - 1] + list(range(32, 64))
+    idx = sorted({i % nb for i in sample})
     o = oracle_mod.Oracle(base["desc"])
     ref = o.fit(base["flux"][idx], base["ivar"][idx], base["mask"][idx], base["init"][idx], cfg.n_iter, lr=cfg.lr)
     pos = {j: n for n, j in enumerate(idx)}
     for i in sample:
-        n = pos[i % 32]
+        n = pos[i % nb]
         assert (np.abs(par[i] - ref["params"][n]) / (o.hi - o.lo)).max() <= TOL_PAR, i
         assert abs(chi[i] / ref["chi2"][n] - 1) <= TOL_CHI2, i
         assert np.abs(err[i] / ref["err"][n] - 1).max() <= TOL_ERR, i
@@ -323,14 +499,32 @@ def test_fit_config1_full_size_sampled(gpu, oracle_mod):
 
 # ------------------------------------------------------------------ streaming variant (rows too long for shared memory)
 
-def test_fit_long_spectrum_uses_streaming_variant(gpu, oracle_mod):
-    """SURVEY.md 8(d) shape "S" (one 17.4 k-pixel segment): its rows do not fit the fused kernel's shared memory, so
-    the library falls back to the lane-per-spectrum kernel with work arrays in global memory; same parity bar."""
-    case = synth.make_case("S", oracle_mod.forward, B=3)
+def test_streaming_variant_fits_match_oracle_on_resident_shapes(gpu, oracle_mod):
+    """variant 2 forced on shapes the resident variant also takes: config 0 in full, a config-1 subset over all 500
+    steps, a two-segment log grid and a linear grid."""
+    case = synth.make_case(0, oracle_mod.forward)
+    check_fit(gpu, oracle_mod, case, case["config"].n_iter, variant=2)
+    case = synth.make_case(1, oracle_mod.forward, B=12)
+    check_fit(gpu, oracle_mod, case, case["config"].n_iter, variant=2)
+    case = make(two_arm_log_config(n_iter=60), oracle_mod, B=7)
+    check_fit(gpu, oracle_mod, case, 60, variant=2)
+    case = make(two_arm_config(n_iter=120), oracle_mod, B=9)
+    check_fit(gpu, oracle_mod, case, 120, variant=2)
+
+
+@pytest.mark.slow
+def test_fit_long_spectrum_streaming_16_at_100_steps(gpu, oracle_mod):
+    """SURVEY.md 8(d) shape "S" (one 17.4 k-pixel segment): its rows do not fit shared memory, so the default variant
+    is the streaming one; first 16 spectra, 100 Adam steps, flux and gradient parity included."""
+    case = synth.make_case("S", oracle_mod.forward, B=16)
     m = gpu.LaspModel(case["desc"])
-    assert not m.uses_v1()
+    assert m.default_variant() == 2 and not m.launch_info(1)["available"]
+    with pytest.raises(gpu.LaspError):
+        m.fit_batch(case["flux"], case["ivar"], case["mask"], case["init"], 1, variant=1)
     m.close()
-    check_fit(gpu, oracle_mod, case, 15)
+    check_model(gpu, oracle_mod, case)
+    check_grad(gpu, oracle_mod, case, case["init"])
+    check_fit(gpu, oracle_mod, case, case["config"].n_iter)
     m1 = gpu.LaspModel(synth.make_case(0, oracle_mod.forward, B=1)["desc"])
-    assert m1.uses_v1()
+    assert m1.default_variant() == 1
     m1.close()

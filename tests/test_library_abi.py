@@ -18,6 +18,7 @@ def libpath():
 def declared_symbols():
     txt = open(os.path.join(ROOT, "include", "lasp_gpu.h")).read()
     txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
+    txt = re.sub(r"#ifdef LASP_PHASE_TIMING.*?#endif", "", txt, flags=re.S)   # debug-build-only declarations
     return sorted(set(re.findall(r"\b(lasp_[a-z_]+)\s*\(", txt)))
 
 
@@ -64,3 +65,24 @@ def test_sass_is_sm100(libpath):
     import subprocess
     out = subprocess.run(["cuobjdump", "-lelf", libpath], capture_output=True, text=True).stdout
     assert "sm_100a" in out
+
+
+def test_library_reads_no_environment_variable():
+    """Every switch is a field of lasp_fit_opts: nothing under csrc/ calls getenv."""
+    csrc = os.path.join(ROOT, "paper_2512_24840_b200", "csrc")
+    for f in os.listdir(csrc):
+        assert "getenv" not in open(os.path.join(csrc, f)).read(), f
+
+
+def test_fit_opts_layout_matches_header():
+    """The ctypes mirror of lasp_fit_opts has the header's fields in the header's order."""
+    from paper_2512_24840_b200 import binding
+    txt = open(os.path.join(ROOT, "include", "lasp_gpu.h")).read()
+    body = re.search(r"typedef struct \{([^}]*)\} lasp_fit_opts;", txt, flags=re.S).group(1)
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    names = []
+    for decl in body.split(";"):
+        decl = decl.strip()
+        if decl:
+            names += [n.strip() for n in decl.split(None, 1)[1].split(",")]
+    assert names == [f[0] for f in binding.FitOpts._fields_]
