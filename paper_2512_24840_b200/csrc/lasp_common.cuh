@@ -21,7 +21,7 @@ struct SegDev {
     int uniform;  // 1: constant km/s per pixel (log grid) -> one kernel per spectrum per step
     float inv_s;  // 1/s (pixels per km/s) when uniform, else the LARGEST 1/s_j of the segment
     float sig_inst;
-    float ta, tb; // Chebyshev node t = ta*(jp - po - halo) + tb, t in [-1,1] over the fitted pixels
+    float ta, tb; // ta = tm = 1/(fit_hi - fit_lo - 1): Chebyshev node t = tm (2 (jp - fit_lo) - (fit_hi - fit_lo - 1)); tb unused
 };
 
 struct ModelDev {

@@ -99,13 +99,29 @@ struct V1Np {          // per-spectrum scalars of a per-pixel-kernel segment
 #define SLOT_STAT(L_) ((L_).VR - 6)   // chi2, ngood, min c, dchi2/dv and dchi2/dsigma* of per-pixel-kernel segments
 
 // per-spectrum scalars in shared memory: SC[idx][GS]
-enum { SC_V = 0, SC_SIG, SC_CHI, SC_NGOOD, SC_CMIN, SC_GV, SC_GS, SC_FAIL, SC_DU, SC_N };   // SC_DU: |du|_inf of the last Adam update
+enum { SC_V = 0, SC_SIG, SC_CHI, SC_NGOOD, SC_CMIN, SC_GV, SC_GS, SC_FAIL, SC_N };
 
 // 32 values per lane -> lane l returns the warp total of value l (31 shuffles)
 __device__ __forceinline__ float xreduce32(float (&x)[32], int lane)
 {
 #pragma unroll
     for (int s = 16; s >= 1; s >>= 1) {
+        const bool up = (lane & s) != 0;
+#pragma unroll
+        for (int i = 0; i < s; ++i) {
+            float send = up ? x[i] : x[i + s];
+            float keep = up ? x[i + s] : x[i];
+            x[i] = keep + __shfl_xor_sync(FULL, send, s);
+        }
+    }
+    return x[0];
+}
+
+// 16 values per lane -> lane l returns the total of value (l & 15) over the 16 lanes of its half-warp (15 shuffles)
+__device__ __forceinline__ float xreduce16(float (&x)[16], int lane)
+{
+#pragma unroll
+    for (int s = 8; s >= 1; s >>= 1) {
         const bool up = (lane & s) != 0;
 #pragma unroll
         for (int i = 0; i < s; ++i) {
@@ -141,6 +157,8 @@ struct V1Block {
     float drift;          // sum of |du|_inf over the steps since the last fresh Gram factor
     int since;            // steps since the last fresh Gram factor
     int momflag;          // this evaluation re-factorises (written after its first barrier, read after its second)
+    int stepmax;          // max over the group of |du|_inf of the last update, as the bits of a non-negative float (atomicMax)
+    unsigned failmask;    // bit seg * GS + g: the last factorisation of that system was not positive definite
     unsigned int nfresh;  // fresh Adam steps of the current group (statistics)
 };
 __shared__ V1Block v1_blk;
@@ -691,6 +709,126 @@ __device__ __noinline__ void v1_phase_emulator_mma(const SegDev &sg, int lo, int
 }
 
 // ------------------------------------------------------------------------------------------
+// Which octet of the fitted range a thread owns in the phases that work with the continuum basis (forward, moments,
+// residual), and the Chebyshev nodes.
+//
+// The internal basis T_n(t) lives on the symmetric nodes  t_j = (2 (j - fit_lo) - (N - 1)) / (N - 1), N = fit_hi - fit_lo
+// (an even number of octets, lasp_gpu.cu), so that the pixel mirrored about the centre of the fitted range has the
+// node -t_j EXACTLY (odd integer numerators), and T_n(-t) = (-1)^n T_n(t).
+//
+// SYM (resident variant): lanes l < 16 and 31 - l of a warp own the mirrored octets p and Noct - 1 - p (pair p = sweep *
+// nt/2 + 16 warp + l).  A sum over both octets  sum_j v_j T_n(t_j)  is then  sum_i T_n(t_i) [v_i + (-1)^n v'_(7-i)]  in
+// one lane's own nodes: lane l takes the even n with v + v', lane 31 - l the odd n with v' - v (its own nodes), each
+// HALF of the basis; a continuum evaluation likewise splits into E(t) = sum_even b_n T_n, O(t) = sum_odd b_n T_n with
+// c(t) = E + O, c(-t) = E - O.  The exchange is 32 shuffles with lane ^ 31.  Halves the FMAs, the recurrences and the
+// transposes of the right-hand side, the moments and the continuum evaluation.
+// !SYM (streaming variant: a sweep must be one contiguous window): thread tid owns octet sweep * nt + tid, full basis.
+// ------------------------------------------------------------------------------------------
+template <bool SYM>
+__device__ __forceinline__ int v1_nsweep(const SegDev &sg)
+{
+    const int noct = (sg.fit_hi - sg.fit_lo) >> 3;
+    return SYM ? ((noct >> 1) + (V1_NT >> 1) - 1) / (V1_NT >> 1) : (noct + V1_NT - 1) / V1_NT;
+}
+
+template <bool SYM>
+__device__ __forceinline__ int v1_oct_of(const SegDev &sg, int sw, bool &act)
+{
+    const int noct = (sg.fit_hi - sg.fit_lo) >> 3;
+    if (SYM) {
+        const int lane = V1_LANE, p = sw * (V1_NT >> 1) + 16 * V1_WARP + (lane < 16 ? lane : 31 - lane);
+        act = p < (noct >> 1);
+        return sg.fit_lo + OCT * (act ? (lane < 16 ? p : noct - 1 - p) : 0);
+    }
+    const int o = sw * V1_NT + V1_TID;
+    act = o < noct;
+    return sg.fit_lo + OCT * o;   // inactive threads never dereference it
+}
+
+// Chebyshev recurrence state for the thread's octet.  Full basis: (pp, pc) = (T_-1, T_0) = (t, 1), step x2 = 2 t.
+// SYM: lanes < 16 walk the even n: (T_-2, T_0) = (T_2, 1); lanes >= 16 the odd n: (T_-1, T_1) = (t, t); step 2 T_2
+// (2 T_2 T_n = T_(n+2) + T_(n-2)).
+template <bool SYM>
+__device__ __forceinline__ void v1_cheb_init(const SegDev &sg, int j0, float (&pp)[OCT], float (&pc)[OCT], float (&x2)[OCT])
+{
+    const int nm1 = sg.fit_hi - sg.fit_lo - 1;
+    const float tm = sg.ta;
+    const bool hi = V1_LANE >= 16;
+#pragma unroll
+    for (int i = 0; i < OCT; ++i) {
+        const float t = tm * (float)(2 * (j0 + i - sg.fit_lo) - nm1);
+        if (SYM) {
+            const float t2 = fmaf(2.f * t, t, -1.f);
+            pp[i] = hi ? t : t2; pc[i] = hi ? t : 1.f; x2[i] = 2.f * t2;
+        } else { pp[i] = t; pc[i] = 1.f; x2[i] = 2.f * t; }
+    }
+}
+
+// sums  sum_i x[g][i] T_n(t_i)  for the basis the lane walks, reduced over the warp into this warp's slots slot0 + n:
+// nred = number of n (rounded up to 8) of the full basis.  `first` overwrites the slots, else accumulates.
+template <bool SYM>
+__device__ __forceinline__ void v1_basis_sums(const float (&x)[GS][OCT], float (&pp)[OCT], float (&pc)[OCT], const float (&x2)[OCT],
+                                              float *red, int slot0, int nred, bool first)
+{
+    const int lane = V1_LANE;
+    if (SYM) {
+        const int hi = lane >> 4;
+        for (int n0 = 0; n0 < (nred >> 1); n0 += 4) {      // four n of this lane's parity per transpose: value (nn, g) at nn*4 + g
+            float X[16];
+#pragma unroll
+            for (int nn = 0; nn < 4; ++nn) {
+#pragma unroll
+                for (int g = 0; g < GS; ++g) {
+                    float sr = 0.f;
+#pragma unroll
+                    for (int i = 0; i < OCT; ++i) sr = fmaf(x[g][i], pc[i], sr);
+                    X[nn * 4 + g] = sr;
+                }
+#pragma unroll
+                for (int i = 0; i < OCT; ++i) { const float nx = fmaf(x2[i], pc[i], -pp[i]); pp[i] = pc[i]; pc[i] = nx; }
+            }
+            const float tot = xreduce16(X, lane);
+            float *r = red + (slot0 + 2 * (n0 + ((lane & 15) >> 2)) + hi) * GS + (lane & 3);
+            if (first) *r = tot; else *r += tot;
+        }
+    } else {
+        for (int n0 = 0; n0 < nred; n0 += 8) {             // eight n per transpose
+            float X[32];
+#pragma unroll
+            for (int nn = 0; nn < 8; ++nn) {
+#pragma unroll
+                for (int g = 0; g < GS; ++g) {
+                    float sr = 0.f;
+#pragma unroll
+                    for (int i = 0; i < OCT; ++i) sr = fmaf(x[g][i], pc[i], sr);
+                    X[nn * 4 + g] = sr;
+                }
+#pragma unroll
+                for (int i = 0; i < OCT; ++i) { const float nx = fmaf(x2[i], pc[i], -pp[i]); pp[i] = pc[i]; pc[i] = nx; }
+            }
+            const float tot = xreduce32(X, lane);
+            float *r = red + (slot0 + n0 + (lane >> 2)) * GS + (lane & 3);
+            if (first) *r = tot; else *r += tot;
+        }
+    }
+}
+
+// SYM: x <- x + (-1)^n x(mirror) for the parity this lane walks (lanes < 16: +, lanes >= 16: -); pixel i of this octet
+// mirrors pixel 7 - i of lane ^ 31's octet
+__device__ __forceinline__ void v1_mirror_combine(float (&x)[GS][OCT])
+{
+    const bool hi = V1_LANE >= 16;
+#pragma unroll
+    for (int g = 0; g < GS; ++g)
+#pragma unroll
+        for (int i = 0; i < OCT / 2; ++i) {
+            const float ra = __shfl_xor_sync(FULL, x[g][OCT - 1 - i], 31), rb = __shfl_xor_sync(FULL, x[g][i], 31);
+            x[g][i] = hi ? x[g][i] - ra : x[g][i] + ra;
+            x[g][OCT - 1 - i] = hi ? x[g][OCT - 1 - i] - rb : x[g][OCT - 1 - i] + rb;
+        }
+}
+
+// ------------------------------------------------------------------------------------------
 // a4 + a5 (accumulation part).  For the thread's octet of the fitted range:
 //   S = G (*) T (or re-read from row A when `stencil` is false), stored to row A;
 //   u = w S^2, v = w S (y - c_prev S);
@@ -709,8 +847,8 @@ __device__ __noinline__ void v1_phase_forward(const SegDev &sg, bool stencil)
     float *red = V1SM + L.oRED + V1_WARP * L.VR * GS;
     // hoisted to registers (the model sits in shared memory; see v1_phase_emulator)
     const int Ppad = v1_blk.M.Ppad, P8 = Ppad >> 3, RL = L.RL, NA = L.NA, n1r = L.n1r, nmomr = L.nmomr, nt8 = V1_NT * OCT;
-    const int fit_lo = sg.fit_lo, fit_hi = sg.fit_hi, torg = sg.po + sg.halo;
-    const float ta = sg.ta, tb = sg.tb;
+    constexpr bool SYM = !STREAM;
+    const int fit_lo = sg.fit_lo;
     float *rowA = v1_rowp(L.oA, sg.po);
     const float *rowT = v1_rowp(L.oT, sg.po);
     float *ag = v1_blk.ag;
@@ -724,11 +862,13 @@ __device__ __noinline__ void v1_phase_forward(const SegDev &sg, bool stencil)
     size_t rowo[GS];
 #pragma unroll
     for (int g = 0; g < GS; ++g) { alo[g] = tap[2 * g]; nag[g] = tap[2 * g + 1]; rowo[g] = (size_t)v1_blk.spec[g] * Ppad; }
-    bool first = true;
-    for (int jb = fit_lo; jb < fit_hi; jb += nt8, first = false) {   // uniform trip count
-        const int j0 = jb + V1_TID * OCT;
-        const bool act = j0 < fit_hi;
+    const int nsweep = v1_nsweep<SYM>(sg);
+    for (int sw = 0; sw < nsweep; ++sw) {   // uniform trip count
+        bool act;
+        const int j0 = v1_oct_of<SYM>(sg, sw, act);
+        const bool first = sw == 0;
         if (STREAM && stencil) {   // this sweep's window of T (written to the global rows by the emulator phase)
+            const int jb = fit_lo + sw * nt8;
             __syncthreads();
             v1_window_load(v1_blk.tg, jb);
             __syncthreads();
@@ -789,32 +929,11 @@ __device__ __noinline__ void v1_phase_forward(const SegDev &sg, bool stencil)
 #pragma unroll
                 for (int i = 0; i < OCT; ++i) v[g][i] = 0.f;
         }
-        // Chebyshev recurrence state: (pp, pc) = (T_{n-1}, T_n), started at (T_{-1}, T_0) = (t, 1)
+        // right-hand side  rhs_n = sum_j v_j T_n(t_j), n <= D
         float pp[OCT], pc[OCT], x2[OCT];
-#pragma unroll
-        for (int i = 0; i < OCT; ++i) {
-            const float t = fmaf(ta, (float)(j0 + i - torg), tb);
-            pp[i] = t; pc[i] = 1.f; x2[i] = 2.f * t;
-        }
-        // right-hand side only, eight n per transpose
-        for (int n0 = 0; n0 < n1r; n0 += 8) {
-            float X[32];
-#pragma unroll
-            for (int nn = 0; nn < 8; ++nn) {
-#pragma unroll
-                for (int g = 0; g < GS; ++g) {
-                    float sr = 0.f;
-#pragma unroll
-                    for (int i = 0; i < OCT; ++i) sr = fmaf(v[g][i], pc[i], sr);
-                    X[nn * 4 + g] = sr;
-                }
-#pragma unroll
-                for (int i = 0; i < OCT; ++i) { const float nx = fmaf(x2[i], pc[i], -pp[i]); pp[i] = pc[i]; pc[i] = nx; }
-            }
-            const float tot = xreduce32(X, V1_LANE);
-            const int slot = nmomr + n0 + (V1_LANE >> 2);
-            if (first) red[slot * GS + (V1_LANE & 3)] = tot; else red[slot * GS + (V1_LANE & 3)] += tot;
-        }
+        v1_cheb_init<SYM>(sg, j0, pp, pc, x2);
+        if (SYM) v1_mirror_combine(v);
+        v1_basis_sums<SYM>(v, pp, pc, x2, red, nmomr, n1r, first);
     }
 }
 
@@ -827,16 +946,15 @@ __device__ __noinline__ void v1_phase_moments(const SegDev &sg)
 {
     const V1Lay &L = v1_blk.L;
     float *red = V1SM + L.oRED + V1_WARP * L.VR * GS;
-    const int Ppad = v1_blk.M.Ppad, P8 = Ppad >> 3, RL = L.RL, nmomr = L.nmomr, nt8 = V1_NT * OCT;
-    const int fit_lo = sg.fit_lo, fit_hi = sg.fit_hi, torg = sg.po + sg.halo;
-    const float ta = sg.ta, tb = sg.tb;
+    constexpr bool SYM = !STREAM;
+    const int Ppad = v1_blk.M.Ppad, P8 = Ppad >> 3, nmomr = L.nmomr;
     const float *rowA = v1_rowp(L.oA, sg.po);
     const float *ag = v1_blk.ag;
     const float *Wg = v1_blk.A.W;
-    bool first = true;
-    for (int jb = fit_lo; jb < fit_hi; jb += nt8, first = false) {
-        const int j0 = jb + V1_TID * OCT;
-        const bool act = j0 < fit_hi;
+    const int nsweep = v1_nsweep<SYM>(sg);
+    for (int sw = 0; sw < nsweep; ++sw) {
+        bool act;
+        const int j0 = v1_oct_of<SYM>(sg, sw, act);
         float u[GS][OCT], pp[OCT], pc[OCT], x2[OCT];
 #pragma unroll
         for (int g = 0; g < GS; ++g) {
@@ -852,29 +970,9 @@ __device__ __noinline__ void v1_phase_moments(const SegDev &sg)
                 for (int i = 0; i < OCT; ++i) u[g][i] = ww[i] * SS[i] * SS[i];
             }
         }
-#pragma unroll
-        for (int i = 0; i < OCT; ++i) {
-            const float t = fmaf(ta, (float)(j0 + i - torg), tb);
-            pp[i] = t; pc[i] = 1.f; x2[i] = 2.f * t;
-        }
-        for (int n0 = 0; n0 < nmomr; n0 += 8) {      // eight n per transpose: value (nn, g) at nn*4 + g
-            float X[32];
-#pragma unroll
-            for (int nn = 0; nn < 8; ++nn) {
-#pragma unroll
-                for (int g = 0; g < GS; ++g) {
-                    float sm_ = 0.f;
-#pragma unroll
-                    for (int i = 0; i < OCT; ++i) sm_ = fmaf(u[g][i], pc[i], sm_);
-                    X[nn * 4 + g] = sm_;
-                }
-#pragma unroll
-                for (int i = 0; i < OCT; ++i) { const float nx = fmaf(x2[i], pc[i], -pp[i]); pp[i] = pc[i]; pc[i] = nx; }
-            }
-            const float tot = xreduce32(X, V1_LANE);
-            const int slot = n0 + (V1_LANE >> 2);
-            if (first) red[slot * GS + (V1_LANE & 3)] = tot; else red[slot * GS + (V1_LANE & 3)] += tot;
-        }
+        v1_cheb_init<SYM>(sg, j0, pp, pc, x2);
+        if (SYM) v1_mirror_combine(u);
+        v1_basis_sums<SYM>(u, pp, pc, x2, red, 0, nmomr, sw == 0);
     }
 }
 
@@ -949,7 +1047,11 @@ __device__ __noinline__ void v1_refactor(int g, int seg)
     }
     const float mine = 1.f / own[lane];
     invd[lane] = mine;
-    if (lane == 0) SMV(L.oSC, SC_N + seg, g) = ok ? 0.f : 1.f;
+    if (lane == 0) {
+        SMV(L.oSC, SC_N + seg, g) = ok ? 0.f : 1.f;
+        const unsigned bit = 1u << (seg * GS + g);   // the adaptive policy re-factorises every step while a system fails
+        if (ok) atomicAnd(&v1_blk.failmask, ~bit); else atomicOr(&v1_blk.failmask, bit);
+    }
     __syncwarp();
     // unit-diagonal factor Lt = L D^-1 (D = diag L) and 1/d^2:  A^-1 = Lt^-T D^-2 Lt^-1
 #pragma unroll 1
@@ -1077,9 +1179,8 @@ __device__ __noinline__ void v1_phase_residual(const SegDev &sg, int rowB, float
     const V1Args &a = v1_blk.A;
     const V1Lay &L = v1_blk.L;
     const float4 *b4 = (const float4 *)(V1SM + L.oB) + rowB;
-    const int Ppad = v1_blk.M.Ppad, P8 = Ppad >> 3, n1 = v1_blk.M.n1, RL = L.RL, nt8 = V1_NT * OCT;
-    const int fit_lo = sg.fit_lo, fit_hi = sg.fit_hi, torg = sg.po + sg.halo;
-    const float ta = sg.ta, tb = sg.tb;
+    constexpr bool SYM = !STREAM;
+    const int Ppad = v1_blk.M.Ppad, P8 = Ppad >> 3, n1 = v1_blk.M.n1;
     float *rowA = v1_rowp(L.oA, sg.po);
     float *ag = v1_blk.ag;
     const float *Yg = a.Y, *Wg = a.W;
@@ -1092,7 +1193,11 @@ __device__ __noinline__ void v1_phase_residual(const SegDev &sg, int rowB, float
     const float *dsg = v1_blk.ds;
 #pragma unroll
     for (int g = 0; g < GS; ++g) { chi[g] = 0.f; ng[g] = 0.f; cmin[g] = 3.0e38f; gvv[g] = 0.f; gss[g] = 0.f; }
-    for (int j0 = fit_lo + V1_TID * OCT; j0 < fit_hi; j0 += nt8) {
+    const int nsweep = v1_nsweep<SYM>(sg);
+    for (int sw = 0; sw < nsweep; ++sw) {
+        bool act;
+        const int j0 = v1_oct_of<SYM>(sg, sw, act);
+        if (!SYM && !act) continue;        // SYM: inactive lanes stay for the exchange (their partner is inactive too)
         float cc[GS][OCT], pp[OCT], pc[OCT], x2[OCT];
         float4 yq[GS][2], wq[GS][2];   // flux / weight from L2, issued before the basis loop hides them
         if (MODE != 0) {
@@ -1103,24 +1208,46 @@ __device__ __noinline__ void v1_phase_residual(const SegDev &sg, int rowB, float
                 wq[g][0] = __ldg((const float4 *)(Wg + ro)); wq[g][1] = __ldg((const float4 *)(Wg + ro) + P8);
             }
         }
-#pragma unroll
-        for (int i = 0; i < OCT; ++i) {
-            const float t = fmaf(ta, (float)(j0 + i - torg), tb);
-            pp[i] = t; pc[i] = 1.f; x2[i] = 2.f * t;
-        }
+        v1_cheb_init<SYM>(sg, j0, pp, pc, x2);
 #pragma unroll
         for (int g = 0; g < GS; ++g)
 #pragma unroll
             for (int i = 0; i < OCT; ++i) cc[g][i] = 0.f;
-        for (int n = 0; n < n1; ++n) {
-            const float4 b = b4[n];
-            const float bg[GS] = {b.x, b.y, b.z, b.w};
+        if (SYM) {
+            // this lane's half of the basis at its own nodes: E = sum_even b_n T_n (lanes < 16) or O = sum_odd b_n T_n
+            // (lanes >= 16); then c(t_i) = E_i - O'_(7-i) on lanes < 16 and c(t'_i) = E_(7-i) + O'_i on lanes >= 16,
+            // the other half coming from lane ^ 31 (whose nodes are the negatives of this lane's)
+            const int hi = V1_LANE >> 4;
+            for (int n = hi; n < n1; n += 2) {
+                const float4 b = b4[n];
+                const float bg[GS] = {b.x, b.y, b.z, b.w};
+#pragma unroll
+                for (int g = 0; g < GS; ++g)
+#pragma unroll
+                    for (int i = 0; i < OCT; ++i) cc[g][i] = fmaf(bg[g], pc[i], cc[g][i]);
+#pragma unroll
+                for (int i = 0; i < OCT; ++i) { const float nx = fmaf(x2[i], pc[i], -pp[i]); pp[i] = pc[i]; pc[i] = nx; }
+            }
 #pragma unroll
             for (int g = 0; g < GS; ++g)
 #pragma unroll
-                for (int i = 0; i < OCT; ++i) cc[g][i] = fmaf(bg[g], pc[i], cc[g][i]);
+                for (int i = 0; i < OCT / 2; ++i) {
+                    const float ra = __shfl_xor_sync(FULL, cc[g][OCT - 1 - i], 31), rb = __shfl_xor_sync(FULL, cc[g][i], 31);
+                    cc[g][i] = hi ? cc[g][i] + ra : cc[g][i] - ra;
+                    cc[g][OCT - 1 - i] = hi ? cc[g][OCT - 1 - i] + rb : cc[g][OCT - 1 - i] - rb;
+                }
+            if (!act) continue;
+        } else {
+            for (int n = 0; n < n1; ++n) {
+                const float4 b = b4[n];
+                const float bg[GS] = {b.x, b.y, b.z, b.w};
 #pragma unroll
-            for (int i = 0; i < OCT; ++i) { const float nx = fmaf(x2[i], pc[i], -pp[i]); pp[i] = pc[i]; pc[i] = nx; }
+                for (int g = 0; g < GS; ++g)
+#pragma unroll
+                    for (int i = 0; i < OCT; ++i) cc[g][i] = fmaf(bg[g], pc[i], cc[g][i]);
+#pragma unroll
+                for (int i = 0; i < OCT; ++i) { const float nx = fmaf(x2[i], pc[i], -pp[i]); pp[i] = pc[i]; pc[i] = nx; }
+            }
         }
 #pragma unroll
         for (int g = 0; g < GS; ++g) {
@@ -1375,19 +1502,16 @@ __device__ __noinline__ void v1_evaluate(bool cold, int momsel, float *xrow, boo
             if (V1_TID == 0 && adam) {   // Gram re-factorisation decision from what the update warps left before the barrier
                 bool fresh = momsel == 1;
                 if (momsel == 2) {
-                    float step = 0.f;
-                    bool fail = false;
-#pragma unroll
-                    for (int g = 0; g < GS; ++g) {
-                        step = fmaxf(step, SMV(L.oSC, SC_DU, g));
-                        for (int q = 0; q < M.n_seg; ++q) fail = fail || SMV(L.oSC, SC_N + q, g) != 0.f;
-                    }
-                    v1_blk.drift += step;
-                    v1_blk.since += 1;
-                    fresh = fail || v1_blk.since >= 64 || v1_blk.drift * step > a.drift_tol;
+                    const float step = __int_as_float(v1_blk.stepmax);
+                    const float drift = v1_blk.drift + step;
+                    const int since = v1_blk.since + 1;
+                    fresh = v1_blk.failmask != 0u || since >= 64 || drift * step > a.drift_tol;
+                    v1_blk.drift = fresh ? 0.f : drift;
+                    v1_blk.since = fresh ? 0 : since;
+                    v1_blk.stepmax = 0;
+                    v1_blk.momflag = fresh ? 1 : 0;
                 }
-                if (fresh) { v1_blk.drift = 0.f; v1_blk.since = 0; v1_blk.nfresh += 1; }
-                v1_blk.momflag = fresh ? 1 : 0;
+                if (fresh) v1_blk.nfresh += 1;
             }
         }
         int lo, hi;
@@ -1559,7 +1683,7 @@ __device__ __noinline__ void v1_update_fast(int g, float ib1, float ib2)
         float du = lane < NP ? fabsf(u - u0) : 0.f;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) du = fmaxf(du, __shfl_xor_sync(FULL, du, o));
-        if (lane == 0) SMV(L.oSC, SC_DU, g) = du;
+        if (lane == 0) atomicMax(&v1_blk.stepmax, __float_as_int(du));
     }
     // ---- a1: de-normalise, emulator inputs (C.2-18/19)
     const float half = (hi - lo) * 0.5f;
@@ -1636,7 +1760,7 @@ __device__ __forceinline__ void v1_init_block(const ModelDev &M, const V1Lay &L,
         v1_blk.ds = a.DS ? a.DS + (size_t)blockIdx.x * 3 * GS * L.SL : nullptr;
         v1_blk.tg = a.TG ? a.TG + (size_t)blockIdx.x * GS * M.Ppad : nullptr;
         v1_blk.ag = a.AG ? a.AG + (size_t)blockIdx.x * GS * M.Ppad : nullptr;
-        v1_blk.drift = 0.f; v1_blk.since = 0; v1_blk.momflag = 0; v1_blk.nfresh = 0;
+        v1_blk.drift = 0.f; v1_blk.since = 0; v1_blk.momflag = 0; v1_blk.nfresh = 0; v1_blk.stepmax = 0; v1_blk.failmask = 0u;
     }
     if (M.L <= 4) {   // one word per term (v1_param_setup)
         for (int k = threadIdx.x; k < M.K; k += blockDim.x) {
@@ -1663,10 +1787,9 @@ __device__ __forceinline__ void v1_set_group(int grp)
     if (threadIdx.x < GS) {
         const long long i = (long long)grp * GS + threadIdx.x;
         v1_blk.spec[threadIdx.x] = i < v1_blk.A.B ? i : v1_blk.A.B - 1;
-        SMV(v1_blk.L.oSC, SC_DU, threadIdx.x) = 0.f;
     }
     if (threadIdx.x == 0) {
-        v1_blk.drift = 0.f; v1_blk.since = 0; v1_blk.momflag = 0; v1_blk.nfresh = 0;
+        v1_blk.drift = 0.f; v1_blk.since = 0; v1_blk.momflag = 0; v1_blk.nfresh = 0; v1_blk.stepmax = 0; v1_blk.failmask = 0u;
     }
 }
 
@@ -1863,7 +1986,7 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
                     }
 #pragma unroll
                     for (int o = 16; o > 0; o >>= 1) du = fmaxf(du, __shfl_xor_sync(FULL, du, o));
-                    if (V1_LANE == 0) SMV(L.oSC, SC_DU, g) = du;   // re-factorisation monitor
+                    if (V1_LANE == 0) atomicMax(&v1_blk.stepmax, __float_as_int(du));   // re-factorisation monitor
                     __syncwarp();
 #ifdef LASP_PHASE_TIMING
                     if (a.dbg && V1_TID == 0) atomicAdd(a.dbg + 17, (unsigned long long)(clock64() - tu0));

@@ -263,15 +263,19 @@ extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx *
         if (jh >= jl) {
             S.fit_lo = S.po + S.halo + ne / CH * CH;
             S.fit_hi = S.po + S.halo + roundup(Ps - ne, CH);
+            if (((S.fit_hi - S.fit_lo) / CH) & 1) S.fit_hi += CH;   // an even number of octets: they pair up about the centre
         } else {
             S.fit_lo = S.fit_hi = S.po + S.halo;
         }
-        double ta = 0.0, tb = 0.0;
-        if (jh > jl) { ta = 2.0 / (jh - jl); tb = -(double)(jl + jh) / (jh - jl); }
-        S.ta = (float)ta; S.tb = (float)tb;
-        // conv[m][n] = (2m+1)/2 int P_m(x) T_n(alpha x + beta) dx, exact by Gauss-Legendre (D+2 nodes)
-        // with the device's float ta, tb so that the conversion matches the basis actually used
-        const double alpha = (double)S.ta * Ps / 2.0, beta = (double)S.ta * Ps / 2.0 + (double)S.tb;
+        // Internal Chebyshev nodes, symmetric about the centre of the octet-aligned fitted range (lasp_fit_v1.cuh):
+        // t_j = tm (2 (j - fit_lo) - (N - 1)), N = fit_hi - fit_lo, tm = 1/(N - 1): |t| <= 1 on every pixel with w != 0
+        const int nfit = S.fit_hi - S.fit_lo;
+        S.ta = nfit > 1 ? (float)(1.0 / (nfit - 1)) : 0.f;
+        S.tb = 0.f;
+        // conv[m][n] = (2m+1)/2 int P_m(x) T_n(alpha x + beta) dx, exact by Gauss-Legendre (D+2 nodes), with the
+        // device's float tm so that the conversion matches the basis actually used; x^ = -1 + 2 j/Ps
+        const double flo_rel = S.fit_lo - (S.po + S.halo);
+        const double alpha = (double)S.ta * Ps, beta = (double)S.ta * (Ps - 2.0 * flo_rel - (nfit - 1));
         std::vector<double> gx, gw;
         gauss_legendre(M.n1 + 1, gx, gw);
         double *cv = conv.data() + (size_t)sg * M.n1 * M.n1;
@@ -700,8 +704,11 @@ extern "C" double lasp_fma_executed_per_spectrum_step(const lasp_ctx *c, double 
     if (!c) return 0.0;
     const ModelDev &M = c->M;
     const double P = M.P, K = M.K, n1 = M.n1, W = mean_taps;
-    const double G = (2.0 * M.D + 1.0) * P + M.n_seg * (n1 * n1 * n1 / 6.0 + n1 * n1 * n1);   // moments, Cholesky, inverse
-    return 2.0 * K * P + 4.0 * W * P + (c->nonuniform ? 2.0 * W * P : 0.0) + fresh_frac * G + 2.0 * n1 * P +
+    // resident variant: mirrored octet pairs share the basis values (T_n(-t) = (-1)^n T_n(t)), so a sum over the basis
+    // costs (D+1) P / 2 FMAs; moments, Cholesky and explicit inverse only on fresh steps
+    const double half = c->res.ok ? 0.5 : 1.0;
+    const double G = half * (2.0 * M.D + 1.0) * P + M.n_seg * (n1 * n1 * n1 / 6.0 + n1 * n1 * n1);
+    return 2.0 * K * P + 4.0 * W * P + (c->nonuniform ? 2.0 * W * P : 0.0) + fresh_frac * G + half * 2.0 * n1 * P +
            M.n_seg * n1 * n1 + 8.0 * P;
 }
 
