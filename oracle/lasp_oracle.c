@@ -17,6 +17,7 @@
  *   residual            Eq. 7   P:133              chi2 / rho
  *   objective           Eq. 9   P:163-167          sum_j w_j r_j^2 (C.2-2, C.2-3)
  *   Adam                step 8  P:169              orc_adam_step
+ *   stopping rules      step 8  P:169-171          orc_stop_rule, orc_fit_stop
  *   error estimate      step 9  P:173              errors_one
  *
  * Parity pins (tests/test_oracle_*.py): numpy legvander/legval, numpy lstsq,
@@ -584,6 +585,82 @@ int orc_fit(const orc_model *m, int64_t B, const double *flux, const double *iva
             if (err) errors_one(m, k, u, y, fd_h, err + i * NP);
         }
         free(u); free(mom); free(vel); free(g);
+        work_free(k);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------- stopping rules (step 8)
+ *
+ * "The optimization is considered converged when any of the following three criteria is satisfied: (1) a maximum of
+ * 5000 iterations is reached; (2) the change in loss over 50 consecutive steps is less than 1e-5; or (3) the loss
+ * increases monotonically over 50 consecutive steps."  Readings (R-2..R-5):
+ *   R-2  the loss of one spectrum is Eq. 9 restricted to it, L = sqrt(chi2 / p) with p = n_pix (Delta-2: the hot path
+ *        minimises sum_i chi2_i, so every spectrum stops on its own loss; with ivar = 1 this is the paper's L for N = 1);
+ *   R-3  criterion (2) is |L_t - L_{t-W}| < tol, W = 50, first testable at t = W + 1;
+ *   R-4  criterion (3) is W consecutive increases L_t > L_{t-1} > ... > L_{t-W};
+ *   R-5  L_t is the loss at the iterate the t-th gradient is taken at (t = 1, 2, ...); the rules are tested, (2)
+ *        before (3), BEFORE update t is applied, and a spectrum that stops at t keeps that iterate: t - 1 updates.
+ *        Criterion (1): after max_iter updates nothing more is applied.
+ * orc_stop_rule scans a loss sequence L[0..n-1] (L[t-1] = L_t) and returns the first t at which (2) or (3) fires
+ * (*rule = 2 or 3), or 0 with *rule = 1 when neither fires within the sequence. */
+int orc_stop_rule(const double *L, int n, int window, double tol, int *rule)
+{
+    int rise = 0;
+    for (int t = 1; t <= n; ++t) {
+        if (t > 1 && L[t - 1] > L[t - 2]) ++rise; else rise = 0;
+        if (t > window && fabs(L[t - 1] - L[t - 1 - window]) < tol) { *rule = 2; return t; }
+        if (rise >= window) { *rule = 3; return t; }
+    }
+    *rule = 1;
+    return 0;
+}
+
+/* lasp_fit_batch with the paper's stopping rules: as orc_fit, but every spectrum stops by R-2..R-5.
+ * n_steps[i] = Adam updates applied; status gets bit 16 (stopped by criterion 2) or 32 (criterion 3). */
+int orc_fit_stop(const orc_model *m, int64_t B, const double *flux, const double *ivar,
+                 const uint8_t *mask, const double *init, int max_iter, double lr, double b1, double b2,
+                 double eps, int window, double tol, double fd_h, double *params, double *cont,
+                 double *chi2, double *err, int32_t *status, int32_t *n_steps)
+{
+    int NP = m->n_labels + 2, P = m->n_pix, nc = m->n_seg * (m->cont_degree + 1);
+#pragma omp parallel
+    {
+        work_t *k = work_new(m);
+        double *u = calloc(NP, 8), *mom = calloc(NP, 8), *vel = calloc(NP, 8), *g = calloc(NP, 8);
+        double *hist = calloc((size_t)max_iter + 1, 8);
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t i = 0; i < B; ++i) {
+            const double *y = flux + i * P;
+            make_weights(m, ivar + i * P, mask ? mask + i * P : NULL, k->w);
+            norm_u(m, init + i * NP, u);
+            memset(mom, 0, 8 * NP);
+            memset(vel, 0, 8 * NP);
+            int rule = 1, rise = 0, applied = 0;
+            for (int t = 1; t <= max_iter; ++t) {
+                double c2 = chi2_at(m, k, u, y, 1, NULL);
+                double L = sqrt(c2 / (double)P);                     /* R-2 */
+                hist[t] = L;
+                if (t > 1 && L > hist[t - 1]) ++rise; else rise = 0;
+                if (t > window && fabs(L - hist[t - window]) < tol) { rule = 2; break; }   /* R-3 */
+                if (rise >= window) { rule = 3; break; }                                    /* R-4 */
+                grad_from_work(k, g);
+                orc_adam_step(NP, u, mom, vel, g, t, lr, b1, b2, eps);
+                applied = t;
+            }
+            int st = 0;
+            double c2 = chi2_at(m, k, u, y, 0, &st);
+            chi2[i] = c2;
+            denorm(m, u, params + i * NP);
+            if (cont) memcpy(cont + i * nc, k->b, 8 * (size_t)nc);
+            st = final_status(k, u, c2, st);
+            if (rule == 2) st |= 16;
+            if (rule == 3) st |= 32;
+            if (status) status[i] = st;
+            if (n_steps) n_steps[i] = applied;
+            if (err) errors_one(m, k, u, y, fd_h, err + i * NP);
+        }
+        free(u); free(mom); free(vel); free(g); free(hist);
         work_free(k);
     }
     return 0;

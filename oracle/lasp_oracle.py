@@ -199,6 +199,33 @@ class Oracle:
         return out
 
 
+    def fit_stop(self, flux, ivar, mask, init, max_iter, lr=0.1, beta1=0.9, beta2=0.999, eps=1e-8, window=50,
+                 tol=1e-5, fd_h=1e-5, want_err=True):
+        """The fit with the paper's stopping rules (orc_fit_stop)."""
+        flux, ivar, mask = self._obs(flux, ivar, mask)
+        B = flux.shape[0]
+        init = self._f64(init).reshape(B, self.NP)
+        params = np.empty((B, self.NP)); cont = np.empty((B, self.nc)); chi2 = np.empty(B)
+        err = np.empty((B, self.NP)) if want_err else None
+        status = np.zeros(B, dtype=np.int32); n_steps = np.zeros(B, dtype=np.int32)
+        lib().orc_fit_stop(C.byref(self.m), C.c_int64(B), _p(flux, _f64p), _p(ivar, _f64p),
+                           _p(mask, _u8p) if mask is not None else None, _p(init, _f64p), C.c_int(max_iter),
+                           C.c_double(lr), C.c_double(beta1), C.c_double(beta2), C.c_double(eps), C.c_int(window),
+                           C.c_double(tol), C.c_double(fd_h), _p(params, _f64p), _p(cont, _f64p), _p(chi2, _f64p),
+                           _p(err, _f64p) if want_err else None, _p(status, _i32p), _p(n_steps, _i32p))
+        return dict(params=params, cont=cont, chi2=chi2, err=err, status=status, n_steps=n_steps)
+
+def stop_rule(L, window=50, tol=1e-5):
+    """First step t (1-based) at which criterion (2) or (3) of P:169-171 fires on the loss sequence L, and the rule
+    (1 = neither within the sequence, then t = 0)."""
+    L = np.ascontiguousarray(L, dtype=np.float64)
+    rule = C.c_int(0)
+    f = lib().orc_stop_rule
+    f.restype = C.c_int
+    t = f(_p(L, _f64p), C.c_int(L.size), C.c_int(window), C.c_double(tol), C.byref(rule))
+    return int(t), int(rule.value)
+
+
 def forward(desc, params, cont):
     """`forward` callable for synth.make_case: model spectra from the oracle."""
     return Oracle(desc).eval_model(params, cont)

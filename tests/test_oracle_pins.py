@@ -120,12 +120,22 @@ def test_emulator_is_einsum_and_constant_term_at_origin(oracle_mod):
     x, phi0, _, _ = o.monomials(np.array([math.sqrt(3500.0 * 8000.0), 3.0, -1.0]))
     assert np.allclose(x, 0.0, atol=1e-6)
     assert np.isclose(phi0[0], 1.0) and np.allclose(phi0[1:], 0.0, atol=1e-6)
-    # brute-force triple loop on the first 7 pixels
-    for j in range(7):
+    # the oracle's own emulator_row, reached through eval_S with no shift and a vanishing width (sigma* = 1e-3 km/s:
+    # H = 1 and the two side taps weigh exp(-1/(2 sigma^2)) = 0, an identity kernel, so S == T), against a brute-force
+    # loop over terms with the monomials multiplied out by hand
+    theta[o.L + 1] = 1e-3
+    S = o.eval_S(theta)[0]
+    xx = np.array([float(d["emu_a"][l]) * (math.log10(theta[l]) if d["label_log10"][l] else float(theta[l]))
+                   + float(d["emu_b"][l]) for l in range(o.L)], dtype=np.float64)
+    for j in list(range(7)) + [d["n_pix"] // 2, d["n_pix"] - 1]:
         acc = 0.0
         for k in range(o.K):
-            acc += phi[k] * float(d["coeffs"][k, j])
-        assert abs(acc - T[j]) < 1e-13
+            mono = 1.0
+            for l in range(o.L):
+                for _ in range(int(d["term_exps"][k, l])):
+                    mono *= xx[l]
+            acc += mono * float(d["coeffs"][k, j])
+        assert abs(acc - S[j]) < 1e-12 and abs(acc - T[j]) < 1e-12
 
 
 # ---------------------------------------------------------------- kernel (Eq. 5)
@@ -493,3 +503,64 @@ def test_status_bits(oracle_mod):
     assert r["status"][1] & 4 and not (r["status"][1] & 1)
     assert r["status"][2] & 8
     assert np.allclose(r["params"][0], init[0], rtol=1e-12)  # zero steps: params = init
+
+
+# ------------------------------------------------------------------ stopping rules (readings R-2..R-5)
+
+def test_stop_rule_change_over_window_closed_form(oracle_mod):
+    """Criterion (2), |L_t - L_{t-50}| < tol: for L_t = a r^t + c the difference is a r^(t-50) (1 - r^50), so the first
+    firing step is known in closed form."""
+    a, r, c, W, tol = 3.0, 0.93, 0.7, 50, 1e-5
+    t = np.arange(1, 600)
+    L = a * r ** t + c
+    tstar = W + int(math.floor(math.log(tol / (a * (1 - r ** W))) / math.log(r))) + 1
+    assert a * r ** (tstar - W) * (1 - r ** W) < tol <= a * r ** (tstar - 1 - W) * (1 - r ** W)
+    assert oracle_mod.stop_rule(L, W, tol) == (tstar, 2)
+    assert oracle_mod.stop_rule(L[:tstar - 1], W, tol) == (0, 1)          # the sequence ends one step early: nothing fires
+    assert oracle_mod.stop_rule(L[:W], W, 1e30) == (0, 1)                 # not testable before t = W + 1 ...
+    assert oracle_mod.stop_rule(L[:W + 1], W, 1e30) == (W + 1, 2)         # ... and fires there however loose the tolerance
+    assert oracle_mod.stop_rule(L, 7, tol)[1] == 2 and oracle_mod.stop_rule(L, 7, tol)[0] < tstar
+
+
+def test_stop_rule_monotone_rise(oracle_mod):
+    """Criterion (3): 50 CONSECUTIVE increases.  A loss that falls for s steps and then rises every step fires at
+    s + 50; one dip resets the count; (2) is tested before (3) when both hold."""
+    W, s = 50, 13
+    fall = 10.0 - 0.5 * np.arange(1, s + 1)              # L_1..L_s strictly falling
+    rise = fall[-1] + 0.3 * np.arange(1, 200)            # then strictly rising: first increase at t = s + 1
+    L = np.concatenate([fall, rise])
+    assert oracle_mod.stop_rule(L, W, 1e-9) == (s + W, 3)
+    L2 = L.copy()
+    L2[s + 30 - 1] = L2[s + 30 - 2] - 1e-3               # a dip at t = s + 30: the run of increases restarts there
+    assert oracle_mod.stop_rule(L2, W, 1e-9) == (s + 30 + W, 3)
+    flat = np.concatenate([fall, fall[-1] + 1e-9 * np.arange(1, 200)])   # rising, but by less than tol per 50 steps
+    assert oracle_mod.stop_rule(flat, W, 1e-5) == (s + W, 2)   # both hold first at t = s + W: (2) is tested first
+    assert oracle_mod.stop_rule(np.ones(120), W, 1e-5) == (W + 1, 2)      # a constant loss is "no change", not a rise
+
+
+def test_fit_with_stopping_rules_is_the_fixed_step_fit_cut_at_the_stop(oracle_mod):
+    """orc_fit_stop against the pinned pieces: with an infinite tolerance every spectrum stops at the first testable
+    step (t = 51: 50 updates, status bit 16); with tol = 0 and no sustained rise it runs to max_iter; and wherever it
+    stops, the result is exactly orc_fit's after that many steps (same trajectory, R-5)."""
+    case = make(small_config(), oracle_mod, B=3)
+    o = oracle_mod.Oracle(case["desc"])
+    args = (case["flux"], case["ivar"], case["mask"], case["init"])
+    r = o.fit_stop(*args, 200, lr=0.05, tol=1e30)
+    assert np.array_equal(r["n_steps"], [50, 50, 50]) and np.all(r["status"] & 16) and not np.any(r["status"] & 32)
+    ref = o.fit(*args, 50, lr=0.05)
+    for k in ("params", "chi2", "cont", "err"):
+        assert np.array_equal(r[k], ref[k]), k
+    r = o.fit_stop(*args, 70, lr=0.05, tol=0.0)
+    assert np.array_equal(r["n_steps"], [70, 70, 70]) and not np.any(r["status"] & 48)
+    assert np.array_equal(r["params"], o.fit(*args, 70, lr=0.05)["params"])
+    # the paper's settings (lr 0.1, tol 1e-5, window 50): stops well before 5000, and the stop step is the one the
+    # rule gives on the loss trace L_t = sqrt(chi2_t / p) of the fixed-step fit (R-2)
+    r = o.fit_stop(*args, 5000, lr=0.1)
+    assert np.all(r["n_steps"] < 2000) and np.all(r["status"] & 48)
+    tr = o.fit(*args, int(r["n_steps"].max()) + 1, lr=0.1, want_trace=True, want_err=False)["trace"]
+    for i in range(3):
+        L = np.sqrt(tr[i, :-1] / case["desc"]["n_pix"])
+        t, rule = oracle_mod.stop_rule(L, 50, 1e-5)
+        assert t == r["n_steps"][i] + 1 and bool(r["status"][i] & (16 if rule == 2 else 32))
+        assert np.array_equal(r["params"][i], o.fit(*[a[i:i + 1] for a in args], int(r["n_steps"][i]), lr=0.1,
+                                                    want_err=False)["params"][0])
