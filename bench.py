@@ -259,8 +259,10 @@ def time_fit(model, data, n_iter, steps, warmup, kw, torch, barrier):
     return out, ev[0].elapsed_time(ev[-1]), step_ms, model.launch_count() - l0
 
 
-def run_other_config(cfg_id, B, torch, local, peaks, n_sms, emulator_path=0):
-    """One timed step (after one warm-up) of another BASELINE.json config at a stated, reduced batch."""
+def run_other_config(cfg_id, B, torch, local, peaks, n_sms, emulator_path=0, paper_stop=False):
+    """One timed step (after one warm-up) of another BASELINE.json config at a stated, reduced batch.
+    paper_stop: the paper's optimiser settings instead of the config's fixed steps: lr 0.1, at most 5000
+    iterations, stop when |L_t - L_(t-50)| < 1e-5 or after 50 consecutive increases (lasp_fit_opts.stop_window)."""
     from paper_2512_24840_b200 import binding, synth
     cfg = synth.CONFIGS[cfg_id]
     desc = synth.make_model_desc(cfg)
@@ -269,15 +271,33 @@ def run_other_config(cfg_id, B, torch, local, peaks, n_sms, emulator_path=0):
     model.reserve(B)
     data = make_device_batch(model, cfg, desc, B, cfg.seed + 17, torch)
     kw = dict(lr=cfg.lr, beta1=cfg.beta1, beta2=cfg.beta2, eps=cfg.eps, emulator_path=emulator_path)
-    out, ms_total, step_ms, _ = time_fit(model, data, cfg.n_iter, 1, 1, kw, torch, torch.cuda.synchronize)
-    roof = roofline_of(model, desc, B, cfg.n_iter, out["params"].cpu().numpy(), step_ms[0], peaks, n_sms)
-    rec = {"workload": f"config {cfg_id} ({cfg.name})", "spectra": B, "full_batch": cfg.B, "adam_steps": cfg.n_iter,
+    n_iter = cfg.n_iter
+    if paper_stop:
+        kw.update(lr=0.1, stop_window=50, stop_tol=1e-5)
+        n_iter = 5000
+    out, ms_total, step_ms, _ = time_fit(model, data, n_iter, 1, 1, kw, torch, torch.cuda.synchronize)
+    # evaluations actually executed per spectrum slot (= n_iter at fixed steps; the group's last stop step otherwise)
+    steps_run = model.last_fit_stats()["group_steps"] * 4.0 / B
+    roof = roofline_of(model, desc, B, steps_run, out["params"].cpu().numpy(), step_ms[0], peaks, n_sms)
+    rec = {"workload": f"config {cfg_id} ({cfg.name})", "spectra": B, "full_batch": cfg.B, "adam_steps": n_iter,
            "n_pix": model.P, "n_terms": model.K, "n_labels": model.L, "n_seg": model.n_seg,
            "value": B / (step_ms[0] * 1e-3), "unit": UNIT, "ms_per_step": step_ms[0],
            "variant": model.default_variant(), "launch": model.launch_info(model.default_variant()),
            "emulator_path": emulator_path, "frac": roof["frac"], "frac_executed": roof["frac_executed"],
            "achieved_tflops": roof["achieved"], "fresh_factor_frac": roof["fresh_factor_frac"],
            "mean_taps": roof["mean_taps"], "status_nonzero_frac": float((out["status"] != 0).float().mean().item())}
+    if paper_stop:
+        ns = out["n_steps"].float()
+        st = out["status"]
+        rec.update({"workload": f"config {cfg_id} shapes with the paper's optimiser settings (lr 0.1, <= 5000 iterations, "
+                                "stopping rules of P:169-171, window 50, tolerance 1e-5)",
+                    "lr": 0.1, "stop_window": 50, "stop_tol": 1e-5,
+                    "steps_to_stop": {"mean": float(ns.mean().item()), "median": float(ns.median().item()),
+                                      "p95": float(ns.quantile(0.95).item()), "max": float(ns.max().item())},
+                    "steps_run_per_group_mean": steps_run,
+                    "stopped_by": {"tolerance": float(((st & 16) != 0).float().mean().item()),
+                                   "rising_loss": float(((st & 32) != 0).float().mean().item()),
+                                   "max_iterations": float(((st & 48) == 0).float().mean().item())}})
     model.close()
     del data, out
     torch.cuda.empty_cache()
@@ -464,6 +484,10 @@ def run_gpu(args):
                 oc[f"config{cid}"] = run_other_config(cid, b, torch, local, peaks, n_sms)
             except Exception as e:   # report, never hide
                 oc[f"config{cid}"] = {"error": f"{type(e).__name__}: {e}"}
+        try:
+            oc["config1_paper_stop"] = run_other_config(1, 65536, torch, local, peaks, n_sms, paper_stop=True)
+        except Exception as e:
+            oc["config1_paper_stop"] = {"error": f"{type(e).__name__}: {e}"}
         line["other_configs"] = oc
     if world == 1 and not args.no_cpu_baseline:
         cores = os.cpu_count() or 1

@@ -63,6 +63,8 @@ extern "C" {
 #define LASP_ST_NONFINITE 2 /* a non-finite value was met */
 #define LASP_ST_NEG_CONT 4  /* continuum c_j <= 0 on a fitted pixel at the solution */
 #define LASP_ST_ON_BOUND 8  /* a parameter ended on its prior bound */
+#define LASP_ST_STOP_TOL 16  /* stopped by criterion (2) of P:169-171: |L_t - L_(t-W)| < stop_tol */
+#define LASP_ST_STOP_RISE 32 /* stopped by criterion (3): the loss rose on W consecutive steps */
 
 typedef struct lasp_ctx lasp_ctx; /* opaque; owns only its own device copies and workspace */
 
@@ -106,6 +108,12 @@ typedef struct {
     int32_t warm;                 /* the first `warm` steps always re-factorise (0 = default 4) */
     int32_t fd_fresh;             /* 1: the 2 NP finite-difference evaluations of the error estimate re-factorise
                                      too (0: they reuse the final evaluation's factor, C.2-22) */
+    int32_t stop_window;          /* the paper's stopping rules (step 8; R-2..R-5): 0 (default) = off,
+                                     exactly n_iter steps (Delta-6); W in [1, 128] (the paper: 50) = every spectrum stops on
+                                     its own loss L_t = sqrt(chi2_t / n_pix) (Eq. 9 restricted to it), tested before update
+                                     t: (1) n_iter updates applied (n_iter is then the paper's "maximum of 5000
+                                     iterations"); (2) |L_t - L_(t-W)| < stop_tol; (3) W consecutive increases */
+    float stop_tol;               /* threshold of criterion (2) (the paper: 1e-5) */
 } lasp_fit_opts;
 
 /* Build a context on `cuda_device`: validates the description, derives the per-pixel velocity
@@ -122,22 +130,23 @@ int lasp_reserve(lasp_ctx *ctx, int64_t B);
  *   params [B*NP] physical; cont [B*n_seg*(D+1)] plain-Legendre coefficients (numpy legval
  *   convention, nodes x_j = -1 + 2(j-o_s)/P_s) or NULL; chi2 [B];
  *   err [B*NP] = sqrt(diag(rho^T rho/(N_good-NP) (J^T J)^-1)) in physical units (P:173,
- *   C.2-22/23; NaN when J^T J is singular) or NULL to skip; status [B] or NULL. */
+ *   C.2-22/23; NaN when J^T J is singular) or NULL to skip; status [B] or NULL;
+ *   n_steps [B] = Adam updates applied to each spectrum (= n_iter unless a stopping rule fired) or NULL. */
 int lasp_fit_batch(lasp_ctx *ctx, int64_t B, const float *flux, const float *ivar,
                    const uint8_t *mask, const float *init, const lasp_fit_opts *opts,
                    float *params, float *cont, float *chi2, float *err, int32_t *status,
-                   void *stream);
+                   int32_t *n_steps, void *stream);
 
 /* The same fit from HOST buffers (pinned memory recommended), for batches that do not fit on the device or
  * arrive from the host (BASELINE.json config 3, "survey-scale stream"): the batch is cut into chunks of
  * `chunk` spectra (0 = 65,536); chunk i+1 is copied host-to-device and chunk i-1's results device-to-host on
  * two copy streams while chunk i is fitted, with ctx-owned double buffers.  All pointers are HOST pointers
- * with the layouts of lasp_fit_batch; mask, cont, err, status may be NULL.  Blocking: returns when every
+ * with the layouts of lasp_fit_batch; mask, cont, err, status, n_steps may be NULL.  Blocking: returns when every
  * result is in host memory.  Per-chunk results are identical to lasp_fit_batch on the same spectra. */
 int lasp_fit_batch_host(lasp_ctx *ctx, int64_t B, const float *flux, const float *ivar,
                         const uint8_t *mask, const float *init, const lasp_fit_opts *opts,
                         float *params, float *cont, float *chi2, float *err, int32_t *status,
-                        int64_t chunk);
+                        int32_t *n_steps, int64_t chunk);
 
 /* Inspection: model_j = c_j S_j (Eq. 1, 5, 6) at given physical params [B*NP] and plain-Legendre cont
  * [B*n_seg*(D+1)]; model [B*n_pix], every pixel (edges included: replicate-edge clamp, C.2-16).  Runs the fit

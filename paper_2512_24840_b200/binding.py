@@ -17,7 +17,7 @@ SYMBOLS = ["lasp_create", "lasp_destroy", "lasp_reserve", "lasp_fit_batch", "las
            "lasp_eval_grad", "lasp_kernel_variant", "lasp_launch_info", "lasp_launch_count", "lasp_fma_per_spectrum_step",
            "lasp_fma_executed_per_spectrum_step", "lasp_last_fit_stats", "lasp_last_error", "lasp_version"]
 
-LASP_ST_NOT_SPD, LASP_ST_NONFINITE, LASP_ST_NEG_CONT, LASP_ST_ON_BOUND = 1, 2, 4, 8
+LASP_ST_NOT_SPD, LASP_ST_NONFINITE, LASP_ST_NEG_CONT, LASP_ST_ON_BOUND, LASP_ST_STOP_TOL, LASP_ST_STOP_RISE = 1, 2, 4, 8, 16, 32
 
 _f32p = C.POINTER(C.c_float)
 _f64p = C.POINTER(C.c_double)
@@ -39,7 +39,8 @@ class ModelDesc(C.Structure):
 class FitOpts(C.Structure):
     _fields_ = [("n_iter", C.c_int32), ("lr", C.c_float), ("beta1", C.c_float), ("beta2", C.c_float),
                 ("eps", C.c_float), ("variant", C.c_int32), ("emulator_path", C.c_int32),
-                ("refresh", C.c_int32), ("warm", C.c_int32), ("fd_fresh", C.c_int32)]
+                ("refresh", C.c_int32), ("warm", C.c_int32), ("fd_fresh", C.c_int32),
+                ("stop_window", C.c_int32), ("stop_tol", C.c_float)]
 
 
 class LaspError(RuntimeError):
@@ -62,9 +63,9 @@ def lib():
         L.lasp_destroy.argtypes = [C.c_void_p]
         L.lasp_reserve.argtypes = [C.c_void_p, C.c_int64]
         L.lasp_fit_batch.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 4 + [C.POINTER(FitOpts)] + \
-                                    [C.c_void_p] * 6
+                                    [C.c_void_p] * 7
         L.lasp_fit_batch_host.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 4 + [C.POINTER(FitOpts)] + \
-                                         [C.c_void_p] * 5 + [C.c_int64]
+                                         [C.c_void_p] * 6 + [C.c_int64]
         L.lasp_eval_model.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 2 + [C.POINTER(FitOpts)] + [C.c_void_p] * 2
         L.lasp_eval_grad.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 4 + [C.POINTER(FitOpts)] + [C.c_void_p] * 5
         L.lasp_kernel_variant.argtypes = [C.c_void_p]
@@ -174,9 +175,9 @@ class LaspModel:
 
     @staticmethod
     def _opts(n_iter=0, lr=1e-2, beta1=0.9, beta2=0.999, eps=1e-8, variant=0, emulator_path=0, refresh=0, warm=0,
-              fd_fresh=0):
+              fd_fresh=0, stop_window=0, stop_tol=1e-5):
         return FitOpts(int(n_iter), lr, beta1, beta2, eps, int(variant), int(emulator_path), int(refresh), int(warm),
-                       int(fd_fresh))
+                       int(fd_fresh), int(stop_window), float(stop_tol))
 
     def launch_count(self) -> int:
         return int(lib().lasp_launch_count(self.ctx))
@@ -185,7 +186,8 @@ class LaspModel:
         return float(lib().lasp_fma_per_spectrum_step(self.ctx, mean_taps))
 
     def fit_batch(self, flux, ivar, mask, init, n_iter, lr=1e-2, beta1=0.9, beta2=0.999, eps=1e-8,
-                  want_err=True, want_cont=True, out=None, emulator_path=0, variant=0, refresh=0, warm=0, fd_fresh=0):
+                  want_err=True, want_cont=True, out=None, emulator_path=0, variant=0, refresh=0, warm=0, fd_fresh=0,
+                  stop_window=0, stop_tol=1e-5):
         """lasp_fit_batch on device tensors; returns dict of device tensors."""
         t = self.torch
         flux = self._dev(flux, t.float32); ivar = self._dev(ivar, t.float32)
@@ -196,18 +198,20 @@ class LaspModel:
             out = dict(params=t.empty((B, self.NP), device=self.device, dtype=t.float32),
                        chi2=t.empty(B, device=self.device, dtype=t.float32),
                        status=t.empty(B, device=self.device, dtype=t.int32),
+                       n_steps=t.empty(B, device=self.device, dtype=t.int32),
                        cont=t.empty((B, self.nc), device=self.device, dtype=t.float32) if want_cont else None,
                        err=t.empty((B, self.NP), device=self.device, dtype=t.float32) if want_err else None)
-        opts = self._opts(n_iter, lr, beta1, beta2, eps, variant, emulator_path, refresh, warm, fd_fresh)
+        opts = self._opts(n_iter, lr, beta1, beta2, eps, variant, emulator_path, refresh, warm, fd_fresh, stop_window,
+                          stop_tol)
         rc = lib().lasp_fit_batch(self.ctx, B, _ptr(flux), _ptr(ivar), _ptr(mask), _ptr(init), C.byref(opts),
                                   _ptr(out["params"]), _ptr(out.get("cont")), _ptr(out["chi2"]),
-                                  _ptr(out.get("err")), _ptr(out["status"]), self._stream())
+                                  _ptr(out.get("err")), _ptr(out["status"]), _ptr(out.get("n_steps")), self._stream())
         self._check(rc, "lasp_fit_batch")
         return out
 
     def fit_batch_host(self, flux, ivar, mask, init, n_iter, lr=1e-2, beta1=0.9, beta2=0.999, eps=1e-8,
                        want_err=True, want_cont=True, chunk=0, out=None, emulator_path=0, variant=0, refresh=0, warm=0,
-                       fd_fresh=0):
+                       fd_fresh=0, stop_window=0, stop_tol=1e-5):
         """lasp_fit_batch_host on HOST tensors (torch CPU tensors, pinned for overlap); returns host tensors.
         The library cuts the batch into chunks and overlaps the copies with the fits."""
         t = self.torch
@@ -227,13 +231,14 @@ class LaspModel:
         if out is None:
             pin = dict(pin_memory=True)
             out = dict(params=t.empty((B, self.NP), dtype=t.float32, **pin), chi2=t.empty(B, dtype=t.float32, **pin),
-                       status=t.empty(B, dtype=t.int32, **pin),
+                       status=t.empty(B, dtype=t.int32, **pin), n_steps=t.empty(B, dtype=t.int32, **pin),
                        cont=t.empty((B, self.nc), dtype=t.float32, **pin) if want_cont else None,
                        err=t.empty((B, self.NP), dtype=t.float32, **pin) if want_err else None)
-        opts = self._opts(n_iter, lr, beta1, beta2, eps, variant, emulator_path, refresh, warm, fd_fresh)
+        opts = self._opts(n_iter, lr, beta1, beta2, eps, variant, emulator_path, refresh, warm, fd_fresh, stop_window,
+                          stop_tol)
         rc = lib().lasp_fit_batch_host(self.ctx, B, _ptr(flux), _ptr(ivar), _ptr(mask), _ptr(init), C.byref(opts),
                                        _ptr(out["params"]), _ptr(out.get("cont")), _ptr(out["chi2"]),
-                                       _ptr(out.get("err")), _ptr(out["status"]), int(chunk))
+                                       _ptr(out.get("err")), _ptr(out["status"]), _ptr(out.get("n_steps")), int(chunk))
         self._check(rc, "lasp_fit_batch_host")
         return out
 

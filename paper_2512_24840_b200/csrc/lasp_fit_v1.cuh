@@ -49,7 +49,7 @@ struct V1Lay {
     int nt8;                // pixels per sweep of the CTA (threads x 8): the streaming window holds nt8 + 2 GUARD
     int SL;                 // longest padded segment: row length of the per-pixel-kernel scratch planes
     // shared-memory offsets (floats)
-    int oT, oA, oU, oM, oV, oX, oPHI, oGW, oGR, oTAP, oMOM, oRHS, oB, oRED, oLF, oQ, oSC, oEXP, oXP, oDPHI, oGSC, oEW, oNP, total;
+    int oT, oA, oU, oM, oV, oX, oPHI, oGW, oGR, oTAP, oMOM, oRHS, oB, oRED, oLF, oQ, oSC, oEXP, oXP, oDPHI, oGSC, oEW, oNP, oHIST, total;
     int emax;               // largest exponent of the monomial table
 };
 
@@ -75,6 +75,10 @@ struct V1Args {
     int refresh;           // >= 1: re-factor every `refresh`-th step;  0: adaptive (drift monitor, at most every 64th)
     int fdfresh;           // 1: re-factor in every finite-difference evaluation of the error estimate
     float drift_tol;       // adaptive: re-factor when (sum of |du|_inf since the last factor) x |du|_inf exceeds this
+    // the paper's stopping rules (lasp_fit_opts.stop_window / .stop_tol): 0 = fixed number of steps
+    int stop_window;       // W <= V1_WMAX
+    float stop_tol;
+    int *nsteps;           // [B] Adam updates applied per spectrum (may be null)
     unsigned long long *dbg;   // optional per-phase cycle counters (LASP_TIMING=1), else null
     // per-pixel broadening kernels (linear grids, C.2-14): 1/s_j and s_j^2 with V1_TPAD replicated entries on
     // both sides, and per-CTA scratch [3][GS][Ppad] for dS/dv, dS/dsigma*, 1/E0 (thread-private pixels)
@@ -86,6 +90,7 @@ struct V1Args {
     int ksteps;            // k-steps of 8 terms in CF (<= 16)
 };
 #define V1_TPAD 256
+#define V1_WMAX 128    // largest stopping-rule window (loss history ring per spectrum)
 
 struct V1Np {          // per-spectrum scalars of a per-pixel-kernel segment
     float v, sigstar, sigtot, hn, hbv, hcap;   // hn = -log2(e)/(2 sigma_tot^2); hbv = |v| + 5 sigma_tot (km/s)
@@ -160,6 +165,11 @@ struct V1Block {
     int stepmax;          // max over the group of |du|_inf of the last update, as the bits of a non-negative float (atomicMax)
     unsigned failmask;    // bit seg * GS + g: the last factorisation of that system was not positive definite
     unsigned int nfresh;  // fresh Adam steps of the current group (statistics)
+    // stopping rules, per spectrum of the group (written by lane 0 of warp g)
+    int stop_rule[GS];    // 0 = still optimising; 2 / 3 = stopped by criterion (2) / (3) of P:169-171
+    int nsteps[GS];       // Adam updates applied
+    int rise[GS];         // consecutive increases of the loss so far
+    float lprev[GS];      // loss at the previous step
 };
 __shared__ V1Block v1_blk;
 #define V1_TID ((int)threadIdx.x)
@@ -1919,6 +1929,37 @@ __device__ __noinline__ void v1_errors(float chi2_g, float ngood_g, bool valid_g
 }
 
 // ------------------------------------------------------------------------------------------
+// The paper's stopping rules (step 8), per spectrum (Delta-2), warp g for spectrum g, called after the t-th
+// evaluation and before update t (readings R-2..R-5 of DESIGN.md, as oracle/lasp_oracle.c orc_fit_stop):
+//   loss L_t = sqrt(chi2_t / n_pix) (Eq. 9 restricted to one spectrum);
+//   (2) |L_t - L_{t-W}| < tol, testable from t = W + 1;  (3) W consecutive increases;  (2) is tested first.
+// Returns true (warp-uniform) when the spectrum goes on and update t is to be applied.  A spectrum that stops keeps
+// its iterate: the group runs on until all its spectra have stopped (or max_iter), the stopped ones frozen.
+// ------------------------------------------------------------------------------------------
+__device__ __noinline__ bool v1_stop_test(int g, int t)
+{
+    const V1Args &a = v1_blk.A;
+    if (v1_blk.stop_rule[g] != 0) return false;
+    float chi2, ngood, cmin;
+    v1_stats(g, chi2, ngood, cmin);
+    const float Lt = sqrtf(chi2 / (float)v1_blk.M.P);
+    int rule = 0;
+    if (V1_LANE == 0) {
+        const int W = a.stop_window, slot = t % W;
+        float *h = V1SM + v1_blk.L.oHIST + g * V1_WMAX;
+        const int rise = (t > 1 && Lt > v1_blk.lprev[g]) ? v1_blk.rise[g] + 1 : 0;
+        if (t > W && fabsf(Lt - h[slot]) < a.stop_tol) rule = 2;      // h[slot] still holds L_(t-W)
+        else if (rise >= W) rule = 3;
+        h[slot] = Lt;
+        v1_blk.rise[g] = rise;
+        v1_blk.lprev[g] = Lt;
+        if (rule) { v1_blk.stop_rule[g] = rule; v1_blk.nsteps[g] = t - 1; }
+    }
+    rule = __shfl_sync(FULL, rule, 0);
+    return rule == 0;
+}
+
+// ------------------------------------------------------------------------------------------
 // lasp_fit_batch: a1-a9 for groups of GS spectra, persistent CTAs
 // ------------------------------------------------------------------------------------------
 template <int MAXT, int MINB, bool STREAM>
@@ -1947,6 +1988,12 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
             v1_param_setup(g);
         }
         float pb1 = 1.f, pb2 = 1.f;
+        const bool stopmode = a.stop_window > 0;
+        if (threadIdx.x < GS) {
+            v1_blk.stop_rule[threadIdx.x] = 0; v1_blk.nsteps[threadIdx.x] = a.n_iter;
+            v1_blk.rise[threadIdx.x] = 0; v1_blk.lprev[threadIdx.x] = 0.f;
+        }
+        int tdone = 0;
         for (int t = 1; t <= a.n_iter; ++t) {
 #ifdef LASP_PHASE_TIMING
             const long long te0 = a.dbg ? clock64() : 0;
@@ -1954,13 +2001,16 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
             // fresh Gram factor on each of the first `warm` steps (the model moves fastest there), then every `refresh`-th
             // step, or (refresh == 0) when the drift monitor asks for it
             const int momsel = t <= a.warm ? 1 : (a.refresh >= 1 ? ((t - 1) % a.refresh == 0 ? 1 : 0) : 2);
-            v1_evaluate<0, STREAM>(t == 1, momsel, nullptr, t > 1 && L.fastw, false, true);
+            v1_evaluate<0, STREAM>(t == 1, momsel, nullptr, t > 1 && L.fastw, stopmode, true);
+            tdone = t;
 #ifdef LASP_PHASE_TIMING
             if (a.dbg && V1_TID == 0) { atomicAdd(a.dbg + 14, (unsigned long long)(clock64() - te0)); atomicAdd(a.dbg + 15, 1ull); }
             const long long tu0 = a.dbg ? clock64() : 0;
 #endif
             pb1 *= a.b1; pb2 *= a.b2;
-            if (g < GS) {
+            bool upd = g < GS;
+            if (stopmode && upd) upd = v1_stop_test(g, t);     // a stopped spectrum keeps its iterate
+            if (upd) {
                 const float ib1 = 1.f / (1.f - pb1), ib2 = 1.f / (1.f - pb2);   // bias corrections (C.2-20)
                 if (L.fastupd) v1_update_fast(g, ib1, ib2);
                 else {
@@ -1997,8 +2047,15 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
 #ifdef LASP_PHASE_TIMING
             if (a.dbg && V1_TID == 0) atomicAdd(a.dbg + 13, (unsigned long long)(clock64() - tu0));
 #endif
+            if (stopmode) {   // the group ends when every spectrum of it has stopped
+                __syncthreads();
+                bool all = true;
+#pragma unroll
+                for (int q = 0; q < GS; ++q) all = all && v1_blk.stop_rule[q] != 0;
+                if (all) break;
+            }
         }
-        if (a.stats && V1_TID == 0) { atomicAdd(a.stats, (unsigned long long)a.n_iter); atomicAdd(a.stats + 1, (unsigned long long)v1_blk.nfresh); }
+        if (a.stats && V1_TID == 0) { atomicAdd(a.stats, (unsigned long long)tdone); atomicAdd(a.stats + 1, (unsigned long long)v1_blk.nfresh); }
         // a9: one more evaluation at the final iterate (C.2-21)
         v1_evaluate<1, STREAM>(a.n_iter == 0, 1, nullptr);
         float chi2 = 0.f, ngood = 0.f, cmin = 0.f;
@@ -2020,6 +2077,8 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
             if (bound) st |= LASP_ST_ON_BOUND;
             if (!fin) st |= LASP_ST_NONFINITE;
             if (ngood > 0.f && cmin <= 0.f) st |= LASP_ST_NEG_CONT;
+            if (v1_blk.stop_rule[g] == 2) st |= LASP_ST_STOP_TOL;
+            if (v1_blk.stop_rule[g] == 3) st |= LASP_ST_STOP_RISE;
             if (valid) {
                 const long long i = v1_blk.spec[g];
                 for (int p = V1_LANE; p < NP; p += 32)
@@ -2027,6 +2086,7 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
                 if (V1_LANE == 0) {
                     a.chi2[i] = chi2;
                     if (a.status) a.status[i] = st;
+                    if (a.nsteps) a.nsteps[i] = v1_blk.nsteps[g];
                 }
                 if (a.cont) v1_write_cont(g, a.cont + i * M.nc);
             }

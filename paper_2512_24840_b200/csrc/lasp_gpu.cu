@@ -63,7 +63,7 @@ struct lasp_ctx {
         int64_t cap = 0;
         float *flux[2] = {}, *ivar[2] = {}, *init[2] = {}, *params[2] = {}, *cont[2] = {}, *chi2[2] = {}, *err[2] = {};
         uint8_t *mask[2] = {};
-        int32_t *status[2] = {};
+        int32_t *status[2] = {}, *nsteps[2] = {};
         cudaStream_t s_in = nullptr, s_out = nullptr, s_fit = nullptr;
         cudaEvent_t in_done[2] = {}, fit_done[2] = {}, out_done[2] = {};
     } hp;
@@ -431,6 +431,7 @@ static void setup_variant(lasp_ctx *c, const cudaDeviceProp &prop, int emax, boo
         L.oEXP = take(std::max((M.K * M.L + 3) / 4, M.K));   // bytes [K][L], or one packed word per term when L <= 4
         L.oXP = take(GS * M.L * (L.emax + 1)); L.oDPHI = take(GS * M.L * M.K); L.oGSC = take(GS * M.NP);
         L.oNP = take(GS * 8);
+        L.oHIST = take(GS * V1_WMAX);
         L.total = o;
         bytes = (size_t)o * sizeof(float);
         if (bytes + 2048 <= prop.sharedMemPerBlockOptin) break;   // + the kernels' static block state
@@ -451,7 +452,7 @@ static void setup_variant(lasp_ctx *c, const cudaDeviceProp &prop, int emax, boo
 // ------------------------------------------------------------------------------------------
 // options, workspace, launches
 // ------------------------------------------------------------------------------------------
-static const lasp_fit_opts kDefaultOpts = {0, 1e-2f, 0.9f, 0.999f, 1e-8f, 0, 0, 0, 0, 0};
+static const lasp_fit_opts kDefaultOpts = {0, 1e-2f, 0.9f, 0.999f, 1e-8f, 0, 0, 0, 0, 0, 0, 0.f};
 
 // variant / emulator path of one call (opts may be null: defaults)
 static int resolve(lasp_ctx *c, const lasp_fit_opts *o, const char *who, const Variant **v, bool *mma)
@@ -462,6 +463,8 @@ static int resolve(lasp_ctx *c, const lasp_fit_opts *o, const char *who, const V
         return fail(c, LASP_ERR_INVALID_ARG, std::string(who) + ": emulator_path must be 0, 1 or 2");
     if (o->refresh < 0 || o->warm < 0 || o->fd_fresh < 0 || o->fd_fresh > 1)
         return fail(c, LASP_ERR_INVALID_ARG, std::string(who) + ": refresh, warm must be >= 0 and fd_fresh 0 or 1");
+    if (o->stop_window < 0 || o->stop_window > V1_WMAX || (o->stop_window > 0 && !(o->stop_tol >= 0.f)))
+        return fail(c, LASP_ERR_INVALID_ARG, std::string(who) + ": stop_window must be in [0, 128] and stop_tol >= 0");
     const Variant *vv = nullptr;
     if (o->variant == 1) vv = c->res.ok ? &c->res : nullptr;
     else if (o->variant == 2) vv = c->str.ok ? &c->str : nullptr;
@@ -594,7 +597,7 @@ static int launch(lasp_ctx *c, const void *const *table, const Variant &v, const
 extern "C" int lasp_fit_batch(lasp_ctx *c, int64_t B, const float *flux, const float *ivar,
                               const uint8_t *mask, const float *init, const lasp_fit_opts *opts,
                               float *params, float *cont, float *chi2, float *err, int32_t *status,
-                              void *stream)
+                              int32_t *n_steps, void *stream)
 {
     if (!c) return fail(nullptr, LASP_ERR_INVALID_ARG, "null ctx");
     if (B < 1 || !flux || !ivar || !init || !opts || !params || !chi2)
@@ -625,6 +628,7 @@ extern "C" int lasp_fit_batch(lasp_ctx *c, int64_t B, const float *flux, const f
     a.refresh = opts->refresh;
     a.fdfresh = opts->fd_fresh;
     a.drift_tol = 6.4e-3f;   // = 64 steps x (1e-2)^2: the fixed schedule the parity suite was tuned at
+    a.stop_window = opts->stop_window; a.stop_tol = opts->stop_tol; a.nsteps = n_steps;
     CUDA_TRY(c, cudaMemsetAsync(c->dqueue, 0, sizeof(unsigned int), st));
     CUDA_TRY(c, cudaMemsetAsync(c->dstats, 0, 2 * sizeof(unsigned long long), st));
     a.queue = c->dqueue;
@@ -733,9 +737,9 @@ static void hostpipe_free(lasp_ctx *c)
     lasp_ctx::HostPipe &h = c->hp;
     for (int s = 0; s < 2; ++s) {
         cudaFree(h.flux[s]); cudaFree(h.ivar[s]); cudaFree(h.mask[s]); cudaFree(h.init[s]);
-        cudaFree(h.params[s]); cudaFree(h.cont[s]); cudaFree(h.chi2[s]); cudaFree(h.err[s]); cudaFree(h.status[s]);
+        cudaFree(h.params[s]); cudaFree(h.cont[s]); cudaFree(h.chi2[s]); cudaFree(h.err[s]); cudaFree(h.status[s]); cudaFree(h.nsteps[s]);
         h.flux[s] = h.ivar[s] = h.init[s] = h.params[s] = h.cont[s] = h.chi2[s] = h.err[s] = nullptr;
-        h.mask[s] = nullptr; h.status[s] = nullptr;
+        h.mask[s] = nullptr; h.status[s] = nullptr; h.nsteps[s] = nullptr;
     }
     h.cap = 0;
 }
@@ -767,6 +771,7 @@ static int hostpipe_reserve(lasp_ctx *c, int64_t chunk)
         CUDA_TRY(c, cudaMalloc(&h.chi2[s], n * sizeof(float)));
         CUDA_TRY(c, cudaMalloc(&h.err[s], n * M.NP * sizeof(float)));
         CUDA_TRY(c, cudaMalloc(&h.status[s], n * sizeof(int32_t)));
+        CUDA_TRY(c, cudaMalloc(&h.nsteps[s], n * sizeof(int32_t)));
     }
     h.cap = chunk;
     return LASP_OK;
@@ -774,7 +779,7 @@ static int hostpipe_reserve(lasp_ctx *c, int64_t chunk)
 
 static int hostpipe_run(lasp_ctx *c, int64_t B, const float *flux, const float *ivar, const uint8_t *mask,
                         const float *init, const lasp_fit_opts *opts, float *params, float *cont, float *chi2,
-                        float *err, int32_t *status, int64_t chunk)
+                        float *err, int32_t *status, int32_t *n_steps, int64_t chunk)
 {
     lasp_ctx::HostPipe &h = c->hp;
     const ModelDev &M = c->M;
@@ -801,7 +806,7 @@ static int hostpipe_run(lasp_ctx *c, int64_t B, const float *flux, const float *
         if (i >= 2) CUDA_TRY(c, cudaStreamWaitEvent(h.s_fit, h.out_done[s], 0));   // slot's old results copied out
         rc = lasp_fit_batch(c, n, h.flux[s], h.ivar[s], mask ? h.mask[s] : nullptr, h.init[s], opts, h.params[s],
                             cont ? h.cont[s] : nullptr, h.chi2[s], err ? h.err[s] : nullptr,
-                            status ? h.status[s] : nullptr, h.s_fit);
+                            status ? h.status[s] : nullptr, n_steps ? h.nsteps[s] : nullptr, h.s_fit);
         if (rc) return rc;
         CUDA_TRY(c, cudaEventRecord(h.fit_done[s], h.s_fit));
         CUDA_TRY(c, cudaStreamWaitEvent(h.s_out, h.fit_done[s], 0));
@@ -810,6 +815,7 @@ static int hostpipe_run(lasp_ctx *c, int64_t B, const float *flux, const float *
         if (cont) CUDA_TRY(c, cudaMemcpyAsync(cont + o * M.nc, h.cont[s], (size_t)n * M.nc * sizeof(float), cudaMemcpyDeviceToHost, h.s_out));
         if (err) CUDA_TRY(c, cudaMemcpyAsync(err + o * M.NP, h.err[s], (size_t)n * M.NP * sizeof(float), cudaMemcpyDeviceToHost, h.s_out));
         if (status) CUDA_TRY(c, cudaMemcpyAsync(status + o, h.status[s], (size_t)n * sizeof(int32_t), cudaMemcpyDeviceToHost, h.s_out));
+        if (n_steps) CUDA_TRY(c, cudaMemcpyAsync(n_steps + o, h.nsteps[s], (size_t)n * sizeof(int32_t), cudaMemcpyDeviceToHost, h.s_out));
         CUDA_TRY(c, cudaEventRecord(h.out_done[s], h.s_out));
     }
     return LASP_OK;
@@ -818,7 +824,7 @@ static int hostpipe_run(lasp_ctx *c, int64_t B, const float *flux, const float *
 extern "C" int lasp_fit_batch_host(lasp_ctx *c, int64_t B, const float *flux, const float *ivar,
                                    const uint8_t *mask, const float *init, const lasp_fit_opts *opts,
                                    float *params, float *cont, float *chi2, float *err, int32_t *status,
-                                   int64_t chunk)
+                                   int32_t *n_steps, int64_t chunk)
 {
     if (!c) return fail(nullptr, LASP_ERR_INVALID_ARG, "null ctx");
     if (B < 1 || !flux || !ivar || !init || !opts || !params || !chi2 || chunk < 0)
@@ -828,7 +834,7 @@ extern "C" int lasp_fit_batch_host(lasp_ctx *c, int64_t B, const float *flux, co
     chunk = std::min<int64_t>(chunk, B);
     int rc = hostpipe_reserve(c, chunk);
     if (rc) return rc;
-    rc = hostpipe_run(c, B, flux, ivar, mask, init, opts, params, cont, chi2, err, status, chunk);
+    rc = hostpipe_run(c, B, flux, ivar, mask, init, opts, params, cont, chi2, err, status, n_steps, chunk);
     // success or not, nothing of this call may still be in flight on the private streams when it returns: the
     // copies read and write the caller's buffers
     const std::string first = c->err;

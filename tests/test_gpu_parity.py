@@ -528,3 +528,60 @@ def test_fit_long_spectrum_streaming_16_at_100_steps(gpu, oracle_mod):
     m1 = gpu.LaspModel(synth.make_case(0, oracle_mod.forward, B=1)["desc"])
     assert m1.default_variant() == 1
     m1.close()
+
+
+# ------------------------------------------------------------------ the paper's stopping rules (NEXT-2)
+
+def test_stopping_rules_structure(gpu, oracle_mod):
+    """stop_window = 50 with an infinite tolerance: every spectrum stops at the first testable step (t = 51, 50 updates,
+    bit LASP_ST_STOP_TOL) and returns exactly the fixed-step fit of 50 steps; with stop_tol = 0 nothing fires, n_iter
+    updates are applied and the result is exactly the fixed-step fit; both as the oracle's orc_fit_stop."""
+    case = synth.make_case(1, oracle_mod.forward, B=10)
+    m = gpu.LaspModel(case["desc"])
+    o = oracle_mod.Oracle(case["desc"])
+    args = (case["flux"], case["ivar"], case["mask"], case["init"])
+    r = m.fit_batch(*args, 200, lr=0.05, stop_window=50, stop_tol=1e30)
+    fixed = m.fit_batch(*args, 50, lr=0.05)
+    assert np.array_equal(r["n_steps"].cpu().numpy(), np.full(10, 50))
+    st = r["status"].cpu().numpy()
+    assert np.all(st & gpu.LASP_ST_STOP_TOL) and not np.any(st & gpu.LASP_ST_STOP_RISE)
+    assert np.array_equal(r["params"].cpu().numpy(), fixed["params"].cpu().numpy())
+    ref = o.fit_stop(*args, 200, lr=0.05, tol=1e30)
+    compare_fit(case, o, r, ref)
+    assert np.array_equal(ref["n_steps"], np.full(10, 50))
+    r = m.fit_batch(*args, 70, lr=0.05, stop_window=50, stop_tol=0.0)
+    fixed = m.fit_batch(*args, 70, lr=0.05)
+    assert np.array_equal(r["n_steps"].cpu().numpy(), np.full(10, 70))
+    assert not np.any(r["status"].cpu().numpy() & (gpu.LASP_ST_STOP_TOL | gpu.LASP_ST_STOP_RISE))
+    assert np.array_equal(r["params"].cpu().numpy(), fixed["params"].cpu().numpy())
+    assert np.array_equal(fixed["n_steps"].cpu().numpy(), np.full(10, 70))      # fixed-step mode reports n_iter
+    m.close()
+
+
+@pytest.mark.slow
+def test_stopping_rules_at_the_papers_settings(gpu, oracle_mod):
+    """lr = 0.1, at most 5000 iterations, window 50, tolerance 1e-5 on config-0 and config-1 subsets.
+    The stop step is decided by a floating-point comparison on a loss that the two sides hold in different precision
+    (fp32 / fp64), so it is unique only up to the step at which |L_t - L_(t-50)| crosses the tolerance within rounding:
+    the rule that fired must be the same, the stop step within a few steps, and parameters / chi2 / status inside the
+    usual tolerances.  Spectra of one CTA group stop at different steps (the stopped ones are frozen while the group
+    runs on): each must equal the kernel's own fixed-step fit cut at its stop step."""
+    for cfg_id, B in ((0, 24), (1, 24)):
+        case = synth.make_case(cfg_id, oracle_mod.forward, B=B)
+        m = gpu.LaspModel(case["desc"])
+        o = oracle_mod.Oracle(case["desc"])
+        args = (case["flux"], case["ivar"], case["mask"], case["init"])
+        r = m.fit_batch(*args, 5000, lr=0.1, stop_window=50, stop_tol=1e-5)
+        ref = o.fit_stop(*args, 5000, lr=0.1)
+        ns, st = r["n_steps"].cpu().numpy(), r["status"].cpu().numpy()
+        assert np.all(ref["n_steps"] < 5000) and np.all(ns < 5000)
+        assert np.array_equal(st & 48, ref["status"] & 48)                      # the same criterion fired
+        assert np.abs(ns - ref["n_steps"]).max() <= 5, (ns, ref["n_steps"])
+        ref_cmp = dict(ref, status=ref["status"])
+        compare_fit(case, o, r, ref_cmp)
+        assert len(set(ns[:4].tolist())) > 1 or len(set(ns.tolist())) > 1         # stop steps do differ between spectra
+        for n in sorted(set(ns.tolist()))[:3]:
+            fixed = m.fit_batch(*args, int(n), lr=0.1)
+            sel = ns == n
+            assert np.array_equal(r["params"].cpu().numpy()[sel], fixed["params"].cpu().numpy()[sel])
+        m.close()
