@@ -564,12 +564,35 @@ __device__ __forceinline__ void v1_group_range(const SegDev &sg, int &lo, int &h
     hi = sg.fit_hi + (rh + OCT - 1) / OCT * OCT;
 }
 
+
+// T range of a phase: the fitted octets plus the group's reach (full = 0), or the whole segment plus the reach, inside
+// the halo (full = 1: lasp_eval_model).  The phases take the segment INDEX and derive everything from the block state:
+// a reference or a range passed in would have to be kept alive across the (non-inlined) phase calls by the caller,
+// i.e. spilled to local memory and reloaded behind every call.
+__device__ __forceinline__ void v1_phase_range(const SegDev &sg, int full, int &lo, int &hi)
+{
+    if (!full) { v1_group_range(sg, lo, hi); return; }
+    const int *tap = (const int *)(V1SM + v1_blk.L.oTAP);
+    int rl = 0, rh = 0;
+#pragma unroll
+    for (int q = 0; q < GS; ++q) {
+        rl = max(rl, 4 * (tap[2 * q] + tap[2 * q + 1] - 1));
+        rh = max(rh, -4 * tap[2 * q] + 4);
+    }
+    const int seg_lo = sg.po + sg.halo, seg_hi = seg_lo + (sg.P + OCT - 1) / OCT * OCT;
+    lo = max(sg.po, seg_lo - (rl + OCT - 1) / OCT * OCT);
+    hi = min(sg.po + sg.len, seg_hi + (rh + OCT - 1) / OCT * OCT);
+}
+
 // ------------------------------------------------------------------------------------------
 // a2: T_j = sum_k phi_k C[k,j] over the padded range [lo,hi) -> shared row T (Eq. 1)
 // ------------------------------------------------------------------------------------------
 template <bool STREAM>
-__device__ __noinline__ void v1_phase_emulator(const SegDev &sg, int lo, int hi)
+__device__ __noinline__ void v1_phase_emulator(int s_, int full)
 {
+    const SegDev &sg = v1_blk.M.seg[s_];
+    int lo, hi;
+    v1_phase_range(sg, full, lo, hi);
     // everything the loop needs is copied to registers first: the model lives in shared memory, and after
     // any shared-memory store the compiler would otherwise have to re-read it
     const float4 *phi4 = (const float4 *)(V1SM + v1_blk.L.oPHI);
@@ -652,8 +675,11 @@ __device__ __forceinline__ void v1_mma_tf32(float (&d)[4], float a0, float a1, f
 
 // NCH = number of chunks of four k-steps (32 terms) whose B fragments are held in registers: K <= 32 * NCH
 template <int NCH>
-__device__ __noinline__ void v1_phase_emulator_mma(const SegDev &sg, int lo, int hi)
+__device__ __noinline__ void v1_phase_emulator_mma(int s_, int full)
 {
+    const SegDev &sg = v1_blk.M.seg[s_];
+    int lo, hi;
+    v1_phase_range(sg, full, lo, hi);
     const int lane = V1_LANE, gid = lane >> 2, tig = lane & 3, K = v1_blk.M.K, ks = v1_blk.A.ksteps;
     const int RL = v1_blk.L.RL, sweep = v1_blk.L.NW * 256;
     const float4 *CF = v1_blk.A.CF + lane;
@@ -849,8 +875,9 @@ __device__ __forceinline__ void v1_mirror_combine(float (&x)[GS][OCT])
 // land in this warp's reduction slots.
 // ------------------------------------------------------------------------------------------
 template <bool UNI, bool STREAM>
-__device__ __noinline__ void v1_phase_forward(const SegDev &sg, bool stencil)
+__device__ __noinline__ void v1_phase_forward(int s_, bool stencil)
 {
+    const SegDev &sg = v1_blk.M.seg[s_];
     const V1Args &a = v1_blk.A;
     const V1Lay &L = v1_blk.L;
     const int *tap = (const int *)(V1SM + L.oTAP);
@@ -952,8 +979,9 @@ __device__ __noinline__ void v1_phase_forward(const SegDev &sg, bool stencil)
 // from L2 again).  Kept apart from v1_phase_forward so that the every-step code stays small.
 // ------------------------------------------------------------------------------------------
 template <bool STREAM>
-__device__ __noinline__ void v1_phase_moments(const SegDev &sg)
+__device__ __noinline__ void v1_phase_moments(int s_)
 {
+    const SegDev &sg = v1_blk.M.seg[s_];
     const V1Lay &L = v1_blk.L;
     float *red = V1SM + L.oRED + V1_WARP * L.VR * GS;
     constexpr bool SYM = !STREAM;
@@ -1184,8 +1212,10 @@ __device__ __noinline__ void v1_phase_solve(int g, int seg, bool refactor)
 // chi2 / ngood / cmin are reduced over the warp and accumulated in this warp's SLOT_STAT slots (zeroed by v1_evaluate).
 // ------------------------------------------------------------------------------------------
 template <int MODE, bool UNI, bool STREAM>
-__device__ __noinline__ void v1_phase_residual(const SegDev &sg, int rowB, float *xrow)
+__device__ __noinline__ void v1_phase_residual(int s_, float *xrow)
 {
+    const SegDev &sg = v1_blk.M.seg[s_];
+    const int rowB = s_ * v1_blk.M.n1;
     const V1Args &a = v1_blk.A;
     const V1Lay &L = v1_blk.L;
     const float4 *b4 = (const float4 *)(V1SM + L.oB) + rowB;
@@ -1336,8 +1366,11 @@ __device__ __noinline__ void v1_phase_residual(const SegDev &sg, int rowB, float
 // the two kernel-parameter gradients), which v1_evaluate zeroed.
 // ------------------------------------------------------------------------------------------
 template <bool UNI, bool STREAM>
-__device__ __noinline__ void v1_phase_adjoint(const SegDev &sg, int lo, int hi)
+__device__ __noinline__ void v1_phase_adjoint(int s_)
 {
+    const SegDev &sg = v1_blk.M.seg[s_];
+    int lo, hi;
+    v1_phase_range(sg, 0, lo, hi);
     const V1Lay &L = v1_blk.L;
     const int *tap = (const int *)(V1SM + L.oTAP);
     const int P4 = v1_blk.M.Ppad >> 2, P8 = v1_blk.M.Ppad >> 3, K = v1_blk.M.K, Kq = L.Kq, NA = L.NA, RL = L.RL, nt8 = V1_NT * OCT;
@@ -1436,6 +1469,35 @@ __device__ __noinline__ void v1_phase_adjoint(const SegDev &sg, int lo, int hi)
     }
 }
 
+// After the first barrier of an evaluation: this warp's Q and statistics slots, which accumulate over sweeps and
+// segments, are zeroed (only now have warps g < GS finished reading the previous evaluation's), and for the
+// evaluations of the Adam loop thread 0 takes the Gram re-factorisation decision (momsel 0 / 1: as told; 2: adaptive,
+// from what the update warps left before the barrier) and publishes it in v1_blk.momflag, read after the next barrier.
+__device__ __forceinline__ void v1_begin_eval(int momsel, bool adam)
+{
+    const V1Lay &L = v1_blk.L;
+    float *red = V1SM + L.oRED + V1_WARP * L.VR * GS;
+    const int q0 = (L.nmomr + L.n1r) * GS;
+    for (int i = q0 + V1_LANE; i < L.VR * GS; i += 32) red[i] = 0.f;
+    __syncwarp();
+    if (V1_LANE < GS) red[(SLOT_STAT(L) + 2) * GS + V1_LANE] = 3.0e38f;
+    __syncwarp();
+    if (V1_TID == 0 && adam) {
+        bool fresh = momsel == 1;
+        if (momsel == 2) {
+            const float step = __int_as_float(v1_blk.stepmax);
+            const float drift = v1_blk.drift + step;
+            const int since = v1_blk.since + 1;
+            fresh = v1_blk.failmask != 0u || since >= 64 || drift * step > v1_blk.A.drift_tol;
+            v1_blk.drift = fresh ? 0.f : drift;
+            v1_blk.since = fresh ? 0 : since;
+            v1_blk.stepmax = 0;
+        }
+        if (fresh) v1_blk.nfresh += 1;
+        v1_blk.momflag = fresh ? 1 : 0;
+    }
+}
+
 // ------------------------------------------------------------------------------------------
 // One evaluation of chi2 (+ gradient) at the u held in shared memory (warps g < GS have run
 // v1_param_setup for their spectrum).  All threads of the CTA call this.
@@ -1469,15 +1531,7 @@ __device__ __noinline__ void v1_evaluate(bool cold, int momsel, float *xrow, boo
     if (M.n_seg > 1 && !L.lfseg) momsel = 1;   // one factor slot shared by the segments: never stale
     bool mom = momsel == 1;
     bool zeroed = false;
-    auto zero_slots = [&]() {
-        float *red = V1SM + L.oRED + V1_WARP * L.VR * GS;
-        const int q0 = (L.nmomr + L.n1r) * GS;
-        for (int i = q0 + V1_LANE; i < L.VR * GS; i += 32) red[i] = 0.f;
-        __syncwarp();
-        if (V1_LANE < GS) red[(SLOT_STAT(L) + 2) * GS + V1_LANE] = 3.0e38f;
-        __syncwarp();
-        zeroed = true;
-    };
+    auto zero_slots = [&]() { v1_begin_eval(momsel, adam); zeroed = true; };
     for (int s = 0; s < M.n_seg; ++s) {
         const SegDev &sg = M.seg[s];
         const int rowB = s * M.n1;
@@ -1507,38 +1561,20 @@ __device__ __noinline__ void v1_evaluate(bool cold, int momsel, float *xrow, boo
         tick(0);
         __syncthreads();
         tick(1);
-        if (!zeroed) {
-            zero_slots();
-            if (V1_TID == 0 && adam) {   // Gram re-factorisation decision from what the update warps left before the barrier
-                bool fresh = momsel == 1;
-                if (momsel == 2) {
-                    const float step = __int_as_float(v1_blk.stepmax);
-                    const float drift = v1_blk.drift + step;
-                    const int since = v1_blk.since + 1;
-                    fresh = v1_blk.failmask != 0u || since >= 64 || drift * step > a.drift_tol;
-                    v1_blk.drift = fresh ? 0.f : drift;
-                    v1_blk.since = fresh ? 0 : since;
-                    v1_blk.stepmax = 0;
-                    v1_blk.momflag = fresh ? 1 : 0;
-                }
-                if (fresh) v1_blk.nfresh += 1;
-            }
-        }
-        int lo, hi;
-        v1_group_range(sg, lo, hi);
+        if (!zeroed) zero_slots();
         if (!STREAM && v1_blk.A.CF) {
             const int ks = v1_blk.A.ksteps;
-            if (ks <= 4) v1_phase_emulator_mma<1>(sg, lo, hi);
-            else if (ks <= 8) v1_phase_emulator_mma<2>(sg, lo, hi);
-            else v1_phase_emulator_mma<4>(sg, lo, hi);
+            if (ks <= 4) v1_phase_emulator_mma<1>(s, 0);
+            else if (ks <= 8) v1_phase_emulator_mma<2>(s, 0);
+            else v1_phase_emulator_mma<4>(s, 0);
         } else
-            v1_phase_emulator<STREAM>(sg, lo, hi);
+            v1_phase_emulator<STREAM>(s, 0);
         tick(2);
         __syncthreads();
         tick(3);
-        if (momsel == 2) mom = v1_blk.momflag != 0;
-        if (sg.uniform) v1_phase_forward<true, STREAM>(sg, true); else v1_phase_forward<false, STREAM>(sg, true);
-        if (mom || cold) v1_phase_moments<STREAM>(sg);   // own octets of row A only: no barrier needed in between
+        if (adam) mom = v1_blk.momflag != 0;
+        if (sg.uniform) v1_phase_forward<true, STREAM>(s, true); else v1_phase_forward<false, STREAM>(s, true);
+        if (mom || cold) v1_phase_moments<STREAM>(s);   // own octets of row A only: no barrier needed in between
         tick(4);
         __syncthreads();
         tick(5);
@@ -1547,21 +1583,21 @@ __device__ __noinline__ void v1_evaluate(bool cold, int momsel, float *xrow, boo
         __syncthreads();
         tick(7);
         if (cold) {
-            v1_phase_residual<0, true, STREAM>(sg, rowB, nullptr);
+            v1_phase_residual<0, true, STREAM>(s, nullptr);
             __syncthreads();   // c_prev written by this thread only, but keep phases aligned
-            v1_phase_forward<true, STREAM>(sg, false);   // S is re-read from row A: no stencil, either kind
+            v1_phase_forward<true, STREAM>(s, false);   // S is re-read from row A: no stencil, either kind
             __syncthreads();
             if (V1_WARP < GS) v1_phase_solve(V1_WARP, s, false);
             __syncthreads();
         }
-        if (MODE == 0 && !stats && sg.uniform) v1_phase_residual<3, true, STREAM>(sg, rowB, xrow);   // Adam step: no statistics
-        else if (sg.uniform) v1_phase_residual<(MODE == 2 ? 2 : 1), true, STREAM>(sg, rowB, xrow);
-        else v1_phase_residual<(MODE == 2 ? 2 : 1), false, STREAM>(sg, rowB, xrow);
+        if (MODE == 0 && !stats && sg.uniform) v1_phase_residual<3, true, STREAM>(s, xrow);   // Adam step: no statistics
+        else if (sg.uniform) v1_phase_residual<(MODE == 2 ? 2 : 1), true, STREAM>(s, xrow);
+        else v1_phase_residual<(MODE == 2 ? 2 : 1), false, STREAM>(s, xrow);
         tick(8);
         __syncthreads();
         tick(9);
         if (MODE == 0) {
-            if (sg.uniform) v1_phase_adjoint<true, STREAM>(sg, lo, hi); else v1_phase_adjoint<false, STREAM>(sg, lo, hi);
+            if (sg.uniform) v1_phase_adjoint<true, STREAM>(s); else v1_phase_adjoint<false, STREAM>(s);
             tick(10);
             __syncthreads();
             tick(11);
@@ -1929,6 +1965,32 @@ __device__ __noinline__ void v1_errors(float chi2_g, float ngood_g, bool valid_g
 }
 
 // ------------------------------------------------------------------------------------------
+// One evaluation of the Adam loop in the common case -- ONE uniform (log-grid) segment, warm start, the kernel weights
+// already prepared by v1_update_fast -- as a straight line of phase calls that keeps NOTHING alive across them: what a
+// later phase needs (the re-factorisation flag, whether statistics are wanted) is re-read from the block state.  In the
+// general v1_evaluate every value kept across a call is spilled to local memory and reloaded behind it, a round trip
+// that misses the small L1 and sits on the critical path six times per step (profiles/r02_ncu.md).
+// ------------------------------------------------------------------------------------------
+template <bool STREAM>
+__device__ __noinline__ void v1_step_hot(int momsel)
+{
+    __syncthreads();
+    v1_begin_eval(momsel, true);
+    v1_phase_emulator<STREAM>(0, 0);
+    __syncthreads();
+    v1_phase_forward<true, STREAM>(0, true);
+    if (v1_blk.momflag != 0) v1_phase_moments<STREAM>(0);
+    __syncthreads();
+    if (V1_WARP < GS) v1_phase_solve(V1_WARP, 0, v1_blk.momflag != 0);
+    __syncthreads();
+    if (v1_blk.A.stop_window > 0) v1_phase_residual<1, true, STREAM>(0, nullptr);   // stopping rules read chi2
+    else v1_phase_residual<3, true, STREAM>(0, nullptr);
+    __syncthreads();
+    v1_phase_adjoint<true, STREAM>(0);
+    __syncthreads();
+}
+
+// ------------------------------------------------------------------------------------------
 // The paper's stopping rules (step 8), per spectrum (Delta-2), warp g for spectrum g, called after the t-th
 // evaluation and before update t (readings R-2..R-5 of DESIGN.md, as oracle/lasp_oracle.c orc_fit_stop):
 //   loss L_t = sqrt(chi2_t / n_pix) (Eq. 9 restricted to one spectrum);
@@ -2001,7 +2063,8 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
             // fresh Gram factor on each of the first `warm` steps (the model moves fastest there), then every `refresh`-th
             // step, or (refresh == 0) when the drift monitor asks for it
             const int momsel = t <= a.warm ? 1 : (a.refresh >= 1 ? ((t - 1) % a.refresh == 0 ? 1 : 0) : 2);
-            v1_evaluate<0, STREAM>(t == 1, momsel, nullptr, t > 1 && L.fastw, stopmode, true);
+            if (t > 1 && L.fastw && !a.CF) v1_step_hot<STREAM>(momsel);
+            else v1_evaluate<0, STREAM>(t == 1, momsel, nullptr, t > 1 && L.fastw, stopmode, true);
             tdone = t;
 #ifdef LASP_PHASE_TIMING
             if (a.dbg && V1_TID == 0) { atomicAdd(a.dbg + 14, (unsigned long long)(clock64() - te0)); atomicAdd(a.dbg + 15, 1ull); }
@@ -2143,8 +2206,9 @@ lasp_v1_grad_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ 
 // nodes x^_j = -1 + 2 (j - o_s)/P_s, by Bonnet's recurrence shared by the GS spectra.
 // ------------------------------------------------------------------------------------------
 template <bool UNI, bool STREAM>
-__device__ __noinline__ void v1_phase_model(const SegDev &sg, int s, int grp)
+__device__ __noinline__ void v1_phase_model(int s, int grp)
 {
+    const SegDev &sg = v1_blk.M.seg[s];
     const V1Args &a = v1_blk.A;
     const V1Lay &L = v1_blk.L;
     const int *tap = (const int *)(V1SM + L.oTAP);
@@ -2230,24 +2294,15 @@ lasp_v1_model_kernel(const __grid_constant__ ModelDev M, const __grid_constant__
             if (g < GS) v1_setup_weights(sg, g);
             __syncthreads();
             // T over the whole segment plus the reach of the group's widest kernel (inside the halo: halo >= H + 18)
-            const int *tap = (const int *)(V1SM + L.oTAP);
-            int rl = 0, rh = 0;
-#pragma unroll
-            for (int q = 0; q < GS; ++q) {
-                rl = max(rl, 4 * (tap[2 * q] + tap[2 * q + 1] - 1));
-                rh = max(rh, -4 * tap[2 * q] + 4);
-            }
-            const int seg_lo = sg.po + sg.halo, seg_hi = seg_lo + (sg.P + OCT - 1) / OCT * OCT;
-            const int lo = max(sg.po, seg_lo - (rl + OCT - 1) / OCT * OCT), hi = min(sg.po + sg.len, seg_hi + (rh + OCT - 1) / OCT * OCT);
             if (!STREAM && a.CF) {
                 const int ks = a.ksteps;
-                if (ks <= 4) v1_phase_emulator_mma<1>(sg, lo, hi);
-                else if (ks <= 8) v1_phase_emulator_mma<2>(sg, lo, hi);
-                else v1_phase_emulator_mma<4>(sg, lo, hi);
+                if (ks <= 4) v1_phase_emulator_mma<1>(s, 1);
+                else if (ks <= 8) v1_phase_emulator_mma<2>(s, 1);
+                else v1_phase_emulator_mma<4>(s, 1);
             } else
-                v1_phase_emulator<STREAM>(sg, lo, hi);
+                v1_phase_emulator<STREAM>(s, 1);
             __syncthreads();
-            if (sg.uniform) v1_phase_model<true, STREAM>(sg, s, grp); else v1_phase_model<false, STREAM>(sg, s, grp);
+            if (sg.uniform) v1_phase_model<true, STREAM>(s, grp); else v1_phase_model<false, STREAM>(s, grp);
             __syncthreads();
         }
     }
