@@ -104,7 +104,7 @@ struct V1Np {          // per-spectrum scalars of a per-pixel-kernel segment
 #define SLOT_STAT(L_) ((L_).VR - 6)   // chi2, ngood, min c, dchi2/dv and dchi2/dsigma* of per-pixel-kernel segments
 
 // per-spectrum scalars in shared memory: SC[idx][GS]
-enum { SC_V = 0, SC_SIG, SC_CHI, SC_NGOOD, SC_CMIN, SC_GV, SC_GS, SC_FAIL, SC_N };
+enum { SC_V = 0, SC_SIG, SC_CHI, SC_NGOOD, SC_CMIN, SC_GV, SC_GS, SC_FAIL, SC_PB1, SC_PB2, SC_N };   // SC_PB*: beta1^t, beta2^t
 
 // 32 values per lane -> lane l returns the warp total of value l (31 shuffles)
 __device__ __forceinline__ float xreduce32(float (&x)[32], int lane)
@@ -165,6 +165,9 @@ struct V1Block {
     int stepmax;          // max over the group of |du|_inf of the last update, as the bits of a non-negative float (atomicMax)
     unsigned failmask;    // bit seg * GS + g: the last factorisation of that system was not positive definite
     unsigned int nfresh;  // fresh Adam steps of the current group (statistics)
+    int t;                // Adam step counter of the current group: evaluations of the Adam loop begun so far (thread 0
+                          // advances it in v1_begin_eval).  The loop state lives here, not in registers: a register kept
+                          // across the (non-inlined) evaluation and update calls is spilled and reloaded from local memory
     // stopping rules, per spectrum of the group (written by lane 0 of warp g)
     int stop_rule[GS];    // 0 = still optimising; 2 / 3 = stopped by criterion (2) / (3) of P:169-171
     int nsteps[GS];       // Adam updates applied
@@ -1495,6 +1498,7 @@ __device__ __forceinline__ void v1_begin_eval(int momsel, bool adam)
         }
         if (fresh) v1_blk.nfresh += 1;
         v1_blk.momflag = fresh ? 1 : 0;
+        v1_blk.t += 1;
     }
 }
 
@@ -1807,6 +1811,7 @@ __device__ __forceinline__ void v1_init_block(const ModelDev &M, const V1Lay &L,
         v1_blk.tg = a.TG ? a.TG + (size_t)blockIdx.x * GS * M.Ppad : nullptr;
         v1_blk.ag = a.AG ? a.AG + (size_t)blockIdx.x * GS * M.Ppad : nullptr;
         v1_blk.drift = 0.f; v1_blk.since = 0; v1_blk.momflag = 0; v1_blk.nfresh = 0; v1_blk.stepmax = 0; v1_blk.failmask = 0u;
+        v1_blk.t = 0;
     }
     if (M.L <= 4) {   // one word per term (v1_param_setup)
         for (int k = threadIdx.x; k < M.K; k += blockDim.x) {
@@ -1836,6 +1841,7 @@ __device__ __forceinline__ void v1_set_group(int grp)
     }
     if (threadIdx.x == 0) {
         v1_blk.drift = 0.f; v1_blk.since = 0; v1_blk.momflag = 0; v1_blk.nfresh = 0; v1_blk.stepmax = 0; v1_blk.failmask = 0u;
+        v1_blk.t = 0;
     }
 }
 
@@ -2049,14 +2055,17 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
             __syncwarp();
             v1_param_setup(g);
         }
-        float pb1 = 1.f, pb2 = 1.f;
         const bool stopmode = a.stop_window > 0;
         if (threadIdx.x < GS) {
             v1_blk.stop_rule[threadIdx.x] = 0; v1_blk.nsteps[threadIdx.x] = a.n_iter;
             v1_blk.rise[threadIdx.x] = 0; v1_blk.lprev[threadIdx.x] = 0.f;
+            SMV(L.oSC, SC_PB1, threadIdx.x) = 1.f; SMV(L.oSC, SC_PB2, threadIdx.x) = 1.f;
         }
-        int tdone = 0;
-        for (int t = 1; t <= a.n_iter; ++t) {
+        // v1_blk.t was zeroed by v1_set_group; every evaluation below starts with a barrier, after which thread 0 advances
+        // it, and ends with one, after which it is read again
+        for (;;) {
+            const int t = *(volatile int *)&v1_blk.t + 1;
+            if (t > a.n_iter) break;
 #ifdef LASP_PHASE_TIMING
             const long long te0 = a.dbg ? clock64() : 0;
 #endif
@@ -2065,15 +2074,17 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
             const int momsel = t <= a.warm ? 1 : (a.refresh >= 1 ? ((t - 1) % a.refresh == 0 ? 1 : 0) : 2);
             if (t > 1 && L.fastw && !a.CF) v1_step_hot<STREAM>(momsel);
             else v1_evaluate<0, STREAM>(t == 1, momsel, nullptr, t > 1 && L.fastw, stopmode, true);
-            tdone = t;
 #ifdef LASP_PHASE_TIMING
             if (a.dbg && V1_TID == 0) { atomicAdd(a.dbg + 14, (unsigned long long)(clock64() - te0)); atomicAdd(a.dbg + 15, 1ull); }
             const long long tu0 = a.dbg ? clock64() : 0;
 #endif
-            pb1 *= a.b1; pb2 *= a.b2;
-            bool upd = g < GS;
-            if (stopmode && upd) upd = v1_stop_test(g, t);     // a stopped spectrum keeps its iterate
+            bool upd = V1_WARP < GS;
+            if (stopmode && upd) upd = v1_stop_test(V1_WARP, *(volatile int *)&v1_blk.t);     // a stopped spectrum keeps its iterate
             if (upd) {
+                const int g = V1_WARP;
+                const float pb1 = SMV(L.oSC, SC_PB1, g) * a.b1, pb2 = SMV(L.oSC, SC_PB2, g) * a.b2;   // beta^t of this spectrum
+                __syncwarp();
+                if (V1_LANE == 0) { SMV(L.oSC, SC_PB1, g) = pb1; SMV(L.oSC, SC_PB2, g) = pb2; }
                 const float ib1 = 1.f / (1.f - pb1), ib2 = 1.f / (1.f - pb2);   // bias corrections (C.2-20)
                 if (L.fastupd) v1_update_fast(g, ib1, ib2);
                 else {
@@ -2118,7 +2129,7 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
                 if (all) break;
             }
         }
-        if (a.stats && V1_TID == 0) { atomicAdd(a.stats, (unsigned long long)tdone); atomicAdd(a.stats + 1, (unsigned long long)v1_blk.nfresh); }
+        if (a.stats && V1_TID == 0) { atomicAdd(a.stats, (unsigned long long)v1_blk.t); atomicAdd(a.stats + 1, (unsigned long long)v1_blk.nfresh); }
         // a9: one more evaluation at the final iterate (C.2-21)
         v1_evaluate<1, STREAM>(a.n_iter == 0, 1, nullptr);
         float chi2 = 0.f, ngood = 0.f, cmin = 0.f;
