@@ -286,34 +286,69 @@ __device__ __forceinline__ void v1_weights_uniform(const SegDev &sg, int g, floa
     H = min(max(H, 0), hcap);   // memory safety outside the prior box (halo >= Hmax + 18)
     const float i2 = 0.5f / (s * s);
     const int a_lo = -(H / 4), na = (H + 3) / 4 - a_lo + 1;
-    float sum = 0.f, s1 = 0.f, s2 = 0.f;
-    for (int i0 = 0; i0 < na * 4; i0 += 32) {
-        const int idx = i0 + V1_LANE;
-        const int k = 4 * (a_lo + (idx >> 2)) - 3 + (idx & 3);
-        const float d = (float)k - mu;
-        const float e = (idx < na * 4 && k >= -H && k <= H) ? expf(-d * d * i2) : 0.f;
-        sum += e; s1 = fmaf(e, d, s1); s2 = fmaf(e * d, d, s2);
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        sum += __shfl_xor_sync(FULL, sum, o); s1 += __shfl_xor_sync(FULL, s1, o); s2 += __shfl_xor_sync(FULL, s2, o);
-    }
-    const float inv = 1.f / sum;
-    const float e1n = s1 * inv, e2n = s2 * inv;       // kbar - mu ; second moment about mu
     const float is2 = 2.f * i2;                        // 1/sigma^2 (pixels)
     const float cmu = is2 * inv_s;                     // dS/dv      = (1/s) sum dg/dmu T
     const float csig = is2 * sqrtf(is2) * (sigstar / sigtot) * inv_s;
-    for (int i0 = 0; i0 < na * 4; i0 += 32) {
-        const int idx = i0 + V1_LANE;
-        if (idx < na * 4) {
+    if (na * 4 <= 64) {
+        // the usual case (H <= 29): a lane owns at most two table entries; the forward tap k and the reversed tap -k of
+        // an entry are exponentiated ONCE, kept in registers over the warp sums and scaled afterwards (this runs on one
+        // warp between two phases of all: every dependent operation is latency on the step's critical path)
+        float ef[2], er[2], df[2], dr[2];
+        float sum = 0.f, s1 = 0.f, s2 = 0.f;
+#pragma unroll
+        for (int it = 0; it < 2; ++it) {
+            const int idx = it * 32 + V1_LANE;
             const int k = 4 * (a_lo + (idx >> 2)) - 3 + (idx & 3);
-            const bool in = (k >= -H) && (k <= H);
-            const float df = (float)k - mu, dr = (float)(-k) - mu;
-            gw[idx] = in ? expf(-df * df * i2) * inv : 0.f;
-            const float gg = in ? expf(-dr * dr * i2) * inv : 0.f;
-            gr[idx] = gg;
-            gr[rs + idx] = gg * (dr - e1n) * cmu;
-            gr[2 * rs + idx] = gg * (dr * dr - e2n) * csig;
+            const bool in = idx < na * 4 && k >= -H && k <= H;
+            df[it] = (float)k - mu; dr[it] = (float)(-k) - mu;
+            ef[it] = in ? expf(-df[it] * df[it] * i2) : 0.f;
+            er[it] = in ? expf(-dr[it] * dr[it] * i2) : 0.f;
+            sum += ef[it]; s1 = fmaf(ef[it], df[it], s1); s2 = fmaf(ef[it] * df[it], df[it], s2);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            sum += __shfl_xor_sync(FULL, sum, o); s1 += __shfl_xor_sync(FULL, s1, o); s2 += __shfl_xor_sync(FULL, s2, o);
+        }
+        const float inv = 1.f / sum;
+        const float e1n = s1 * inv, e2n = s2 * inv;       // kbar - mu ; second moment about mu
+#pragma unroll
+        for (int it = 0; it < 2; ++it) {
+            const int idx = it * 32 + V1_LANE;
+            if (idx < na * 4) {
+                gw[idx] = ef[it] * inv;
+                const float gg = er[it] * inv;
+                gr[idx] = gg;
+                gr[rs + idx] = gg * (dr[it] - e1n) * cmu;
+                gr[2 * rs + idx] = gg * (dr[it] * dr[it] - e2n) * csig;
+            }
+        }
+    } else {
+        float sum = 0.f, s1 = 0.f, s2 = 0.f;
+        for (int i0 = 0; i0 < na * 4; i0 += 32) {
+            const int idx = i0 + V1_LANE;
+            const int k = 4 * (a_lo + (idx >> 2)) - 3 + (idx & 3);
+            const float d = (float)k - mu;
+            const float e = (idx < na * 4 && k >= -H && k <= H) ? expf(-d * d * i2) : 0.f;
+            sum += e; s1 = fmaf(e, d, s1); s2 = fmaf(e * d, d, s2);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            sum += __shfl_xor_sync(FULL, sum, o); s1 += __shfl_xor_sync(FULL, s1, o); s2 += __shfl_xor_sync(FULL, s2, o);
+        }
+        const float inv = 1.f / sum;
+        const float e1n = s1 * inv, e2n = s2 * inv;       // kbar - mu ; second moment about mu
+        for (int i0 = 0; i0 < na * 4; i0 += 32) {
+            const int idx = i0 + V1_LANE;
+            if (idx < na * 4) {
+                const int k = 4 * (a_lo + (idx >> 2)) - 3 + (idx & 3);
+                const bool in = (k >= -H) && (k <= H);
+                const float df = (float)k - mu, dr = (float)(-k) - mu;
+                gw[idx] = in ? expf(-df * df * i2) * inv : 0.f;
+                const float gg = in ? expf(-dr * dr * i2) * inv : 0.f;
+                gr[idx] = gg;
+                gr[rs + idx] = gg * (dr - e1n) * cmu;
+                gr[2 * rs + idx] = gg * (dr * dr - e2n) * csig;
+            }
         }
     }
     if (V1_LANE == 0) {
