@@ -18,6 +18,7 @@
  *   objective           Eq. 9   P:163-167          sum_j w_j r_j^2 (C.2-2, C.2-3)
  *   Adam                step 8  P:169              orc_adam_step
  *   stopping rules      step 8  P:169-171          orc_stop_rule, orc_fit_stop
+ *   Clean masking       step 6  P:137-161, P:171   orc_clean_update, orc_fit_clean
  *   error estimate      step 9  P:173              errors_one
  *
  * Parity pins (tests/test_oracle_*.py): numpy legvander/legval, numpy lstsq,
@@ -661,6 +662,151 @@ int orc_fit_stop(const orc_model *m, int64_t B, const double *flux, const double
             if (err) errors_one(m, k, u, y, fd_h, err + i * NP);
         }
         free(u); free(mom); free(vel); free(g); free(hist);
+        work_free(k);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------- Clean-strategy masking (step 6, Eq. 8)
+ *
+ * One mask update of one spectrum, from the residuals at the current iterate.  Readings (R-7..R-12):
+ *   R-7  eps_j = sqrt(w_j) r_j, r = y - c S (Eq. 7 in the weighted form of Delta-1; the paper's case is w = 1), and the
+ *        flux-gradient allowance G_j = sqrt(w_j) max(|M_j - M_(j-1)|, |M_j - M_(j+1)|), M = c S (the corrected model of
+ *        Eq. 7), with only the neighbour that exists at a segment end; the unmasked pixels U are those with w_j > 0;
+ *   R-8  sigma_eps = population standard deviation (about the mean) of eps over U; sigma'_eps the same over U without the
+ *        pixels clipped by B and C;
+ *   R-9  masks accumulate: a pixel clipped by an update stays clipped (A <- A B C D);
+ *   R-10 B: excess_j = |eps_j| - f_shift G_j > k sigma, k = 3; if more than 3 % of U is clipped, k = 4, then 5, then 7
+ *        (the first k that clips at most 3 %, else 7);
+ *   R-11 C: the neighbours j' = j +- 1 (same segment, in U, not in B) of every j in B with excess_j' > 2 sigma;
+ *   R-12 D: starting from O = B + C, synchronously: every neighbour j' (same segment, in U, not in O) of a j in O with
+ *        eps_j eps_j' > 0, |eps_j'| <= |eps_j| and excess_j' > sigma' joins O; repeated until nothing joins, at most 20 times.
+ * w is updated in place (clipped pixels get 0); returns the number of pixels clipped by this update, *k_used the k of B. */
+static double pop_std(const double *eps, const uint8_t *use, int P, int *n_out)
+{
+    double s = 0.0, s2 = 0.0;
+    int n = 0;
+    for (int j = 0; j < P; ++j)
+        if (use[j]) { s += eps[j]; ++n; }
+    if (n_out) *n_out = n;
+    if (n == 0) return 0.0;
+    double mean = s / n;
+    for (int j = 0; j < P; ++j)
+        if (use[j]) s2 += (eps[j] - mean) * (eps[j] - mean);
+    return sqrt(s2 / n);
+}
+
+int orc_clean_update(int P, int n_seg, const int32_t *seg_offset, const double *r, const double *M, double *w,
+                     double fshift, int *k_used)
+{
+    double *eps = calloc(P, 8), *exc = calloc(P, 8);
+    uint8_t *U = calloc(P, 1), *O = calloc(P, 1), *use = calloc(P, 1), *add = calloc(P, 1);
+    int *seg = calloc(P, sizeof(int));
+    for (int s = 0; s < n_seg; ++s)
+        for (int j = seg_offset[s]; j < seg_offset[s + 1]; ++j) seg[j] = s;
+    for (int j = 0; j < P; ++j) {
+        U[j] = w[j] > 0.0;
+        double sw = U[j] ? sqrt(w[j]) : 0.0;
+        int s = seg[j], o = seg_offset[s], e = seg_offset[s + 1];
+        double g = 0.0;
+        if (j - 1 >= o) g = fmax(g, fabs(M[j] - M[j - 1]));
+        if (j + 1 < e) g = fmax(g, fabs(M[j] - M[j + 1]));
+        eps[j] = sw * r[j];
+        exc[j] = fabs(eps[j]) - fshift * sw * g;                    /* R-7 */
+    }
+    int nU = 0;
+    double sigma = pop_std(eps, U, P, &nU);                          /* R-8 */
+    static const double ks[4] = {3.0, 4.0, 5.0, 7.0};
+    int kk = 3;
+    for (int t = 0; t < 4; ++t) {                                    /* R-10 */
+        int n = 0;
+        for (int j = 0; j < P; ++j) n += U[j] && exc[j] > ks[t] * sigma;
+        kk = (int)ks[t];
+        if ((double)n <= 0.03 * (double)nU) break;
+    }
+    if (k_used) *k_used = kk;
+    for (int j = 0; j < P; ++j) O[j] = U[j] && exc[j] > (double)kk * sigma;
+    memcpy(add, O, P);
+    for (int j = 0; j < P; ++j) {                                    /* R-11 */
+        if (!O[j]) continue;
+        int s = seg[j], o = seg_offset[s], e = seg_offset[s + 1];
+        for (int d = -1; d <= 1; d += 2) {
+            int q = j + d;
+            if (q < o || q >= e || !U[q] || O[q]) continue;
+            if (exc[q] > 2.0 * sigma) add[q] = 1;
+        }
+    }
+    memcpy(O, add, P);
+    for (int j = 0; j < P; ++j) use[j] = U[j] && !O[j];
+    double sigma2 = pop_std(eps, use, P, NULL);
+    for (int it = 0; it < 20; ++it) {                                /* R-12 */
+        int changed = 0;
+        memcpy(add, O, P);
+        for (int j = 0; j < P; ++j) {
+            if (!O[j]) continue;
+            int s = seg[j], o = seg_offset[s], e = seg_offset[s + 1];
+            for (int d = -1; d <= 1; d += 2) {
+                int q = j + d;
+                if (q < o || q >= e || !U[q] || O[q]) continue;
+                if (eps[j] * eps[q] > 0.0 && fabs(eps[q]) <= fabs(eps[j]) && exc[q] > sigma2) { add[q] = 1; changed = 1; }
+            }
+        }
+        memcpy(O, add, P);
+        if (!changed) break;
+    }
+    int n = 0;
+    for (int j = 0; j < P; ++j)
+        if (O[j]) { w[j] = 0.0; ++n; }                               /* R-9 */
+    free(eps); free(exc); free(U); free(O); free(use); free(add); free(seg);
+    return n;
+}
+
+/* lasp_fit_batch with the Clean strategy: as orc_fit (fixed n_iter steps), and after update t, t = every, 2 every, ...
+ * (at most max_updates times; the paper: every 30 steps, up to 11) the mask is updated from the residuals at
+ * the new iterate, with f_shift = 0.5 for the first update and 0.2 afterwards.  mask_out[i*P+j] = 1 where the
+ * pixel still takes part at the end. */
+int orc_fit_clean(const orc_model *m, int64_t B, const double *flux, const double *ivar,
+                  const uint8_t *mask, const double *init, int n_iter, double lr, double b1, double b2,
+                  double eps_adam, int every, int max_updates, double fd_h, double *params, double *cont,
+                  double *chi2, double *err, int32_t *status, uint8_t *mask_out, int32_t *n_clipped)
+{
+    int NP = m->n_labels + 2, P = m->n_pix, nc = m->n_seg * (m->cont_degree + 1);
+#pragma omp parallel
+    {
+        work_t *k = work_new(m);
+        double *u = calloc(NP, 8), *mom = calloc(NP, 8), *vel = calloc(NP, 8), *g = calloc(NP, 8);
+        double *Mod = calloc(P, 8);
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t i = 0; i < B; ++i) {
+            const double *y = flux + i * P;
+            make_weights(m, ivar + i * P, mask ? mask + i * P : NULL, k->w);
+            norm_u(m, init + i * NP, u);
+            memset(mom, 0, 8 * NP);
+            memset(vel, 0, 8 * NP);
+            int updates = 0, clipped = 0;
+            for (int t = 1; t <= n_iter; ++t) {
+                chi2_at(m, k, u, y, 1, NULL);
+                grad_from_work(k, g);
+                orc_adam_step(NP, u, mom, vel, g, t, lr, b1, b2, eps_adam);
+                if (every > 0 && t % every == 0 && updates < max_updates) {
+                    chi2_at(m, k, u, y, 0, NULL);                    /* residuals at the new iterate */
+                    for (int j = 0; j < P; ++j) Mod[j] = k->c[j] * k->S[j];
+                    clipped += orc_clean_update(P, m->n_seg, m->seg_offset, k->r, Mod, k->w, updates == 0 ? 0.5 : 0.2, NULL);
+                    ++updates;
+                }
+            }
+            int st = 0;
+            double c2 = chi2_at(m, k, u, y, 0, &st);
+            chi2[i] = c2;
+            denorm(m, u, params + i * NP);
+            if (cont) memcpy(cont + i * nc, k->b, 8 * (size_t)nc);
+            st = final_status(k, u, c2, st);
+            if (status) status[i] = st;
+            if (mask_out) for (int j = 0; j < P; ++j) mask_out[i * P + j] = k->w[j] != 0.0;
+            if (n_clipped) n_clipped[i] = clipped;
+            if (err) errors_one(m, k, u, y, fd_h, err + i * NP);
+        }
+        free(u); free(mom); free(vel); free(g); free(Mod);
         work_free(k);
     }
     return 0;

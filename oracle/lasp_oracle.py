@@ -215,6 +215,23 @@ class Oracle:
                            _p(err, _f64p) if want_err else None, _p(status, _i32p), _p(n_steps, _i32p))
         return dict(params=params, cont=cont, chi2=chi2, err=err, status=status, n_steps=n_steps)
 
+    def fit_clean(self, flux, ivar, mask, init, n_iter, lr=1e-2, beta1=0.9, beta2=0.999, eps=1e-8, every=30, max_updates=11,
+                  fd_h=1e-5, want_err=True):
+        """The fixed-step fit with the Clean strategy (orc_fit_clean)."""
+        flux, ivar, mask = self._obs(flux, ivar, mask)
+        B = flux.shape[0]
+        init = self._f64(init).reshape(B, self.NP)
+        params = np.empty((B, self.NP)); cont = np.empty((B, self.nc)); chi2 = np.empty(B)
+        err = np.empty((B, self.NP)) if want_err else None
+        status = np.zeros(B, dtype=np.int32); n_clipped = np.zeros(B, dtype=np.int32)
+        mask_out = np.zeros((B, self.P), dtype=np.uint8)
+        lib().orc_fit_clean(C.byref(self.m), C.c_int64(B), _p(flux, _f64p), _p(ivar, _f64p),
+                            _p(mask, _u8p) if mask is not None else None, _p(init, _f64p), C.c_int(n_iter),
+                            C.c_double(lr), C.c_double(beta1), C.c_double(beta2), C.c_double(eps), C.c_int(every),
+                            C.c_int(max_updates), C.c_double(fd_h), _p(params, _f64p), _p(cont, _f64p), _p(chi2, _f64p),
+                            _p(err, _f64p) if want_err else None, _p(status, _i32p), _p(mask_out, _u8p), _p(n_clipped, _i32p))
+        return dict(params=params, cont=cont, chi2=chi2, err=err, status=status, mask=mask_out, n_clipped=n_clipped)
+
 def stop_rule(L, window=50, tol=1e-5):
     """First step t (1-based) at which criterion (2) or (3) of P:169-171 fires on the loss sequence L, and the rule
     (1 = neither within the sequence, then t = 0)."""
@@ -224,6 +241,19 @@ def stop_rule(L, window=50, tol=1e-5):
     f.restype = C.c_int
     t = f(_p(L, _f64p), C.c_int(L.size), C.c_int(window), C.c_double(tol), C.byref(rule))
     return int(t), int(rule.value)
+
+
+def clean_update(r, M, w, seg_offset, fshift):
+    """One Clean-strategy mask update (orc_clean_update): returns (new weights, number clipped, k used)."""
+    r = np.ascontiguousarray(r, dtype=np.float64); M = np.ascontiguousarray(M, dtype=np.float64)
+    w = np.array(w, dtype=np.float64)
+    seg = np.ascontiguousarray(seg_offset, dtype=np.int32)
+    k = C.c_int(0)
+    f = lib().orc_clean_update
+    f.restype = C.c_int
+    n = f(C.c_int(r.size), C.c_int(seg.size - 1), _p(seg, _i32p), _p(r, _f64p), _p(M, _f64p), _p(w, _f64p),
+          C.c_double(fshift), C.byref(k))
+    return w, int(n), int(k.value)
 
 
 def forward(desc, params, cont):

@@ -564,3 +564,146 @@ def test_fit_with_stopping_rules_is_the_fixed_step_fit_cut_at_the_stop(oracle_mo
         assert t == r["n_steps"][i] + 1 and bool(r["status"][i] & (16 if rule == 2 else 32))
         assert np.array_equal(r["params"][i], o.fit(*[a[i:i + 1] for a in args], int(r["n_steps"][i]), lr=0.1,
                                                     want_err=False)["params"][0])
+
+
+# ------------------------------------------------------------------ Clean-strategy masking (P:137-161; readings R-7..R-12)
+
+def _baseline(n):
+    """+1 on even pixels, -1 on odd ones: mean 0, mean square 1."""
+    return np.where(np.arange(n) % 2 == 0, 1.0, -1.0)
+
+
+def _sigma(eps, use):
+    """Population standard deviation about the mean, written out (R-8)."""
+    e = eps[use]
+    mean = e.sum() / e.size
+    return math.sqrt(((e - mean) ** 2).sum() / e.size)
+
+
+def test_clean_primary_mask_and_threshold_escalation(oracle_mod):
+    """Pass B: |eps| - f G > k sigma with k = 3, relaxed to 4, 5, 7 while more than 3 % would be clipped."""
+    n = 400
+    one, flat, seg = np.ones(n), np.zeros(n), [0, n]
+    r = _baseline(n); r[100] = 10.0
+    # sigma^2 = 499/400 - (9/400)^2: 3 sigma = 3.35 -> only the spike goes, its neighbours (-1: other sign, below every threshold) stay
+    assert abs(_sigma(r, one > 0) - math.sqrt(499 / 400 - (9 / 400) ** 2)) < 1e-12
+    w, nc, k = oracle_mod.clean_update(r, flat, one, seg, 0.5)
+    assert (nc, k) == (1, 3) and np.array_equal(np.flatnonzero(w == 0), [100])
+    # 16 spikes of 4.2 (4 % of the pixels): all above 3 sigma = 3.85, none above 4 sigma = 5.14 -> k = 4 clips nothing
+    r = _baseline(n); r[20:340:20] = 4.2
+    s = _sigma(r, one > 0)
+    assert 3 * s < 4.2 < 4 * s
+    w, nc, k = oracle_mod.clean_update(r, flat, one, seg, 0.5)
+    assert (nc, k) == (0, 4) and np.all(w == 1)
+    # 12 spikes of 5 and 4 of 9: k = 3 would clip all 16 (4 %), k = 4 only the four of 9 (1 %)
+    r = _baseline(n); r[20:340:20] = 5.0; r[[40, 120, 200, 280]] = 9.0
+    s = _sigma(r, one > 0)
+    assert 3 * s < 5.0 < 4 * s < 9.0
+    w, nc, k = oracle_mod.clean_update(r, flat, one, seg, 0.5)
+    assert (nc, k) == (4, 4) and np.array_equal(np.flatnonzero(w == 0), [40, 120, 200, 280])
+    # masked pixels (w = 0) are neither counted nor clipped, whatever their residual; weights whiten the residual (R-7)
+    r = _baseline(n); r[100] = 10.0; r[250] = 1e6
+    w0 = one.copy(); w0[250] = 0.0
+    w, nc, k = oracle_mod.clean_update(r, flat, w0, seg, 0.5)
+    assert nc == 1 and np.array_equal(np.flatnonzero(w == 0), [100, 250])
+    r = _baseline(n); r[100] = 2.5; w4 = one.copy(); w4[100] = 16.0          # eps_100 = 4 * 2.5 = 10
+    w, nc, k = oracle_mod.clean_update(r, flat, w4, seg, 0.5)
+    assert nc == 1 and w[100] == 0
+
+
+def test_clean_flux_gradient_allowance(oracle_mod):
+    """G_j = max(|M_j - M_(j-1)|, |M_j - M_(j+1)|) excuses a residual that a small wavelength shift explains: at a step of
+    8 in the model a residual of 6 passes with f_shift = 0.5 (6 - 4 = 2 < 3 sigma) and is clipped with 0.2 (6 - 1.6 = 4.4)."""
+    n = 400
+    M = np.where(np.arange(n) >= 200, 8.0, 0.0)
+    r = _baseline(n); r[200] = 6.0
+    s = _sigma(r, np.ones(n) > 0)
+    assert 6 - 0.5 * 8 < 3 * s < 6 - 0.2 * 8
+    w, nc, _ = oracle_mod.clean_update(r, M, np.ones(n), [0, n], 0.5)
+    assert nc == 0
+    w, nc, _ = oracle_mod.clean_update(r, M, np.ones(n), [0, n], 0.2)
+    assert nc == 1 and w[200] == 0
+    # only the neighbour that exists counts at a segment end: the step between pixels 199 | 200 is invisible when they
+    # belong to different segments
+    w, nc, _ = oracle_mod.clean_update(r, M, np.ones(n), [0, 200, n], 0.5)
+    assert nc == 1 and w[200] == 0
+
+
+def test_clean_adjacent_and_neighbourhood_masks(oracle_mod):
+    """Pass C (2 sigma next to a primary outlier) and pass D (same sign, not larger, above sigma', repeated
+    synchronously at most 20 times)."""
+    n = 1000
+    one, flat = np.ones(n), np.zeros(n)
+    # C: 2.9 lies between 2 sigma and 3 sigma; next to the spike it is clipped, on its own (pixel 300) it is not;
+    # across a segment boundary it is not a neighbour
+    r = _baseline(n); r[100] = 10.0; r[101] = 2.9; r[300] = 2.9
+    s = _sigma(r, one > 0)
+    assert 2 * s < 2.9 < 3 * s
+    w, nc, _ = oracle_mod.clean_update(r, flat, one, [0, n], 0.5)
+    assert np.array_equal(np.flatnonzero(w == 0), [100, 101])
+    w, nc, _ = oracle_mod.clean_update(r, flat, one, [0, 101, n], 0.5)
+    assert np.array_equal(np.flatnonzero(w == 0), [100])
+    # D: a ramp 1.98, 1.96, ... 1.40 behind a spike of 12: below 2 sigma (not C), above sigma', same sign, never larger than
+    # the pixel before it -> one more pixel joins per iteration, and the 20-iteration cap leaves 521..530 in
+    r = _baseline(n); r[500] = 12.0; r[501:531] = 2.0 - 0.02 * np.arange(1, 31)
+    s = _sigma(r, one > 0)
+    use = one > 0; use[500] = False
+    s2 = _sigma(r, use)
+    assert r[501] < 2 * s and r[530] > 1.05 * s2 and 1.0 < s2      # the +1 baseline pixels stay below sigma'
+    w, nc, _ = oracle_mod.clean_update(r, flat, one, [0, n], 0.5)
+    assert np.array_equal(np.flatnonzero(w == 0), np.arange(500, 521)) and nc == 21
+    # the ramp is eaten only while it does not rise and keeps its sign
+    r = _baseline(n); r[300] = 12.0; r[301] = 1.8; r[302] = 1.9; r[700] = 12.0; r[701] = 1.8; r[702] = -1.7
+    w, nc, _ = oracle_mod.clean_update(r, flat, one, [0, n], 0.5)
+    assert np.array_equal(np.flatnonzero(w == 0), [300, 301, 700, 701])
+    # ... and on the other side of the spike too (descending towards lower pixels)
+    r = _baseline(n); r[400] = 12.0; r[399] = 1.8; r[398] = 1.7; r[397] = 1.6
+    w, nc, _ = oracle_mod.clean_update(r, flat, one, [0, n], 0.5)
+    assert np.array_equal(np.flatnonzero(w == 0), [397, 398, 399, 400])
+
+
+def test_fit_with_clean_strategy(oracle_mod):
+    """orc_fit_clean against the pinned pieces: without updates it is orc_fit; its first update is orc_clean_update applied
+    to the residuals of the pinned fit at that step with f_shift = 0.5; and on spectra hit by cosmic-ray-like spikes it
+    clips those pixels and lands closer to the truth than the fit without Clean."""
+    case = make(small_config(mask_frac=0.0, snr=(60.0, 60.0)), oracle_mod, B=4)
+    o = oracle_mod.Oracle(case["desc"])
+    flux = case["flux"].copy()
+    P = case["desc"]["n_pix"]
+    hit = np.array([150, 151, 152, 300, 420])
+    flux[:, hit] += 1.5                                   # ~90 sigma at SNR 60
+    args = (flux, case["ivar"], case["mask"], case["init"])
+    plain = o.fit(*args, 60, lr=0.03)
+    same = o.fit_clean(*args, 60, lr=0.03, every=0)
+    for k in ("params", "chi2", "cont", "err"):
+        assert np.array_equal(plain[k], same[k]), k
+    assert np.array_equal(same["mask"], (case["ivar"] * case["mask"] != 0) & _not_edge(case))
+    # first update after step 30
+    at30 = o.fit(*args, 30, lr=0.03, want_err=False)
+    M = o.eval_model(at30["params"], at30["cont"])
+    one = o.fit_clean(*args, 30, lr=0.03, every=30, max_updates=1, want_err=False)
+    for i in range(4):
+        w0 = (case["ivar"][i].astype(np.float64) * case["mask"][i]) * _not_edge(case)[i]
+        w1, nc, _ = oracle_mod.clean_update(flux[i].astype(np.float64) - M[i], M[i], w0, case["desc"]["seg_offset"], 0.5)
+        assert np.array_equal(one["mask"][i], w1 != 0) and one["n_clipped"][i] == nc
+        assert np.all(one["mask"][i][hit] == 0)
+    assert np.array_equal(one["params"], at30["params"])
+    # the paper's schedule (every 30 steps, up to 11 updates) over 400 steps
+    clean = o.fit_clean(*args, 400, lr=0.03)
+    dirty = o.fit(*args, 400, lr=0.03)
+    rng = (o.hi - o.lo)
+    e_clean = (np.abs(clean["params"] - case["truth"]) / rng).max()
+    e_dirty = (np.abs(dirty["params"] - case["truth"]) / rng).max()
+    assert np.all(clean["mask"][:, hit] == 0) and e_clean < 0.5 * e_dirty
+    assert np.all(clean["n_clipped"] >= hit.size) and np.all(clean["n_clipped"] < 0.05 * P)
+
+
+def _not_edge(case):
+    d = case["desc"]
+    keep = np.ones((case["B"], d["n_pix"]), dtype=bool)
+    for k in range(d["n_seg"]):
+        a, b = d["seg_offset"][k], d["seg_offset"][k + 1]
+        ne = d["seg_n_edge"][k]
+        keep[:, a:a + ne] = False
+        keep[:, b - ne:b] = False
+    return keep
