@@ -259,10 +259,11 @@ def time_fit(model, data, n_iter, steps, warmup, kw, torch, barrier):
     return out, ev[0].elapsed_time(ev[-1]), step_ms, model.launch_count() - l0
 
 
-def run_other_config(cfg_id, B, torch, local, peaks, n_sms, emulator_path=0, paper_stop=False):
+def run_other_config(cfg_id, B, torch, local, peaks, n_sms, emulator_path=0, paper_stop=False, clean=False):
     """One timed step (after one warm-up) of another BASELINE.json config at a stated, reduced batch.
     paper_stop: the paper's optimiser settings instead of the config's fixed steps: lr 0.1, at most 5000
-    iterations, stop when |L_t - L_(t-50)| < 1e-5 or after 50 consecutive increases (lasp_fit_opts.stop_window)."""
+    iterations, stop when |L_t - L_(t-50)| < 1e-5 or after 50 consecutive increases (lasp_fit_opts.stop_window).
+    clean: the Clean strategy on the paper's schedule (mask update every 30 steps, at most 11)."""
     from paper_2512_24840_b200 import binding, synth
     cfg = synth.CONFIGS[cfg_id]
     desc = synth.make_model_desc(cfg)
@@ -275,6 +276,8 @@ def run_other_config(cfg_id, B, torch, local, peaks, n_sms, emulator_path=0, pap
     if paper_stop:
         kw.update(lr=0.1, stop_window=50, stop_tol=1e-5)
         n_iter = 5000
+    if clean:
+        kw.update(clean_every=30, clean_max=11)
     out, ms_total, step_ms, _ = time_fit(model, data, n_iter, 1, 1, kw, torch, torch.cuda.synchronize)
     # evaluations actually executed per spectrum slot (= n_iter at fixed steps; the group's last stop step otherwise)
     steps_run = model.last_fit_stats()["group_steps"] * 4.0 / B
@@ -298,6 +301,14 @@ def run_other_config(cfg_id, B, torch, local, peaks, n_sms, emulator_path=0, pap
                     "stopped_by": {"tolerance": float(((st & 16) != 0).float().mean().item()),
                                    "rising_loss": float(((st & 32) != 0).float().mean().item()),
                                    "max_iterations": float(((st & 48) == 0).float().mean().item())}})
+    if clean:
+        ne = int(desc["seg_n_edge"][0])     # one segment (the library refuses Clean otherwise); edge pixels never take part
+        inner = slice(ne, model.P - ne)
+        w0 = ((data["ivar"][:, inner] != 0) & (data["mask"][:, inner] != 0)).sum(dim=1).float()
+        kept = out["mask_out"].sum(dim=1, dtype=torch.float32)
+        rec.update({"workload": f"config {cfg_id} shapes with the Clean strategy (mask update every 30 steps, at most 11)",
+                    "clean_every": 30, "clean_max": 11,
+                    "clipped_frac_of_unmasked": float(((w0 - kept) / w0.clamp_min(1.0)).mean().item())})
     model.close()
     del data, out
     torch.cuda.empty_cache()
@@ -426,7 +437,7 @@ def run_gpu(args):
     h2d = sum(v.numel() * v.element_size() for v in host.values())
     e2e_chunk = max(GS_CHUNK, B // 8)
     hout = model.fit_batch_host(host["flux"], host["ivar"], host["mask"], host["init"], n_iter, chunk=e2e_chunk, **kw)
-    d2h = sum(v.numel() * v.element_size() for v in hout.values())
+    d2h = sum(v.numel() * v.element_size() for v in hout.values() if v is not None)
     e2e_steps = max(1, min(args.steps, 3))
     barrier()
     t0 = time.perf_counter()
@@ -488,6 +499,10 @@ def run_gpu(args):
             oc["config1_paper_stop"] = run_other_config(1, 65536, torch, local, peaks, n_sms, paper_stop=True)
         except Exception as e:
             oc["config1_paper_stop"] = {"error": f"{type(e).__name__}: {e}"}
+        try:
+            oc["config1_clean"] = run_other_config(1, 65536, torch, local, peaks, n_sms, clean=True)
+        except Exception as e:
+            oc["config1_clean"] = {"error": f"{type(e).__name__}: {e}"}
         line["other_configs"] = oc
     if world == 1 and not args.no_cpu_baseline:
         cores = os.cpu_count() or 1

@@ -114,6 +114,14 @@ typedef struct {
                                      t: (1) n_iter updates applied (n_iter is then the paper's "maximum of 5000
                                      iterations"); (2) |L_t - L_(t-W)| < stop_tol; (3) W consecutive increases */
     float stop_tol;               /* threshold of criterion (2) (the paper: 1e-5) */
+    int32_t clean_every;          /* the Clean strategy (step 6, Eq. 8; R-7..R-12): 0 (default) = No Clean;
+                                     e > 0 = after update t, t = e, 2e, ... the residuals are re-evaluated at the new iterate
+                                     and the pixel mask is updated (primary 3-sigma clipping with threshold escalation and the
+                                     flux-gradient allowance f_shift = 0.5 first, 0.2 afterwards; adjacent pixels at 2 sigma;
+                                     neighbourhood growth); clipped pixels stay clipped.  The paper: every 30 steps.
+                                     Needs the resident variant, one segment whose fitted range is one sweep of the CTA, and
+                                     stop_window = 0, else LASP_ERR_UNSUPPORTED */
+    int32_t clean_max;            /* at most this many mask updates per spectrum (0 = default 11) */
 } lasp_fit_opts;
 
 /* Build a context on `cuda_device`: validates the description, derives the per-pixel velocity
@@ -131,22 +139,24 @@ int lasp_reserve(lasp_ctx *ctx, int64_t B);
  *   convention, nodes x_j = -1 + 2(j-o_s)/P_s) or NULL; chi2 [B];
  *   err [B*NP] = sqrt(diag(rho^T rho/(N_good-NP) (J^T J)^-1)) in physical units (P:173,
  *   C.2-22/23; NaN when J^T J is singular) or NULL to skip; status [B] or NULL;
- *   n_steps [B] = Adam updates applied to each spectrum (= n_iter unless a stopping rule fired) or NULL. */
+ *   n_steps [B] = Adam updates applied to each spectrum (= n_iter unless a stopping rule fired) or NULL;
+ *   mask_out [B*n_pix] u8 = 1 where the pixel took part in the final evaluation (weight ivar * mask != 0, not an edge
+ *   pixel, not clipped by the Clean strategy) or NULL. */
 int lasp_fit_batch(lasp_ctx *ctx, int64_t B, const float *flux, const float *ivar,
                    const uint8_t *mask, const float *init, const lasp_fit_opts *opts,
                    float *params, float *cont, float *chi2, float *err, int32_t *status,
-                   int32_t *n_steps, void *stream);
+                   int32_t *n_steps, uint8_t *mask_out, void *stream);
 
 /* The same fit from HOST buffers (pinned memory recommended), for batches that do not fit on the device or
  * arrive from the host (BASELINE.json config 3, "survey-scale stream"): the batch is cut into chunks of
  * `chunk` spectra (0 = 65,536); chunk i+1 is copied host-to-device and chunk i-1's results device-to-host on
  * two copy streams while chunk i is fitted, with ctx-owned double buffers.  All pointers are HOST pointers
- * with the layouts of lasp_fit_batch; mask, cont, err, status, n_steps may be NULL.  Blocking: returns when every
+ * with the layouts of lasp_fit_batch; mask, cont, err, status, n_steps, mask_out may be NULL.  Blocking: returns when every
  * result is in host memory.  Per-chunk results are identical to lasp_fit_batch on the same spectra. */
 int lasp_fit_batch_host(lasp_ctx *ctx, int64_t B, const float *flux, const float *ivar,
                         const uint8_t *mask, const float *init, const lasp_fit_opts *opts,
                         float *params, float *cont, float *chi2, float *err, int32_t *status,
-                        int32_t *n_steps, int64_t chunk);
+                        int32_t *n_steps, uint8_t *mask_out, int64_t chunk);
 
 /* Inspection: model_j = c_j S_j (Eq. 1, 5, 6) at given physical params [B*NP] and plain-Legendre cont
  * [B*n_seg*(D+1)]; model [B*n_pix], every pixel (edges included: replicate-edge clamp, C.2-16).  Runs the fit

@@ -40,7 +40,8 @@ class FitOpts(C.Structure):
     _fields_ = [("n_iter", C.c_int32), ("lr", C.c_float), ("beta1", C.c_float), ("beta2", C.c_float),
                 ("eps", C.c_float), ("variant", C.c_int32), ("emulator_path", C.c_int32),
                 ("refresh", C.c_int32), ("warm", C.c_int32), ("fd_fresh", C.c_int32),
-                ("stop_window", C.c_int32), ("stop_tol", C.c_float)]
+                ("stop_window", C.c_int32), ("stop_tol", C.c_float),
+                ("clean_every", C.c_int32), ("clean_max", C.c_int32)]
 
 
 class LaspError(RuntimeError):
@@ -63,9 +64,9 @@ def lib():
         L.lasp_destroy.argtypes = [C.c_void_p]
         L.lasp_reserve.argtypes = [C.c_void_p, C.c_int64]
         L.lasp_fit_batch.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 4 + [C.POINTER(FitOpts)] + \
-                                    [C.c_void_p] * 7
+                                    [C.c_void_p] * 8
         L.lasp_fit_batch_host.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 4 + [C.POINTER(FitOpts)] + \
-                                         [C.c_void_p] * 6 + [C.c_int64]
+                                         [C.c_void_p] * 7 + [C.c_int64]
         L.lasp_eval_model.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 2 + [C.POINTER(FitOpts)] + [C.c_void_p] * 2
         L.lasp_eval_grad.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 4 + [C.POINTER(FitOpts)] + [C.c_void_p] * 5
         L.lasp_kernel_variant.argtypes = [C.c_void_p]
@@ -175,9 +176,9 @@ class LaspModel:
 
     @staticmethod
     def _opts(n_iter=0, lr=1e-2, beta1=0.9, beta2=0.999, eps=1e-8, variant=0, emulator_path=0, refresh=0, warm=0,
-              fd_fresh=0, stop_window=0, stop_tol=1e-5):
+              fd_fresh=0, stop_window=0, stop_tol=1e-5, clean_every=0, clean_max=0):
         return FitOpts(int(n_iter), lr, beta1, beta2, eps, int(variant), int(emulator_path), int(refresh), int(warm),
-                       int(fd_fresh), int(stop_window), float(stop_tol))
+                       int(fd_fresh), int(stop_window), float(stop_tol), int(clean_every), int(clean_max))
 
     def launch_count(self) -> int:
         return int(lib().lasp_launch_count(self.ctx))
@@ -187,8 +188,9 @@ class LaspModel:
 
     def fit_batch(self, flux, ivar, mask, init, n_iter, lr=1e-2, beta1=0.9, beta2=0.999, eps=1e-8,
                   want_err=True, want_cont=True, out=None, emulator_path=0, variant=0, refresh=0, warm=0, fd_fresh=0,
-                  stop_window=0, stop_tol=1e-5):
-        """lasp_fit_batch on device tensors; returns dict of device tensors."""
+                  stop_window=0, stop_tol=1e-5, clean_every=0, clean_max=0):
+        """lasp_fit_batch on device tensors; returns dict of device tensors (`mask_out`: the pixels that took part in
+        the final evaluation; clean_every > 0 turns the Clean strategy on)."""
         t = self.torch
         flux = self._dev(flux, t.float32); ivar = self._dev(ivar, t.float32)
         mask = self._dev(mask, t.uint8); init = self._dev(init, t.float32)
@@ -199,19 +201,21 @@ class LaspModel:
                        chi2=t.empty(B, device=self.device, dtype=t.float32),
                        status=t.empty(B, device=self.device, dtype=t.int32),
                        n_steps=t.empty(B, device=self.device, dtype=t.int32),
+                       mask_out=t.empty((B, self.P), device=self.device, dtype=t.uint8),
                        cont=t.empty((B, self.nc), device=self.device, dtype=t.float32) if want_cont else None,
                        err=t.empty((B, self.NP), device=self.device, dtype=t.float32) if want_err else None)
         opts = self._opts(n_iter, lr, beta1, beta2, eps, variant, emulator_path, refresh, warm, fd_fresh, stop_window,
-                          stop_tol)
+                          stop_tol, clean_every, clean_max)
         rc = lib().lasp_fit_batch(self.ctx, B, _ptr(flux), _ptr(ivar), _ptr(mask), _ptr(init), C.byref(opts),
                                   _ptr(out["params"]), _ptr(out.get("cont")), _ptr(out["chi2"]),
-                                  _ptr(out.get("err")), _ptr(out["status"]), _ptr(out.get("n_steps")), self._stream())
+                                  _ptr(out.get("err")), _ptr(out["status"]), _ptr(out.get("n_steps")),
+                                  _ptr(out.get("mask_out")), self._stream())
         self._check(rc, "lasp_fit_batch")
         return out
 
     def fit_batch_host(self, flux, ivar, mask, init, n_iter, lr=1e-2, beta1=0.9, beta2=0.999, eps=1e-8,
                        want_err=True, want_cont=True, chunk=0, out=None, emulator_path=0, variant=0, refresh=0, warm=0,
-                       fd_fresh=0, stop_window=0, stop_tol=1e-5):
+                       fd_fresh=0, stop_window=0, stop_tol=1e-5, clean_every=0, clean_max=0, want_mask=False):
         """lasp_fit_batch_host on HOST tensors (torch CPU tensors, pinned for overlap); returns host tensors.
         The library cuts the batch into chunks and overlaps the copies with the fits."""
         t = self.torch
@@ -232,13 +236,15 @@ class LaspModel:
             pin = dict(pin_memory=True)
             out = dict(params=t.empty((B, self.NP), dtype=t.float32, **pin), chi2=t.empty(B, dtype=t.float32, **pin),
                        status=t.empty(B, dtype=t.int32, **pin), n_steps=t.empty(B, dtype=t.int32, **pin),
+                       mask_out=t.empty((B, self.P), dtype=t.uint8, **pin) if want_mask else None,
                        cont=t.empty((B, self.nc), dtype=t.float32, **pin) if want_cont else None,
                        err=t.empty((B, self.NP), dtype=t.float32, **pin) if want_err else None)
         opts = self._opts(n_iter, lr, beta1, beta2, eps, variant, emulator_path, refresh, warm, fd_fresh, stop_window,
-                          stop_tol)
+                          stop_tol, clean_every, clean_max)
         rc = lib().lasp_fit_batch_host(self.ctx, B, _ptr(flux), _ptr(ivar), _ptr(mask), _ptr(init), C.byref(opts),
                                        _ptr(out["params"]), _ptr(out.get("cont")), _ptr(out["chi2"]),
-                                       _ptr(out.get("err")), _ptr(out["status"]), _ptr(out.get("n_steps")), int(chunk))
+                                       _ptr(out.get("err")), _ptr(out["status"]), _ptr(out.get("n_steps")),
+                                       _ptr(out.get("mask_out")), int(chunk))
         self._check(rc, "lasp_fit_batch_host")
         return out
 

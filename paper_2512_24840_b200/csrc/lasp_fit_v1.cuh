@@ -79,6 +79,9 @@ struct V1Args {
     int stop_window;       // W <= V1_WMAX
     float stop_tol;
     int *nsteps;           // [B] Adam updates applied per spectrum (may be null)
+    // Clean strategy (lasp_fit_opts.clean_every / .clean_max): 0 = No Clean
+    int clean_every, clean_max;
+    unsigned char *mask_out;   // [B][P] 1 where the pixel still takes part at the end (may be null)
     unsigned long long *dbg;   // optional per-phase cycle counters (LASP_TIMING=1), else null
     // per-pixel broadening kernels (linear grids, C.2-14): 1/s_j and s_j^2 with V1_TPAD replicated entries on
     // both sides, and per-CTA scratch [3][GS][Ppad] for dS/dv, dS/dsigma*, 1/E0 (thread-private pixels)
@@ -173,6 +176,9 @@ struct V1Block {
     int nsteps[GS];       // Adam updates applied
     int rise[GS];         // consecutive increases of the loss so far
     float lprev[GS];      // loss at the previous step
+    // Clean strategy (thread 0)
+    int force;            // the next Adam evaluation re-factorises whatever the policy says
+    int nclean;           // mask updates done for the current group
 };
 __shared__ V1Block v1_blk;
 #define V1_TID ((int)threadIdx.x)
@@ -981,7 +987,7 @@ __device__ __noinline__ void v1_phase_forward(int s_, bool stencil)
                 // flux / weight / c_prev rows come from L2: issue the loads first, the stencil hides them
                 const size_t ro = rowo[g] + (j0 >> 1);   // split-octet layout: half h of octet o at h*Ppad/2 + 4 o
                 const float4 y0 = __ldg((const float4 *)(Yg + ro)), y1 = __ldg((const float4 *)(Yg + ro) + P8);
-                const float4 w0 = __ldg((const float4 *)(Wg + ro)), w1 = __ldg((const float4 *)(Wg + ro) + P8);
+                const float4 w0 = __ldcg((const float4 *)(Wg + ro)), w1 = __ldcg((const float4 *)(Wg + ro) + P8);
                 const float4 *cp4 = (const float4 *)(cpg + g * Ppad + (j0 >> 1));
                 const float4 c0 = __ldcg(cp4), c1 = __ldcg(cp4 + P8);
                 float S[1][OCT];
@@ -1038,7 +1044,7 @@ __device__ __noinline__ void v1_phase_moments(int s_)
             for (int i = 0; i < OCT; ++i) u[g][i] = 0.f;
             if (act) {
                 const size_t ro = (size_t)v1_blk.spec[g] * Ppad + (j0 >> 1);
-                const float4 w0 = __ldg((const float4 *)(Wg + ro)), w1 = __ldg((const float4 *)(Wg + ro) + P8);
+                const float4 w0 = __ldcg((const float4 *)(Wg + ro)), w1 = __ldcg((const float4 *)(Wg + ro) + P8);
                 float SS[OCT];
                 v1_oct_load<STREAM>(rowA, ag, g, j0, SS);
                 const float ww[OCT] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
@@ -1283,7 +1289,7 @@ __device__ __noinline__ void v1_phase_residual(int s_, float *xrow)
             for (int g = 0; g < GS; ++g) {
                 const size_t ro = rowo[g] + (j0 >> 1);
                 yq[g][0] = __ldg((const float4 *)(Yg + ro)); yq[g][1] = __ldg((const float4 *)(Yg + ro) + P8);
-                wq[g][0] = __ldg((const float4 *)(Wg + ro)); wq[g][1] = __ldg((const float4 *)(Wg + ro) + P8);
+                wq[g][0] = __ldcg((const float4 *)(Wg + ro)); wq[g][1] = __ldcg((const float4 *)(Wg + ro) + P8);
             }
         }
         v1_cheb_init<SYM>(sg, j0, pp, pc, x2);
@@ -1349,8 +1355,10 @@ __device__ __noinline__ void v1_phase_residual(int s_, float *xrow)
                 }
                 av[i] = -2.f * wr * cc[g][i];
                 if (MODE == 2) rho[i] = sqrtf(ww[i]) * r;
+                if (MODE == 4) { av[i] = sqrtf(ww[i]) * r; rho[i] = cc[g][i] * SS[i]; }   // eps and M = c S for the mask update
             }
-            if (!uniform) {
+            if (MODE == 4) v1_oct_store<STREAM>(v1_rowp(L.oT, sg.po), v1_blk.tg, g, j0, rho);
+            if (!uniform && MODE != 4) {
                 // per-pixel kernels: the two kernel-parameter gradients close here (dS/dv, dS/dsigma* were kept by the
                 // forward pass), and the adjoint handed to the stencil is a/E0 (each source pixel's own normalisation)
                 const float4 *d4 = (const float4 *)(dsg + g * L.SL + ((j0 - sg.po) >> 1));
@@ -1521,12 +1529,14 @@ __device__ __forceinline__ void v1_begin_eval(int momsel, bool adam)
     if (V1_LANE < GS) red[(SLOT_STAT(L) + 2) * GS + V1_LANE] = 3.0e38f;
     __syncwarp();
     if (V1_TID == 0 && adam) {
-        bool fresh = momsel == 1;
+        const bool force = v1_blk.force != 0;   // the weights changed (Clean mask update)
+        bool fresh = momsel == 1 || force;
+        v1_blk.force = 0;
         if (momsel == 2) {
             const float step = __int_as_float(v1_blk.stepmax);
             const float drift = v1_blk.drift + step;
             const int since = v1_blk.since + 1;
-            fresh = v1_blk.failmask != 0u || since >= 64 || drift * step > v1_blk.A.drift_tol;
+            fresh = force || v1_blk.failmask != 0u || since >= 64 || drift * step > v1_blk.A.drift_tol;
             v1_blk.drift = fresh ? 0.f : drift;
             v1_blk.since = fresh ? 0 : since;
             v1_blk.stepmax = 0;
@@ -1546,7 +1556,8 @@ __device__ __forceinline__ void v1_begin_eval(int momsel, bool adam)
 //               factor") and read by all after the second: fresh when a segment's system was flagged not positive
 //               definite, when 64 steps have passed, or when (sum of |du|_inf since the last fresh factor) x
 //               (|du|_inf of the last update) > drift_tol.  `adam` marks the evaluations of the Adam loop (statistics).
-//   MODE 0: chi2 + gradient partials (Q slots) ; MODE 1: chi2 only ; MODE 2: chi2 + rho -> xrow.
+//   MODE 0: chi2 + gradient partials (Q slots) ; MODE 1: chi2 only ; MODE 2: chi2 + rho -> xrow ;
+//   MODE 4: eps = sqrt(w) r -> row A and M = c S -> row T, for the Clean mask update (no statistics).
 // On return (after the closing barrier) the per-warp reduction slots hold chi2 / ngood / min c (not with `stats`
 // false on uniform segments: the Adam steps do not read them) and, for MODE 0, the q / dv / dsigma partials.
 // ------------------------------------------------------------------------------------------
@@ -1630,8 +1641,8 @@ __device__ __noinline__ void v1_evaluate(bool cold, int momsel, float *xrow, boo
             __syncthreads();
         }
         if (MODE == 0 && !stats && sg.uniform) v1_phase_residual<3, true, STREAM>(s, xrow);   // Adam step: no statistics
-        else if (sg.uniform) v1_phase_residual<(MODE == 2 ? 2 : 1), true, STREAM>(s, xrow);
-        else v1_phase_residual<(MODE == 2 ? 2 : 1), false, STREAM>(s, xrow);
+        else if (sg.uniform) v1_phase_residual<(MODE == 2 || MODE == 4 ? MODE : 1), true, STREAM>(s, xrow);
+        else v1_phase_residual<(MODE == 2 || MODE == 4 ? MODE : 1), false, STREAM>(s, xrow);
         tick(8);
         __syncthreads();
         tick(9);
@@ -2032,6 +2043,225 @@ __device__ __noinline__ void v1_step_hot(int momsel)
 }
 
 // ------------------------------------------------------------------------------------------
+// Clean-strategy mask update (step 6, Eq. 8; the schedule of P:171), readings R-7..R-12 of DESIGN.md as
+// oracle/lasp_oracle.c orc_clean_update states them.  One resident segment whose fitted range is one sweep of the
+// CTA: thread t owns octet t of the fitted range and keeps eps, the excess and its flags in registers; neighbours
+// across octets are read from row T, which holds eps_j for the pixels clipped so far by this update and 0 elsewhere.
+// On entry (after v1_evaluate<4>) row A holds eps = sqrt(w) r and row T the corrected model M = c S at the current
+// iterate.  The decisions (sigma, thresholds) are taken in double from the float residuals.  Clipped pixels get w = 0
+// in the staged weight plane, for good (R-9); the next Adam step re-factorises the Gram matrix.
+// ------------------------------------------------------------------------------------------
+template <int NV>
+__device__ __forceinline__ void v1_block_sum(double (&x)[NV][GS])
+{
+    const V1Lay &L = v1_blk.L;
+    // the Q slots of the reduction area are free between an evaluation and the next one's first barrier
+    double *red = (double *)(V1SM + L.oRED + (L.nmomr + L.n1r) * GS);
+    const int wst = L.VR * GS / 2;
+#pragma unroll
+    for (int v = 0; v < NV; ++v)
+#pragma unroll
+        for (int g = 0; g < GS; ++g) {
+            double s = x[v][g];
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(FULL, s, o);
+            if (V1_LANE == 0) red[V1_WARP * wst + v * GS + g] = s;
+        }
+    __syncthreads();
+#pragma unroll
+    for (int v = 0; v < NV; ++v)
+#pragma unroll
+        for (int g = 0; g < GS; ++g) {
+            double s = 0.0;
+            for (int w = 0; w < L.NW; ++w) s += red[w * wst + v * GS + g];
+            x[v][g] = s;
+        }
+    __syncthreads();
+}
+
+__device__ __forceinline__ float v1_row_elem(const float *rowsm, int g, int jp)
+{
+    const float4 *p = (const float4 *)(rowsm + g * v1_blk.L.RL);
+    return ((const float *)&p[SW4(jp >> 2)])[jp & 3];
+}
+
+// population standard deviation of eps over the pixels flagged in `use` (bit g*8+i), per spectrum (R-8)
+__device__ __forceinline__ void v1_clean_sigma(const float (&eps)[GS][OCT], unsigned use, double (&sigma)[GS], double (&n)[GS])
+{
+    double s[2][GS];
+#pragma unroll
+    for (int g = 0; g < GS; ++g) {
+        s[0][g] = 0.0; s[1][g] = 0.0;
+#pragma unroll
+        for (int i = 0; i < OCT; ++i)
+            if ((use >> (g * OCT + i)) & 1u) { s[0][g] += (double)eps[g][i]; s[1][g] += 1.0; }
+    }
+    v1_block_sum<2>(s);
+    double d[1][GS];
+#pragma unroll
+    for (int g = 0; g < GS; ++g) {
+        n[g] = s[1][g];
+        const double mean = n[g] > 0.0 ? s[0][g] / n[g] : 0.0;
+        d[0][g] = 0.0;
+#pragma unroll
+        for (int i = 0; i < OCT; ++i)
+            if ((use >> (g * OCT + i)) & 1u) { const double e = (double)eps[g][i] - mean; d[0][g] += e * e; }
+    }
+    v1_block_sum<1>(d);
+#pragma unroll
+    for (int g = 0; g < GS; ++g) sigma[g] = n[g] > 0.0 ? sqrt(d[0][g] / n[g]) : 0.0;
+}
+
+__device__ __noinline__ void v1_clean_update(float fshift)
+{
+    const SegDev &sg = v1_blk.M.seg[0];
+    const V1Lay &L = v1_blk.L;
+    const int Ppad = v1_blk.M.Ppad, P8 = Ppad >> 3;
+    const int j0 = sg.fit_lo + V1_TID * OCT;
+    const bool act = j0 < sg.fit_hi;
+    const int r0 = j0 - (sg.po + sg.halo);   // real index of this octet's first pixel
+    float *rowA = v1_rowp(L.oA, sg.po), *rowT = v1_rowp(L.oT, sg.po);
+    float *Wg = const_cast<float *>(v1_blk.A.W);
+    float eps[GS][OCT], exc[GS][OCT];
+    unsigned U = 0u, O = 0u;   // bit g * 8 + i
+#pragma unroll
+    for (int g = 0; g < GS; ++g) {
+#pragma unroll
+        for (int i = 0; i < OCT; ++i) { eps[g][i] = 0.f; exc[g][i] = 0.f; }
+        if (!act) continue;
+        float Mv[OCT + 2], ww[OCT];
+        {
+            float m8[OCT];
+            v1_oct_load<false>(rowA, nullptr, g, j0, eps[g]);
+            v1_oct_load<false>(rowT, nullptr, g, j0, m8);
+            Mv[0] = v1_row_elem(rowT, g, j0 - 1);
+            Mv[OCT + 1] = v1_row_elem(rowT, g, j0 + OCT);
+#pragma unroll
+            for (int i = 0; i < OCT; ++i) Mv[i + 1] = m8[i];
+            const float4 *w4 = (const float4 *)(Wg + (size_t)v1_blk.spec[g] * Ppad + (j0 >> 1));
+            const float4 w0 = __ldcg(w4), w1 = __ldcg(w4 + P8);
+            ww[0] = w0.x; ww[1] = w0.y; ww[2] = w0.z; ww[3] = w0.w; ww[4] = w1.x; ww[5] = w1.y; ww[6] = w1.z; ww[7] = w1.w;
+        }
+#pragma unroll
+        for (int i = 0; i < OCT; ++i) {
+            const int jr = r0 + i;
+            float gm = 0.f;   // R-7: only the neighbour that exists at a segment end
+            if (jr >= 1) gm = fabsf(Mv[i + 1] - Mv[i]);
+            if (jr + 1 < sg.P) gm = fmaxf(gm, fabsf(Mv[i + 1] - Mv[i + 2]));
+            if (ww[i] > 0.f) U |= 1u << (g * OCT + i);
+            exc[g][i] = fabsf(eps[g][i]) - fshift * sqrtf(ww[i]) * gm;
+        }
+    }
+    double sigma[GS], nU[GS];
+    v1_clean_sigma(eps, U, sigma, nU);      // (its barriers also end every thread's reads of M in row T)
+    // B (R-10): k = 3, escalated to 4, 5, 7 while more than 3 % of U would be clipped
+    double cnt[4][GS];
+    const double ks[4] = {3.0, 4.0, 5.0, 7.0};
+#pragma unroll
+    for (int t = 0; t < 4; ++t)
+#pragma unroll
+        for (int g = 0; g < GS; ++g) {
+            cnt[t][g] = 0.0;
+#pragma unroll
+            for (int i = 0; i < OCT; ++i)
+                if (((U >> (g * OCT + i)) & 1u) && (double)exc[g][i] > ks[t] * sigma[g]) cnt[t][g] += 1.0;
+        }
+    v1_block_sum<4>(cnt);
+#pragma unroll
+    for (int g = 0; g < GS; ++g) {
+        double kk = 7.0;
+        if (cnt[0][g] <= 0.03 * nU[g]) kk = 3.0;
+        else if (cnt[1][g] <= 0.03 * nU[g]) kk = 4.0;
+        else if (cnt[2][g] <= 0.03 * nU[g]) kk = 5.0;
+#pragma unroll
+        for (int i = 0; i < OCT; ++i)
+            if (((U >> (g * OCT + i)) & 1u) && (double)exc[g][i] > kk * sigma[g]) O |= 1u << (g * OCT + i);
+    }
+    // row T <- eps of the clipped pixels, 0 elsewhere (guards and the rest of the row included)
+    for (int i = V1_TID; i < GS * L.RL / 4; i += V1_NT) ((float4 *)(V1SM + L.oT))[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    __syncthreads();
+    auto publish = [&]() {
+        if (!act) return;
+#pragma unroll
+        for (int g = 0; g < GS; ++g) {
+            float f[OCT];
+#pragma unroll
+            for (int i = 0; i < OCT; ++i) f[i] = ((O >> (g * OCT + i)) & 1u) ? eps[g][i] : 0.f;
+            v1_oct_store<false>(rowT, nullptr, g, j0, f);
+        }
+    };
+    // flags of the octet's pixels and of the two pixels beside it
+    auto flags = [&](int g, float (&f)[OCT + 2]) {
+        f[0] = v1_row_elem(rowT, g, j0 - 1);
+        f[OCT + 1] = v1_row_elem(rowT, g, j0 + OCT);
+#pragma unroll
+        for (int i = 0; i < OCT; ++i) f[i + 1] = ((O >> (g * OCT + i)) & 1u) ? eps[g][i] : 0.f;
+    };
+    publish();
+    __syncthreads();
+    // C (R-11): neighbours of B with excess > 2 sigma
+    {
+        unsigned add = 0u;
+        if (act) {
+#pragma unroll
+            for (int g = 0; g < GS; ++g) {
+                float f[OCT + 2];
+                flags(g, f);
+#pragma unroll
+                for (int i = 0; i < OCT; ++i) {
+                    const unsigned bit = 1u << (g * OCT + i);
+                    if ((U & bit) && !(O & bit) && (f[i] != 0.f || f[i + 2] != 0.f) && (double)exc[g][i] > 2.0 * sigma[g]) add |= bit;
+                }
+            }
+        }
+        __syncthreads();   // every thread has read the B flags
+        O |= add;
+        publish();
+        __syncthreads();
+    }
+    double sigma2[GS], n2[GS];
+    v1_clean_sigma(eps, U & ~O, sigma2, n2);
+    // D (R-12): synchronous growth along same-sign, non-increasing |eps| with excess > sigma', at most 20 rounds
+    for (int it = 0; it < 20; ++it) {
+        unsigned add = 0u;
+        if (act) {
+#pragma unroll
+            for (int g = 0; g < GS; ++g) {
+                float f[OCT + 2];
+                flags(g, f);
+#pragma unroll
+                for (int i = 0; i < OCT; ++i) {
+                    const unsigned bit = 1u << (g * OCT + i);
+                    if (!(U & bit) || (O & bit) || !((double)exc[g][i] > sigma2[g])) continue;
+                    const float e = eps[g][i], l = f[i], r = f[i + 2];
+                    if ((l != 0.f && l * e > 0.f && fabsf(e) <= fabsf(l)) || (r != 0.f && r * e > 0.f && fabsf(e) <= fabsf(r))) add |= bit;
+                }
+            }
+        }
+        const int changed = __syncthreads_or(add != 0u);   // also: every thread has read this round's flags
+        O |= add;
+        if (add) publish();
+        __syncthreads();
+        if (!changed) break;
+    }
+    // R-9: the clipped pixels leave the fit for good
+    if (act && O) {
+#pragma unroll
+        for (int g = 0; g < GS; ++g) {
+            if (!((O >> (g * OCT)) & 0xffu)) continue;
+            float4 *w4 = (float4 *)(Wg + (size_t)v1_blk.spec[g] * Ppad + (j0 >> 1));
+            float4 w0 = __ldcg(w4), w1 = __ldcg(w4 + P8);
+            const unsigned o = O >> (g * OCT);
+            if (o & 1u) w0.x = 0.f;  if (o & 2u) w0.y = 0.f;  if (o & 4u) w0.z = 0.f;  if (o & 8u) w0.w = 0.f;
+            if (o & 16u) w1.x = 0.f; if (o & 32u) w1.y = 0.f; if (o & 64u) w1.z = 0.f; if (o & 128u) w1.w = 0.f;
+            w4[0] = w0; w4[P8] = w1;
+        }
+    }
+    if (V1_TID == 0) { v1_blk.force = 1; v1_blk.nclean += 1; }
+    __syncthreads();
+}
+
+// ------------------------------------------------------------------------------------------
 // The paper's stopping rules (step 8), per spectrum (Delta-2), warp g for spectrum g, called after the t-th
 // evaluation and before update t (readings R-2..R-5 of DESIGN.md, as oracle/lasp_oracle.c orc_fit_stop):
 //   loss L_t = sqrt(chi2_t / n_pix) (Eq. 9 restricted to one spectrum);
@@ -2065,7 +2295,9 @@ __device__ __noinline__ bool v1_stop_test(int g, int t)
 // ------------------------------------------------------------------------------------------
 // lasp_fit_batch: a1-a9 for groups of GS spectra, persistent CTAs
 // ------------------------------------------------------------------------------------------
-template <int MAXT, int MINB, bool STREAM>
+// CLEAN: the instantiation with the Clean-strategy mask updates in the loop (resident variant only); the default one
+// carries none of that code (the step path is instruction-cache bound, profiles/r02_ncu.md)
+template <int MAXT, int MINB, bool STREAM, bool CLEAN = false>
 __global__ void __launch_bounds__(MAXT, MINB)
 lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V1Lay L, const V1Args a)
 {
@@ -2094,6 +2326,7 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
         if (threadIdx.x < GS) {
             v1_blk.stop_rule[threadIdx.x] = 0; v1_blk.nsteps[threadIdx.x] = a.n_iter;
             v1_blk.rise[threadIdx.x] = 0; v1_blk.lprev[threadIdx.x] = 0.f;
+            v1_blk.force = 0; v1_blk.nclean = 0;
             SMV(L.oSC, SC_PB1, threadIdx.x) = 1.f; SMV(L.oSC, SC_PB2, threadIdx.x) = 1.f;
         }
         // v1_blk.t was zeroed by v1_set_group; every evaluation below starts with a barrier, after which thread 0 advances
@@ -2156,6 +2389,15 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
 #ifdef LASP_PHASE_TIMING
             if (a.dbg && V1_TID == 0) atomicAdd(a.dbg + 13, (unsigned long long)(clock64() - tu0));
 #endif
+            if constexpr (CLEAN && !STREAM) {
+                if (a.clean_every > 0) {   // Clean: mask update after update t, t = every, 2 every, ...
+                    __syncthreads();
+                    if (v1_blk.t % a.clean_every == 0 && v1_blk.nclean < a.clean_max) {
+                        v1_evaluate<4, false>(false, 1, nullptr, L.fastw != 0);   // residuals at the new iterate, re-solved
+                        v1_clean_update(v1_blk.nclean == 0 ? 0.5f : 0.2f);       // f_shift
+                    }
+                }
+            }
             if (stopmode) {   // the group ends when every spectrum of it has stopped
                 __syncthreads();
                 bool all = true;
@@ -2201,6 +2443,21 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
             }
         }
         if (a.err) v1_errors<STREAM>(chi2, ngood, valid);
+        if (a.mask_out) {   // the final mask: the staged weights are zero at the edges, at ivar * mask = 0 and where Clean clipped
+            for (int g2 = 0; g2 < GS; ++g2) {
+                if ((long long)grp * GS + g2 >= a.B) break;
+                const float *wrow = a.W + (size_t)v1_blk.spec[g2] * M.Ppad;
+                unsigned char *mrow = a.mask_out + (size_t)v1_blk.spec[g2] * M.P;
+                for (int s = 0; s < M.n_seg; ++s) {
+                    const SegDev &sg = M.seg[s];
+                    for (int r = V1_TID; r < sg.P; r += V1_NT) {
+                        const int jp = sg.po + sg.halo + r;
+                        const float w = __ldcg(wrow + ((jp & 4) ? (M.Ppad >> 1) : 0) + (jp >> 3) * 4 + (jp & 3));
+                        mrow[sg.o + r] = w != 0.f ? 1 : 0;
+                    }
+                }
+            }
+        }
         grp = grp_next;
     }
 }

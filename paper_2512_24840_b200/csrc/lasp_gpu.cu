@@ -20,6 +20,8 @@ static const double kC_KMS = 299792.458;
 enum { KV_RES192 = 0, KV_RES384 = 1, KV_STREAM = 2, KV_N = 3 };
 static const void *kFit[KV_N] = {(const void *)lasp_v1_fit_kernel<192, 2, false>, (const void *)lasp_v1_fit_kernel<384, 1, false>,
                                  (const void *)lasp_v1_fit_kernel<192, 2, true>};
+static const void *kFitClean[KV_N] = {(const void *)lasp_v1_fit_kernel<192, 2, false, true>,
+                                        (const void *)lasp_v1_fit_kernel<384, 1, false, true>, nullptr};
 static const void *kGrad[KV_N] = {(const void *)lasp_v1_grad_kernel<192, 2, false>, (const void *)lasp_v1_grad_kernel<384, 1, false>,
                                   (const void *)lasp_v1_grad_kernel<192, 2, true>};
 static const void *kModel[KV_N] = {(const void *)lasp_v1_model_kernel<192, 2, false>, (const void *)lasp_v1_model_kernel<384, 1, false>,
@@ -64,6 +66,7 @@ struct lasp_ctx {
         float *flux[2] = {}, *ivar[2] = {}, *init[2] = {}, *params[2] = {}, *cont[2] = {}, *chi2[2] = {}, *err[2] = {};
         uint8_t *mask[2] = {};
         int32_t *status[2] = {}, *nsteps[2] = {};
+        uint8_t *maskout[2] = {};
         cudaStream_t s_in = nullptr, s_out = nullptr, s_fit = nullptr;
         cudaEvent_t in_done[2] = {}, fit_done[2] = {}, out_done[2] = {};
     } hp;
@@ -261,8 +264,10 @@ extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx *
         const int ne = d->seg_n_edge[sg];
         const int jl = ne, jh = Ps - 1 - ne;
         if (jh >= jl) {
-            S.fit_lo = S.po + S.halo + ne / CH * CH;
-            S.fit_hi = S.po + S.halo + roundup(Ps - ne, CH);
+            // the pixels beside the first and the last one that can carry weight are included: the Clean mask update
+            // takes the model's flux gradient across them (R-7)
+            S.fit_lo = S.po + S.halo + (ne > 0 ? (ne - 1) / CH * CH : 0);
+            S.fit_hi = S.po + S.halo + roundup(ne > 0 ? Ps - ne + 1 : Ps, CH);
             if (((S.fit_hi - S.fit_lo) / CH) & 1) S.fit_hi += CH;   // an even number of octets: they pair up about the centre
         } else {
             S.fit_lo = S.fit_hi = S.po + S.halo;
@@ -437,9 +442,9 @@ static void setup_variant(lasp_ctx *c, const cudaDeviceProp &prop, int emax, boo
         if (bytes + 2048 <= prop.sharedMemPerBlockOptin) break;   // + the kernels' static block state
     }
     if (L.lfseg < 0) return;
-    const void *fs[3] = {kFit[v.kv], kGrad[v.kv], kModel[v.kv]};
+    const void *fs[4] = {kFit[v.kv], kGrad[v.kv], kModel[v.kv], kFitClean[v.kv]};
     for (const void *f : fs)
-        if (cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess) { cudaGetLastError(); return; }
+        if (f && cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess) { cudaGetLastError(); return; }
     int per_sm = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kFit[v.kv], nt, bytes) != cudaSuccess || per_sm < 1) {
         cudaGetLastError();
@@ -452,7 +457,7 @@ static void setup_variant(lasp_ctx *c, const cudaDeviceProp &prop, int emax, boo
 // ------------------------------------------------------------------------------------------
 // options, workspace, launches
 // ------------------------------------------------------------------------------------------
-static const lasp_fit_opts kDefaultOpts = {0, 1e-2f, 0.9f, 0.999f, 1e-8f, 0, 0, 0, 0, 0, 0, 0.f};
+static const lasp_fit_opts kDefaultOpts = {0, 1e-2f, 0.9f, 0.999f, 1e-8f, 0, 0, 0, 0, 0, 0, 0.f, 0, 0};
 
 // variant / emulator path of one call (opts may be null: defaults)
 static int resolve(lasp_ctx *c, const lasp_fit_opts *o, const char *who, const Variant **v, bool *mma)
@@ -465,6 +470,8 @@ static int resolve(lasp_ctx *c, const lasp_fit_opts *o, const char *who, const V
         return fail(c, LASP_ERR_INVALID_ARG, std::string(who) + ": refresh, warm must be >= 0 and fd_fresh 0 or 1");
     if (o->stop_window < 0 || o->stop_window > V1_WMAX || (o->stop_window > 0 && !(o->stop_tol >= 0.f)))
         return fail(c, LASP_ERR_INVALID_ARG, std::string(who) + ": stop_window must be in [0, 128] and stop_tol >= 0");
+    if (o->clean_every < 0 || o->clean_max < 0)
+        return fail(c, LASP_ERR_INVALID_ARG, std::string(who) + ": clean_every and clean_max must be >= 0");
     const Variant *vv = nullptr;
     if (o->variant == 1) vv = c->res.ok ? &c->res : nullptr;
     else if (o->variant == 2) vv = c->str.ok ? &c->str : nullptr;
@@ -597,7 +604,7 @@ static int launch(lasp_ctx *c, const void *const *table, const Variant &v, const
 extern "C" int lasp_fit_batch(lasp_ctx *c, int64_t B, const float *flux, const float *ivar,
                               const uint8_t *mask, const float *init, const lasp_fit_opts *opts,
                               float *params, float *cont, float *chi2, float *err, int32_t *status,
-                              int32_t *n_steps, void *stream)
+                              int32_t *n_steps, uint8_t *mask_out, void *stream)
 {
     if (!c) return fail(nullptr, LASP_ERR_INVALID_ARG, "null ctx");
     if (B < 1 || !flux || !ivar || !init || !opts || !params || !chi2)
@@ -610,6 +617,15 @@ extern "C" int lasp_fit_batch(lasp_ctx *c, int64_t B, const float *flux, const f
     bool mma = false;
     int rc = resolve(c, opts, "lasp_fit_batch", &v, &mma);
     if (rc) return rc;
+    if (opts->clean_every > 0) {
+        // the mask update keeps one octet of the fitted range per thread and reads its neighbours from the resident rows
+        const SegDev &S0 = c->M.seg[0];
+        if (v != &c->res || c->M.n_seg != 1 || (S0.fit_hi - S0.fit_lo) / OCT > v->nt)
+            return fail(c, LASP_ERR_UNSUPPORTED, "lasp_fit_batch: the Clean strategy needs the resident variant and one segment "
+                                                 "whose fitted range is one sweep of the CTA");
+        if (opts->stop_window > 0)
+            return fail(c, LASP_ERR_UNSUPPORTED, "lasp_fit_batch: the Clean strategy runs a fixed number of steps (stop_window = 0)");
+    }
     DeviceGuard dg(c->device);
     rc = workspace(c, B, *v, true, true, err != nullptr);
     if (rc) return rc;
@@ -629,6 +645,8 @@ extern "C" int lasp_fit_batch(lasp_ctx *c, int64_t B, const float *flux, const f
     a.fdfresh = opts->fd_fresh;
     a.drift_tol = 6.4e-3f;   // = 64 steps x (1e-2)^2: the fixed schedule the parity suite was tuned at
     a.stop_window = opts->stop_window; a.stop_tol = opts->stop_tol; a.nsteps = n_steps;
+    a.clean_every = opts->clean_every; a.clean_max = opts->clean_max > 0 ? opts->clean_max : 11;
+    a.mask_out = mask_out;
     CUDA_TRY(c, cudaMemsetAsync(c->dqueue, 0, sizeof(unsigned int), st));
     CUDA_TRY(c, cudaMemsetAsync(c->dstats, 0, 2 * sizeof(unsigned long long), st));
     a.queue = c->dqueue;
@@ -638,7 +656,7 @@ extern "C" int lasp_fit_batch(lasp_ctx *c, int64_t B, const float *flux, const f
     CUDA_TRY(c, cudaMemsetAsync(c->ddbg, 0, 24 * sizeof(unsigned long long), st));
     a.dbg = c->ddbg;
 #endif
-    return launch(c, kFit, *v, a, st);
+    return launch(c, opts->clean_every > 0 ? kFitClean : kFit, *v, a, st);
 }
 
 extern "C" int lasp_eval_grad(lasp_ctx *c, int64_t B, const float *flux, const float *ivar,
@@ -737,9 +755,9 @@ static void hostpipe_free(lasp_ctx *c)
     lasp_ctx::HostPipe &h = c->hp;
     for (int s = 0; s < 2; ++s) {
         cudaFree(h.flux[s]); cudaFree(h.ivar[s]); cudaFree(h.mask[s]); cudaFree(h.init[s]);
-        cudaFree(h.params[s]); cudaFree(h.cont[s]); cudaFree(h.chi2[s]); cudaFree(h.err[s]); cudaFree(h.status[s]); cudaFree(h.nsteps[s]);
+        cudaFree(h.params[s]); cudaFree(h.cont[s]); cudaFree(h.chi2[s]); cudaFree(h.err[s]); cudaFree(h.status[s]); cudaFree(h.nsteps[s]); cudaFree(h.maskout[s]);
         h.flux[s] = h.ivar[s] = h.init[s] = h.params[s] = h.cont[s] = h.chi2[s] = h.err[s] = nullptr;
-        h.mask[s] = nullptr; h.status[s] = nullptr; h.nsteps[s] = nullptr;
+        h.mask[s] = nullptr; h.status[s] = nullptr; h.nsteps[s] = nullptr; h.maskout[s] = nullptr;
     }
     h.cap = 0;
 }
@@ -772,6 +790,7 @@ static int hostpipe_reserve(lasp_ctx *c, int64_t chunk)
         CUDA_TRY(c, cudaMalloc(&h.err[s], n * M.NP * sizeof(float)));
         CUDA_TRY(c, cudaMalloc(&h.status[s], n * sizeof(int32_t)));
         CUDA_TRY(c, cudaMalloc(&h.nsteps[s], n * sizeof(int32_t)));
+        CUDA_TRY(c, cudaMalloc(&h.maskout[s], n * M.P));
     }
     h.cap = chunk;
     return LASP_OK;
@@ -779,7 +798,7 @@ static int hostpipe_reserve(lasp_ctx *c, int64_t chunk)
 
 static int hostpipe_run(lasp_ctx *c, int64_t B, const float *flux, const float *ivar, const uint8_t *mask,
                         const float *init, const lasp_fit_opts *opts, float *params, float *cont, float *chi2,
-                        float *err, int32_t *status, int32_t *n_steps, int64_t chunk)
+                        float *err, int32_t *status, int32_t *n_steps, uint8_t *mask_out, int64_t chunk)
 {
     lasp_ctx::HostPipe &h = c->hp;
     const ModelDev &M = c->M;
@@ -806,7 +825,8 @@ static int hostpipe_run(lasp_ctx *c, int64_t B, const float *flux, const float *
         if (i >= 2) CUDA_TRY(c, cudaStreamWaitEvent(h.s_fit, h.out_done[s], 0));   // slot's old results copied out
         rc = lasp_fit_batch(c, n, h.flux[s], h.ivar[s], mask ? h.mask[s] : nullptr, h.init[s], opts, h.params[s],
                             cont ? h.cont[s] : nullptr, h.chi2[s], err ? h.err[s] : nullptr,
-                            status ? h.status[s] : nullptr, n_steps ? h.nsteps[s] : nullptr, h.s_fit);
+                            status ? h.status[s] : nullptr, n_steps ? h.nsteps[s] : nullptr,
+                            mask_out ? h.maskout[s] : nullptr, h.s_fit);
         if (rc) return rc;
         CUDA_TRY(c, cudaEventRecord(h.fit_done[s], h.s_fit));
         CUDA_TRY(c, cudaStreamWaitEvent(h.s_out, h.fit_done[s], 0));
@@ -816,6 +836,7 @@ static int hostpipe_run(lasp_ctx *c, int64_t B, const float *flux, const float *
         if (err) CUDA_TRY(c, cudaMemcpyAsync(err + o * M.NP, h.err[s], (size_t)n * M.NP * sizeof(float), cudaMemcpyDeviceToHost, h.s_out));
         if (status) CUDA_TRY(c, cudaMemcpyAsync(status + o, h.status[s], (size_t)n * sizeof(int32_t), cudaMemcpyDeviceToHost, h.s_out));
         if (n_steps) CUDA_TRY(c, cudaMemcpyAsync(n_steps + o, h.nsteps[s], (size_t)n * sizeof(int32_t), cudaMemcpyDeviceToHost, h.s_out));
+        if (mask_out) CUDA_TRY(c, cudaMemcpyAsync(mask_out + o * M.P, h.maskout[s], (size_t)n * M.P, cudaMemcpyDeviceToHost, h.s_out));
         CUDA_TRY(c, cudaEventRecord(h.out_done[s], h.s_out));
     }
     return LASP_OK;
@@ -824,7 +845,7 @@ static int hostpipe_run(lasp_ctx *c, int64_t B, const float *flux, const float *
 extern "C" int lasp_fit_batch_host(lasp_ctx *c, int64_t B, const float *flux, const float *ivar,
                                    const uint8_t *mask, const float *init, const lasp_fit_opts *opts,
                                    float *params, float *cont, float *chi2, float *err, int32_t *status,
-                                   int32_t *n_steps, int64_t chunk)
+                                   int32_t *n_steps, uint8_t *mask_out, int64_t chunk)
 {
     if (!c) return fail(nullptr, LASP_ERR_INVALID_ARG, "null ctx");
     if (B < 1 || !flux || !ivar || !init || !opts || !params || !chi2 || chunk < 0)
@@ -834,7 +855,7 @@ extern "C" int lasp_fit_batch_host(lasp_ctx *c, int64_t B, const float *flux, co
     chunk = std::min<int64_t>(chunk, B);
     int rc = hostpipe_reserve(c, chunk);
     if (rc) return rc;
-    rc = hostpipe_run(c, B, flux, ivar, mask, init, opts, params, cont, chi2, err, status, n_steps, chunk);
+    rc = hostpipe_run(c, B, flux, ivar, mask, init, opts, params, cont, chi2, err, status, n_steps, mask_out, chunk);
     // success or not, nothing of this call may still be in flight on the private streams when it returns: the
     // copies read and write the caller's buffers
     const std::string first = c->err;

@@ -585,3 +585,118 @@ def test_stopping_rules_at_the_papers_settings(gpu, oracle_mod):
             sel = ns == n
             assert np.array_equal(r["params"].cpu().numpy()[sel], fixed["params"].cpu().numpy()[sel])
         m.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# Clean-strategy masking, against oracle/lasp_oracle.c orc_fit_clean
+# ------------------------------------------------------------------------------------------------
+def _contaminate(case, seed):
+    """Cosmic-ray-like spikes and a few-pixel emission feature on every spectrum (what the Clean strategy is for)."""
+    rng = np.random.default_rng(seed)
+    flux = case["flux"].copy()
+    P = case["desc"]["n_pix"]
+    hits = []
+    for i in range(case["B"]):
+        j = rng.choice(np.arange(40, P - 40), size=6, replace=False)
+        amp = rng.uniform(0.4, 2.0, size=6) * np.median(np.abs(flux[i]))
+        flux[i, j] += amp.astype(flux.dtype)
+        k = int(rng.integers(60, P - 60))
+        bump = np.array([0.3, 0.8, 1.0, 0.7, 0.25]) * 0.9 * np.median(np.abs(flux[i]))
+        flux[i, k:k + 5] += bump.astype(flux.dtype)
+        hits.append(np.concatenate([j, [k + 1, k + 2, k + 3]]))
+    return flux, hits
+
+
+def _check_clean(gpu, oracle_mod, case, n_iter, lr, every=30, seed=5, min_same=0.75):
+    m = gpu.LaspModel(case["desc"])
+    o = oracle_mod.Oracle(case["desc"])
+    flux, hits = _contaminate(case, seed)
+    args = (flux, case["ivar"], case["mask"], case["init"])
+    r = m.fit_batch(*args, n_iter, lr=lr, clean_every=every)
+    ref = o.fit_clean(*args, n_iter, lr=lr, every=every)
+    mg = r["mask_out"].cpu().numpy()
+    B, P = mg.shape
+    # integer work: the masks.  The clipping thresholds compare float residuals (fp32 here, fp64 in the oracle) with
+    # k sigma, so a pixel within rounding of a threshold may fall on either side: what is unique is compared exactly
+    # (every pixel the oracle clips by a clear margin, every pixel it keeps by a clear margin), the rest must be few.
+    w0 = np.stack([fit_weights(case, i) for i in range(B)]) > 0
+    assert not np.any(mg & ~w0) and not np.any(ref["mask"] & ~w0)              # masks only shrink (R-9)
+    diff = (mg != ref["mask"]).sum(axis=1)
+    same = diff == 0
+    assert same.mean() >= min_same, diff
+    assert diff.sum() <= 2e-4 * B * P + 2, diff
+    for i in range(B):
+        inside = w0[i][hits[i]]
+        assert np.all(mg[i][hits[i]][inside] == 0), i                           # the injected outliers are gone
+    clipped = (w0 & (mg == 0)).sum(axis=1)
+    assert np.all(clipped >= 6) and np.all(clipped < 0.06 * P)
+    # the final evaluation, at identical parameters and identical mask: chi2 and continuum
+    par = r["params"].cpu().numpy().astype(np.float64)
+    chi_same, _, cont_same, st_same = o.eval_grad(flux, case["ivar"], mg, par)
+    chi = r["chi2"].cpu().numpy().astype(np.float64)
+    assert np.abs(chi / chi_same - 1).max() <= TOL_CHI2
+    assert np.array_equal(r["status"].cpu().numpy(), st_same)
+    gc = r["cont"].cpu().numpy().astype(np.float64)
+    for i in range(B):
+        keep = mg[i] > 0
+        ratio = cont_values(case["desc"], gc, i)[keep] / cont_values(case["desc"], cont_same, i)[keep]
+        assert np.abs(ratio - 1).max() <= TOL_CONT, (i, np.abs(ratio - 1).max())
+    # the whole fit, where the two sides took the same clipping decisions
+    dpar = np.abs(par - ref["params"]) / (o.hi - o.lo)
+    assert dpar[same].max() <= TOL_PAR, dpar.max(axis=1)
+    assert np.abs(chi[same] / ref["chi2"][same] - 1).max() <= 10 * TOL_CHI2
+    e = r["err"].cpu().numpy().astype(np.float64)
+    ok = same & np.isfinite(ref["err"]).all(axis=1)
+    assert np.abs(e[ok] / ref["err"][ok] - 1).max() <= TOL_ERR
+    # where a borderline pixel differs the fits still agree to a few tolerances (one pixel of ~1e3 changes little)
+    assert dpar.max() <= 5 * TOL_PAR, dpar.max(axis=1)
+    m.close()
+    return r, ref, same
+
+
+def test_clean_strategy_small_model(gpu, oracle_mod):
+    """Config-0-like single-segment model, mask updates after steps 30, 60, 90, 120 of 150."""
+    case = make(small_config(snr=(60.0, 60.0)), oracle_mod, B=18)     # 18: a ragged last group
+    _check_clean(gpu, oracle_mod, case, 150, 0.03)
+
+
+def test_clean_strategy_config1_shapes(gpu, oracle_mod):
+    """LAMOST-like spectra (config 1 shapes), the paper's schedule (every 30 steps, at most 11 updates): 12 updates
+    would fit into 360 steps, the 12th must not happen (the oracle stops at 11 too)."""
+    case = synth.make_case(1, oracle_mod.forward, B=12)
+    _check_clean(gpu, oracle_mod, case, 365, 0.02)
+
+
+def test_clean_off_reports_the_input_mask(gpu, oracle_mod):
+    """mask_out without Clean is the staged mask: ivar * mask != 0 away from the segment edges, on several segments too;
+    and a fit with clean_every > n_iter is bit-identical to the fit without Clean."""
+    for case in (make(two_arm_config(), oracle_mod), make(small_config(), oracle_mod, B=6)):
+        m = gpu.LaspModel(case["desc"])
+        args = (case["flux"], case["ivar"], case["mask"], case["init"])
+        r = m.fit_batch(*args, 5)
+        w0 = np.stack([fit_weights(case, i) for i in range(case["B"])]) > 0
+        assert np.array_equal(r["mask_out"].cpu().numpy() > 0, w0)
+        if case["desc"]["n_seg"] == 1:
+            r2 = m.fit_batch(*args, 5, clean_every=30)
+            for k in ("params", "chi2", "cont", "err", "mask_out"):
+                assert np.array_equal(r[k].cpu().numpy(), r2[k].cpu().numpy(), equal_nan=True), k
+        m.close()
+
+
+def test_clean_unsupported_combinations(gpu, oracle_mod):
+    """Several segments, the streaming variant, and Clean together with the stopping rules: LASP_ERR_UNSUPPORTED."""
+    case = make(two_arm_config(), oracle_mod)
+    m = gpu.LaspModel(case["desc"])
+    with pytest.raises(gpu.LaspError, match="Clean"):
+        m.fit_batch(case["flux"], case["ivar"], case["mask"], case["init"], 5, clean_every=2)
+    m.close()
+    case = make(small_config(), oracle_mod, B=4)
+    m = gpu.LaspModel(case["desc"])
+    args = (case["flux"], case["ivar"], case["mask"], case["init"])
+    with pytest.raises(gpu.LaspError, match="Clean"):
+        m.fit_batch(*args, 5, clean_every=2, variant=2)
+    with pytest.raises(gpu.LaspError, match="Clean"):
+        m.fit_batch(*args, 5, clean_every=2, stop_window=3)
+    with pytest.raises(gpu.LaspError):
+        m.fit_batch(*args, 5, clean_every=-1)
+    m.close()
