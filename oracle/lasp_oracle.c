@@ -761,14 +761,18 @@ int orc_clean_update(int P, int n_seg, const int32_t *seg_offset, const double *
     return n;
 }
 
-/* lasp_fit_batch with the Clean strategy: as orc_fit (fixed n_iter steps), and after update t, t = every, 2 every, ...
+/* lasp_fit_batch with the Clean strategy: as orc_fit (window = 0: fixed n_iter steps) or as orc_fit_stop (window > 0:
+ * the stopping rules of P:169-171, R-2..R-5, n_iter the maximum), and after update t, t = every, 2 every, ...
  * (at most max_updates times; the paper: every 30 steps, up to 11) the mask is updated from the residuals at
- * the new iterate, with f_shift = 0.5 for the first update and 0.2 afterwards.  mask_out[i*P+j] = 1 where the
- * pixel still takes part at the end. */
+ * the new iterate, with f_shift = 0.5 for the first update and 0.2 afterwards.  A spectrum that has stopped
+ * gets no further mask update (its optimisation is over, "during the optimization").  The loss of R-2 keeps its
+ * denominator n_pix when pixels are clipped (Eq. 9 divides by p N, not by the number of unmasked pixels).
+ * mask_out[i*P+j] = 1 where the pixel still takes part at the end; n_steps[i] = Adam updates applied. */
 int orc_fit_clean(const orc_model *m, int64_t B, const double *flux, const double *ivar,
                   const uint8_t *mask, const double *init, int n_iter, double lr, double b1, double b2,
-                  double eps_adam, int every, int max_updates, double fd_h, double *params, double *cont,
-                  double *chi2, double *err, int32_t *status, uint8_t *mask_out, int32_t *n_clipped)
+                  double eps_adam, int every, int max_updates, int window, double tol, double fd_h, double *params,
+                  double *cont, double *chi2, double *err, int32_t *status, uint8_t *mask_out, int32_t *n_clipped,
+                  int32_t *n_steps)
 {
     int NP = m->n_labels + 2, P = m->n_pix, nc = m->n_seg * (m->cont_degree + 1);
 #pragma omp parallel
@@ -776,6 +780,7 @@ int orc_fit_clean(const orc_model *m, int64_t B, const double *flux, const doubl
         work_t *k = work_new(m);
         double *u = calloc(NP, 8), *mom = calloc(NP, 8), *vel = calloc(NP, 8), *g = calloc(NP, 8);
         double *Mod = calloc(P, 8);
+        double *hist = calloc((size_t)n_iter + 1, 8);
 #pragma omp for schedule(dynamic, 1)
         for (int64_t i = 0; i < B; ++i) {
             const double *y = flux + i * P;
@@ -783,11 +788,19 @@ int orc_fit_clean(const orc_model *m, int64_t B, const double *flux, const doubl
             norm_u(m, init + i * NP, u);
             memset(mom, 0, 8 * NP);
             memset(vel, 0, 8 * NP);
-            int updates = 0, clipped = 0;
+            int updates = 0, clipped = 0, rule = 1, rise = 0, applied = 0;
             for (int t = 1; t <= n_iter; ++t) {
-                chi2_at(m, k, u, y, 1, NULL);
+                double c2t = chi2_at(m, k, u, y, 1, NULL);
+                if (window > 0) {                                    /* as orc_fit_stop */
+                    double L = sqrt(c2t / (double)P);
+                    hist[t] = L;
+                    if (t > 1 && L > hist[t - 1]) ++rise; else rise = 0;
+                    if (t > window && fabs(L - hist[t - window]) < tol) { rule = 2; break; }
+                    if (rise >= window) { rule = 3; break; }
+                }
                 grad_from_work(k, g);
                 orc_adam_step(NP, u, mom, vel, g, t, lr, b1, b2, eps_adam);
+                applied = t;
                 if (every > 0 && t % every == 0 && updates < max_updates) {
                     chi2_at(m, k, u, y, 0, NULL);                    /* residuals at the new iterate */
                     for (int j = 0; j < P; ++j) Mod[j] = k->c[j] * k->S[j];
@@ -801,12 +814,15 @@ int orc_fit_clean(const orc_model *m, int64_t B, const double *flux, const doubl
             denorm(m, u, params + i * NP);
             if (cont) memcpy(cont + i * nc, k->b, 8 * (size_t)nc);
             st = final_status(k, u, c2, st);
+            if (rule == 2) st |= 16;
+            if (rule == 3) st |= 32;
             if (status) status[i] = st;
+            if (n_steps) n_steps[i] = applied;
             if (mask_out) for (int j = 0; j < P; ++j) mask_out[i * P + j] = k->w[j] != 0.0;
             if (n_clipped) n_clipped[i] = clipped;
             if (err) errors_one(m, k, u, y, fd_h, err + i * NP);
         }
-        free(u); free(mom); free(vel); free(g); free(Mod);
+        free(u); free(mom); free(vel); free(g); free(Mod); free(hist);
         work_free(k);
     }
     return 0;

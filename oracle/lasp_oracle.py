@@ -216,21 +216,24 @@ class Oracle:
         return dict(params=params, cont=cont, chi2=chi2, err=err, status=status, n_steps=n_steps)
 
     def fit_clean(self, flux, ivar, mask, init, n_iter, lr=1e-2, beta1=0.9, beta2=0.999, eps=1e-8, every=30, max_updates=11,
-                  fd_h=1e-5, want_err=True):
-        """The fixed-step fit with the Clean strategy (orc_fit_clean)."""
+                  window=0, tol=1e-5, fd_h=1e-5, want_err=True):
+        """The fit with the Clean strategy (orc_fit_clean): fixed n_iter steps (window = 0) or the
+        stopping rules of P:169-171 (window > 0, n_iter the maximum)."""
         flux, ivar, mask = self._obs(flux, ivar, mask)
         B = flux.shape[0]
         init = self._f64(init).reshape(B, self.NP)
         params = np.empty((B, self.NP)); cont = np.empty((B, self.nc)); chi2 = np.empty(B)
         err = np.empty((B, self.NP)) if want_err else None
-        status = np.zeros(B, dtype=np.int32); n_clipped = np.zeros(B, dtype=np.int32)
+        status = np.zeros(B, dtype=np.int32); n_clipped = np.zeros(B, dtype=np.int32); n_steps = np.zeros(B, dtype=np.int32)
         mask_out = np.zeros((B, self.P), dtype=np.uint8)
         lib().orc_fit_clean(C.byref(self.m), C.c_int64(B), _p(flux, _f64p), _p(ivar, _f64p),
                             _p(mask, _u8p) if mask is not None else None, _p(init, _f64p), C.c_int(n_iter),
                             C.c_double(lr), C.c_double(beta1), C.c_double(beta2), C.c_double(eps), C.c_int(every),
-                            C.c_int(max_updates), C.c_double(fd_h), _p(params, _f64p), _p(cont, _f64p), _p(chi2, _f64p),
-                            _p(err, _f64p) if want_err else None, _p(status, _i32p), _p(mask_out, _u8p), _p(n_clipped, _i32p))
-        return dict(params=params, cont=cont, chi2=chi2, err=err, status=status, mask=mask_out, n_clipped=n_clipped)
+                            C.c_int(max_updates), C.c_int(window), C.c_double(tol), C.c_double(fd_h), _p(params, _f64p),
+                            _p(cont, _f64p), _p(chi2, _f64p), _p(err, _f64p) if want_err else None, _p(status, _i32p),
+                            _p(mask_out, _u8p), _p(n_clipped, _i32p), _p(n_steps, _i32p))
+        return dict(params=params, cont=cont, chi2=chi2, err=err, status=status, mask=mask_out, n_clipped=n_clipped,
+                    n_steps=n_steps)
 
 def stop_rule(L, window=50, tol=1e-5):
     """First step t (1-based) at which criterion (2) or (3) of P:169-171 fires on the loss sequence L, and the rule

@@ -698,6 +698,38 @@ def test_fit_with_clean_strategy(oracle_mod):
     assert np.all(clean["n_clipped"] >= hit.size) and np.all(clean["n_clipped"] < 0.05 * P)
 
 
+def test_fit_with_clean_strategy_and_stopping_rules(oracle_mod):
+    """orc_fit_clean with window > 0 against the pinned pieces: without mask updates it is orc_fit_stop; with an infinite
+    tolerance every spectrum stops at the first testable step (t = window + 1, `window` updates applied) and the result
+    is the fixed-step Clean fit of `window` steps, the mask update after step 30 included; with tolerance 0 nothing
+    fires and it is the fixed-step Clean fit; and a mask update postpones criterion (2): the clipped outliers make the
+    loss drop, so the stop comes later than that of the same fit without Clean on clean data never would."""
+    case = make(small_config(mask_frac=0.0, snr=(60.0, 60.0)), oracle_mod, B=3)
+    o = oracle_mod.Oracle(case["desc"])
+    flux = case["flux"].copy()
+    flux[:, [150, 151, 300]] += 1.5
+    args = (flux, case["ivar"], case["mask"], case["init"])
+    a = o.fit_clean(*args, 120, lr=0.05, every=0, window=20, tol=1e-4)
+    b = o.fit_stop(*args, 120, lr=0.05, window=20, tol=1e-4)
+    for k in ("params", "chi2", "cont", "err", "status", "n_steps"):
+        assert np.array_equal(a[k], b[k], equal_nan=True), k
+    a = o.fit_clean(*args, 200, lr=0.05, every=30, window=40, tol=1e30)
+    b = o.fit_clean(*args, 40, lr=0.05, every=30)
+    assert np.array_equal(a["n_steps"], np.full(3, 40)) and np.all(a["status"] & 16)
+    for k in ("params", "chi2", "cont", "err", "mask", "n_clipped"):
+        assert np.array_equal(a[k], b[k], equal_nan=True), k
+    assert np.all(a["n_clipped"] >= 3)
+    a = o.fit_clean(*args, 70, lr=0.05, every=30, window=40, tol=0.0)
+    b = o.fit_clean(*args, 70, lr=0.05, every=30)
+    assert np.array_equal(a["n_steps"], np.full(3, 70)) and not np.any(a["status"] & 48)
+    for k in ("params", "chi2", "cont", "err", "mask"):
+        assert np.array_equal(a[k], b[k], equal_nan=True), k
+    # a spectrum that has stopped gets no further mask update: stop at t = 21 (before the first update at step 30)
+    a = o.fit_clean(*args, 200, lr=0.05, every=30, window=20, tol=1e30)
+    assert np.array_equal(a["n_steps"], np.full(3, 20)) and np.all(a["n_clipped"] == 0)
+    assert np.array_equal(a["mask"], (case["ivar"] * case["mask"] != 0) & _not_edge(case))
+
+
 def _not_edge(case):
     d = case["desc"]
     keep = np.ones((case["B"], d["n_pix"]), dtype=bool)
