@@ -306,7 +306,7 @@ def run_other_config(cfg_id, B, torch, local, peaks, n_sms, emulator_path=0, pap
         inner = slice(ne, model.P - ne)
         w0 = ((data["ivar"][:, inner] != 0) & (data["mask"][:, inner] != 0)).sum(dim=1).float()
         kept = out["mask_out"].sum(dim=1, dtype=torch.float32)
-        rec.update({"workload": f"config {cfg_id} shapes with the Clean strategy (mask update every 30 steps, at most 11)",
+        rec.update({"workload": rec["workload"] + " + the Clean strategy (mask update every 30 steps, at most 11)",
                     "clean_every": 30, "clean_max": 11,
                     "clipped_frac_of_unmasked": float(((w0 - kept) / w0.clamp_min(1.0)).mean().item())})
     model.close()
@@ -503,6 +503,10 @@ def run_gpu(args):
             oc["config1_clean"] = run_other_config(1, 65536, torch, local, peaks, n_sms, clean=True)
         except Exception as e:
             oc["config1_clean"] = {"error": f"{type(e).__name__}: {e}"}
+        try:
+            oc["config1_paper_stop_clean"] = run_other_config(1, 65536, torch, local, peaks, n_sms, paper_stop=True, clean=True)
+        except Exception as e:
+            oc["config1_paper_stop_clean"] = {"error": f"{type(e).__name__}: {e}"}
         line["other_configs"] = oc
     if world == 1 and not args.no_cpu_baseline:
         cores = os.cpu_count() or 1

@@ -119,8 +119,9 @@ typedef struct {
                                      and the pixel mask is updated (primary 3-sigma clipping with threshold escalation and the
                                      flux-gradient allowance f_shift = 0.5 first, 0.2 afterwards; adjacent pixels at 2 sigma;
                                      neighbourhood growth); clipped pixels stay clipped.  The paper: every 30 steps.
-                                     Needs the resident variant, one segment whose fitted range is one sweep of the CTA, and
-                                     stop_window = 0, else LASP_ERR_UNSUPPORTED */
+                                     With the stopping rules on, a spectrum that has stopped gets no further update.
+                                     Needs the resident variant and one segment whose fitted range is one sweep of the
+                                     CTA, else LASP_ERR_UNSUPPORTED */
     int32_t clean_max;            /* at most this many mask updates per spectrum (0 = default 11) */
 } lasp_fit_opts;
 

@@ -2248,7 +2248,7 @@ __device__ __noinline__ void v1_clean_update(float fshift)
     if (act && O) {
 #pragma unroll
         for (int g = 0; g < GS; ++g) {
-            if (!((O >> (g * OCT)) & 0xffu)) continue;
+            if (!((O >> (g * OCT)) & 0xffu) || v1_blk.stop_rule[g] != 0) continue;   // a stopped spectrum keeps its mask
             float4 *w4 = (float4 *)(Wg + (size_t)v1_blk.spec[g] * Ppad + (j0 >> 1));
             float4 w0 = __ldcg(w4), w1 = __ldcg(w4 + P8);
             const unsigned o = O >> (g * OCT);

@@ -623,8 +623,6 @@ extern "C" int lasp_fit_batch(lasp_ctx *c, int64_t B, const float *flux, const f
         if (v != &c->res || c->M.n_seg != 1 || (S0.fit_hi - S0.fit_lo) / OCT > v->nt)
             return fail(c, LASP_ERR_UNSUPPORTED, "lasp_fit_batch: the Clean strategy needs the resident variant and one segment "
                                                  "whose fitted range is one sweep of the CTA");
-        if (opts->stop_window > 0)
-            return fail(c, LASP_ERR_UNSUPPORTED, "lasp_fit_batch: the Clean strategy runs a fixed number of steps (stop_window = 0)");
     }
     DeviceGuard dg(c->device);
     rc = workspace(c, B, *v, true, true, err != nullptr);

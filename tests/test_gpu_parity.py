@@ -684,7 +684,7 @@ def test_clean_off_reports_the_input_mask(gpu, oracle_mod):
 
 
 def test_clean_unsupported_combinations(gpu, oracle_mod):
-    """Several segments, the streaming variant, and Clean together with the stopping rules: LASP_ERR_UNSUPPORTED."""
+    """Several segments and the streaming variant: LASP_ERR_UNSUPPORTED."""
     case = make(two_arm_config(), oracle_mod)
     m = gpu.LaspModel(case["desc"])
     with pytest.raises(gpu.LaspError, match="Clean"):
@@ -695,8 +695,39 @@ def test_clean_unsupported_combinations(gpu, oracle_mod):
     args = (case["flux"], case["ivar"], case["mask"], case["init"])
     with pytest.raises(gpu.LaspError, match="Clean"):
         m.fit_batch(*args, 5, clean_every=2, variant=2)
-    with pytest.raises(gpu.LaspError, match="Clean"):
-        m.fit_batch(*args, 5, clean_every=2, stop_window=3)
     with pytest.raises(gpu.LaspError):
         m.fit_batch(*args, 5, clean_every=-1)
+    m.close()
+
+
+def test_clean_strategy_with_stopping_rules(gpu, oracle_mod):
+    """The paper's full loop: lr 0.1, stopping rules (window 50, tolerance 1e-5) and mask updates every 30
+    steps in the same run, on contaminated config-1 shapes.  Stop steps are unique only up to the rounding of the
+    tolerance test (as in test_stopping_rules_at_the_papers_settings), the masks up to threshold rounding."""
+    case = synth.make_case(1, oracle_mod.forward, B=12)
+    m = gpu.LaspModel(case["desc"])
+    o = oracle_mod.Oracle(case["desc"])
+    flux, hits = _contaminate(case, 9)
+    args = (flux, case["ivar"], case["mask"], case["init"])
+    r = m.fit_batch(*args, 5000, lr=0.1, stop_window=50, stop_tol=1e-5, clean_every=30)
+    ref = o.fit_clean(*args, 5000, lr=0.1, every=30, window=50, tol=1e-5)
+    ns, st, mg = r["n_steps"].cpu().numpy(), r["status"].cpu().numpy(), r["mask_out"].cpu().numpy()
+    assert np.all(ref["n_steps"] < 5000) and np.array_equal(st & 48, ref["status"] & 48)
+    assert np.abs(ns - ref["n_steps"]).max() <= 5, (ns, ref["n_steps"])
+    diff = (mg != ref["mask"]).sum(axis=1)
+    assert (diff == 0).mean() >= 0.75 and diff.sum() <= 4, diff
+    same = diff == 0
+    par = r["params"].cpu().numpy().astype(np.float64)
+    dpar = np.abs(par - ref["params"]) / (o.hi - o.lo)
+    assert dpar[same].max() <= TOL_PAR, dpar.max(axis=1)
+    chi = r["chi2"].cpu().numpy().astype(np.float64)
+    assert np.abs(chi[same] / ref["chi2"][same] - 1).max() <= 10 * TOL_CHI2
+    for i in range(case["B"]):
+        assert np.all(mg[i][hits[i]] == 0) or not np.all(fit_weights(case, i)[hits[i]] > 0)
+    # structure: infinite tolerance with window 40 = the fixed-step Clean fit of 40 steps (one mask update, after step 30)
+    a = m.fit_batch(*args, 200, lr=0.05, stop_window=40, stop_tol=1e30, clean_every=30)
+    b = m.fit_batch(*args, 40, lr=0.05, clean_every=30)
+    assert np.array_equal(a["n_steps"].cpu().numpy(), np.full(12, 40))
+    for k in ("params", "mask_out"):
+        assert np.array_equal(a[k].cpu().numpy(), b[k].cpu().numpy()), k
     m.close()
