@@ -19,6 +19,7 @@
  *   Adam                step 8  P:169              orc_adam_step
  *   stopping rules      step 8  P:169-171          orc_stop_rule, orc_fit_stop
  *   Clean masking       step 6  P:137-161, P:171   orc_clean_update, orc_fit_clean
+ *   LM optimiser        NEXT-4  P:54-58, P:397     orc_fit_lm (Marquardt's method written out; R-13)
  *   error estimate      step 9  P:173              errors_one
  *
  * Parity pins (tests/test_oracle_*.py): numpy legvander/legval, numpy lstsq,
@@ -823,6 +824,105 @@ int orc_fit_clean(const orc_model *m, int64_t B, const double *flux, const doubl
             if (err) errors_one(m, k, u, y, fd_h, err + i * NP);
         }
         free(u); free(mom); free(vel); free(g); free(Mod); free(hist);
+        work_free(k);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------- Levenberg-Marquardt on the NP x NP system
+ *
+ * The paper's LASP-CurveFit minimises the same chi2 with scipy.optimize.curve_fit, and its future work asks
+ * for "curvature awareness" in LASP-Adam-GPU.  Neither passage states an algorithm; this is Marquardt's method
+ * written out on the objective of steps 5-7 (reading R-13 of DESIGN.md):
+ *   rho(u) = sqrt(w) (y - c(u) S(u)) with the continuum re-solved at every u (variable projection, as step 9);
+ *   J by central differences of step h in u (as errors_one), A = J^T J, g = J^T rho;
+ *   lambda = lambda0; chi2 = |rho(u)|^2; then n_iter times:
+ *     solve (A + lambda diag(A)) delta = -g  (Cholesky; delta = 0 when it is not positive definite);
+ *     u' = clip(u + delta, [-1, 1]); chi2' = |rho(u')|^2;
+ *     chi2' < chi2: u = u', chi2 = chi2', lambda = max(lambda / 10, 1e-10), one more accepted step;
+ *     otherwise (NaN included): u stays, lambda = min(10 lambda, 1e10).
+ * Then the final evaluation, status and error estimate of orc_fit.  n_steps[i] = accepted steps. */
+static void lm_residual(const orc_model *m, work_t *k, const double *u, const double *y, double *rho, double *c2)
+{
+    *c2 = chi2_at(m, k, u, y, 0, NULL);
+    for (int j = 0; j < k->P; ++j) rho[j] = sqrt(k->w[j]) * k->r[j];
+}
+
+int orc_fit_lm(const orc_model *m, int64_t B, const double *flux, const double *ivar,
+               const uint8_t *mask, const double *init, int n_iter, double lambda0, double fd_h,
+               double *params, double *cont, double *chi2, double *err, int32_t *status, int32_t *n_steps,
+               double *trace)
+{
+    int NP = m->n_labels + 2, P = m->n_pix, nc = m->n_seg * (m->cont_degree + 1);
+#pragma omp parallel
+    {
+        work_t *k = work_new(m);
+        double *u = calloc(NP, 8), *ut = calloc(NP, 8), *up = calloc(NP, 8), *g = calloc(NP, 8);
+        double *J = calloc((size_t)NP * P, 8), *rho = calloc(P, 8), *rp = calloc(P, 8), *rm = calloc(P, 8);
+        double *A = calloc((size_t)NP * NP, 8), *N = calloc((size_t)NP * NP, 8);
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t i = 0; i < B; ++i) {
+            const double *y = flux + i * P;
+            make_weights(m, ivar + i * P, mask ? mask + i * P : NULL, k->w);
+            norm_u(m, init + i * NP, u);
+            double lam = lambda0, c2;
+            int accepted = 0;
+            lm_residual(m, k, u, y, rho, &c2);
+            if (trace) trace[i * (n_iter + 1)] = c2;
+            for (int t = 1; t <= n_iter; ++t) {
+                for (int p = 0; p < NP; ++p) {
+                    double cc;
+                    memcpy(up, u, 8 * NP);
+                    up[p] = u[p] + fd_h;
+                    lm_residual(m, k, up, y, rp, &cc);
+                    up[p] = u[p] - fd_h;
+                    lm_residual(m, k, up, y, rm, &cc);
+                    for (int j = 0; j < P; ++j) J[(size_t)p * P + j] = (rp[j] - rm[j]) / (2.0 * fd_h);
+                }
+                for (int a = 0; a < NP; ++a) {
+                    double s = 0.0;
+                    for (int j = 0; j < P; ++j) s += J[(size_t)a * P + j] * rho[j];
+                    g[a] = s;
+                    for (int b = 0; b < NP; ++b) {
+                        double acc = 0.0;
+                        for (int j = 0; j < P; ++j) acc += J[(size_t)a * P + j] * J[(size_t)b * P + j];
+                        A[a * NP + b] = acc;
+                    }
+                }
+                memcpy(N, A, 8 * (size_t)NP * NP);
+                for (int a = 0; a < NP; ++a) N[a * NP + a] += lam * A[a * NP + a];
+                memcpy(ut, u, 8 * NP);
+                if (!cholesky(N, NP)) {
+                    for (int a = 0; a < NP; ++a) up[a] = -g[a];
+                    chol_solve(N, NP, up);
+                    for (int a = 0; a < NP; ++a) {
+                        double v = u[a] + up[a];
+                        ut[a] = v < -1.0 ? -1.0 : (v > 1.0 ? 1.0 : v);
+                    }
+                }
+                double c2t;
+                lm_residual(m, k, ut, y, rp, &c2t);
+                if (c2t < c2) {
+                    memcpy(u, ut, 8 * NP);
+                    memcpy(rho, rp, 8 * (size_t)P);
+                    c2 = c2t;
+                    lam = fmax(lam / 10.0, 1e-10);
+                    ++accepted;
+                } else
+                    lam = fmin(lam * 10.0, 1e10);
+                if (trace) trace[i * (n_iter + 1) + t] = c2;
+            }
+            int st = 0;
+            double cf = chi2_at(m, k, u, y, 0, &st);
+            chi2[i] = cf;
+            denorm(m, u, params + i * NP);
+            if (cont) memcpy(cont + i * nc, k->b, 8 * (size_t)nc);
+            st = final_status(k, u, cf, st);
+            if (status) status[i] = st;
+            if (n_steps) n_steps[i] = accepted;
+            if (err) errors_one(m, k, u, y, fd_h, err + i * NP);
+        }
+        free(u); free(ut); free(up); free(g); free(J); free(rho); free(rp); free(rm); free(A); free(N);
         work_free(k);
     }
     return 0;

@@ -235,6 +235,23 @@ class Oracle:
         return dict(params=params, cont=cont, chi2=chi2, err=err, status=status, mask=mask_out, n_clipped=n_clipped,
                     n_steps=n_steps)
 
+    def fit_lm(self, flux, ivar, mask, init, n_iter, lambda0=1e-3, fd_h=1e-5, want_err=True, want_trace=False):
+        """Levenberg-Marquardt on the NP x NP system (NEXT-4; orc_fit_lm): n_iter LM iterations from `init`."""
+        flux, ivar, mask = self._obs(flux, ivar, mask)
+        B = flux.shape[0]
+        init = self._f64(init).reshape(B, self.NP)
+        params = np.empty((B, self.NP)); cont = np.empty((B, self.nc)); chi2 = np.empty(B)
+        err = np.empty((B, self.NP)) if want_err else None
+        status = np.zeros(B, dtype=np.int32); n_steps = np.zeros(B, dtype=np.int32)
+        trace = np.zeros((B, n_iter + 1)) if want_trace else None
+        lib().orc_fit_lm(C.byref(self.m), C.c_int64(B), _p(flux, _f64p), _p(ivar, _f64p),
+                         _p(mask, _u8p) if mask is not None else None, _p(init, _f64p), C.c_int(n_iter),
+                         C.c_double(lambda0), C.c_double(fd_h), _p(params, _f64p), _p(cont, _f64p), _p(chi2, _f64p),
+                         _p(err, _f64p) if want_err else None, _p(status, _i32p), _p(n_steps, _i32p),
+                         _p(trace, _f64p) if want_trace else None)
+        return dict(params=params, cont=cont, chi2=chi2, err=err, status=status, n_steps=n_steps, trace=trace)
+
+
 def stop_rule(L, window=50, tol=1e-5):
     """First step t (1-based) at which criterion (2) or (3) of P:169-171 fires on the loss sequence L, and the rule
     (1 = neither within the sequence, then t = 0)."""

@@ -730,6 +730,89 @@ def test_fit_with_clean_strategy_and_stopping_rules(oracle_mod):
     assert np.array_equal(a["mask"], (case["ivar"] * case["mask"] != 0) & _not_edge(case))
 
 
+# ------------------------------------------------------------------------------------------------
+# Levenberg-Marquardt on the NP x NP system (orc_fit_lm, reading R-13)
+# ------------------------------------------------------------------------------------------------
+def _lm_case(oracle_mod, **kw):
+    case = make(small_config(snr=(60.0, 60.0), **kw), oracle_mod, B=3)
+    d = case["desc"]
+    o = oracle_mod.Oracle(d)
+    ne = d["seg_n_edge"][0]
+    ws = []
+    for i in range(3):
+        w = case["ivar"][i].astype(np.float64) * case["mask"][i]
+        w[:ne] = 0; w[-ne:] = 0
+        ws.append(w)
+    return case, d, o, ws
+
+
+def test_lm_first_step_is_marquardts_formula(oracle_mod):
+    """One LM iteration rebuilt in numpy from the numpy residual of the error-estimate pins (eval_S + lstsq): J by central
+    differences, delta = -(J^T J + lambda diag(J^T J))^-1 J^T rho, accepted because chi2 falls; a wrong sign, a missing
+    diagonal scaling or an undamped step fails it.  lambda = 10 makes damping matter (a Gauss-Newton step differs)."""
+    case, d, o, ws = _lm_case(oracle_mod)
+    for lam in (1e-3, 10.0):
+        r = o.fit_lm(case["flux"], case["ivar"], case["mask"], case["init"], 1, lambda0=lam, want_err=False, want_trace=True)
+        for i in range(3):
+            y = case["flux"][i].astype(np.float64)
+            u = o.norm_u(case["init"][i])
+            h = 1e-5
+            J = np.empty((d["n_pix"], o.NP))
+            for p in range(o.NP):
+                up, um = u.copy(), u.copy()
+                up[p] += h; um[p] -= h
+                J[:, p] = (_numpy_rho(o, d, y, ws[i], up) - _numpy_rho(o, d, y, ws[i], um)) / (2 * h)
+            rho = _numpy_rho(o, d, y, ws[i], u)
+            A = J.T @ J
+            delta = -np.linalg.solve(A + lam * np.diag(np.diag(A)), J.T @ rho)
+            gn = -np.linalg.solve(A, J.T @ rho)
+            un = np.clip(u + delta, -1, 1)
+            rn = _numpy_rho(o, d, y, ws[i], un)
+            assert rn @ rn < rho @ rho and r["n_steps"][i] == 1
+            assert np.allclose(o.norm_u(r["params"][i]), un, atol=1e-9)
+            assert np.isclose(r["trace"][i, 0], rho @ rho, rtol=1e-10) and np.isclose(r["trace"][i, 1], rn @ rn, rtol=1e-9)
+            if lam == 10.0:
+                assert np.abs(delta - gn).max() > 1e-3          # the damped step is not the Gauss-Newton step
+
+
+def test_lm_converges_to_the_library_minimiser(oracle_mod):
+    """The minimum orc_fit_lm reaches is the one scipy.optimize.least_squares(method="lm") (MINPACK) finds on the numpy
+    residual, to 1e-6 of the prior range; chi2 never rises along the way; the analytic gradient of the oracle vanishes
+    there; and the fixed-step Adam fit lands on the same point."""
+    from scipy.optimize import least_squares
+    case, d, o, ws = _lm_case(oracle_mod)
+    r = o.fit_lm(case["flux"], case["ivar"], case["mask"], case["init"], 12, want_trace=True)
+    assert np.all(np.diff(r["trace"], axis=1) <= 0) and np.all(r["n_steps"] >= 3) and np.all(r["n_steps"] <= 12)
+    g0 = np.abs(o.eval_grad(case["flux"], case["ivar"], case["mask"], case["init"])[1]).max(axis=1)
+    g1 = np.abs(o.eval_grad(case["flux"], case["ivar"], case["mask"], r["params"])[1]).max(axis=1)
+    assert np.all(g1 < 1e-6 * g0)
+    for i in range(3):
+        y = case["flux"][i].astype(np.float64)
+        sol = least_squares(lambda u: _numpy_rho(o, d, y, ws[i], u), o.norm_u(case["init"][i]), method="lm",
+                            xtol=1e-14, ftol=1e-14, gtol=1e-14)
+        assert np.abs(o.norm_u(r["params"][i]) - sol.x).max() < 2e-6, np.abs(o.norm_u(r["params"][i]) - sol.x)
+        assert np.isclose(r["chi2"][i], 2 * sol.cost, rtol=1e-9)
+    adam = o.fit(case["flux"], case["ivar"], case["mask"], case["init"], 1500, lr=0.02, want_err=False)
+    assert (np.abs(adam["params"] - r["params"]) / (o.hi - o.lo)).max() < 1e-4
+    # zero iterations: the evaluation at the initial guess
+    z = o.fit_lm(case["flux"], case["ivar"], case["mask"], case["init"], 0, want_err=False)
+    assert np.allclose(z["params"], case["init"]) and np.all(z["n_steps"] == 0)
+
+
+def test_lm_noise_free_recovery_and_rejected_steps(oracle_mod):
+    """On noise-free spectra LM returns the truth (chi2 -> 0) from the offset starts; and with a huge initial damping the
+    first steps are tiny but accepted, while a start AT the minimum rejects everything (chi2 cannot fall): n_steps counts
+    accepted steps only and the iterate never moves uphill."""
+    case = make(small_config(mask_frac=0.0), oracle_mod, B=3, noise_free=True)
+    o = oracle_mod.Oracle(case["desc"])
+    r = o.fit_lm(case["flux"], case["ivar"], case["mask"], case["init"], 15, want_err=False)
+    assert (np.abs(r["params"] - case["truth"]) / (o.hi - o.lo)).max() < 1e-6
+    assert np.all(r["chi2"] < 1e-12 * o.fit_lm(case["flux"], case["ivar"], case["mask"], case["init"], 0, want_err=False)["chi2"])
+    again = o.fit_lm(case["flux"], case["ivar"], case["mask"], r["params"], 4, want_err=False, want_trace=True)
+    assert np.all(np.diff(again["trace"], axis=1) <= 0)
+    assert (np.abs(again["params"] - r["params"]) / (o.hi - o.lo)).max() < 1e-7
+
+
 def _not_edge(case):
     d = case["desc"]
     keep = np.ones((case["B"], d["n_pix"]), dtype=bool)
