@@ -259,11 +259,12 @@ def time_fit(model, data, n_iter, steps, warmup, kw, torch, barrier):
     return out, ev[0].elapsed_time(ev[-1]), step_ms, model.launch_count() - l0
 
 
-def run_other_config(cfg_id, B, torch, local, peaks, n_sms, emulator_path=0, paper_stop=False, clean=False):
+def run_other_config(cfg_id, B, torch, local, peaks, n_sms, emulator_path=0, paper_stop=False, clean=False, lm=0):
     """One timed step (after one warm-up) of another BASELINE.json config at a stated, reduced batch.
     paper_stop: the paper's optimiser settings instead of the config's fixed steps: lr 0.1, at most 5000
     iterations, stop when |L_t - L_(t-50)| < 1e-5 or after 50 consecutive increases (lasp_fit_opts.stop_window).
-    clean: the Clean strategy on the paper's schedule (mask update every 30 steps, at most 11)."""
+    clean: the Clean strategy on the paper's schedule (mask update every 30 steps, at most 11).
+    lm: that many Levenberg-Marquardt iterations instead of Adam (lasp_fit_opts.optimizer = 1)."""
     from paper_2512_24840_b200 import binding, synth
     cfg = synth.CONFIGS[cfg_id]
     desc = synth.make_model_desc(cfg)
@@ -278,9 +279,14 @@ def run_other_config(cfg_id, B, torch, local, peaks, n_sms, emulator_path=0, pap
         n_iter = 5000
     if clean:
         kw.update(clean_every=30, clean_max=11)
+    if lm:
+        kw.update(optimizer=1)
+        n_iter = lm
     out, ms_total, step_ms, _ = time_fit(model, data, n_iter, 1, 1, kw, torch, torch.cuda.synchronize)
     # evaluations actually executed per spectrum slot (= n_iter at fixed steps; the group's last stop step otherwise)
     steps_run = model.last_fit_stats()["group_steps"] * 4.0 / B
+    if lm:
+        steps_run = float(lm * (2 * model.NP + 1) + 1)   # evaluations (no adjoint pass): 2 NP for J + 1 trial per iteration
     roof = roofline_of(model, desc, B, steps_run, out["params"].cpu().numpy(), step_ms[0], peaks, n_sms)
     rec = {"workload": f"config {cfg_id} ({cfg.name})", "spectra": B, "full_batch": cfg.B, "adam_steps": n_iter,
            "n_pix": model.P, "n_terms": model.K, "n_labels": model.L, "n_seg": model.n_seg,
@@ -301,6 +307,23 @@ def run_other_config(cfg_id, B, torch, local, peaks, n_sms, emulator_path=0, pap
                     "stopped_by": {"tolerance": float(((st & 16) != 0).float().mean().item()),
                                    "rising_loss": float(((st & 32) != 0).float().mean().item()),
                                    "max_iterations": float(((st & 48) == 0).float().mean().item())}})
+    if lm:
+        # the same minimum as the config's Adam fit: compared on the first 4,096 spectra
+        n = min(B, 4096)
+        sub = {k: v[:n] for k, v in data.items()}
+        adam = model.fit_batch(sub["flux"], sub["ivar"], sub["mask"], sub["init"], cfg.n_iter, lr=cfg.lr, want_err=False)
+        rng_ = torch.tensor(np.asarray(desc["hi"]) - np.asarray(desc["lo"]), device=out["params"].device, dtype=torch.float32)
+        d = ((adam["params"] - out["params"][:n]).abs() / rng_).max(dim=1).values
+        ns = out["n_steps"].float()
+        rec.update({"workload": f"config {cfg_id} shapes, {lm} Levenberg-Marquardt iterations instead of {cfg.n_iter} Adam steps "
+                                "(lasp_fit_opts.optimizer = 1)",
+                    "optimizer": "lm", "lm_iterations": lm, "evaluations_per_spectrum": steps_run,
+                    "accepted_steps_mean": float(ns.mean().item()),
+                    "vs_adam_fit_max_dparam_over_range": {"median": float(d.median().item()),
+                                                          "p99": float(d.quantile(0.99).item()), "max": float(d.max().item())},
+                    "frac": None, "frac_executed": None,
+                    "note": "the FMA formulas of SURVEY 8(d) count an Adam step (forward + adjoint); an LM evaluation has no "
+                            "adjoint pass, so no roofline fraction is quoted for this line"})
     if clean:
         ne = int(desc["seg_n_edge"][0])     # one segment (the library refuses Clean otherwise); edge pixels never take part
         inner = slice(ne, model.P - ne)
@@ -503,6 +526,10 @@ def run_gpu(args):
             oc["config1_clean"] = run_other_config(1, 65536, torch, local, peaks, n_sms, clean=True)
         except Exception as e:
             oc["config1_clean"] = {"error": f"{type(e).__name__}: {e}"}
+        try:
+            oc["config1_lm"] = run_other_config(1, 65536, torch, local, peaks, n_sms, lm=12)
+        except Exception as e:
+            oc["config1_lm"] = {"error": f"{type(e).__name__}: {e}"}
         try:
             oc["config1_paper_stop_clean"] = run_other_config(1, 65536, torch, local, peaks, n_sms, paper_stop=True, clean=True)
         except Exception as e:

@@ -123,6 +123,15 @@ typedef struct {
                                      Needs the resident variant and one segment whose fitted range is one sweep of the
                                      CTA, else LASP_ERR_UNSUPPORTED */
     int32_t clean_max;            /* at most this many mask updates per spectrum (0 = default 11) */
+    int32_t optimizer;            /* 0 (default): Adam, the paper's method (step 8).  1: Levenberg-Marquardt on the
+                                     NP x NP system (the route of LASP-CurveFit, and the
+                                     "curvature awareness" the paper plans; R-13): n_iter LM iterations, each
+                                     the central-difference Jacobian of the re-solved whitened residual (2 NP evaluations),
+                                     (J^T J + lambda diag J^T J) delta = -J^T rho in fp64, u' = clip(u + delta) and one trial
+                                     evaluation; chi2 falls: accept, lambda / 10, else reject, lambda x 10.  lr, beta1, beta2,
+                                     eps are ignored; n_steps reports the accepted steps.  Not together with clean_every or
+                                     stop_window (LASP_ERR_UNSUPPORTED) */
+    float lm_lambda0;             /* initial damping lambda (0 = default 1e-3) */
 } lasp_fit_opts;
 
 /* Build a context on `cuda_device`: validates the description, derives the per-pixel velocity

@@ -41,7 +41,8 @@ class FitOpts(C.Structure):
                 ("eps", C.c_float), ("variant", C.c_int32), ("emulator_path", C.c_int32),
                 ("refresh", C.c_int32), ("warm", C.c_int32), ("fd_fresh", C.c_int32),
                 ("stop_window", C.c_int32), ("stop_tol", C.c_float),
-                ("clean_every", C.c_int32), ("clean_max", C.c_int32)]
+                ("clean_every", C.c_int32), ("clean_max", C.c_int32),
+                ("optimizer", C.c_int32), ("lm_lambda0", C.c_float)]
 
 
 class LaspError(RuntimeError):
@@ -176,9 +177,10 @@ class LaspModel:
 
     @staticmethod
     def _opts(n_iter=0, lr=1e-2, beta1=0.9, beta2=0.999, eps=1e-8, variant=0, emulator_path=0, refresh=0, warm=0,
-              fd_fresh=0, stop_window=0, stop_tol=1e-5, clean_every=0, clean_max=0):
+              fd_fresh=0, stop_window=0, stop_tol=1e-5, clean_every=0, clean_max=0, optimizer=0, lm_lambda0=0.0):
         return FitOpts(int(n_iter), lr, beta1, beta2, eps, int(variant), int(emulator_path), int(refresh), int(warm),
-                       int(fd_fresh), int(stop_window), float(stop_tol), int(clean_every), int(clean_max))
+                       int(fd_fresh), int(stop_window), float(stop_tol), int(clean_every), int(clean_max), int(optimizer),
+                       float(lm_lambda0))
 
     def launch_count(self) -> int:
         return int(lib().lasp_launch_count(self.ctx))
@@ -188,9 +190,9 @@ class LaspModel:
 
     def fit_batch(self, flux, ivar, mask, init, n_iter, lr=1e-2, beta1=0.9, beta2=0.999, eps=1e-8,
                   want_err=True, want_cont=True, out=None, emulator_path=0, variant=0, refresh=0, warm=0, fd_fresh=0,
-                  stop_window=0, stop_tol=1e-5, clean_every=0, clean_max=0):
+                  stop_window=0, stop_tol=1e-5, clean_every=0, clean_max=0, optimizer=0, lm_lambda0=0.0):
         """lasp_fit_batch on device tensors; returns dict of device tensors (`mask_out`: the pixels that took part in
-        the final evaluation; clean_every > 0 turns the Clean strategy on)."""
+        the final evaluation; clean_every > 0 turns the Clean strategy on; optimizer = 1: Levenberg-Marquardt)."""
         t = self.torch
         flux = self._dev(flux, t.float32); ivar = self._dev(ivar, t.float32)
         mask = self._dev(mask, t.uint8); init = self._dev(init, t.float32)
@@ -205,7 +207,7 @@ class LaspModel:
                        cont=t.empty((B, self.nc), device=self.device, dtype=t.float32) if want_cont else None,
                        err=t.empty((B, self.NP), device=self.device, dtype=t.float32) if want_err else None)
         opts = self._opts(n_iter, lr, beta1, beta2, eps, variant, emulator_path, refresh, warm, fd_fresh, stop_window,
-                          stop_tol, clean_every, clean_max)
+                          stop_tol, clean_every, clean_max, optimizer, lm_lambda0)
         rc = lib().lasp_fit_batch(self.ctx, B, _ptr(flux), _ptr(ivar), _ptr(mask), _ptr(init), C.byref(opts),
                                   _ptr(out["params"]), _ptr(out.get("cont")), _ptr(out["chi2"]),
                                   _ptr(out.get("err")), _ptr(out["status"]), _ptr(out.get("n_steps")),
@@ -215,7 +217,8 @@ class LaspModel:
 
     def fit_batch_host(self, flux, ivar, mask, init, n_iter, lr=1e-2, beta1=0.9, beta2=0.999, eps=1e-8,
                        want_err=True, want_cont=True, chunk=0, out=None, emulator_path=0, variant=0, refresh=0, warm=0,
-                       fd_fresh=0, stop_window=0, stop_tol=1e-5, clean_every=0, clean_max=0, want_mask=False):
+                       fd_fresh=0, stop_window=0, stop_tol=1e-5, clean_every=0, clean_max=0, want_mask=False,
+                       optimizer=0, lm_lambda0=0.0):
         """lasp_fit_batch_host on HOST tensors (torch CPU tensors, pinned for overlap); returns host tensors.
         The library cuts the batch into chunks and overlaps the copies with the fits."""
         t = self.torch
@@ -240,7 +243,7 @@ class LaspModel:
                        cont=t.empty((B, self.nc), dtype=t.float32, **pin) if want_cont else None,
                        err=t.empty((B, self.NP), dtype=t.float32, **pin) if want_err else None)
         opts = self._opts(n_iter, lr, beta1, beta2, eps, variant, emulator_path, refresh, warm, fd_fresh, stop_window,
-                          stop_tol, clean_every, clean_max)
+                          stop_tol, clean_every, clean_max, optimizer, lm_lambda0)
         rc = lib().lasp_fit_batch_host(self.ctx, B, _ptr(flux), _ptr(ivar), _ptr(mask), _ptr(init), C.byref(opts),
                                        _ptr(out["params"]), _ptr(out.get("cont")), _ptr(out["chi2"]),
                                        _ptr(out.get("err")), _ptr(out["status"]), _ptr(out.get("n_steps")),

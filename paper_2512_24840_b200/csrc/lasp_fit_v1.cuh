@@ -81,6 +81,7 @@ struct V1Args {
     int *nsteps;           // [B] Adam updates applied per spectrum (may be null)
     // Clean strategy (lasp_fit_opts.clean_every / .clean_max): 0 = No Clean
     int clean_every, clean_max;
+    float lm_lambda0;      // lasp_fit_opts.optimizer = 1 (the LM instantiation of the fit kernel): initial damping
     unsigned char *mask_out;   // [B][P] 1 where the pixel still takes part at the end (may be null)
     unsigned long long *dbg;   // optional per-phase cycle counters (LASP_TIMING=1), else null
     // per-pixel broadening kernels (linear grids, C.2-14): 1/s_j and s_j^2 with V1_TPAD replicated entries on
@@ -179,6 +180,9 @@ struct V1Block {
     // Clean strategy (thread 0)
     int force;            // the next Adam evaluation re-factorises whatever the policy says
     int nclean;           // mask updates done for the current group
+    // Levenberg-Marquardt (lane 0 of warp g)
+    float lm_lambda[GS], lm_chi2[GS];
+    int lm_acc[GS];       // the last trial step was accepted
 };
 __shared__ V1Block v1_blk;
 #define V1_TID ((int)threadIdx.x)
@@ -1891,17 +1895,18 @@ __device__ __forceinline__ void v1_set_group(int grp)
     }
 }
 
-// a9: error estimate (P:173; C.2-22/23).  J by central differences of the re-solved whitened
-// residual rho(u), Sigma = rho^T rho/(N_good - NP) (J^T J)^-1, err_p = sqrt(Sigma_pp) (hi_p - lo_p)/2.
+// Jacobian of the re-solved whitened residual rho(u) by central differences of step fd_h in u (C.2-22):
+// planes 1 .. NP of `xj` receive J_p on the fitted pixels (plane 0 is scratch).  `fresh_first`: the first of the 2 NP
+// evaluations re-factorises whatever the fd_fresh option says (the LM loop calls this after a rejected trial step,
+// when the factor and the warm start belong to another point).
 template <bool STREAM>
-__device__ __noinline__ void v1_errors(float chi2_g, float ngood_g, bool valid_g)
+__device__ __noinline__ void v1_jacobian(float *xj, bool fresh_first)
 {
     const V1Args &a = v1_blk.A;
     const ModelDev &M = v1_blk.M;
     const V1Lay &L = v1_blk.L;
     const int NP = M.NP;
     const size_t plane = (size_t)GS * M.Ppad;
-    float *xj = a.XJ + (size_t)blockIdx.x * (1 + NP) * plane;
     for (int p = 0; p < NP; ++p) {
         float u0 = 0.f;
         if (V1_WARP < GS) {
@@ -1914,7 +1919,7 @@ __device__ __noinline__ void v1_errors(float chi2_g, float ngood_g, bool valid_g
         // The factor of the final evaluation serves all 2 NP perturbed ones: a step of fd_h changes the Gram matrix
         // by a relative ~1e-3, so one refinement from the neighbouring solution leaves that fraction of the
         // continuum's response, far inside the 1e-2 the estimate is held to.
-        v1_evaluate<2, STREAM>(false, a.fdfresh != 0, xj);
+        v1_evaluate<2, STREAM>(false, (a.fdfresh != 0 || (fresh_first && p == 0)) ? 1 : 0, xj);
         if (V1_WARP < GS) {
             if (V1_LANE == 0) SMV(L.oU, p, V1_WARP) = u0 - a.fd_h;
             __syncwarp();
@@ -1944,9 +1949,19 @@ __device__ __noinline__ void v1_errors(float chi2_g, float ngood_g, bool valid_g
         }
         __syncthreads();
     }
-    // N = J^T J (packed lower), fp64 accumulation across warps in shared memory (aliases the factor area)
+}
+
+// N = X^T X (packed lower, N[g * npair + p (p + 1) / 2 + q]) of the first `ncol` columns X_p = plane 1 + p of `xj`, fp64
+// accumulation across warps in shared memory (the factor area: the next evaluation that needs a factor re-factorises).
+// ncol = NP: J^T J;  ncol = NP + 1 with rho(u) in plane 1 + NP: also J^T rho (row NP) and |rho|^2.
+template <bool STREAM>
+__device__ __noinline__ void v1_normal_eq(const float *xj, int ncol)
+{
+    const ModelDev &M = v1_blk.M;
+    const V1Lay &L = v1_blk.L;
+    const size_t plane = (size_t)GS * M.Ppad;
     double *N = (double *)(V1SM + L.oLF);
-    const int npair = NP * (NP + 1) / 2;
+    const int npair = ncol * (ncol + 1) / 2;
     for (int i = V1_TID; i < GS * npair; i += V1_NT) N[i] = 0.0;
     __syncthreads();
     for (int s = 0; s < M.n_seg; ++s) {
@@ -1982,6 +1997,23 @@ __device__ __noinline__ void v1_errors(float chi2_g, float ngood_g, bool valid_g
         }
     }
     __syncthreads();
+}
+
+// a9: error estimate (P:173; C.2-22/23).  J by central differences of the re-solved whitened
+// residual rho(u), Sigma = rho^T rho/(N_good - NP) (J^T J)^-1, err_p = sqrt(Sigma_pp) (hi_p - lo_p)/2.
+template <bool STREAM>
+__device__ __noinline__ void v1_errors(float chi2_g, float ngood_g, bool valid_g)
+{
+    const V1Args &a = v1_blk.A;
+    const ModelDev &M = v1_blk.M;
+    const V1Lay &L = v1_blk.L;
+    const int NP = M.NP;
+    const size_t plane = (size_t)GS * M.Ppad;
+    float *xj = a.XJ + (size_t)blockIdx.x * (2 + NP) * plane;
+    v1_jacobian<STREAM>(xj, false);
+    v1_normal_eq<STREAM>(xj, NP);
+    double *N = (double *)(V1SM + L.oLF);
+    const int npair = NP * (NP + 1) / 2;
     if (V1_WARP < GS && V1_LANE == 0) {
         const int g = V1_WARP;
         double *Ng = N + g * npair;
@@ -2011,6 +2043,99 @@ __device__ __noinline__ void v1_errors(float chi2_g, float ngood_g, bool valid_g
                 e = (float)(sqrt(s2 * nrm) * (double)(M.hi[p] - M.lo[p]) * 0.5);
             }
             if (valid_g) a.err[v1_blk.spec[g] * NP + p] = e;
+        }
+    }
+    __syncthreads();
+}
+
+// ------------------------------------------------------------------------------------------
+// Levenberg-Marquardt on the NP x NP system (reading R-13 of DESIGN.md, as
+// oracle/lasp_oracle.c orc_fit_lm): one iteration = the Jacobian of the re-solved whitened residual (2 NP evaluations),
+// the normal equations in fp64, the damped step (A + lambda diag A) delta = -g by Cholesky on lane 0 of the
+// spectrum's warp, one trial evaluation, and the accept / reject decision per spectrum.
+// Planes of xj: 0 trial residual / scratch, 1 .. NP the Jacobian, 1 + NP the residual at the current iterate.
+// ------------------------------------------------------------------------------------------
+template <bool STREAM>
+__device__ __noinline__ void v1_lm_iteration(float *xj)
+{
+    const V1Args &a = v1_blk.A;
+    const ModelDev &M = v1_blk.M;
+    const V1Lay &L = v1_blk.L;
+    const int NP = M.NP, g = V1_WARP;
+    const size_t plane = (size_t)GS * M.Ppad;
+    v1_jacobian<STREAM>(xj, true);
+    v1_normal_eq<STREAM>(xj, NP + 1);
+    if (g < GS) {
+        if (V1_LANE == 0) {
+            const int npair = (NP + 1) * (NP + 2) / 2;
+            double *Ng = (double *)(V1SM + L.oLF) + g * npair;
+            const double lam = (double)v1_blk.lm_lambda[g];
+            double d[LASP_NPMAX];
+            bool ok = true;
+            for (int p = 0; p < NP; ++p) Ng[p * (p + 1) / 2 + p] *= 1.0 + lam;
+            for (int p = 0; p < NP && ok; ++p)
+                for (int q = 0; q <= p; ++q) {
+                    double s = Ng[p * (p + 1) / 2 + q];
+                    for (int k = 0; k < q; ++k) s -= Ng[p * (p + 1) / 2 + k] * Ng[q * (q + 1) / 2 + k];
+                    if (p == q) {
+                        if (!(s > 0.0)) { ok = false; break; }
+                        Ng[p * (p + 1) / 2 + p] = sqrt(s);
+                    } else
+                        Ng[p * (p + 1) / 2 + q] = s / Ng[q * (q + 1) / 2 + q];
+                }
+            if (ok) {
+                const double *gr = Ng + NP * (NP + 1) / 2;   // row NP: J^T rho
+                for (int p = 0; p < NP; ++p) {               // L z = -g
+                    double s = -gr[p];
+                    for (int k = 0; k < p; ++k) s -= Ng[p * (p + 1) / 2 + k] * d[k];
+                    d[p] = s / Ng[p * (p + 1) / 2 + p];
+                }
+                for (int p = NP - 1; p >= 0; --p) {          // L^T delta = z
+                    double s = d[p];
+                    for (int k = p + 1; k < NP; ++k) s -= Ng[k * (k + 1) / 2 + p] * d[k];
+                    d[p] = s / Ng[p * (p + 1) / 2 + p];
+                }
+            }
+            for (int p = 0; p < NP; ++p) {
+                const float u0 = SMV(L.oU, p, g);
+                SMV(L.oM, p, g) = u0;                        // the Adam moments are not used here: the iterate to fall back to
+                float u = ok ? (float)((double)u0 + d[p]) : u0;
+                u = u < -1.f ? -1.f : (u > 1.f ? 1.f : u);
+                SMV(L.oU, p, g) = u;
+            }
+        }
+        __syncwarp();
+        v1_param_setup(g);
+    }
+    v1_evaluate<2, STREAM>(false, 1, xj);
+    if (g < GS) {
+        float c2t, ngood, cmin;
+        v1_stats(g, c2t, ngood, cmin);
+        const bool acc = c2t < v1_blk.lm_chi2[g];            // NaN: rejected
+        __syncwarp();
+        if (V1_LANE == 0) {
+            v1_blk.lm_acc[g] = acc ? 1 : 0;
+            if (acc) {
+                v1_blk.lm_chi2[g] = c2t;
+                v1_blk.lm_lambda[g] = fmaxf(v1_blk.lm_lambda[g] * 0.1f, 1e-10f);
+                v1_blk.nsteps[g] += 1;
+            } else {
+                v1_blk.lm_lambda[g] = fminf(v1_blk.lm_lambda[g] * 10.f, 1e10f);
+                for (int p = 0; p < NP; ++p) SMV(L.oU, p, g) = SMV(L.oM, p, g);
+            }
+        }
+        __syncwarp();
+        if (!acc) v1_param_setup(g);
+    }
+    __syncthreads();
+    // the accepted trial residuals become the residual at the iterate
+    for (int g2 = 0; g2 < GS; ++g2) {
+        if (!v1_blk.lm_acc[g2]) continue;
+        for (int s = 0; s < M.n_seg; ++s) {
+            const SegDev &sg = M.seg[s];
+            const float4 *src = (const float4 *)(xj + (size_t)g2 * M.Ppad);
+            float4 *dst = (float4 *)(xj + (1 + NP) * plane + (size_t)g2 * M.Ppad);
+            for (int q = (sg.fit_lo >> 2) + V1_TID; q < (sg.fit_hi >> 2); q += V1_NT) dst[q] = src[q];
         }
     }
     __syncthreads();
@@ -2295,9 +2420,10 @@ __device__ __noinline__ bool v1_stop_test(int g, int t)
 // ------------------------------------------------------------------------------------------
 // lasp_fit_batch: a1-a9 for groups of GS spectra, persistent CTAs
 // ------------------------------------------------------------------------------------------
-// CLEAN: the instantiation with the Clean-strategy mask updates in the loop (resident variant only); the default one
-// carries none of that code (the step path is instruction-cache bound, profiles/r02_ncu.md)
-template <int MAXT, int MINB, bool STREAM, bool CLEAN = false>
+// The Clean-strategy mask updates (resident variant only) and the LM loop live in instantiations of their own: the default
+// one carries none of that code (the step path is instruction-cache bound, profiles/r02_ncu.md).
+// OPT 0: Adam;  1: Adam with the Clean-strategy mask updates;  2: Levenberg-Marquardt (n_iter LM iterations)
+template <int MAXT, int MINB, bool STREAM, int OPT = 0>
 __global__ void __launch_bounds__(MAXT, MINB)
 lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V1Lay L, const V1Args a)
 {
@@ -2329,6 +2455,22 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
             v1_blk.force = 0; v1_blk.nclean = 0;
             SMV(L.oSC, SC_PB1, threadIdx.x) = 1.f; SMV(L.oSC, SC_PB2, threadIdx.x) = 1.f;
         }
+        if constexpr (OPT == 2) {
+            float *xj = a.XJ + (size_t)blockIdx.x * (2 + NP) * GS * M.Ppad;
+            v1_evaluate<2, STREAM>(true, 1, xj + (size_t)(1 + NP) * GS * M.Ppad);   // rho at the initial guess
+            if (g < GS) {
+                float c2, ngood, cmin;
+                v1_stats(g, c2, ngood, cmin);
+                if (V1_LANE == 0) { v1_blk.lm_chi2[g] = c2; v1_blk.lm_lambda[g] = a.lm_lambda0; v1_blk.nsteps[g] = 0; }
+            }
+            for (;;) {
+                __syncthreads();
+                if (v1_blk.t >= a.n_iter) break;
+                __syncthreads();
+                if (V1_TID == 0) v1_blk.t += 1;
+                v1_lm_iteration<STREAM>(xj);
+            }
+        } else
         // v1_blk.t was zeroed by v1_set_group; every evaluation below starts with a barrier, after which thread 0 advances
         // it, and ends with one, after which it is read again
         for (;;) {
@@ -2389,7 +2531,7 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
 #ifdef LASP_PHASE_TIMING
             if (a.dbg && V1_TID == 0) atomicAdd(a.dbg + 13, (unsigned long long)(clock64() - tu0));
 #endif
-            if constexpr (CLEAN && !STREAM) {
+            if constexpr (OPT == 1 && !STREAM) {
                 if (a.clean_every > 0) {   // Clean: mask update after update t, t = every, 2 every, ...
                     __syncthreads();
                     if (v1_blk.t % a.clean_every == 0 && v1_blk.nclean < a.clean_max) {
@@ -2408,7 +2550,7 @@ lasp_v1_fit_kernel(const __grid_constant__ ModelDev M, const __grid_constant__ V
         }
         if (a.stats && V1_TID == 0) { atomicAdd(a.stats, (unsigned long long)v1_blk.t); atomicAdd(a.stats + 1, (unsigned long long)v1_blk.nfresh); }
         // a9: one more evaluation at the final iterate (C.2-21)
-        v1_evaluate<1, STREAM>(a.n_iter == 0, 1, nullptr);
+        v1_evaluate<1, STREAM>(OPT != 2 && a.n_iter == 0, 1, nullptr);
         float chi2 = 0.f, ngood = 0.f, cmin = 0.f;
         if (g < GS) {
             v1_stats(g, chi2, ngood, cmin);

@@ -20,8 +20,10 @@ static const double kC_KMS = 299792.458;
 enum { KV_RES192 = 0, KV_RES384 = 1, KV_STREAM = 2, KV_N = 3 };
 static const void *kFit[KV_N] = {(const void *)lasp_v1_fit_kernel<192, 2, false>, (const void *)lasp_v1_fit_kernel<384, 1, false>,
                                  (const void *)lasp_v1_fit_kernel<192, 2, true>};
-static const void *kFitClean[KV_N] = {(const void *)lasp_v1_fit_kernel<192, 2, false, true>,
-                                        (const void *)lasp_v1_fit_kernel<384, 1, false, true>, nullptr};
+static const void *kFitClean[KV_N] = {(const void *)lasp_v1_fit_kernel<192, 2, false, 1>,
+                                        (const void *)lasp_v1_fit_kernel<384, 1, false, 1>, nullptr};
+static const void *kFitLM[KV_N] = {(const void *)lasp_v1_fit_kernel<192, 2, false, 2>, (const void *)lasp_v1_fit_kernel<384, 1, false, 2>,
+                                     (const void *)lasp_v1_fit_kernel<384, 1, true, 2>};
 static const void *kGrad[KV_N] = {(const void *)lasp_v1_grad_kernel<192, 2, false>, (const void *)lasp_v1_grad_kernel<384, 1, false>,
                                   (const void *)lasp_v1_grad_kernel<192, 2, true>};
 static const void *kModel[KV_N] = {(const void *)lasp_v1_model_kernel<192, 2, false>, (const void *)lasp_v1_model_kernel<384, 1, false>,
@@ -442,7 +444,7 @@ static void setup_variant(lasp_ctx *c, const cudaDeviceProp &prop, int emax, boo
         if (bytes + 2048 <= prop.sharedMemPerBlockOptin) break;   // + the kernels' static block state
     }
     if (L.lfseg < 0) return;
-    const void *fs[4] = {kFit[v.kv], kGrad[v.kv], kModel[v.kv], kFitClean[v.kv]};
+    const void *fs[5] = {kFit[v.kv], kGrad[v.kv], kModel[v.kv], kFitClean[v.kv], kFitLM[v.kv]};
     for (const void *f : fs)
         if (f && cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess) { cudaGetLastError(); return; }
     int per_sm = 0;
@@ -457,7 +459,7 @@ static void setup_variant(lasp_ctx *c, const cudaDeviceProp &prop, int emax, boo
 // ------------------------------------------------------------------------------------------
 // options, workspace, launches
 // ------------------------------------------------------------------------------------------
-static const lasp_fit_opts kDefaultOpts = {0, 1e-2f, 0.9f, 0.999f, 1e-8f, 0, 0, 0, 0, 0, 0, 0.f, 0, 0};
+static const lasp_fit_opts kDefaultOpts = {0, 1e-2f, 0.9f, 0.999f, 1e-8f, 0, 0, 0, 0, 0, 0, 0.f, 0, 0, 0, 0.f};
 
 // variant / emulator path of one call (opts may be null: defaults)
 static int resolve(lasp_ctx *c, const lasp_fit_opts *o, const char *who, const Variant **v, bool *mma)
@@ -472,6 +474,8 @@ static int resolve(lasp_ctx *c, const lasp_fit_opts *o, const char *who, const V
         return fail(c, LASP_ERR_INVALID_ARG, std::string(who) + ": stop_window must be in [0, 128] and stop_tol >= 0");
     if (o->clean_every < 0 || o->clean_max < 0)
         return fail(c, LASP_ERR_INVALID_ARG, std::string(who) + ": clean_every and clean_max must be >= 0");
+    if (o->optimizer < 0 || o->optimizer > 1 || !(o->lm_lambda0 >= 0.f))
+        return fail(c, LASP_ERR_INVALID_ARG, std::string(who) + ": optimizer must be 0 (Adam) or 1 (Levenberg-Marquardt), lm_lambda0 >= 0");
     const Variant *vv = nullptr;
     if (o->variant == 1) vv = c->res.ok ? &c->res : nullptr;
     else if (o->variant == 2) vv = c->str.ok ? &c->str : nullptr;
@@ -509,7 +513,7 @@ static int workspace(lasp_ctx *c, int64_t B, const Variant &v, bool need_planes,
     }
     if (need_xj && ctas > c->xj_ctas) {
         cudaFree(c->dXJ); c->dXJ = nullptr; c->xj_ctas = 0;
-        CUDA_TRY(c, cudaMalloc(&c->dXJ, ctas * (size_t)(1 + M.NP) * GS * M.Ppad * sizeof(float)));
+        CUDA_TRY(c, cudaMalloc(&c->dXJ, ctas * (size_t)(2 + M.NP) * GS * M.Ppad * sizeof(float)));
         c->xj_ctas = ctas;
     }
     if (&v == &c->str && ctas > c->tg_ctas) {
@@ -609,7 +613,8 @@ extern "C" int lasp_fit_batch(lasp_ctx *c, int64_t B, const float *flux, const f
     if (!c) return fail(nullptr, LASP_ERR_INVALID_ARG, "null ctx");
     if (B < 1 || !flux || !ivar || !init || !opts || !params || !chi2)
         return fail(c, LASP_ERR_INVALID_ARG, "lasp_fit_batch: null pointer or B < 1");
-    if (opts->n_iter < 0 || !(opts->lr > 0.f) || !(opts->beta1 >= 0.f && opts->beta1 < 1.f) ||
+    const bool lm = opts->optimizer == 1;
+    if (opts->n_iter < 0 || (!lm && !(opts->lr > 0.f)) || !(opts->beta1 >= 0.f && opts->beta1 < 1.f) ||
         !(opts->beta2 >= 0.f && opts->beta2 < 1.f) || !(opts->eps >= 0.f))
         return fail(c, LASP_ERR_INVALID_ARG, "lasp_fit_batch: bad Adam hyper-parameters");
     if (B > (int64_t)1 << 30) return fail(c, LASP_ERR_UNSUPPORTED, "B too large");
@@ -624,8 +629,11 @@ extern "C" int lasp_fit_batch(lasp_ctx *c, int64_t B, const float *flux, const f
             return fail(c, LASP_ERR_UNSUPPORTED, "lasp_fit_batch: the Clean strategy needs the resident variant and one segment "
                                                  "whose fitted range is one sweep of the CTA");
     }
+    if (lm && (opts->clean_every > 0 || opts->stop_window > 0))
+        return fail(c, LASP_ERR_UNSUPPORTED, "lasp_fit_batch: the Levenberg-Marquardt optimiser runs n_iter iterations without the "
+                                             "Clean strategy or the stopping rules");
     DeviceGuard dg(c->device);
-    rc = workspace(c, B, *v, true, true, err != nullptr);
+    rc = workspace(c, B, *v, true, true, err != nullptr || lm);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     rc = ws_acquire(c, st);
@@ -645,6 +653,7 @@ extern "C" int lasp_fit_batch(lasp_ctx *c, int64_t B, const float *flux, const f
     a.stop_window = opts->stop_window; a.stop_tol = opts->stop_tol; a.nsteps = n_steps;
     a.clean_every = opts->clean_every; a.clean_max = opts->clean_max > 0 ? opts->clean_max : 11;
     a.mask_out = mask_out;
+    a.lm_lambda0 = opts->lm_lambda0 > 0.f ? opts->lm_lambda0 : 1e-3f;
     CUDA_TRY(c, cudaMemsetAsync(c->dqueue, 0, sizeof(unsigned int), st));
     CUDA_TRY(c, cudaMemsetAsync(c->dstats, 0, 2 * sizeof(unsigned long long), st));
     a.queue = c->dqueue;
@@ -654,7 +663,7 @@ extern "C" int lasp_fit_batch(lasp_ctx *c, int64_t B, const float *flux, const f
     CUDA_TRY(c, cudaMemsetAsync(c->ddbg, 0, 24 * sizeof(unsigned long long), st));
     a.dbg = c->ddbg;
 #endif
-    return launch(c, opts->clean_every > 0 ? kFitClean : kFit, *v, a, st);
+    return launch(c, lm ? kFitLM : (opts->clean_every > 0 ? kFitClean : kFit), *v, a, st);
 }
 
 extern "C" int lasp_eval_grad(lasp_ctx *c, int64_t B, const float *flux, const float *ivar,
