@@ -19,6 +19,7 @@
  *   Adam                step 8  P:169              orc_adam_step
  *   stopping rules      step 8  P:169-171          orc_stop_rule, orc_fit_stop
  *   Clean masking       step 6  P:137-161, P:171   orc_clean_update, orc_fit_clean
+ *   resampler           step 3  Eq. 2-4, P:78-109  orc_obs_nodes, orc_resample, orc_resample_coeffs
  *   LM optimiser        NEXT-4  P:54-58, P:397     orc_fit_lm (Marquardt's method written out; R-13)
  *   error estimate      step 9  P:173              errors_one
  *
@@ -926,6 +927,55 @@ int orc_fit_lm(const orc_model *m, int64_t B, const double *flux, const double *
         work_free(k);
     }
     return 0;
+}
+
+/* ------------------------------------------------------- flux-conserving resampler (step 3, Eq. 2-4; NEXT-3)
+ *
+ * The model spectrum T_1..T_q lives on a linear grid lam1 + (m-1) dlam1; its integration nodes are lam1 + (m - 1/2) dlam1,
+ * m = 0..q.  Eq. 2: the cumulative integral 0, T_1 dlam1, ..., sum T_i dlam1 on those nodes; Eq. 3: linear
+ * interpolation of it onto the observed integration nodes; Eq. 4: T'_i = (F(node_(i+1)) - F(node_i)) / (node_(i+1) - node_i).
+ * Reading R-14: outside the model's nodes the integrated flux is held at its end values (the clamp of the
+ * usual interp routines), i.e. the model carries no flux there.  orc_obs_nodes: the observed integration nodes of P:92,
+ * lambda'' = exp(lambda_2i -+ dlambda_2 / 2) in the base the grid is stored in (log10 here): per segment, nodes at the
+ * midpoints in log-wavelength of neighbouring pixels and half a step beyond the first and the last pixel -- on a uniform
+ * log grid exactly the paper's. */
+void orc_obs_nodes(const double *loglam, int p, double *nodes)
+{
+    if (p == 1) { nodes[0] = pow(10.0, loglam[0] - 0.5e-4); nodes[1] = pow(10.0, loglam[0] + 0.5e-4); return; }
+    nodes[0] = pow(10.0, loglam[0] - 0.5 * (loglam[1] - loglam[0]));
+    for (int i = 1; i < p; ++i) nodes[i] = pow(10.0, 0.5 * (loglam[i - 1] + loglam[i]));
+    nodes[p] = pow(10.0, loglam[p - 1] + 0.5 * (loglam[p - 1] - loglam[p - 2]));
+}
+
+void orc_resample(int q, double lam1, double dlam1, const double *T, int p, const double *nodes, double *out)
+{
+    double *cum = calloc((size_t)q + 1, 8), *F = calloc((size_t)p + 1, 8);
+    for (int m = 1; m <= q; ++m) cum[m] = cum[m - 1] + T[m - 1] * dlam1;             /* Eq. 2 */
+    for (int i = 0; i <= p; ++i) {                                                   /* Eq. 3 */
+        double t = (nodes[i] - (lam1 - 0.5 * dlam1)) / dlam1;                        /* position in units of model nodes */
+        if (t <= 0.0) F[i] = cum[0];
+        else if (t >= (double)q) F[i] = cum[q];
+        else {
+            int m = (int)floor(t);
+            F[i] = cum[m] + (cum[m + 1] - cum[m]) * (t - (double)m);
+        }
+    }
+    for (int i = 0; i < p; ++i) out[i] = (F[i + 1] - F[i]) / (nodes[i + 1] - nodes[i]);   /* Eq. 4 */
+    free(cum); free(F);
+}
+
+/* The resampler applied to every row of a coefficient table [K][q] -> [K][n_pix] (Delta-4: it is linear and does not
+ * depend on the parameters, so resampling the coefficients once equals resampling every model spectrum). */
+void orc_resample_coeffs(int K, int q, double lam1, double dlam1, const double *coef, int n_pix, int n_seg,
+                         const int32_t *seg_offset, const double *loglam, double *out)
+{
+    double *nodes = calloc((size_t)n_pix + 1, 8);
+    for (int s = 0; s < n_seg; ++s) {
+        int o = seg_offset[s], ps = seg_offset[s + 1] - o;
+        orc_obs_nodes(loglam + o, ps, nodes);
+        for (int k = 0; k < K; ++k) orc_resample(q, lam1, dlam1, coef + (size_t)k * q, ps, nodes, out + (size_t)k * n_pix + o);
+    }
+    free(nodes);
 }
 
 /* Pins call these two directly. */

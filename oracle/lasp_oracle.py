@@ -252,6 +252,34 @@ class Oracle:
         return dict(params=params, cont=cont, chi2=chi2, err=err, status=status, n_steps=n_steps, trace=trace)
 
 
+def obs_nodes(loglam):
+    """Observed integration nodes of P:92 for one segment (orc_obs_nodes)."""
+    ll = np.ascontiguousarray(loglam, dtype=np.float64)
+    out = np.empty(ll.size + 1)
+    lib().orc_obs_nodes(_p(ll, _f64p), C.c_int(ll.size), _p(out, _f64p))
+    return out
+
+
+def resample(T, lam1, dlam1, nodes):
+    """Flux-conserving resampling of one model spectrum (Eq. 2-4; orc_resample)."""
+    T = np.ascontiguousarray(T, dtype=np.float64); nodes = np.ascontiguousarray(nodes, dtype=np.float64)
+    out = np.empty(nodes.size - 1)
+    lib().orc_resample(C.c_int(T.size), C.c_double(lam1), C.c_double(dlam1), _p(T, _f64p), C.c_int(out.size),
+                       _p(nodes, _f64p), _p(out, _f64p))
+    return out
+
+
+def resample_coeffs(coef, lam1, dlam1, seg_offset, loglam):
+    """Every row of a [K, q] coefficient table onto the observed grid (orc_resample_coeffs)."""
+    coef = np.ascontiguousarray(coef, dtype=np.float64)
+    seg = np.ascontiguousarray(seg_offset, dtype=np.int32); ll = np.ascontiguousarray(loglam, dtype=np.float64)
+    out = np.empty((coef.shape[0], ll.size))
+    lib().orc_resample_coeffs(C.c_int(coef.shape[0]), C.c_int(coef.shape[1]), C.c_double(lam1), C.c_double(dlam1),
+                              _p(coef, _f64p), C.c_int(ll.size), C.c_int(seg.size - 1), _p(seg, _i32p), _p(ll, _f64p),
+                              _p(out, _f64p))
+    return out
+
+
 def stop_rule(L, window=50, tol=1e-5):
     """First step t (1-based) at which criterion (2) or (3) of P:169-171 fires on the loss sequence L, and the rule
     (1 = neither within the sequence, then t = 0)."""

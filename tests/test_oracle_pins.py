@@ -822,3 +822,68 @@ def _not_edge(case):
         keep[:, a:a + ne] = False
         keep[:, b - ne:b] = False
     return keep
+
+
+# ------------------------------------------------------------------------------------------------
+# Flux-conserving resampler (step 3, Eq. 2-4): orc_obs_nodes, orc_resample
+# ------------------------------------------------------------------------------------------------
+ELODIE_LAM1, ELODIE_DLAM, ELODIE_Q = 3900.0, 0.2, 14501      # 3900-6800 A, 14,501 flux points
+
+
+def test_resampler_nodes_are_the_papers(oracle_mod):
+    """lambda''_i = exp(lambda_21 + (2i - 3) dlambda_2 / 2): on the LAMOST grid (log10 step 1e-4, 4200-5700 A, the
+    1327 pixels of P:227) p + 1 nodes, each pixel centre the geometric mean of its two nodes, node ratio 10^1e-4."""
+    ll = synth.loglam_grid("log10", 4200.0, 5700.0, 1e-4)
+    assert ll.size == 1327
+    n = oracle_mod.obs_nodes(ll)
+    assert n.size == 1328
+    assert np.allclose(np.sqrt(n[:-1] * n[1:]), 10.0 ** ll, rtol=1e-14)
+    assert np.allclose(n[1:] / n[:-1], 10.0 ** 1e-4, rtol=1e-12)
+    assert np.isclose(n[0], np.exp(np.log(4200.0) - 0.5 * 1e-4 * np.log(10.0)), rtol=1e-14)
+
+
+def test_resampler_conserves_flux_and_reproduces_constants(oracle_mod):
+    """Closed forms: a constant spectrum stays that constant; the integral over the observed bins equals the integral of
+    the model over the same wavelength range (flux conservation, Carnall 2017); observed nodes equal to the model's nodes
+    give the model back; merging aligned pairs of model pixels gives their means; and bins beyond the model's range
+    receive only the flux inside it (R-14)."""
+    rng = np.random.default_rng(3)
+    T = 1.0 + 0.3 * rng.standard_normal(ELODIE_Q)
+    nodes = oracle_mod.obs_nodes(synth.loglam_grid("log10", 4200.0, 5700.0, 1e-4))
+    assert np.allclose(oracle_mod.resample(np.full(ELODIE_Q, 2.5), ELODIE_LAM1, ELODIE_DLAM, nodes), 2.5, rtol=1e-12)
+    out = oracle_mod.resample(T, ELODIE_LAM1, ELODIE_DLAM, nodes)
+    # brute force: the piecewise-constant model integrated over [nodes[0], nodes[-1]]
+    edges = ELODIE_LAM1 + (np.arange(ELODIE_Q + 1) - 0.5) * ELODIE_DLAM
+    ov = np.clip(np.minimum(edges[1:], nodes[-1]) - np.maximum(edges[:-1], nodes[0]), 0.0, None)
+    assert np.isclose((out * np.diff(nodes)).sum(), (T * ov).sum(), rtol=1e-12)
+    # every bin, brute force by overlaps
+    for i in (0, 1, 500, 1326):
+        o = np.clip(np.minimum(edges[1:], nodes[i + 1]) - np.maximum(edges[:-1], nodes[i]), 0.0, None)
+        assert np.isclose(out[i], (T * o).sum() / (nodes[i + 1] - nodes[i]), rtol=1e-11)
+    assert np.allclose(oracle_mod.resample(T, ELODIE_LAM1, ELODIE_DLAM, edges), T, rtol=1e-11)
+    assert np.allclose(oracle_mod.resample(T[:1000], ELODIE_LAM1, ELODIE_DLAM, edges[:1001:2]),
+                       0.5 * (T[0:1000:2] + T[1:1000:2]), rtol=1e-11)
+    beyond = np.array([edges[0] - 1.0, edges[0] + 0.1, edges[0] + 0.3])
+    got = oracle_mod.resample(T, ELODIE_LAM1, ELODIE_DLAM, beyond)
+    assert np.isclose(got[0], T[0] * 0.1 / 1.1, rtol=1e-12) and np.isclose(got[1], (0.1 * T[0] + 0.1 * T[1]) / 0.2, rtol=1e-11)
+
+
+def test_resampler_is_numpy_cumsum_interp_and_linear(oracle_mod):
+    """The library-routine form of Eq. 2-4 (numpy cumsum + interp + diff), and Delta-4: resampling is linear, so
+    resample(phi . C) = phi . resample(C) -- what lets the coefficient table be resampled once."""
+    rng = np.random.default_rng(4)
+    C_ = rng.standard_normal((5, ELODIE_Q))
+    ll = synth.loglam_grid("log10", 4200.0, 5700.0, 1e-4)
+    nodes = oracle_mod.obs_nodes(ll)
+    edges = ELODIE_LAM1 + (np.arange(ELODIE_Q + 1) - 0.5) * ELODIE_DLAM
+    for k in range(2):
+        cum = np.concatenate([[0.0], np.cumsum(C_[k] * ELODIE_DLAM)])
+        ref = np.diff(np.interp(nodes, edges, cum)) / np.diff(nodes)
+        assert np.allclose(oracle_mod.resample(C_[k], ELODIE_LAM1, ELODIE_DLAM, nodes), ref, rtol=1e-9, atol=1e-12)
+    phi = rng.standard_normal(5)
+    R = oracle_mod.resample_coeffs(C_, ELODIE_LAM1, ELODIE_DLAM, [0, ll.size], ll)
+    assert np.allclose(oracle_mod.resample(phi @ C_, ELODIE_LAM1, ELODIE_DLAM, nodes), phi @ R, rtol=1e-9, atol=1e-12)
+    # two segments are resampled independently, each with its own end nodes
+    R2 = oracle_mod.resample_coeffs(C_, ELODIE_LAM1, ELODIE_DLAM, [0, 700, ll.size], ll)
+    assert np.allclose(R2[:, :699], R[:, :699], rtol=1e-12) and np.allclose(R2[:, 701:], R[:, 701:], rtol=1e-12)
+    assert np.allclose(R2[:, 699:701], R[:, 699:701], rtol=1e-9)          # uniform log grid: the same nodes either way
