@@ -206,6 +206,20 @@ double lasp_fma_executed_per_spectrum_step(const lasp_ctx *ctx, double mean_taps
  * loops (groups of 4 spectra x n_iter), out2[1] = those that re-factorised the continuum Gram matrix. */
 int lasp_last_fit_stats(lasp_ctx *ctx, double *out2);
 
+/* Flux-conserving resampling (step 3 of the paper, Eq. 2-4) of an emulator coefficient
+ * table from the model's linear wavelength grid onto an observed grid, once, ahead of lasp_create (the operation is linear
+ * and independent of the stellar parameters, so resampling the coefficients equals resampling every model spectrum).
+ *   coef_model [n_terms*q] f32, DEVICE: row k on the grid lam1 + m dlam1 (Angstrom), m = 0..q-1 (ELODIE: 3900 A, 0.2 A,
+ *   q = 14,501); loglam [n_pix] f64 and seg_offset [n_seg+1] i32, HOST: the observed grid as in lasp_model_desc;
+ *   coef_obs [n_terms*n_pix] f32, DEVICE: the result, ready for lasp_model_desc.coeffs (after a copy to the host).
+ * Observed integration nodes: per segment the midpoints in log-wavelength between neighbouring pixels and half a
+ * step beyond the first and last pixel (on a uniform log grid exactly the paper's exp(lambda -+ dlambda/2)).  Bins beyond
+ * the model's range receive only the flux inside it (R-14).  Runs on `stream` of `cuda_device` and BLOCKS until
+ * done; no ctx is needed; errors are reported through lasp_last_error(NULL). */
+int lasp_resample_coeffs(int cuda_device, int32_t n_terms, int32_t q, double lam1, double dlam1,
+                         const float *coef_model, int32_t n_pix, int32_t n_seg, const int32_t *seg_offset,
+                         const double *loglam, float *coef_obs, void *stream);
+
 const char *lasp_last_error(const lasp_ctx *ctx); /* ctx-owned string; "" if none; ctx may be NULL */
 int lasp_version(void);
 

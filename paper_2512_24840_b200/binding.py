@@ -15,7 +15,8 @@ LIB_PATH = os.path.join(_HERE, "liblasp_gpu.so")
 
 SYMBOLS = ["lasp_create", "lasp_destroy", "lasp_reserve", "lasp_fit_batch", "lasp_fit_batch_host", "lasp_eval_model",
            "lasp_eval_grad", "lasp_kernel_variant", "lasp_launch_info", "lasp_launch_count", "lasp_fma_per_spectrum_step",
-           "lasp_fma_executed_per_spectrum_step", "lasp_last_fit_stats", "lasp_last_error", "lasp_version"]
+           "lasp_fma_executed_per_spectrum_step", "lasp_last_fit_stats", "lasp_resample_coeffs", "lasp_last_error",
+           "lasp_version"]
 
 LASP_ST_NOT_SPD, LASP_ST_NONFINITE, LASP_ST_NEG_CONT, LASP_ST_ON_BOUND, LASP_ST_STOP_TOL, LASP_ST_STOP_RISE = 1, 2, 4, 8, 16, 32
 
@@ -70,6 +71,8 @@ def lib():
                                          [C.c_void_p] * 7 + [C.c_int64]
         L.lasp_eval_model.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 2 + [C.POINTER(FitOpts)] + [C.c_void_p] * 2
         L.lasp_eval_grad.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 4 + [C.POINTER(FitOpts)] + [C.c_void_p] * 5
+        L.lasp_resample_coeffs.argtypes = [C.c_int, C.c_int32, C.c_int32, C.c_double, C.c_double, C.c_void_p, C.c_int32,
+                                           C.c_int32, _i32p, _f64p, C.c_void_p, C.c_void_p]
         L.lasp_kernel_variant.argtypes = [C.c_void_p]
         L.lasp_kernel_variant.restype = C.c_int
         L.lasp_launch_info.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int32)]
@@ -93,6 +96,28 @@ def _p(a, t):
 
 def _ptr(t):
     return C.c_void_p(t.data_ptr()) if t is not None else None
+
+
+def resample_coeffs(coef_model, lam1, dlam1, seg_offset, loglam, device: int = 0):
+    """lasp_resample_coeffs: a [K, q] coefficient table (device tensor or numpy array) on the model's linear grid
+    lam1 + m dlam1 -> a [K, n_pix] float32 device tensor on the observed grid (Eq. 2-4 of the paper)."""
+    import torch
+    if not torch.cuda.is_available():
+        raise LaspError("no CUDA device: the LASP path runs only in its sm_100a kernels")
+    dev = torch.device("cuda", device)
+    if not isinstance(coef_model, torch.Tensor):
+        coef_model = torch.from_numpy(np.ascontiguousarray(coef_model, dtype=np.float32))
+    coef_model = coef_model.to(dev, torch.float32).contiguous()
+    seg = np.ascontiguousarray(seg_offset, dtype=np.int32)
+    ll = np.ascontiguousarray(loglam, dtype=np.float64)
+    K, q = coef_model.shape
+    out = torch.empty((K, ll.size), device=dev, dtype=torch.float32)
+    st = C.c_void_p(torch.cuda.current_stream(dev).cuda_stream)
+    rc = lib().lasp_resample_coeffs(device, K, q, float(lam1), float(dlam1), _ptr(coef_model), ll.size, seg.size - 1,
+                                    _p(seg, _i32p), _p(ll, _f64p), _ptr(out), st)
+    if rc != 0:
+        raise LaspError(f"lasp_resample_coeffs failed ({rc}): {lib().lasp_last_error(None).decode()}")
+    return out
 
 
 class LaspModel:

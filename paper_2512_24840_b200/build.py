@@ -8,7 +8,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblasp_gpu.so")
 SOURCES = ["lasp_gpu.cu"]
-DEPS = ["lasp_gpu.cu", "lasp_fit_v1.cuh", "lasp_common.cuh", os.path.join("..", "..", "include", "lasp_gpu.h")]
+DEPS = ["lasp_gpu.cu", "lasp_fit_v1.cuh", "lasp_common.cuh", "lasp_resample.cuh", os.path.join("..", "..", "include", "lasp_gpu.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC"]
 

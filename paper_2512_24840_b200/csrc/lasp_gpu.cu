@@ -11,6 +11,7 @@
 #include <vector>
 
 #include "lasp_fit_v1.cuh"
+#include "lasp_resample.cuh"
 
 #define LASP_VERSION 200
 static const double kC_KMS = 299792.458;
@@ -752,6 +753,53 @@ extern "C" int lasp_last_fit_stats(lasp_ctx *c, double *out2)
     CUDA_TRY(c, cudaMemcpy(h, c->dstats, sizeof(h), cudaMemcpyDeviceToHost));
     out2[0] = (double)h[0]; out2[1] = (double)h[1];
     return LASP_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// lasp_resample_coeffs: the flux-conserving resampler (Eq. 2-4) applied once to a coefficient table
+// ------------------------------------------------------------------------------------------
+extern "C" int lasp_resample_coeffs(int cuda_device, int32_t n_terms, int32_t q, double lam1, double dlam1,
+                                    const float *coef_model, int32_t n_pix, int32_t n_seg, const int32_t *seg_offset,
+                                    const double *loglam, float *coef_obs, void *stream)
+{
+    if (n_terms < 1 || q < 1 || !(dlam1 > 0.0) || !coef_model || n_pix < 1 || n_seg < 1 || !seg_offset || !loglam || !coef_obs)
+        return fail(nullptr, LASP_ERR_INVALID_ARG, "lasp_resample_coeffs: null pointer or bad size");
+    if (seg_offset[0] != 0 || seg_offset[n_seg] != n_pix)
+        return fail(nullptr, LASP_ERR_INVALID_ARG, "lasp_resample_coeffs: seg_offset must run from 0 to n_pix");
+    // observed integration nodes: per segment, midpoints in log-wavelength between neighbouring pixels and half a
+    // step beyond the first and the last pixel; lo[i], hi[i] are the two nodes of pixel i
+    std::vector<double> nodes(2 * (size_t)n_pix);
+    double *lo = nodes.data(), *hi = nodes.data() + n_pix;
+    for (int s = 0; s < n_seg; ++s) {
+        const int o = seg_offset[s], e = seg_offset[s + 1];
+        if (e <= o) return fail(nullptr, LASP_ERR_INVALID_ARG, "lasp_resample_coeffs: empty segment");
+        for (int j = o; j < e; ++j) {
+            const double left = j > o ? 0.5 * (loglam[j - 1] + loglam[j])
+                                      : loglam[j] - 0.5 * (e - o > 1 ? loglam[j + 1] - loglam[j] : 1e-4);
+            const double right = j + 1 < e ? 0.5 * (loglam[j] + loglam[j + 1])
+                                           : loglam[j] + 0.5 * (e - o > 1 ? loglam[j] - loglam[j - 1] : 1e-4);
+            if (!(right > left)) return fail(nullptr, LASP_ERR_INVALID_ARG, "lasp_resample_coeffs: loglam must increase within a segment");
+            lo[j] = pow(10.0, left); hi[j] = pow(10.0, right);
+        }
+    }
+    int prev_dev = -1;
+    cudaGetDevice(&prev_dev);
+    if (cudaSetDevice(cuda_device) != cudaSuccess) { cudaGetLastError(); return fail(nullptr, LASP_ERR_CUDA, "lasp_resample_coeffs: cudaSetDevice failed"); }
+    cudaStream_t st = (cudaStream_t)stream;
+    double *dn = nullptr;
+    int rc = LASP_OK;
+    cudaError_t e = cudaMalloc(&dn, nodes.size() * sizeof(double));
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dn, nodes.data(), nodes.size() * sizeof(double), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) {
+        const dim3 grid((n_pix + 127) / 128, n_terms);
+        lasp_resample_kernel<<<grid, 128, 0, st>>>(q, lam1 - 0.5 * dlam1, dlam1, coef_model, n_pix, dn, dn + n_pix, coef_obs);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);   // the node table is freed below: a one-off precompute, blocking
+    if (e != cudaSuccess) rc = fail(nullptr, LASP_ERR_CUDA, std::string("lasp_resample_coeffs: ") + cudaGetErrorString(e));
+    cudaFree(dn);
+    if (prev_dev >= 0) cudaSetDevice(prev_dev);
+    return rc;
 }
 
 // ------------------------------------------------------------------------------------------

@@ -796,3 +796,58 @@ def test_lm_zero_iterations_and_unsupported(gpu, oracle_mod):
     with pytest.raises(gpu.LaspError):
         m.fit_batch(*args, 3, optimizer=2)
     m.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# Flux-conserving resampler (step 3, Eq. 2-4), against orc_resample_coeffs
+# ------------------------------------------------------------------------------------------------
+def _elodie_like_table(K, seed):
+    """A [K, 14501] coefficient table on the ELODIE grid (3900-6800 A, 0.2 A): smooth rows with narrow lines."""
+    rng = np.random.default_rng(seed)
+    q = 14501
+    lam = 3900.0 + 0.2 * np.arange(q)
+    C_ = np.empty((K, q))
+    for k in range(K):
+        base = rng.normal() * np.sin(lam / rng.uniform(40.0, 400.0) + rng.uniform(0, 6.28))
+        lines = np.zeros(q)
+        for c0 in rng.uniform(3900.0, 6800.0, 60):
+            lines -= rng.uniform(0.05, 0.6) * np.exp(-0.5 * ((lam - c0) / rng.uniform(0.15, 0.8)) ** 2)
+        C_[k] = (1.0 if k == 0 else 0.0) + 0.2 * base + lines
+    return C_.astype(np.float32)
+
+
+def test_resample_coeffs_lamost_grid(gpu, oracle_mod):
+    """26 terms x 14,501 model pixels onto the 1327-pixel LAMOST grid of P:227 (4200-5700 A, log10 step 1e-4): every
+    element within 1e-6 of the scale of its row (float output of an fp64 sum), flux conserved."""
+    C_ = _elodie_like_table(26, 11)
+    ll = synth.loglam_grid("log10", 4200.0, 5700.0, 1e-4)
+    got = gpu.resample_coeffs(C_, 3900.0, 0.2, [0, ll.size], ll).cpu().numpy().astype(np.float64)
+    ref = oracle_mod.resample_coeffs(C_.astype(np.float64), 3900.0, 0.2, [0, ll.size], ll)
+    assert got.shape == ref.shape == (26, 1327)
+    scale = np.abs(ref).max(axis=1, keepdims=True)
+    assert (np.abs(got - ref) / scale).max() <= 1e-6
+    nodes = oracle_mod.obs_nodes(ll)
+    assert np.allclose((got * np.diff(nodes)).sum(axis=1), (ref * np.diff(nodes)).sum(axis=1), rtol=1e-6, atol=1e-4)
+
+
+def test_resample_coeffs_segments_ragged_and_out_of_range(gpu, oracle_mod):
+    """Three linear-grid arms (DESI-like, 0.8 A) reaching beyond both ends of the model grid, a one-pixel segment, a
+    non-multiple-of-128 pixel count, and bins narrower than a model pixel (upsampling): all as the oracle; bins wholly
+    outside the model carry zero."""
+    C_ = _elodie_like_table(7, 12)
+    lam = 3600.0 + 0.8 * np.arange(4200)                       # 3600 .. 6959 A: both ends beyond 3900-6800
+    ll = np.log10(lam)
+    seg = [0, 1500, 1501, 4200]
+    got = gpu.resample_coeffs(C_, 3900.0, 0.2, seg, ll).cpu().numpy().astype(np.float64)
+    ref = oracle_mod.resample_coeffs(C_.astype(np.float64), 3900.0, 0.2, seg, ll)
+    scale = np.abs(ref).max(axis=1, keepdims=True)
+    assert (np.abs(got - ref) / scale).max() <= 1e-6
+    assert np.all(got[:, lam < 3899.0] == 0.0) and np.all(got[:, lam > 6801.0] == 0.0)
+    fine = np.log10(4500.0 + 0.05 * np.arange(777))            # 0.05 A bins inside 0.2 A model pixels
+    got = gpu.resample_coeffs(C_, 3900.0, 0.2, [0, 777], fine).cpu().numpy().astype(np.float64)
+    ref = oracle_mod.resample_coeffs(C_.astype(np.float64), 3900.0, 0.2, [0, 777], fine)
+    assert (np.abs(got - ref) / np.abs(ref).max(axis=1, keepdims=True)).max() <= 1e-6
+    with pytest.raises(gpu.LaspError):
+        gpu.resample_coeffs(C_, 3900.0, 0.0, [0, 777], fine)
+    with pytest.raises(gpu.LaspError):
+        gpu.resample_coeffs(C_, 3900.0, 0.2, [0, 700], fine)
