@@ -52,6 +52,12 @@ typedef struct {
     const double *emu_a, *emu_b;  /* [L] */
     int32_t cont_degree;          /* D */
     const int32_t *seg_n_edge;    /* [n_seg] */
+    /* piecewise emulator (Eq. 1's f_1..f_5; NEXT-3): n_models polynomial models share the term table,
+     * term k belongs to model term_model[k]; model r has weight omega_r(theta_0) (orc_blend_weight).  n_models <= 1:
+     * one polynomial (Delta-5), the two pointers are not read. */
+    int32_t n_models;
+    const uint8_t *term_model;    /* [K] */
+    const double *model_blend;    /* [n_models*4]: lo0, lo1, hi0, hi1 in the units of label 0 */
 } orc_model;
 
 /* ------------------------------------------------------------------ grid */
@@ -106,8 +112,34 @@ static void norm_u(const orc_model *m, const double *theta, double *u)
     for (int p = 0; p < NP; ++p) u[p] = 2.0 * (theta[p] - m->lo[p]) / (m->hi[p] - m->lo[p]) - 1.0;
 }
 
-/* Eq. 1 in the single-polynomial reading (Delta-5): x_l = a_l tau_l(theta_l) + b_l ;
- * phi_k = prod_l x_l^{e_kl} ; dphi[l*K+k] = d phi_k / d x_l ; dx_dtheta[l] (C.1 last line). */
+/* Weight of model r of the piecewise emulator at label 0 = theta0 (Eq. 1: the five Teff regimes of P:72-76 are three
+ * polynomial models, cold <= 4550 K, warm 4000-9000 K, hot >= 7000 K, that overlap in 4000-4550 K and 7000-9000 K).
+ * The paper does not say how the two models of an overlap are combined.  Reading R-15 (PARITY UNPINNED against
+ * the paper, pinned only to its own definition): a cross-fade linear in tau(theta0) (log10 Teff) --
+ *   omega_r = up * down,  up = clamp((tau - tau(lo0)) / (tau(lo1) - tau(lo0)), 0, 1)  (1 when lo1 <= lo0),
+ *                         down = clamp((tau(hi1) - tau) / (tau(hi1) - tau(hi0)), 0, 1)  (1 when hi1 <= hi0);
+ * the derivative is the slope strictly inside a ramp and 0 elsewhere (the kinks at the regime borders are the gradient
+ * discontinuities the paper blames for Adam's instability near log Teff = 3.95). */
+void orc_blend_weight(const orc_model *m, int r, double theta0, double *w, double *dw_dtheta)
+{
+    const double *bl = m->model_blend + 4 * r;
+    int lg = m->label_log10[0];
+    double tau = lg ? log10(theta0) : theta0, dtau = lg ? 1.0 / (theta0 * log(10.0)) : 1.0;
+    double up = 1.0, dup = 0.0, dn = 1.0, ddn = 0.0;
+    if (bl[1] > bl[0]) {
+        double a = lg ? log10(bl[0]) : bl[0], b = lg ? log10(bl[1]) : bl[1], t = (tau - a) / (b - a);
+        if (t <= 0.0) up = 0.0; else if (t >= 1.0) up = 1.0; else { up = t; dup = dtau / (b - a); }
+    }
+    if (bl[3] > bl[2]) {
+        double a = lg ? log10(bl[2]) : bl[2], b = lg ? log10(bl[3]) : bl[3], t = (b - tau) / (b - a);
+        if (t <= 0.0) dn = 0.0; else if (t >= 1.0) dn = 1.0; else { dn = t; ddn = -dtau / (b - a); }
+    }
+    *w = up * dn;
+    *dw_dtheta = dup * dn + up * ddn;
+}
+
+/* Eq. 1: x_l = a_l tau_l(theta_l) + b_l ; phi_k = omega_r(k) prod_l x_l^{e_kl} (omega = 1 in the single-polynomial
+ * reading, Delta-5) ; dphi[l*K+k] = d phi_k / d x_l ; dx_dtheta[l] (C.1 last line). */
 void orc_monomials(const orc_model *m, const double *theta, double *x, double *phi, double *dphi,
                    double *dx_dtheta)
 {
@@ -137,6 +169,15 @@ void orc_monomials(const orc_model *m, const double *theta, double *x, double *p
                 }
             }
             dphi[l * K + k] = d;
+        }
+    }
+    if (m->n_models > 1) {
+        for (int k = 0; k < K; ++k) {
+            double w, dw;
+            orc_blend_weight(m, m->term_model[k], theta[0], &w, &dw);
+            for (int l = 0; l < L; ++l) dphi[l * K + k] *= w;
+            dphi[0 * K + k] += dw / dx_dtheta[0] * phi[k];      /* d omega / d x_0, chain rule through theta_0 */
+            phi[k] *= w;
         }
     }
 }

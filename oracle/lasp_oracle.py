@@ -29,6 +29,7 @@ class _Model(C.Structure):
         ("term_exps", _u8p), ("coeffs", _f64p), ("lo", _f64p), ("hi", _f64p),
         ("label_log10", _u8p), ("emu_a", _f64p), ("emu_b", _f64p),
         ("cont_degree", C.c_int32), ("seg_n_edge", _i32p),
+        ("n_models", C.c_int32), ("term_model", _u8p), ("model_blend", _f64p),
     ]
 
 
@@ -73,11 +74,15 @@ class Oracle:
         k["emu_a"] = np.ascontiguousarray(desc["emu_a"], dtype=np.float64)
         k["emu_b"] = np.ascontiguousarray(desc["emu_b"], dtype=np.float64)
         k["seg_n_edge"] = np.ascontiguousarray(desc["seg_n_edge"], dtype=np.int32)
+        self.n_models = int(desc.get("n_models", 0))
+        k["term_model"] = np.ascontiguousarray(desc.get("term_model", np.zeros(self.K)), dtype=np.uint8)
+        k["model_blend"] = np.ascontiguousarray(desc.get("model_blend", np.zeros(4)), dtype=np.float64).reshape(-1)
         self.m = _Model(self.P, self.n_seg, _p(k["seg_offset"], _i32p), _p(k["loglam"], _f64p),
                         _p(k["seg_sigma_inst"], _f64p), self.L, self.K, _p(k["term_exps"], _u8p),
                         _p(k["coeffs"], _f64p), _p(k["lo"], _f64p), _p(k["hi"], _f64p),
                         _p(k["label_log10"], _u8p), _p(k["emu_a"], _f64p), _p(k["emu_b"], _f64p),
-                        self.D, _p(k["seg_n_edge"], _i32p))
+                        self.D, _p(k["seg_n_edge"], _i32p), self.n_models, _p(k["term_model"], _u8p),
+                        _p(k["model_blend"], _f64p))
         self.lo = k["lo"]; self.hi = k["hi"]
 
     # ---- helpers
@@ -103,6 +108,11 @@ class Oracle:
         lib().orc_monomials(C.byref(self.m), _p(theta, _f64p), _p(x, _f64p), _p(phi, _f64p),
                             _p(dphi, _f64p), _p(dx, _f64p))
         return x, phi, dphi, dx
+
+    def blend_weight(self, r, theta0):
+        w = C.c_double(0.0); dw = C.c_double(0.0)
+        lib().orc_blend_weight(C.byref(self.m), C.c_int(r), C.c_double(theta0), C.byref(w), C.byref(dw))
+        return w.value, dw.value
 
     @staticmethod
     def legendre(x, D):

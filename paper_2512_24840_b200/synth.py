@@ -70,6 +70,13 @@ class Config:
     beta2: float = 0.999
     eps: float = 1e-8
     seed: int = field(default=0)
+    # piecewise emulator (Eq. 1's f_1..f_5): terms per polynomial model, e.g. (25, 26, 19) for the
+    # cold / warm / hot models of P:187, and for each model (lo0, lo1, hi0, hi1) in K: its weight rises over [lo0, lo1] and
+    # falls over [hi0, hi1] (0, 0 = no ramp on that side).  Empty: one polynomial.
+    models: tuple = ()
+    model_blend: tuple = ()
+    teff_box: tuple = ()       # prior box of Teff (default BOX["teff"])
+    teff_truth: tuple = ()     # range of the true Teff (default 4000-7500 K)
 
     def __post_init__(self):
         idx = self.cfg if isinstance(self.cfg, int) else 9
@@ -91,6 +98,12 @@ CONFIGS = {
               105, 13, 30, 300, (50.0, 50.0), "const", 0.05, 64),
     "S": Config("S", "long-stream", 4096, "log10", 3600.0, 9800.0, 2.5e-5, None, (0.0,), 26, 3, 30,
                 100, (50.0, 50.0), "const", 0.03, 16),
+    # the paper's own emulator layout: three polynomial models with 25 / 26 / 19 terms (cold <= 4550 K, warm
+    # 4000-9000 K, hot >= 7000 K) on the 1327 LAMOST pixels of 4200-5700 A; Teff spans all five regimes of P:72-76
+    "E": Config("E", "elodie-like", 16384, "log10", 4200.0, 5700.0, 1e-4, None, (0.0,), 70, 3, 30, 500,
+                (10.0, 200.0), "const", 0.03, 32, models=(25, 26, 19),
+                model_blend=((0.0, 0.0, 4000.0, 4550.0), (4000.0, 4550.0, 7000.0, 9000.0), (7000.0, 9000.0, 0.0, 0.0)),
+                teff_box=(3100.0, 12000.0), teff_truth=(3500.0, 11000.0)),
 }
 
 
@@ -136,10 +149,15 @@ def make_model_desc(c: Config, seed: int | None = None) -> dict:
     seg = np.asarray(c.seg_bounds if c.seg_bounds is not None else (0, P), dtype=np.int32)
     assert seg[-1] == P, (seg, P)
     L, K = c.L, c.K
-    exps = monomial_exps(L, K)
-    lo = np.array([BOX["teff"][0], BOX["logg"][0], BOX["feh"][0]] + [BOX["abund"][0]] * (L - 3)
+    if c.models:
+        assert sum(c.models) == K
+        exps = np.concatenate([monomial_exps(L, kr) for kr in c.models])
+    else:
+        exps = monomial_exps(L, K)
+    tbox = c.teff_box if c.teff_box else BOX["teff"]
+    lo = np.array([tbox[0], BOX["logg"][0], BOX["feh"][0]] + [BOX["abund"][0]] * (L - 3)
                   + [BOX["rv"][0], BOX["sigma"][0]], dtype=np.float32)
-    hi = np.array([BOX["teff"][1], BOX["logg"][1], BOX["feh"][1]] + [BOX["abund"][1]] * (L - 3)
+    hi = np.array([tbox[1], BOX["logg"][1], BOX["feh"][1]] + [BOX["abund"][1]] * (L - 3)
                   + [BOX["rv"][1], BOX["sigma"][1]], dtype=np.float32)
     label_log10 = np.zeros(L, dtype=np.uint8)
     label_log10[0] = 1
@@ -151,8 +169,25 @@ def make_model_desc(c: Config, seed: int | None = None) -> dict:
     emu_b = (-(thi + tlo) / (thi - tlo)).astype(np.float32)
     # coefficients: flux 1 +- 0.3
     rms = np.prod(np.sqrt(1.0 / (2.0 * exps.astype(np.float64) + 1.0)), axis=1)
-    coeffs = rng.standard_normal((K, P)) * (0.3 / math.sqrt(max(K - 1, 1))) / rms[:, None]
-    coeffs[0, :] = 1.0
+    extra = {}
+    if c.models:
+        # one master polynomial (the longest model's terms), and every model a copy of its leading terms with each term
+        # scaled by 1 + 0.05 N(0,1): the models agree to a few percent where they overlap, as fitted models of one library do
+        km = max(c.models)
+        master = rng.standard_normal((km, P)) * (0.3 / math.sqrt(km - 1)) / rms[:km, None]
+        master[0, :] = 1.0
+        parts = []
+        for kr in c.models:
+            scale = 1.0 + 0.05 * rng.standard_normal(kr)
+            scale[0] = 1.0
+            parts.append(master[:kr] * scale[:, None])
+        coeffs = np.concatenate(parts)
+        extra = dict(n_models=len(c.models),
+                     term_model=np.concatenate([np.full(kr, r, dtype=np.uint8) for r, kr in enumerate(c.models)]),
+                     model_blend=np.asarray(c.model_blend, dtype=np.float32))
+    else:
+        coeffs = rng.standard_normal((K, P)) * (0.3 / math.sqrt(max(K - 1, 1))) / rms[:, None]
+        coeffs[0, :] = 1.0
     # edge exclusion from the prior box: ceil((max|v| + 5 sigma_tot,max)/s_min)
     n_edge = np.zeros(seg.size - 1, dtype=np.int32)
     vmax = float(max(abs(lo[L]), abs(hi[L])))
@@ -166,7 +201,7 @@ def make_model_desc(c: Config, seed: int | None = None) -> dict:
         seg_sigma_inst=np.asarray(c.sigma_inst, dtype=np.float32),
         n_labels=L, n_terms=K, term_exps=exps, coeffs=coeffs.astype(np.float32),
         lo=lo, hi=hi, label_log10=label_log10, emu_a=emu_a, emu_b=emu_b,
-        cont_degree=c.D, seg_n_edge=n_edge, _rng=rng,
+        cont_degree=c.D, seg_n_edge=n_edge, _rng=rng, **extra,
     )
 
 
@@ -174,7 +209,8 @@ def draw_params(c: Config, desc: dict, B: int, rng: np.random.Generator) -> dict
     """Truth, continuum coefficients, SNR and initial guesses for B spectra (draw order fixed)."""
     L = c.L
     truth = np.empty((B, L + 2), dtype=np.float64)
-    truth[:, 0] = rng.uniform(4000.0, 7500.0, B)
+    tt = c.teff_truth if c.teff_truth else (4000.0, 7500.0)
+    truth[:, 0] = rng.uniform(tt[0], tt[1], B)
     truth[:, 1] = rng.uniform(1.0, 5.0, B)
     truth[:, 2] = rng.uniform(-2.5, 0.5, B)
     for l in range(3, L):

@@ -887,3 +887,69 @@ def test_resampler_is_numpy_cumsum_interp_and_linear(oracle_mod):
     R2 = oracle_mod.resample_coeffs(C_, ELODIE_LAM1, ELODIE_DLAM, [0, 700, ll.size], ll)
     assert np.allclose(R2[:, :699], R[:, :699], rtol=1e-12) and np.allclose(R2[:, 701:], R[:, 701:], rtol=1e-12)
     assert np.allclose(R2[:, 699:701], R[:, 699:701], rtol=1e-9)          # uniform log grid: the same nodes either way
+
+
+# ------------------------------------------------------------------------------------------------
+# Piecewise emulator: three polynomial models over five Teff regimes (Eq. 1; NEXT-3, reading R-15)
+# ------------------------------------------------------------------------------------------------
+def _single_model_desc(desc, r):
+    """The description of model r alone (n_models = 0: the single-polynomial path pinned above)."""
+    sel = np.asarray(desc["term_model"]) == r
+    d = {k: v for k, v in desc.items() if k not in ("n_models", "term_model", "model_blend")}
+    d["n_terms"] = int(sel.sum())
+    d["term_exps"] = np.asarray(desc["term_exps"])[sel]
+    d["coeffs"] = np.asarray(desc["coeffs"])[sel]
+    return d
+
+
+def test_piecewise_emulator_regimes_and_blend(oracle_mod):
+    """P:72-76 / P:187 on the three-model config: in the pure regimes (<= 4000 K, 4550-7000 K, > 9000 K) the spectrum is the
+    one model's own polynomial (the single-polynomial path, built here from that model's terms alone); in the overlaps
+    it is omega_a f_a + omega_b f_b with the weights linear in log10 Teff, retyped here; weights sum to one everywhere and
+    the spectrum is continuous across the four regime borders."""
+    case = synth.make_case("E", oracle_mod.forward, B=1)
+    d = case["desc"]
+    o = oracle_mod.Oracle(d)
+    singles = [oracle_mod.Oracle(_single_model_desc(d, r)) for r in range(3)]
+    assert [s.K for s in singles] == [25, 26, 19]                       # P:187: 25, 26, 19 non-zero coefficients
+    base = np.array([5000.0, 3.1, -0.7, 35.0, 80.0])
+
+    def S(orc, teff):
+        p = base.copy(); p[0] = teff
+        return orc.eval_S(p[None, :])[0]
+
+    for teff, r in ((3300.0, 0), (4000.0, 0), (4550.0, 1), (6000.0, 1), (7000.0, 1), (9000.0, 2), (11500.0, 2)):
+        assert np.allclose(S(o, teff), S(singles[r], teff), rtol=1e-12, atol=1e-14), teff
+    for teff, (a, b), (t0, t1) in ((4200.0, (0, 1), (4000.0, 4550.0)), (4500.0, (0, 1), (4000.0, 4550.0)),
+                                   (7300.0, (1, 2), (7000.0, 9000.0)), (8800.0, (1, 2), (7000.0, 9000.0))):
+        wb = (np.log10(teff) - np.log10(t0)) / (np.log10(t1) - np.log10(t0))
+        ref = (1.0 - wb) * S(singles[a], teff) + wb * S(singles[b], teff)
+        assert np.allclose(S(o, teff), ref, rtol=1e-12, atol=1e-14), teff
+        assert not np.allclose(S(o, teff), S(singles[a], teff), rtol=1e-4)        # the blend is not one model
+    for teff in np.linspace(3100.0, 12000.0, 90):
+        w = [o.blend_weight(r, teff)[0] for r in range(3)]
+        assert abs(sum(w) - 1.0) < 1e-14 and min(w) >= 0.0
+    for border in (4000.0, 4550.0, 7000.0, 9000.0):
+        assert np.abs(S(o, border * (1 + 1e-9)) - S(o, border * (1 - 1e-9))).max() < 1e-6
+
+
+def test_piecewise_emulator_gradient_vs_fd(oracle_mod):
+    """The analytic gradient with the d omega / d Teff term against central differences of the re-solved chi2, inside both
+    overlaps and in a pure regime (a dropped or mis-signed weight derivative fails the Teff component)."""
+    case = synth.make_case("E", oracle_mod.forward, B=3)
+    o = oracle_mod.Oracle(case["desc"])
+    init = case["init"].astype(np.float64).copy()
+    init[:, 0] = (4300.0, 8000.0, 5600.0)
+    chi2, grad, cont, st = o.eval_grad(case["flux"], case["ivar"], case["mask"], init)
+    for i in range(3):
+        u = o.norm_u(init[i])
+        for p in range(o.NP):
+            h = 1e-6
+            up, um = u.copy(), u.copy()
+            up[p] += h; um[p] -= h
+            fd = (o.chi2_u(case["flux"][i], case["ivar"][i], case["mask"][i], up)
+                  - o.chi2_u(case["flux"][i], case["ivar"][i], case["mask"][i], um)) / (2 * h)
+            assert abs(fd - grad[i, p]) <= 2e-6 * np.abs(grad[i]).max(), (i, p, fd, grad[i, p])
+    # the weight derivative matters: without it the Teff component would be off by more than the tolerance
+    w, dw = o.blend_weight(0, 4300.0)
+    assert dw < 0 and abs(dw * 4300.0 * np.log(10.0) * (np.log10(4550.0) - np.log10(4000.0)) + 1.0) < 1e-12
