@@ -56,6 +56,7 @@ extern "C" {
 #define LASP_MAX_SEG 8
 #define LASP_MAX_LABELS 30
 #define LASP_MAX_TERMS 512
+#define LASP_MAX_MODELS 4
 #define LASP_MAX_DEGREE 31 /* D+1 <= 32: one continuum row per warp lane in the solver */
 
 /* status[i] bits */
@@ -85,6 +86,15 @@ typedef struct {
     int32_t cont_degree;         /* D <= LASP_MAX_DEGREE, same for every segment */
     const int32_t *seg_n_edge;   /* [n_seg] pixels excluded from objective and WLS at each end of the
                                     segment (C.2-17) */
+    /* Piecewise emulator (Eq. 1's f_1..f_5: five Teff regimes served by three polynomial models, cold <= 4550 K,
+     * warm 4000-9000 K, hot >= 7000 K).  n_models <= 1: one polynomial, the two pointers
+     * are not read.  Otherwise term k of the shared term table belongs to model term_model[k] and the spectrum is
+     * sum_r omega_r(theta_0) f_r(theta): omega_r rises linearly in tau_0(theta_0) (log10 when label_log10[0]) from 0 at
+     * lo0 to 1 at lo1 and falls from 1 at hi0 to 0 at hi1 (a side with lo1 <= lo0, resp. hi1 <= hi0, has no ramp).
+     * The paper does not give the weights inside the overlaps: this is reading R-15 of DESIGN.md. */
+    int32_t n_models;            /* <= LASP_MAX_MODELS */
+    const uint8_t *term_model;   /* [K] */
+    const float *model_blend;    /* [n_models*4]: lo0, lo1, hi0, hi1 in the units of label 0 */
 } lasp_model_desc;
 
 typedef struct {

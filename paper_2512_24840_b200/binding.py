@@ -34,6 +34,7 @@ class ModelDesc(C.Structure):
         ("term_exps", _u8p), ("coeffs", _f32p), ("lo", _f32p), ("hi", _f32p),
         ("label_log10", _u8p), ("emu_a", _f32p), ("emu_b", _f32p),
         ("cont_degree", C.c_int32), ("seg_n_edge", _i32p),
+        ("n_models", C.c_int32), ("term_model", _u8p), ("model_blend", _f32p),
     ]
 
 
@@ -144,11 +145,15 @@ class LaspModel:
         k["emu_a"] = np.ascontiguousarray(desc["emu_a"], dtype=np.float32)
         k["emu_b"] = np.ascontiguousarray(desc["emu_b"], dtype=np.float32)
         k["seg_n_edge"] = np.ascontiguousarray(desc["seg_n_edge"], dtype=np.int32)
+        self.n_models = int(desc.get("n_models", 0))
+        k["term_model"] = np.ascontiguousarray(desc.get("term_model", np.zeros(self.K)), dtype=np.uint8)
+        k["model_blend"] = np.ascontiguousarray(desc.get("model_blend", np.zeros(4)), dtype=np.float32).reshape(-1)
         d = ModelDesc(self.P, self.n_seg, _p(k["seg_offset"], _i32p), _p(k["loglam"], _f64p),
                       _p(k["seg_sigma_inst"], _f32p), self.L, self.K, _p(k["term_exps"], _u8p),
                       _p(k["coeffs"], _f32p), _p(k["lo"], _f32p), _p(k["hi"], _f32p),
                       _p(k["label_log10"], _u8p), _p(k["emu_a"], _f32p), _p(k["emu_b"], _f32p),
-                      self.D, _p(k["seg_n_edge"], _i32p))
+                      self.D, _p(k["seg_n_edge"], _i32p), self.n_models, _p(k["term_model"], _u8p),
+                      _p(k["model_blend"], _f32p))
         self.ctx = C.c_void_p()
         rc = lib().lasp_create(C.byref(d), device, C.byref(self.ctx))
         if rc != 0:

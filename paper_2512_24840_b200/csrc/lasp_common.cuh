@@ -32,6 +32,12 @@ struct ModelDev {
     float lo[LASP_NPMAX], hi[LASP_NPMAX];
     float emu_a[LASP_MAX_LABELS], emu_b[LASP_MAX_LABELS];
     uint8_t label_log10[LASP_MAX_LABELS];
+    // piecewise emulator (lasp_model_desc.n_models > 1): model of every term, and per model the two ramps of its weight
+    // in emulator-input units x_0: up = clamp((x_0 - bl_u0) bl_ui, 0, 1), down = clamp((bl_d1 - x_0) bl_di, 0, 1)
+    // (bl_ui / bl_di = 0: no ramp on that side)
+    int n_models;
+    const uint8_t *term_model;
+    float bl_u0[LASP_MAX_MODELS], bl_ui[LASP_MAX_MODELS], bl_d1[LASP_MAX_MODELS], bl_di[LASP_MAX_MODELS];
 };
 
 // a1: emulator input x_l = a_l tau_l(theta_l) + b_l (Eq. 1, C.2-19)

@@ -49,7 +49,7 @@ struct V1Lay {
     int nt8;                // pixels per sweep of the CTA (threads x 8): the streaming window holds nt8 + 2 GUARD
     int SL;                 // longest padded segment: row length of the per-pixel-kernel scratch planes
     // shared-memory offsets (floats)
-    int oT, oA, oU, oM, oV, oX, oPHI, oGW, oGR, oTAP, oMOM, oRHS, oB, oRED, oLF, oQ, oSC, oEXP, oXP, oDPHI, oGSC, oEW, oNP, oHIST, total;
+    int oT, oA, oU, oM, oV, oX, oPHI, oGW, oGR, oTAP, oMOM, oRHS, oB, oRED, oLF, oQ, oSC, oEXP, oXP, oDPHI, oGSC, oEW, oNP, oHIST, oTM, total;
     int emax;               // largest exponent of the monomial table
 };
 
@@ -195,6 +195,49 @@ __shared__ V1Block v1_blk;
 // ------------------------------------------------------------------------------------------
 // a1: de-normalise, emulator inputs, monomials (Eq. 1, C.2-18/19).  Warp g, spectrum g.
 // ------------------------------------------------------------------------------------------
+// Piecewise emulator (Eq. 1's f_1..f_5; reading R-15): phi_k <- omega_r(k)(x_0) phi_k and the product rule
+// on d phi_k / d x_0, omega_r = up * down with the two ramps linear in x_0; the derivative of a ramp is its slope strictly
+// inside it and 0 elsewhere (as oracle/lasp_oracle.c orc_blend_weight).  Warp g, after phi and dphi have been written.
+__device__ __forceinline__ void v1_blend(int g)
+{
+    const ModelDev &M = v1_blk.M;
+    const V1Lay &L = v1_blk.L;
+    const int K = M.K, nl = M.L;
+    const uint8_t *tm = (const uint8_t *)(V1SM + L.oTM);
+    const float x0 = SMV(L.oX, 0, g);
+    float w[LASP_MAX_MODELS], dw[LASP_MAX_MODELS];
+#pragma unroll
+    for (int r = 0; r < LASP_MAX_MODELS; ++r) {
+        float up = 1.f, dup = 0.f, dn = 1.f, ddn = 0.f;
+        if (r < M.n_models) {
+            if (M.bl_ui[r] != 0.f) {
+                const float t = (x0 - M.bl_u0[r]) * M.bl_ui[r];
+                if (t <= 0.f) up = 0.f; else if (t < 1.f) { up = t; dup = M.bl_ui[r]; }
+            }
+            if (M.bl_di[r] != 0.f) {
+                const float t = (M.bl_d1[r] - x0) * M.bl_di[r];
+                if (t <= 0.f) dn = 0.f; else if (t < 1.f) { dn = t; ddn = -M.bl_di[r]; }
+            }
+        }
+        w[r] = up * dn;
+        dw[r] = dup * dn + up * ddn;
+    }
+    for (int k = V1_LANE; k < K; k += 32) {
+        const int r = tm[k];
+        float wr = w[0], dwr = dw[0];
+#pragma unroll
+        for (int q = 1; q < LASP_MAX_MODELS; ++q)
+            if (r == q) { wr = w[q]; dwr = dw[q]; }
+        const float ph = SMV(L.oPHI, k, g);
+        SMV(L.oPHI, k, g) = wr * ph;
+        for (int l = 0; l < nl; ++l) {
+            const float d = SMV(L.oDPHI, l * K + k, g);
+            SMV(L.oDPHI, l * K + k, g) = wr * d + (l == 0 ? dwr * ph : 0.f);
+        }
+    }
+    __syncwarp();
+}
+
 __device__ __noinline__ void v1_param_setup(int g)
 {
     const ModelDev &M = v1_blk.M;
@@ -252,6 +295,7 @@ __device__ __noinline__ void v1_param_setup(int g)
             }
         }
         __syncwarp();
+        if (M.n_models) v1_blend(g);
         return;
     }
     for (int k = V1_LANE; k < K; k += 32) {
@@ -270,6 +314,7 @@ __device__ __noinline__ void v1_param_setup(int g)
         }
     }
     __syncwarp();
+    if (M.n_models) v1_blend(g);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -1871,6 +1916,8 @@ __device__ __forceinline__ void v1_init_block(const ModelDev &M, const V1Lay &L,
         }
     } else
         for (int i = threadIdx.x; i < M.K * M.L; i += blockDim.x) ((uint8_t *)(V1SM + L.oEXP))[i] = M.exps[i];
+    if (M.n_models)
+        for (int k = threadIdx.x; k < M.K; k += blockDim.x) ((uint8_t *)(V1SM + L.oTM))[k] = M.term_model[k];
     for (int i = threadIdx.x; i < GS * L.Kq; i += blockDim.x) V1SM[L.oPHI + i] = 0.f;   // phi is zero past K
     // rows T and A: zero-weight taps multiply whatever lies in the window, so it must at least be finite
     // (streaming: one window buffer, oA == oT, and the global rows, which may hold another launch's values)

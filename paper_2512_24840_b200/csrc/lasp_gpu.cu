@@ -41,7 +41,7 @@ struct Variant {          // one way of launching the kernels for this model
 struct lasp_ctx {
     ModelDev M;
     int device = 0, num_sms = 0;
-    uint8_t *dexps = nullptr;
+    uint8_t *dexps = nullptr, *dtermmodel = nullptr;
     double *dconv = nullptr;
     int *dnedge = nullptr;
     long long launches = 0;
@@ -158,7 +158,7 @@ extern "C" int lasp_destroy(lasp_ctx *c)
 {
     if (!c) return LASP_OK;
     DeviceGuard dg(c->device);
-    cudaFree(c->dexps); cudaFree(c->dconv); cudaFree(c->dnedge);
+    cudaFree(c->dexps); cudaFree(c->dtermmodel); cudaFree(c->dconv); cudaFree(c->dnedge);
     cudaFree(c->dC1); cudaFree(c->dCF); cudaFree(c->dIS); cudaFree(c->dS2); cudaFree(c->dDS); cudaFree(c->dY); cudaFree(c->dW);
     cudaFree(c->dCP); cudaFree(c->dXJ); cudaFree(c->dTG); cudaFree(c->dAG); cudaFree(c->dqueue); cudaFree(c->dstats);
 #ifdef LASP_PHASE_TIMING
@@ -191,6 +191,16 @@ extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx *
     if (d->seg_offset[0] != 0 || d->seg_offset[nseg] != P)
         return fail(nullptr, LASP_ERR_INVALID_ARG, "seg_offset must start at 0 and end at n_pix");
     const int NP = L + 2;
+    if (d->n_models < 0 || d->n_models > LASP_MAX_MODELS)
+        return fail(nullptr, d->n_models < 0 ? LASP_ERR_INVALID_ARG : LASP_ERR_UNSUPPORTED, "n_models must be in [0, LASP_MAX_MODELS]");
+    if (d->n_models > 1) {
+        if (!d->term_model || !d->model_blend) return fail(nullptr, LASP_ERR_INVALID_ARG, "n_models > 1 needs term_model and model_blend");
+        for (int k = 0; k < K; ++k)
+            if (d->term_model[k] >= d->n_models) return fail(nullptr, LASP_ERR_INVALID_ARG, "term_model entry >= n_models");
+        for (int i = 0; i < 4 * d->n_models; ++i)
+            if (!std::isfinite(d->model_blend[i]) || (d->label_log10[0] && d->model_blend[i] < 0.f))
+                return fail(nullptr, LASP_ERR_INVALID_ARG, "model_blend must be finite (and >= 0 for a log10 label)");
+    }
     for (int p = 0; p < NP; ++p)
         if (!(d->lo[p] < d->hi[p])) return fail(nullptr, LASP_ERR_INVALID_ARG, "lo >= hi");
     if (!(d->lo[L + 1] > 0.f)) return fail(nullptr, LASP_ERR_INVALID_ARG, "sigma lower bound must be > 0");
@@ -372,6 +382,20 @@ extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx *
     CUDA_TRY_C(cudaMemset(c->dstats, 0, 2 * sizeof(unsigned long long)));
     CUDA_TRY_C(cudaEventCreateWithFlags(&c->ws_event, cudaEventDisableTiming));
     M.exps = c->dexps; M.conv = c->dconv;
+    M.n_models = d->n_models > 1 ? d->n_models : 0;
+    if (M.n_models) {
+        CUDA_TRY_C(cudaMalloc(&c->dtermmodel, (size_t)K));
+        CUDA_TRY_C(cudaMemcpy(c->dtermmodel, d->term_model, (size_t)K, cudaMemcpyHostToDevice));
+        M.term_model = c->dtermmodel;
+        // the ramps in emulator-input units x_0 = emu_a tau_0(theta_0) + emu_b (fp64 here, floats on the device)
+        auto X0 = [&](double th) { return (double)d->emu_a[0] * (d->label_log10[0] ? log10(th) : th) + (double)d->emu_b[0]; };
+        for (int r = 0; r < M.n_models; ++r) {
+            const float *bl = d->model_blend + 4 * r;
+            M.bl_u0[r] = M.bl_ui[r] = M.bl_d1[r] = M.bl_di[r] = 0.f;
+            if (bl[1] > bl[0]) { M.bl_u0[r] = (float)X0(bl[0]); M.bl_ui[r] = (float)(1.0 / (X0(bl[1]) - X0(bl[0]))); }
+            if (bl[3] > bl[2]) { M.bl_d1[r] = (float)X0(bl[3]); M.bl_di[r] = (float)(1.0 / (X0(bl[3]) - X0(bl[2]))); }
+        }
+    }
     int emax = 0;
     for (int i = 0; i < K * L; ++i) emax = std::max(emax, (int)d->term_exps[i]);
     setup_variant(c, prop, emax, false, c->res);
@@ -419,7 +443,7 @@ static void setup_variant(lasp_ctx *c, const cudaDeviceProp &prop, int emax, boo
     L.n1r = roundup(M.n1, 8);
     L.nmomr = L.n1r + roundup(std::max(M.nmom - L.n1r, 0), 8);
     L.VR = L.nmomr + L.n1r + roundup(M.K + 2, 8) + 6;
-    L.fastupd = (M.L >= 1 && M.L <= 4 && M.K + 2 <= 32 && L.NW <= 12) ? 1 : 0;
+    L.fastupd = (M.L >= 1 && M.L <= 4 && M.K + 2 <= 32 && L.NW <= 12 && M.n_models == 0) ? 1 : 0;
     L.fastw = (L.fastupd && M.n_seg == 1 && M.seg[0].uniform && M.seg[0].fit_hi > M.seg[0].fit_lo) ? 1 : 0;
     size_t bytes = 0;
     for (L.lfseg = 1; L.lfseg >= 0; --L.lfseg) {   // a factor slot per segment if shared memory allows it
@@ -440,6 +464,7 @@ static void setup_variant(lasp_ctx *c, const cudaDeviceProp &prop, int emax, boo
         L.oXP = take(GS * M.L * (L.emax + 1)); L.oDPHI = take(GS * M.L * M.K); L.oGSC = take(GS * M.NP);
         L.oNP = take(GS * 8);
         L.oHIST = take(GS * V1_WMAX);
+        L.oTM = take(M.n_models ? (M.K + 3) / 4 : 0);
         L.total = o;
         bytes = (size_t)o * sizeof(float);
         if (bytes + 2048 <= prop.sharedMemPerBlockOptin) break;   // + the kernels' static block state

@@ -851,3 +851,35 @@ def test_resample_coeffs_segments_ragged_and_out_of_range(gpu, oracle_mod):
         gpu.resample_coeffs(C_, 3900.0, 0.0, [0, 777], fine)
     with pytest.raises(gpu.LaspError):
         gpu.resample_coeffs(C_, 3900.0, 0.2, [0, 700], fine)
+
+
+# ------------------------------------------------------------------------------------------------
+# Piecewise emulator: three polynomial models over five Teff regimes (Eq. 1; NEXT-3, reading R-15)
+# ------------------------------------------------------------------------------------------------
+def _regime_params(case):
+    """Parameters that visit every regime, both overlaps and the four borders' neighbourhoods."""
+    teff = np.array([3300.0, 3990.0, 4010.0, 4275.0, 4540.0, 4560.0, 5800.0, 6990.0, 7010.0, 8000.0, 8990.0, 9010.0, 11500.0])
+    p = np.repeat(case["truth"][:1].astype(np.float64), teff.size, axis=0)
+    p[:, 0] = teff
+    return p
+
+
+def test_piecewise_emulator_flux_and_gradient(gpu, oracle_mod):
+    """Config E (25 / 26 / 19 terms, 1327 LAMOST pixels): lasp_eval_model within 1e-5 and lasp_eval_grad within 1e-4 of the
+    oracle in every regime and inside both cross-fades (the Teff component carries the d omega / d Teff term)."""
+    case = synth.make_case("E", oracle_mod.forward, B=13)
+    params = _regime_params(case)
+    for path in (1, 2):
+        check_model(gpu, oracle_mod, case, emulator_path=path)
+        check_model(gpu, oracle_mod, case, params=params, emulator_path=path)
+    check_grad(gpu, oracle_mod, case, case["init"])
+    check_grad(gpu, oracle_mod, case, params)
+    check_grad(gpu, oracle_mod, case, params, variant=2)
+
+
+def test_piecewise_emulator_fit(gpu, oracle_mod):
+    """Fits on config E (Teff from 3500 to 11000 K, initial guesses up to 500 K away: iterates cross regime borders), 300
+    Adam steps, and 10 LM iterations, against the oracle."""
+    case = synth.make_case("E", oracle_mod.forward, B=24)
+    check_fit(gpu, oracle_mod, case, 300)
+    _check_lm(gpu, oracle_mod, case, 10)
