@@ -513,7 +513,7 @@ def run_gpu(args):
         # the other single-GPU configs of BASELINE.json, one timed step each at a stated reduced batch, and the
         # survey's long-spectrum shape on the streaming variant
         oc = {}
-        for cid, b in ((2, 32768), (4, 32768), ("S", 4096)):
+        for cid, b in ((2, 32768), (4, 32768), ("S", 4096), ("E", 16384)):
             try:
                 oc[f"config{cid}"] = run_other_config(cid, b, torch, local, peaks, n_sms)
             except Exception as e:   # report, never hide
