@@ -20,14 +20,19 @@
  *   stopping rules      step 8  P:169-171          orc_stop_rule, orc_fit_stop
  *   Clean masking       step 6  P:137-161, P:171   orc_clean_update, orc_fit_clean
  *   resampler           step 3  Eq. 2-4, P:78-109  orc_obs_nodes, orc_resample, orc_resample_coeffs
+ *   piecewise emulator  Eq. 1   P:72-76, P:187     orc_blend_weight (R-15, parity unpinned), orc_monomials
  *   LM optimiser        NEXT-4  P:54-58, P:397     orc_fit_lm (Marquardt's method written out; R-13)
  *   error estimate      step 9  P:173              errors_one
  *
  * Parity pins (tests/test_oracle_*.py): numpy legvander/legval, numpy lstsq,
  * numpy convolve, central finite differences of chi2 (with re-solve), closed-form
  * first Adam step and torch.optim.Adam, textbook OLS covariance, Monte-Carlo
- * scatter, noise-free recovery, the 1327-pixel grid of P:227.  No function here
- * is "parity unpinned".
+ * scatter, noise-free recovery, the 1327-pixel grid of P:227; closed-form stop steps;
+ * constructed outlier patterns for the Clean passes; scipy least_squares (MINPACK) for the
+ * LM minimiser; flux conservation and numpy cumsum + interp for the resampler.
+ * PARITY UNPINNED (against the paper): orc_blend_weight -- the paper gives the regimes and
+ * the three models but not the weights inside the overlaps; reading R-15 of
+ * DESIGN.md is pinned to its own definition only.  No other function is unpinned.
  *
  * Build: gcc -O2 -fopenmp -shared -fPIC -o liblasp_oracle.so lasp_oracle.c -lm
  * (threads run over spectra only; each spectrum is computed serially.)
