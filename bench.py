@@ -233,13 +233,24 @@ def roofline_of(model, desc, B, n_iter, params, kern_ms, peaks, n_sms, clocks=No
 
 def ncu_record(key):
     """Counters of one `ncu --set full` capture of this launch shape, copied from the committed summary
-    profiles/r02_ncu_metrics.json (null when that shape was not captured): never measured under the bench itself."""
-    p = os.path.join(ROOT, "profiles", "r02_ncu_metrics.json")
+    profiles/r02_ncu_metrics.csv (None when that shape was not captured): never measured under the bench itself."""
+    import csv
+    p = os.path.join(ROOT, "profiles", "r02_ncu_metrics.csv")
     if not os.path.exists(p):
         return None
-    with open(p) as f:
-        d = json.load(f)
-    return d.get(key)
+    with open(p, newline="") as f:
+        for row in csv.DictReader(f):
+            if row.get("key") == key:
+                out = {}
+                for k, v in row.items():
+                    if k == "key":
+                        continue
+                    try:
+                        out[k] = float(v)
+                    except (TypeError, ValueError):
+                        out[k] = v
+                return out
+    return None
 
 
 def time_fit(model, data, n_iter, steps, warmup, kw, torch, barrier):
@@ -483,7 +494,7 @@ def run_gpu(args):
     key = f"config{args.config}_B{B}_n{n_iter}"
     rec = ncu_record(key)
     if rec:
-        roof["traffic"] = rec.get("dram_bytes")
+        roof["traffic"] = rec.get("dram_bytes_per_launch")
         roof["traffic_source"] = rec.get("source")
         roof["ncu_pipe_fma"] = rec.get("pipe_fma_pct")
         roof["ncu_issue_active"] = rec.get("issue_active_pct")
