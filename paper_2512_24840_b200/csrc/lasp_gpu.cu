@@ -471,8 +471,15 @@ static void setup_variant(lasp_ctx *c, const cudaDeviceProp &prop, int emax, boo
     }
     if (L.lfseg < 0) return;
     const void *fs[5] = {kFit[v.kv], kGrad[v.kv], kModel[v.kv], kFitClean[v.kv], kFitLM[v.kv]};
-    for (const void *f : fs)
-        if (f && cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess) { cudaGetLastError(); return; }
+    // The limit is an attribute of the kernel function on this device, shared by every ctx: only ever raise it (a second
+    // ctx with shorter rows must not take away what the launches of the first one need)
+    for (const void *f : fs) {
+        if (!f) continue;
+        cudaFuncAttributes at;
+        if (cudaFuncGetAttributes(&at, f) != cudaSuccess) { cudaGetLastError(); return; }
+        if ((int)bytes > at.maxDynamicSharedSizeBytes &&
+            cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess) { cudaGetLastError(); return; }
+    }
     int per_sm = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kFit[v.kv], nt, bytes) != cudaSuccess || per_sm < 1) {
         cudaGetLastError();

@@ -883,3 +883,23 @@ def test_piecewise_emulator_fit(gpu, oracle_mod):
     case = synth.make_case("E", oracle_mod.forward, B=24)
     check_fit(gpu, oracle_mod, case, 300)
     _check_lm(gpu, oracle_mod, case, 10)
+
+
+def test_two_live_contexts_of_different_shapes(gpu, oracle_mod):
+    """The dynamic shared-memory limit is an attribute of the kernel function, shared by every ctx on the device: creating
+    a second ctx for a smaller model must not lower it under the first one's launches (cudaLaunchKernel: invalid argument),
+    in either order of creation and use."""
+    big = synth.make_case(1, oracle_mod.forward, B=6)
+    small = make(small_config(), oracle_mod, B=5)
+    m_big = gpu.LaspModel(big["desc"])
+    m_small = gpu.LaspModel(small["desc"])                 # created after, launched before
+    for m, case in ((m_small, small), (m_big, big), (m_small, small)):
+        o = oracle_mod.Oracle(case["desc"])
+        g = m.eval_grad(case["flux"], case["ivar"], case["mask"], case["init"])
+        chi2, grad, _, _ = o.eval_grad(case["flux"], case["ivar"], case["mask"], case["init"])
+        gg = g["grad_u"].cpu().numpy().astype(np.float64)
+        assert (np.abs(gg - grad).max(axis=1) / np.abs(grad).max(axis=1)).max() <= TOL_GRAD
+        r = m.fit_batch(case["flux"], case["ivar"], case["mask"], case["init"], 3)
+        assert np.isfinite(r["chi2"].cpu().numpy()).all()
+        m.eval_model(case["truth"], case["cont"])
+    m_big.close(); m_small.close()
