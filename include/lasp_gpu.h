@@ -216,6 +216,23 @@ double lasp_fma_executed_per_spectrum_step(const lasp_ctx *ctx, double mean_taps
  * loops (groups of 4 spectra x n_iter), out2[1] = those that re-factorised the continuum Gram matrix. */
 int lasp_last_fit_stats(lasp_ctx *ctx, double *out2);
 
+/* lasp_eval_grad for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): same arguments, same kernels, same results, but the staged flux / weight planes and the per-CTA
+ * scratch live in ONE file-scope device array of LASP_STATIC_SCRATCH_BYTES that every GPU loading the library holds until
+ * the process exits; its device address is taken once, in lasp_create, with the ctx's device current.  The call
+ * allocates nothing (no cudaMalloc / cudaFree, no allocating library routine): one memset, two kernel launches and the
+ * ctx's event calls on `stream`.
+ * Limit: 2 B Ppad + (per-CTA scratch of min(ceil(B/4), resident CTAs) groups) floats must fit the array, Ppad = padded
+ * pixels per spectrum (n_pix + 2 halos per segment); about B <= 750 spectra of the 1,550-pixel LAMOST-like shape, B <= 150
+ * of the 7,781-pixel three-arm shape.  Larger calls return LASP_ERR_UNSUPPORTED with the sizes in lasp_last_error.
+ * The array is shared by EVERY ctx and call on the device and keeps the last call's contents: everything the kernels
+ * read is rewritten or cleared by the call itself, but two calls that overlap on the GPU (different streams or ctxs)
+ * race -- serialise them.  Does not share scratch with lasp_eval_grad / lasp_fit_batch (the ctx workspace). */
+#define LASP_STATIC_SCRATCH_BYTES (16u << 20)
+int lasp_eval_grad_static(lasp_ctx *ctx, int64_t B, const float *flux, const float *ivar,
+                          const uint8_t *mask, const float *params, const lasp_fit_opts *opts,
+                          float *chi2, float *grad_u, float *cont, int32_t *status, void *stream);
+
 /* Flux-conserving resampling (step 3 of the paper, Eq. 2-4) of an emulator coefficient
  * table from the model's linear wavelength grid onto an observed grid, once, ahead of lasp_create (the operation is linear
  * and independent of the stellar parameters, so resampling the coefficients equals resampling every model spectrum).

@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "liblasp_gpu.so")
 
 SYMBOLS = ["lasp_create", "lasp_destroy", "lasp_reserve", "lasp_fit_batch", "lasp_fit_batch_host", "lasp_eval_model",
-           "lasp_eval_grad", "lasp_kernel_variant", "lasp_launch_info", "lasp_launch_count", "lasp_fma_per_spectrum_step",
+           "lasp_eval_grad", "lasp_eval_grad_static", "lasp_kernel_variant", "lasp_launch_info", "lasp_launch_count", "lasp_fma_per_spectrum_step",
            "lasp_fma_executed_per_spectrum_step", "lasp_last_fit_stats", "lasp_resample_coeffs", "lasp_last_error",
            "lasp_version"]
 
@@ -72,6 +72,7 @@ def lib():
                                          [C.c_void_p] * 7 + [C.c_int64]
         L.lasp_eval_model.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 2 + [C.POINTER(FitOpts)] + [C.c_void_p] * 2
         L.lasp_eval_grad.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 4 + [C.POINTER(FitOpts)] + [C.c_void_p] * 5
+        L.lasp_eval_grad_static.argtypes = L.lasp_eval_grad.argtypes
         L.lasp_resample_coeffs.argtypes = [C.c_int, C.c_int32, C.c_int32, C.c_double, C.c_double, C.c_void_p, C.c_int32,
                                            C.c_int32, _i32p, _f64p, C.c_void_p, C.c_void_p]
         L.lasp_kernel_variant.argtypes = [C.c_void_p]
@@ -306,3 +307,23 @@ class LaspModel:
                                   _ptr(chi2), _ptr(grad), _ptr(cont), _ptr(status), self._stream())
         self._check(rc, "lasp_eval_grad")
         return dict(chi2=chi2, grad_u=grad, cont=cont, status=status)
+
+    def eval_grad_static(self, flux, ivar, mask, params, variant=0, emulator_path=0, out=None):
+        """lasp_eval_grad_static: as eval_grad, but the library allocates nothing (its scratch is a fixed 16 MiB device
+        array: small batches only, and calls must not overlap on the GPU).  Pass `out` (dict of device tensors chi2,
+        grad_u, cont, status) to keep this wrapper from allocating the outputs too."""
+        t = self.torch
+        flux = self._dev(flux, t.float32); ivar = self._dev(ivar, t.float32)
+        mask = self._dev(mask, t.uint8); params = self._dev(params, t.float32)
+        B = flux.shape[0]
+        if out is None:
+            out = dict(chi2=t.empty(B, device=self.device, dtype=t.float32),
+                       grad_u=t.empty((B, self.NP), device=self.device, dtype=t.float32),
+                       cont=t.empty((B, self.nc), device=self.device, dtype=t.float32),
+                       status=t.empty(B, device=self.device, dtype=t.int32))
+        opts = self._opts(variant=variant, emulator_path=emulator_path)
+        rc = lib().lasp_eval_grad_static(self.ctx, B, _ptr(flux), _ptr(ivar), _ptr(mask), _ptr(params), C.byref(opts),
+                                         _ptr(out["chi2"]), _ptr(out["grad_u"]), _ptr(out["cont"]), _ptr(out["status"]),
+                                         self._stream())
+        self._check(rc, "lasp_eval_grad_static")
+        return out

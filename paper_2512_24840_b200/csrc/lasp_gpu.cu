@@ -30,6 +30,11 @@ static const void *kGrad[KV_N] = {(const void *)lasp_v1_grad_kernel<192, 2, fals
 static const void *kModel[KV_N] = {(const void *)lasp_v1_model_kernel<192, 2, false>, (const void *)lasp_v1_model_kernel<384, 1, false>,
                                    (const void *)lasp_v1_model_kernel<192, 2, true>};
 
+// Scratch of the allocation-free entry point lasp_eval_grad_static: one array per GPU that loads this library, held
+// until the process exits.  In HOST code this name is only a stand-in for the symbol, not a device address: lasp_create
+// asks the runtime for the address (cudaGetSymbolAddress, with the ctx's device current) and keeps it in the ctx.
+static __device__ __align__(256) float lasp_static_scratch[LASP_STATIC_SCRATCH_BYTES / sizeof(float)];
+
 struct Variant {          // one way of launching the kernels for this model
     bool ok = false;
     int kv = 0;           // kernel instantiation
@@ -60,6 +65,7 @@ struct lasp_ctx {
     unsigned long long *dstats = nullptr;   // [0] group-steps of the Adam loops, [1] of them with a fresh Gram factor
     cudaEvent_t ws_event = nullptr;
     bool ws_pending = false;
+    float *static_ws = nullptr;   // device address of lasp_static_scratch on this ctx's device
 #ifdef LASP_PHASE_TIMING
     unsigned long long *ddbg = nullptr;
 #endif
@@ -381,6 +387,7 @@ extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx *
     CUDA_TRY_C(cudaMalloc(&c->dstats, 2 * sizeof(unsigned long long)));
     CUDA_TRY_C(cudaMemset(c->dstats, 0, 2 * sizeof(unsigned long long)));
     CUDA_TRY_C(cudaEventCreateWithFlags(&c->ws_event, cudaEventDisableTiming));
+    CUDA_TRY_C(cudaGetSymbolAddress((void **)&c->static_ws, lasp_static_scratch));   // this device's copy of the array
     M.exps = c->dexps; M.conv = c->dconv;
     M.n_models = d->n_models > 1 ? d->n_models : 0;
     if (M.n_models) {
@@ -720,6 +727,59 @@ extern "C" int lasp_eval_grad(lasp_ctx *c, int64_t B, const float *flux, const f
     if (rc) return rc;
     V1Args a;
     base_args(c, *v, mma, B, a);
+    a.gparams = params; a.chi2 = chi2; a.grad_u = grad_u; a.cont = cont; a.status = status;
+    return launch(c, kGrad, *v, a, st);
+}
+
+// lasp_eval_grad without any allocation: the staged planes and the per-CTA scratch are carved out of lasp_static_scratch.
+// Calls nothing that allocates (no cudaMalloc / cudaFree, no library routine): two kernel launches, one memset, two event
+// calls.  The array is shared by every ctx and every call on the device and keeps the last call's contents: the stage kernel
+// rewrites every padded pixel of the planes it uses, the per-CTA part is cleared here, and calls that overlap on the GPU
+// (different streams, different ctxs) race -- the caller serialises them.
+extern "C" int lasp_eval_grad_static(lasp_ctx *c, int64_t B, const float *flux, const float *ivar,
+                                     const uint8_t *mask, const float *params, const lasp_fit_opts *opts, float *chi2,
+                                     float *grad_u, float *cont, int32_t *status, void *stream)
+{
+    if (!c) return fail(nullptr, LASP_ERR_INVALID_ARG, "null ctx");
+    if (B < 1 || !flux || !ivar || !params || !chi2 || !grad_u)
+        return fail(c, LASP_ERR_INVALID_ARG, "lasp_eval_grad_static: null pointer or B < 1");
+    const Variant *v = nullptr;
+    bool mma = false;
+    int rc = resolve(c, opts, "lasp_eval_grad_static", &v, &mma);
+    if (rc) return rc;
+    if (!c->static_ws) return fail(c, LASP_ERR_CUDA, "lasp_eval_grad_static: the static scratch has no device address");
+    const ModelDev &M = c->M;
+    const size_t cap = LASP_STATIC_SCRATCH_BYTES / sizeof(float);
+    const size_t ngroups = ((size_t)B + GS - 1) / GS;
+    const size_t grid = std::min(ngroups, (size_t)c->num_sms * v->cta_per_sm);
+    auto up = [](size_t n) { return (n + 63) / 64 * 64; };   // 256-byte steps
+    const size_t n_plane = up((size_t)B * M.Ppad), n_cp = up(grid * GS * M.Ppad);
+    const size_t n_ds = c->nonuniform ? up(grid * 3 * GS * v->L.SL) : 0;
+    const size_t n_tg = v == &c->str ? n_cp : 0;
+    const size_t need = 2 * n_plane + n_cp + n_ds + 2 * n_tg;
+    if (B > (int64_t)1 << 30 || need > cap)
+        return fail(c, LASP_ERR_UNSUPPORTED, "lasp_eval_grad_static: B = " + std::to_string(B) + " spectra of " +
+                    std::to_string(M.Ppad) + " padded pixels need " + std::to_string(need * sizeof(float)) +
+                    " bytes of scratch, the static array holds " + std::to_string((size_t)LASP_STATIC_SCRATCH_BYTES) +
+                    " (use lasp_eval_grad, which allocates)");
+    DeviceGuard dg(c->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    rc = ws_acquire(c, st);
+    if (rc) return rc;
+    float *Y = c->static_ws, *W = Y + n_plane, *per_cta = W + n_plane;
+    CUDA_TRY(c, cudaMemsetAsync(per_cta, 0, (n_cp + n_ds + 2 * n_tg) * sizeof(float), st));
+    lasp_v1_stage_kernel<<<(unsigned)B, 256, 0, st>>>(M, c->dnedge, flux, ivar, mask, Y, W);
+    c->launches += 1;
+    CUDA_TRY(c, cudaGetLastError());
+    V1Args a;
+    memset(&a, 0, sizeof(a));
+    a.Y = Y; a.W = W; a.C1 = c->dC1; a.B = B;
+    a.CP = per_cta;
+    a.IS = c->dIS; a.S2 = c->dS2;
+    if (n_ds) a.DS = per_cta + n_cp;
+    if (n_tg) { a.TG = per_cta + n_cp + n_ds; a.AG = a.TG + n_tg; }
+    if (mma) { a.CF = c->dCF; a.ksteps = c->cf_ksteps; }
+    a.ngroups = (int)ngroups;
     a.gparams = params; a.chi2 = chi2; a.grad_u = grad_u; a.cont = cont; a.status = status;
     return launch(c, kGrad, *v, a, st);
 }
