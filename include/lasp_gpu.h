@@ -198,7 +198,7 @@ int lasp_eval_grad(lasp_ctx *ctx, int64_t B, const float *flux, const float *iva
 int lasp_kernel_variant(const lasp_ctx *ctx);
 
 /* Launch shape of variant 1 (resident) or 2 (streaming): out4 = {available, threads per CTA, CTAs per SM,
- * dynamic shared memory in bytes}. */
+ * dynamic shared memory in bytes of a call without the stopping rules (with them: + 16 stop_window bytes)}. */
 int lasp_launch_info(const lasp_ctx *ctx, int variant, int32_t *out4);
 
 /* Number of kernels launched by this ctx so far (bench.py reports it as gpu_launches). */

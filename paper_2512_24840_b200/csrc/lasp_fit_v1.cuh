@@ -185,6 +185,7 @@ struct V1Block {
     int lm_acc[GS];       // the last trial step was accepted
 };
 __shared__ V1Block v1_blk;
+static_assert(sizeof(V1Block) <= 1792, "the block state is part of the shared-memory budget that keeps two config-1 CTAs under the 196 KB carveout (setup_variant in lasp_gpu.cu)");
 #define V1_TID ((int)threadIdx.x)
 #define V1_LANE ((int)(threadIdx.x & 31))
 #define V1_WARP ((int)(threadIdx.x >> 5))
@@ -2451,7 +2452,7 @@ __device__ __noinline__ bool v1_stop_test(int g, int t)
     int rule = 0;
     if (V1_LANE == 0) {
         const int W = a.stop_window, slot = t % W;
-        float *h = V1SM + v1_blk.L.oHIST + g * V1_WMAX;
+        float *h = V1SM + v1_blk.L.oHIST + g * W;
         const int rise = (t > 1 && Lt > v1_blk.lprev[g]) ? v1_blk.rise[g] + 1 : 0;
         if (t > W && fabsf(Lt - h[slot]) < a.stop_tol) rule = 2;      // h[slot] still holds L_(t-W)
         else if (rise >= W) rule = 3;

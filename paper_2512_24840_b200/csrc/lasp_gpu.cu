@@ -145,7 +145,7 @@ extern "C" int lasp_launch_info(const lasp_ctx *c, int variant, int32_t *out4)
 {
     if (!c || !out4 || variant < 1 || variant > 2) return LASP_ERR_INVALID_ARG;
     const Variant &v = variant == 1 ? c->res : c->str;
-    out4[0] = v.ok; out4[1] = v.nt; out4[2] = v.cta_per_sm; out4[3] = v.L.total * 4;
+    out4[0] = v.ok; out4[1] = v.nt; out4[2] = v.cta_per_sm; out4[3] = v.L.oHIST * 4;
     return LASP_OK;
 }
 
@@ -470,8 +470,13 @@ static void setup_variant(lasp_ctx *c, const cudaDeviceProp &prop, int emax, boo
         L.oEXP = take(std::max((M.K * M.L + 3) / 4, M.K));   // bytes [K][L], or one packed word per term when L <= 4
         L.oXP = take(GS * M.L * (L.emax + 1)); L.oDPHI = take(GS * M.L * M.K); L.oGSC = take(GS * M.NP);
         L.oNP = take(GS * 8);
-        L.oHIST = take(GS * V1_WMAX);
         L.oTM = take(M.n_models ? (M.K + 3) / 4 : 0);
+        // LAST: the loss history of the stopping rules, GS rings of stop_window entries.  A launch asks for what its call
+        // needs (launch(): oHIST + GS * stop_window floats), the layout is sized for the largest window.  Not cosmetic: with
+        // two CTAs per SM the config-1 shape sits 0.1 % under a shared-memory carveout step -- 2 x (dynamic + static block
+        // state + 1 KB reserved) <= 196 KB leaves 60 KB of L1, one byte more selects the 228 KB carveout and 28 KB of L1,
+        // which costs 2 % (L1 hit rate of the table / plane loads 12.6 % -> 5.2 %, measured)
+        L.oHIST = take(GS * V1_WMAX);
         L.total = o;
         bytes = (size_t)o * sizeof(float);
         if (bytes + 2048 <= prop.sharedMemPerBlockOptin) break;   // + the kernels' static block state
@@ -638,7 +643,7 @@ static void base_args(lasp_ctx *c, const Variant &v, bool mma, int64_t B, V1Args
 static int launch(lasp_ctx *c, const void *const *table, const Variant &v, const V1Args &a, cudaStream_t st)
 {
     const int grid = std::min(a.ngroups, c->num_sms * v.cta_per_sm);
-    const size_t smem = (size_t)v.L.total * sizeof(float);
+    const size_t smem = (size_t)(v.L.oHIST + GS * a.stop_window) * sizeof(float);   // see setup_variant
     void *args[3] = {(void *)&c->M, (void *)&v.L, (void *)&a};
     CUDA_TRY(c, cudaLaunchKernel(table[v.kv], dim3(grid), dim3(v.nt), args, smem, st));
     c->launches += 1;

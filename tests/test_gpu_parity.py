@@ -903,3 +903,18 @@ def test_two_live_contexts_of_different_shapes(gpu, oracle_mod):
         assert np.isfinite(r["chi2"].cpu().numpy()).all()
         m.eval_model(case["truth"], case["cont"])
     m_big.close(); m_small.close()
+
+
+def test_config1_launch_stays_under_the_196k_carveout(gpu):
+    """Two CTAs of the config-1 shape must fit the 196 KB shared-memory carveout (60 KB of L1 left; the next step, 228 KB,
+    leaves 28 KB and costs 2 %): 2 x (dynamic + static block state <= 1792 + 1024 reserved) <= 200,704 B,
+    without the stopping rules and with the paper's window of 50."""
+    cfg = synth.CONFIGS[1]
+    desc = synth.make_model_desc(cfg)
+    desc.pop("_rng")
+    m = gpu.LaspModel(desc)
+    info = m.launch_info(1)
+    assert info["available"] and info["ctas_per_sm"] == 2 and info["threads"] == 192
+    for window in (0, 50):
+        assert 2 * (info["smem_bytes"] + 16 * window + 1792 + 1024) <= 196 * 1024, info
+    m.close()
