@@ -26,6 +26,8 @@ def probe(tmp_path_factory):
     L.probe_tcgen05.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_float)]
     L.probe_ffma.restype = ctypes.c_double
     L.probe_ffma.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int]
+    L.probe_ffma2.restype = ctypes.c_double
+    L.probe_ffma2.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int]
     return L
 
 
@@ -54,13 +56,16 @@ def test_tcgen05_tf32_narrow_n_against_ffma(probe, capsys):
         mac = 128 * n_cols * 8 / cyc
         rows.append((n_cols, n_tiles, n_acc, cyc, mac))
     tf = probe.probe_ffma(296, 192, 20000)
-    assert tf > 30.0
+    tf2 = probe.probe_ffma2(296, 192, 20000)
+    assert tf > 30.0 and tf2 > 30.0
     lines = ["pipe probe (B200): tcgen05.mma.cta_group::1.kind::tf32, M=128, K=8, A/B from shared memory",
              "  N   A tiles  accumulators   cycles/MMA   MAC/clk/SM   useful MAC/clk/SM with [hi|lo] split operands (x 1/4)"]
     for n_cols, n_tiles, n_acc, cyc, mac in rows:
         lines.append(f"  {n_cols:3d}  {n_tiles:3d}      {n_acc:3d}         {cyc:8.2f}     {mac:8.1f}     {mac / 4:8.1f}")
     lines.append(f"FP32 pipe, acc[4][8] += p[g]*c[i] from registers, 296 x 192 threads: {tf:.1f} TFLOP/s "
                  f"= {tf * 1e12 / 2 / 148 / 1.965e9:.1f} FMA/clk/SM")
+    lines.append(f"the same block with packed fma.rn.f32x2 (FFMA2, half the instructions): {tf2:.1f} TFLOP/s "
+                 f"= {tf2 * 1e12 / 2 / 148 / 1.965e9:.1f} FMA/clk/SM")
     text = "\n".join(lines)
     with capsys.disabled():
         print("\n" + text)
