@@ -1003,7 +1003,11 @@ extern "C" int lasp_fit_batch_host(lasp_ctx *c, int64_t B, const float *flux, co
     if (B < 1 || !flux || !ivar || !init || !opts || !params || !chi2 || chunk < 0)
         return fail(c, LASP_ERR_INVALID_ARG, "lasp_fit_batch_host: null pointer, B < 1 or chunk < 0");
     DeviceGuard dg(c->device);
-    if (chunk == 0) chunk = 65536;
+    // 0 = automatic: two chunks when the batch is small (the second upload and the first download overlap a fit; measured
+    // on config 1, 65,536 spectra: 72.5 k spectra/s with 2 chunks, 70.7 k with 8, 65.6 k with 16 -- every launch costs a ramp
+    // and a tail of partly idle SMs), never more than 131,072 spectra per chunk (device buffers), a multiple of GS so that
+    // the CTA groups are those of one lasp_fit_batch call over the whole batch
+    if (chunk == 0) chunk = std::min<int64_t>(131072, std::max<int64_t>(4096, ((B + 1) / 2 + GS - 1) / GS * GS));
     chunk = std::min<int64_t>(chunk, B);
     int rc = hostpipe_reserve(c, chunk);
     if (rc) return rc;
