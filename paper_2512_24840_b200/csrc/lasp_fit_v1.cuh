@@ -84,9 +84,9 @@ struct V1Args {
     float lm_lambda0;      // lasp_fit_opts.optimizer = 1 (the LM instantiation of the fit kernel): initial damping
     unsigned char *mask_out;   // [B][P] 1 where the pixel still takes part at the end (may be null)
     unsigned long long *dbg;   // optional per-phase cycle counters (LASP_TIMING=1), else null
-    // per-pixel broadening kernels (linear grids, C.2-14): 1/s_j and s_j^2 with V1_TPAD replicated entries on
+    // per-pixel broadening kernels (linear grids, C.2-14): 1/s_j and s_j with V1_TPAD replicated entries on
     // both sides, and per-CTA scratch [3][GS][Ppad] for dS/dv, dS/dsigma*, 1/E0 (thread-private pixels)
-    const float *IS, *S2;
+    const float *IS, *SJ;
     float *DS;
     unsigned int *queue;   // work-queue counter for the fit kernel (zeroed before the launch), may be null
     unsigned long long *stats;   // [0] += Adam group-steps, [1] += those with a fresh Gram factor (may be null)
@@ -98,6 +98,7 @@ struct V1Args {
 
 struct V1Np {          // per-spectrum scalars of a per-pixel-kernel segment
     float v, sigstar, sigtot, hn, hbv, hcap;   // hn = -log2(e)/(2 sigma_tot^2); hbv = |v| + 5 sigma_tot (km/s)
+    float an;                                  // sqrt(log2(e)/2) / sigma_tot: a_j = an s_j scales offsets so that the weight is 2^(-d^2)
 };
 
 
@@ -425,6 +426,7 @@ __device__ __noinline__ void v1_setup_weights(const SegDev &sg, int g)
             V1Np *np = (V1Np *)(V1SM + L.oNP) + g;
             np->v = v; np->sigstar = sigstar; np->sigtot = sigtot;
             np->hn = -0.72134752044f / (sigtot * sigtot);        // -log2(e)/2 / sigma_tot^2
+            np->an = 0.84932180029f / sigtot;
             np->hbv = fabsf(v) + 5.f * sigtot;
             np->hcap = (float)(sg.halo - 18);
             const int H = (int)ceilf(fminf(np->hbv * sg.inv_s, np->hcap));
@@ -543,20 +545,47 @@ __device__ __forceinline__ float v1_ex2(float x)
     return y;
 }
 
+// One group of four taps k = k0 .. k0 + 3 of the forward stencil for the thread's eight pixels.  The weight is
+// e = 2^(-d^2) with d = (k - mu_i) a_i, a_i = sqrt(log2(e) / 2) / sigma_i (one FFMA, one FMUL, one ex2); the kernel moments
+// are accumulated in the scaled offset d and rescaled once per pixel.  MASK = false: every tap of the group lies inside the
+// support of every pixel of the (active part of the) warp, so the support test is left out.
+template <bool MASK>
+__device__ __forceinline__ void v1_np_taps_forward(const float (&Wd)[12], int k0, const float (&aa)[OCT], const float (&bb)[OCT],
+                                                   const float (&hb)[OCT], float (&A0)[OCT], float (&A1)[OCT], float (&A2)[OCT],
+                                                   float (&E0)[OCT], float (&E1)[OCT], float (&E2)[OCT])
+{
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        const float kf = (float)(k0 + r);
+        const float ak1 = fabsf(kf) - 1.f;
+#pragma unroll
+        for (int i = 0; i < OCT; ++i) {
+            const float d = fmaf(kf, aa[i], -bb[i]);
+            float e = v1_ex2(d * -d);
+            if (MASK) e = (ak1 < hb[i]) ? e : 0.f;
+            const float Tv = Wd[i + 3 - r];
+            const float ed = e * d, edd = ed * d;
+            E0[i] += e; E1[i] += ed; E2[i] += edd;
+            A0[i] = fmaf(e, Tv, A0[i]); A1[i] = fmaf(ed, Tv, A1[i]); A2[i] = fmaf(edd, Tv, A2[i]);
+        }
+    }
+}
+
 __device__ __forceinline__ void v1_np_forward_octet(const float4 *__restrict__ row4, int j0, const V1Np &p,
-                                                    const float (&is)[OCT], const float (&s2)[OCT],
+                                                    const float (&is)[OCT], const float (&sj)[OCT],
                                                     float (&S)[OCT], float (&DSV)[OCT], float (&DSS)[OCT],
                                                     float (&EI)[OCT])
 {
-    float mu[OCT], ni2[OCT], hb[OCT];
+    float aa[OCT], bb[OCT], hb[OCT];
     float A0[OCT], A1[OCT], A2[OCT], E0[OCT], E1[OCT], E2[OCT];
-    float hmx = 0.f;
+    float hmx = 0.f, hmn = 3.0e38f;
 #pragma unroll
     for (int i = 0; i < OCT; ++i) {
-        mu[i] = p.v * is[i];
-        ni2[i] = p.hn * s2[i];
+        aa[i] = p.an * sj[i];
+        bb[i] = p.v * is[i] * aa[i];
         hb[i] = fminf(p.hbv * is[i], p.hcap);
         hmx = fmaxf(hmx, hb[i]);
+        hmn = fminf(hmn, hb[i]);
         A0[i] = A1[i] = A2[i] = E0[i] = E1[i] = E2[i] = 0.f;
     }
     const int H = (int)ceilf(hmx);
@@ -566,21 +595,10 @@ __device__ __forceinline__ void v1_np_forward_octet(const float4 *__restrict__ r
     for (int ai = 0; ai < na; ++ai) {
         const float4 qa = row4[SW4(q - ai)];
         const float Wd[12] = {qa.x, qa.y, qa.z, qa.w, qb.x, qb.y, qb.z, qb.w, qc.x, qc.y, qc.z, qc.w};
-#pragma unroll
-        for (int r = 0; r < 4; ++r) {
-            const float kf = (float)(4 * (a_lo + ai) - 3 + r);
-            const float ak1 = fabsf(kf) - 1.f;
-#pragma unroll
-            for (int i = 0; i < OCT; ++i) {
-                const float d = kf - mu[i];
-                float e = v1_ex2(d * d * ni2[i]);
-                e = (ak1 < hb[i]) ? e : 0.f;
-                const float Tv = Wd[i + 3 - r];
-                const float ed = e * d, edd = ed * d;
-                E0[i] += e; E1[i] += ed; E2[i] += edd;
-                A0[i] = fmaf(e, Tv, A0[i]); A1[i] = fmaf(ed, Tv, A1[i]); A2[i] = fmaf(edd, Tv, A2[i]);
-            }
-        }
+        const int k0 = 4 * (a_lo + ai) - 3;
+        const bool inside = (float)(max(abs(k0), abs(k0 + 3)) - 1) < hmn;   // |k| <= ceil(x)  <=>  |k| - 1 < x
+        if (__all_sync(__activemask(), inside)) v1_np_taps_forward<false>(Wd, k0, aa, bb, hb, A0, A1, A2, E0, E1, E2);
+        else v1_np_taps_forward<true>(Wd, k0, aa, bb, hb, A0, A1, A2, E0, E1, E2);
         qc = qb; qb = qa;
     }
     const float rs = p.sigstar / p.sigtot;
@@ -589,18 +607,39 @@ __device__ __forceinline__ void v1_np_forward_octet(const float4 *__restrict__ r
         const float inv = 1.f / E0[i];
         S[i] = A0[i] * inv;
         EI[i] = inv;
-        const float is2 = ni2[i] * -1.3862943611f;   // 1/sigma_j^2 = 2 i2 = -2 ln2 * ni2
-        const float smu = (A1[i] * inv - E1[i] * inv * S[i]) * is2;
-        const float ssg = (A2[i] * inv - E2[i] * inv * S[i]) * is2 * sqrtf(is2);
+        // moments in the scaled offset: A1 = a A1', A2 = a^2 A2' (E likewise) and 1/sigma_j^2 = 2 ln2 a^2, so both
+        // derivatives come out as (.)' times a constant times a
+        const float smu = (A1[i] * inv - E1[i] * inv * S[i]) * (1.3862943611f * aa[i]);
+        const float ssg = (A2[i] * inv - E2[i] * inv * S[i]) * (1.6322368749f * aa[i]);
         DSV[i] = smu * is[i];
         DSS[i] = ssg * rs * is[i];
     }
 }
 
 // adjoint:  t_i = sum_j a'_j e_{j,j-i},  a' = a/E0 (row A).  With k' = j... the window over SOURCE pixels slides
-// like the forward one; each source carries its own (mu, sigma, H).  istab/s2tab point at padded pixel 0.
+// like the forward one; each source carries its own (mu, sigma, H).  istab/sjtab point at padded pixel 0.
+template <bool MASK>
+__device__ __forceinline__ void v1_np_taps_adjoint(const float (&Wd)[12], int k0, const float (&aa)[12], const float (&bb)[12],
+                                                   const float (&hb)[12], float (&t)[OCT])
+{
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        // target i reads source m = i+3-r at lag k' = k0 + r: source j = i - k' contributes e_{j, k = j - i = -k'}
+        const float kf = (float)(k0 + r);
+        const float ak1 = fabsf(kf) - 1.f;
+#pragma unroll
+        for (int i = 0; i < OCT; ++i) {
+            const int m = i + 3 - r;
+            const float d = fmaf(-kf, aa[m], -bb[m]);
+            float e = v1_ex2(d * -d);
+            if (MASK) e = (ak1 < hb[m]) ? e : 0.f;
+            t[i] = fmaf(Wd[m], e, t[i]);
+        }
+    }
+}
+
 __device__ __forceinline__ void v1_np_adjoint_octet(const float4 *__restrict__ row4, int j0, int H, const V1Np &p,
-                                                    const float *__restrict__ istab, const float *__restrict__ s2tab,
+                                                    const float *__restrict__ istab, const float *__restrict__ sjtab,
                                                     float (&t)[OCT])
 {
 #pragma unroll
@@ -612,32 +651,24 @@ __device__ __forceinline__ void v1_np_adjoint_octet(const float4 *__restrict__ r
         const int q = wb >> 2;
         const float4 w0 = row4[SW4(q)], w1 = row4[SW4(q + 1)], w2 = row4[SW4(q + 2)];
         const float Wd[12] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w, w2.x, w2.y, w2.z, w2.w};
-        float mu[12], ni2[12], hb[12];
+        float aa[12], bb[12], hb[12];
+        float hmn = 3.0e38f;
 #pragma unroll
         for (int m4 = 0; m4 < 3; ++m4) {
-            const float4 i4 = __ldg((const float4 *)(istab + wb) + m4), s4 = __ldg((const float4 *)(s2tab + wb) + m4);
+            const float4 i4 = __ldg((const float4 *)(istab + wb) + m4), s4 = __ldg((const float4 *)(sjtab + wb) + m4);
             const float ii[4] = {i4.x, i4.y, i4.z, i4.w}, ss[4] = {s4.x, s4.y, s4.z, s4.w};
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
-                mu[m4 * 4 + c] = p.v * ii[c];
-                ni2[m4 * 4 + c] = p.hn * ss[c];
+                aa[m4 * 4 + c] = p.an * ss[c];
+                bb[m4 * 4 + c] = p.v * ii[c] * aa[m4 * 4 + c];
                 hb[m4 * 4 + c] = fminf(p.hbv * ii[c], p.hcap);
+                hmn = fminf(hmn, hb[m4 * 4 + c]);
             }
         }
-#pragma unroll
-        for (int r = 0; r < 4; ++r) {
-            // target i reads source m = i+3-r at lag k' = 4a-3+r, i.e. kernel offset k = j - i = -k'... (j = i - k')
-            const float kf = (float)(4 * a - 3 + r);
-            const float ak1 = fabsf(kf) - 1.f;
-#pragma unroll
-            for (int i = 0; i < OCT; ++i) {
-                const int m = i + 3 - r;
-                const float d = -kf - mu[m];               // source j = i - k' contributes e_{j, k = j - i = -k'}
-                float e = v1_ex2(d * d * ni2[m]);
-                e = (ak1 < hb[m]) ? e : 0.f;
-                t[i] = fmaf(Wd[m], e, t[i]);
-            }
-        }
+        const int k0 = 4 * a - 3;
+        const bool inside = (float)(max(abs(k0), abs(k0 + 3)) - 1) < hmn;
+        if (__all_sync(__activemask(), inside)) v1_np_taps_adjoint<false>(Wd, k0, aa, bb, hb, t);
+        else v1_np_taps_adjoint<true>(Wd, k0, aa, bb, hb, t);
     }
 }
 
@@ -987,7 +1018,7 @@ __device__ __noinline__ void v1_phase_forward(int s_, bool stencil)
     const float *Yg = a.Y, *Wg = a.W;
     const float *cpg = v1_blk.cp;
     constexpr bool uniform = UNI;
-    const float *ISg = a.IS + V1_TPAD, *S2g = a.S2 + V1_TPAD;
+    const float *ISg = a.IS + V1_TPAD, *SJg = a.SJ + V1_TPAD;
     float *dsg = v1_blk.ds;
     int alo[GS], nag[GS];
     size_t rowo[GS];
@@ -1008,17 +1039,17 @@ __device__ __noinline__ void v1_phase_forward(int s_, bool stencil)
         if (!uniform && stencil && act) {
             // per-pixel kernels: a pass of its own (it needs most of the register file): S -> row A, and its two
             // kernel-parameter derivatives and 1/E0 -> thread-private scratch
-            float isv[OCT], s2v[OCT];
+            float isv[OCT], sjv[OCT];
             {
                 const float4 a0 = __ldg((const float4 *)(ISg + j0)), a1 = __ldg((const float4 *)(ISg + j0) + 1);
-                const float4 b0 = __ldg((const float4 *)(S2g + j0)), b1 = __ldg((const float4 *)(S2g + j0) + 1);
+                const float4 b0 = __ldg((const float4 *)(SJg + j0)), b1 = __ldg((const float4 *)(SJg + j0) + 1);
                 isv[0] = a0.x; isv[1] = a0.y; isv[2] = a0.z; isv[3] = a0.w; isv[4] = a1.x; isv[5] = a1.y; isv[6] = a1.z; isv[7] = a1.w;
-                s2v[0] = b0.x; s2v[1] = b0.y; s2v[2] = b0.z; s2v[3] = b0.w; s2v[4] = b1.x; s2v[5] = b1.y; s2v[6] = b1.z; s2v[7] = b1.w;
+                sjv[0] = b0.x; sjv[1] = b0.y; sjv[2] = b0.z; sjv[3] = b0.w; sjv[4] = b1.x; sjv[5] = b1.y; sjv[6] = b1.z; sjv[7] = b1.w;
             }
             for (int g = 0; g < GS; ++g) {
                 float Sg[OCT], DV[OCT], DG[OCT], EI[OCT];
                 const V1Np np = ((const V1Np *)(V1SM + L.oNP))[g];
-                v1_np_forward_octet((const float4 *)(rowT + g * RL), j0, np, isv, s2v, Sg, DV, DG, EI);
+                v1_np_forward_octet((const float4 *)(rowT + g * RL), j0, np, isv, sjv, Sg, DV, DG, EI);
                 v1_oct_store<STREAM>(rowA, ag, g, j0, Sg);
                 // scratch planes [3][GS][SL], segment-relative, split-octet (thread-private pixels, L2-resident)
                 float4 *d4 = (float4 *)(dsg + g * L.SL + ((j0 - sg.po) >> 1));
@@ -1478,7 +1509,7 @@ __device__ __noinline__ void v1_phase_adjoint(int s_)
     const float4 *gr4 = (const float4 *)(V1SM + L.oGR);
     int alo[GS], nag[GS];
     constexpr bool uniform = UNI;
-    const float *ISg = v1_blk.A.IS + V1_TPAD, *S2g = v1_blk.A.S2 + V1_TPAD;
+    const float *ISg = v1_blk.A.IS + V1_TPAD, *SJg = v1_blk.A.SJ + V1_TPAD;
     V1Np npp[UNI ? 1 : GS];
 #pragma unroll
     for (int g = 0; g < GS; ++g) { alo[g] = tap[2 * g]; nag[g] = tap[2 * g + 1]; if (!UNI) npp[UNI ? 0 : g] = ((const V1Np *)(V1SM + L.oNP))[g]; }
@@ -1500,7 +1531,7 @@ __device__ __noinline__ void v1_phase_adjoint(int s_)
                 // a linear grid): bound the loop by the kernel of the farthest source in reach
                 const int hseg = 4 * (alo[g] + nag[g] - 1);
                 const float hb = fminf(npp[UNI ? 0 : g].hbv * fmaxf(__ldg(ISg + j0 + OCT - 1 + hseg), __ldg(ISg + j0 - hseg)), npp[UNI ? 0 : g].hcap);
-                v1_np_adjoint_octet((const float4 *)(rowA + g * RL), j0, (int)ceilf(hb), npp[UNI ? 0 : g], ISg, S2g, t[g]);
+                v1_np_adjoint_octet((const float4 *)(rowA + g * RL), j0, (int)ceilf(hb), npp[UNI ? 0 : g], ISg, SJg, t[g]);
             } else if (act) {
                 float acc[3][OCT];
                 v1_stencil_octet<3>((const float4 *)(rowA + g * RL), j0, alo[g], nag[g], gr4 + g * NA, wstride4, acc);
@@ -2710,7 +2741,7 @@ __device__ __noinline__ void v1_phase_model(int s, int grp)
     const float *rowT = v1_rowp(L.oT, sg.po);
     const float4 *gw4 = (const float4 *)(V1SM + L.oGW);
     const float *bco = V1SM + L.oB + s * n1 * GS;
-    const float *ISg = a.IS + V1_TPAD, *S2g = a.S2 + V1_TPAD;
+    const float *ISg = a.IS + V1_TPAD, *SJg = a.SJ + V1_TPAD;
     for (int jb = seg_lo; jb < seg_hi; jb += nt8) {   // uniform trip count
         const int j0 = jb + V1_TID * OCT;
         if (STREAM) {
@@ -2723,12 +2754,12 @@ __device__ __noinline__ void v1_phase_model(int s, int grp)
         // The continuum factor is evaluated in fp64: near x^ = +-1 a degree-30 Legendre sum moves by ~n^2/2 per unit of
         // x^, so an fp32 node (6e-8) alone costs up to ~1e-5 of the flux there (measured 1.2e-5 on config-2 shapes),
         // the whole tolerance.  S, the part shared with the fit, stays in fp32.
-        float isv[OCT], s2v[OCT];
+        float isv[OCT], sjv[OCT];
         double xx[OCT];
 #pragma unroll
         for (int i = 0; i < OCT; ++i) {
             xx[i] = (double)(2 * (j0 + i - seg_lo) - sg.P) / (double)sg.P;
-            if (!UNI) { isv[i] = __ldg(ISg + j0 + i); s2v[i] = __ldg(S2g + j0 + i); }
+            if (!UNI) { isv[i] = __ldg(ISg + j0 + i); sjv[i] = __ldg(SJg + j0 + i); }
         }
 #pragma unroll 1
         for (int g = 0; g < GS; ++g) {   // one spectrum at a time (an inspection kernel: the basis recurrence is not shared)
@@ -2741,7 +2772,7 @@ __device__ __noinline__ void v1_phase_model(int s, int grp)
             } else {
                 float DV[OCT], DG[OCT], EI[OCT];
                 const V1Np np = ((const V1Np *)(V1SM + L.oNP))[g];
-                v1_np_forward_octet((const float4 *)(rowT + g * RL), j0, np, isv, s2v, S, DV, DG, EI);
+                v1_np_forward_octet((const float4 *)(rowT + g * RL), j0, np, isv, sjv, S, DV, DG, EI);
             }
             double cc[OCT], pp[OCT], pc[OCT];
 #pragma unroll

@@ -51,7 +51,7 @@ struct lasp_ctx {
     int *dnedge = nullptr;
     long long launches = 0;
     bool nonuniform = false;
-    float *dIS = nullptr, *dS2 = nullptr;
+    float *dIS = nullptr, *dSJ = nullptr;
     Variant res, str;     // resident and streaming variants
     float *dC1 = nullptr;
     float4 *dCF = nullptr;   // coefficient table as tf32 [hi|lo] MMA fragments (emulator_path 2)
@@ -165,7 +165,7 @@ extern "C" int lasp_destroy(lasp_ctx *c)
     if (!c) return LASP_OK;
     DeviceGuard dg(c->device);
     cudaFree(c->dexps); cudaFree(c->dtermmodel); cudaFree(c->dconv); cudaFree(c->dnedge);
-    cudaFree(c->dC1); cudaFree(c->dCF); cudaFree(c->dIS); cudaFree(c->dS2); cudaFree(c->dDS); cudaFree(c->dY); cudaFree(c->dW);
+    cudaFree(c->dC1); cudaFree(c->dCF); cudaFree(c->dIS); cudaFree(c->dSJ); cudaFree(c->dDS); cudaFree(c->dY); cudaFree(c->dW);
     cudaFree(c->dCP); cudaFree(c->dXJ); cudaFree(c->dTG); cudaFree(c->dAG); cudaFree(c->dqueue); cudaFree(c->dstats);
 #ifdef LASP_PHASE_TIMING
     cudaFree(c->ddbg);
@@ -365,17 +365,17 @@ extern "C" int lasp_create(const lasp_model_desc *d, int cuda_device, lasp_ctx *
         CUDA_TRY_C(cudaMalloc(&c->dCF, CF.size() * sizeof(float)));
         CUDA_TRY_C(cudaMemcpy(c->dCF, CF.data(), CF.size() * sizeof(float), cudaMemcpyHostToDevice));
     }
-    {   // 1/s_j and s_j^2 for the per-pixel kernels, V1_TPAD replicated entries on both sides
-        std::vector<float> is1(M.Ppad + 2 * V1_TPAD), s21(M.Ppad + 2 * V1_TPAD);
+    {   // 1/s_j and s_j for the per-pixel kernels, V1_TPAD replicated entries on both sides
+        std::vector<float> is1(M.Ppad + 2 * V1_TPAD), sj1(M.Ppad + 2 * V1_TPAD);
         for (int q = 0; q < M.Ppad + 2 * V1_TPAD; ++q) {
             const int jp = std::min(std::max(q - V1_TPAD, 0), M.Ppad - 1);
             is1[q] = isp[jp];
-            s21[q] = (float)(1.0 / ((double)isp[jp] * (double)isp[jp]));
+            sj1[q] = (float)(1.0 / (double)isp[jp]);
         }
         CUDA_TRY_C(cudaMalloc(&c->dIS, is1.size() * sizeof(float)));
         CUDA_TRY_C(cudaMemcpy(c->dIS, is1.data(), is1.size() * sizeof(float), cudaMemcpyHostToDevice));
-        CUDA_TRY_C(cudaMalloc(&c->dS2, s21.size() * sizeof(float)));
-        CUDA_TRY_C(cudaMemcpy(c->dS2, s21.data(), s21.size() * sizeof(float), cudaMemcpyHostToDevice));
+        CUDA_TRY_C(cudaMalloc(&c->dSJ, sj1.size() * sizeof(float)));
+        CUDA_TRY_C(cudaMemcpy(c->dSJ, sj1.data(), sj1.size() * sizeof(float), cudaMemcpyHostToDevice));
     }
     CUDA_TRY_C(cudaMalloc(&c->dexps, (size_t)K * L));
     CUDA_TRY_C(cudaMemcpy(c->dexps, d->term_exps, (size_t)K * L, cudaMemcpyHostToDevice));
@@ -634,7 +634,7 @@ static void base_args(lasp_ctx *c, const Variant &v, bool mma, int64_t B, V1Args
 {
     memset(&a, 0, sizeof(a));
     a.Y = c->dY; a.W = c->dW; a.C1 = c->dC1; a.CP = c->dCP; a.B = B;
-    a.IS = c->dIS; a.S2 = c->dS2; a.DS = c->dDS;
+    a.IS = c->dIS; a.SJ = c->dSJ; a.DS = c->dDS;
     if (&v == &c->str) { a.TG = c->dTG; a.AG = c->dAG; }
     if (mma) { a.CF = c->dCF; a.ksteps = c->cf_ksteps; }
     a.ngroups = (int)((B + GS - 1) / GS);
@@ -780,7 +780,7 @@ extern "C" int lasp_eval_grad_static(lasp_ctx *c, int64_t B, const float *flux, 
     memset(&a, 0, sizeof(a));
     a.Y = Y; a.W = W; a.C1 = c->dC1; a.B = B;
     a.CP = per_cta;
-    a.IS = c->dIS; a.S2 = c->dS2;
+    a.IS = c->dIS; a.SJ = c->dSJ;
     if (n_ds) a.DS = per_cta + n_cp;
     if (n_tg) { a.TG = per_cta + n_cp + n_ds; a.AG = a.TG + n_tg; }
     if (mma) { a.CF = c->dCF; a.ksteps = c->cf_ksteps; }
