@@ -672,6 +672,36 @@ __device__ __forceinline__ void v1_np_adjoint_octet(const float4 *__restrict__ r
     }
 }
 
+// Per-pixel kernels (linear grids): the stencil pass of spectra [g0, g1) for the octet at j0: S -> row A, and its two
+// kernel-parameter derivatives and 1/E0 -> the scratch planes [3][GS][SL] (segment-relative, split-octet, L2-resident).
+template <bool STREAM>
+__device__ __forceinline__ void v1_np_forward_pass(const SegDev &sg, const float *rowT, float *rowA, int j0, int g0, int g1)
+{
+    const V1Lay &L = v1_blk.L;
+    const float *ISg = v1_blk.A.IS + V1_TPAD, *SJg = v1_blk.A.SJ + V1_TPAD;
+    float *dsg = v1_blk.ds;
+    float isv[OCT], sjv[OCT];
+    {
+        const float4 a0 = __ldg((const float4 *)(ISg + j0)), a1 = __ldg((const float4 *)(ISg + j0) + 1);
+        const float4 b0 = __ldg((const float4 *)(SJg + j0)), b1 = __ldg((const float4 *)(SJg + j0) + 1);
+        isv[0] = a0.x; isv[1] = a0.y; isv[2] = a0.z; isv[3] = a0.w; isv[4] = a1.x; isv[5] = a1.y; isv[6] = a1.z; isv[7] = a1.w;
+        sjv[0] = b0.x; sjv[1] = b0.y; sjv[2] = b0.z; sjv[3] = b0.w; sjv[4] = b1.x; sjv[5] = b1.y; sjv[6] = b1.z; sjv[7] = b1.w;
+    }
+    for (int g = g0; g < g1; ++g) {
+        float Sg[OCT], DV[OCT], DG[OCT], EI[OCT];
+        const V1Np np = ((const V1Np *)(V1SM + L.oNP))[g];
+        v1_np_forward_octet((const float4 *)(rowT + g * L.RL), j0, np, isv, sjv, Sg, DV, DG, EI);
+        v1_oct_store<STREAM>(rowA, v1_blk.ag, g, j0, Sg);
+        float4 *d4 = (float4 *)(dsg + g * L.SL + ((j0 - sg.po) >> 1));
+        const int S8 = L.SL >> 3, SP = GS * (L.SL >> 2);
+        d4[0] = make_float4(DV[0], DV[1], DV[2], DV[3]); d4[S8] = make_float4(DV[4], DV[5], DV[6], DV[7]);
+        d4 += SP;
+        d4[0] = make_float4(DG[0], DG[1], DG[2], DG[3]); d4[S8] = make_float4(DG[4], DG[5], DG[6], DG[7]);
+        d4 += SP;
+        d4[0] = make_float4(EI[0], EI[1], EI[2], EI[3]); d4[S8] = make_float4(EI[4], EI[5], EI[6], EI[7]);
+    }
+}
+
 // padded pixel range [lo,hi) on which T is needed by the forward stencils of the group's fitted octets
 // (group a reads row[j0-4a .. j0-4a+11]); the adjoint pass runs on the same range.  Kept tight: config 1
 // has 188 fitted octets and 192 threads, so 16 pixels of reach on each side still fit one sweep.
@@ -1024,6 +1054,21 @@ __device__ __noinline__ void v1_phase_forward(int s_, bool stencil)
     size_t rowo[GS];
 #pragma unroll
     for (int g = 0; g < GS; ++g) { alo[g] = tap[2 * g]; nag[g] = tap[2 * g + 1]; rowo[g] = (size_t)v1_blk.spec[g] * Ppad; }
+    if (!uniform && stencil && !STREAM) {
+        // Per-pixel kernels, resident rows: the stencil runs as two passes of its own ahead of the basis sums, thread t
+        // on octet t for the first two spectra and on octet N - 1 - t for the other two.  On a linear grid the kernels
+        // widen by 15-25 % from the blue to the red end of an arm: with the mirrored-pair mapping of the basis sums
+        // (lanes < 16 blue, lanes >= 16 red, warp 0 at the two ends) half of every warp waits for the other half and every
+        // warp for warp 0; here the lanes of a warp work on neighbouring octets and every thread gets one octet of each
+        // half.  S goes through row A either way; the barrier hands it to the threads that sum it.
+        const int noct = (sg.fit_hi - sg.fit_lo) / OCT;
+        for (int pass = 0; pass < 2; ++pass)
+            for (int ob = 0; ob < noct; ob += V1_NT) {
+                const int o = pass ? noct - 1 - (ob + V1_TID) : ob + V1_TID;
+                if (o >= 0 && o < noct) v1_np_forward_pass<STREAM>(sg, rowT, rowA, fit_lo + o * OCT, 2 * pass, 2 * pass + 2);
+            }
+        __syncthreads();
+    }
     const int nsweep = v1_nsweep<SYM>(sg);
     for (int sw = 0; sw < nsweep; ++sw) {   // uniform trip count
         bool act;
@@ -1036,31 +1081,7 @@ __device__ __noinline__ void v1_phase_forward(int s_, bool stencil)
             __syncthreads();
             rowT = v1_rowp(L.oT, jb);
         }
-        if (!uniform && stencil && act) {
-            // per-pixel kernels: a pass of its own (it needs most of the register file): S -> row A, and its two
-            // kernel-parameter derivatives and 1/E0 -> thread-private scratch
-            float isv[OCT], sjv[OCT];
-            {
-                const float4 a0 = __ldg((const float4 *)(ISg + j0)), a1 = __ldg((const float4 *)(ISg + j0) + 1);
-                const float4 b0 = __ldg((const float4 *)(SJg + j0)), b1 = __ldg((const float4 *)(SJg + j0) + 1);
-                isv[0] = a0.x; isv[1] = a0.y; isv[2] = a0.z; isv[3] = a0.w; isv[4] = a1.x; isv[5] = a1.y; isv[6] = a1.z; isv[7] = a1.w;
-                sjv[0] = b0.x; sjv[1] = b0.y; sjv[2] = b0.z; sjv[3] = b0.w; sjv[4] = b1.x; sjv[5] = b1.y; sjv[6] = b1.z; sjv[7] = b1.w;
-            }
-            for (int g = 0; g < GS; ++g) {
-                float Sg[OCT], DV[OCT], DG[OCT], EI[OCT];
-                const V1Np np = ((const V1Np *)(V1SM + L.oNP))[g];
-                v1_np_forward_octet((const float4 *)(rowT + g * RL), j0, np, isv, sjv, Sg, DV, DG, EI);
-                v1_oct_store<STREAM>(rowA, ag, g, j0, Sg);
-                // scratch planes [3][GS][SL], segment-relative, split-octet (thread-private pixels, L2-resident)
-                float4 *d4 = (float4 *)(dsg + g * L.SL + ((j0 - sg.po) >> 1));
-                const int S8 = L.SL >> 3, SP = GS * (L.SL >> 2);
-                d4[0] = make_float4(DV[0], DV[1], DV[2], DV[3]); d4[S8] = make_float4(DV[4], DV[5], DV[6], DV[7]);
-                d4 += SP;
-                d4[0] = make_float4(DG[0], DG[1], DG[2], DG[3]); d4[S8] = make_float4(DG[4], DG[5], DG[6], DG[7]);
-                d4 += SP;
-                d4[0] = make_float4(EI[0], EI[1], EI[2], EI[3]); d4[S8] = make_float4(EI[4], EI[5], EI[6], EI[7]);
-            }
-        }
+        if (!uniform && stencil && STREAM && act) v1_np_forward_pass<STREAM>(sg, rowT, rowA, j0, 0, GS);
         float v[GS][OCT];
         if (act) {
 #pragma unroll
