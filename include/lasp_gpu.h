@@ -14,8 +14,11 @@
  *                                  re-solved by weighted least squares in EVERY evaluation
  *                                  (Eq. 6; C.2-4)
  * and returns parameters, continuum coefficients, chi2, the error estimate of P:173 and status
- * bits.  Every step runs in hand-written sm_100a CUDA kernels; there is no CPU fallback, and the
- * library reads no environment variable: every switch is a field of lasp_fit_opts.
+ * bits.  Beyond that path: the paper's stopping rules (stop_window), its Clean-strategy
+ * pixel masking (clean_every), a Levenberg-Marquardt optimiser (optimizer), the three-model / five-regime
+ * emulator (lasp_model_desc.n_models) and the flux-conserving resampler (lasp_resample_coeffs).
+ * Every step runs in hand-written sm_100a CUDA kernels; there is no CPU fallback, and the library reads
+ * no environment variable: every switch is a field of lasp_fit_opts or of lasp_model_desc.
  *
  * Conventions
  *  - All functions return 0 (LASP_OK) or a negative LASP_ERR_* code; they never throw or abort.
@@ -104,7 +107,7 @@ typedef struct {
                                      streaming); 1 resident (LASP_ERR_UNSUPPORTED when they do not fit); 2 streaming
                                      (rows in L2-resident global scratch, swept through a shared-memory window:
                                      any row length).  Same arithmetic, same results to rounding order. */
-    int32_t emulator_path;        /* emulator contraction T = phi.C (Eq. 1): 0 auto (= 1: measured faster, DESIGN.md 6.3a),
+    int32_t emulator_path;        /* emulator contraction T = phi.C (Eq. 1): 0 auto (= 1: measured faster, DESIGN.md 6.4),
                                      1 FP32 FMA, 2 tensor pipe: mma.sync TF32 with both operands split x = hi + lo
                                      (3xTF32-class accuracy); 2 needs the resident variant and n_terms <= 128, else
                                      LASP_ERR_UNSUPPORTED; other values LASP_ERR_INVALID_ARG */
