@@ -484,6 +484,15 @@ __device__ __forceinline__ float *v1_rowp(int off, int org)
     return V1SM + off + v1_blk.L.GUARD - org;
 }
 
+// coefficient-table stream: read through L2 without taking lines in the (small) L1, which the flux / weight / c_prev planes
+// of the two resident CTAs re-use between the forward and the residual phase
+__device__ __forceinline__ float4 v1_ld_table(const float4 *p)
+{
+    float4 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    return v;
+}
+
 // streaming variant: copy padded pixels [jb - GUARD, jb + nt8 + GUARD) of the GS global rows `src` ([GS][Ppad], plain
 // layout) into the window buffer with the SW4 addressing of the resident rows: 128-bit coalesced loads, the halo of
 // 2 GUARD pixels is re-read by the neighbouring sweep.  Pixels outside [0, Ppad) read as zero.  Callers bracket it
@@ -769,8 +778,8 @@ __device__ __noinline__ void v1_phase_emulator(int s_, int full)
         auto load4 = [&](int k0, float4 (&buf)[8]) {
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                buf[2 * u] = __ldg(c4 + (k0 + u) * P4);
-                buf[2 * u + 1] = __ldg(c4 + (k0 + u) * P4 + P8);
+                buf[2 * u] = v1_ld_table(c4 + (k0 + u) * P4);
+                buf[2 * u + 1] = v1_ld_table(c4 + (k0 + u) * P4 + P8);
             }
         };
         auto mul4 = [&](int k0, const float4 (&buf)[8]) {
@@ -1576,8 +1585,8 @@ __device__ __noinline__ void v1_phase_adjoint(int s_)
         auto load4 = [&](int kb, float4 (&buf)[8]) {
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                buf[2 * u] = __ldg(c4 + (kb + u) * P4);
-                buf[2 * u + 1] = __ldg(c4 + (kb + u) * P4 + P8);
+                buf[2 * u] = v1_ld_table(c4 + (kb + u) * P4);
+                buf[2 * u + 1] = v1_ld_table(c4 + (kb + u) * P4 + P8);
             }
         };
         load4(0, bufA);
