@@ -484,10 +484,14 @@ __device__ __forceinline__ float *v1_rowp(int off, int org)
     return V1SM + off + v1_blk.L.GUARD - org;
 }
 
-// coefficient-table stream: read through L2 without taking lines in the (small) L1, which the flux / weight / c_prev planes
-// of the two resident CTAs re-use between the forward and the residual phase
+// coefficient-table stream.  TNA (the steady-state step of the resident two-CTA shape, v1_step_hot): read through L2 without
+// taking lines in the small L1, which the flux / weight / c_prev planes of the two resident CTAs re-use between the forward
+// and the residual phase (config 1: +0.6 %).  Elsewhere the plain read-only path: with one CTA per SM or the streaming
+// variant's global rows the same hint costs 2-5 % (config 4, shape S; measured).
+template <bool TNA>
 __device__ __forceinline__ float4 v1_ld_table(const float4 *p)
 {
+    if (!TNA) return __ldg(p);
     float4 v;
     asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
     return v;
@@ -751,7 +755,7 @@ __device__ __forceinline__ void v1_phase_range(const SegDev &sg, int full, int &
 // ------------------------------------------------------------------------------------------
 // a2: T_j = sum_k phi_k C[k,j] over the padded range [lo,hi) -> shared row T (Eq. 1)
 // ------------------------------------------------------------------------------------------
-template <bool STREAM>
+template <bool STREAM, bool TNA = false>
 __device__ __noinline__ void v1_phase_emulator(int s_, int full)
 {
     const SegDev &sg = v1_blk.M.seg[s_];
@@ -778,8 +782,8 @@ __device__ __noinline__ void v1_phase_emulator(int s_, int full)
         auto load4 = [&](int k0, float4 (&buf)[8]) {
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                buf[2 * u] = v1_ld_table(c4 + (k0 + u) * P4);
-                buf[2 * u + 1] = v1_ld_table(c4 + (k0 + u) * P4 + P8);
+                buf[2 * u] = v1_ld_table<TNA>(c4 + (k0 + u) * P4);
+                buf[2 * u + 1] = v1_ld_table<TNA>(c4 + (k0 + u) * P4 + P8);
             }
         };
         auto mul4 = [&](int k0, const float4 (&buf)[8]) {
@@ -1522,7 +1526,7 @@ __device__ __noinline__ void v1_phase_residual(int s_, float *xrow)
 // Partial sums go through register transposes into this warp's Q slots (pseudo-terms K, K+1 carry
 // the two kernel-parameter gradients), which v1_evaluate zeroed.
 // ------------------------------------------------------------------------------------------
-template <bool UNI, bool STREAM>
+template <bool UNI, bool STREAM, bool TNA = false>
 __device__ __noinline__ void v1_phase_adjoint(int s_)
 {
     const SegDev &sg = v1_blk.M.seg[s_];
@@ -1585,8 +1589,8 @@ __device__ __noinline__ void v1_phase_adjoint(int s_)
         auto load4 = [&](int kb, float4 (&buf)[8]) {
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                buf[2 * u] = v1_ld_table(c4 + (kb + u) * P4);
-                buf[2 * u + 1] = v1_ld_table(c4 + (kb + u) * P4 + P8);
+                buf[2 * u] = v1_ld_table<TNA>(c4 + (kb + u) * P4);
+                buf[2 * u + 1] = v1_ld_table<TNA>(c4 + (kb + u) * P4 + P8);
             }
         };
         load4(0, bufA);
@@ -2262,7 +2266,7 @@ __device__ __noinline__ void v1_step_hot(int momsel)
 {
     __syncthreads();
     v1_begin_eval(momsel, true);
-    v1_phase_emulator<STREAM>(0, 0);
+    v1_phase_emulator<STREAM, !STREAM>(0, 0);
     __syncthreads();
     v1_phase_forward<true, STREAM>(0, true);
     if (v1_blk.momflag != 0) v1_phase_moments<STREAM>(0);
@@ -2272,7 +2276,7 @@ __device__ __noinline__ void v1_step_hot(int momsel)
     if (v1_blk.A.stop_window > 0) v1_phase_residual<1, true, STREAM>(0, nullptr);   // stopping rules read chi2
     else v1_phase_residual<3, true, STREAM>(0, nullptr);
     __syncthreads();
-    v1_phase_adjoint<true, STREAM>(0);
+    v1_phase_adjoint<true, STREAM, !STREAM>(0);
     __syncthreads();
 }
 
