@@ -431,6 +431,14 @@ def test_fit_batch_host_matches_device_call(gpu, oracle_mod):
         assert torch.equal(host[k], dev[k].cpu()), k
     nomask = m.fit_batch_host(case["flux"], case["ivar"], None, case["init"], 5, chunk=0, want_err=False, want_cont=False)
     assert nomask["err"] is None and torch.isfinite(nomask["chi2"]).all()
+    # chunk = 0 (automatic) on a batch large enough for two chunks: 9,001 spectra -> 4,504 + 4,497, groups as in one call
+    n = 9001
+    tile = lambda a: np.tile(a, (n // 37 + 1, 1))[:n]
+    big = {k: tile(case[k]) for k in ("flux", "ivar", "mask", "init")}
+    dev = m.fit_batch(big["flux"], big["ivar"], big["mask"], big["init"], 6, want_err=False)
+    host = m.fit_batch_host(big["flux"], big["ivar"], big["mask"], big["init"], 6, chunk=0, want_err=False)
+    for k in ("params", "chi2", "cont", "status"):
+        assert torch.equal(host[k], dev[k].cpu()), k
     m.close()
 
 
