@@ -926,3 +926,24 @@ def test_config1_launch_stays_under_the_196k_carveout(gpu):
     for window in (0, 50):
         assert 2 * (info["smem_bytes"] + 16 * window + 1792 + 1024) <= 196 * 1024, info
     m.close()
+
+
+def test_stopping_rules_streaming_variant_and_largest_window(gpu, oracle_mod):
+    """The stopping rules on the streaming variant stop at the resident variant's steps (same arithmetic, other rounding
+    order: parameters within the tolerance, same criterion), and the largest window (128: the launch then asks for the
+    whole history ring, lasp_gpu.cu launch()) works."""
+    case = synth.make_case(1, oracle_mod.forward, B=12)
+    m = gpu.LaspModel(case["desc"])
+    o = oracle_mod.Oracle(case["desc"])
+    args = (case["flux"], case["ivar"], case["mask"], case["init"])
+    a = m.fit_batch(*args, 5000, lr=0.1, stop_window=50, stop_tol=1e-5, variant=1)
+    b = m.fit_batch(*args, 5000, lr=0.1, stop_window=50, stop_tol=1e-5, variant=2)
+    na, nb = a["n_steps"].cpu().numpy(), b["n_steps"].cpu().numpy()
+    assert np.abs(na - nb).max() <= 5 and np.array_equal(a["status"].cpu().numpy(), b["status"].cpu().numpy())
+    d = np.abs(a["params"].cpu().numpy() - b["params"].cpu().numpy()) / (o.hi - o.lo)
+    assert d.max() <= TOL_PAR
+    c = m.fit_batch(*args, 400, lr=0.02, stop_window=128, stop_tol=1e-5)      # (a tolerance near the fp32 resolution of
+    ref = o.fit_stop(*args, 400, lr=0.02, window=128, tol=1e-5)                # L ~ 1, e.g. 1e-7, moves the stop by ~10 steps)
+    assert np.abs(c["n_steps"].cpu().numpy() - ref["n_steps"]).max() <= 5
+    assert np.array_equal(c["status"].cpu().numpy() & 48, ref["status"] & 48)
+    m.close()
