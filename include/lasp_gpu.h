@@ -172,8 +172,9 @@ int lasp_fit_batch(lasp_ctx *ctx, int64_t B, const float *flux, const float *iva
 
 /* The same fit from HOST buffers (pinned memory recommended), for batches that do not fit on the device or
  * arrive from the host (BASELINE.json config 3, "survey-scale stream"): the batch is cut into chunks of
- * `chunk` spectra (0 = automatic: half the batch, at least 4,096 and at most 131,072 spectra; every launch costs a ramp
- * and a tail of partly idle SMs, so few large chunks beat many small ones); chunk i+1 is copied host-to-device and chunk
+ * `chunk` spectra (0 = automatic: a short first chunk -- four full rounds of the persistent grid, whose fit hides the next
+ * upload -- then chunks of up to 131,072 spectra: every launch costs a ramp and a tail of partly idle SMs, so few large
+ * chunks beat many small ones); chunk i+1 is copied host-to-device and chunk
  * i-1's results device-to-host on two copy streams while chunk i is fitted, with ctx-owned double buffers.  All pointers are HOST pointers
  * with the layouts of lasp_fit_batch; mask, cont, err, status, n_steps, mask_out may be NULL.  Blocking: returns when every
  * result is in host memory.  Per-chunk results are identical to lasp_fit_batch on the same spectra. */

@@ -950,14 +950,20 @@ static int hostpipe_reserve(lasp_ctx *c, int64_t chunk)
 
 static int hostpipe_run(lasp_ctx *c, int64_t B, const float *flux, const float *ivar, const uint8_t *mask,
                         const float *init, const lasp_fit_opts *opts, float *params, float *cont, float *chi2,
-                        float *err, int32_t *status, int32_t *n_steps, uint8_t *mask_out, int64_t chunk)
+                        float *err, int32_t *status, int32_t *n_steps, uint8_t *mask_out, int64_t first, int64_t chunk)
 {
+    // chunk 0 holds `first` spectra, every later one `chunk` (the last one what is left)
     lasp_ctx::HostPipe &h = c->hp;
     const ModelDev &M = c->M;
-    const int64_t nchunk = (B + chunk - 1) / chunk;
+    const int64_t nchunk = 1 + (B - first + chunk - 1) / chunk;
+    auto span = [&](int64_t i, int64_t &o, int64_t &n) {
+        o = i == 0 ? 0 : first + (i - 1) * chunk;
+        n = i == 0 ? first : std::min(chunk, B - o);
+    };
     auto upload = [&](int64_t i) -> int {
         const int s = (int)(i & 1);
-        const int64_t o = i * chunk, n = std::min(chunk, B - o);
+        int64_t o, n;
+        span(i, o, n);
         // the slot's previous fit (chunk i-2) must be done reading its inputs
         if (i >= 2) CUDA_TRY(c, cudaStreamWaitEvent(h.s_in, h.fit_done[s], 0));
         CUDA_TRY(c, cudaMemcpyAsync(h.flux[s], flux + o * M.P, (size_t)n * M.P * sizeof(float), cudaMemcpyHostToDevice, h.s_in));
@@ -971,7 +977,8 @@ static int hostpipe_run(lasp_ctx *c, int64_t B, const float *flux, const float *
     if (rc) return rc;
     for (int64_t i = 0; i < nchunk; ++i) {
         const int s = (int)(i & 1);
-        const int64_t o = i * chunk, n = std::min(chunk, B - o);
+        int64_t o, n;
+        span(i, o, n);
         if (i + 1 < nchunk) { rc = upload(i + 1); if (rc) return rc; }
         CUDA_TRY(c, cudaStreamWaitEvent(h.s_fit, h.in_done[s], 0));
         if (i >= 2) CUDA_TRY(c, cudaStreamWaitEvent(h.s_fit, h.out_done[s], 0));   // slot's old results copied out
@@ -1003,15 +1010,27 @@ extern "C" int lasp_fit_batch_host(lasp_ctx *c, int64_t B, const float *flux, co
     if (B < 1 || !flux || !ivar || !init || !opts || !params || !chi2 || chunk < 0)
         return fail(c, LASP_ERR_INVALID_ARG, "lasp_fit_batch_host: null pointer, B < 1 or chunk < 0");
     DeviceGuard dg(c->device);
-    // 0 = automatic: two chunks when the batch is small (the second upload and the first download overlap a fit; measured
-    // on config 1, 65,536 spectra: 72.5 k spectra/s with 2 chunks, 70.7 k with 8, 65.6 k with 16 -- every launch costs a ramp
-    // and a tail of partly idle SMs), never more than 131,072 spectra per chunk (device buffers), a multiple of GS so that
-    // the CTA groups are those of one lasp_fit_batch call over the whole batch
-    if (chunk == 0) chunk = std::min<int64_t>(131072, std::max<int64_t>(4096, ((B + 1) / 2 + GS - 1) / GS * GS));
-    chunk = std::min<int64_t>(chunk, B);
-    int rc = hostpipe_reserve(c, chunk);
+    // 0 = automatic.  Every launch costs a ramp and a tail of partly idle SMs, and nothing overlaps the first upload, so: a
+    // short first chunk -- four full rounds of the persistent grid (4 x SMs x CTAs per SM x GS spectra), whose fit hides the
+    // next upload -- then chunks as large as the device buffers allow (131,072 spectra).  Measured on config 1, 65,536
+    // spectra: 70.7 k spectra/s with 8 equal chunks, 73.0 k with 2, 73.4 k with 4,736 + 60,800 (the device-resident call:
+    // 74.0 k in the same run).  All sizes are multiples of GS, so the CTA groups are those of one lasp_fit_batch call over the whole batch.
+    int64_t first_n = 0;
+    if (chunk == 0) {
+        const Variant *v = nullptr;
+        bool mma = false;
+        int rc0 = resolve(c, opts, "lasp_fit_batch_host", &v, &mma);
+        if (rc0) return rc0;
+        first_n = 4 * (int64_t)c->num_sms * v->cta_per_sm * GS;
+        if (B < 2 * first_n) first_n = B;                       // too small to overlap anything
+        chunk = std::min<int64_t>(131072, std::max<int64_t>(GS, (B - first_n + GS - 1) / GS * GS));
+    } else {
+        chunk = std::min<int64_t>(chunk, B);
+        first_n = chunk;
+    }
+    int rc = hostpipe_reserve(c, std::max(first_n, chunk));
     if (rc) return rc;
-    rc = hostpipe_run(c, B, flux, ivar, mask, init, opts, params, cont, chi2, err, status, n_steps, mask_out, chunk);
+    rc = hostpipe_run(c, B, flux, ivar, mask, init, opts, params, cont, chi2, err, status, n_steps, mask_out, first_n, chunk);
     // success or not, nothing of this call may still be in flight on the private streams when it returns: the
     // copies read and write the caller's buffers
     const std::string first = c->err;
