@@ -86,3 +86,39 @@ def test_fit_opts_layout_matches_header():
         if decl:
             names += [n.strip() for n in decl.split(None, 1)[1].split(",")]
     assert names == [f[0] for f in binding.FitOpts._fields_]
+
+
+def test_model_desc_layout_matches_header():
+    """The ctypes mirror of lasp_model_desc has the header's fields in the header's order (pointers and scalars alike)."""
+    from paper_2512_24840_b200 import binding
+    txt = open(os.path.join(ROOT, "include", "lasp_gpu.h")).read()
+    body = re.search(r"typedef struct \{([^}]*)\} lasp_model_desc;", txt, flags=re.S).group(1)
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    names = []
+    for decl in body.split(";"):
+        decl = decl.strip()
+        if decl:
+            tail = decl.rsplit(None, 1)[0] if "," not in decl else decl
+            parts = decl.replace("*", " ").split(",")
+            names.append(parts[0].split()[-1])
+            names += [p.strip() for p in parts[1:]]
+    assert names == [f[0] for f in binding.ModelDesc._fields_]
+
+
+def test_reference_arm_prints_the_contract_line():
+    """`bench.py --impl reference` times the oracle alone and prints one JSON line with the contract's keys."""
+    import json
+    import subprocess
+    import sys
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--steps", "1", "--warmup", "0",
+                          "--config", "0", "--ref-spectra", "8"], capture_output=True, text=True, cwd=ROOT, timeout=600)
+    assert out.returncode == 0, out.stderr[-2000:]
+    line = json.loads([l for l in out.stdout.splitlines() if l.startswith("{")][-1])
+    assert line["impl"] == "reference" and line["metric"] == "spectra fitted/sec (fixed Adam steps)" and line["value"] > 0
+    assert line["gpu_launches"] == 0 and line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["cores"] >= 1
+    assert line["e2e"] == {"value": line["value"], "unit": line["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+    env = dict(os.environ, RANK="1", WORLD_SIZE="2")
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "1",
+                          "--warmup", "0", "--config", "0", "--ref-spectra", "8"], capture_output=True, text=True, cwd=ROOT,
+                         timeout=600, env=env)
+    assert out.returncode == 0 and out.stdout.strip() == ""       # ranks other than 0 exit without work
